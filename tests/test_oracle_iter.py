@@ -1,0 +1,34 @@
+"""Invariants of the oracle's iterative analysis (O6, Alg. 2).  The absolute rms values are not printed by
+the paper ("parity unpinned"); what is fixed is tested: equality with the plain composition of O3/O4,
+monotone decrease, and convergence to the input for band-limited maps with lmax <= 2 nside
+("errors of both modes are negligible")."""
+import numpy as np
+
+from oracle import oracle as O
+from paper_2208_10154_b200 import inputs
+
+
+def test_iter_equals_composition_and_converges():
+    nside, lmax, niter = 8, 15, 3                                # lmax = 2 nside - 1
+    alm_true = inputs.gaussian_alm(lmax, [0, 1, 2], seed=41)
+    maps = O.synthesis(nside, lmax, alm_true)
+    alm, rms = O.analysis_iter(nside, lmax, maps, niter)
+    a = O.analysis(nside, lmax, maps)
+    rms_ref = []
+    for _ in range(niter):
+        r = maps - O.synthesis(nside, lmax, a)
+        rms_ref.append(np.sqrt((r[:, 0, :] ** 2).mean(axis=1)))
+        a = a + O.analysis(nside, lmax, r)
+    assert np.abs(alm - a).max() < 1e-15
+    assert np.allclose(rms, np.array(rms_ref), rtol=1e-12)
+    assert np.all(rms[1:] < 0.2 * rms[:-1])                      # falls by much more than 5x per round
+    err0 = np.abs(O.analysis(nside, lmax, maps) - alm_true).max()
+    err3 = np.abs(alm - alm_true).max()
+    assert err3 < 1e-2 * err0
+
+
+def test_iter_zero_rounds_is_plain_analysis():
+    nside, lmax = 4, 7
+    maps = np.random.default_rng(5).standard_normal((2, 1, 12 * nside * nside))
+    alm, rms = O.analysis_iter(nside, lmax, maps, 0)
+    assert np.array_equal(alm, O.analysis(nside, lmax, maps)) and rms.shape[0] == 0
