@@ -1,0 +1,94 @@
+/*
+ * sht.h -- C ABI of the B200-native batched spherical-harmonic-transform library
+ * (hot path of arXiv:2208.10154, "Accelerating spherical harmonic transforms for a large number of sky maps").
+ *
+ * What the calls compute (citations are /root/reference/PAPER.md line numbers):
+ *   sht_analysis      Alg. 1: a_lm^k = sum_theta P_lm(theta) T_m^k(theta)     (eq. 1-3, :35-60)
+ *                     spin 2: (A^E; iA^B)_m = [[F+,F-],[F-,F+]]_m (Q; iU)_m                      (eq. 14, :139)
+ *   sht_synthesis     eq. 4-5: T_m = P_m^t A_m, then a backward FFT ring by ring;
+ *                     spin 2: eq. 15 (:143)
+ *   sht_analysis_iter Alg. 2, the "traditional" iteration of HEALPix (:300), kept
+ *                     between T_m^k(theta) and a_lm because the ring FFT is lossless (item 8, :227)
+ * on the HEALPix RING grid with constant quadrature weight dsigma = 4 pi / N_pix (:39),
+ * mmax = lmax (Alg. 1 loops m = 0..lmax, :191).  Readings of everything the paper leaves open are
+ * listed in DESIGN.md ("Readings of the paper").
+ *
+ * Conventions
+ *   - extern "C", plain pointers and sizes; no C++ or torch types; nothing throws, exits or aborts.
+ *   - Every entry returns sht_status_t; arguments are validated before anything is launched.
+ *   - `maps`, `alm`, `resid_rms` of the device entries are DEVICE pointers owned by the caller
+ *     (FP64, dense, 16-byte aligned); inputs are never modified; outputs are fully overwritten.
+ *   - Device entries are asynchronous on `stream` (a cudaStream_t passed as void*, NULL = default
+ *     stream); the library synchronises only in plan create/destroy and in the *_host entries.
+ *   - A plan is used from one host thread at a time; distinct plans are independent.
+ *   - There is no CPU fallback: without a CUDA device plan creation fails with SHT_ERR_CUDA.
+ *
+ * Layouts (ncomp = 1 for spin 0, 2 for spin 2)
+ *   maps : [nmaps][ncomp][npix]    double, RING pixel order, components (Q,U); npix = 12 nside^2
+ *   alm  : [nmaps][ncomp][nalm][2] double (re,im), components (E,B), m >= 0 only, m-major:
+ *          idx(l,m) = m (2 lmax + 1 - m)/2 + l,  nalm = (lmax+1)(lmax+2)/2.
+ *          Im(a_l0) is ignored on input and written as 0; spin 2: l < 2 ignored on input, written 0.
+ */
+#ifndef SHT_B200_H
+#define SHT_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sht_plan_s* sht_plan_t;            /* opaque, owned by the library */
+
+typedef enum {
+    SHT_OK = 0,
+    SHT_ERR_INVALID_ARG = -1,
+    SHT_ERR_UNSUPPORTED = -2,
+    SHT_ERR_ALLOC = -3,
+    SHT_ERR_CUDA = -4,
+    SHT_ERR_NULL = -5
+} sht_status_t;
+
+/* Plan: nside >= 1 (any integer, RING scheme), lmax >= 0 (spin 2: lmax >= 2), nmaps >= 1 (spin 2: number of
+ * (Q,U) pairs), spin in {0, 2}.  Builds on the current CUDA device: ring tables, FFT twiddles, recurrence
+ * coefficients, the l_safe / seed table of PAPER.md:230-232 (item 11) and the T_m^k(theta) workspace.
+ * This is the paper's "initialisation overhead", paid once and timed separately.
+ * If the workspace for all nmaps does not fit, maps are processed in chunks internally. */
+sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, int nmaps, int spin);
+sht_status_t sht_plan_destroy(sht_plan_t plan);   /* NULL is a no-op returning SHT_OK */
+
+/* Alg. 1: maps (device, in) -> alm (device, out). */
+sht_status_t sht_analysis(sht_plan_t plan, const double* maps, double* alm, void* stream);
+/* eq. 4-5: alm (device, in) -> maps (device, out). */
+sht_status_t sht_synthesis(sht_plan_t plan, const double* alm, double* maps, void* stream);
+/* Alg. 2: a(0) = analysis(map); niter x { a += analysis(map - synthesis(a)) }, niter >= 0.
+ * resid_rms (device, may be NULL): [niter][nmaps*ncomp]; entry n = rms over pixels of
+ * map - synthesis(a(n)) at the start of round n. */
+sht_status_t sht_analysis_iter(sht_plan_t plan, const double* maps, double* alm, int niter,
+                               double* resid_rms, void* stream);
+
+/* Same transforms on HOST buffers (pinned or pageable; same layouts).  Each call copies its input to the
+ * device, runs the device entry and copies the result back, in map chunks on the plan's own streams,
+ * and returns after the result is complete in host memory.  These are the end-to-end calls bench.py times. */
+sht_status_t sht_analysis_host(sht_plan_t plan, const double* maps_host, double* alm_host);
+sht_status_t sht_synthesis_host(sht_plan_t plan, const double* alm_host, double* maps_host);
+
+/* Introspection (host, pure). */
+long long sht_npix(int nside);                       /* 12 nside^2                                  */
+long long sht_nalm(int lmax);                        /* (lmax+1)(lmax+2)/2                          */
+long long sht_alm_index(int lmax, int l, int m);     /* m(2 lmax+1-m)/2 + l; -1 if out of range     */
+size_t sht_plan_workspace_bytes(sht_plan_t plan);    /* device bytes held by the plan               */
+int sht_plan_chunk_maps(sht_plan_t plan);            /* maps processed per internal chunk           */
+long long sht_plan_kernel_launches(sht_plan_t plan); /* kernels launched by this plan so far        */
+const char* sht_status_string(sht_status_t s);       /* static storage                              */
+const char* sht_last_error(sht_plan_t plan);         /* plan-owned, valid until the next call       */
+
+/* Measurement helper used by bench.py for the roofline denominator: runs a register-resident
+ * DMMA.8x8x4 loop on every SM for about `ms` milliseconds and returns the sustained FP64
+ * tensor-core rate in TFLOP/s (<= 0 on error).  Not part of the transform path. */
+double sht_measure_fp64_mma_peak(double ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHT_B200_H */

@@ -1,0 +1,272 @@
+// sht_api.cu -- the C ABI of include/sht.h: argument checks, map chunking, stage sequencing.
+#include <cstdio>
+#include <cstring>
+#include "sht_internal.h"
+
+using namespace sht;
+
+namespace sht {
+
+// sum of squares per (map, component) for the residual rms of Alg. 2 (reading G18 in DESIGN.md)
+__global__ void k_sumsq(const double* __restrict__ x, long long npix, double* __restrict__ acc)
+{
+    const double* row = x + (size_t)blockIdx.y * npix;
+    double s = 0.0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < npix; i += (long long)gridDim.x * blockDim.x) {
+        const double v = row[i];
+        s = fma(v, v, s);
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    __shared__ double ws[32];
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        s = threadIdx.x < (blockDim.x >> 5) ? ws[threadIdx.x] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (threadIdx.x == 0) atomicAdd(acc + blockIdx.y, s);
+    }
+}
+
+__global__ void k_rms_finish(const double* __restrict__ acc, int n, double inv_npix, double* __restrict__ out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = sqrt(acc[i] * inv_npix);
+}
+
+// register-resident DMMA loop for the roofline denominator
+__global__ void k_mma_peak(double* out, int iters)
+{
+    double c[16][2];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { c[i][0] = 0.0; c[i][1] = 0.0; }
+    const double a = 1.0 + threadIdx.x * 1e-9, b = 1e-9;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};"
+                         : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += c[i][0] + c[i][1];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+}  // namespace sht
+
+static sht_status_t cuda_fail(sht_plan_t pl, const char* what, cudaError_t e)
+{
+    snprintf(pl->err, sizeof(pl->err), "%s: %s", what, cudaGetErrorString(e));
+    return SHT_ERR_CUDA;
+}
+
+#define SHT_TRY(call, what)                                   \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail(pl, what, e__); \
+    } while (0)
+
+// maps[kmap0 .. kmap0+kmaps) -> alm[kalm0 .. kalm0+kmaps)
+static sht_status_t analysis_chunk(sht_plan_t pl, const double* maps, int kmap0, double* alm, int kalm0, double* F,
+                                   int kmaps, bool accumulate, cudaStream_t st)
+{
+    SHT_TRY(launch_ring_analysis(pl, maps, F, kmap0, kmaps, st), "ring analysis");
+    SHT_TRY(launch_legendre_analysis(pl, F, alm, kalm0, kmaps, accumulate, st), "legendre analysis");
+    return SHT_OK;
+}
+
+// alm[kalm0 ..) -> maps[kmap0 ..); with sub_from: maps = sub_from[ksub0 ..] - synthesis
+static sht_status_t synthesis_chunk(sht_plan_t pl, const double* alm, int kalm0, double* maps, int kmap0, double* F,
+                                    int kmaps, const double* sub_from, int ksub0, cudaStream_t st)
+{
+    SHT_TRY(launch_legendre_synthesis(pl, alm, F, kalm0, kmaps, st), "legendre synthesis");
+    SHT_TRY(launch_ring_synthesis(pl, F, maps, kmap0, kmaps, sub_from, ksub0, st), "ring synthesis");
+    return SHT_OK;
+}
+
+extern "C" sht_status_t sht_analysis(sht_plan_t pl, const double* maps, double* alm, void* stream)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (!maps || !alm) { snprintf(pl->err, sizeof(pl->err), "null data pointer"); return SHT_ERR_NULL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int k0 = 0; k0 < pl->nmaps; k0 += pl->chunk) {
+        const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
+        sht_status_t s = analysis_chunk(pl, maps, k0, alm, k0, pl->F, kmaps, false, st);
+        if (s != SHT_OK) return s;
+    }
+    return SHT_OK;
+}
+
+extern "C" sht_status_t sht_synthesis(sht_plan_t pl, const double* alm, double* maps, void* stream)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (!maps || !alm) { snprintf(pl->err, sizeof(pl->err), "null data pointer"); return SHT_ERR_NULL; }
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int k0 = 0; k0 < pl->nmaps; k0 += pl->chunk) {
+        const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
+        sht_status_t s = synthesis_chunk(pl, alm, k0, maps, k0, pl->F, kmaps, nullptr, 0, st);
+        if (s != SHT_OK) return s;
+    }
+    return SHT_OK;
+}
+
+extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, double* alm, int niter,
+                                          double* resid_rms, void* stream)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (!maps || !alm) { snprintf(pl->err, sizeof(pl->err), "null data pointer"); return SHT_ERR_NULL; }
+    if (niter < 0) { snprintf(pl->err, sizeof(pl->err), "niter < 0"); return SHT_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const DevicePlan& d = pl->d;
+    // residual maps of one chunk + sum-of-squares accumulators (stream-ordered scratch)
+    double* res = nullptr; double* acc = nullptr;
+    if (niter > 0) {
+        SHT_TRY(cudaMallocAsync((void**)&res, (size_t)pl->chunk * d.ncomp * d.npix * sizeof(double), st), "residual scratch");
+        SHT_TRY(cudaMallocAsync((void**)&acc, (size_t)pl->chunk * d.ncomp * sizeof(double), st), "rms scratch");
+    }
+    sht_status_t s = SHT_OK;
+    for (int k0 = 0; k0 < pl->nmaps && s == SHT_OK; k0 += pl->chunk) {
+        const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
+        s = analysis_chunk(pl, maps, k0, alm, k0, pl->F, kmaps, false, st);
+        for (int it = 0; it < niter && s == SHT_OK; ++it) {
+            // r = map - synthesis(a): `res` is indexed from the chunk start, maps/alm from map 0
+            s = synthesis_chunk(pl, alm, k0, res, 0, pl->F, kmaps, maps, k0, st);
+            if (s != SHT_OK) break;
+            if (resid_rms) {
+                const int nrow = kmaps * d.ncomp;
+                SHT_TRY(cudaMemsetAsync(acc, 0, (size_t)nrow * sizeof(double), st), "rms memset");
+                dim3 grid(64, nrow);
+                k_sumsq<<<grid, 256, 0, st>>>(res, d.npix, acc);
+                k_rms_finish<<<(nrow + 127) / 128, 128, 0, st>>>(acc, nrow, 1.0 / (double)d.npix,
+                                                                 resid_rms + (size_t)it * pl->nmaps * d.ncomp + (size_t)k0 * d.ncomp);
+                pl->launches += 2;
+                SHT_TRY(cudaGetLastError(), "rms kernels");
+            }
+            s = analysis_chunk(pl, res, 0, alm, k0, pl->F, kmaps, true, st);
+        }
+    }
+    if (res) cudaFreeAsync(res, st);
+    if (acc) cudaFreeAsync(acc, st);
+    return s;
+}
+
+// ---- host-buffer entries: chunked H2D -> transform -> D2H on two streams ---------------------------
+static sht_status_t host_setup(sht_plan_t pl)
+{
+    if (pl->host_ready) return SHT_OK;
+    const DevicePlan& d = pl->d;
+    // chunk of the host path: at most kpad/2 maps (two chunks in flight), a multiple of the k-tile
+    int hc = pl->nmaps >= 2 * KTILE_MAPS ? ((pl->nmaps / 8 + KTILE_MAPS - 1) / KTILE_MAPS) * KTILE_MAPS : pl->nmaps;
+    if (hc > d.kpad) hc = d.kpad;
+    pl->host_chunk = hc;
+    const size_t mbytes = (size_t)hc * d.ncomp * d.npix * sizeof(double);
+    const size_t abytes = (size_t)hc * d.ncomp * d.nalm * 2 * sizeof(double);
+    for (int i = 0; i < 2; ++i) {
+        SHT_TRY(cudaMalloc((void**)&pl->stage_maps[i], mbytes), "host-path map staging");
+        SHT_TRY(cudaMalloc((void**)&pl->stage_alm[i], abytes), "host-path alm staging");
+        SHT_TRY(cudaStreamCreateWithFlags(&pl->hstream[i], cudaStreamNonBlocking), "host-path stream");
+    }
+    // second workspace so that two chunks can be in flight; both hold kpad columns per row
+    SHT_TRY(cudaMalloc((void**)&pl->F2, pl->F_bytes), "host-path second workspace");
+    SHT_TRY(cudaMemset(pl->F2, 0, pl->F_bytes), "host-path workspace memset");
+    pl->host_ready = true;
+    return SHT_OK;
+}
+
+static sht_status_t host_run(sht_plan_t pl, const double* in_host, double* out_host, bool analysis)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (!in_host || !out_host) { snprintf(pl->err, sizeof(pl->err), "null data pointer"); return SHT_ERR_NULL; }
+    sht_status_t s = host_setup(pl);
+    if (s != SHT_OK) return s;
+    const DevicePlan& d = pl->d;
+    const size_t map_elems = (size_t)d.ncomp * d.npix, alm_elems = (size_t)d.ncomp * d.nalm * 2;
+    const size_t in_elems = analysis ? map_elems : alm_elems, out_elems = analysis ? alm_elems : map_elems;
+    int idx = 0;
+    for (int k0 = 0; k0 < pl->nmaps; k0 += pl->host_chunk, ++idx) {
+        const int b = idx & 1;
+        const int kmaps = pl->nmaps - k0 < pl->host_chunk ? pl->nmaps - k0 : pl->host_chunk;
+        cudaStream_t st = pl->hstream[b];
+        double* dmaps = pl->stage_maps[b]; double* dalm = pl->stage_alm[b];
+        double* din = analysis ? dmaps : dalm; double* dout = analysis ? dalm : dmaps;
+        double* F = b ? pl->F2 : pl->F;
+        SHT_TRY(cudaMemcpyAsync(din, in_host + (size_t)k0 * in_elems, (size_t)kmaps * in_elems * sizeof(double),
+                                cudaMemcpyHostToDevice, st), "H2D");
+        // staging buffers are indexed from the chunk start: pass k0 = 0
+        s = analysis ? analysis_chunk(pl, dmaps, 0, dalm, 0, F, kmaps, false, st)
+                     : synthesis_chunk(pl, dalm, 0, dmaps, 0, F, kmaps, nullptr, 0, st);
+        if (s != SHT_OK) return s;
+        SHT_TRY(cudaMemcpyAsync(out_host + (size_t)k0 * out_elems, dout, (size_t)kmaps * out_elems * sizeof(double),
+                                cudaMemcpyDeviceToHost, st), "D2H");
+    }
+    SHT_TRY(cudaStreamSynchronize(pl->hstream[0]), "host-path sync");
+    SHT_TRY(cudaStreamSynchronize(pl->hstream[1]), "host-path sync");
+    return SHT_OK;
+}
+
+extern "C" sht_status_t sht_analysis_host(sht_plan_t pl, const double* maps_host, double* alm_host)
+{
+    return host_run(pl, maps_host, alm_host, true);
+}
+
+extern "C" sht_status_t sht_synthesis_host(sht_plan_t pl, const double* alm_host, double* maps_host)
+{
+    return host_run(pl, alm_host, maps_host, false);
+}
+
+// ---- introspection -----------------------------------------------------------------------------------
+extern "C" long long sht_npix(int nside) { return 12LL * nside * nside; }
+extern "C" long long sht_nalm(int lmax) { return (long long)(lmax + 1) * (lmax + 2) / 2; }
+extern "C" long long sht_alm_index(int lmax, int l, int m)
+{
+    if (lmax < 0 || m < 0 || l < m || l > lmax) return -1;
+    return (long long)m * (2 * lmax + 1 - m) / 2 + l;
+}
+extern "C" size_t sht_plan_workspace_bytes(sht_plan_t pl) { return pl ? pl->F_bytes + pl->table_bytes : 0; }
+extern "C" int sht_plan_chunk_maps(sht_plan_t pl) { return pl ? pl->chunk : 0; }
+extern "C" long long sht_plan_kernel_launches(sht_plan_t pl) { return pl ? pl->launches : 0; }
+extern "C" const char* sht_status_string(sht_status_t s)
+{
+    switch (s) {
+        case SHT_OK: return "ok";
+        case SHT_ERR_INVALID_ARG: return "invalid argument";
+        case SHT_ERR_UNSUPPORTED: return "unsupported configuration";
+        case SHT_ERR_ALLOC: return "allocation failed";
+        case SHT_ERR_CUDA: return "CUDA error";
+        case SHT_ERR_NULL: return "null pointer";
+    }
+    return "unknown status";
+}
+extern "C" const char* sht_last_error(sht_plan_t pl) { return pl ? pl->err : ""; }
+
+extern "C" double sht_measure_fp64_mma_peak(double ms)
+{
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1.0;
+    if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1.0;
+    const int threads = 512, iters = 4000;
+    double* out = nullptr;
+    if (cudaMalloc((void**)&out, (size_t)nsm * threads * sizeof(double)) != cudaSuccess) return -1.0;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    k_mma_peak<<<nsm, threads>>>(out, iters);                     // warm-up
+    cudaDeviceSynchronize();
+    const double flops_per_launch = (double)nsm * (threads / 32) * iters * 16.0 * 512.0;
+    double best = -1.0, elapsed = 0.0;
+    // launches back to back until `ms` of device time has passed; report the sustained rate
+    int n = 0;
+    cudaEventRecord(e0);
+    while (elapsed < ms && n < 100000) {
+        for (int r = 0; r < 8; ++r) k_mma_peak<<<nsm, threads>>>(out, iters);
+        n += 8;
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float t = 0.f;
+        cudaEventElapsedTime(&t, e0, e1);
+        elapsed = t;
+    }
+    if (elapsed > 0.0 && cudaGetLastError() == cudaSuccess) best = flops_per_launch * n / (elapsed * 1e-3) * 1e-12;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    return best;
+}

@@ -1,0 +1,314 @@
+// sht_plan.cu -- plan creation: ring tables, FFT twiddles / radix lists, recurrence coefficients and the
+// l_safe / seed table of PAPER.md:230-232 (item 11: "the recursion starts from safe positions ... computed
+// once and saved as an input table l_safe(m, theta)").
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#include "sht_internal.h"
+
+namespace sht {
+
+// ------------------------------------------------------------------------------------------------
+// Seed kernel.  One thread per (m, p).  lambda_mm = c_m sin^m(theta) is formed as a
+// (mantissa, exponent) pair so that it cannot underflow, then the three-term recurrence
+//   lambda_l = alpha_l z lambda_{l-1} - beta_l lambda_{l-2}
+// is stepped with a shared power-of-two exponent until |lambda_l| >= 2^-70 (~8.5e-22, below the paper's
+// example threshold 1e-20).  That l is l_safe(m,p); the two values before it are stored as plain doubles,
+// so the hot kernels run an unscaled recurrence from there and treat lambda below l_safe as zero.
+// ------------------------------------------------------------------------------------------------
+constexpr int SEED_THRESH_EXP = -70;
+
+__device__ inline void renorm(double& f, int& e)
+{
+    int t;
+    f = frexp(f, &t);
+    e += t;
+}
+
+__global__ void k_seed_table(DevicePlan d, const double* __restrict__ cm, int* __restrict__ lstart,
+                             double2* __restrict__ seed)
+{
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)(d.lmax + 1) * d.nh;
+    if (gid >= total) return;
+    const int m = (int)(gid / d.nh), p = (int)(gid % d.nh);
+    const double z = d.z[p];
+    // sin^m(theta) by binary powering on (mantissa, exponent)
+    double bf; int be;
+    bf = frexp(sqrt(d.sin2[p]), &be);
+    double rf = 1.0; int re = 0;
+    for (int n = m; n > 0; n >>= 1) {
+        if (n & 1) { rf *= bf; re += be; renorm(rf, re); }
+        bf *= bf; be *= 2; renorm(bf, be);
+    }
+    double cur = cm[m] * rf; int E = re;
+    renorm(cur, E);                              // lambda_mm = cur * 2^E, |cur| in [0.5, 1)
+    double prev = 0.0, prev2 = 0.0;
+    int ls = d.lmax + 1;
+    double x1 = 0.0, x2 = 0.0;
+    if (ilogb(cur) + E >= SEED_THRESH_EXP) {
+        ls = m; x1 = 0.0; x2 = ldexp(cur, E);    // coef(l = m) = (0, -1) reproduces lambda_mm = x2
+    } else {
+        const double2* cf = d.coef + ((long long)m * (2 * d.lmax + 1 - m) / 2);
+        for (int l = m + 1; l <= d.lmax; ++l) {
+            const double2 ab = cf[l];
+            const double nxt = ab.x * z * cur - ab.y * prev;
+            prev2 = prev; prev = cur; cur = nxt;
+            if (fabs(cur) > 0x1p200) { cur *= 0x1p-200; prev *= 0x1p-200; prev2 *= 0x1p-200; E += 200; }
+            if (cur != 0.0 && ilogb(cur) + E >= SEED_THRESH_EXP) {
+                ls = l; x1 = ldexp(prev, E); x2 = ldexp(prev2, E);
+                break;
+            }
+        }
+    }
+    lstart[gid] = ls;
+    seed[gid] = make_double2(x1, x2);
+}
+
+cudaError_t launch_seed_table(const DevicePlan& d, const double* cm, int* lstart, double2* seed, cudaStream_t st)
+{
+    const long long total = (long long)(d.lmax + 1) * d.nh;
+    const int bs = 128;
+    k_seed_table<<<(unsigned)((total + bs - 1) / bs), bs, 0, st>>>(d, cm, lstart, seed);
+    return cudaGetLastError();
+}
+
+}  // namespace sht
+
+using namespace sht;
+
+// ------------------------------------------------------------------------------------------------
+// host-side table construction
+// ------------------------------------------------------------------------------------------------
+static const long double PI_LD = 3.14159265358979323846264338327950288419716939937510L;
+
+static void factorize_ring(int n, std::vector<int>& out)
+{
+    // n = 4 q.  Radix-4 passes first, then 2, then the odd primes of q in increasing order.
+    int r = n;
+    while (r % 4 == 0) { out.push_back(4); r /= 4; }
+    while (r % 2 == 0) { out.push_back(2); r /= 2; }
+    for (int f = 3; (long long)f * f <= r; f += 2)
+        while (r % f == 0) { out.push_back(f); r /= f; }
+    if (r > 1) out.push_back(r);
+}
+
+static int largest_factor(const std::vector<int>& f)
+{
+    int m = 1;
+    for (int v : f) m = v > m ? v : m;
+    return m;
+}
+
+template <typename T>
+static cudaError_t upload(sht_plan_s* pl, const std::vector<T>& h, const T** dptr)
+{
+    void* p = nullptr;
+    size_t bytes = h.size() * sizeof(T);
+    if (bytes == 0) bytes = sizeof(T);
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) return e;
+    pl->dev_allocs[pl->n_allocs++] = p;
+    pl->table_bytes += bytes;
+    if (!h.empty()) e = cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+    *dptr = (const T*)p;
+    return e;
+}
+
+static sht_status_t fail(sht_plan_s* pl, sht_status_t s, const char* what, cudaError_t e)
+{
+    snprintf(pl->err, sizeof(pl->err), "%s: %s", what, e == cudaSuccess ? "" : cudaGetErrorString(e));
+    return s;
+}
+
+// maps per CTA of the ring kernels: as many as fit next to one scratch ring in the smem budget,
+// a power of two <= 16 so that workspace runs are 32-byte-sector aligned.
+static int ring_kt(int n, size_t budget)
+{
+    long long fit = (long long)(budget / ((size_t)n * sizeof(double2))) - 1;
+    int kt = 1;
+    while (kt * 2 <= fit && kt < 16) kt *= 2;
+    return kt;
+}
+
+size_t sht::ring_fft_smem_bytes(int n, int kt) { return (size_t)(kt + 1) * n * sizeof(double2); }
+
+extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, int nmaps, int spin)
+{
+    if (!out) return SHT_ERR_NULL;
+    *out = nullptr;
+    if (nside < 1 || nside > 8192 || lmax < 0 || nmaps < 1 || (spin != 0 && spin != 2)) return SHT_ERR_INVALID_ARG;
+    if (spin == 2 && lmax < 2) return SHT_ERR_INVALID_ARG;
+    if (lmax > 16383) return SHT_ERR_UNSUPPORTED;
+
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess || ndev == 0) return SHT_ERR_CUDA;      // no CPU fallback
+
+    sht_plan_s* pl = (sht_plan_s*)calloc(1, sizeof(sht_plan_s));
+    if (!pl) return SHT_ERR_ALLOC;
+    DevicePlan& d = pl->d;
+    d.nside = nside; d.lmax = lmax; d.spin = spin; d.ncomp = spin == 2 ? 2 : 1;
+    d.nh = 2 * nside;
+    d.npix = 12LL * nside * nside;
+    d.nalm = (long long)(lmax + 1) * (lmax + 2) / 2;
+    pl->nmaps = nmaps;
+
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceProp prop;
+    cudaGetDeviceProperties(&prop, dev);
+    pl->sm_count = prop.multiProcessorCount;
+    const size_t smem_budget = 200 * 1024;
+
+    // ---- ring pairs, twiddles, radix lists ----------------------------------------------------
+    std::vector<RingPair> rings(d.nh);
+    std::vector<double> zs(d.nh), sin2s(d.nh);
+    std::vector<double2> tw;
+    std::vector<int> radix;
+    std::vector<int> tw_off_of_q(nside + 1, -1), fac_off_of_q(nside + 1, -1), nfac_of_q(nside + 1, 0);
+    pl->max_ring = 4 * nside;
+    for (int q = 1; q <= nside; ++q) {
+        const int n = 4 * q;
+        tw_off_of_q[q] = (int)tw.size();
+        for (int j = 0; j < 2 * n; ++j) {
+            long double ang = PI_LD * (long double)j / (long double)n;
+            tw.push_back(make_double2((double)cosl(ang), (double)-sinl(ang)));
+        }
+        std::vector<int> f;
+        factorize_ring(n, f);
+        if ((int)f.size() > MAX_RADIX_LIST) { free(pl); return SHT_ERR_UNSUPPORTED; }
+        fac_off_of_q[q] = (int)radix.size();
+        nfac_of_q[q] = (int)f.size();
+        for (int v : f) radix.push_back(v);
+        (void)largest_factor;
+    }
+    const long long ns = nside;
+    for (int p = 0; p < d.nh; ++p) {
+        const long long i = p + 1;                       // north ring index, 1 .. 2 nside
+        RingPair& r = rings[p];
+        long double absz, s2;
+        if (i < ns) {
+            r.n = (int)(4 * i);
+            long double omz = (long double)(i * i) / (long double)(3 * ns * ns);
+            absz = 1.0L - omz; s2 = omz * (2.0L - omz);
+            r.shift = 1;
+            r.start_n = 2 * i * (i - 1);
+        } else {
+            r.n = (int)(4 * ns);
+            absz = (long double)(4 * ns - 2 * i) / (long double)(3 * ns);
+            s2 = (1.0L - absz) * (1.0L + absz);
+            r.shift = ((i - ns) % 2 == 0) ? 1 : 0;
+            r.start_n = 2 * ns * (ns - 1) + (i - ns) * 4 * ns;
+        }
+        r.start_s = (i == 2 * ns) ? -1 : d.npix - r.start_n - r.n;
+        const int q = r.n / 4;
+        r.tw_off = tw_off_of_q[q]; r.fac_off = fac_off_of_q[q]; r.nfac = nfac_of_q[q];
+        r.kt = ring_kt(r.n, smem_budget);
+        r.nb = 0; r.chirp_off = r.bfilt_off = r.btw_off = 0;
+        zs[p] = (double)absz; sin2s[p] = (double)s2;
+    }
+    pl->fft_smem = 0;
+    pl->ring_kt_min = rings[d.nh - 1].kt;
+    for (int p = 0; p < d.nh; ++p) {
+        size_t b = ring_fft_smem_bytes(rings[p].n, rings[p].kt);
+        if (b > pl->fft_smem) pl->fft_smem = b;
+    }
+    if (pl->fft_smem > 220 * 1024) { free(pl); return SHT_ERR_UNSUPPORTED; }
+
+    // ---- recurrence coefficients (alpha_lm, beta_lm), m-major ---------------------------------
+    //   lambda_l = alpha_l z lambda_{l-1} - beta_l lambda_{l-2},
+    //   alpha_lm = sqrt((4 l^2 - 1)/(l^2 - m^2)),  beta_lm = alpha_lm / alpha_{l-1,m}
+    //   slot l = m holds (0, -1) so that the same step reproduces the seed lambda_mm from the state (0, lambda_mm).
+    std::vector<double2> coef((size_t)d.nalm);
+    std::vector<double> cm(lmax + 1);
+    {
+        long double c = sqrtl(1.0L / (4.0L * PI_LD));
+        cm[0] = (double)c;
+        for (int m = 1; m <= lmax; ++m) { c = -c * sqrtl((2.0L * m + 1.0L) / (2.0L * m)); cm[m] = (double)c; }
+    }
+    for (int m = 0; m <= lmax; ++m) {
+        const size_t base = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
+        long double aprev = 0.0L;
+        coef[base + m] = make_double2(0.0, -1.0);
+        for (int l = m + 1; l <= lmax; ++l) {
+            long double l2 = (long double)l * l, m2 = (long double)m * m;
+            long double a = sqrtl((4.0L * l2 - 1.0L) / (l2 - m2));
+            long double b = (l == m + 1) ? 0.0L : a / aprev;
+            coef[base + l] = make_double2((double)a, (double)b);
+            aprev = a;
+        }
+    }
+    // spin-2 per-l constants: N_l = 2 / sqrt((l-1) l (l+1) (l+2)); (unused slots for l < 2 are 0)
+    std::vector<double2> spin2c(lmax + 1, make_double2(0.0, 0.0));
+    for (int l = 2; l <= lmax; ++l) {
+        long double L = l;
+        spin2c[l] = make_double2((double)(2.0L / sqrtl((L - 1.0L) * L * (L + 1.0L) * (L + 2.0L))), 0.0);
+    }
+
+    const double* d_cm = nullptr;
+    if ((ce = upload(pl, rings, &d.rings)) != cudaSuccess || (ce = upload(pl, zs, &d.z)) != cudaSuccess ||
+        (ce = upload(pl, sin2s, &d.sin2)) != cudaSuccess || (ce = upload(pl, tw, &d.tw)) != cudaSuccess ||
+        (ce = upload(pl, radix, &d.radix)) != cudaSuccess || (ce = upload(pl, coef, &d.coef)) != cudaSuccess ||
+        (ce = upload(pl, spin2c, &d.spin2c)) != cudaSuccess || (ce = upload(pl, cm, &d_cm)) != cudaSuccess) {
+        sht_plan_destroy(pl);
+        return SHT_ERR_ALLOC;
+    }
+
+    // ---- l_safe / seed table ------------------------------------------------------------------
+    {
+        const size_t cells = (size_t)(lmax + 1) * d.nh;
+        int* ls = nullptr; double2* sd = nullptr;
+        if (cudaMalloc(&ls, cells * sizeof(int)) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+        pl->dev_allocs[pl->n_allocs++] = ls;
+        if (cudaMalloc(&sd, cells * sizeof(double2)) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+        pl->dev_allocs[pl->n_allocs++] = sd;
+        pl->table_bytes += cells * (sizeof(int) + sizeof(double2));
+        d.lstart = ls; d.seed = sd;
+        ce = launch_seed_table(d, d_cm, ls, sd, 0);
+        if (ce == cudaSuccess) ce = cudaDeviceSynchronize();
+        if (ce != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
+    }
+
+    // ---- workspace: T_m^k(theta) for one chunk of maps ----------------------------------------
+    {
+        size_t freeb = 0, totalb = 0;
+        cudaMemGetInfo(&freeb, &totalb);
+        const size_t per_map = (size_t)d.nh * (lmax + 1) * d.ncomp * 2 * sizeof(double2);
+        size_t budget = (size_t)(0.6 * (double)freeb);
+        const size_t cap = (size_t)64 << 30;
+        if (budget > cap) budget = cap;
+        long long fit = (long long)(budget / per_map) / KTILE_MAPS * KTILE_MAPS;
+        if (fit < KTILE_MAPS) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+        long long need = ((long long)nmaps + KTILE_MAPS - 1) / KTILE_MAPS * KTILE_MAPS;
+        d.kpad = (int)(need < fit ? need : fit);
+        pl->chunk = d.kpad < nmaps ? d.kpad : nmaps;
+        pl->F_bytes = per_map * d.kpad;
+        if (cudaMalloc(&pl->F, pl->F_bytes) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+        // padded map columns are never written by the ring kernels: keep them finite (zero) forever
+        if (cudaMemset(pl->F, 0, pl->F_bytes) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
+    }
+    if (cudaDeviceSynchronize() != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
+    pl->err[0] = 0;
+    (void)fail;
+    *out = pl;
+    return SHT_OK;
+}
+
+extern "C" sht_status_t sht_plan_destroy(sht_plan_t pl)
+{
+    if (!pl) return SHT_OK;
+    cudaDeviceSynchronize();
+    for (int i = 0; i < pl->n_allocs; ++i) cudaFree(pl->dev_allocs[i]);
+    if (pl->F) cudaFree(pl->F);
+    if (pl->F2) cudaFree(pl->F2);
+    for (int i = 0; i < 2; ++i) {
+        if (pl->stage_maps[i]) cudaFree(pl->stage_maps[i]);
+        if (pl->stage_alm[i]) cudaFree(pl->stage_alm[i]);
+        if (pl->hstream[i]) cudaStreamDestroy(pl->hstream[i]);
+    }
+    free(pl);
+    return SHT_OK;
+}

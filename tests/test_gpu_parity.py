@@ -1,0 +1,130 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the same
+seeded inputs.  Tolerance (BASELINE.json north_star; metric = DESIGN.md reading G22): per map
+max|x - ref| / max|ref| <= 1e-10 in FP64."""
+import numpy as np
+import pytest
+
+from paper_2208_10154_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+def _dev():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch.device("cuda:0")
+
+
+def _gpu_synthesis(plan, alm):
+    import torch
+    a = torch.from_numpy(np.ascontiguousarray(alm)).to(_dev())
+    maps = torch.full((plan.nmaps, plan.ncomp, plan.npix), float("nan"), dtype=torch.float64, device=_dev())
+    plan.sht_synthesis(a, maps)
+    torch.cuda.synchronize()
+    return maps.cpu().numpy()
+
+
+def _gpu_analysis(plan, maps):
+    import torch
+    mp = torch.from_numpy(np.ascontiguousarray(maps)).to(_dev())
+    alm = torch.full((plan.nmaps, plan.ncomp, plan.nalm), float("nan"), dtype=torch.complex128, device=_dev())
+    plan.sht_analysis(mp, alm)
+    torch.cuda.synchronize()
+    return alm.cpu().numpy()
+
+
+@pytest.mark.parametrize("nside,lmax,nmaps", [
+    (1, 2, 1), (1, 0, 3), (2, 5, 2), (3, 8, 5), (4, 11, 8), (5, 14, 3), (8, 23, 70), (16, 47, 8),
+    (16, 20, 4), (16, 63, 2), (32, 95, 130),
+])
+def test_spin0_small_full(nside, lmax, nmaps):
+    """both directions, every output element; ragged map counts, odd nside, lmax below / above 3 nside - 1"""
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan
+    alm = inputs.gaussian_alm(lmax, np.arange(nmaps), seed=100 + nside)
+    if lmax < 2:
+        alm[:] = np.random.default_rng(1).standard_normal(alm.shape)
+    plan = Plan(nside, lmax, nmaps, 0)
+    ref_maps = O.synthesis(nside, lmax, alm)
+    got_maps = _gpu_synthesis(plan, alm)
+    assert inputs.rel_err(got_maps, ref_maps) <= TOL
+    noisy = ref_maps + inputs.white_noise(nside, np.arange(nmaps), 7, 1e-3)
+    ref_alm = O.analysis(nside, lmax, noisy)
+    got_alm = _gpu_analysis(plan, noisy)
+    assert inputs.rel_err(got_alm, ref_alm) <= TOL
+    ls, ms = inputs.ell_of_index(lmax)
+    assert np.all(got_alm[:, :, ms == 0].imag == 0.0)
+    plan.destroy()
+
+
+def test_config1():
+    """BASELINE.json configs[0]: nside 16, lmax 47, 8 maps: synthesise, analyse back, compare both."""
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan
+    c = inputs.CONFIGS[1]
+    alm = inputs.gaussian_alm(c["lmax"], np.arange(c["nmaps"]), c["seed"])
+    plan = Plan(c["nside"], c["lmax"], c["nmaps"], 0)
+    ref_maps = O.synthesis(c["nside"], c["lmax"], alm)
+    assert inputs.rel_err(_gpu_synthesis(plan, alm), ref_maps) <= TOL
+    assert inputs.rel_err(_gpu_analysis(plan, ref_maps), O.analysis(c["nside"], c["lmax"], ref_maps)) <= TOL
+    plan.destroy()
+
+
+def test_config2_sampled_maps():
+    """BASELINE.json configs[1]: nside 128, lmax 383, 256 maps, white noise sigma 1e-3 added after synthesis.
+    All 256 maps go through the GPU; 8 of them are compared against the oracle in full."""
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan
+    c = inputs.CONFIGS[2]
+    nside, lmax, nmaps = c["nside"], c["lmax"], c["nmaps"]
+    ks = np.array([0, 1, 2, 3, 127, 128, 254, 255])
+    alm = inputs.gaussian_alm(lmax, np.arange(nmaps), c["seed"])
+    plan = Plan(nside, lmax, nmaps, 0)
+    got_maps = _gpu_synthesis(plan, alm)
+    ref_maps = O.synthesis(nside, lmax, alm[ks])
+    assert inputs.rel_err(got_maps[ks], ref_maps) <= TOL
+    # analysis input: oracle-synthesised maps + white noise for the sampled maps, seeded noise elsewhere
+    maps_in = inputs.white_noise(nside, np.arange(nmaps), c["seed"], 1.0)
+    maps_in[ks] = ref_maps + inputs.white_noise(nside, ks, c["seed"], c["noise_sigma"])
+    got_alm = _gpu_analysis(plan, maps_in)
+    ref_alm = O.analysis(nside, lmax, maps_in[ks])
+    assert inputs.rel_err(got_alm[ks], ref_alm) <= TOL
+    plan.destroy()
+
+
+def test_host_entries_match_device_entries():
+    import torch
+    from paper_2208_10154_b200.binding import Plan
+    nside, lmax, nmaps = 16, 47, 200
+    alm = inputs.gaussian_alm(lmax, np.arange(nmaps), 5)
+    plan = Plan(nside, lmax, nmaps, 0)
+    dev_maps = _gpu_synthesis(plan, alm)
+    host_maps = np.full_like(dev_maps, np.nan)
+    plan.sht_synthesis_host(np.ascontiguousarray(alm), host_maps)
+    assert np.array_equal(host_maps, dev_maps)
+    dev_alm = _gpu_analysis(plan, dev_maps)
+    host_alm = np.full_like(dev_alm, np.nan)
+    plan.sht_analysis_host(dev_maps, host_alm)
+    assert np.array_equal(host_alm, dev_alm)
+    plan.destroy()
+
+
+def test_iterative_analysis_small():
+    import torch
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan
+    nside, lmax, nmaps, niter = 16, 31, 5, 3
+    alm_true = inputs.gaussian_alm(lmax, np.arange(nmaps), 77)
+    maps = O.synthesis(nside, lmax, alm_true)
+    ref_alm, ref_rms = O.analysis_iter(nside, lmax, maps, niter)
+    plan = Plan(nside, lmax, nmaps, 0)
+    mp = torch.from_numpy(maps).to(_dev())
+    alm = torch.zeros((nmaps, 1, plan.nalm), dtype=torch.complex128, device=_dev())
+    rms = torch.zeros((niter, nmaps), dtype=torch.float64, device=_dev())
+    plan.sht_analysis_iter(mp, alm, niter, rms)
+    torch.cuda.synchronize()
+    assert inputs.rel_err(alm.cpu().numpy(), ref_alm) <= TOL
+    # rms falls by orders of magnitude per round: compare relative to the first residual
+    assert np.abs(rms.cpu().numpy() - ref_rms).max() <= 1e-9 * ref_rms[0].max()
+    plan.destroy()
