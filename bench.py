@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark: batched FP64 analysis + synthesis of HEALPix maps on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch: sht_synthesis (a_lm -> maps) followed by
+sht_analysis (maps -> a_lm) of all `nmaps` maps of the workload (BASELINE.json metric: maps/s of
+analysis+synthesis in FP64 at nside=512, lmax=1535; workload = BASELINE.json configs[2], K = 1000 maps).
+`value` is measured with inputs resident in HBM; `e2e` through the host-buffer C-ABI entries
+(sht_synthesis_host / sht_analysis_host) with pinned host buffers, H2D/D2H inside the timed region.
+N > 1 (torchrun): every rank runs the same workload on its own maps (weak scaling, no collective on the
+data path; maps are independent units).
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+from paper_2208_10154_b200 import inputs  # noqa: E402
+
+METRIC = "maps/sec (analysis+synthesis, FP64) at nside=512 lmax=1535"
+FP64_NOMINAL_TFLOPS = 37.2     # 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz
+
+
+def read_measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0}, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def legendre_flops_per_direction(c):
+    """folded, unpruned algorithmic flops n_alm * N_h * 2K * 2 (x4 for spin 2)."""
+    f = inputs.nalm(c["lmax"]) * (2 * c["nside"]) * 2 * c["nmaps"] * 2
+    return f * (4 if c["spin"] == 2 else 1)
+
+
+def min_hbm_bytes_per_direction(c, kpad):
+    ncomp = 2 if c["spin"] == 2 else 1
+    maps = 8 * inputs.npix(c["nside"]) * c["nmaps"] * ncomp
+    alm = 16 * inputs.nalm(c["lmax"]) * c["nmaps"] * ncomp
+    F = 16 * (c["lmax"] + 1) * (2 * c["nside"]) * 2 * c["nmaps"] * ncomp
+    return maps + alm + 2 * F
+
+
+def cpu_baseline(c, nsample=8, stride=16):
+    """The oracle as it stands, timed on the host cores on a bounded sample: `nsample` maps, every
+    `stride`-th ring for synthesis and every `stride`-th m for analysis; cost extrapolated x stride
+    (rings and m values are sampled uniformly, so the sample has the workload's cost mix)."""
+    from oracle import oracle as O
+    nside, lmax = c["nside"], c["lmax"]
+    ks = np.arange(nsample)
+    alm = inputs.gaussian_alm(lmax, ks, c["seed"], c["spin"])
+    rl = list(range(1, 4 * nside, stride))
+    ml = list(range(0, lmax + 1, stride))
+    t0 = time.time()
+    maps = O.synthesis(nside, lmax, alm, spin=c["spin"], rlist=rl)
+    t1 = time.time()
+    O.analysis(nside, lmax, maps, spin=c["spin"], mlist=ml)
+    t2 = time.time()
+    fr = len(rl) / (4 * nside - 1)
+    fm = len(ml) / (lmax + 1)
+    t_full = (t1 - t0) / fr + (t2 - t1) / fm
+    return {"value": nsample / t_full, "unit": "maps/s", "cores": O.num_threads(), "kind": "oracle",
+            "sample": "%d maps; synthesis of every %dth ring (%d of %d) + analysis of every %dth m (%d of %d), "
+                      "time extrapolated to all rings / all m; %.1f s of wall time"
+                      % (nsample, stride, len(rl), 4 * nside - 1, stride, len(ml), lmax + 1, t2 - t0)}
+
+
+def run_reference(args, c):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    vals = []
+    for _ in range(args.warmup):
+        cpu_baseline(c, nsample=2, stride=64)
+    last = None
+    for _ in range(args.steps):
+        last = cpu_baseline(c, nsample=4, stride=32)
+        vals.append(last["value"])
+    v = float(np.mean(vals))
+    last["value"] = v
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "maps/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * c["nmaps"] / v,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": c["name"], "nside": c["nside"], "lmax": c["lmax"], "nmaps": c["nmaps"],
+                       "spin": c["spin"]},
+            "cpu_baseline": last,
+            "e2e": {"value": v, "unit": "maps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--nmaps", type=int, default=0, help="override the workload's map count (debug only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    c = dict(inputs.CONFIGS[args.config])
+    if args.nmaps:
+        c["nmaps"] = args.nmaps
+        c["name"] += "_nmaps%d_DEBUG" % args.nmaps
+    if args.impl == "reference":
+        return run_reference(args, c)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2208_10154_b200.binding import Plan, sht_measure_fp64_mma_peak
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    nside, lmax, nmaps, spin = c["nside"], c["lmax"], c["nmaps"], c["spin"]
+    ncomp = 2 if spin == 2 else 1
+    npix, nalm = inputs.npix(nside), inputs.nalm(lmax)
+
+    # ---- seeded synthetic inputs, resident in HBM (each rank its own maps: weak scaling) --------------
+    alm = torch.empty((nmaps, ncomp, nalm), dtype=torch.complex128, device=dev)
+    blk = 50
+    for k0 in range(0, nmaps, blk):
+        ks = np.arange(k0, min(nmaps, k0 + blk)) + rank * nmaps
+        alm[k0:k0 + len(ks)] = torch.from_numpy(inputs.gaussian_alm(lmax, ks, c["seed"], spin)).to(dev)
+    maps = torch.empty((nmaps, ncomp, npix), dtype=torch.float64, device=dev)
+    alm_out = torch.empty_like(alm)
+
+    t0 = time.time()
+    plan = Plan(nside, lmax, nmaps, spin)
+    torch.cuda.synchronize()
+    plan_s = time.time() - t0
+    stream = torch.cuda.current_stream()
+
+    def step():
+        plan.sht_synthesis(alm, maps, stream)
+        plan.sht_analysis(maps, alm_out, stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    plan.sht_plan_set_timing(True)
+    l0 = plan.kernel_launches()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    launches = plan.kernel_launches() - l0
+    stage_ms, stage_n = plan.sht_plan_stage_ms()
+    plan.sht_plan_set_timing(False)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * nmaps / (ms_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (Legendre contraction, both directions) -----------------------
+    peaks, peak_src = read_measured_peaks()
+    fl_dir = legendre_flops_per_direction(c)
+    leg_ms = stage_ms[1] + stage_ms[2]
+    leg_n = max(1, stage_n[1] + stage_n[2])
+    leg_launch_ms = leg_ms / leg_n
+    flops_per_launch = fl_dir * 2 * args.steps / leg_n
+    achieved = flops_per_launch / (leg_launch_ms * 1e-3) * 1e-12
+    mma_peak = sht_measure_fp64_mma_peak(300.0)
+    roofline = {"bound": "tensor", "kernel": "k_legendre_analysis + k_legendre_synthesis (DMMA.8x8x4, FP64)",
+                "achieved": achieved, "peak": mma_peak, "unit": "TFLOP/s", "frac": achieved / mma_peak,
+                "traffic": None,
+                "peak_source": "FP64 DMMA.8x8x4 register-resident loop measured live in this run "
+                               "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = %.1f; "
+                               "rule-derived bf16 %s x 45/2250 = %.1f)"
+                               % (FP64_NOMINAL_TFLOPS, peak_src, peaks.get("bf16_tflops", 0) * 45.0 / 2250.0),
+                "algorithmic_flops_per_launch": flops_per_launch, "launch_ms": leg_launch_ms,
+                "share_of_step": leg_ms / ms_total}
+    ring_ms = stage_ms[0] + stage_ms[3]
+    ring_bytes = 2 * args.steps * (8 * npix * nmaps * ncomp + 16 * (lmax + 1) * 2 * nside * 2 * nmaps * ncomp)
+    ring_gbs = ring_bytes / (ring_ms * 1e-3) * 1e-9 if ring_ms > 0 else None
+    stages = {"ring_fft_analysis_ms": stage_ms[0] / args.steps, "legendre_analysis_ms": stage_ms[1] / args.steps,
+              "legendre_synthesis_ms": stage_ms[2] / args.steps, "ring_fft_synthesis_ms": stage_ms[3] / args.steps,
+              "ring_fft_hbm": {"bound": "hbm", "achieved": ring_gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
+                               "frac": (ring_gbs / peaks["hbm_gbs"]) if ring_gbs else None,
+                               "algorithmic_bytes": "maps (8 B/px) + workspace (16 B per (m, ring, map))",
+                               "peak_source": peak_src},
+              "min_hbm_bytes_per_direction": min_hbm_bytes_per_direction(c, 0)}
+
+    # ---- end to end through the host-buffer ABI entries ------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        try:
+            h_alm = torch.empty((nmaps, ncomp, nalm), dtype=torch.complex128).pin_memory()
+            h_maps = torch.empty((nmaps, ncomp, npix), dtype=torch.float64).pin_memory()
+            h_alm_out = torch.empty((nmaps, ncomp, nalm), dtype=torch.complex128).pin_memory()
+            h_alm.copy_(alm.cpu())
+            # device buffers of the resident run are not needed any more
+            del alm_out
+            torch.cuda.empty_cache()
+            plan.sht_synthesis_host(h_alm, h_maps)          # warm-up (also allocates the staging buffers)
+            plan.sht_analysis_host(h_maps, h_alm_out)
+            if world > 1:
+                dist.barrier()
+            nrep = max(1, min(args.steps, 2))
+            t0 = time.perf_counter()
+            for _ in range(nrep):
+                plan.sht_synthesis_host(h_alm, h_maps)
+                plan.sht_analysis_host(h_maps, h_alm_out)
+            torch.cuda.synchronize()
+            dt = (time.perf_counter() - t0) / nrep
+            if world > 1:
+                t = torch.tensor([dt], dtype=torch.float64, device=dev)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                dt = float(t.item())
+            bytes_alm = h_alm.numel() * 16
+            bytes_maps = h_maps.numel() * 8
+            e2e = {"value": world * nmaps / dt, "unit": "maps/s", "h2d_bytes_per_step": bytes_alm + bytes_maps,
+                   "d2h_bytes_per_step": bytes_alm + bytes_maps, "ms_per_step": dt * 1e3,
+                   "api": "sht_synthesis_host + sht_analysis_host (pinned host buffers, chunked H2D/compute/D2H)"}
+        except Exception as ex:  # host memory too small for pinned copies of the workload, etc.
+            e2e = {"value": None, "unit": "maps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                   "error": str(ex)[:200]}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_baseline(c)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": "maps/s", "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": c["name"], "nside": nside, "lmax": lmax, "nmaps_per_gpu": nmaps, "spin": spin,
+                           "l2": "inputs (%.1f GB maps, %.1f GB a_lm per GPU) are far larger than the 126 MB L2"
+                                 % (8e-9 * npix * nmaps * ncomp, 16e-9 * nalm * nmaps * ncomp),
+                           "plan_create_s": plan_s, "chunk_maps": plan.chunk_maps(),
+                           "workspace_GB": plan.workspace_bytes() * 1e-9},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                "stages": stages, "cpu_baseline": cpu}
+        print(json.dumps(line))
+    plan.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -83,6 +83,14 @@ long long sht_plan_kernel_launches(sht_plan_t plan); /* kernels launched by this
 const char* sht_status_string(sht_status_t s);       /* static storage                              */
 const char* sht_last_error(sht_plan_t plan);         /* plan-owned, valid until the next call       */
 
+/* Per-stage device timing (measurement only; PAPER.md:54 quotes the FFT + FFT-mapping share of the time).
+ * With timing enabled every kernel launched by the plan on the caller's stream is bracketed by CUDA events.
+ * sht_plan_stage_ms waits for the recorded events and returns, accumulated since the last call, the device
+ * milliseconds ms[4] and launch counts n[4] of: 0 ring-FFT analysis, 1 Legendre analysis, 2 Legendre synthesis,
+ * 3 ring-FFT synthesis; then resets the accumulation.  At most 256 launches are kept between two calls. */
+sht_status_t sht_plan_set_timing(sht_plan_t plan, int enable);
+sht_status_t sht_plan_stage_ms(sht_plan_t plan, double* ms4, int* n4);
+
 /* Measurement helper used by bench.py for the roofline denominator: runs a register-resident
  * DMMA.8x8x4 loop on every SM for about `ms` milliseconds and returns the sustained FP64
  * tensor-core rate in TFLOP/s (<= 0 on error).  Not part of the transform path. */

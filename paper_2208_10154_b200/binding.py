@@ -50,6 +50,10 @@ _lib.sht_status_string.argtypes = [_i]
 _lib.sht_status_string.restype = ctypes.c_char_p
 _lib.sht_last_error.argtypes = [_vp]
 _lib.sht_last_error.restype = ctypes.c_char_p
+_lib.sht_plan_set_timing.argtypes = [_vp, _i]
+_lib.sht_plan_set_timing.restype = _i
+_lib.sht_plan_stage_ms.argtypes = [_vp, ctypes.POINTER(_d), ctypes.POINTER(_i)]
+_lib.sht_plan_stage_ms.restype = _i
 _lib.sht_measure_fp64_mma_peak.argtypes = [_d]
 _lib.sht_measure_fp64_mma_peak.restype = _d
 
@@ -57,7 +61,7 @@ EXPORTED = [
     "sht_plan_create", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter",
     "sht_analysis_host", "sht_synthesis_host", "sht_npix", "sht_nalm", "sht_alm_index",
     "sht_plan_workspace_bytes", "sht_plan_chunk_maps", "sht_plan_kernel_launches", "sht_status_string",
-    "sht_last_error", "sht_measure_fp64_mma_peak",
+    "sht_last_error", "sht_measure_fp64_mma_peak", "sht_plan_set_timing", "sht_plan_stage_ms",
 ]
 
 
@@ -136,6 +140,16 @@ class Plan:
 
     def sht_synthesis_host(self, alm_host, maps_host):
         self._check(_lib.sht_synthesis_host(self._h, _ptr(alm_host), _ptr(maps_host)), "sht_synthesis_host")
+
+    def sht_plan_set_timing(self, enable):
+        self._check(_lib.sht_plan_set_timing(self._h, 1 if enable else 0), "sht_plan_set_timing")
+
+    def sht_plan_stage_ms(self):
+        """-> (ms[4], n[4]) for ring-FFT analysis, Legendre analysis, Legendre synthesis, ring-FFT synthesis"""
+        ms = (_d * 4)()
+        n = (_i * 4)()
+        self._check(_lib.sht_plan_stage_ms(self._h, ms, n), "sht_plan_stage_ms")
+        return list(ms), list(n)
 
     def workspace_bytes(self):
         return int(_lib.sht_plan_workspace_bytes(self._h))

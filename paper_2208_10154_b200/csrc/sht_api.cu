@@ -66,21 +66,67 @@ static sht_status_t cuda_fail(sht_plan_t pl, const char* what, cudaError_t e)
         if (e__ != cudaSuccess) return cuda_fail(pl, what, e__); \
     } while (0)
 
-// maps[kmap0 .. kmap0+kmaps) -> alm[kalm0 .. kalm0+kmaps)
-static sht_status_t analysis_chunk(sht_plan_t pl, const double* maps, int kmap0, double* alm, int kalm0, double* F,
-                                   int kmaps, bool accumulate, cudaStream_t st)
+// ---- optional per-stage timing ---------------------------------------------------------------------
+static int timing_begin(sht_plan_t pl, int stage, cudaStream_t st)
 {
-    SHT_TRY(launch_ring_analysis(pl, maps, F, kmap0, kmaps, st), "ring analysis");
-    SHT_TRY(launch_legendre_analysis(pl, F, alm, kalm0, kmaps, accumulate, st), "legendre analysis");
+    if (!pl->timing || pl->n_ev >= 256) return -1;
+    const int i = pl->n_ev++;
+    if (!pl->ev0[i]) { cudaEventCreate(&pl->ev0[i]); cudaEventCreate(&pl->ev1[i]); }
+    pl->ev_stage[i] = stage;
+    cudaEventRecord(pl->ev0[i], st);
+    return i;
+}
+static void timing_end(sht_plan_t pl, int i, cudaStream_t st)
+{
+    if (i >= 0) cudaEventRecord(pl->ev1[i], st);
+}
+
+extern "C" sht_status_t sht_plan_set_timing(sht_plan_t pl, int enable)
+{
+    if (!pl) return SHT_ERR_NULL;
+    pl->timing = enable != 0;
+    pl->n_ev = 0;
+    return SHT_OK;
+}
+
+extern "C" sht_status_t sht_plan_stage_ms(sht_plan_t pl, double* ms4, int* n4)
+{
+    if (!pl || !ms4 || !n4) return SHT_ERR_NULL;
+    for (int s = 0; s < 4; ++s) { ms4[s] = 0.0; n4[s] = 0; }
+    for (int i = 0; i < pl->n_ev; ++i) {
+        float t = 0.f;
+        cudaError_t e = cudaEventSynchronize(pl->ev1[i]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, pl->ev0[i], pl->ev1[i]);
+        if (e != cudaSuccess) { snprintf(pl->err, sizeof(pl->err), "stage timing: %s", cudaGetErrorString(e)); return SHT_ERR_CUDA; }
+        ms4[pl->ev_stage[i]] += t; n4[pl->ev_stage[i]]++;
+    }
+    pl->n_ev = 0;
+    return SHT_OK;
+}
+
+// maps[kmap0 .. kmap0+kmaps) -> alm[kalm0 .. kalm0+kmaps)
+static sht_status_t analysis_chunk(sht_plan_t pl, const DevicePlan& d, const double* maps, int kmap0, double* alm,
+                                   int kalm0, double* F, int kmaps, bool accumulate, cudaStream_t st)
+{
+    int t = timing_begin(pl, 0, st);
+    SHT_TRY(launch_ring_analysis(pl, d, maps, F, kmap0, kmaps, st), "ring analysis");
+    timing_end(pl, t, st);
+    t = timing_begin(pl, 1, st);
+    SHT_TRY(launch_legendre_analysis(pl, d, F, alm, kalm0, kmaps, accumulate, st), "legendre analysis");
+    timing_end(pl, t, st);
     return SHT_OK;
 }
 
 // alm[kalm0 ..) -> maps[kmap0 ..); with sub_from: maps = sub_from[ksub0 ..] - synthesis
-static sht_status_t synthesis_chunk(sht_plan_t pl, const double* alm, int kalm0, double* maps, int kmap0, double* F,
-                                    int kmaps, const double* sub_from, int ksub0, cudaStream_t st)
+static sht_status_t synthesis_chunk(sht_plan_t pl, const DevicePlan& d, const double* alm, int kalm0, double* maps,
+                                    int kmap0, double* F, int kmaps, const double* sub_from, int ksub0, cudaStream_t st)
 {
-    SHT_TRY(launch_legendre_synthesis(pl, alm, F, kalm0, kmaps, st), "legendre synthesis");
-    SHT_TRY(launch_ring_synthesis(pl, F, maps, kmap0, kmaps, sub_from, ksub0, st), "ring synthesis");
+    int t = timing_begin(pl, 2, st);
+    SHT_TRY(launch_legendre_synthesis(pl, d, alm, F, kalm0, kmaps, st), "legendre synthesis");
+    timing_end(pl, t, st);
+    t = timing_begin(pl, 3, st);
+    SHT_TRY(launch_ring_synthesis(pl, d, F, maps, kmap0, kmaps, sub_from, ksub0, st), "ring synthesis");
+    timing_end(pl, t, st);
     return SHT_OK;
 }
 
@@ -91,7 +137,7 @@ extern "C" sht_status_t sht_analysis(sht_plan_t pl, const double* maps, double* 
     cudaStream_t st = (cudaStream_t)stream;
     for (int k0 = 0; k0 < pl->nmaps; k0 += pl->chunk) {
         const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
-        sht_status_t s = analysis_chunk(pl, maps, k0, alm, k0, pl->F, kmaps, false, st);
+        sht_status_t s = analysis_chunk(pl, pl->d, maps, k0, alm, k0, pl->F, kmaps, false, st);
         if (s != SHT_OK) return s;
     }
     return SHT_OK;
@@ -104,7 +150,7 @@ extern "C" sht_status_t sht_synthesis(sht_plan_t pl, const double* alm, double* 
     cudaStream_t st = (cudaStream_t)stream;
     for (int k0 = 0; k0 < pl->nmaps; k0 += pl->chunk) {
         const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
-        sht_status_t s = synthesis_chunk(pl, alm, k0, maps, k0, pl->F, kmaps, nullptr, 0, st);
+        sht_status_t s = synthesis_chunk(pl, pl->d, alm, k0, maps, k0, pl->F, kmaps, nullptr, 0, st);
         if (s != SHT_OK) return s;
     }
     return SHT_OK;
@@ -127,10 +173,10 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
     sht_status_t s = SHT_OK;
     for (int k0 = 0; k0 < pl->nmaps && s == SHT_OK; k0 += pl->chunk) {
         const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
-        s = analysis_chunk(pl, maps, k0, alm, k0, pl->F, kmaps, false, st);
+        s = analysis_chunk(pl, pl->d, maps, k0, alm, k0, pl->F, kmaps, false, st);
         for (int it = 0; it < niter && s == SHT_OK; ++it) {
             // r = map - synthesis(a): `res` is indexed from the chunk start, maps/alm from map 0
-            s = synthesis_chunk(pl, alm, k0, res, 0, pl->F, kmaps, maps, k0, st);
+            s = synthesis_chunk(pl, pl->d, alm, k0, res, 0, pl->F, kmaps, maps, k0, st);
             if (s != SHT_OK) break;
             if (resid_rms) {
                 const int nrow = kmaps * d.ncomp;
@@ -142,7 +188,7 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
                 pl->launches += 2;
                 SHT_TRY(cudaGetLastError(), "rms kernels");
             }
-            s = analysis_chunk(pl, res, 0, alm, k0, pl->F, kmaps, true, st);
+            s = analysis_chunk(pl, pl->d, res, 0, alm, k0, pl->F, kmaps, true, st);
         }
     }
     if (res) cudaFreeAsync(res, st);
@@ -155,9 +201,18 @@ static sht_status_t host_setup(sht_plan_t pl)
 {
     if (pl->host_ready) return SHT_OK;
     const DevicePlan& d = pl->d;
-    // chunk of the host path: at most kpad/2 maps (two chunks in flight), a multiple of the k-tile
-    int hc = pl->nmaps >= 2 * KTILE_MAPS ? ((pl->nmaps / 8 + KTILE_MAPS - 1) / KTILE_MAPS) * KTILE_MAPS : pl->nmaps;
-    if (hc > d.kpad) hc = d.kpad;
+    // chunk of the host path: two chunks are in flight and share the plan's workspace, each with
+    // host_kpad <= kpad/2 columns per row (a multiple of the k-tile); a single chunk if the plan is that small
+    int hc;
+    if (d.kpad >= 2 * KTILE_MAPS) {
+        hc = ((pl->nmaps / 8 + KTILE_MAPS - 1) / KTILE_MAPS) * KTILE_MAPS;
+        if (hc < KTILE_MAPS) hc = KTILE_MAPS;
+        if (hc > d.kpad / 2 / KTILE_MAPS * KTILE_MAPS) hc = d.kpad / 2 / KTILE_MAPS * KTILE_MAPS;
+        pl->host_kpad = hc;
+    } else {
+        hc = pl->chunk;
+        pl->host_kpad = d.kpad;
+    }
     pl->host_chunk = hc;
     const size_t mbytes = (size_t)hc * d.ncomp * d.npix * sizeof(double);
     const size_t abytes = (size_t)hc * d.ncomp * d.nalm * 2 * sizeof(double);
@@ -166,9 +221,6 @@ static sht_status_t host_setup(sht_plan_t pl)
         SHT_TRY(cudaMalloc((void**)&pl->stage_alm[i], abytes), "host-path alm staging");
         SHT_TRY(cudaStreamCreateWithFlags(&pl->hstream[i], cudaStreamNonBlocking), "host-path stream");
     }
-    // second workspace so that two chunks can be in flight; both hold kpad columns per row
-    SHT_TRY(cudaMalloc((void**)&pl->F2, pl->F_bytes), "host-path second workspace");
-    SHT_TRY(cudaMemset(pl->F2, 0, pl->F_bytes), "host-path workspace memset");
     pl->host_ready = true;
     return SHT_OK;
 }
@@ -182,19 +234,23 @@ static sht_status_t host_run(sht_plan_t pl, const double* in_host, double* out_h
     const DevicePlan& d = pl->d;
     const size_t map_elems = (size_t)d.ncomp * d.npix, alm_elems = (size_t)d.ncomp * d.nalm * 2;
     const size_t in_elems = analysis ? map_elems : alm_elems, out_elems = analysis ? alm_elems : map_elems;
+    DevicePlan dh = d;
+    dh.kpad = pl->host_kpad;
+    const bool two = (2 * (size_t)pl->host_kpad <= (size_t)d.kpad);
+    const size_t f_half = (size_t)d.nh * (d.lmax + 1) * d.ncomp * 2 * pl->host_kpad * 2;   // doubles per chunk workspace
     int idx = 0;
     for (int k0 = 0; k0 < pl->nmaps; k0 += pl->host_chunk, ++idx) {
-        const int b = idx & 1;
+        const int b = two ? (idx & 1) : 0;
         const int kmaps = pl->nmaps - k0 < pl->host_chunk ? pl->nmaps - k0 : pl->host_chunk;
         cudaStream_t st = pl->hstream[b];
         double* dmaps = pl->stage_maps[b]; double* dalm = pl->stage_alm[b];
         double* din = analysis ? dmaps : dalm; double* dout = analysis ? dalm : dmaps;
-        double* F = b ? pl->F2 : pl->F;
+        double* F = pl->F + (size_t)b * f_half;
         SHT_TRY(cudaMemcpyAsync(din, in_host + (size_t)k0 * in_elems, (size_t)kmaps * in_elems * sizeof(double),
                                 cudaMemcpyHostToDevice, st), "H2D");
         // staging buffers are indexed from the chunk start: pass k0 = 0
-        s = analysis ? analysis_chunk(pl, dmaps, 0, dalm, 0, F, kmaps, false, st)
-                     : synthesis_chunk(pl, dalm, 0, dmaps, 0, F, kmaps, nullptr, 0, st);
+        s = analysis ? analysis_chunk(pl, dh, dmaps, 0, dalm, 0, F, kmaps, false, st)
+                     : synthesis_chunk(pl, dh, dalm, 0, dmaps, 0, F, kmaps, nullptr, 0, st);
         if (s != SHT_OK) return s;
         SHT_TRY(cudaMemcpyAsync(out_host + (size_t)k0 * out_elems, dout, (size_t)kmaps * out_elems * sizeof(double),
                                 cudaMemcpyDeviceToHost, st), "D2H");

@@ -65,23 +65,28 @@ struct sht_plan_s {
     // host-entry staging (allocated on first use)
     double* stage_maps[2];
     double* stage_alm[2];
-    double* F2;                     // second workspace for the ping-pong host path
+    int host_kpad;                  // workspace columns per row in the host path (two chunks share F)
     int host_chunk;
     cudaStream_t hstream[2];
     bool host_ready;
+    // optional per-stage timing (sht_plan_set_timing)
+    bool timing;
+    int n_ev;
+    cudaEvent_t ev0[256], ev1[256];
+    int ev_stage[256];
 };
 
 namespace sht {
 
 // ring FFT stage (sht_ring_fft.cu)
-cudaError_t launch_ring_analysis(sht_plan_s* pl, const double* maps, double* F, int k0, int kmaps, cudaStream_t st);
+cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st);
 // maps of the chunk are maps[k0 .. k0+kmaps); if sub_from != nullptr the output is sub_from[ksub0 + k] - synthesis
-cudaError_t launch_ring_synthesis(sht_plan_s* pl, const double* F, double* maps, int k0, int kmaps,
+cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps,
                                   const double* sub_from, int ksub0, cudaStream_t st);
 // Legendre stage (sht_legendre.cu)
-cudaError_t launch_legendre_analysis(sht_plan_s* pl, const double* F, double* alm, int k0, int kmaps,
+cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st);
-cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
+cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
 // plan-time seed table (sht_plan.cu)
 cudaError_t launch_seed_table(const DevicePlan& d, const double* cm, int* lstart, double2* seed, cudaStream_t st);
 size_t ring_fft_smem_bytes(int max_ring, int kt);

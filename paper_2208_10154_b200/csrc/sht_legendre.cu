@@ -292,26 +292,26 @@ static size_t synthesis_smem()
     return a > b ? a : b;
 }
 
-cudaError_t launch_legendre_analysis(sht_plan_s* pl, const double* F, double* alm, int k0, int kmaps,
+cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st)
 {
-    const size_t sm = analysis_smem(pl->d.nh);
+    const size_t sm = analysis_smem(d.nh);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
-    k_legendre_analysis<<<(pl->d.lmax + 1) * nkt, LEG_THREADS, sm, st>>>(pl->d, F, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
+    k_legendre_analysis<<<(d.lmax + 1) * nkt, LEG_THREADS, sm, st>>>(d, F, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
 }
 
-cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const double* alm, double* F, int k0, int kmaps, cudaStream_t st)
+cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st)
 {
     const size_t sm = synthesis_smem();
     cudaError_t e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
-    const int npb = (pl->d.nh + S_PB - 1) / S_PB;
-    k_legendre_synthesis<<<(pl->d.lmax + 1) * nkt * npb, LEG_THREADS, sm, st>>>(pl->d, alm, F, k0, kmaps, nkt, npb);
+    const int npb = (d.nh + S_PB - 1) / S_PB;
+    k_legendre_synthesis<<<(d.lmax + 1) * nkt * npb, LEG_THREADS, sm, st>>>(d, alm, F, k0, kmaps, nkt, npb);
     pl->launches++;
     return cudaGetLastError();
 }

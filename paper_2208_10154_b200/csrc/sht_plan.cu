@@ -303,7 +303,10 @@ extern "C" sht_status_t sht_plan_destroy(sht_plan_t pl)
     cudaDeviceSynchronize();
     for (int i = 0; i < pl->n_allocs; ++i) cudaFree(pl->dev_allocs[i]);
     if (pl->F) cudaFree(pl->F);
-    if (pl->F2) cudaFree(pl->F2);
+    for (int i = 0; i < 256; ++i) {
+        if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
+        if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
+    }
     for (int i = 0; i < 2; ++i) {
         if (pl->stage_maps[i]) cudaFree(pl->stage_maps[i]);
         if (pl->stage_alm[i]) cudaFree(pl->stage_alm[i]);

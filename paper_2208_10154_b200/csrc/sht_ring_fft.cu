@@ -256,7 +256,7 @@ static int ring_kt_min(const sht_plan_s* pl)
     return pl->ring_kt_min;
 }
 
-cudaError_t launch_ring_analysis(sht_plan_s* pl, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
+cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
 {
     static bool attr_set = false;
     if (!attr_set) {
@@ -265,13 +265,13 @@ cudaError_t launch_ring_analysis(sht_plan_s* pl, const double* maps, double* F, 
         attr_set = true;
     }
     const int ktmin = ring_kt_min(pl);
-    dim3 grid((kmaps + ktmin - 1) / ktmin, pl->d.nh, pl->d.ncomp);
-    k_ring_analysis<<<grid, 256, pl->fft_smem, st>>>(pl->d, maps, F, k0, kmaps);
+    dim3 grid((kmaps + ktmin - 1) / ktmin, d.nh, d.ncomp);
+    k_ring_analysis<<<grid, 256, pl->fft_smem, st>>>(d, maps, F, k0, kmaps);
     pl->launches++;
     return cudaGetLastError();
 }
 
-cudaError_t launch_ring_synthesis(sht_plan_s* pl, const double* F, double* maps, int k0, int kmaps,
+cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps,
                                   const double* sub_from, int ksub0, cudaStream_t st)
 {
     static bool attr_set = false;
@@ -281,8 +281,8 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const double* F, double* maps,
         attr_set = true;
     }
     const int ktmin = ring_kt_min(pl);
-    dim3 grid((kmaps + ktmin - 1) / ktmin, pl->d.nh, pl->d.ncomp);
-    k_ring_synthesis<<<grid, 256, pl->fft_smem, st>>>(pl->d, F, maps, k0, kmaps, sub_from, ksub0);
+    dim3 grid((kmaps + ktmin - 1) / ktmin, d.nh, d.ncomp);
+    k_ring_synthesis<<<grid, 256, pl->fft_smem, st>>>(d, F, maps, k0, kmaps, sub_from, ksub0);
     pl->launches++;
     return cudaGetLastError();
 }
