@@ -236,6 +236,7 @@ static sht_status_t host_run(sht_plan_t pl, const double* in_host, double* out_h
     const size_t in_elems = analysis ? map_elems : alm_elems, out_elems = analysis ? alm_elems : map_elems;
     DevicePlan dh = d;
     dh.kpad = pl->host_kpad;
+    dh.nkg = dh.kpad / KG;
     const bool two = (2 * (size_t)pl->host_kpad <= (size_t)d.kpad);
     const size_t f_half = (size_t)d.nh * (d.lmax + 1) * d.ncomp * 2 * pl->host_kpad * 2;   // doubles per chunk workspace
     int idx = 0;

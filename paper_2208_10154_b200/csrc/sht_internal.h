@@ -1,5 +1,6 @@
 // sht_internal.h -- plan structure and kernel launchers of the B200 batched-SHT library (not installed).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cstddef>
 #include <cstdint>
@@ -7,10 +8,15 @@
 
 namespace sht {
 
-// ---- tile constants shared by the ring-FFT and Legendre kernels --------------------------------
-constexpr int KTILE_MAPS = 64;               // maps per Legendre k-tile
+// ---- constants shared by the ring-FFT and Legendre kernels ------------------------------------------
+constexpr int KG = 4;                        // maps per workspace group (one 128-byte line = E|O of 4 maps)
+constexpr int KTILE_MAPS = 64;               // maps per Legendre k-tile (spin 0); spin 2: 32 (Q,U) pairs
 constexpr int NK = 2 * KTILE_MAPS;           // real columns per k-tile (re,im interleaved)
 constexpr int MAX_RADIX_LIST = 16;           // factors of one ring length
+constexpr int RING_THREADS = 512;            // threads per CTA of the ring kernels
+constexpr int RING_EMAX = 8192;              // complex elements (ring length x maps) one ring CTA holds in smem
+constexpr int RING_EMAX_OOP = 6400;          // same for rings that need an out-of-place pass (two buffers)
+constexpr int RING_NCLASS = 4;               // launch classes of the ring kernels (by dynamic smem size)
 
 // One folded ring pair p = 0 .. nh-1: north ring i = p+1 and its mirror 4 nside - i (PAPER.md:211 grid;
 // north_star: "ring pairs symmetric about the equator folded").  The equator (p = nh-1) has no partner.
@@ -20,30 +26,40 @@ struct RingPair {
     long long start_n;     // first pixel of the north ring
     long long start_s;     // first pixel of the south ring, -1 for the equator
     int tw_off;            // offset (double2 units) of this ring length's table W_{2n}[j] = exp(-i pi j / n)
-    int fac_off;           // offset into the radix list
+    int fac_off;           // offset into the radix list (forward order; the inverse transform runs it backwards)
     int nfac;              // number of radix passes
-    int kt;                // maps per CTA of the ring-FFT kernels for this ring length
-    // Bluestein (chirp-z) for ring lengths with a large prime factor: nb = 0 means plain mixed radix
-    int nb;                // power-of-two convolution length >= 2n-1 (0 if unused)
-    int chirp_off;         // offset (double2) of chirp[j] = exp(-i pi j^2 / n), j = 0..n-1
-    int bfilt_off;         // offset (double2) of FFT_nb(conj-chirp filter) / nb
-    int btw_off;           // offset (double2) of W_{nb}[j] = exp(-2 pi i j / nb), j = 0..nb-1
+    int kt;                // maps per CTA of the ring kernels for this ring length (power of two <= 16)
+    int oop;               // 1: the radix list has a second generic (prime >= 11) pass, done out of place
+    int mlim;              // only m < mlim are needed from / for this ring (ring optimisation)
+    int perm_off;          // offset of this ring length's table perm[bin] = position after the forward transform
 };
 
 struct DevicePlan {
     int nside, lmax, spin, ncomp, nh;
     long long npix, nalm;
-    int kpad;                       // complex columns per workspace row (multiple of KTILE_MAPS)
+    int kpad;                       // map slots per workspace row (multiple of KTILE_MAPS)
+    int nkg;                        // kpad / KG
     const RingPair* rings;          // [nh]
     const double* z;                // [nh] cos(theta_p)
     const double* sin2;             // [nh] sin^2(theta_p)
     const double2* tw;              // all twiddle tables
     const int* radix;               // all radix lists
+    const unsigned short* perm;     // all digit-reversal tables (bin -> position in the transformed buffer)
     const double2* coef;            // [nalm] (alpha_lm, beta_lm), m-major like alm
     const int* lstart;              // [lmax+1][nh] l_safe(m, p)
     const double2* seed;            // [lmax+1][nh] (lambda_{ls-1}, lambda_{ls-2})
     const double2* spin2c;          // [lmax+1] per-l constants for spin 2 (unused for spin 0)
+    const int* mlim;                // [nh] copy of RingPair::mlim (monotone non-decreasing in p)
 };
+
+// Workspace F (both directions): T_m^k(theta) of PAPER.md:52 for one chunk of maps,
+//   F[p][kg][m][comp][h][kk][re,im]   doubles,   kg = k / KG, kk = k % KG,
+// h = 0/1 = E/O (north+south, north-south) on the analysis side, north/south on the synthesis side.
+// One (p, kg, m, comp) cell is a 128-byte line.  Returns the double2 index of (.., h, kk = 0).
+__host__ __device__ __forceinline__ size_t f_cell(const DevicePlan& d, int p, int kg, int m, int comp, int h)
+{
+    return (((((size_t)p * d.nkg + kg) * (size_t)(d.lmax + 1) + m) * d.ncomp + comp) * 2 + h) * KG;
+}
 
 }  // namespace sht
 
@@ -51,14 +67,16 @@ struct sht_plan_s {
     sht::DevicePlan d;
     int nmaps;
     int chunk;                      // maps per internal chunk
-    double* F;                      // workspace [nh][lmax+1][ncomp][2][kpad][2]
+    double* F;                      // workspace, layout above
     size_t F_bytes;
     size_t table_bytes;
-    void* dev_allocs[24];
+    void* dev_allocs[32];
     int n_allocs;
-    int max_ring;                   // largest ring length
-    int ring_kt_min;                // maps per ring-kernel CTA at the largest ring length
-    size_t fft_smem;                // dynamic smem of the ring kernels
+    // ring-kernel launch classes: rings grouped by the dynamic shared memory their CTA needs
+    int* class_rings[sht::RING_NCLASS];     // device lists of ring-pair indices
+    int class_count[sht::RING_NCLASS];
+    int class_ktmin[sht::RING_NCLASS];      // smallest kt in the class (decides grid.x)
+    size_t class_smem[sht::RING_NCLASS];
     int sm_count;
     long long launches;
     char err[512];
@@ -89,6 +107,5 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
 // plan-time seed table (sht_plan.cu)
 cudaError_t launch_seed_table(const DevicePlan& d, const double* cm, int* lstart, double2* seed, cudaStream_t st);
-size_t ring_fft_smem_bytes(int max_ring, int kt);
 
 }  // namespace sht

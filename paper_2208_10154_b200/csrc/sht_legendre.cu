@@ -72,7 +72,10 @@ k_legendre_analysis(DevicePlan d, const double* __restrict__ F, double* __restri
         {
             int lo = 0, hi = nh;                     // first p with lsp[p] < l0 + A_ML
             while (lo < hi) { int mid = (lo + hi) >> 1; if (lsp[mid] < l0 + A_ML) hi = mid; else lo = mid + 1; }
-            pstart = lo & ~3;
+            // rings with mlim[p] <= m were never written to the workspace (and have lambda = 0 throughout)
+            int lo2 = 0, hi2 = nh;
+            while (lo2 < hi2) { int mid = (lo2 + hi2) >> 1; if (d.mlim[mid] > m) hi2 = mid; else lo2 = mid + 1; }
+            pstart = lo > lo2 ? lo : lo2;
         }
         if (tid < A_ML) {
             const int l = l0 + tid;
@@ -94,8 +97,8 @@ k_legendre_analysis(DevicePlan d, const double* __restrict__ F, double* __restri
                 const int p = pc + r;
                 double2 v = make_double2(0.0, 0.0);
                 if (p < nh) {
-                    const size_t row = (((size_t)p * (lmax + 1) + m) * d.ncomp + comp) * 2 + h;
-                    v = Fc[row * d.kpad + (size_t)kt * KTILE_MAPS + col2];
+                    const int k = kt * KTILE_MAPS + col2;
+                    v = Fc[f_cell(d, p, k >> 2, m, comp, h) + (k & 3)];
                 }
                 *reinterpret_cast<double2*>(&S.X[h][r][2 * col2]) = v;
             }
@@ -197,6 +200,7 @@ k_legendre_synthesis(DevicePlan d, const double* __restrict__ alm, double* __res
     }
     // the ring of the block closest to the equator starts first (l_safe decreases with p)
     const int plast = min(pb + S_PB, nh) - 1;
+    if (m >= d.mlim[plast]) return;                    // no ring of this block takes part in order m (never read)
     const int lfirst = d.lstart[(size_t)m * nh + plast];
     const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
     const double2* almc = reinterpret_cast<const double2*>(alm);
@@ -278,10 +282,10 @@ k_legendre_synthesis(DevicePlan d, const double* __restrict__ alm, double* __res
         if (p >= nh) continue;
         const double2 ee = *reinterpret_cast<const double2*>(&Cs[r * SC + 2 * col2]);
         const double2 oo = *reinterpret_cast<const double2*>(&Cs[(S_PB + r) * SC + 2 * col2]);
-        const size_t row = (((size_t)p * (lmax + 1) + m) * d.ncomp + comp) * 2;
-        double2* dst = Fc + row * d.kpad + (size_t)kt * KTILE_MAPS + col2;
+        const int k = kt * KTILE_MAPS + col2;
+        double2* dst = Fc + f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
         dst[0] = make_double2(ee.x + oo.x, ee.y + oo.y);
-        dst[d.kpad] = make_double2(ee.x - oo.x, ee.y - oo.y);
+        dst[KG] = make_double2(ee.x - oo.x, ee.y - oo.y);
     }
 }
 

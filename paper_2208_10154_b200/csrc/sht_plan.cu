@@ -84,22 +84,21 @@ using namespace sht;
 // ------------------------------------------------------------------------------------------------
 static const long double PI_LD = 3.14159265358979323846264338327950288419716939937510L;
 
-static void factorize_ring(int n, std::vector<int>& out)
+// Radix list of ring length n = 4 q in forward (analysis) order: primes >= 11 first (largest first; the first
+// pass is fused with the global load, further ones run out of place), then 4s, a 2, and the 3s, 5s, 7s,
+// which run in place.  The inverse transform (synthesis) walks the same list backwards.
+static int factorize_ring(int n, std::vector<int>& out)
 {
-    // n = 4 q.  Radix-4 passes first, then 2, then the odd primes of q in increasing order.
+    std::vector<int> small, big;
     int r = n;
-    while (r % 4 == 0) { out.push_back(4); r /= 4; }
-    while (r % 2 == 0) { out.push_back(2); r /= 2; }
+    while (r % 4 == 0) { small.push_back(4); r /= 4; }
+    while (r % 2 == 0) { small.push_back(2); r /= 2; }
     for (int f = 3; (long long)f * f <= r; f += 2)
-        while (r % f == 0) { out.push_back(f); r /= f; }
-    if (r > 1) out.push_back(r);
-}
-
-static int largest_factor(const std::vector<int>& f)
-{
-    int m = 1;
-    for (int v : f) m = v > m ? v : m;
-    return m;
+        while (r % f == 0) { (f <= 7 ? small : big).push_back(f); r /= f; }
+    if (r > 1) (r <= 7 ? small : big).push_back(r);
+    for (size_t i = big.size(); i-- > 0;) out.push_back(big[i]);
+    for (int v : small) out.push_back(v);
+    return (int)big.size();
 }
 
 template <typename T>
@@ -123,23 +122,19 @@ static sht_status_t fail(sht_plan_s* pl, sht_status_t s, const char* what, cudaE
     return s;
 }
 
-// maps per CTA of the ring kernels: as many as fit next to one scratch ring in the smem budget,
-// a power of two <= 16 so that workspace runs are 32-byte-sector aligned.
-static int ring_kt(int n, size_t budget)
+// maps per CTA of the ring kernels: the largest power of two <= 16 whose rings fit the CTA's element budget
+static int ring_kt(int n, int cap)
 {
-    long long fit = (long long)(budget / ((size_t)n * sizeof(double2))) - 1;
     int kt = 1;
-    while (kt * 2 <= fit && kt < 16) kt *= 2;
+    while (kt * 2 <= 16 && kt * 2 * n <= cap) kt *= 2;
     return kt;
 }
-
-size_t sht::ring_fft_smem_bytes(int n, int kt) { return (size_t)(kt + 1) * n * sizeof(double2); }
 
 extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, int nmaps, int spin)
 {
     if (!out) return SHT_ERR_NULL;
     *out = nullptr;
-    if (nside < 1 || nside > 8192 || lmax < 0 || nmaps < 1 || (spin != 0 && spin != 2)) return SHT_ERR_INVALID_ARG;
+    if (nside < 1 || nside > 2048 || lmax < 0 || nmaps < 1 || (spin != 0 && spin != 2)) return SHT_ERR_INVALID_ARG;
     if (spin == 2 && lmax < 2) return SHT_ERR_INVALID_ARG;
     if (lmax > 16383) return SHT_ERR_UNSUPPORTED;
 
@@ -161,15 +156,14 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
     cudaDeviceProp prop;
     cudaGetDeviceProperties(&prop, dev);
     pl->sm_count = prop.multiProcessorCount;
-    const size_t smem_budget = 200 * 1024;
-
     // ---- ring pairs, twiddles, radix lists ----------------------------------------------------
     std::vector<RingPair> rings(d.nh);
     std::vector<double> zs(d.nh), sin2s(d.nh);
     std::vector<double2> tw;
     std::vector<int> radix;
-    std::vector<int> tw_off_of_q(nside + 1, -1), fac_off_of_q(nside + 1, -1), nfac_of_q(nside + 1, 0);
-    pl->max_ring = 4 * nside;
+    std::vector<unsigned short> perm;
+    std::vector<int> perm_off_of_q(nside + 1, 0);
+    std::vector<int> tw_off_of_q(nside + 1, -1), fac_off_of_q(nside + 1, -1), nfac_of_q(nside + 1, 0), nbig_of_q(nside + 1, 0);
     for (int q = 1; q <= nside; ++q) {
         const int n = 4 * q;
         tw_off_of_q[q] = (int)tw.size();
@@ -178,12 +172,19 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
             tw.push_back(make_double2((double)cosl(ang), (double)-sinl(ang)));
         }
         std::vector<int> f;
-        factorize_ring(n, f);
+        nbig_of_q[q] = factorize_ring(n, f);
         if ((int)f.size() > MAX_RADIX_LIST) { free(pl); return SHT_ERR_UNSUPPORTED; }
         fac_off_of_q[q] = (int)radix.size();
         nfac_of_q[q] = (int)f.size();
         for (int v : f) radix.push_back(v);
-        (void)largest_factor;
+        // forward (decimation in frequency) output order: bin k = s_1 + R_1 (s_2 + R_2 (...)) sits at
+        // position s_1 n/R_1 + s_2 n/(R_1 R_2) + ...
+        perm_off_of_q[q] = (int)perm.size();
+        for (int k = 0; k < n; ++k) {
+            int kk = k, pos = 0, M = n;
+            for (int v : f) { const int sdig = kk % v; kk /= v; M /= v; pos += sdig * M; }
+            perm.push_back((unsigned short)pos);
+        }
     }
     const long long ns = nside;
     for (int p = 0; p < d.nh; ++p) {
@@ -206,17 +207,12 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
         r.start_s = (i == 2 * ns) ? -1 : d.npix - r.start_n - r.n;
         const int q = r.n / 4;
         r.tw_off = tw_off_of_q[q]; r.fac_off = fac_off_of_q[q]; r.nfac = nfac_of_q[q];
-        r.kt = ring_kt(r.n, smem_budget);
-        r.nb = 0; r.chirp_off = r.bfilt_off = r.btw_off = 0;
+        r.perm_off = perm_off_of_q[q];
+        r.oop = nbig_of_q[q] >= 2 ? 1 : 0;
+        r.kt = ring_kt(r.n, r.oop ? RING_EMAX_OOP : RING_EMAX);
+        r.mlim = lmax + 1;                               // tightened below from the l_safe table
         zs[p] = (double)absz; sin2s[p] = (double)s2;
     }
-    pl->fft_smem = 0;
-    pl->ring_kt_min = rings[d.nh - 1].kt;
-    for (int p = 0; p < d.nh; ++p) {
-        size_t b = ring_fft_smem_bytes(rings[p].n, rings[p].kt);
-        if (b > pl->fft_smem) pl->fft_smem = b;
-    }
-    if (pl->fft_smem > 220 * 1024) { free(pl); return SHT_ERR_UNSUPPORTED; }
 
     // ---- recurrence coefficients (alpha_lm, beta_lm), m-major ---------------------------------
     //   lambda_l = alpha_l z lambda_{l-1} - beta_l lambda_{l-2},
@@ -249,9 +245,9 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
     }
 
     const double* d_cm = nullptr;
-    if ((ce = upload(pl, rings, &d.rings)) != cudaSuccess || (ce = upload(pl, zs, &d.z)) != cudaSuccess ||
+    if ((ce = upload(pl, zs, &d.z)) != cudaSuccess ||
         (ce = upload(pl, sin2s, &d.sin2)) != cudaSuccess || (ce = upload(pl, tw, &d.tw)) != cudaSuccess ||
-        (ce = upload(pl, radix, &d.radix)) != cudaSuccess || (ce = upload(pl, coef, &d.coef)) != cudaSuccess ||
+        (ce = upload(pl, radix, &d.radix)) != cudaSuccess || (ce = upload(pl, perm, &d.perm)) != cudaSuccess || (ce = upload(pl, coef, &d.coef)) != cudaSuccess ||
         (ce = upload(pl, spin2c, &d.spin2c)) != cudaSuccess || (ce = upload(pl, cm, &d_cm)) != cudaSuccess) {
         sht_plan_destroy(pl);
         return SHT_ERR_ALLOC;
@@ -270,6 +266,49 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
         ce = launch_seed_table(d, d_cm, ls, sd, 0);
         if (ce == cudaSuccess) ce = cudaDeviceSynchronize();
         if (ce != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
+
+        // ring optimisation (item 10): ring p takes part in order m only if lambda_lm(theta_p) reaches
+        // the threshold for some l <= lmax, i.e. l_safe(m, p) <= lmax.  mlim[p] = 1 + the largest such m, made
+        // monotone towards the equator; the ring kernels and the Legendre kernels both use exactly this bound,
+        // so a workspace cell is read iff it was written.
+        std::vector<int> hls(cells);
+        if (cudaMemcpy(hls.data(), ls, cells * sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
+        std::vector<int> mlim(d.nh, 1);
+        int run = 1;
+        for (int p = 0; p < d.nh; ++p) {
+            int mm = 0;
+            for (int m = lmax; m > 0; --m)
+                if (hls[(size_t)m * d.nh + p] <= lmax) { mm = m; break; }
+            if (mm + 1 > run) run = mm + 1;
+            mlim[p] = run;
+            rings[p].mlim = run;
+        }
+        if ((ce = upload(pl, rings, &d.rings)) != cudaSuccess || (ce = upload(pl, mlim, &d.mlim)) != cudaSuccess) {
+            sht_plan_destroy(pl);
+            return SHT_ERR_ALLOC;
+        }
+    }
+
+    // ---- ring-kernel launch classes (by dynamic shared memory per CTA) --------------------------
+    {
+        const size_t lim[RING_NCLASS] = {72 * 1024, 110 * 1024, 128 * 1024, 224 * 1024};
+        std::vector<int> lists[RING_NCLASS];
+        for (int c = 0; c < RING_NCLASS; ++c) { pl->class_smem[c] = 0; pl->class_ktmin[c] = 16; }
+        for (int p = 0; p < d.nh; ++p) {
+            const size_t b = (size_t)rings[p].n * rings[p].kt * sizeof(double2) * (rings[p].oop ? 2 : 1);
+            int c = 0;
+            while (c < RING_NCLASS && b > lim[c]) ++c;
+            if (c == RING_NCLASS) { sht_plan_destroy(pl); return SHT_ERR_UNSUPPORTED; }
+            lists[c].push_back(p);
+            if (b > pl->class_smem[c]) pl->class_smem[c] = b;
+            if (rings[p].kt < pl->class_ktmin[c]) pl->class_ktmin[c] = rings[p].kt;
+        }
+        for (int c = 0; c < RING_NCLASS; ++c) {
+            pl->class_count[c] = (int)lists[c].size();
+            const int* dp = nullptr;
+            if (upload(pl, lists[c], &dp) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+            pl->class_rings[c] = const_cast<int*>(dp);
+        }
     }
 
     // ---- workspace: T_m^k(theta) for one chunk of maps ----------------------------------------
@@ -284,6 +323,7 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
         if (fit < KTILE_MAPS) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
         long long need = ((long long)nmaps + KTILE_MAPS - 1) / KTILE_MAPS * KTILE_MAPS;
         d.kpad = (int)(need < fit ? need : fit);
+        d.nkg = d.kpad / KG;
         pl->chunk = d.kpad < nmaps ? d.kpad : nmaps;
         pl->F_bytes = per_map * d.kpad;
         if (cudaMalloc(&pl->F, pl->F_bytes) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }

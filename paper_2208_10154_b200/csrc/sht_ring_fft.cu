@@ -7,16 +7,26 @@
 //   synthesis (PAPER.md:66-70 eq. 4, :78): ring spectrum Y[b] = sum_{m = b mod N} (w_m/2) d_m
 //       + sum_{m = -b mod N} (w_m/2) conj(d_m), d_m = e^{+i m phi0} T_m, followed by the backward DFT.
 //
-// One CTA owns one ring pair and `kt` maps.  The north and the south ring of a map are packed as the real
-// and imaginary part of ONE complex sequence (two real transforms for the price of one complex transform);
-// the complex FFT is an out-of-place Stockham autosort FFT in shared memory with a per-ring-length radix
-// list (4, 2, then the odd primes of N/4; a generic radix-R pass covers every prime).  No cuFFT.
+// One CTA owns one ring pair and `kt` maps (kt * N <= RING_EMAX complex elements, all resident in shared
+// memory, map index fastest so that every pass touches shared memory contiguously).  The north and the south
+// ring of a map are packed as the real and imaginary part of ONE complex sequence (two real transforms for
+// the price of one complex transform).  The complex FFT is an in-place mixed-radix transform: forward =
+// decimation in frequency (natural order in, digit-reversed out), backward = decimation in time (digit-
+// reversed in, natural out), so no pass needs a second buffer and the bin <-> position permutation is folded
+// into the FFT-mapping step through a plan-time table.  Radices 4, 2, 3, 5, 7 are register butterflies; a
+// prime factor >= 11 of the ring length is a direct O(R^2) stage placed at the global-memory end of the
+// transform (first forward stage / last backward stage, fused with the map load / store); a second such
+// prime runs out of place between two shared buffers.  No cuFFT.
 //
-// Workspace layout (both directions): F[p][m][comp][h][k][2] doubles, h = 0/1 = E/O (analysis) or
-// north/south (synthesis), k fastest so that the Legendre stage reads dense [ring x (re,im of 64 maps)] rows.
+// Workspace layout (both directions): F[p][kg][m][comp][h][kk][2] doubles (sht_internal.h), h = 0/1 = E/O
+// (analysis) or north/south (synthesis): a CTA writes / reads whole 128-byte lines for kt >= 4.
+// Only m < mlim(p) is produced / consumed (ring optimisation).
+// Spin 2: component 1 of the workspace holds i*U (PAPER.md:111, 215 item 1: "all-real" products).
 #include "sht_internal.h"
 
 namespace sht {
+
+constexpr int NT = RING_THREADS;
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b)
 {
@@ -34,256 +44,396 @@ __device__ __forceinline__ double2 twiddle(const double2* __restrict__ tw2, int 
     return w;
 }
 
-// One Stockham pass of radix R over `in` (length N) into `out`; p = product of the radices already done.
-template <bool INV>
-__device__ void pass_radix4(const double2* in, double2* out, int N, int p, const double2* tw2, int tid, int nt)
+// cos / sin of 2 pi k / R for the odd register radices
+__host__ __device__ constexpr double dft_cos(int R, int k)
 {
-    const int T = N >> 2, unit = N / (4 * p);
-    for (int i = tid; i < T; i += nt) {
-        const int k = i % p, e = k * unit;
-        double2 u0 = in[i];
-        double2 u1 = cmul(in[i + T], twiddle<INV>(tw2, e));
-        double2 u2 = cmul(in[i + 2 * T], twiddle<INV>(tw2, 2 * e));
-        double2 u3 = cmul(in[i + 3 * T], twiddle<INV>(tw2, 3 * e));
-        double2 v0 = cadd(u0, u2), v1 = csub(u0, u2), v2 = cadd(u1, u3), d = csub(u1, u3);
-        double2 v3 = INV ? make_double2(-d.y, d.x) : make_double2(d.y, -d.x);   // (+-i) (u1 - u3)
-        const int j = (i - k) * 4 + k;
-        out[j] = cadd(v0, v2);
-        out[j + p] = cadd(v1, v3);
-        out[j + 2 * p] = csub(v0, v2);
-        out[j + 3 * p] = csub(v1, v3);
+    return k == 0 ? 1.0
+         : R == 3 ? -0.5
+         : R == 5 ? ((k == 1 || k == 4) ? 0.3090169943749474241 : -0.8090169943749474241)
+         : (k == 1 || k == 6) ? 0.62348980185873353053
+         : (k == 2 || k == 5) ? -0.22252093395631440429
+                              : -0.90096886790241912624;
+}
+__host__ __device__ constexpr double dft_sin(int R, int k)
+{
+    return k == 0 ? 0.0
+         : R == 3 ? (k == 1 ? 0.86602540378443864676 : -0.86602540378443864676)
+         : R == 5 ? (k == 1 ? 0.95105651629515357212 : k == 2 ? 0.58778525229247312917
+                   : k == 3 ? -0.58778525229247312917 : -0.95105651629515357212)
+         : (k == 1 ? 0.78183148246802980871 : k == 2 ? 0.97492791218182360702 : k == 3 ? 0.43388373911755812048
+          : k == 4 ? -0.43388373911755812048 : k == 5 ? -0.97492791218182360702 : -0.78183148246802980871);
+}
+
+// R-point DFT in registers: u[s] <- sum_r u[r] exp(-+ 2 pi i r s / R)   (- forward, + if INV)
+template <int R, bool INV>
+__device__ __forceinline__ void bfly(double2 (&u)[R])
+{
+    if constexpr (R == 2) {
+        const double2 a = u[0], b = u[1];
+        u[0] = cadd(a, b); u[1] = csub(a, b);
+    } else if constexpr (R == 4) {
+        const double2 v0 = cadd(u[0], u[2]), v1 = csub(u[0], u[2]), v2 = cadd(u[1], u[3]), dd = csub(u[1], u[3]);
+        const double2 v3 = INV ? make_double2(-dd.y, dd.x) : make_double2(dd.y, -dd.x);   // (+-i)(u1 - u3)
+        u[0] = cadd(v0, v2); u[1] = cadd(v1, v3); u[2] = csub(v0, v2); u[3] = csub(v1, v3);
+    } else {
+        constexpr int H = (R - 1) / 2;
+        double2 a[H], b[H];
+#pragma unroll
+        for (int j = 1; j <= H; ++j) { a[j - 1] = cadd(u[j], u[R - j]); b[j - 1] = csub(u[j], u[R - j]); }
+        const double2 u0 = u[0];
+        double2 sum = u0;
+#pragma unroll
+        for (int j = 0; j < H; ++j) sum = cadd(sum, a[j]);
+        u[0] = sum;
+#pragma unroll
+        for (int s = 1; s <= H; ++s) {
+            double2 re = u0, im = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int j = 1; j <= H; ++j) {
+                const double c = dft_cos(R, (j * s) % R), sn = dft_sin(R, (j * s) % R);
+                re.x = fma(c, a[j - 1].x, re.x); re.y = fma(c, a[j - 1].y, re.y);
+                im.x = fma(sn, b[j - 1].x, im.x); im.y = fma(sn, b[j - 1].y, im.y);
+            }
+            // forward: X_s = re - i im, X_{R-s} = re + i im; backward: the other way round
+            const double2 lo = make_double2(re.x + im.y, re.y - im.x), hi = make_double2(re.x - im.y, re.y + im.x);
+            u[s] = INV ? hi : lo;
+            u[R - s] = INV ? lo : hi;
+        }
     }
 }
 
-template <bool INV>
-__device__ void pass_radix2(const double2* in, double2* out, int N, int p, const double2* tw2, int tid, int nt)
+// ---- forward stages (decimation in frequency, in place) ------------------------------------------------
+// Stage with sub-length L and radix R, M = L / R: for each block base (multiple of L) and j < M the elements
+// base + j + r M are replaced by W_L^{j s} sum_r x_r W_R^{r s}.  GIN: first stage (L = N), reads the maps.
+template <int R, bool GIN, class LD>
+__device__ __forceinline__ void dif_stage(double2* buf, int N, int L, int kt, int ktsh, const double2* __restrict__ tw2, LD ld)
 {
-    const int T = N >> 1, unit = N / (2 * p);
-    for (int i = tid; i < T; i += nt) {
-        const int k = i % p;
-        double2 u0 = in[i];
-        double2 u1 = cmul(in[i + T], twiddle<INV>(tw2, k * unit));
-        const int j = (i - k) * 2 + k;
-        out[j] = cadd(u0, u1);
-        out[j + p] = csub(u0, u1);
+    const int M = L / R, nw = (N / R) << ktsh, tstep = N / L;
+    for (int w = threadIdx.x; w < nw; w += NT) {
+        const int kk = w & (kt - 1), bf = w >> ktsh;
+        const int blk = bf / M, j = bf - blk * M;
+        const int e0 = blk * L + j;
+        double2 u[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) u[r] = GIN ? ld(e0 + r * M, kk) : buf[((e0 + r * M) << ktsh) + kk];
+        bfly<R, false>(u);
+        if (M > 1) {
+#pragma unroll
+            for (int s = 1; s < R; ++s) u[s] = cmul(u[s], twiddle<false>(tw2, j * s * tstep));
+        }
+#pragma unroll
+        for (int s = 0; s < R; ++s) buf[((e0 + s * M) << ktsh) + kk] = u[s];
     }
+    __syncthreads();
 }
 
-// generic radix: one thread per output element, R complex multiply-adds each
-template <bool INV>
-__device__ void pass_generic(const double2* in, double2* out, int N, int R, int p, const double2* tw2, int tid, int nt)
+// direct O(R^2) stage for a prime R >= 11: one thread per output element; src -> dst (different buffers, or
+// src = the maps when GIN)
+template <bool GIN, class LD>
+__device__ __forceinline__ void dif_generic(const double2* src, double2* dst, int N, int L, int R, int kt, int ktsh,
+                                            const double2* __restrict__ tw2, LD ld)
 {
-    const int T = N / R, pr = p * R, unit = N / pr, sstep = N / R;
-    for (int o = tid; o < N; o += nt) {
-        const int blk = o / pr, rem = o - blk * pr;
-        const int s = rem / p, k = rem - s * p;
-        const int i = blk * p + k;
-        int es = (int)(((long long)k * unit + (long long)s * sstep) % N);
+    const int M = L / R, nout = N << ktsh, tstep = N / L, rstep = N / R;
+    for (int o = threadIdx.x; o < nout; o += NT) {
+        const int kk = o & (kt - 1), pos = o >> ktsh;
+        const int blk = pos / L, rem = pos - blk * L;
+        const int s = rem / M, j = rem - s * M;
+        const int e0 = blk * L + j;
+        const int es = s * rstep;                          // exponent step of W_N per r: r s N / R
         int e = 0;
         double2 acc = make_double2(0.0, 0.0);
         for (int r = 0; r < R; ++r) {
-            double2 w = twiddle<INV>(tw2, e);
-            double2 v = in[i + r * T];
-            acc.x = fma(v.x, w.x, fma(-v.y, w.y, acc.x));
-            acc.y = fma(v.x, w.y, fma(v.y, w.x, acc.y));
+            const double2 x = GIN ? ld(e0 + r * M, kk) : src[((e0 + r * M) << ktsh) + kk];
+            const double2 w = twiddle<false>(tw2, e);
+            acc.x = fma(x.x, w.x, fma(-x.y, w.y, acc.x));
+            acc.y = fma(x.x, w.y, fma(x.y, w.x, acc.y));
             e += es; if (e >= N) e -= N;
         }
-        out[o] = acc;
-    }
-}
-
-// complex FFT of buf (length N) by all threads of the CTA; result is left in buf.
-template <bool INV>
-__device__ void fft_cta(double2* buf, double2* scratch, int N, const int* __restrict__ radix, int nfac,
-                        const double2* __restrict__ tw2)
-{
-    const int tid = threadIdx.x, nt = blockDim.x;
-    double2* src = buf; double2* dst = scratch;
-    int p = 1;
-    for (int f = 0; f < nfac; ++f) {
-        const int R = radix[f];
-        if (R == 4) pass_radix4<INV>(src, dst, N, p, tw2, tid, nt);
-        else if (R == 2) pass_radix2<INV>(src, dst, N, p, tw2, tid, nt);
-        else pass_generic<INV>(src, dst, N, R, p, tw2, tid, nt);
-        p *= R;
-        __syncthreads();
-        double2* t = src; src = dst; dst = t;
-    }
-    if (src != buf) {
-        for (int i = tid; i < N; i += nt) buf[i] = src[i];
-        __syncthreads();
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// analysis: maps -> F (E/O folded, phase shifted, aliased to every m)
-// grid (kblocks, nh, ncomp)
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_ring_analysis(DevicePlan d, const double* __restrict__ maps,
-                                                      double* __restrict__ F, int k0, int kmaps)
-{
-    extern __shared__ double2 smem[];
-    const int p = blockIdx.y, comp = blockIdx.z;
-    const RingPair rp = d.rings[p];
-    const int N = rp.n, kt = rp.kt;
-    const int kbase = blockIdx.x * kt;
-    if (kbase >= kmaps) return;
-    const int tid = threadIdx.x, nt = blockDim.x;
-    double2* scratch = smem + (size_t)kt * N;
-    const double2* tw2 = d.tw + rp.tw_off;
-    const int* radix = d.radix + rp.fac_off;
-
-    // load: z[n] = T_north[n] + i T_south[n]
-    for (int kk = 0; kk < kt; ++kk) {
-        double2* buf = smem + (size_t)kk * N;
-        const int k = kbase + kk;
-        if (k < kmaps) {
-            const double* mp = maps + ((size_t)(k0 + k) * d.ncomp + comp) * d.npix;
-            const double* north = mp + rp.start_n;
-            const double* south = rp.start_s >= 0 ? mp + rp.start_s : nullptr;
-            for (int n = tid; n < N; n += nt)
-                buf[n] = make_double2(__ldg(north + n), south ? __ldg(south + n) : 0.0);
-        } else {
-            for (int n = tid; n < N; n += nt) buf[n] = make_double2(0.0, 0.0);
-        }
+        if (M > 1) acc = cmul(acc, twiddle<false>(tw2, j * s * tstep));
+        dst[(pos << ktsh) + kk] = acc;
     }
     __syncthreads();
-    for (int kk = 0; kk < kt; ++kk) fft_cta<false>(smem + (size_t)kk * N, scratch, N, radix, rp.nfac, tw2);
+}
 
-    // FFT mapping: m -> bin on the frequency circle, phase, fold; k fastest in the output
-    const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
-    const int total = (d.lmax + 1) * kt;
+// ---- backward stages (decimation in time, in place): the exact adjoints of the forward stages ----------
+template <int R, bool GOUT, class ST>
+__device__ __forceinline__ void dit_stage(double2* buf, int N, int L, int kt, int ktsh, const double2* __restrict__ tw2, ST st)
+{
+    const int M = L / R, nw = (N / R) << ktsh, tstep = N / L;
+    for (int w = threadIdx.x; w < nw; w += NT) {
+        const int kk = w & (kt - 1), bf = w >> ktsh;
+        const int blk = bf / M, j = bf - blk * M;
+        const int e0 = blk * L + j;
+        double2 u[R];
+#pragma unroll
+        for (int s = 0; s < R; ++s) u[s] = buf[((e0 + s * M) << ktsh) + kk];
+        if (M > 1) {
+#pragma unroll
+            for (int s = 1; s < R; ++s) u[s] = cmul(u[s], twiddle<true>(tw2, j * s * tstep));
+        }
+        bfly<R, true>(u);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (GOUT) st(e0 + r * M, kk, u[r]);
+            else buf[((e0 + r * M) << ktsh) + kk] = u[r];
+        }
+    }
+    if (!GOUT) __syncthreads();
+}
+
+template <bool GOUT, class ST>
+__device__ __forceinline__ void dit_generic(const double2* src, double2* dst, int N, int L, int R, int kt, int ktsh,
+                                            const double2* __restrict__ tw2, ST st)
+{
+    const int M = L / R, nout = N << ktsh, tstep = N / L, rstep = N / R;
+    for (int o = threadIdx.x; o < nout; o += NT) {
+        const int kk = o & (kt - 1), pos = o >> ktsh;
+        const int blk = pos / L, rem = pos - blk * L;
+        const int r = rem / M, j = rem - r * M;
+        const int e0 = blk * L + j;
+        int es = j * tstep + r * rstep;                    // exponent step per s: s (j N / L + r N / R)
+        if (es >= N) es -= N;
+        int e = 0;
+        double2 acc = make_double2(0.0, 0.0);
+        for (int s = 0; s < R; ++s) {
+            const double2 x = src[((e0 + s * M) << ktsh) + kk];
+            const double2 w = twiddle<true>(tw2, e);
+            acc.x = fma(x.x, w.x, fma(-x.y, w.y, acc.x));
+            acc.y = fma(x.x, w.y, fma(x.y, w.x, acc.y));
+            e += es; if (e >= N) e -= N;
+        }
+        if (GOUT) st(pos, kk, acc);
+        else dst[(pos << ktsh) + kk] = acc;
+    }
+    if (!GOUT) __syncthreads();
+}
+
+// ------------------------------------------------------------------------------------------------
+// analysis: maps -> F (E/O folded, phase shifted, aliased to every m < mlim)
+// grid (map blocks, rings of the launch class, ncomp)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* __restrict__ ring_list,
+                                                     const double* __restrict__ maps, double* __restrict__ F,
+                                                     int k0, int kmaps)
+{
+    extern __shared__ double2 smem[];
+    const int p = ring_list[blockIdx.y], comp = blockIdx.z;
+    const RingPair rp = d.rings[p];
+    const int N = rp.n, kt = rp.kt, ktsh = __ffs(kt) - 1;
+    const int kbase = blockIdx.x * kt;
+    if (kbase >= kmaps) return;
+    const int tid = threadIdx.x;
+    const double2* tw2 = d.tw + rp.tw_off;
+    const int* radix = d.radix + rp.fac_off;
+    const unsigned short* perm = d.perm + rp.perm_off;
     const bool equator = rp.start_s < 0;
-    for (int idx = tid; idx < total; idx += nt) {
-        const int kk = idx % kt, m = idx / kt;
-        if (kbase + kk >= kmaps) continue;
-        const double2* Z = smem + (size_t)kk * N;
+
+    // z[n] = T_north[n] + i T_south[n] of map kbase + kk
+    const size_t map_stride = (size_t)d.ncomp * d.npix;
+    const double* mbase = maps + ((size_t)(k0 + kbase) * d.ncomp + comp) * d.npix;
+    const long long sn = rp.start_n, ss = rp.start_s;
+    auto ld = [&](int e, int kk) -> double2 {
+        if (kbase + kk >= kmaps) return make_double2(0.0, 0.0);
+        const double* mp = mbase + (size_t)kk * map_stride;
+        return make_double2(__ldg(mp + sn + e), equator ? 0.0 : __ldg(mp + ss + e));
+    };
+
+    double2* cur = smem;
+    int L = N;
+    for (int f = 0; f < rp.nfac; ++f) {
+        const int R = radix[f];
+        if (f == 0) {
+            switch (R) {
+                case 2: dif_stage<2, true>(cur, N, L, kt, ktsh, tw2, ld); break;
+                case 3: dif_stage<3, true>(cur, N, L, kt, ktsh, tw2, ld); break;
+                case 4: dif_stage<4, true>(cur, N, L, kt, ktsh, tw2, ld); break;
+                case 5: dif_stage<5, true>(cur, N, L, kt, ktsh, tw2, ld); break;
+                case 7: dif_stage<7, true>(cur, N, L, kt, ktsh, tw2, ld); break;
+                default: dif_generic<true>(nullptr, cur, N, L, R, kt, ktsh, tw2, ld); break;
+            }
+        } else {
+            switch (R) {
+                case 2: dif_stage<2, false>(cur, N, L, kt, ktsh, tw2, ld); break;
+                case 3: dif_stage<3, false>(cur, N, L, kt, ktsh, tw2, ld); break;
+                case 4: dif_stage<4, false>(cur, N, L, kt, ktsh, tw2, ld); break;
+                case 5: dif_stage<5, false>(cur, N, L, kt, ktsh, tw2, ld); break;
+                case 7: dif_stage<7, false>(cur, N, L, kt, ktsh, tw2, ld); break;
+                default: {
+                    double2* other = (cur == smem) ? smem + ((size_t)N << ktsh) : smem;
+                    dif_generic<false>(cur, other, N, L, R, kt, ktsh, tw2, ld);
+                    cur = other;
+                } break;
+            }
+        }
+        L /= R;
+    }
+
+    // FFT mapping: m -> bin on the frequency circle (stored at position perm[bin]), phase, fold
+    const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
+    const int total = rp.mlim << ktsh;
+    double2* Fc = reinterpret_cast<double2*>(F);
+    for (int idx = tid; idx < total; idx += NT) {
+        const int kk = idx & (kt - 1), m = idx >> ktsh;
+        const int k = kbase + kk;
+        if (k >= kmaps) continue;
         const int b = m % N, bc = b == 0 ? 0 : N - b;
-        const double2 A = Z[b], B = Z[bc];
+        const double2 A = cur[((int)perm[b] << ktsh) + kk], B = cur[((int)perm[bc] << ktsh) + kk];
         // G_north = (A + conj B)/2, G_south = (A - conj B)/(2i)
         const double2 gn = make_double2(0.5 * (A.x + B.x), 0.5 * (A.y - B.y));
         const double2 gs = make_double2(0.5 * (A.y + B.y), -0.5 * (A.x - B.x));
-        double2 ph = __ldg(tw2 + (int)(((long long)m * rp.shift) % (2 * N)));     // e^{-i m phi0}
-        ph.x *= dsig; ph.y *= dsig;
+        double2 ph = make_double2(dsig, 0.0);
+        if (rp.shift) {                                   // e^{-i m phi0}, phi0 = pi / N
+            ph = __ldg(tw2 + (m % (2 * N)));
+            ph.x *= dsig; ph.y *= dsig;
+        }
         double2 E, O;
         if (equator) { E = cmul(ph, gn); O = make_double2(0.0, 0.0); }
         else { E = cmul(ph, cadd(gn, gs)); O = cmul(ph, csub(gn, gs)); }
-        const size_t row = (((size_t)p * (d.lmax + 1) + m) * d.ncomp + comp) * 2;
-        double2* Fe = reinterpret_cast<double2*>(F) + row * d.kpad + kbase + kk;
-        Fe[0] = E;
-        Fe[d.kpad] = O;
+        if (comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }      // i U
+        const size_t cell = f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
+        Fc[cell] = E;
+        Fc[cell + KG] = O;
     }
 }
 
 // ------------------------------------------------------------------------------------------------
 // synthesis: F (north/south T_m) -> maps.  If sub_from != nullptr: maps = sub_from - synthesis.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_ring_synthesis(DevicePlan d, const double* __restrict__ F,
-                                                       double* __restrict__ maps, int k0, int kmaps,
-                                                       const double* __restrict__ sub_from, int ksub0)
+__global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* __restrict__ ring_list,
+                                                      const double* __restrict__ F, double* __restrict__ maps,
+                                                      int k0, int kmaps, const double* __restrict__ sub_from, int ksub0)
 {
     extern __shared__ double2 smem[];
-    const int p = blockIdx.y, comp = blockIdx.z;
+    const int p = ring_list[blockIdx.y], comp = blockIdx.z;
     const RingPair rp = d.rings[p];
-    const int N = rp.n, kt = rp.kt;
+    const int N = rp.n, kt = rp.kt, ktsh = __ffs(kt) - 1;
     const int kbase = blockIdx.x * kt;
     if (kbase >= kmaps) return;
-    const int tid = threadIdx.x, nt = blockDim.x;
-    double2* scratch = smem + (size_t)kt * N;
+    const int tid = threadIdx.x;
     const double2* tw2 = d.tw + rp.tw_off;
     const int* radix = d.radix + rp.fac_off;
+    const unsigned short* perm = d.perm + rp.perm_off;
     const bool equator = rp.start_s < 0;
+    const int mlim = rp.mlim;
+    double2* cur = smem;
 
-    // ring spectrum of the packed sequence: Zin[b] = Y_north[b] + i Y_south[b]
-    const int total = N * kt;
-    for (int idx = tid; idx < total; idx += nt) {
-        const int kk = idx % kt, b = idx / kt;
+    // ring spectrum of the packed sequence, Z[b] = Y_north[b] + i Y_south[b]; bins b <= N/2 are assembled
+    // from the workspace (each cell read once), bins N - b follow from the Hermitian symmetry of Y_n, Y_s
+    const double2* Fc = reinterpret_cast<const double2*>(F);
+    const int total = (N / 2 + 1) << ktsh;
+    for (int idx = tid; idx < total; idx += NT) {
+        const int kk = idx & (kt - 1), b = idx >> ktsh;
+        const int k = kbase + kk;
         double2 yn = make_double2(0.0, 0.0), ys = make_double2(0.0, 0.0);
-        if (kbase + kk < kmaps) {
-            // m = b (mod N): + (w/2) d_m ;  m = -b (mod N): + (w/2) conj(d_m)
+        if (k < kmaps) {
+            // m = b (mod N): + (w/2) d_m ;  m = -b (mod N): + (w/2) conj(d_m);  d_m = e^{+i m phi0} T_m
             for (int pass = 0; pass < 2; ++pass) {
                 const int mfirst = pass == 0 ? b : (b == 0 ? 0 : N - b);
-                for (int m = mfirst; m <= d.lmax; m += N) {
+                for (int m = mfirst; m < mlim; m += N) {
                     const double w = (m == 0) ? 0.5 : 1.0;
-                    double2 ph = __ldg(tw2 + (int)(((long long)m * rp.shift) % (2 * N)));
-                    ph.y = -ph.y;                                                   // e^{+i m phi0}
-                    const size_t row = (((size_t)p * (d.lmax + 1) + m) * d.ncomp + comp) * 2;
-                    const double2* Fr = reinterpret_cast<const double2*>(F) + row * d.kpad + kbase + kk;
-                    double2 dn = cmul(ph, Fr[0]);
-                    double2 ds = cmul(ph, Fr[d.kpad]);
+                    double2 ph = make_double2(1.0, 0.0);
+                    if (rp.shift) { ph = __ldg(tw2 + (m % (2 * N))); ph.y = -ph.y; }
+                    const size_t cell = f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
+                    double2 fn = Fc[cell], fs = Fc[cell + KG];
+                    if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }   // U = -i (iU)
+                    double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
                     if (pass == 1) { dn.y = -dn.y; ds.y = -ds.y; }
                     yn.x = fma(w, dn.x, yn.x); yn.y = fma(w, dn.y, yn.y);
                     ys.x = fma(w, ds.x, ys.x); ys.y = fma(w, ds.y, ys.y);
                 }
             }
         }
-        // Y_n + i Y_s
-        smem[(size_t)kk * N + b] = equator ? yn : make_double2(yn.x - ys.y, yn.y + ys.x);
+        if (equator) ys = make_double2(0.0, 0.0);
+        if (b == 0 || 2 * b == N) { yn.y = 0.0; ys.y = 0.0; }
+        cur[((int)perm[b] << ktsh) + kk] = make_double2(yn.x - ys.y, yn.y + ys.x);
+        if (b > 0 && 2 * b < N)
+            cur[((int)perm[N - b] << ktsh) + kk] = make_double2(yn.x + ys.y, ys.x - yn.y);
     }
     __syncthreads();
-    for (int kk = 0; kk < kt; ++kk) fft_cta<true>(smem + (size_t)kk * N, scratch, N, radix, rp.nfac, tw2);
 
-    for (int kk = 0; kk < kt; ++kk) {
-        const int k = kbase + kk;
-        if (k >= kmaps) break;
-        const double2* buf = smem + (size_t)kk * N;
-        const size_t off = ((size_t)(k0 + k) * d.ncomp + comp) * d.npix;
-        double* north = maps + off + rp.start_n;
-        double* south = equator ? nullptr : maps + off + rp.start_s;
-        if (sub_from) {
-            const size_t soff = ((size_t)(ksub0 + k) * d.ncomp + comp) * d.npix;
-            const double* rn = sub_from + soff + rp.start_n;
-            const double* rs = equator ? nullptr : sub_from + soff + rp.start_s;
-            for (int n = tid; n < N; n += nt) {
-                const double2 v = buf[n];
-                north[n] = rn[n] - v.x;
-                if (south) south[n] = rs[n] - v.y;
+    const size_t map_stride = (size_t)d.ncomp * d.npix;
+    double* obase = maps + ((size_t)(k0 + kbase) * d.ncomp + comp) * d.npix;
+    const double* sbase = sub_from ? sub_from + ((size_t)(ksub0 + kbase) * d.ncomp + comp) * d.npix : nullptr;
+    const long long sn = rp.start_n, ss = rp.start_s;
+    auto st = [&](int e, int kk, double2 v) {
+        if (kbase + kk >= kmaps) return;
+        double* mp = obase + (size_t)kk * map_stride;
+        if (sbase) {
+            const double* sp = sbase + (size_t)kk * map_stride;
+            mp[sn + e] = sp[sn + e] - v.x;
+            if (!equator) mp[ss + e] = sp[ss + e] - v.y;
+        } else {
+            mp[sn + e] = v.x;
+            if (!equator) mp[ss + e] = v.y;
+        }
+    };
+
+    int L = 1;
+    for (int f = rp.nfac - 1; f >= 0; --f) {
+        const int R = radix[f];
+        L *= R;
+        if (f == 0) {
+            switch (R) {
+                case 2: dit_stage<2, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 3: dit_stage<3, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 4: dit_stage<4, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 5: dit_stage<5, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 7: dit_stage<7, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                default: dit_generic<true>(cur, nullptr, N, L, R, kt, ktsh, tw2, st); break;
             }
         } else {
-            for (int n = tid; n < N; n += nt) {
-                const double2 v = buf[n];
-                north[n] = v.x;
-                if (south) south[n] = v.y;
+            switch (R) {
+                case 2: dit_stage<2, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 3: dit_stage<3, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 4: dit_stage<4, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 5: dit_stage<5, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 7: dit_stage<7, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                default: {
+                    double2* other = (cur == smem) ? smem + ((size_t)N << ktsh) : smem;
+                    dit_generic<false>(cur, other, N, L, R, kt, ktsh, tw2, st);
+                    cur = other;
+                } break;
             }
         }
     }
 }
 
-static int ring_kt_min(const sht_plan_s* pl)
+static cudaError_t ring_attr(sht_plan_s* pl)
 {
-    // the longest ring has the fewest maps per CTA; it decides the grid width (CTAs beyond a ring's own
-    // count exit at once)
-    return pl->ring_kt_min;
+    static bool attr_set = false;
+    if (attr_set) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(k_ring_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_ring_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
+    if (e == cudaSuccess) attr_set = true;
+    (void)pl;
+    return e;
 }
 
 cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_ring_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
+    cudaError_t e = ring_attr(pl);
+    if (e != cudaSuccess) return e;
+    // longest rings first: their CTAs are the slowest
+    for (int c = RING_NCLASS - 1; c >= 0; --c) {
+        if (pl->class_count[c] == 0) continue;
+        dim3 grid((kmaps + pl->class_ktmin[c] - 1) / pl->class_ktmin[c], pl->class_count[c], d.ncomp);
+        k_ring_analysis<<<grid, NT, pl->class_smem[c], st>>>(d, pl->class_rings[c], maps, F, k0, kmaps);
+        pl->launches++;
     }
-    const int ktmin = ring_kt_min(pl);
-    dim3 grid((kmaps + ktmin - 1) / ktmin, d.nh, d.ncomp);
-    k_ring_analysis<<<grid, 256, pl->fft_smem, st>>>(d, maps, F, k0, kmaps);
-    pl->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps,
                                   const double* sub_from, int ksub0, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_ring_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
+    cudaError_t e = ring_attr(pl);
+    if (e != cudaSuccess) return e;
+    for (int c = RING_NCLASS - 1; c >= 0; --c) {
+        if (pl->class_count[c] == 0) continue;
+        dim3 grid((kmaps + pl->class_ktmin[c] - 1) / pl->class_ktmin[c], pl->class_count[c], d.ncomp);
+        k_ring_synthesis<<<grid, NT, pl->class_smem[c], st>>>(d, pl->class_rings[c], F, maps, k0, kmaps, sub_from, ksub0);
+        pl->launches++;
     }
-    const int ktmin = ring_kt_min(pl);
-    dim3 grid((kmaps + ktmin - 1) / ktmin, d.nh, d.ncomp);
-    k_ring_synthesis<<<grid, 256, pl->fft_smem, st>>>(d, F, maps, k0, kmaps, sub_from, ksub0);
-    pl->launches++;
     return cudaGetLastError();
 }
 
