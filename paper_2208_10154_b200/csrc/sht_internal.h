@@ -16,6 +16,7 @@ constexpr int MAX_RADIX_LIST = 16;           // factors of one ring length
 constexpr int RING_THREADS = 512;            // threads per CTA of the ring kernels
 constexpr int RING_EMAX = 8192;              // complex elements (ring length x maps) one ring CTA holds in smem
 constexpr int RING_EMAX_OOP = 6400;          // same for rings that need an out-of-place pass (two buffers)
+constexpr int BLUESTEIN_MIN_PRIME = 37;      // smallest prime factor of a ring length that switches to Bluestein
 constexpr int RING_NCLASS = 4;               // launch classes of the ring kernels (by dynamic smem size)
 
 // One folded ring pair p = 0 .. nh-1: north ring i = p+1 and its mirror 4 nside - i (PAPER.md:211 grid;
@@ -32,6 +33,12 @@ struct RingPair {
     int oop;               // 1: the radix list has a second generic (prime >= 11) pass, done out of place
     int mlim;              // only m < mlim are needed from / for this ring (ring optimisation)
     int perm_off;          // offset of this ring length's table perm[bin] = position after the forward transform
+    // Bluestein (chirp-z) rings: ring lengths with a prime factor > BLUESTEIN_MIN_PRIME are transformed as a
+    // circular convolution of power-of-two length lc >= 2 n - 1 (lc = 0: plain mixed radix)
+    int lc;
+    int b_tw_off;          // offset (double2) of W_{2 lc}[j] = exp(-i pi j / lc)
+    int b_fac_off, b_nfac; // radix list of the length-lc transform (4s and a 2)
+    int hf_off;            // offset (double2) of FFT_lc(conj chirp) / lc in forward-output position order
 };
 
 struct DevicePlan {

@@ -5,6 +5,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <utility>
 #include <vector>
 #include "sht_internal.h"
 
@@ -122,6 +124,31 @@ static sht_status_t fail(sht_plan_s* pl, sht_status_t s, const char* what, cudaE
     return s;
 }
 
+// plan-time power-of-two FFT in long double (iterative radix 2), for the Bluestein filter spectra
+static void host_fft_pow2(std::vector<long double>& re, std::vector<long double>& im)
+{
+    const size_t n = re.size();
+    for (size_t i = 1, j = 0; i < n; ++i) {
+        size_t bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) { std::swap(re[i], re[j]); std::swap(im[i], im[j]); }
+    }
+    for (size_t len = 2; len <= n; len <<= 1) {
+        const size_t half = len >> 1;
+        for (size_t k = 0; k < half; ++k) {
+            const long double ang = -2.0L * PI_LD * (long double)k / (long double)len;
+            const long double wr = cosl(ang), wi = sinl(ang);
+            for (size_t i = k; i < n; i += len) {
+                const size_t j = i + half;
+                const long double tr = re[j] * wr - im[j] * wi, ti = re[j] * wi + im[j] * wr;
+                re[j] = re[i] - tr; im[j] = im[i] - ti;
+                re[i] += tr; im[i] += ti;
+            }
+        }
+    }
+}
+
 // maps per CTA of the ring kernels: the largest power of two <= 16 whose rings fit the CTA's element budget
 static int ring_kt(int n, int cap)
 {
@@ -162,7 +189,8 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
     std::vector<double2> tw;
     std::vector<int> radix;
     std::vector<unsigned short> perm;
-    std::vector<int> perm_off_of_q(nside + 1, 0);
+    std::vector<int> perm_off_of_q(nside + 1, 0), lc_of_q(nside + 1, 0), hf_off_of_q(nside + 1, 0);
+    std::map<int, int> pow2_tw_off, pow2_fac_off, pow2_nfac;
     std::vector<int> tw_off_of_q(nside + 1, -1), fac_off_of_q(nside + 1, -1), nfac_of_q(nside + 1, 0), nbig_of_q(nside + 1, 0);
     for (int q = 1; q <= nside; ++q) {
         const int n = 4 * q;
@@ -177,6 +205,47 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
         fac_off_of_q[q] = (int)radix.size();
         nfac_of_q[q] = (int)f.size();
         for (int v : f) radix.push_back(v);
+        int maxp = 1;
+        for (int v : f) maxp = v > maxp ? v : maxp;
+        int lc = 0;
+        if (maxp >= BLUESTEIN_MIN_PRIME) {
+            lc = 4;
+            while (lc < 2 * n - 1) lc *= 2;
+            if (lc > RING_EMAX) lc = 0;                  // does not fit one CTA: stay with the direct stage
+        }
+        lc_of_q[q] = lc;
+        if (lc) {
+            if (!pow2_tw_off.count(lc)) {
+                pow2_tw_off[lc] = (int)tw.size();
+                for (int j = 0; j < 2 * lc; ++j) {
+                    long double ang = PI_LD * (long double)j / (long double)lc;
+                    tw.push_back(make_double2((double)cosl(ang), (double)-sinl(ang)));
+                }
+                pow2_fac_off[lc] = (int)radix.size();
+                int r = lc, cnt = 0;
+                while (r % 4 == 0) { radix.push_back(4); r /= 4; ++cnt; }
+                if (r == 2) { radix.push_back(2); ++cnt; }
+                pow2_nfac[lc] = cnt;
+            }
+            // filter h_j = conj(c_j) = exp(+i pi j^2 / n) at j = -(n-1) .. n-1 (mod lc); Hf = FFT_lc(h) / lc
+            std::vector<long double> hr(lc, 0.0L), hi(lc, 0.0L);
+            for (int j = 0; j < n; ++j) {
+                const long long e = ((long long)j * j) % (2LL * n);
+                const long double ang = PI_LD * (long double)e / (long double)n;
+                hr[j] = cosl(ang); hi[j] = sinl(ang);
+                if (j > 0) { hr[lc - j] = hr[j]; hi[lc - j] = hi[j]; }
+            }
+            host_fft_pow2(hr, hi);
+            hf_off_of_q[q] = (int)tw.size();
+            const int fo = pow2_fac_off[lc], nf = pow2_nfac[lc];
+            std::vector<double2> hf(lc);
+            for (int k = 0; k < lc; ++k) {
+                int kk = k, pos = 0, M = lc;
+                for (int i2 = 0; i2 < nf; ++i2) { const int v = radix[fo + i2]; const int sdig = kk % v; kk /= v; M /= v; pos += sdig * M; }
+                hf[pos] = make_double2((double)(hr[k] / lc), (double)(hi[k] / lc));
+            }
+            tw.insert(tw.end(), hf.begin(), hf.end());
+        }
         // forward (decimation in frequency) output order: bin k = s_1 + R_1 (s_2 + R_2 (...)) sits at
         // position s_1 n/R_1 + s_2 n/(R_1 R_2) + ...
         perm_off_of_q[q] = (int)perm.size();
@@ -208,8 +277,17 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
         const int q = r.n / 4;
         r.tw_off = tw_off_of_q[q]; r.fac_off = fac_off_of_q[q]; r.nfac = nfac_of_q[q];
         r.perm_off = perm_off_of_q[q];
-        r.oop = nbig_of_q[q] >= 2 ? 1 : 0;
-        r.kt = ring_kt(r.n, r.oop ? RING_EMAX_OOP : RING_EMAX);
+        r.lc = lc_of_q[q];
+        r.b_tw_off = r.b_fac_off = r.b_nfac = r.hf_off = 0;
+        if (r.lc) {
+            r.b_tw_off = pow2_tw_off[r.lc]; r.b_fac_off = pow2_fac_off[r.lc]; r.b_nfac = pow2_nfac[r.lc];
+            r.hf_off = hf_off_of_q[q];
+            r.oop = 0;
+            r.kt = ring_kt(r.lc, RING_EMAX);
+        } else {
+            r.oop = nbig_of_q[q] >= 2 ? 1 : 0;
+            r.kt = ring_kt(r.n, r.oop ? RING_EMAX_OOP : RING_EMAX);
+        }
         r.mlim = lmax + 1;                               // tightened below from the l_safe table
         zs[p] = (double)absz; sin2s[p] = (double)s2;
     }
@@ -295,7 +373,7 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
         std::vector<int> lists[RING_NCLASS];
         for (int c = 0; c < RING_NCLASS; ++c) { pl->class_smem[c] = 0; pl->class_ktmin[c] = 16; }
         for (int p = 0; p < d.nh; ++p) {
-            const size_t b = (size_t)rings[p].n * rings[p].kt * sizeof(double2) * (rings[p].oop ? 2 : 1);
+            const size_t b = (size_t)(rings[p].lc ? rings[p].lc : rings[p].n) * rings[p].kt * sizeof(double2) * (rings[p].oop ? 2 : 1);
             int c = 0;
             while (c < RING_NCLASS && b > lim[c]) ++c;
             if (c == RING_NCLASS) { sht_plan_destroy(pl); return SHT_ERR_UNSUPPORTED; }

@@ -208,39 +208,16 @@ __device__ __forceinline__ void dit_generic(const double2* src, double2* dst, in
     if (!GOUT) __syncthreads();
 }
 
-// ------------------------------------------------------------------------------------------------
-// analysis: maps -> F (E/O folded, phase shifted, aliased to every m < mlim)
-// grid (map blocks, rings of the launch class, ncomp)
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* __restrict__ ring_list,
-                                                     const double* __restrict__ maps, double* __restrict__ F,
-                                                     int k0, int kmaps)
+// ---- transform drivers -----------------------------------------------------------------------------------
+// forward transform of length N over the radix list (first stage reads through `ld`); returns the buffer that
+// holds the result (bin k at position perm[k])
+template <class LD>
+__device__ __forceinline__ double2* fft_forward(double2* smem, int N, const int* __restrict__ radix, int nfac, int kt, int ktsh,
+                                                const double2* __restrict__ tw2, LD ld)
 {
-    extern __shared__ double2 smem[];
-    const int p = ring_list[blockIdx.y], comp = blockIdx.z;
-    const RingPair rp = d.rings[p];
-    const int N = rp.n, kt = rp.kt, ktsh = __ffs(kt) - 1;
-    const int kbase = blockIdx.x * kt;
-    if (kbase >= kmaps) return;
-    const int tid = threadIdx.x;
-    const double2* tw2 = d.tw + rp.tw_off;
-    const int* radix = d.radix + rp.fac_off;
-    const unsigned short* perm = d.perm + rp.perm_off;
-    const bool equator = rp.start_s < 0;
-
-    // z[n] = T_north[n] + i T_south[n] of map kbase + kk
-    const size_t map_stride = (size_t)d.ncomp * d.npix;
-    const double* mbase = maps + ((size_t)(k0 + kbase) * d.ncomp + comp) * d.npix;
-    const long long sn = rp.start_n, ss = rp.start_s;
-    auto ld = [&](int e, int kk) -> double2 {
-        if (kbase + kk >= kmaps) return make_double2(0.0, 0.0);
-        const double* mp = mbase + (size_t)kk * map_stride;
-        return make_double2(__ldg(mp + sn + e), equator ? 0.0 : __ldg(mp + ss + e));
-    };
-
     double2* cur = smem;
     int L = N;
-    for (int f = 0; f < rp.nfac; ++f) {
+    for (int f = 0; f < nfac; ++f) {
         const int R = radix[f];
         if (f == 0) {
             switch (R) {
@@ -267,6 +244,127 @@ __global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* _
         }
         L /= R;
     }
+    return cur;
+}
+
+// backward transform: `cur` holds bin k at position perm[k]; the last stage writes through `st`
+template <class ST>
+__device__ __forceinline__ void fft_backward(double2* smem, double2* cur, int N, const int* __restrict__ radix, int nfac, int kt,
+                                             int ktsh, const double2* __restrict__ tw2, ST st)
+{
+    int L = 1;
+    for (int f = nfac - 1; f >= 0; --f) {
+        const int R = radix[f];
+        L *= R;
+        if (f == 0) {
+            switch (R) {
+                case 2: dit_stage<2, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 3: dit_stage<3, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 4: dit_stage<4, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 5: dit_stage<5, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 7: dit_stage<7, true>(cur, N, L, kt, ktsh, tw2, st); break;
+                default: dit_generic<true>(cur, nullptr, N, L, R, kt, ktsh, tw2, st); break;
+            }
+        } else {
+            switch (R) {
+                case 2: dit_stage<2, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 3: dit_stage<3, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 4: dit_stage<4, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 5: dit_stage<5, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 7: dit_stage<7, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                default: {
+                    double2* other = (cur == smem) ? smem + ((size_t)N << ktsh) : smem;
+                    dit_generic<false>(cur, other, N, L, R, kt, ktsh, tw2, st);
+                    cur = other;
+                } break;
+            }
+        }
+    }
+}
+
+// Bluestein (chirp-z) circular convolution of power-of-two length Lc, in place in `buf`:
+//   buf <- IFFT_Lc( FFT_Lc(x) . Hf ),  x delivered by `ld` (first forward stage), result handed to `st` by the
+// last backward stage when GOUT, else left in buf in natural order.  Hf is stored in forward-output position order.
+template <bool GIN, bool GOUT, bool CONJ, class LD, class ST>
+__device__ __forceinline__ void bluestein_conv(double2* buf, int Lc, const int* __restrict__ radix, int nfac, int kt, int ktsh,
+                                               const double2* __restrict__ btw, const double2* __restrict__ hf, LD ld, ST st)
+{
+    int L = Lc;
+    for (int f = 0; f < nfac; ++f) {
+        const int R = radix[f];
+        if (GIN && f == 0) {
+            if (R == 4) dif_stage<4, true>(buf, Lc, L, kt, ktsh, btw, ld);
+            else dif_stage<2, true>(buf, Lc, L, kt, ktsh, btw, ld);
+        } else {
+            if (R == 4) dif_stage<4, false>(buf, Lc, L, kt, ktsh, btw, ld);
+            else dif_stage<2, false>(buf, Lc, L, kt, ktsh, btw, ld);
+        }
+        L /= R;
+    }
+    const int tot = Lc << ktsh;
+    for (int i = threadIdx.x; i < tot; i += NT) {
+        double2 h = __ldg(hf + (i >> ktsh));
+        if (CONJ) h.y = -h.y;
+        buf[i] = cmul(buf[i], h);
+    }
+    __syncthreads();
+    L = 1;
+    for (int f = nfac - 1; f >= 0; --f) {
+        const int R = radix[f];
+        L *= R;
+        if (GOUT && f == 0) {
+            if (R == 4) dit_stage<4, true>(buf, Lc, L, kt, ktsh, btw, st);
+            else dit_stage<2, true>(buf, Lc, L, kt, ktsh, btw, st);
+        } else {
+            if (R == 4) dit_stage<4, false>(buf, Lc, L, kt, ktsh, btw, st);
+            else dit_stage<2, false>(buf, Lc, L, kt, ktsh, btw, st);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// analysis: maps -> F (E/O folded, phase shifted, aliased to every m < mlim)
+// grid (map blocks, rings of the launch class, ncomp)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* __restrict__ ring_list,
+                                                     const double* __restrict__ maps, double* __restrict__ F,
+                                                     int k0, int kmaps)
+{
+    extern __shared__ double2 smem[];
+    const int p = ring_list[blockIdx.y], comp = blockIdx.z;
+    const RingPair rp = d.rings[p];
+    const int N = rp.n, kt = rp.kt, ktsh = __ffs(kt) - 1;
+    const int kbase = blockIdx.x * kt;
+    if (kbase >= kmaps) return;
+    const int tid = threadIdx.x;
+    const double2* tw2 = d.tw + rp.tw_off;
+    const unsigned short* perm = d.perm + rp.perm_off;
+    const bool equator = rp.start_s < 0;
+    const bool blue = rp.lc > 0;
+
+    // z[n] = T_north[n] + i T_south[n] of map kbase + kk
+    const size_t map_stride = (size_t)d.ncomp * d.npix;
+    const double* mbase = maps + ((size_t)(k0 + kbase) * d.ncomp + comp) * d.npix;
+    const long long sn = rp.start_n, ss = rp.start_s;
+    auto ld = [&](int e, int kk) -> double2 {
+        if (kbase + kk >= kmaps) return make_double2(0.0, 0.0);
+        const double* mp = mbase + (size_t)kk * map_stride;
+        return make_double2(__ldg(mp + sn + e), equator ? 0.0 : __ldg(mp + ss + e));
+    };
+
+    double2* cur = smem;
+    if (!blue) {
+        cur = fft_forward(smem, N, d.radix + rp.fac_off, rp.nfac, kt, ktsh, tw2, ld);
+    } else {
+        // X_b = c_b sum_n (x_n c_n) conj(c)_{b-n},  c_n = exp(-i pi n^2 / N) = W_{2N}^{n^2 mod 2N}
+        auto ldc = [&](int e, int kk) -> double2 {
+            if (e >= N) return make_double2(0.0, 0.0);
+            return cmul(ld(e, kk), __ldg(tw2 + (e * e) % (2 * N)));
+        };
+        auto nost = [](int, int, double2) {};
+        bluestein_conv<true, false, false>(smem, rp.lc, d.radix + rp.b_fac_off, rp.b_nfac, kt, ktsh, d.tw + rp.b_tw_off,
+                                           d.tw + rp.hf_off, ldc, nost);
+    }
 
     // FFT mapping: m -> bin on the frequency circle (stored at position perm[bin]), phase, fold
     const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
@@ -277,7 +375,13 @@ __global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* _
         const int k = kbase + kk;
         if (k >= kmaps) continue;
         const int b = m % N, bc = b == 0 ? 0 : N - b;
-        const double2 A = cur[((int)perm[b] << ktsh) + kk], B = cur[((int)perm[bc] << ktsh) + kk];
+        double2 A, B;
+        if (!blue) {
+            A = cur[((int)perm[b] << ktsh) + kk]; B = cur[((int)perm[bc] << ktsh) + kk];
+        } else {
+            A = cmul(cur[(b << ktsh) + kk], __ldg(tw2 + (b * b) % (2 * N)));
+            B = cmul(cur[(bc << ktsh) + kk], __ldg(tw2 + (bc * bc) % (2 * N)));
+        }
         // G_north = (A + conj B)/2, G_south = (A - conj B)/(2i)
         const double2 gn = make_double2(0.5 * (A.x + B.x), 0.5 * (A.y - B.y));
         const double2 gs = make_double2(0.5 * (A.y + B.y), -0.5 * (A.x - B.x));
@@ -311,9 +415,9 @@ __global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* 
     if (kbase >= kmaps) return;
     const int tid = threadIdx.x;
     const double2* tw2 = d.tw + rp.tw_off;
-    const int* radix = d.radix + rp.fac_off;
     const unsigned short* perm = d.perm + rp.perm_off;
     const bool equator = rp.start_s < 0;
+    const bool blue = rp.lc > 0;
     const int mlim = rp.mlim;
     double2* cur = smem;
 
@@ -345,9 +449,25 @@ __global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* 
         }
         if (equator) ys = make_double2(0.0, 0.0);
         if (b == 0 || 2 * b == N) { yn.y = 0.0; ys.y = 0.0; }
-        cur[((int)perm[b] << ktsh) + kk] = make_double2(yn.x - ys.y, yn.y + ys.x);
-        if (b > 0 && 2 * b < N)
-            cur[((int)perm[N - b] << ktsh) + kk] = make_double2(yn.x + ys.y, ys.x - yn.y);
+        const double2 zb = make_double2(yn.x - ys.y, yn.y + ys.x);
+        const double2 zc = make_double2(yn.x + ys.y, ys.x - yn.y);           // Z[N - b]
+        if (!blue) {
+            cur[((int)perm[b] << ktsh) + kk] = zb;
+            if (b > 0 && 2 * b < N) cur[((int)perm[N - b] << ktsh) + kk] = zc;
+        } else {
+            // x_n = conj(c)_n sum_b (Z_b conj(c)_b) c_{n-b}
+            double2 c = __ldg(tw2 + (b * b) % (2 * N)); c.y = -c.y;
+            cur[(b << ktsh) + kk] = cmul(zb, c);
+            if (b > 0 && 2 * b < N) {
+                const int bb = N - b;
+                double2 c2 = __ldg(tw2 + (bb * bb) % (2 * N)); c2.y = -c2.y;
+                cur[(bb << ktsh) + kk] = cmul(zc, c2);
+            }
+        }
+    }
+    if (blue) {
+        const int tot = rp.lc << ktsh;
+        for (int i = (N << ktsh) + tid; i < tot; i += NT) cur[i] = make_double2(0.0, 0.0);
     }
     __syncthreads();
 
@@ -368,33 +488,17 @@ __global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* 
         }
     };
 
-    int L = 1;
-    for (int f = rp.nfac - 1; f >= 0; --f) {
-        const int R = radix[f];
-        L *= R;
-        if (f == 0) {
-            switch (R) {
-                case 2: dit_stage<2, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 3: dit_stage<3, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 4: dit_stage<4, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 5: dit_stage<5, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 7: dit_stage<7, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                default: dit_generic<true>(cur, nullptr, N, L, R, kt, ktsh, tw2, st); break;
-            }
-        } else {
-            switch (R) {
-                case 2: dit_stage<2, false>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 3: dit_stage<3, false>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 4: dit_stage<4, false>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 5: dit_stage<5, false>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 7: dit_stage<7, false>(cur, N, L, kt, ktsh, tw2, st); break;
-                default: {
-                    double2* other = (cur == smem) ? smem + ((size_t)N << ktsh) : smem;
-                    dit_generic<false>(cur, other, N, L, R, kt, ktsh, tw2, st);
-                    cur = other;
-                } break;
-            }
-        }
+    if (!blue) {
+        fft_backward(smem, cur, N, d.radix + rp.fac_off, rp.nfac, kt, ktsh, tw2, st);
+    } else {
+        auto stc = [&](int e, int kk, double2 v) {
+            if (e >= N) return;
+            double2 c = __ldg(tw2 + (e * e) % (2 * N)); c.y = -c.y;
+            st(e, kk, cmul(v, c));
+        };
+        auto nold = [](int, int) -> double2 { return make_double2(0.0, 0.0); };
+        bluestein_conv<false, true, true>(smem, rp.lc, d.radix + rp.b_fac_off, rp.b_nfac, kt, ktsh, d.tw + rp.b_tw_off,
+                                          d.tw + rp.hf_off, nold, stc);
     }
 }
 

@@ -37,6 +37,8 @@ def _gpu_analysis(plan, maps):
 @pytest.mark.parametrize("nside,lmax,nmaps", [
     (1, 2, 1), (1, 0, 3), (2, 5, 2), (3, 8, 5), (4, 11, 8), (5, 14, 3), (8, 23, 70), (16, 47, 8),
     (16, 20, 4), (16, 63, 2), (32, 95, 130),
+    (48, 143, 5),      # ring lengths 4*37, 4*41, 4*43, 4*47: Bluestein rings
+    (160, 64, 3),      # ring lengths 4*121, 4*143: two direct prime stages (out of place), Bluestein up to 4*157
 ])
 def test_spin0_small_full(nside, lmax, nmaps):
     """both directions, every output element; ragged map counts, odd nside, lmax below / above 3 nside - 1"""
