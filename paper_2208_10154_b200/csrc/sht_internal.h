@@ -12,6 +12,7 @@ namespace sht {
 constexpr int KG = 4;                        // maps per workspace group (one 128-byte line = E|O of 4 maps)
 constexpr int KTILE_MAPS = 64;               // maps per Legendre k-tile (spin 0); spin 2: 32 (Q,U) pairs
 constexpr int NK = 2 * KTILE_MAPS;           // real columns per k-tile (re,im interleaved)
+constexpr int LEG_A_ML = 128;                // l rows per tile of the Legendre analysis kernel
 constexpr int MAX_RADIX_LIST = 16;           // factors of one ring length
 constexpr int RING_THREADS = 512;            // threads per CTA of the ring kernels
 constexpr int RING_EMAX = 8192;              // complex elements (ring length x maps) one ring CTA holds in smem
@@ -57,6 +58,8 @@ struct DevicePlan {
     const double2* seed;            // [lmax+1][nh] (lambda_{ls-1}, lambda_{ls-2})
     const double2* spin2c;          // [lmax+1] per-l constants for spin 2 (unused for spin 0)
     const int* mlim;                // [nh] copy of RingPair::mlim (monotone non-decreasing in p)
+    const int* pst;                 // [lmax+1][ntile_max] first ring pair that takes part in l tile t of order m
+    int ntile_max;                  // l tiles of order 0
 };
 
 // Workspace F (both directions): T_m^k(theta) of PAPER.md:52 for one chunk of maps,
@@ -112,6 +115,7 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st);
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
+size_t legendre_smem_bytes(int nh, int ntile_max);
 // plan-time seed table (sht_plan.cu)
 cudaError_t launch_seed_table(const DevicePlan& d, const double* cm, int* lstart, double2* seed, cudaStream_t st);
 

@@ -1,14 +1,19 @@
 // sht_legendre.cu -- subsystem (2): fused Legendre recurrence + FP64 tensor-core (DMMA.8x8x4) contraction,
-// and subsystem (3): the m-major a_lm scatter / gather in its prologue / epilogue.
+// and subsystem (3): the m-major a_lm scatter / gather in its epilogue / prologue.
 //
 //   analysis  (PAPER.md:56-60 eq. 3, :95 eq. 7):  A_m = P_m T_m, contraction over ring pairs p,
 //       a_lm^k = sum_p lambda_lm(theta_p) X_p^k,  X = E (l+m even) or O (l+m odd)   [N/S fold]
 //   synthesis (PAPER.md:74-76 eq. 5, :97 eq. 7):  T_m = P_m^t A_m, contraction over l,
 //       Ee_p = sum_{l+m even} lambda_lm(theta_p) a_lm,  Oo_p likewise; north = Ee + Oo, south = Ee - Oo.
 //
-// lambda_lm tiles are produced on the fly by the three-term recurrence, started at the
-// plan's l_safe(m,p) (item 11), written to shared memory and consumed as DMMA A fragments;
-// rings whose lambda is below threshold for a whole tile are skipped (ring optimisation, item 10, :229).
+// Both kernels are warp specialised (12 warps): 8 consumer warps issue DMMA on a 128 x 128 CTA tile (each warp
+// 64 x 32, accumulators in registers -- FP64 has no tcgen05/TMEM path on sm_100a, DMMA.8x8x4 is the native FP64
+// tensor instruction), one producer warp streams the operand tiles (T_m^k(theta) resp. a_lm) with TMA
+// (cp.async.bulk.tensor, 128-byte swizzle) into an mbarrier-guarded ring of shared-memory stages, and generator
+// warps run the three-term recurrence from the plan's l_safe(m,p) (item 11)
+// into the same stages.  The lambda tile and the operand tile of a stage are released together by the consumers.
+// Rings whose lambda is below threshold for a whole tile are skipped (ring optimisation, item 10, :229).
+#include <cstdio>
 #include "sht_internal.h"
 
 namespace sht {
@@ -19,165 +24,232 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// ---- tile shapes ---------------------------------------------------------------------------------
-constexpr int LEG_THREADS = 512;     // 16 warps as 4 (M) x 4 (N); each warp owns a 32 x 32 block of C
-constexpr int A_ML = 128;            // analysis: l rows per tile (64 of each parity class)
-constexpr int A_PC = 32;             // analysis: ring pairs per contraction chunk
-constexpr int A_SX = NK + 4;         // X tile row stride (doubles), = 4 mod 16: conflict-free B fragments
-constexpr int A_SL = A_PC + 2;       // lambda tile row stride, = 2 mod 8: conflict-free A fragments
-constexpr int S_PB = 64;             // synthesis: ring pairs per tile (Ee rows + Oo rows = 128 C rows)
-constexpr int S_LC = 32;             // synthesis: l values per contraction chunk (16 of each parity)
-constexpr int S_SA = 2 * S_LC + 2;   // a_lm tile stride per map (doubles), = 2 mod 16
-constexpr int S_SL = S_PB + 2;       // lambda tile row stride, = 2 mod 8
+// ---- mbarrier / TMA wrappers ---------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2, int c3)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+        : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map)
+{
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// ---- tile shapes ---------------------------------------------------------------------------------------
+constexpr int LEG_CONSUMER_WARPS = 8;        // 2 (l parity class) x 4 (32-column slices); warp tile 64 x 32
+constexpr int LEG_THREADS = 384;             // + warp 8: TMA producer, warps 9,10: lambda generators, warp 11 idle
+constexpr int A_ML = LEG_A_ML;               // analysis: l rows per tile (64 of each parity class)
+constexpr int A_PC = 32;                     // analysis: ring pairs per stage (two TMA boxes of 16)
+constexpr int A_SL = 66;                     // lambda tile: stride (doubles) between rings, = 2 mod 8: conflict-free A fragments
+constexpr int A_STAGES = 2;
+constexpr int A_XBYTES = A_PC * NK * 2 * 8;  // E and O rows of a stage: 64 KB
+constexpr int A_LBYTES = 2 * A_PC * A_SL * 8;
+constexpr int A_STAGE_BYTES = A_XBYTES + A_LBYTES;
+static_assert(A_STAGE_BYTES % 1024 == 0, "stages must keep the 1024-byte alignment of the swizzled TMA boxes");
+constexpr int S_PB = 64;                     // synthesis: ring pairs per CTA tile (Ee rows + Oo rows = 128 C rows)
+constexpr int S_LC = 32;                     // synthesis: l values per stage (16 of each parity, four TMA boxes of 8 l)
+constexpr int S_SL = 66;                     // lambda tile: stride (doubles) between l rows, = 2 mod 8
+constexpr int S_STAGES = 4;
+constexpr int S_ABYTES = S_LC * KTILE_MAPS * 16;     // a_lm tile of a stage: 32 KB
+constexpr int S_LBYTES = S_LC * S_SL * 8;
+constexpr int S_STAGE_BYTES = (S_ABYTES + S_LBYTES + 1023) / 1024 * 1024;
+constexpr int S_SC = NK + 4;                 // epilogue staging row stride (doubles)
+static_assert(2 * S_PB * S_SC * 8 <= S_STAGES * S_STAGE_BYTES, "epilogue staging reuses the stage memory");
 
 // ------------------------------------------------------------------------------------------------
-// analysis kernel: one CTA per (m, k-tile); loops over l tiles (outer) and ring chunks (inner).
+// analysis kernel: one CTA per (m, k-tile); l tiles outer, ring chunks inner.
+// Stage layout: [X: 2 boxes x (16 kg x 16 p x 128 B, 128B-swizzled)] [lambda: 2 classes x 32 p x A_SL]
 // ------------------------------------------------------------------------------------------------
-struct AnalysisSmem {
-    double X[2][A_PC][A_SX];         // E and O rows of the chunk
-    double L[A_ML][A_SL];            // lambda[l - l0][p - pc]
-    double2 coef[A_ML];              // (alpha, beta) of the tile's l values
-};
-
 __global__ void __launch_bounds__(LEG_THREADS, 1)
-k_legendre_analysis(DevicePlan d, const double* __restrict__ F, double* __restrict__ alm, int k0, int kmaps,
+k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
                     int nkt, int accumulate)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    AnalysisSmem& S = *reinterpret_cast<AnalysisSmem*>(smem_raw);
-    double* st1 = reinterpret_cast<double*>(smem_raw + sizeof(AnalysisSmem));   // lambda_{l-1} per ring
-    double* st2 = st1 + d.nh;                                                    // lambda_{l-2}
-    int* lsp = reinterpret_cast<int*>(st2 + d.nh);                               // l_safe per ring
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char* stage_base = smem_raw;
+    double2* state = reinterpret_cast<double2*>(smem_raw + A_STAGES * A_STAGE_BYTES);      // (lambda_{l-1}, lambda_{l-2}) per ring
+    uint64_t* full = reinterpret_cast<uint64_t*>(state + d.nh);
+    uint64_t* empty = full + A_STAGES;
+    int* pst = reinterpret_cast<int*>(empty + A_STAGES);                                   // first ring of every l tile
 
     const int m = blockIdx.x / nkt, kt = blockIdx.x % nkt;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm = warp >> 2, wn = warp & 3;
-    const int cls = wm >> 1;                         // 0: l - m even (uses E), 1: odd (uses O)
-    const int rbase = (wm & 1) * 32;                 // first row of this warp inside its parity class
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
+    const int ntile = (lmax - m) / A_ML + 1;
 
-    for (int p = tid; p < nh; p += LEG_THREADS) {
-        const double2 sd = d.seed[(size_t)m * nh + p];
-        st1[p] = sd.x; st2[p] = sd.y;
-        lsp[p] = d.lstart[(size_t)m * nh + p];
+    for (int p = tid; p < nh; p += LEG_THREADS) state[p] = d.seed[(size_t)m * nh + p];
+    for (int t = tid; t < ntile; t += LEG_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
+    if (tid == 0) {
+        for (int s = 0; s < A_STAGES; ++s) { mbar_init(full + s, 1 + 32); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
+        fence_barrier_init();
+        tma_prefetch_desc(&tmF);
     }
     __syncthreads();
-    const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
-    const double2* Fc = reinterpret_cast<const double2*>(F);
 
-    for (int l0 = m; l0 <= lmax; l0 += A_ML) {
-        // first ring that has any non-negligible lambda in this l tile (l_safe decreases towards the equator)
-        int pstart;
-        {
-            int lo = 0, hi = nh;                     // first p with lsp[p] < l0 + A_ML
-            while (lo < hi) { int mid = (lo + hi) >> 1; if (lsp[mid] < l0 + A_ML) hi = mid; else lo = mid + 1; }
-            // rings with mlim[p] <= m were never written to the workspace (and have lambda = 0 throughout)
-            int lo2 = 0, hi2 = nh;
-            while (lo2 < hi2) { int mid = (lo2 + hi2) >> 1; if (d.mlim[mid] > m) hi2 = mid; else lo2 = mid + 1; }
-            pstart = lo > lo2 ? lo : lo2;
-        }
-        if (tid < A_ML) {
-            const int l = l0 + tid;
-            S.coef[tid] = (l <= lmax) ? coefm[l] : make_double2(0.0, 0.0);
-        }
-        double c[4][4][2];
+    if (warp < LEG_CONSUMER_WARPS) {
+        // ===== consumers: C[l, k'] += lambda[l, p] X[p, k'] =====
+        const int cls = warp >> 2, wn = warp & 3;      // cls 0: l - m even (uses E), 1: odd (uses O)
+        const int g = lane >> 2, t = lane & 3;
+        double c[8][4][2];
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
+        for (int i = 0; i < 8; ++i)
 #pragma unroll
             for (int j = 0; j < 4; ++j) { c[i][j][0] = 0.0; c[i][j][1] = 0.0; }
-
-        for (int pc = pstart; pc < nh; pc += A_PC) {
-            __syncthreads();                         // previous chunk consumed, coef visible
-            // ---- X tile: rows pc .. pc+A_PC-1, E and O, 128 real columns of this k-tile
-            for (int e = tid; e < 2 * A_PC * (NK / 2); e += LEG_THREADS) {
-                const int col2 = e % (NK / 2);       // complex column
-                const int r = (e / (NK / 2)) % A_PC;
-                const int h = e / ((NK / 2) * A_PC);
-                const int p = pc + r;
-                double2 v = make_double2(0.0, 0.0);
-                if (p < nh) {
-                    const int k = kt * KTILE_MAPS + col2;
-                    v = Fc[f_cell(d, p, k >> 2, m, comp, h) + (k & 3)];
+        int stage = 0; uint32_t phase = 0;
+        const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
+        for (int tile = 0; tile < ntile; ++tile) {
+            const int l0 = m + tile * A_ML;
+            for (int pc = pst[tile]; pc < nh; pc += A_PC) {
+                mbar_wait(full + stage, phase);
+                const double* Xs = reinterpret_cast<const double*>(stage_base + (size_t)stage * A_STAGE_BYTES);
+                const double* Ls = Xs + A_XBYTES / 8 + cls * (A_PC * A_SL);
+#pragma unroll
+                for (int ks = 0; ks < A_PC / 4; ++ks) {
+                    const int sub = ks >> 2, ksl = ks & 3;
+                    const int pl = 8 * (ksl >> 1) + 2 * t + (ksl & 1);        // ring inside the 16-ring box
+                    double a[8], b[4];
+                    const double* La = Ls + (16 * sub + pl) * A_SL + g;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
+                    const double* Xb = Xs + sub * 4096 + pl * 16 + ((((4 * cls + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) b[j] = Xb[(4 * wn + j) * 256];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
                 }
-                *reinterpret_cast<double2*>(&S.X[h][r][2 * col2]) = v;
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + stage);
+                if (++stage == A_STAGES) { stage = 0; phase ^= 1; }
             }
-            // ---- lambda tile: thread t < A_PC walks ring pc + t through the tile's l values
-            if (tid < A_PC) {
-                const int p = pc + tid;
+            // ---- epilogue: scatter to the m-major alm layout; a lane holds (re, im) of one (l, map)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int l = l0 + 2 * (8 * i + g) + cls;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int kk = kt * KTILE_MAPS + wn * 16 + 4 * j + t;
+                    if (l <= lmax && kk < kmaps) {
+                        double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + l;
+                        double2 v = make_double2(c[i][j][0], m == 0 ? 0.0 : c[i][j][1]);
+                        if (accumulate) { const double2 o = *dst; v.x += o.x; v.y += o.y; }
+                        *dst = v;
+                    }
+                    c[i][j][0] = 0.0; c[i][j][1] = 0.0;
+                }
+            }
+        }
+    } else if (warp == LEG_CONSUMER_WARPS) {
+        // ===== TMA producer: the E/O rows of 32 rings x 64 maps per stage =====
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            for (int tile = 0; tile < ntile; ++tile) {
+                for (int pc = pst[tile]; pc < nh; pc += A_PC) {
+                    mbar_wait(empty + stage, phase ^ 1);
+                    unsigned char* Xs = stage_base + (size_t)stage * A_STAGE_BYTES;
+                    mbar_arrive_expect_tx(full + stage, A_XBYTES);
+                    tma_load_4d(Xs, &tmF, full + stage, 0, pc, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
+                    tma_load_4d(Xs + A_XBYTES / 2, &tmF, full + stage, 0, pc + 16, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
+                    if (++stage == A_STAGES) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp <= LEG_CONSUMER_WARPS + 2) {
+        // ===== lambda generators: warp w fills the chunks with index = w (mod 2); lane = ring inside the chunk =====
+        const int gw = warp - LEG_CONSUMER_WARPS - 1;
+        const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+        int chunk = 0;
+        for (int tile = 0; tile < ntile; ++tile) {
+            const int l0 = m + tile * A_ML;
+            // a ring's state written in the previous l tile may come from the other generator warp
+            named_bar_sync(1, 64);
+            for (int pc = pst[tile]; pc < nh; pc += A_PC, ++chunk) {
+                if ((chunk & 1) != gw) continue;
+                const int stage = chunk % A_STAGES;
+                const uint32_t phase = (chunk / A_STAGES) & 1;
+                const int p = pc + lane;
+                double x1 = 0.0, x2 = 0.0, z = 0.0;
+                int ls = lmax + 1;
                 if (p < nh) {
-                    double x1 = st1[p], x2 = st2[p];
-                    const int ls = lsp[p];
-                    const double z = d.z[p];
+                    const double2 sd = state[p];
+                    x1 = sd.x; x2 = sd.y; z = d.z[p];
+                    ls = d.lstart[(size_t)m * nh + p];
+                }
+                mbar_wait(empty + stage, phase ^ 1);
+                double* Ls = reinterpret_cast<double*>(stage_base + (size_t)stage * A_STAGE_BYTES + A_XBYTES) + lane * A_SL;
+                const int lend = min(lmax - l0 + 1, A_ML);          // rows of this tile that exist
 #pragma unroll 4
-                    for (int r = 0; r < A_ML; ++r) {
-                        const int l = l0 + r;
-                        double v = 0.0;
-                        if (l >= ls && l <= lmax) {
-                            const double2 ab = S.coef[r];
+                for (int r = 0; r < A_ML; ++r) {
+                    double v = 0.0;
+                    if (r < lend) {
+                        const double2 ab = __ldg(coefm + l0 + r);
+                        if (l0 + r >= ls) {
                             v = fma(ab.x * z, x1, -(ab.y * x2));
                             x2 = x1; x1 = v;
                         }
-                        S.L[r][tid] = v;
                     }
-                    st1[p] = x1; st2[p] = x2;
-                } else {
-                    for (int r = 0; r < A_ML; ++r) S.L[r][tid] = 0.0;
+                    Ls[(r & 1) * (A_PC * A_SL) + (r >> 1)] = v;
                 }
-            }
-            __syncthreads();
-            // ---- DMMA: C[l, k'] += lambda[l, p] X[p, k']
-#pragma unroll
-            for (int ks = 0; ks < A_PC / 4; ++ks) {
-                double a[4], b[4];
-#pragma unroll
-                for (int i = 0; i < 4; ++i)
-                    a[i] = S.L[2 * (rbase + 8 * i + (lane >> 2)) + cls][4 * ks + (lane & 3)];
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    b[j] = S.X[cls][4 * ks + (lane & 3)][wn * 32 + 8 * j + (lane >> 2)];
-#pragma unroll
-                for (int i = 0; i < 4; ++i)
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
+                if (p < nh) state[p] = make_double2(x1, x2);
+                mbar_arrive(full + stage);
             }
         }
-        // ---- epilogue: scatter to the m-major alm layout; a lane holds (re, im) of one (l, map)
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int l = l0 + 2 * (rbase + 8 * i + (lane >> 2)) + cls;
-            if (l > lmax) continue;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int kk = kt * KTILE_MAPS + wn * 16 + 4 * j + (lane & 3);
-                if (kk >= kmaps) continue;
-                double2* dst = reinterpret_cast<double2*>(alm) +
-                               ((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + ((long long)m * (2 * lmax + 1 - m) / 2) + l;
-                double2 v = make_double2(c[i][j][0], m == 0 ? 0.0 : c[i][j][1]);
-                if (accumulate) { const double2 o = *dst; v.x += o.x; v.y += o.y; }
-                *dst = v;
-            }
-        }
-        __syncthreads();                             // coef / L reuse by the next l tile
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// synthesis kernel: one CTA per (m, ring block of 64, k-tile); loops over l chunks.
+// synthesis kernel: one CTA per (m, block of 64 ring pairs, k-tile); loops over l chunks of 32.
+// Stage layout: [a_lm: 4 boxes x (64 maps x 8 l x 16 B, 128B-swizzled)] [lambda: 32 l x S_SL]
 // ------------------------------------------------------------------------------------------------
-struct SynthesisSmem {
-    double A[KTILE_MAPS][S_SA];      // a_lm tile: [map][l - lc][re,im]
-    double L[S_LC][S_SL];            // lambda[l - lc][p - pb]
-    double2 coef[S_LC];
-};
-
 __global__ void __launch_bounds__(LEG_THREADS, 1)
-k_legendre_synthesis(DevicePlan d, const double* __restrict__ alm, double* __restrict__ F, int k0, int kmaps,
+k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
                      int nkt, int npb)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    SynthesisSmem& S = *reinterpret_cast<SynthesisSmem*>(smem_raw);
-    double* Cs = reinterpret_cast<double*>(smem_raw);          // epilogue staging, reuses the mainloop smem
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char* stage_base = smem_raw;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S_STAGES * S_STAGE_BYTES);
+    uint64_t* empty = full + S_STAGES;
+    int* lmin_s = reinterpret_cast<int*>(empty + S_STAGES);
 
     // block order: m slowest (long m first), then ring block, k-tile fastest
     const int kt = blockIdx.x % nkt;
@@ -185,125 +257,206 @@ k_legendre_synthesis(DevicePlan d, const double* __restrict__ alm, double* __res
     const int m = blockIdx.x / (nkt * npb);
     const int pb = pbi * S_PB;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm = warp >> 2, wn = warp & 3;
-    const int cls = wm >> 1;
-    const int rbase = (wm & 1) * 32;
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
-
-    // per-ring recurrence state lives in registers of threads 0..S_PB-1
-    double x1 = 0.0, x2 = 0.0, z = 0.0;
-    int ls = lmax + 1;
-    if (tid < S_PB && pb + tid < nh) {
-        const double2 sd = d.seed[(size_t)m * nh + pb + tid];
-        x1 = sd.x; x2 = sd.y; ls = d.lstart[(size_t)m * nh + pb + tid]; z = d.z[pb + tid];
-    }
-    // the ring of the block closest to the equator starts first (l_safe decreases with p)
     const int plast = min(pb + S_PB, nh) - 1;
     if (m >= d.mlim[plast]) return;                    // no ring of this block takes part in order m (never read)
-    const int lfirst = d.lstart[(size_t)m * nh + plast];
-    const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
-    const double2* almc = reinterpret_cast<const double2*>(alm);
 
-    double c[4][4][2];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { c[i][j][0] = 0.0; c[i][j][1] = 0.0; }
-
+    if (tid == 0) {
+        for (int s = 0; s < S_STAGES; ++s) { mbar_init(full + s, 1 + 64); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
+        fence_barrier_init();
+        tma_prefetch_desc(&tmA);
+        *lmin_s = lmax + 1;
+    }
+    __syncthreads();
+    if (tid < S_PB && pb + tid < nh) atomicMin(lmin_s, d.lstart[(size_t)m * nh + pb + tid]);
+    __syncthreads();
+    const int lmin = *lmin_s;
     // chunks are aligned to m so that (l - m) even <-> even local index
-    const int cfirst = (lfirst > lmax) ? (lmax + 1) : m + ((lfirst - m) / S_LC) * S_LC;
-    for (int lc = cfirst; lc <= lmax; lc += S_LC) {
-        __syncthreads();
-        if (tid < S_LC) {
-            const int l = lc + tid;
-            S.coef[tid] = (l <= lmax) ? coefm[l] : make_double2(0.0, 0.0);
-        }
-        // ---- a_lm tile, straight from the m-major ABI layout (one contiguous run per map)
-        for (int e = tid; e < KTILE_MAPS * S_LC; e += LEG_THREADS) {
-            const int ll = e % S_LC, kk = e / S_LC;
-            const int l = lc + ll, k = kt * KTILE_MAPS + kk;
-            double2 v = make_double2(0.0, 0.0);
-            if (l <= lmax && k < kmaps) {
-                v = almc[((size_t)(k0 + k) * d.ncomp + comp) * d.nalm + ((long long)m * (2 * lmax + 1 - m) / 2) + l];
-                if (m == 0) v.y = 0.0;
+    const int cfirst = (lmin > lmax) ? (lmax + 1) : m + ((lmin - m) / S_LC) * S_LC;
+    const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
+
+    if (warp < LEG_CONSUMER_WARPS) {
+        // ===== consumers: C[p, k'] += lambda[l, p] a[l, k'] over the l of this warp's parity class =====
+        const int cls = warp >> 2, wn = warp & 3;
+        const int g = lane >> 2, t = lane & 3;
+        double c[8][4][2];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { c[i][j][0] = 0.0; c[i][j][1] = 0.0; }
+        int stage = 0; uint32_t phase = 0;
+        const bool kill_im = (m == 0) && (g & 1);      // Im(a_l0) is ignored
+        for (int lc = cfirst; lc <= lmax; lc += S_LC) {
+            mbar_wait(full + stage, phase);
+            const double* As = reinterpret_cast<const double*>(stage_base + (size_t)stage * S_STAGE_BYTES);
+            const double* Ls = As + S_ABYTES / 8;
+#pragma unroll
+            for (int ks = 0; ks < S_LC / 8; ++ks) {
+                double a[8], b[4];
+                const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int row = 16 * wn + 4 * j + (g >> 1);               // map inside the k-tile
+                    const double v = As[ks * 1024 + row * 16 + ((((2 * t + cls) ^ (row & 7)) << 1) | (g & 1))];
+                    b[j] = kill_im ? 0.0 : v;
+                }
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
             }
-            *reinterpret_cast<double2*>(&S.A[kk][2 * ll]) = v;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + stage);
+            if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
         }
-        __syncthreads();                              // coef visible to the generator threads
-        if (tid < S_PB) {
-#pragma unroll 4
+        // ---- epilogue: exchange Ee / Oo through smem, write north = Ee + Oo, south = Ee - Oo lines
+        named_bar_sync(2, LEG_CONSUMER_WARPS * 32);   // every consumer is done with the stage memory
+        double* Cs = reinterpret_cast<double*>(smem_raw);
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int row = cls * S_PB + 8 * i + g;
+                const int col = wn * 32 + 8 * j + 2 * t;
+                *reinterpret_cast<double2*>(&Cs[row * S_SC + col]) = make_double2(c[i][j][0], c[i][j][1]);
+            }
+        named_bar_sync(2, LEG_CONSUMER_WARPS * 32);
+        double2* Fc = reinterpret_cast<double2*>(F);
+        for (int e = tid; e < S_PB * (NK / 2); e += LEG_CONSUMER_WARPS * 32) {
+            const int col2 = e % (NK / 2), r = e / (NK / 2);
+            const int p = pb + r;
+            if (p >= nh) continue;
+            const double2 ee = *reinterpret_cast<const double2*>(&Cs[r * S_SC + 2 * col2]);
+            const double2 oo = *reinterpret_cast<const double2*>(&Cs[(S_PB + r) * S_SC + 2 * col2]);
+            const int k = kt * KTILE_MAPS + col2;
+            double2* dst = Fc + f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
+            dst[0] = make_double2(ee.x + oo.x, ee.y + oo.y);
+            dst[KG] = make_double2(ee.x - oo.x, ee.y - oo.y);
+        }
+    } else if (warp == LEG_CONSUMER_WARPS) {
+        // ===== TMA producer: a_lm of 32 l x 64 maps per stage, straight from the m-major ABI layout =====
+        if (lane == 0) {
+            int stage = 0; uint32_t phase = 0;
+            const int row0 = (k0 + kt * KTILE_MAPS) * d.ncomp + comp;
+            for (int lc = cfirst; lc <= lmax; lc += S_LC) {
+                mbar_wait(empty + stage, phase ^ 1);
+                unsigned char* As = stage_base + (size_t)stage * S_STAGE_BYTES;
+                mbar_arrive_expect_tx(full + stage, S_ABYTES);
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    tma_load_2d(As + q * (S_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0);
+                if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else if (warp <= LEG_CONSUMER_WARPS + 2) {
+        // ===== lambda generators: 64 lanes = the 64 rings of the block, recurrence state in registers =====
+        const int rl = (warp - LEG_CONSUMER_WARPS - 1) * 32 + lane;
+        const int p = pb + rl;
+        double x1 = 0.0, x2 = 0.0, z = 0.0;
+        int ls = lmax + 1;
+        if (p < nh) {
+            const double2 sd = d.seed[(size_t)m * nh + p];
+            x1 = sd.x; x2 = sd.y; ls = d.lstart[(size_t)m * nh + p]; z = d.z[p];
+        }
+        const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+        int stage = 0; uint32_t phase = 0;
+        for (int lc = cfirst; lc <= lmax; lc += S_LC) {
+            mbar_wait(empty + stage, phase ^ 1);
+            double* Ls = reinterpret_cast<double*>(stage_base + (size_t)stage * S_STAGE_BYTES + S_ABYTES) + rl;
+#pragma unroll 8
             for (int r = 0; r < S_LC; ++r) {
                 const int l = lc + r;
                 double v = 0.0;
-                if (l >= ls && l <= lmax) {
-                    const double2 ab = S.coef[r];
-                    v = fma(ab.x * z, x1, -(ab.y * x2));
-                    x2 = x1; x1 = v;
+                if (l <= lmax) {
+                    const double2 ab = __ldg(coefm + l);
+                    if (l >= ls) {
+                        v = fma(ab.x * z, x1, -(ab.y * x2));
+                        x2 = x1; x1 = v;
+                    }
                 }
-                S.L[r][tid] = v;
+                Ls[r * S_SL] = v;
             }
+            mbar_arrive(full + stage);
+            if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
         }
-        __syncthreads();
-        // ---- DMMA: C[p, k'] += lambda[l, p] a[l, k'] over the chunk's l of this warp's parity class
-#pragma unroll
-        for (int ks = 0; ks < S_LC / 8; ++ks) {
-            double a[4], b[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-                a[i] = S.L[2 * (4 * ks + (lane & 3)) + cls][rbase + 8 * i + (lane >> 2)];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int n = wn * 32 + 8 * j + (lane >> 2);          // real column: map n/2, part n&1
-                b[j] = S.A[n >> 1][2 * (2 * (4 * ks + (lane & 3)) + cls) + (n & 1)];
-            }
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
-        }
-    }
-    // ---- epilogue: exchange Ee / Oo through smem, write north = Ee + Oo, south = Ee - Oo rows
-    __syncthreads();
-    constexpr int SC = NK + 4;
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int row = cls * S_PB + rbase + 8 * i + (lane >> 2);
-            const int col = wn * 32 + 8 * j + 2 * (lane & 3);
-            *reinterpret_cast<double2*>(&Cs[row * SC + col]) = make_double2(c[i][j][0], c[i][j][1]);
-        }
-    __syncthreads();
-    double2* Fc = reinterpret_cast<double2*>(F);
-    for (int e = tid; e < S_PB * (NK / 2); e += LEG_THREADS) {
-        const int col2 = e % (NK / 2), r = e / (NK / 2);
-        const int p = pb + r;
-        if (p >= nh) continue;
-        const double2 ee = *reinterpret_cast<const double2*>(&Cs[r * SC + 2 * col2]);
-        const double2 oo = *reinterpret_cast<const double2*>(&Cs[(S_PB + r) * SC + 2 * col2]);
-        const int k = kt * KTILE_MAPS + col2;
-        double2* dst = Fc + f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
-        dst[0] = make_double2(ee.x + oo.x, ee.y + oo.y);
-        dst[KG] = make_double2(ee.x - oo.x, ee.y - oo.y);
     }
 }
 
-static size_t analysis_smem(int nh) { return sizeof(AnalysisSmem) + (size_t)nh * (2 * sizeof(double) + sizeof(int)); }
-static size_t synthesis_smem()
+// ---- host side: tensor maps and launches ---------------------------------------------------------------
+typedef CUresult (*PFN_tmapEncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                        const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                        CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static PFN_tmapEncodeTiled tmap_encoder()
 {
-    size_t a = sizeof(SynthesisSmem), b = (size_t)2 * S_PB * (NK + 4) * sizeof(double);
-    return a > b ? a : b;
+    static PFN_tmapEncodeTiled fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (PFN_tmapEncodeTiled)p;
+    }
+    return fn;
+}
+
+// workspace F[p][kg][m*ncomp+comp][16 doubles] as a 4-D tensor (innermost first: 16 doubles, p, kg, m*ncomp+comp);
+// box = one 128-byte line x 16 rings x 16 map groups x 1 order
+static cudaError_t make_tmap_F(const DevicePlan& d, const double* F, CUtensorMap* tm)
+{
+    PFN_tmapEncodeTiled enc = tmap_encoder();
+    if (!enc) return cudaErrorNotSupported;
+    const cuuint64_t mc = (cuuint64_t)(d.lmax + 1) * d.ncomp;
+    const cuuint64_t dims[4] = {16, (cuuint64_t)d.nh, (cuuint64_t)d.nkg, mc};
+    const cuuint64_t strides[3] = {(cuuint64_t)d.nkg * mc * 128, mc * 128, 128};
+    const cuuint32_t box[4] = {16, 16, 16, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(F), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+// alm[row = map*ncomp+comp][nalm*2 doubles] as a 2-D tensor; box = 8 l (128 bytes) x 64 rows
+static cudaError_t make_tmap_alm(const DevicePlan& d, const double* alm, long long rows, CUtensorMap* tm)
+{
+    PFN_tmapEncodeTiled enc = tmap_encoder();
+    if (!enc) return cudaErrorNotSupported;
+    const cuuint64_t dims[2] = {(cuuint64_t)d.nalm * 2, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)d.nalm * 16};
+    const cuuint32_t box[2] = {16, KTILE_MAPS};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(alm), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+static size_t analysis_smem(int nh, int ntile)
+{
+    return (size_t)A_STAGES * A_STAGE_BYTES + (size_t)nh * sizeof(double2) + 2 * A_STAGES * sizeof(uint64_t) + (size_t)ntile * sizeof(int);
+}
+static size_t synthesis_smem() { return (size_t)S_STAGES * S_STAGE_BYTES + 2 * S_STAGES * sizeof(uint64_t) + 16; }
+
+size_t legendre_smem_bytes(int nh, int ntile_max)
+{
+    const size_t a = analysis_smem(nh, ntile_max), s = synthesis_smem();
+    return a > s ? a : s;
 }
 
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st)
 {
-    const size_t sm = analysis_smem(d.nh);
+    const size_t sm = analysis_smem(d.nh, d.ntile_max);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
+    CUtensorMap tmF;
+    if ((e = make_tmap_F(d, F, &tmF)) != cudaSuccess) return e;
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
-    k_legendre_analysis<<<(d.lmax + 1) * nkt, LEG_THREADS, sm, st>>>(d, F, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
+    k_legendre_analysis<<<(d.lmax + 1) * nkt, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -313,9 +466,11 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
     const size_t sm = synthesis_smem();
     cudaError_t e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
+    CUtensorMap tmA;
+    if ((e = make_tmap_alm(d, alm, (long long)(k0 + kmaps) * d.ncomp, &tmA)) != cudaSuccess) return e;
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
-    k_legendre_synthesis<<<(d.lmax + 1) * nkt * npb, LEG_THREADS, sm, st>>>(d, alm, F, k0, kmaps, nkt, npb);
+    k_legendre_synthesis<<<(d.lmax + 1) * nkt * npb, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb);
     pl->launches++;
     return cudaGetLastError();
 }

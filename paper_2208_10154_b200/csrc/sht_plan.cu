@@ -361,6 +361,23 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
             mlim[p] = run;
             rings[p].mlim = run;
         }
+        // first ring pair of every (m, l tile) of the Legendre analysis kernel: the smallest p >= the ring-pruning
+        // bound whose recurrence has started before the end of the tile (no monotonicity of l_safe assumed)
+        d.ntile_max = lmax / LEG_A_ML + 1;
+        std::vector<int> pst((size_t)(lmax + 1) * d.ntile_max, d.nh);
+        for (int m = 0; m <= lmax; ++m) {
+            int* row = pst.data() + (size_t)m * d.ntile_max;
+            const int nt = (lmax - m) / LEG_A_ML + 1;
+            for (int p = 0; p < d.nh; ++p) {
+                if (mlim[p] <= m) continue;
+                const int lsv = hls[(size_t)m * d.nh + p];
+                if (lsv > lmax) continue;
+                const int jt = (lsv - m) / LEG_A_ML;
+                if (jt < nt && p < row[jt]) row[jt] = p;
+            }
+            for (int t = 1; t < nt; ++t) if (row[t - 1] < row[t]) row[t] = row[t - 1];
+        }
+        if ((ce = upload(pl, pst, &d.pst)) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
         if ((ce = upload(pl, rings, &d.rings)) != cudaSuccess || (ce = upload(pl, mlim, &d.mlim)) != cudaSuccess) {
             sht_plan_destroy(pl);
             return SHT_ERR_ALLOC;
