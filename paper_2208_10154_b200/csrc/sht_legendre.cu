@@ -108,7 +108,8 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     double2* state = reinterpret_cast<double2*>(smem_raw + A_STAGES * A_STAGE_BYTES);      // (lambda_{l-1}, lambda_{l-2}) per ring
     uint64_t* full = reinterpret_cast<uint64_t*>(state + d.nh);
     uint64_t* empty = full + A_STAGES;
-    int* pst = reinterpret_cast<int*>(empty + A_STAGES);                                   // first ring of every l tile
+    double2* cft = reinterpret_cast<double2*>(empty + A_STAGES);                           // (alpha, beta) of the current l tile
+    int* pst = reinterpret_cast<int*>(cft + A_ML);                                         // first ring of every l tile
 
     const int m = blockIdx.x / nkt, kt = blockIdx.x % nkt;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -197,12 +198,24 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     } else if (warp <= LEG_CONSUMER_WARPS + 2) {
         // ===== lambda generators: warp w fills the chunks with index = w (mod 2); lane = ring inside the chunk =====
         const int gw = warp - LEG_CONSUMER_WARPS - 1;
+        const int gl = gw * 32 + lane;                          // 0 .. 63
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+        // (alpha, beta) of an l tile are staged in shared memory once per tile (a dependent global load per
+        // recurrence step would cost an L2 round trip per l); rows past lmax get (0, 0)
+        auto load_cf = [&](int l0, int j) -> double2 {
+            const int l = l0 + gl + 64 * j;
+            return l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+        };
+        double2 cf0 = load_cf(m, 0), cf1 = load_cf(m, 1);
         int chunk = 0;
         for (int tile = 0; tile < ntile; ++tile) {
             const int l0 = m + tile * A_ML;
-            // a ring's state written in the previous l tile may come from the other generator warp
+            // both generator warps are done with the previous tile (its coefficients, and a ring's state written
+            // in the previous l tile may come from the other generator warp)
             named_bar_sync(1, 64);
+            cft[gl] = cf0; cft[gl + 64] = cf1;
+            named_bar_sync(1, 64);
+            if (tile + 1 < ntile) { cf0 = load_cf(l0 + A_ML, 0); cf1 = load_cf(l0 + A_ML, 1); }
             for (int pc = pst[tile]; pc < nh; pc += A_PC, ++chunk) {
                 if ((chunk & 1) != gw) continue;
                 const int stage = chunk % A_STAGES;
@@ -215,19 +228,16 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                     x1 = sd.x; x2 = sd.y; z = d.z[p];
                     ls = d.lstart[(size_t)m * nh + p];
                 }
+                const int rs = ls - l0;                             // first row of the tile with a started recurrence
                 mbar_wait(empty + stage, phase ^ 1);
                 double* Ls = reinterpret_cast<double*>(stage_base + (size_t)stage * A_STAGE_BYTES + A_XBYTES) + lane * A_SL;
-                const int lend = min(lmax - l0 + 1, A_ML);          // rows of this tile that exist
-#pragma unroll 4
+#pragma unroll 8
                 for (int r = 0; r < A_ML; ++r) {
-                    double v = 0.0;
-                    if (r < lend) {
-                        const double2 ab = __ldg(coefm + l0 + r);
-                        if (l0 + r >= ls) {
-                            v = fma(ab.x * z, x1, -(ab.y * x2));
-                            x2 = x1; x1 = v;
-                        }
-                    }
+                    const double2 ab = cft[r];
+                    const double t = fma(ab.x * z, x1, -(ab.y * x2));
+                    const bool on = r >= rs;
+                    const double v = on ? t : 0.0;
+                    x2 = on ? x1 : x2; x1 = on ? t : x1;
                     Ls[(r & 1) * (A_PC * A_SL) + (r >> 1)] = v;
                 }
                 if (p < nh) state[p] = make_double2(x1, x2);
@@ -249,7 +259,8 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
     unsigned char* stage_base = smem_raw;
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S_STAGES * S_STAGE_BYTES);
     uint64_t* empty = full + S_STAGES;
-    int* lmin_s = reinterpret_cast<int*>(empty + S_STAGES);
+    double2* cfs = reinterpret_cast<double2*>(empty + S_STAGES);      // 2 generator warps x 2 buffers x S_LC (alpha, beta)
+    int* lmin_s = reinterpret_cast<int*>(cfs + 4 * S_LC);
 
     // block order: m slowest (long m first), then ring block, k-tile fastest
     const int kt = blockIdx.x % nkt;
@@ -353,7 +364,8 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
         }
     } else if (warp <= LEG_CONSUMER_WARPS + 2) {
         // ===== lambda generators: 64 lanes = the 64 rings of the block, recurrence state in registers =====
-        const int rl = (warp - LEG_CONSUMER_WARPS - 1) * 32 + lane;
+        const int gw = warp - LEG_CONSUMER_WARPS - 1;
+        const int rl = gw * 32 + lane;
         const int p = pb + rl;
         double x1 = 0.0, x2 = 0.0, z = 0.0;
         int ls = lmax + 1;
@@ -362,24 +374,34 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
             x1 = sd.x; x2 = sd.y; ls = d.lstart[(size_t)m * nh + p]; z = d.z[p];
         }
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
-        int stage = 0; uint32_t phase = 0;
+        // (alpha, beta) of the next l chunk are fetched by the 32 lanes in one coalesced load while the current chunk
+        // is computed, and handed round through a per-warp shared buffer (a dependent global load per recurrence
+        // step would cost an L2 round trip per l)
+        double2* cfw = cfs + gw * (2 * S_LC);
+        auto load_cf = [&](int lc) -> double2 {
+            const int l = lc + lane;
+            return l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+        };
+        double2 cf = load_cf(cfirst);
+        int stage = 0, buf = 0; uint32_t phase = 0;
         for (int lc = cfirst; lc <= lmax; lc += S_LC) {
+            cfw[buf * S_LC + lane] = cf;
+            __syncwarp();
+            cf = load_cf(lc + S_LC);
+            const int rs = ls - lc;
             mbar_wait(empty + stage, phase ^ 1);
             double* Ls = reinterpret_cast<double*>(stage_base + (size_t)stage * S_STAGE_BYTES + S_ABYTES) + rl;
 #pragma unroll 8
             for (int r = 0; r < S_LC; ++r) {
-                const int l = lc + r;
-                double v = 0.0;
-                if (l <= lmax) {
-                    const double2 ab = __ldg(coefm + l);
-                    if (l >= ls) {
-                        v = fma(ab.x * z, x1, -(ab.y * x2));
-                        x2 = x1; x1 = v;
-                    }
-                }
+                const double2 ab = cfw[buf * S_LC + r];
+                const double t = fma(ab.x * z, x1, -(ab.y * x2));
+                const bool on = r >= rs;
+                const double v = on ? t : 0.0;
+                x2 = on ? x1 : x2; x1 = on ? t : x1;
                 Ls[r * S_SL] = v;
             }
             mbar_arrive(full + stage);
+            buf ^= 1;
             if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
         }
     }
@@ -437,9 +459,10 @@ static cudaError_t make_tmap_alm(const DevicePlan& d, const double* alm, long lo
 
 static size_t analysis_smem(int nh, int ntile)
 {
-    return (size_t)A_STAGES * A_STAGE_BYTES + (size_t)nh * sizeof(double2) + 2 * A_STAGES * sizeof(uint64_t) + (size_t)ntile * sizeof(int);
+    return (size_t)A_STAGES * A_STAGE_BYTES + (size_t)nh * sizeof(double2) + 2 * A_STAGES * sizeof(uint64_t) +
+           (size_t)A_ML * sizeof(double2) + (size_t)ntile * sizeof(int);
 }
-static size_t synthesis_smem() { return (size_t)S_STAGES * S_STAGE_BYTES + 2 * S_STAGES * sizeof(uint64_t) + 16; }
+static size_t synthesis_smem() { return (size_t)S_STAGES * S_STAGE_BYTES + 2 * S_STAGES * sizeof(uint64_t) + 4 * S_LC * sizeof(double2) + 16; }
 
 size_t legendre_smem_bytes(int nh, int ntile_max)
 {
