@@ -116,6 +116,11 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
                                      bool accumulate, cudaStream_t st);
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
 size_t legendre_smem_bytes(int nh, int ntile_max);
+// spin 2 (sht_legendre_spin2.cu); the spin-0 launchers dispatch to these
+cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
+                                           bool accumulate, cudaStream_t st);
+cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps,
+                                            cudaStream_t st);
 // plan-time seed table (sht_plan.cu)
 cudaError_t launch_seed_table(const DevicePlan& d, const double* cm, int* lstart, double2* seed, cudaStream_t st);
 

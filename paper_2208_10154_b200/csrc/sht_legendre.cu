@@ -14,65 +14,9 @@
 // into the same stages.  The lambda tile and the operand tile of a stage are released together by the consumers.
 // Rings whose lambda is below threshold for a whole tile are skipped (ring optimisation, item 10, :229).
 #include <cstdio>
-#include "sht_internal.h"
+#include "sht_legendre_common.cuh"
 
 namespace sht {
-
-__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b)
-{
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1},{%2},{%3},{%0,%1};"
-                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
-// ---- mbarrier / TMA wrappers ---------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2, int c3)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
-        : "memory");
-}
-__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map)
-{
-    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
-}
-__device__ __forceinline__ void named_bar_sync(int id, int nthreads)
-{
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
 
 // ---- tile shapes ---------------------------------------------------------------------------------------
 constexpr int LEG_CONSUMER_WARPS = 8;        // 2 (l parity class) x 4 (32-column slices); warp tile 64 x 32
@@ -92,7 +36,7 @@ constexpr int S_STAGES = 4;
 constexpr int S_ABYTES = S_LC * KTILE_MAPS * 16;     // a_lm tile of a stage: 32 KB
 constexpr int S_LBYTES = S_LC * S_SL * 8;
 constexpr int S_STAGE_BYTES = (S_ABYTES + S_LBYTES + 1023) / 1024 * 1024;
-constexpr int S_SC = NK + 4;                 // epilogue staging row stride (doubles)
+constexpr int S_SC = NK + 8;                 // epilogue staging row stride (doubles)
 static_assert(2 * S_PB * S_SC * 8 <= S_STAGES * S_STAGE_BYTES, "epilogue staging reuses the stage memory");
 
 // ------------------------------------------------------------------------------------------------
@@ -408,53 +352,13 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
 }
 
 // ---- host side: tensor maps and launches ---------------------------------------------------------------
-typedef CUresult (*PFN_tmapEncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                        const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                        CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static PFN_tmapEncodeTiled tmap_encoder()
-{
-    static PFN_tmapEncodeTiled fn = nullptr;
-    if (!fn) {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (PFN_tmapEncodeTiled)p;
-    }
-    return fn;
-}
-
-// workspace F[p][kg][m*ncomp+comp][16 doubles] as a 4-D tensor (innermost first: 16 doubles, p, kg, m*ncomp+comp);
-// box = one 128-byte line x 16 rings x 16 map groups x 1 order
-static cudaError_t make_tmap_F(const DevicePlan& d, const double* F, CUtensorMap* tm)
-{
-    PFN_tmapEncodeTiled enc = tmap_encoder();
-    if (!enc) return cudaErrorNotSupported;
-    const cuuint64_t mc = (cuuint64_t)(d.lmax + 1) * d.ncomp;
-    const cuuint64_t dims[4] = {16, (cuuint64_t)d.nh, (cuuint64_t)d.nkg, mc};
-    const cuuint64_t strides[3] = {(cuuint64_t)d.nkg * mc * 128, mc * 128, 128};
-    const cuuint32_t box[4] = {16, 16, 16, 1};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(F), dims, strides, box, estr,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
-}
-
 // alm[row = map*ncomp+comp][nalm*2 doubles] as a 2-D tensor; box = 8 l (128 bytes) x 64 rows
 static cudaError_t make_tmap_alm(const DevicePlan& d, const double* alm, long long rows, CUtensorMap* tm)
 {
-    PFN_tmapEncodeTiled enc = tmap_encoder();
-    if (!enc) return cudaErrorNotSupported;
     const cuuint64_t dims[2] = {(cuuint64_t)d.nalm * 2, (cuuint64_t)rows};
     const cuuint64_t strides[1] = {(cuuint64_t)d.nalm * 16};
     const cuuint32_t box[2] = {16, KTILE_MAPS};
-    const cuuint32_t estr[2] = {1, 1};
-    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(alm), dims, strides, box, estr,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+    return make_tmap_f64(tm, alm, 2, dims, strides, box);
 }
 
 static size_t analysis_smem(int nh, int ntile)
@@ -473,11 +377,12 @@ size_t legendre_smem_bytes(int nh, int ntile_max)
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st)
 {
+    if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st);
     const size_t sm = analysis_smem(d.nh, d.ntile_max);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tmF;
-    if ((e = make_tmap_F(d, F, &tmF)) != cudaSuccess) return e;
+    if ((e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, &tmF)) != cudaSuccess) return e;
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     k_legendre_analysis<<<(d.lmax + 1) * nkt, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
     pl->launches++;
@@ -486,6 +391,7 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
 
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st)
 {
+    if (d.spin == 2) return launch_legendre_synthesis_spin2(pl, d, alm, F, k0, kmaps, st);
     const size_t sm = synthesis_smem();
     cudaError_t e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;

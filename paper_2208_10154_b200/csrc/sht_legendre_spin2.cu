@@ -1,0 +1,473 @@
+// sht_legendre_spin2.cu -- subsystem (2) for spin 2: fused lambda recurrence -> F+/F- (App. A.2)
+// -> FP64 tensor-core contraction of the 2 x 2 block products of eq. 14 / eq. 15, and subsystem (3): the E/B
+// combination a_E = A^E, a_B = -i (iA^B) (eq. 10) in the epilogue / operand fetch.
+//
+//   analysis  (eq. 14):  (A^E; iA^B)_m = [[F+, F-], [F-, F+]]_m (Q; iU)_m      contraction over ring pairs
+//   synthesis (eq. 15):  (Q; iU)_m = [[F+, F-], [F-, F+]]_m^t (A^E; iA^B)_m    contraction over l
+// with F+ = -X1, F- = -X2 (eq. A5; reading G12),
+//   X1_lm = N_l { -[(l - m^2)/s^2 + l(l-1)/2] lambda_lm + (x/s^2) c_lm lambda_{l-1,m} }
+//   X2_lm = N_l (m/s^2) { c_lm lambda_{l-1,m} - (l-1) x lambda_lm },
+//   N_l = 2/sqrt((l-1) l (l+1)(l+2)), c_lm = sqrt((2l+1)/(2l-1) (l^2 - m^2)), x = cos(theta), s = sin(theta).
+// Under theta -> pi - theta F+ has the parity (-1)^(l+m) of lambda and F- the opposite one, so for l - m even F+
+// meets the E-folded (north + south) and F- the O-folded (north - south) ring coefficients, and vice versa for
+// l - m odd.  One pass over the Q and iU tiles of a stage feeds both outputs (item 12).
+//
+// Same warp-specialised structure as the spin-0 kernels: 8 DMMA consumer warps (CTA tile 128 x 128 real outputs), but
+// the four remaining warps all generate (lane = ring x sign of F), and lane 0 of the generator that owns a stage
+// also issues its TMA loads.
+#include "sht_legendre_common.cuh"
+
+namespace sht {
+
+constexpr int LEG2_THREADS = 384;
+constexpr int LEG_CONSUMER_WARPS_S2 = 8;
+constexpr int P_KT = 32;                        // (Q,U) pairs per k-tile: 32 pairs x (E,B) x (re,im) = 128 real columns
+constexpr int P_KG = P_KT / KG;                 // workspace map groups per k-tile
+constexpr int A2_ML = LEG_A_ML;                 // analysis: l rows per tile (64 of each parity class)
+constexpr int A2_PC = 16;                       // analysis: ring pairs per stage
+constexpr int A2_SL = 66;                       // F tile: stride (doubles) between rings, = 2 mod 8
+constexpr int A2_XBYTES = A2_PC * P_KG * 2 * 128;           // Q and iU lines of a stage: 32 KB
+constexpr int A2_LBYTES = 2 * 2 * A2_PC * A2_SL * 8;        // [sign][class][ring][l/2]
+constexpr int A2_STAGE_BYTES = A2_XBYTES + A2_LBYTES;
+static_assert(A2_STAGE_BYTES % 1024 == 0, "stages must keep the 1024-byte alignment of the swizzled TMA boxes");
+constexpr int S2_PB = 64;                       // synthesis: ring pairs per CTA
+constexpr int S2_LC = 32;                       // synthesis: l values per stage
+constexpr int S2_SL = 66;
+constexpr int S2_ABYTES = S2_LC * 2 * P_KT * 16;            // a_E, a_B of a stage: 32 KB
+constexpr int S2_LBYTES = 2 * S2_LC * S2_SL * 8;            // [sign][l][ring]
+constexpr int S2_STAGE_BYTES = S2_ABYTES + S2_LBYTES;
+static_assert(S2_STAGE_BYTES % 1024 == 0, "stages must keep the 1024-byte alignment of the swizzled TMA boxes");
+constexpr int S2_SC = 128 + 8;                  // epilogue staging row stride (doubles)
+
+// per-l constants of F+/F- for order m: tp = (t1, t2) = N_l (l - m^2, l(l-1)/2), tm = (t4, 0) = N_l (l-1, 0),
+// t3 = N_l c_lm; all zero for l < 2 (reading G13) and beyond lmax
+__device__ __forceinline__ void spin2_consts(const DevicePlan& d, int l, int m, double2& tp, double2& tm, double& t3)
+{
+    tp = make_double2(0.0, 0.0); tm = make_double2(0.0, 0.0); t3 = 0.0;
+    if (l >= 2 && l <= d.lmax) {
+        const double nl = __ldg(&d.spin2c[l].x);
+        const double L = (double)l, M = (double)m;
+        tp = make_double2(nl * (L - M * M), nl * (0.5 * L * (L - 1.0)));
+        tm = make_double2(nl * (L - 1.0), 0.0);
+        t3 = nl * sqrt((2.0 * L + 1.0) * (L - M) * (L + M) / (2.0 * L - 1.0));
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// analysis, spin 2: one CTA per (m, k-tile of 32 pairs); l tiles outer, ring chunks of 16 inner.
+// Stage: [X: comp(Q,iU) x 8 kg x 16 p x 128 B, 128B-swizzled] [F: sign(+,-) x class x 16 p x A2_SL]
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(LEG2_THREADS, 1)
+k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
+                          int nkt, int accumulate, int nst)
+{
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char* stage_base = smem_raw;
+    double2* state = reinterpret_cast<double2*>(smem_raw + (size_t)nst * A2_STAGE_BYTES);   // (lambda_{l-1}, lambda_{l-2}) per ring
+    uint64_t* full = reinterpret_cast<uint64_t*>(state + d.nh);
+    uint64_t* empty = full + 4;
+    double2* cft = reinterpret_cast<double2*>(empty + 4);        // (alpha, beta) of the current l tile
+    double2* ctu = cft + A2_ML;                                  // [sign][l]: (t1, t2) / (t4, 0)
+    double* ct3 = reinterpret_cast<double*>(ctu + 2 * A2_ML);
+    int* pst = reinterpret_cast<int*>(ct3 + A2_ML);
+
+    const int m = blockIdx.x / nkt, kt = blockIdx.x % nkt;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lmax = d.lmax, nh = d.nh;
+    const int ntile = (lmax - m) / A2_ML + 1;
+
+    for (int p = tid; p < nh; p += LEG2_THREADS) state[p] = d.seed[(size_t)m * nh + p];
+    for (int t = tid; t < ntile; t += LEG2_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
+    if (tid == 0) {
+        for (int s = 0; s < nst; ++s) { mbar_init(full + s, 1 + 32); mbar_init(empty + s, LEG_CONSUMER_WARPS_S2); }
+        fence_barrier_init();
+        tma_prefetch_desc(&tmF);
+    }
+    __syncthreads();
+
+    if (warp < 8) {
+        // ===== consumers: (A^E, iA^B)[l, pair] += F+[l, p] (Q, iU)^{X(cls)}[p, pair] + F-[l, p] (iU, Q)^{X(1-cls)}[p, pair]
+        const int cls = warp >> 2, wn = warp & 3;
+        const int g = lane >> 2, t = lane & 3;
+        double cE[8][2][2], cB[8][2][2];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) { cE[i][j][0] = cE[i][j][1] = 0.0; cB[i][j][0] = cB[i][j][1] = 0.0; }
+        int stage = 0; uint32_t phase = 0;
+        const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
+        for (int tile = 0; tile < ntile; ++tile) {
+            const int l0 = m + tile * A2_ML;
+            for (int pc = pst[tile]; pc < nh; pc += A2_PC) {
+                mbar_wait(full + stage, phase);
+                const double* Xs = reinterpret_cast<const double*>(stage_base + (size_t)stage * A2_STAGE_BYTES);
+                const double* Ls = Xs + A2_XBYTES / 8;
+#pragma unroll
+                for (int ks = 0; ks < A2_PC / 4; ++ks) {
+                    const int pl = 8 * (ks >> 1) + 2 * t + (ks & 1);          // ring inside the 16-ring box
+#pragma unroll
+                    for (int sg = 0; sg < 2; ++sg) {
+                        // sg = 0: F+ with the fold of this class; sg = 1: F- with the other fold and swapped components
+                        const int h = cls ^ sg;
+                        double a[8], bq[2], bu[2];
+                        const double* La = Ls + ((sg * 2 + cls) * A2_PC + pl) * A2_SL + g;
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
+                        const double* Xb = Xs + pl * 16 + ((((4 * h + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
+#pragma unroll
+                        for (int j = 0; j < 2; ++j) {
+                            bq[j] = Xb[(2 * wn + j) * 256];
+                            bu[j] = Xb[(P_KG + 2 * wn + j) * 256];
+                        }
+#pragma unroll
+                        for (int i = 0; i < 8; ++i)
+#pragma unroll
+                            for (int j = 0; j < 2; ++j) {
+                                dmma884(cE[i][j][0], cE[i][j][1], a[i], sg ? bu[j] : bq[j]);
+                                dmma884(cB[i][j][0], cB[i][j][1], a[i], sg ? bq[j] : bu[j]);
+                            }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + stage);
+                if (++stage == nst) { stage = 0; phase ^= 1; }
+            }
+            // ---- epilogue: a_E = A^E, a_B = -i (iA^B), scattered to the m-major alm layout
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int l = l0 + 2 * (8 * i + g) + cls;
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const int kk = kt * P_KT + (2 * wn + j) * KG + t;
+                    if (l <= lmax && kk < kmaps) {
+                        double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * 2) * d.nalm + moff + l;
+                        double2 ve = make_double2(cE[i][j][0], m == 0 ? 0.0 : cE[i][j][1]);
+                        double2 vb = make_double2(cB[i][j][1], m == 0 ? 0.0 : -cB[i][j][0]);
+                        if (accumulate) {
+                            const double2 oe = dst[0], ob = dst[d.nalm];
+                            ve.x += oe.x; ve.y += oe.y; vb.x += ob.x; vb.y += ob.y;
+                        }
+                        dst[0] = ve;
+                        dst[d.nalm] = vb;
+                    }
+                    cE[i][j][0] = cE[i][j][1] = 0.0; cB[i][j][0] = cB[i][j][1] = 0.0;
+                }
+            }
+        }
+    } else {
+        // ===== generators (warps 8 .. 8+nst-1): generator g owns stage g, i.e. the chunks c = g (mod nst) -- a warp that
+        // ran further ahead than the number of stages would defeat the parity waits; lane = (ring 0..15) + 16 (sign of F).
+        // Lane 0 also issues the TMA load of the chunk's Q / iU lines as soon as the stage is free.
+        const int gw = warp - 8;
+        if (gw >= nst) return;
+        const int ngen = nst * 32;
+        const int rr = lane & 15, sg = lane >> 4;
+        const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+        // per-l constants of the next tile: generators 0 and 1 fetch 64 l each while the current tile is computed
+        const int gl = gw * 64 + lane;
+        auto load_consts = [&](int l0, int j, double2& ab, double2& tp, double2& tm, double& t3) {
+            const int l = l0 + gl + 32 * j;
+            ab = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+            spin2_consts(d, l, m, tp, tm, t3);
+        };
+        double2 nab[2], ntp[2], ntm[2]; double nt3[2];
+        if (gw < 2) { load_consts(m, 0, nab[0], ntp[0], ntm[0], nt3[0]); load_consts(m, 1, nab[1], ntp[1], ntm[1], nt3[1]); }
+        int chunk = 0;
+        for (int tile = 0; tile < ntile; ++tile) {
+            const int l0 = m + tile * A2_ML;
+            named_bar_sync(1, ngen);                            // every generator is done with the previous tile
+            if (gw < 2) {
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const int i = gl + 32 * j;
+                    cft[i] = nab[j]; ctu[i] = ntp[j]; ctu[A2_ML + i] = ntm[j]; ct3[i] = nt3[j];
+                }
+            }
+            named_bar_sync(1, ngen);
+            if (gw < 2 && tile + 1 < ntile) {
+                load_consts(l0 + A2_ML, 0, nab[0], ntp[0], ntm[0], nt3[0]);
+                load_consts(l0 + A2_ML, 1, nab[1], ntp[1], ntm[1], nt3[1]);
+            }
+            for (int pc = pst[tile]; pc < nh; pc += A2_PC, ++chunk) {
+                const int stage = chunk % nst;
+                if (stage != gw) continue;
+                const uint32_t phase = (chunk / nst) & 1;
+                const int p = pc + rr;
+                double x1 = 0.0, x2 = 0.0, z = 0.0, is2 = 0.0;
+                int ls = lmax + 1;
+                if (p < nh) {
+                    const double2 sd = state[p];
+                    x1 = sd.x; x2 = sd.y; z = d.z[p]; is2 = 1.0 / d.sin2[p];
+                    ls = d.lstart[(size_t)m * nh + p];
+                }
+                const double ra = sg ? (double)m * z * is2 : is2;       // multiplies t1 (F+) / t4 (F-)
+                const double rc = sg ? (double)m * is2 : z * is2;       // multiplies t3
+                const int rs = ls - l0;
+                mbar_wait(empty + stage, phase ^ 1);
+                unsigned char* Xs = stage_base + (size_t)stage * A2_STAGE_BYTES;
+                if (lane == 0) {
+                    mbar_arrive_expect_tx(full + stage, A2_XBYTES);
+                    tma_load_4d(Xs, &tmF, full + stage, 0, pc, kt * P_KG, m * 2);
+                }
+                double* Ls = reinterpret_cast<double*>(Xs + A2_XBYTES) + (sg * 2 * A2_PC + rr) * A2_SL;
+                const double2* tu = ctu + sg * A2_ML;
+#pragma unroll 4
+                for (int r = 0; r < A2_ML; ++r) {
+                    const double2 ab = cft[r];
+                    const double2 uv = tu[r];
+                    const double t3 = ct3[r];
+                    const double lam = fma(ab.x * z, x1, -(ab.y * x2));
+                    const double U = fma(uv.x, ra, uv.y), W = t3 * rc;
+                    const double f = fma(lam, U, -(x1 * W));             // x1 = lambda_{l-1}
+                    const bool on = r >= rs;
+                    x2 = on ? x1 : x2; x1 = on ? lam : x1;
+                    Ls[(r & 1) * (A2_PC * A2_SL) + (r >> 1)] = on ? f : 0.0;
+                }
+                if (sg == 0 && p < nh) state[p] = make_double2(x1, x2);
+                mbar_arrive(full + stage);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// synthesis, spin 2: one CTA per (m, block of 64 ring pairs, k-tile of 32 pairs); loops over l chunks of 32.
+// Stage: [a_lm: 4 boxes (8 l each) x comp(E,B) x 32 pairs x 128 B, 128B-swizzled] [F: sign x 32 l x S2_SL]
+// With Qe = sum_{l-m even} F+ A^E + sum_{l-m odd} F- iA^B (even under the fold) and Qo the complementary sums,
+// Q(north) = Qe + Qo, Q(south) = Qe - Qo; iU likewise with A^E and iA^B exchanged.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(LEG2_THREADS, 1)
+k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
+                           int nkt, int npb)
+{
+    constexpr int NST = 3;
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char* stage_base = smem_raw;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + NST * S2_STAGE_BYTES);
+    uint64_t* empty = full + 4;
+    double2* cfs = reinterpret_cast<double2*>(empty + 4);       // 4 generator warps x 2 buffers x S2_LC x (ab, uv, t3)
+    int* lmin_s = reinterpret_cast<int*>(cfs + 4 * 2 * S2_LC * 3);
+
+    const int kt = blockIdx.x % nkt;
+    const int pbi = (blockIdx.x / nkt) % npb;
+    const int m = blockIdx.x / (nkt * npb);
+    const int pb = pbi * S2_PB;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int lmax = d.lmax, nh = d.nh;
+    const int plast = min(pb + S2_PB, nh) - 1;
+    if (m >= d.mlim[plast]) return;                    // no ring of this block takes part in order m (never read)
+
+    if (tid == 0) {
+        for (int s = 0; s < NST; ++s) { mbar_init(full + s, 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS_S2); }
+        fence_barrier_init();
+        tma_prefetch_desc(&tmA);
+        *lmin_s = lmax + 1;
+    }
+    __syncthreads();
+    if (tid < S2_PB && pb + tid < nh) atomicMin(lmin_s, d.lstart[(size_t)m * nh + pb + tid]);
+    __syncthreads();
+    const int lmin = *lmin_s;
+    const int cfirst = (lmin > lmax) ? (lmax + 1) : m + ((lmin - m) / S2_LC) * S2_LC;
+    const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
+
+    if (warp < 8) {
+        // ===== consumers: warp (par, wn): rows = 64 rings of the even (par 0) / odd (par 1) fold part, 8 pairs =====
+        const int par = warp >> 2, wn = warp & 3;
+        const int g = lane >> 2, t = lane & 3;
+        double cQ[8][2][2], cU[8][2][2];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) { cQ[i][j][0] = cQ[i][j][1] = 0.0; cU[i][j][0] = cU[i][j][1] = 0.0; }
+        int stage = 0; uint32_t phase = 0;
+        const int im = g & 1;
+        const bool zero_e = (m == 0) && im;               // Im(a_l0) is ignored
+        const bool zero_b = (m == 0) && !im;
+        // per-lane offsets (doubles): F rows of the 4 l of a step with sign sg, a_lm element of pair j for sign sg
+        const int la0 = (2 * t + par) * S2_SL + g;                             // sg = 0: class = par
+        const int la1 = (S2_LC + 2 * t + (par ^ 1)) * S2_SL + g;               // sg = 1: class = 1 - par
+        const int c0 = par, c1 = par ^ 1;
+        int ab0[2], ab1[2];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int pr = 8 * wn + 4 * j + (g >> 1);                          // pair inside the k-tile
+            ab0[j] = pr * 16 + (((2 * t + par) ^ (pr & 7)) << 1);
+            ab1[j] = pr * 16 + (((2 * t + (par ^ 1)) ^ (pr & 7)) << 1);
+        }
+        for (int lc = cfirst; lc <= lmax; lc += S2_LC) {
+            mbar_wait(full + stage, phase);
+            const double* As = reinterpret_cast<const double*>(stage_base + (size_t)stage * S2_STAGE_BYTES);
+            const double* Ls = As + S2_ABYTES / 8;
+            const int lrow = lc + 2 * t - 2;                // (l - 2) of this lane's first row of box 0, without the class bit
+#pragma unroll
+            for (int ks = 0; ks < S2_LC / 4; ++ks) {
+                // box q of 8 l; sg = 0: the 4 l whose class matches this warp's fold part (F+), sg = 1: the others (F-)
+                const int q = ks >> 1, sg = ks & 1;
+                double a[8], be[2], bb[2];
+                const double* La = Ls + (sg ? la1 : la0) + 8 * q * S2_SL;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
+                // rows outside 2 <= l <= lmax are not this order's input: l < 2 is ignored (reading G13) and the tail of
+                // the last chunk holds the next order's first entries (its ignored l < 2 slots among them)
+                const bool dead = (unsigned)(lrow + 8 * q + (sg ? c1 : c0)) > (unsigned)(lmax - 2);
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const double* Ab = As + q * 1024 + (sg ? ab1[j] : ab0[j]);
+                    const double e = Ab[im];                    // A^E: (re, im) of a_E
+                    const double b = Ab[P_KT * 16 + (im ^ 1)];  // iA^B = (-Im a_B, Re a_B)
+                    be[j] = (dead || zero_e) ? 0.0 : e;
+                    bb[j] = (dead || zero_b) ? 0.0 : (im ? b : -b);
+                }
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        dmma884(cQ[i][j][0], cQ[i][j][1], a[i], sg ? bb[j] : be[j]);
+                        dmma884(cU[i][j][0], cU[i][j][1], a[i], sg ? be[j] : bb[j]);
+                    }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + stage);
+            if (++stage == NST) { stage = 0; phase ^= 1; }
+        }
+        // ---- epilogue: exchange the even / odd fold parts through smem, write north = e + o, south = e - o lines
+        named_bar_sync(2, 256);                           // every consumer is done with the stage memory
+        double* Cs = reinterpret_cast<double*>(smem_raw);
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int row = par * S2_PB + 8 * i + g;
+                const int col = 2 * (8 * wn + 4 * j + t);                       // (pair, re/im) of component Q
+                *reinterpret_cast<double2*>(&Cs[row * S2_SC + col]) = make_double2(cQ[i][j][0], cQ[i][j][1]);
+                *reinterpret_cast<double2*>(&Cs[row * S2_SC + 2 * P_KT + col]) = make_double2(cU[i][j][0], cU[i][j][1]);
+            }
+        named_bar_sync(2, 256);
+        double2* Fc = reinterpret_cast<double2*>(F);
+        for (int e = tid; e < S2_PB * 2 * P_KT; e += 256) {
+            const int pr = e % P_KT, comp = (e / P_KT) & 1, r = e / (2 * P_KT);
+            const int p = pb + r;
+            if (p >= nh) continue;
+            const double2 ev = *reinterpret_cast<const double2*>(&Cs[r * S2_SC + comp * 2 * P_KT + 2 * pr]);
+            const double2 od = *reinterpret_cast<const double2*>(&Cs[(S2_PB + r) * S2_SC + comp * 2 * P_KT + 2 * pr]);
+            const int k = kt * P_KT + pr;
+            double2* dst = Fc + f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
+            dst[0] = make_double2(ev.x + od.x, ev.y + od.y);
+            dst[KG] = make_double2(ev.x - od.x, ev.y - od.y);
+        }
+    } else {
+        // ===== generators (warps 8..11): warp = (sign of F) x (half of the 64 rings), recurrence state in registers;
+        // lane 0 of generator 0 issues the TMA loads of a_E / a_B for the stage
+        const int gw = warp - 8;
+        const int sg = gw >> 1;
+        const int rl = (gw & 1) * 32 + lane;
+        const int p = pb + rl;
+        double x1 = 0.0, x2 = 0.0, z = 0.0, is2 = 0.0;
+        int ls = lmax + 1;
+        if (p < nh) {
+            const double2 sd = d.seed[(size_t)m * nh + p];
+            x1 = sd.x; x2 = sd.y; ls = d.lstart[(size_t)m * nh + p]; z = d.z[p]; is2 = 1.0 / d.sin2[p];
+        }
+        const double ra = sg ? (double)m * z * is2 : is2;
+        const double rc = sg ? (double)m * is2 : z * is2;
+        const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+        double2* cfw = cfs + gw * (2 * S2_LC * 3);
+        double2 nab, nuv; double nt3;
+        auto load_consts = [&](int lc) {
+            const int l = lc + lane;
+            nab = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+            double2 tp, tm;
+            spin2_consts(d, l, m, tp, tm, nt3);
+            nuv = sg ? tm : tp;
+        };
+        load_consts(cfirst);
+        int stage = 0, buf = 0; uint32_t phase = 0;
+        const int row0 = k0 + kt * P_KT;
+        for (int lc = cfirst; lc <= lmax; lc += S2_LC) {
+            double2* cb = cfw + buf * (S2_LC * 3);
+            cb[lane] = nab; cb[S2_LC + lane] = nuv; cb[2 * S2_LC + lane] = make_double2(nt3, 0.0);
+            __syncwarp();
+            load_consts(lc + S2_LC);
+            const int rs = ls - lc;
+            mbar_wait(empty + stage, phase ^ 1);
+            unsigned char* As = stage_base + (size_t)stage * S2_STAGE_BYTES;
+            if (gw == 0 && lane == 0) {
+                mbar_arrive_expect_tx(full + stage, S2_ABYTES);
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    tma_load_3d(As + q * (S2_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0, 0);
+            }
+            double* Ls = reinterpret_cast<double*>(As + S2_ABYTES) + sg * S2_LC * S2_SL + rl;
+#pragma unroll 4
+            for (int r = 0; r < S2_LC; ++r) {
+                const double2 ab = cb[r];
+                const double2 uv = cb[S2_LC + r];
+                const double t3 = cb[2 * S2_LC + r].x;
+                const double lam = fma(ab.x * z, x1, -(ab.y * x2));
+                const double U = fma(uv.x, ra, uv.y), W = t3 * rc;
+                const double f = fma(lam, U, -(x1 * W));
+                const bool on = r >= rs;
+                x2 = on ? x1 : x2; x1 = on ? lam : x1;
+                Ls[r * S2_SL] = on ? f : 0.0;
+            }
+            mbar_arrive(full + stage);
+            buf ^= 1;
+            if (++stage == NST) { stage = 0; phase ^= 1; }
+        }
+    }
+}
+
+// ---- host side -------------------------------------------------------------------------------------------
+// alm[pair][comp][nalm*2 doubles] as a 3-D tensor (innermost first: doubles of one (pair, comp) row, pair, comp);
+// box = 8 l (128 bytes) x 32 pairs x (E, B): lands in shared memory as [comp][pair][128 B]
+static cudaError_t make_tmap_alm_spin2(const DevicePlan& d, const double* alm, long long pairs, CUtensorMap* tm)
+{
+    const cuuint64_t dims[3] = {(cuuint64_t)d.nalm * 2, (cuuint64_t)pairs, 2};
+    const cuuint64_t strides[2] = {(cuuint64_t)d.nalm * 32, (cuuint64_t)d.nalm * 16};
+    const cuuint32_t box[3] = {16, P_KT, 2};
+    return make_tmap_f64(tm, alm, 3, dims, strides, box);
+}
+
+static size_t analysis2_smem(int nh, int ntile, int nst)
+{
+    return (size_t)nst * A2_STAGE_BYTES + (size_t)nh * sizeof(double2) + 8 * sizeof(uint64_t) +
+           (size_t)A2_ML * (3 * sizeof(double2) + sizeof(double)) + (size_t)ntile * sizeof(int);
+}
+static size_t synthesis2_smem()
+{
+    return (size_t)3 * S2_STAGE_BYTES + 8 * sizeof(uint64_t) + (size_t)4 * 2 * S2_LC * 3 * sizeof(double2) + 16;
+}
+
+cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
+                                           bool accumulate, cudaStream_t st)
+{
+    int nst = 3;
+    if (analysis2_smem(d.nh, d.ntile_max, nst) > (size_t)227 * 1024) nst = 2;
+    const size_t sm = analysis2_smem(d.nh, d.ntile_max, nst);
+    if (sm > (size_t)227 * 1024) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis_spin2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    CUtensorMap tmF;
+    if ((e = make_tmap_F(d, F, P_KG, 2, &tmF)) != cudaSuccess) return e;
+    const int nkt = (kmaps + P_KT - 1) / P_KT;
+    k_legendre_analysis_spin2<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, nst);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps,
+                                            cudaStream_t st)
+{
+    const size_t sm = synthesis2_smem();
+    cudaError_t e = cudaFuncSetAttribute(k_legendre_synthesis_spin2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    CUtensorMap tmA;
+    if ((e = make_tmap_alm_spin2(d, alm, (long long)(k0 + kmaps), &tmA)) != cudaSuccess) return e;
+    const int nkt = (kmaps + P_KT - 1) / P_KT;
+    const int npb = (d.nh + S2_PB - 1) / S2_PB;
+    k_legendre_synthesis_spin2<<<(d.lmax + 1) * nkt * npb, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace sht

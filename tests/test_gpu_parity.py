@@ -60,6 +60,45 @@ def test_spin0_small_full(nside, lmax, nmaps):
     plan.destroy()
 
 
+@pytest.mark.parametrize("nside,lmax,nmaps", [
+    (1, 2, 1), (2, 5, 3), (3, 8, 5), (4, 11, 33), (8, 23, 40), (16, 47, 8), (16, 30, 4), (16, 63, 2), (32, 95, 70),
+    (48, 143, 3), (64, 300, 2),
+])
+def test_spin2_small_full(nside, lmax, nmaps):
+    """spin 2, both directions, every output element (Q,U <-> E,B); ragged pair counts, odd nside, lmax above 3 nside - 1"""
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan
+    alm = inputs.gaussian_alm(lmax, np.arange(nmaps), seed=200 + nside, spin=2)
+    plan = Plan(nside, lmax, nmaps, 2)
+    ref_maps = O.synthesis(nside, lmax, alm, spin=2)
+    got_maps = _gpu_synthesis(plan, alm)
+    assert inputs.rel_err(got_maps, ref_maps) <= TOL
+    noisy = ref_maps + inputs.white_noise(nside, np.arange(nmaps), 9, 1e-3, spin=2)
+    ref_alm = O.analysis(nside, lmax, noisy, spin=2)
+    got_alm = _gpu_analysis(plan, noisy)
+    assert inputs.rel_err(got_alm, ref_alm) <= TOL
+    ls, ms = inputs.ell_of_index(lmax)
+    assert np.all(got_alm[:, :, ms == 0].imag == 0.0)
+    assert np.all(got_alm[:, :, ls < 2] == 0.0)
+    plan.destroy()
+
+
+def test_spin2_ignores_low_l_and_im_m0_on_input():
+    """l < 2 and Im(a_l0) are ignored on input (readings G13, section 1), even if they hold NaN"""
+    from paper_2208_10154_b200.binding import Plan
+    nside, lmax, nmaps = 8, 23, 5
+    alm = inputs.gaussian_alm(lmax, np.arange(nmaps), seed=31, spin=2)
+    plan = Plan(nside, lmax, nmaps, 2)
+    base = _gpu_synthesis(plan, alm)
+    ls, ms = inputs.ell_of_index(lmax)
+    dirty = alm.copy()
+    dirty[:, :, ls < 2] = np.nan
+    dirty[:, :, ms == 0] = dirty[:, :, ms == 0].real + 1j * 5.0
+    dirty[:, :, ls < 2] = np.nan
+    assert np.array_equal(_gpu_synthesis(plan, dirty), base)
+    plan.destroy()
+
+
 def test_config1():
     """BASELINE.json configs[0]: nside 16, lmax 47, 8 maps: synthesise, analyse back, compare both."""
     from oracle import oracle as O
