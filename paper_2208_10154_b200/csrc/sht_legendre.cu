@@ -45,12 +45,15 @@ static_assert(2 * S_PB * S_SC * 8 <= S_STAGES * S_STAGE_BYTES, "epilogue staging
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
-                    int nkt, int accumulate)
+                    int nkt, int accumulate, double2* __restrict__ gstate)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
-    double2* state = reinterpret_cast<double2*>(smem_raw + A_STAGES * A_STAGE_BYTES);      // (lambda_{l-1}, lambda_{l-2}) per ring
-    uint64_t* full = reinterpret_cast<uint64_t*>(state + d.nh);
+    // (lambda_{l-1}, lambda_{l-2}) per ring, carried from one l tile to the next: in shared memory, or (when 2 nside
+    // ring pairs x 16 B do not fit beside the stages, nside >= 1024) in a per-CTA global scratch row
+    double2* smem_state = reinterpret_cast<double2*>(smem_raw + A_STAGES * A_STAGE_BYTES);
+    double2* state = gstate ? gstate + (size_t)blockIdx.x * d.nh : smem_state;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_state + (gstate ? 0 : d.nh));
     uint64_t* empty = full + A_STAGES;
     double2* cft = reinterpret_cast<double2*>(empty + A_STAGES);                           // (alpha, beta) of the current l tile
     int* pst = reinterpret_cast<int*>(cft + A_ML);                                         // first ring of every l tile
@@ -361,9 +364,9 @@ static cudaError_t make_tmap_alm(const DevicePlan& d, const double* alm, long lo
     return make_tmap_f64(tm, alm, 2, dims, strides, box);
 }
 
-static size_t analysis_smem(int nh, int ntile)
+static size_t analysis_smem(int nh, int ntile, bool state_in_smem = true)
 {
-    return (size_t)A_STAGES * A_STAGE_BYTES + (size_t)nh * sizeof(double2) + 2 * A_STAGES * sizeof(uint64_t) +
+    return (size_t)A_STAGES * A_STAGE_BYTES + (state_in_smem ? (size_t)nh * sizeof(double2) : 0) + 2 * A_STAGES * sizeof(uint64_t) +
            (size_t)A_ML * sizeof(double2) + (size_t)ntile * sizeof(int);
 }
 static size_t synthesis_smem() { return (size_t)S_STAGES * S_STAGE_BYTES + 2 * S_STAGES * sizeof(uint64_t) + 4 * S_LC * sizeof(double2) + 16; }
@@ -378,15 +381,25 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
                                      bool accumulate, cudaStream_t st)
 {
     if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st);
-    const size_t sm = analysis_smem(d.nh, d.ntile_max);
-    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (e != cudaSuccess) return e;
-    CUtensorMap tmF;
-    if ((e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, &tmF)) != cudaSuccess) return e;
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
-    k_legendre_analysis<<<(d.lmax + 1) * nkt, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
-    pl->launches++;
-    return cudaGetLastError();
+    const unsigned grid = (unsigned)((d.lmax + 1) * nkt);
+    size_t sm = analysis_smem(d.nh, d.ntile_max);
+    double2* gstate = nullptr;
+    cudaError_t e;
+    if (sm > (size_t)227 * 1024) {
+        sm = analysis_smem(d.nh, d.ntile_max, false);
+        if ((e = cudaMallocAsync((void**)&gstate, (size_t)grid * d.nh * sizeof(double2), st)) != cudaSuccess) return e;
+    }
+    e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    CUtensorMap tmF;
+    if (e == cudaSuccess) e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, &tmF);
+    if (e == cudaSuccess) {
+        k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, gstate);
+        pl->launches++;
+        e = cudaGetLastError();
+    }
+    if (gstate) cudaFreeAsync(gstate, st);
+    return e;
 }
 
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st)
