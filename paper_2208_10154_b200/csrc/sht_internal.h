@@ -14,8 +14,9 @@ constexpr int KTILE_MAPS = 64;               // maps per Legendre k-tile (spin 0
 constexpr int NK = 2 * KTILE_MAPS;           // real columns per k-tile (re,im interleaved)
 constexpr int LEG_A_ML = 128;                // l rows per tile of the Legendre analysis kernel
 constexpr int MAX_RADIX_LIST = 16;           // factors of one ring length
-constexpr int RING_THREADS = 512;            // threads per CTA of the ring kernels
-constexpr int RING_EMAX = 8192;              // complex elements (ring length x maps) one ring CTA holds in smem
+constexpr int RING_THREADS = 256;            // threads per CTA of the ring kernels (two CTAs per SM)
+constexpr int RING_EMAX = 8192;              // most complex elements (ring length x maps) one ring CTA holds in smem
+constexpr int RING_ETARGET = 4096;           // preferred element count: 64 KB + padding, two or three CTAs per SM
 constexpr int RING_EMAX_OOP = 6400;          // same for rings that need an out-of-place pass (two buffers)
 constexpr int BLUESTEIN_MIN_PRIME = 37;      // smallest prime factor of a ring length that switches to Bluestein
 constexpr int RING_NCLASS = 4;               // launch classes of the ring kernels (by dynamic smem size)
@@ -40,6 +41,8 @@ struct RingPair {
     int b_tw_off;          // offset (double2) of W_{2 lc}[j] = exp(-i pi j / lc)
     int b_fac_off, b_nfac; // radix list of the length-lc transform (4s and a 2)
     int hf_off;            // offset (double2) of FFT_lc(conj chirp) / lc in forward-output position order
+    int psh;               // shared-memory padding: one element every 2^psh (power-of-two transforms), 31 = none
+    int nbuf;              // elements per map of one transform buffer, padding included
 };
 
 struct DevicePlan {

@@ -149,11 +149,40 @@ static void host_fft_pow2(std::vector<long double>& re, std::vector<long double>
     }
 }
 
-// maps per CTA of the ring kernels: the largest power of two <= 16 whose rings fit the CTA's element budget
-static int ring_kt(int n, int cap)
+// Kernel-side radix list: the power-of-two run of `f` (4s and at most one 2) is regrouped into register-fused
+// passes, code 16 = two radix-4 stages, code 8 = a radix-4 and a radix-2 stage (grouped from the back, so that the
+// last pass is the widest); other factors are copied.  The output order of the transform is unchanged, so the
+// digit-reversal table is built from the plain list.
+static void group_radices(const std::vector<int>& f, std::vector<int>& g)
+{
+    size_t i = 0;
+    while (i < f.size()) {
+        if (f[i] != 4 && f[i] != 2) { g.push_back(f[i]); ++i; continue; }
+        int c4 = 0;
+        while (i < f.size() && f[i] == 4) { ++c4; ++i; }
+        const bool has2 = i < f.size() && f[i] == 2;
+        if (has2) ++i;
+        int pairable = c4 - ((has2 && c4 > 0) ? 1 : 0);
+        if (pairable & 1) { g.push_back(4); --pairable; }
+        for (int q = 0; q < pairable / 2; ++q) g.push_back(16);
+        if (has2) g.push_back(c4 > 0 ? 8 : 2);
+    }
+}
+
+// shared-memory padding shift of a pure power-of-two transform whose last pass is a fused 16 / 8 (31 = no padding)
+static int pad_shift(const std::vector<int>& g, bool pure_pow2)
+{
+    if (!pure_pow2 || g.empty()) return 31;
+    return g.back() == 16 ? 4 : g.back() == 8 ? 3 : 31;
+}
+
+// maps per CTA of the ring kernels: the largest power of two <= 16 whose buffers stay within 72 KB (two or three
+// CTAs per SM); at least 2 maps (whole 32-byte sectors of the workspace lines) if that still fits one CTA per SM
+static int ring_kt(size_t bytes_per_map)
 {
     int kt = 1;
-    while (kt * 2 <= 16 && kt * 2 * n <= cap) kt *= 2;
+    while (kt * 2 <= 16 && (size_t)(kt * 2) * bytes_per_map <= (size_t)72 * 1024) kt *= 2;
+    if (kt < 2 && 2 * bytes_per_map <= (size_t)224 * 1024) kt = 2;
     return kt;
 }
 
@@ -192,6 +221,8 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
     std::vector<int> perm_off_of_q(nside + 1, 0), lc_of_q(nside + 1, 0), hf_off_of_q(nside + 1, 0);
     std::map<int, int> pow2_tw_off, pow2_fac_off, pow2_nfac;
     std::vector<int> tw_off_of_q(nside + 1, -1), fac_off_of_q(nside + 1, -1), nfac_of_q(nside + 1, 0), nbig_of_q(nside + 1, 0);
+    std::vector<int> psh_of_q(nside + 1, 31);
+    std::map<int, int> pow2_psh;
     for (int q = 1; q <= nside; ++q) {
         const int n = 4 * q;
         tw_off_of_q[q] = (int)tw.size();
@@ -202,9 +233,14 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
         std::vector<int> f;
         nbig_of_q[q] = factorize_ring(n, f);
         if ((int)f.size() > MAX_RADIX_LIST) { free(pl); return SHT_ERR_UNSUPPORTED; }
-        fac_off_of_q[q] = (int)radix.size();
-        nfac_of_q[q] = (int)f.size();
-        for (int v : f) radix.push_back(v);
+        {
+            std::vector<int> g;
+            group_radices(f, g);
+            fac_off_of_q[q] = (int)radix.size();
+            nfac_of_q[q] = (int)g.size();
+            for (int v : g) radix.push_back(v);
+            psh_of_q[q] = pad_shift(g, (n & (n - 1)) == 0);
+        }
         int maxp = 1;
         for (int v : f) maxp = v > maxp ? v : maxp;
         int lc = 0;
@@ -221,11 +257,15 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
                     long double ang = PI_LD * (long double)j / (long double)lc;
                     tw.push_back(make_double2((double)cosl(ang), (double)-sinl(ang)));
                 }
+                std::vector<int> pf, pg;
+                int r = lc;
+                while (r % 4 == 0) { pf.push_back(4); r /= 4; }
+                if (r == 2) pf.push_back(2);
+                group_radices(pf, pg);
                 pow2_fac_off[lc] = (int)radix.size();
-                int r = lc, cnt = 0;
-                while (r % 4 == 0) { radix.push_back(4); r /= 4; ++cnt; }
-                if (r == 2) { radix.push_back(2); ++cnt; }
-                pow2_nfac[lc] = cnt;
+                for (int v : pg) radix.push_back(v);
+                pow2_nfac[lc] = (int)pg.size();
+                pow2_psh[lc] = pad_shift(pg, true);
             }
             // filter h_j = conj(c_j) = exp(+i pi j^2 / n) at j = -(n-1) .. n-1 (mod lc); Hf = FFT_lc(h) / lc
             std::vector<long double> hr(lc, 0.0L), hi(lc, 0.0L);
@@ -237,11 +277,12 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
             }
             host_fft_pow2(hr, hi);
             hf_off_of_q[q] = (int)tw.size();
-            const int fo = pow2_fac_off[lc], nf = pow2_nfac[lc];
+            std::vector<int> lf;
+            for (int r = lc; r > 1;) { const int v = (r % 4 == 0) ? 4 : 2; lf.push_back(v); r /= v; }
             std::vector<double2> hf(lc);
             for (int k = 0; k < lc; ++k) {
                 int kk = k, pos = 0, M = lc;
-                for (int i2 = 0; i2 < nf; ++i2) { const int v = radix[fo + i2]; const int sdig = kk % v; kk /= v; M /= v; pos += sdig * M; }
+                for (int v : lf) { const int sdig = kk % v; kk /= v; M /= v; pos += sdig * M; }
                 hf[pos] = make_double2((double)(hr[k] / lc), (double)(hi[k] / lc));
             }
             tw.insert(tw.end(), hf.begin(), hf.end());
@@ -283,11 +324,14 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
             r.b_tw_off = pow2_tw_off[r.lc]; r.b_fac_off = pow2_fac_off[r.lc]; r.b_nfac = pow2_nfac[r.lc];
             r.hf_off = hf_off_of_q[q];
             r.oop = 0;
-            r.kt = ring_kt(r.lc, RING_EMAX);
+            r.psh = pow2_psh[r.lc];
+            r.nbuf = r.lc + (r.lc >> r.psh);
         } else {
             r.oop = nbig_of_q[q] >= 2 ? 1 : 0;
-            r.kt = ring_kt(r.n, r.oop ? RING_EMAX_OOP : RING_EMAX);
+            r.psh = psh_of_q[q];
+            r.nbuf = r.n + (r.n >> r.psh);
         }
+        r.kt = ring_kt((size_t)r.nbuf * sizeof(double2) * (r.oop ? 2 : 1));
         r.mlim = lmax + 1;                               // tightened below from the l_safe table
         zs[p] = (double)absz; sin2s[p] = (double)s2;
     }
@@ -386,11 +430,11 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
 
     // ---- ring-kernel launch classes (by dynamic shared memory per CTA) --------------------------
     {
-        const size_t lim[RING_NCLASS] = {72 * 1024, 110 * 1024, 128 * 1024, 224 * 1024};
+        const size_t lim[RING_NCLASS] = {72 * 1024, 113 * 1024, 160 * 1024, 224 * 1024};
         std::vector<int> lists[RING_NCLASS];
         for (int c = 0; c < RING_NCLASS; ++c) { pl->class_smem[c] = 0; pl->class_ktmin[c] = 16; }
         for (int p = 0; p < d.nh; ++p) {
-            const size_t b = (size_t)(rings[p].lc ? rings[p].lc : rings[p].n) * rings[p].kt * sizeof(double2) * (rings[p].oop ? 2 : 1);
+            const size_t b = (size_t)rings[p].nbuf * rings[p].kt * sizeof(double2) * (rings[p].oop ? 2 : 1);
             int c = 0;
             while (c < RING_NCLASS && b > lim[c]) ++c;
             if (c == RING_NCLASS) { sht_plan_destroy(pl); return SHT_ERR_UNSUPPORTED; }

@@ -26,7 +26,40 @@
 
 namespace sht {
 
-constexpr int NT = RING_THREADS;
+constexpr int NT = 2 * RING_THREADS;             // launch bound; CTAs run RING_THREADS threads (two per SM) or twice that
+
+// Shared-memory position of element e of map kk: maps fastest, and for power-of-two transforms one element of padding
+// every 2^psh elements, so that the last (stride 8 or 16) register pass is free of bank conflicts (psh = 31: none).
+struct Lay {
+    int ktsh, psh;
+    __device__ __forceinline__ int operator()(int e, int kk) const { return ((e + (e >> psh)) << ktsh) + kk; }
+};
+
+// exp(-2 pi i k / 16)
+__host__ __device__ constexpr double w16_cos(int k)
+{
+    return (k & 15) == 0 ? 1.0 : (k & 15) == 1 ? 0.92387953251128675613 : (k & 15) == 2 ? 0.70710678118654752440
+         : (k & 15) == 3 ? 0.38268343236508977173 : (k & 15) == 4 ? 0.0 : (k & 15) == 5 ? -0.38268343236508977173
+         : (k & 15) == 6 ? -0.70710678118654752440 : (k & 15) == 7 ? -0.92387953251128675613 : (k & 15) == 8 ? -1.0
+         : (k & 15) == 9 ? -0.92387953251128675613 : (k & 15) == 10 ? -0.70710678118654752440
+         : (k & 15) == 11 ? -0.38268343236508977173 : (k & 15) == 12 ? 0.0 : (k & 15) == 13 ? 0.38268343236508977173
+         : (k & 15) == 14 ? 0.70710678118654752440 : 0.92387953251128675613;
+}
+__host__ __device__ constexpr double w16_sin(int k) { return w16_cos(k + 4); }     // -sin(2 pi k/16) = cos(2 pi (k+4)/16)
+// multiply by exp(-+ 2 pi i k / 16) (k compile-time), - forward, + if INV
+template <int K, bool INV>
+__device__ __forceinline__ double2 mul_w16(double2 a)
+{
+    constexpr int k = K & 15;
+    if constexpr (k == 0) return a;
+    else if constexpr (k == 4) return INV ? make_double2(-a.y, a.x) : make_double2(a.y, -a.x);
+    else if constexpr (k == 8) return make_double2(-a.x, -a.y);
+    else if constexpr (k == 12) return INV ? make_double2(a.y, -a.x) : make_double2(-a.y, a.x);
+    else {
+        constexpr double c = w16_cos(k), sn = INV ? -w16_sin(k) : w16_sin(k);      // w = c + i sn
+        return make_double2(fma(a.x, c, -(a.y * sn)), fma(a.x, sn, a.y * c));
+    }
+}
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b)
 {
@@ -106,23 +139,120 @@ __device__ __forceinline__ void bfly(double2 (&u)[R])
 // Stage with sub-length L and radix R, M = L / R: for each block base (multiple of L) and j < M the elements
 // base + j + r M are replaced by W_L^{j s} sum_r x_r W_R^{r s}.  GIN: first stage (L = N), reads the maps.
 template <int R, bool GIN, class LD>
-__device__ __forceinline__ void dif_stage(double2* buf, int N, int L, int kt, int ktsh, const double2* __restrict__ tw2, LD ld)
+__device__ __forceinline__ void dif_stage(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, LD ld)
 {
-    const int M = L / R, nw = (N / R) << ktsh, tstep = N / L;
-    for (int w = threadIdx.x; w < nw; w += NT) {
-        const int kk = w & (kt - 1), bf = w >> ktsh;
+    const int M = L / R, nw = (N / R) << lay.ktsh, tstep = N / L;
+    for (int w = threadIdx.x; w < nw; w += blockDim.x) {
+        const int kk = w & (kt - 1), bf = w >> lay.ktsh;
         const int blk = bf / M, j = bf - blk * M;
         const int e0 = blk * L + j;
         double2 u[R];
 #pragma unroll
-        for (int r = 0; r < R; ++r) u[r] = GIN ? ld(e0 + r * M, kk) : buf[((e0 + r * M) << ktsh) + kk];
+        for (int r = 0; r < R; ++r) u[r] = GIN ? ld(e0 + r * M, kk) : buf[lay(e0 + r * M, kk)];
         bfly<R, false>(u);
         if (M > 1) {
 #pragma unroll
             for (int s = 1; s < R; ++s) u[s] = cmul(u[s], twiddle<false>(tw2, j * s * tstep));
         }
 #pragma unroll
-        for (int s = 0; s < R; ++s) buf[((e0 + s * M) << ktsh) + kk] = u[s];
+        for (int s = 0; s < R; ++s) buf[lay(e0 + s * M, kk)] = u[s];
+    }
+    __syncthreads();
+}
+
+// Two consecutive radix-4 stages (sub-lengths L and L/4) on the 16 elements base + j + c L/16 held in registers:
+// identical arithmetic and output order to dif_stage<4> twice, one shared-memory round trip instead of two.
+template <bool GIN, class LD>
+__device__ __forceinline__ void dif_stage16(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, LD ld)
+{
+    const int M = L >> 4, nw = (N >> 4) << lay.ktsh, tstep = N / L;
+    for (int w = threadIdx.x; w < nw; w += blockDim.x) {
+        const int kk = w & (kt - 1), bf = w >> lay.ktsh;
+        const int blk = bf / M, j = bf - blk * M;
+        const int e0 = blk * L + j;
+        double2 u[16];
+#pragma unroll
+        for (int c = 0; c < 16; ++c) u[c] = GIN ? ld(e0 + c * M, kk) : buf[lay(e0 + c * M, kk)];
+        double2 ta[4], tb[4];
+        if (M > 1) {
+#pragma unroll
+            for (int s = 1; s < 4; ++s) ta[s] = twiddle<false>(tw2, j * s * tstep);
+        }
+        // stage A: radix 4 over the elements a + 4 r; twiddle W_L^{(j + a M) s} = W_L^{j s} W_16^{a s}
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            double2 v[4] = {u[a], u[a + 4], u[a + 8], u[a + 12]};
+            bfly<4, false>(v);
+            v[1] = a == 0 ? v[1] : a == 1 ? mul_w16<1, false>(v[1]) : a == 2 ? mul_w16<2, false>(v[1]) : mul_w16<3, false>(v[1]);
+            v[2] = a == 0 ? v[2] : a == 1 ? mul_w16<2, false>(v[2]) : a == 2 ? mul_w16<4, false>(v[2]) : mul_w16<6, false>(v[2]);
+            v[3] = a == 0 ? v[3] : a == 1 ? mul_w16<3, false>(v[3]) : a == 2 ? mul_w16<6, false>(v[3]) : mul_w16<9, false>(v[3]);
+            if (M > 1) {
+#pragma unroll
+                for (int s = 1; s < 4; ++s) v[s] = cmul(v[s], ta[s]);
+            }
+#pragma unroll
+            for (int s = 0; s < 4; ++s) u[a + 4 * s] = v[s];
+        }
+        // stage B: radix 4 inside each quarter s (elements 4 s + r'); twiddle W_{L/4}^{j s'}
+        if (M > 1) {
+#pragma unroll
+            for (int s = 1; s < 4; ++s) tb[s] = twiddle<false>(tw2, 4 * j * s * tstep);
+        }
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            double2 v[4] = {u[4 * s], u[4 * s + 1], u[4 * s + 2], u[4 * s + 3]};
+            bfly<4, false>(v);
+            if (M > 1) {
+#pragma unroll
+                for (int q = 1; q < 4; ++q) v[q] = cmul(v[q], tb[q]);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) buf[lay(e0 + (4 * s + q) * M, kk)] = v[q];
+        }
+    }
+    __syncthreads();
+}
+
+// A radix-4 stage (sub-length L) followed by a radix-2 stage (sub-length L/4) on 8 elements in registers.
+template <bool GIN, class LD>
+__device__ __forceinline__ void dif_stage8(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, LD ld)
+{
+    const int M = L >> 3, nw = (N >> 3) << lay.ktsh, tstep = N / L;
+    for (int w = threadIdx.x; w < nw; w += blockDim.x) {
+        const int kk = w & (kt - 1), bf = w >> lay.ktsh;
+        const int blk = bf / M, j = bf - blk * M;
+        const int e0 = blk * L + j;
+        double2 u[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) u[c] = GIN ? ld(e0 + c * M, kk) : buf[lay(e0 + c * M, kk)];
+        double2 ta[4], tb;
+        if (M > 1) {
+#pragma unroll
+            for (int s = 1; s < 4; ++s) ta[s] = twiddle<false>(tw2, j * s * tstep);
+            tb = twiddle<false>(tw2, 4 * j * tstep);
+        }
+        // stage A: radix 4 over the elements a + 2 r; twiddle W_L^{(j + a M) s} = W_L^{j s} W_8^{a s}
+#pragma unroll
+        for (int a = 0; a < 2; ++a) {
+            double2 v[4] = {u[a], u[a + 2], u[a + 4], u[a + 6]};
+            bfly<4, false>(v);
+            if (a == 1) { v[1] = mul_w16<2, false>(v[1]); v[2] = mul_w16<4, false>(v[2]); v[3] = mul_w16<6, false>(v[3]); }
+            if (M > 1) {
+#pragma unroll
+                for (int s = 1; s < 4; ++s) v[s] = cmul(v[s], ta[s]);
+            }
+#pragma unroll
+            for (int s = 0; s < 4; ++s) u[a + 2 * s] = v[s];
+        }
+        // stage B: radix 2 inside each quarter s (elements 2 s, 2 s + 1); twiddle W_{L/4}^{j}
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            const double2 x0 = cadd(u[2 * s], u[2 * s + 1]);
+            double2 x1 = csub(u[2 * s], u[2 * s + 1]);
+            if (M > 1) x1 = cmul(x1, tb);
+            buf[lay(e0 + (2 * s) * M, kk)] = x0;
+            buf[lay(e0 + (2 * s + 1) * M, kk)] = x1;
+        }
     }
     __syncthreads();
 }
@@ -130,12 +260,12 @@ __device__ __forceinline__ void dif_stage(double2* buf, int N, int L, int kt, in
 // direct O(R^2) stage for a prime R >= 11: one thread per output element; src -> dst (different buffers, or
 // src = the maps when GIN)
 template <bool GIN, class LD>
-__device__ __forceinline__ void dif_generic(const double2* src, double2* dst, int N, int L, int R, int kt, int ktsh,
+__device__ __forceinline__ void dif_generic(const double2* src, double2* dst, int N, int L, int R, int kt, Lay lay,
                                             const double2* __restrict__ tw2, LD ld)
 {
-    const int M = L / R, nout = N << ktsh, tstep = N / L, rstep = N / R;
-    for (int o = threadIdx.x; o < nout; o += NT) {
-        const int kk = o & (kt - 1), pos = o >> ktsh;
+    const int M = L / R, nout = N << lay.ktsh, tstep = N / L, rstep = N / R;
+    for (int o = threadIdx.x; o < nout; o += blockDim.x) {
+        const int kk = o & (kt - 1), pos = o >> lay.ktsh;
         const int blk = pos / L, rem = pos - blk * L;
         const int s = rem / M, j = rem - s * M;
         const int e0 = blk * L + j;
@@ -143,30 +273,30 @@ __device__ __forceinline__ void dif_generic(const double2* src, double2* dst, in
         int e = 0;
         double2 acc = make_double2(0.0, 0.0);
         for (int r = 0; r < R; ++r) {
-            const double2 x = GIN ? ld(e0 + r * M, kk) : src[((e0 + r * M) << ktsh) + kk];
+            const double2 x = GIN ? ld(e0 + r * M, kk) : src[lay(e0 + r * M, kk)];
             const double2 w = twiddle<false>(tw2, e);
             acc.x = fma(x.x, w.x, fma(-x.y, w.y, acc.x));
             acc.y = fma(x.x, w.y, fma(x.y, w.x, acc.y));
             e += es; if (e >= N) e -= N;
         }
         if (M > 1) acc = cmul(acc, twiddle<false>(tw2, j * s * tstep));
-        dst[(pos << ktsh) + kk] = acc;
+        dst[lay(pos, kk)] = acc;
     }
     __syncthreads();
 }
 
 // ---- backward stages (decimation in time, in place): the exact adjoints of the forward stages ----------
 template <int R, bool GOUT, class ST>
-__device__ __forceinline__ void dit_stage(double2* buf, int N, int L, int kt, int ktsh, const double2* __restrict__ tw2, ST st)
+__device__ __forceinline__ void dit_stage(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, ST st)
 {
-    const int M = L / R, nw = (N / R) << ktsh, tstep = N / L;
-    for (int w = threadIdx.x; w < nw; w += NT) {
-        const int kk = w & (kt - 1), bf = w >> ktsh;
+    const int M = L / R, nw = (N / R) << lay.ktsh, tstep = N / L;
+    for (int w = threadIdx.x; w < nw; w += blockDim.x) {
+        const int kk = w & (kt - 1), bf = w >> lay.ktsh;
         const int blk = bf / M, j = bf - blk * M;
         const int e0 = blk * L + j;
         double2 u[R];
 #pragma unroll
-        for (int s = 0; s < R; ++s) u[s] = buf[((e0 + s * M) << ktsh) + kk];
+        for (int s = 0; s < R; ++s) u[s] = buf[lay(e0 + s * M, kk)];
         if (M > 1) {
 #pragma unroll
             for (int s = 1; s < R; ++s) u[s] = cmul(u[s], twiddle<true>(tw2, j * s * tstep));
@@ -175,19 +305,116 @@ __device__ __forceinline__ void dit_stage(double2* buf, int N, int L, int kt, in
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             if (GOUT) st(e0 + r * M, kk, u[r]);
-            else buf[((e0 + r * M) << ktsh) + kk] = u[r];
+            else buf[lay(e0 + r * M, kk)] = u[r];
+        }
+    }
+    if (!GOUT) __syncthreads();
+}
+
+// adjoint of dif_stage16: the radix-4 stage of sub-length L/4, then the one of sub-length L, in registers
+template <bool GOUT, class ST>
+__device__ __forceinline__ void dit_stage16(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, ST st)
+{
+    const int M = L >> 4, nw = (N >> 4) << lay.ktsh, tstep = N / L;
+    for (int w = threadIdx.x; w < nw; w += blockDim.x) {
+        const int kk = w & (kt - 1), bf = w >> lay.ktsh;
+        const int blk = bf / M, j = bf - blk * M;
+        const int e0 = blk * L + j;
+        double2 u[16];
+#pragma unroll
+        for (int c = 0; c < 16; ++c) u[c] = buf[lay(e0 + c * M, kk)];
+        double2 ta[4], tb[4];
+        if (M > 1) {
+#pragma unroll
+            for (int s = 1; s < 4; ++s) tb[s] = twiddle<true>(tw2, 4 * j * s * tstep);
+        }
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            double2 v[4] = {u[4 * s], u[4 * s + 1], u[4 * s + 2], u[4 * s + 3]};
+            if (M > 1) {
+#pragma unroll
+                for (int q = 1; q < 4; ++q) v[q] = cmul(v[q], tb[q]);
+            }
+            bfly<4, true>(v);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) u[4 * s + q] = v[q];
+        }
+        if (M > 1) {
+#pragma unroll
+            for (int s = 1; s < 4; ++s) ta[s] = twiddle<true>(tw2, j * s * tstep);
+        }
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            double2 v[4] = {u[a], u[a + 4], u[a + 8], u[a + 12]};
+            if (M > 1) {
+#pragma unroll
+                for (int s = 1; s < 4; ++s) v[s] = cmul(v[s], ta[s]);
+            }
+            v[1] = a == 0 ? v[1] : a == 1 ? mul_w16<1, true>(v[1]) : a == 2 ? mul_w16<2, true>(v[1]) : mul_w16<3, true>(v[1]);
+            v[2] = a == 0 ? v[2] : a == 1 ? mul_w16<2, true>(v[2]) : a == 2 ? mul_w16<4, true>(v[2]) : mul_w16<6, true>(v[2]);
+            v[3] = a == 0 ? v[3] : a == 1 ? mul_w16<3, true>(v[3]) : a == 2 ? mul_w16<6, true>(v[3]) : mul_w16<9, true>(v[3]);
+            bfly<4, true>(v);
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                if (GOUT) st(e0 + (a + 4 * r) * M, kk, v[r]);
+                else buf[lay(e0 + (a + 4 * r) * M, kk)] = v[r];
+            }
+        }
+    }
+    if (!GOUT) __syncthreads();
+}
+
+// adjoint of dif_stage8
+template <bool GOUT, class ST>
+__device__ __forceinline__ void dit_stage8(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, ST st)
+{
+    const int M = L >> 3, nw = (N >> 3) << lay.ktsh, tstep = N / L;
+    for (int w = threadIdx.x; w < nw; w += blockDim.x) {
+        const int kk = w & (kt - 1), bf = w >> lay.ktsh;
+        const int blk = bf / M, j = bf - blk * M;
+        const int e0 = blk * L + j;
+        double2 u[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) u[c] = buf[lay(e0 + c * M, kk)];
+        double2 ta[4], tb;
+        if (M > 1) {
+#pragma unroll
+            for (int s = 1; s < 4; ++s) ta[s] = twiddle<true>(tw2, j * s * tstep);
+            tb = twiddle<true>(tw2, 4 * j * tstep);
+        }
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            const double2 x0 = u[2 * s];
+            const double2 x1 = M > 1 ? cmul(u[2 * s + 1], tb) : u[2 * s + 1];
+            u[2 * s] = cadd(x0, x1);
+            u[2 * s + 1] = csub(x0, x1);
+        }
+#pragma unroll
+        for (int a = 0; a < 2; ++a) {
+            double2 v[4] = {u[a], u[a + 2], u[a + 4], u[a + 6]};
+            if (M > 1) {
+#pragma unroll
+                for (int s = 1; s < 4; ++s) v[s] = cmul(v[s], ta[s]);
+            }
+            if (a == 1) { v[1] = mul_w16<2, true>(v[1]); v[2] = mul_w16<4, true>(v[2]); v[3] = mul_w16<6, true>(v[3]); }
+            bfly<4, true>(v);
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                if (GOUT) st(e0 + (a + 2 * r) * M, kk, v[r]);
+                else buf[lay(e0 + (a + 2 * r) * M, kk)] = v[r];
+            }
         }
     }
     if (!GOUT) __syncthreads();
 }
 
 template <bool GOUT, class ST>
-__device__ __forceinline__ void dit_generic(const double2* src, double2* dst, int N, int L, int R, int kt, int ktsh,
+__device__ __forceinline__ void dit_generic(const double2* src, double2* dst, int N, int L, int R, int kt, Lay lay,
                                             const double2* __restrict__ tw2, ST st)
 {
-    const int M = L / R, nout = N << ktsh, tstep = N / L, rstep = N / R;
-    for (int o = threadIdx.x; o < nout; o += NT) {
-        const int kk = o & (kt - 1), pos = o >> ktsh;
+    const int M = L / R, nout = N << lay.ktsh, tstep = N / L, rstep = N / R;
+    for (int o = threadIdx.x; o < nout; o += blockDim.x) {
+        const int kk = o & (kt - 1), pos = o >> lay.ktsh;
         const int blk = pos / L, rem = pos - blk * L;
         const int r = rem / M, j = rem - r * M;
         const int e0 = blk * L + j;
@@ -196,24 +423,26 @@ __device__ __forceinline__ void dit_generic(const double2* src, double2* dst, in
         int e = 0;
         double2 acc = make_double2(0.0, 0.0);
         for (int s = 0; s < R; ++s) {
-            const double2 x = src[((e0 + s * M) << ktsh) + kk];
+            const double2 x = src[lay(e0 + s * M, kk)];
             const double2 w = twiddle<true>(tw2, e);
             acc.x = fma(x.x, w.x, fma(-x.y, w.y, acc.x));
             acc.y = fma(x.x, w.y, fma(x.y, w.x, acc.y));
             e += es; if (e >= N) e -= N;
         }
         if (GOUT) st(pos, kk, acc);
-        else dst[(pos << ktsh) + kk] = acc;
+        else dst[lay(pos, kk)] = acc;
     }
     if (!GOUT) __syncthreads();
 }
 
 // ---- transform drivers -----------------------------------------------------------------------------------
+// The plan's radix list holds 2, 3, 4, 5, 7, primes >= 11, and the codes 16 (two radix-4 stages fused in registers)
+// and 8 (a radix-4 and a radix-2 stage fused).
 // forward transform of length N over the radix list (first stage reads through `ld`); returns the buffer that
 // holds the result (bin k at position perm[k])
 template <class LD>
-__device__ __forceinline__ double2* fft_forward(double2* smem, int N, const int* __restrict__ radix, int nfac, int kt, int ktsh,
-                                                const double2* __restrict__ tw2, LD ld)
+__device__ __forceinline__ double2* fft_forward(double2* smem, int N, int nbuf, const int* __restrict__ radix, int nfac, int kt,
+                                                Lay lay, const double2* __restrict__ tw2, LD ld)
 {
     double2* cur = smem;
     int L = N;
@@ -221,23 +450,27 @@ __device__ __forceinline__ double2* fft_forward(double2* smem, int N, const int*
         const int R = radix[f];
         if (f == 0) {
             switch (R) {
-                case 2: dif_stage<2, true>(cur, N, L, kt, ktsh, tw2, ld); break;
-                case 3: dif_stage<3, true>(cur, N, L, kt, ktsh, tw2, ld); break;
-                case 4: dif_stage<4, true>(cur, N, L, kt, ktsh, tw2, ld); break;
-                case 5: dif_stage<5, true>(cur, N, L, kt, ktsh, tw2, ld); break;
-                case 7: dif_stage<7, true>(cur, N, L, kt, ktsh, tw2, ld); break;
-                default: dif_generic<true>(nullptr, cur, N, L, R, kt, ktsh, tw2, ld); break;
+                case 2: dif_stage<2, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 3: dif_stage<3, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 4: dif_stage<4, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 5: dif_stage<5, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 7: dif_stage<7, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 8: dif_stage8<true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 16: dif_stage16<true>(cur, N, L, kt, lay, tw2, ld); break;
+                default: dif_generic<true>(nullptr, cur, N, L, R, kt, lay, tw2, ld); break;
             }
         } else {
             switch (R) {
-                case 2: dif_stage<2, false>(cur, N, L, kt, ktsh, tw2, ld); break;
-                case 3: dif_stage<3, false>(cur, N, L, kt, ktsh, tw2, ld); break;
-                case 4: dif_stage<4, false>(cur, N, L, kt, ktsh, tw2, ld); break;
-                case 5: dif_stage<5, false>(cur, N, L, kt, ktsh, tw2, ld); break;
-                case 7: dif_stage<7, false>(cur, N, L, kt, ktsh, tw2, ld); break;
+                case 2: dif_stage<2, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 3: dif_stage<3, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 4: dif_stage<4, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 5: dif_stage<5, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 7: dif_stage<7, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 8: dif_stage8<false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 16: dif_stage16<false>(cur, N, L, kt, lay, tw2, ld); break;
                 default: {
-                    double2* other = (cur == smem) ? smem + ((size_t)N << ktsh) : smem;
-                    dif_generic<false>(cur, other, N, L, R, kt, ktsh, tw2, ld);
+                    double2* other = (cur == smem) ? smem + nbuf : smem;
+                    dif_generic<false>(cur, other, N, L, R, kt, lay, tw2, ld);
                     cur = other;
                 } break;
             }
@@ -249,8 +482,8 @@ __device__ __forceinline__ double2* fft_forward(double2* smem, int N, const int*
 
 // backward transform: `cur` holds bin k at position perm[k]; the last stage writes through `st`
 template <class ST>
-__device__ __forceinline__ void fft_backward(double2* smem, double2* cur, int N, const int* __restrict__ radix, int nfac, int kt,
-                                             int ktsh, const double2* __restrict__ tw2, ST st)
+__device__ __forceinline__ void fft_backward(double2* smem, double2* cur, int N, int nbuf, const int* __restrict__ radix, int nfac,
+                                             int kt, Lay lay, const double2* __restrict__ tw2, ST st)
 {
     int L = 1;
     for (int f = nfac - 1; f >= 0; --f) {
@@ -258,23 +491,27 @@ __device__ __forceinline__ void fft_backward(double2* smem, double2* cur, int N,
         L *= R;
         if (f == 0) {
             switch (R) {
-                case 2: dit_stage<2, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 3: dit_stage<3, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 4: dit_stage<4, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 5: dit_stage<5, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 7: dit_stage<7, true>(cur, N, L, kt, ktsh, tw2, st); break;
-                default: dit_generic<true>(cur, nullptr, N, L, R, kt, ktsh, tw2, st); break;
+                case 2: dit_stage<2, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 3: dit_stage<3, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 4: dit_stage<4, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 5: dit_stage<5, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 7: dit_stage<7, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 8: dit_stage8<true>(cur, N, L, kt, lay, tw2, st); break;
+                case 16: dit_stage16<true>(cur, N, L, kt, lay, tw2, st); break;
+                default: dit_generic<true>(cur, nullptr, N, L, R, kt, lay, tw2, st); break;
             }
         } else {
             switch (R) {
-                case 2: dit_stage<2, false>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 3: dit_stage<3, false>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 4: dit_stage<4, false>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 5: dit_stage<5, false>(cur, N, L, kt, ktsh, tw2, st); break;
-                case 7: dit_stage<7, false>(cur, N, L, kt, ktsh, tw2, st); break;
+                case 2: dit_stage<2, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 3: dit_stage<3, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 4: dit_stage<4, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 5: dit_stage<5, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 7: dit_stage<7, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 8: dit_stage8<false>(cur, N, L, kt, lay, tw2, st); break;
+                case 16: dit_stage16<false>(cur, N, L, kt, lay, tw2, st); break;
                 default: {
-                    double2* other = (cur == smem) ? smem + ((size_t)N << ktsh) : smem;
-                    dit_generic<false>(cur, other, N, L, R, kt, ktsh, tw2, st);
+                    double2* other = (cur == smem) ? smem + nbuf : smem;
+                    dit_generic<false>(cur, other, N, L, R, kt, lay, tw2, st);
                     cur = other;
                 } break;
             }
@@ -286,26 +523,32 @@ __device__ __forceinline__ void fft_backward(double2* smem, double2* cur, int N,
 //   buf <- IFFT_Lc( FFT_Lc(x) . Hf ),  x delivered by `ld` (first forward stage), result handed to `st` by the
 // last backward stage when GOUT, else left in buf in natural order.  Hf is stored in forward-output position order.
 template <bool GIN, bool GOUT, bool CONJ, class LD, class ST>
-__device__ __forceinline__ void bluestein_conv(double2* buf, int Lc, const int* __restrict__ radix, int nfac, int kt, int ktsh,
+__device__ __forceinline__ void bluestein_conv(double2* buf, int Lc, const int* __restrict__ radix, int nfac, int kt, Lay lay,
                                                const double2* __restrict__ btw, const double2* __restrict__ hf, LD ld, ST st)
 {
     int L = Lc;
     for (int f = 0; f < nfac; ++f) {
         const int R = radix[f];
         if (GIN && f == 0) {
-            if (R == 4) dif_stage<4, true>(buf, Lc, L, kt, ktsh, btw, ld);
-            else dif_stage<2, true>(buf, Lc, L, kt, ktsh, btw, ld);
+            if (R == 16) dif_stage16<true>(buf, Lc, L, kt, lay, btw, ld);
+            else if (R == 8) dif_stage8<true>(buf, Lc, L, kt, lay, btw, ld);
+            else if (R == 4) dif_stage<4, true>(buf, Lc, L, kt, lay, btw, ld);
+            else dif_stage<2, true>(buf, Lc, L, kt, lay, btw, ld);
         } else {
-            if (R == 4) dif_stage<4, false>(buf, Lc, L, kt, ktsh, btw, ld);
-            else dif_stage<2, false>(buf, Lc, L, kt, ktsh, btw, ld);
+            if (R == 16) dif_stage16<false>(buf, Lc, L, kt, lay, btw, ld);
+            else if (R == 8) dif_stage8<false>(buf, Lc, L, kt, lay, btw, ld);
+            else if (R == 4) dif_stage<4, false>(buf, Lc, L, kt, lay, btw, ld);
+            else dif_stage<2, false>(buf, Lc, L, kt, lay, btw, ld);
         }
         L /= R;
     }
-    const int tot = Lc << ktsh;
-    for (int i = threadIdx.x; i < tot; i += NT) {
-        double2 h = __ldg(hf + (i >> ktsh));
+    const int tot = Lc << lay.ktsh;
+    for (int i = threadIdx.x; i < tot; i += blockDim.x) {
+        const int e = i >> lay.ktsh, kk = i & (kt - 1);
+        double2 h = __ldg(hf + e);
         if (CONJ) h.y = -h.y;
-        buf[i] = cmul(buf[i], h);
+        const int a = lay(e, kk);
+        buf[a] = cmul(buf[a], h);
     }
     __syncthreads();
     L = 1;
@@ -313,11 +556,15 @@ __device__ __forceinline__ void bluestein_conv(double2* buf, int Lc, const int* 
         const int R = radix[f];
         L *= R;
         if (GOUT && f == 0) {
-            if (R == 4) dit_stage<4, true>(buf, Lc, L, kt, ktsh, btw, st);
-            else dit_stage<2, true>(buf, Lc, L, kt, ktsh, btw, st);
+            if (R == 16) dit_stage16<true>(buf, Lc, L, kt, lay, btw, st);
+            else if (R == 8) dit_stage8<true>(buf, Lc, L, kt, lay, btw, st);
+            else if (R == 4) dit_stage<4, true>(buf, Lc, L, kt, lay, btw, st);
+            else dit_stage<2, true>(buf, Lc, L, kt, lay, btw, st);
         } else {
-            if (R == 4) dit_stage<4, false>(buf, Lc, L, kt, ktsh, btw, st);
-            else dit_stage<2, false>(buf, Lc, L, kt, ktsh, btw, st);
+            if (R == 16) dit_stage16<false>(buf, Lc, L, kt, lay, btw, st);
+            else if (R == 8) dit_stage8<false>(buf, Lc, L, kt, lay, btw, st);
+            else if (R == 4) dit_stage<4, false>(buf, Lc, L, kt, lay, btw, st);
+            else dit_stage<2, false>(buf, Lc, L, kt, lay, btw, st);
         }
     }
 }
@@ -326,7 +573,7 @@ __device__ __forceinline__ void bluestein_conv(double2* buf, int Lc, const int* 
 // analysis: maps -> F (E/O folded, phase shifted, aliased to every m < mlim)
 // grid (map blocks, rings of the launch class, ncomp)
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* __restrict__ ring_list,
+__global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int* __restrict__ ring_list,
                                                      const double* __restrict__ maps, double* __restrict__ F,
                                                      int k0, int kmaps)
 {
@@ -334,9 +581,11 @@ __global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* _
     const int p = ring_list[blockIdx.y], comp = blockIdx.z;
     const RingPair rp = d.rings[p];
     const int N = rp.n, kt = rp.kt, ktsh = __ffs(kt) - 1;
+    const Lay lay{ktsh, rp.psh};
+    const int nbuf = rp.nbuf << ktsh;                     // elements of one transform buffer (padding included)
     const int kbase = blockIdx.x * kt;
     if (kbase >= kmaps) return;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, nt = blockDim.x;
     const double2* tw2 = d.tw + rp.tw_off;
     const unsigned short* perm = d.perm + rp.perm_off;
     const bool equator = rp.start_s < 0;
@@ -354,7 +603,7 @@ __global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* _
 
     double2* cur = smem;
     if (!blue) {
-        cur = fft_forward(smem, N, d.radix + rp.fac_off, rp.nfac, kt, ktsh, tw2, ld);
+        cur = fft_forward(smem, N, nbuf, d.radix + rp.fac_off, rp.nfac, kt, lay, tw2, ld);
     } else {
         // X_b = c_b sum_n (x_n c_n) conj(c)_{b-n},  c_n = exp(-i pi n^2 / N) = W_{2N}^{n^2 mod 2N}
         auto ldc = [&](int e, int kk) -> double2 {
@@ -362,7 +611,7 @@ __global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* _
             return cmul(ld(e, kk), __ldg(tw2 + (e * e) % (2 * N)));
         };
         auto nost = [](int, int, double2) {};
-        bluestein_conv<true, false, false>(smem, rp.lc, d.radix + rp.b_fac_off, rp.b_nfac, kt, ktsh, d.tw + rp.b_tw_off,
+        bluestein_conv<true, false, false>(smem, rp.lc, d.radix + rp.b_fac_off, rp.b_nfac, kt, lay, d.tw + rp.b_tw_off,
                                            d.tw + rp.hf_off, ldc, nost);
     }
 
@@ -370,17 +619,18 @@ __global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* _
     const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
     const int total = rp.mlim << ktsh;
     double2* Fc = reinterpret_cast<double2*>(F);
-    for (int idx = tid; idx < total; idx += NT) {
+#pragma unroll 2
+    for (int idx = tid; idx < total; idx += nt) {
         const int kk = idx & (kt - 1), m = idx >> ktsh;
         const int k = kbase + kk;
         if (k >= kmaps) continue;
         const int b = m % N, bc = b == 0 ? 0 : N - b;
         double2 A, B;
         if (!blue) {
-            A = cur[((int)perm[b] << ktsh) + kk]; B = cur[((int)perm[bc] << ktsh) + kk];
+            A = cur[lay((int)perm[b], kk)]; B = cur[lay((int)perm[bc], kk)];
         } else {
-            A = cmul(cur[(b << ktsh) + kk], __ldg(tw2 + (b * b) % (2 * N)));
-            B = cmul(cur[(bc << ktsh) + kk], __ldg(tw2 + (bc * bc) % (2 * N)));
+            A = cmul(cur[lay(b, kk)], __ldg(tw2 + (b * b) % (2 * N)));
+            B = cmul(cur[lay(bc, kk)], __ldg(tw2 + (bc * bc) % (2 * N)));
         }
         // G_north = (A + conj B)/2, G_south = (A - conj B)/(2i)
         const double2 gn = make_double2(0.5 * (A.x + B.x), 0.5 * (A.y - B.y));
@@ -403,7 +653,7 @@ __global__ void __launch_bounds__(NT) k_ring_analysis(DevicePlan d, const int* _
 // ------------------------------------------------------------------------------------------------
 // synthesis: F (north/south T_m) -> maps.  If sub_from != nullptr: maps = sub_from - synthesis.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* __restrict__ ring_list,
+__global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const int* __restrict__ ring_list,
                                                       const double* __restrict__ F, double* __restrict__ maps,
                                                       int k0, int kmaps, const double* __restrict__ sub_from, int ksub0)
 {
@@ -411,9 +661,11 @@ __global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* 
     const int p = ring_list[blockIdx.y], comp = blockIdx.z;
     const RingPair rp = d.rings[p];
     const int N = rp.n, kt = rp.kt, ktsh = __ffs(kt) - 1;
+    const Lay lay{ktsh, rp.psh};
+    const int nbuf = rp.nbuf << ktsh;                     // elements of one transform buffer (padding included)
     const int kbase = blockIdx.x * kt;
     if (kbase >= kmaps) return;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, nt = blockDim.x;
     const double2* tw2 = d.tw + rp.tw_off;
     const unsigned short* perm = d.perm + rp.perm_off;
     const bool equator = rp.start_s < 0;
@@ -425,7 +677,7 @@ __global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* 
     // from the workspace (each cell read once), bins N - b follow from the Hermitian symmetry of Y_n, Y_s
     const double2* Fc = reinterpret_cast<const double2*>(F);
     const int total = (N / 2 + 1) << ktsh;
-    for (int idx = tid; idx < total; idx += NT) {
+    for (int idx = tid; idx < total; idx += nt) {
         const int kk = idx & (kt - 1), b = idx >> ktsh;
         const int k = kbase + kk;
         double2 yn = make_double2(0.0, 0.0), ys = make_double2(0.0, 0.0);
@@ -452,22 +704,22 @@ __global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* 
         const double2 zb = make_double2(yn.x - ys.y, yn.y + ys.x);
         const double2 zc = make_double2(yn.x + ys.y, ys.x - yn.y);           // Z[N - b]
         if (!blue) {
-            cur[((int)perm[b] << ktsh) + kk] = zb;
-            if (b > 0 && 2 * b < N) cur[((int)perm[N - b] << ktsh) + kk] = zc;
+            cur[lay((int)perm[b], kk)] = zb;
+            if (b > 0 && 2 * b < N) cur[lay((int)perm[N - b], kk)] = zc;
         } else {
             // x_n = conj(c)_n sum_b (Z_b conj(c)_b) c_{n-b}
             double2 c = __ldg(tw2 + (b * b) % (2 * N)); c.y = -c.y;
-            cur[(b << ktsh) + kk] = cmul(zb, c);
+            cur[lay(b, kk)] = cmul(zb, c);
             if (b > 0 && 2 * b < N) {
                 const int bb = N - b;
                 double2 c2 = __ldg(tw2 + (bb * bb) % (2 * N)); c2.y = -c2.y;
-                cur[(bb << ktsh) + kk] = cmul(zc, c2);
+                cur[lay(bb, kk)] = cmul(zc, c2);
             }
         }
     }
     if (blue) {
         const int tot = rp.lc << ktsh;
-        for (int i = (N << ktsh) + tid; i < tot; i += NT) cur[i] = make_double2(0.0, 0.0);
+        for (int i = (N << ktsh) + tid; i < tot; i += nt) cur[lay(i >> ktsh, i & (kt - 1))] = make_double2(0.0, 0.0);
     }
     __syncthreads();
 
@@ -489,7 +741,7 @@ __global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* 
     };
 
     if (!blue) {
-        fft_backward(smem, cur, N, d.radix + rp.fac_off, rp.nfac, kt, ktsh, tw2, st);
+        fft_backward(smem, cur, N, nbuf, d.radix + rp.fac_off, rp.nfac, kt, lay, tw2, st);
     } else {
         auto stc = [&](int e, int kk, double2 v) {
             if (e >= N) return;
@@ -497,10 +749,13 @@ __global__ void __launch_bounds__(NT) k_ring_synthesis(DevicePlan d, const int* 
             st(e, kk, cmul(v, c));
         };
         auto nold = [](int, int) -> double2 { return make_double2(0.0, 0.0); };
-        bluestein_conv<false, true, true>(smem, rp.lc, d.radix + rp.b_fac_off, rp.b_nfac, kt, ktsh, d.tw + rp.b_tw_off,
+        bluestein_conv<false, true, true>(smem, rp.lc, d.radix + rp.b_fac_off, rp.b_nfac, kt, lay, d.tw + rp.b_tw_off,
                                           d.tw + rp.hf_off, nold, stc);
     }
 }
+
+// CTAs that share an SM with another one run RING_THREADS threads; a CTA that owns the SM runs twice as many
+static int ring_threads(size_t smem) { return smem <= (size_t)113 * 1024 ? RING_THREADS : 2 * RING_THREADS; }
 
 static cudaError_t ring_attr(sht_plan_s* pl)
 {
@@ -521,7 +776,7 @@ cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const doub
     for (int c = RING_NCLASS - 1; c >= 0; --c) {
         if (pl->class_count[c] == 0) continue;
         dim3 grid((kmaps + pl->class_ktmin[c] - 1) / pl->class_ktmin[c], pl->class_count[c], d.ncomp);
-        k_ring_analysis<<<grid, NT, pl->class_smem[c], st>>>(d, pl->class_rings[c], maps, F, k0, kmaps);
+        k_ring_analysis<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c], st>>>(d, pl->class_rings[c], maps, F, k0, kmaps);
         pl->launches++;
     }
     return cudaGetLastError();
@@ -535,7 +790,7 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
     for (int c = RING_NCLASS - 1; c >= 0; --c) {
         if (pl->class_count[c] == 0) continue;
         dim3 grid((kmaps + pl->class_ktmin[c] - 1) / pl->class_ktmin[c], pl->class_count[c], d.ncomp);
-        k_ring_synthesis<<<grid, NT, pl->class_smem[c], st>>>(d, pl->class_rings[c], F, maps, k0, kmaps, sub_from, ksub0);
+        k_ring_synthesis<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c], st>>>(d, pl->class_rings[c], F, maps, k0, kmaps, sub_from, ksub0);
         pl->launches++;
     }
     return cudaGetLastError();
