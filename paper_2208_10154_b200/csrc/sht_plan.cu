@@ -100,7 +100,10 @@ static int factorize_ring(int n, std::vector<int>& out)
     if (r > 1) (r <= 7 ? small : big).push_back(r);
     for (size_t i = big.size(); i-- > 0;) out.push_back(big[i]);
     for (int v : small) out.push_back(v);
-    return (int)big.size();
+    // primes 11 .. 31 run in place (register stages); only larger ones (rings too long for Bluestein) need two buffers
+    int ngeneric = 0;
+    for (int v : big) ngeneric += v >= BLUESTEIN_MIN_PRIME ? 1 : 0;
+    return ngeneric;
 }
 
 template <typename T>

@@ -257,6 +257,41 @@ __device__ __forceinline__ void dif_stage8(double2* buf, int N, int L, int kt, L
     __syncthreads();
 }
 
+// Direct stage for a prime 11 <= R <= 31: one thread owns a whole butterfly, its R inputs live in registers, every
+// output is a dot product with a row of W_R (read through the W_N table, the same address for the whole warp);
+// in place.  R^2 complex multiply-adds per butterfly, but one pass and no second buffer.
+template <int R, bool GIN, class LD>
+__device__ __forceinline__ void dif_prime(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, LD ld)
+{
+    const int M = L / R, nw = (N / R) << lay.ktsh, tstep = N / L, rstep = 2 * (N / R);
+    for (int w = threadIdx.x; w < nw; w += blockDim.x) {
+        const int kk = w & (kt - 1), bf = w >> lay.ktsh;
+        const int blk = bf / M, j = bf - blk * M;
+        const int e0 = blk * L + j;
+        double2 x[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) x[r] = GIN ? ld(e0 + r * M, kk) : buf[lay(e0 + r * M, kk)];
+        double2 sum = x[0];
+#pragma unroll
+        for (int r = 1; r < R; ++r) sum = cadd(sum, x[r]);
+        buf[lay(e0, kk)] = sum;
+        for (int sx = 1; sx < R; ++sx) {
+            double2 acc = x[0];
+            int idx = 0;
+#pragma unroll
+            for (int r = 1; r < R; ++r) {
+                idx += sx; if (idx >= R) idx -= R;
+                const double2 wv = __ldg(tw2 + idx * rstep);             // W_R^{r s}
+                acc.x = fma(x[r].x, wv.x, fma(-x[r].y, wv.y, acc.x));
+                acc.y = fma(x[r].x, wv.y, fma(x[r].y, wv.x, acc.y));
+            }
+            if (M > 1) acc = cmul(acc, twiddle<false>(tw2, j * sx * tstep));
+            buf[lay(e0 + sx * M, kk)] = acc;
+        }
+    }
+    __syncthreads();
+}
+
 // direct O(R^2) stage for a prime R >= 11: one thread per output element; src -> dst (different buffers, or
 // src = the maps when GIN)
 template <bool GIN, class LD>
@@ -408,6 +443,43 @@ __device__ __forceinline__ void dit_stage8(double2* buf, int N, int L, int kt, L
     if (!GOUT) __syncthreads();
 }
 
+// adjoint of dif_prime
+template <int R, bool GOUT, class ST>
+__device__ __forceinline__ void dit_prime(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, ST st)
+{
+    const int M = L / R, nw = (N / R) << lay.ktsh, tstep = N / L, rstep = 2 * (N / R);
+    for (int w = threadIdx.x; w < nw; w += blockDim.x) {
+        const int kk = w & (kt - 1), bf = w >> lay.ktsh;
+        const int blk = bf / M, j = bf - blk * M;
+        const int e0 = blk * L + j;
+        double2 x[R];
+#pragma unroll
+        for (int sx = 0; sx < R; ++sx) x[sx] = buf[lay(e0 + sx * M, kk)];
+        if (M > 1) {
+#pragma unroll
+            for (int sx = 1; sx < R; ++sx) x[sx] = cmul(x[sx], twiddle<true>(tw2, j * sx * tstep));
+        }
+        double2 sum = x[0];
+#pragma unroll
+        for (int sx = 1; sx < R; ++sx) sum = cadd(sum, x[sx]);
+        if (GOUT) st(e0, kk, sum); else buf[lay(e0, kk)] = sum;
+        for (int r = 1; r < R; ++r) {
+            double2 acc = x[0];
+            int idx = 0;
+#pragma unroll
+            for (int sx = 1; sx < R; ++sx) {
+                idx += r; if (idx >= R) idx -= R;
+                double2 wv = __ldg(tw2 + idx * rstep);                   // conj W_R^{r s}
+                wv.y = -wv.y;
+                acc.x = fma(x[sx].x, wv.x, fma(-x[sx].y, wv.y, acc.x));
+                acc.y = fma(x[sx].x, wv.y, fma(x[sx].y, wv.x, acc.y));
+            }
+            if (GOUT) st(e0 + r * M, kk, acc); else buf[lay(e0 + r * M, kk)] = acc;
+        }
+    }
+    if (!GOUT) __syncthreads();
+}
+
 template <bool GOUT, class ST>
 __device__ __forceinline__ void dit_generic(const double2* src, double2* dst, int N, int L, int R, int kt, Lay lay,
                                             const double2* __restrict__ tw2, ST st)
@@ -457,6 +529,13 @@ __device__ __forceinline__ double2* fft_forward(double2* smem, int N, int nbuf, 
                 case 7: dif_stage<7, true>(cur, N, L, kt, lay, tw2, ld); break;
                 case 8: dif_stage8<true>(cur, N, L, kt, lay, tw2, ld); break;
                 case 16: dif_stage16<true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 11: dif_prime<11, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 13: dif_prime<13, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 17: dif_prime<17, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 19: dif_prime<19, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 23: dif_prime<23, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 29: dif_prime<29, true>(cur, N, L, kt, lay, tw2, ld); break;
+                case 31: dif_prime<31, true>(cur, N, L, kt, lay, tw2, ld); break;
                 default: dif_generic<true>(nullptr, cur, N, L, R, kt, lay, tw2, ld); break;
             }
         } else {
@@ -468,6 +547,13 @@ __device__ __forceinline__ double2* fft_forward(double2* smem, int N, int nbuf, 
                 case 7: dif_stage<7, false>(cur, N, L, kt, lay, tw2, ld); break;
                 case 8: dif_stage8<false>(cur, N, L, kt, lay, tw2, ld); break;
                 case 16: dif_stage16<false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 11: dif_prime<11, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 13: dif_prime<13, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 17: dif_prime<17, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 19: dif_prime<19, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 23: dif_prime<23, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 29: dif_prime<29, false>(cur, N, L, kt, lay, tw2, ld); break;
+                case 31: dif_prime<31, false>(cur, N, L, kt, lay, tw2, ld); break;
                 default: {
                     double2* other = (cur == smem) ? smem + nbuf : smem;
                     dif_generic<false>(cur, other, N, L, R, kt, lay, tw2, ld);
@@ -498,6 +584,13 @@ __device__ __forceinline__ void fft_backward(double2* smem, double2* cur, int N,
                 case 7: dit_stage<7, true>(cur, N, L, kt, lay, tw2, st); break;
                 case 8: dit_stage8<true>(cur, N, L, kt, lay, tw2, st); break;
                 case 16: dit_stage16<true>(cur, N, L, kt, lay, tw2, st); break;
+                case 11: dit_prime<11, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 13: dit_prime<13, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 17: dit_prime<17, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 19: dit_prime<19, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 23: dit_prime<23, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 29: dit_prime<29, true>(cur, N, L, kt, lay, tw2, st); break;
+                case 31: dit_prime<31, true>(cur, N, L, kt, lay, tw2, st); break;
                 default: dit_generic<true>(cur, nullptr, N, L, R, kt, lay, tw2, st); break;
             }
         } else {
@@ -509,6 +602,13 @@ __device__ __forceinline__ void fft_backward(double2* smem, double2* cur, int N,
                 case 7: dit_stage<7, false>(cur, N, L, kt, lay, tw2, st); break;
                 case 8: dit_stage8<false>(cur, N, L, kt, lay, tw2, st); break;
                 case 16: dit_stage16<false>(cur, N, L, kt, lay, tw2, st); break;
+                case 11: dit_prime<11, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 13: dit_prime<13, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 17: dit_prime<17, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 19: dit_prime<19, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 23: dit_prime<23, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 29: dit_prime<29, false>(cur, N, L, kt, lay, tw2, st); break;
+                case 31: dit_prime<31, false>(cur, N, L, kt, lay, tw2, st); break;
                 default: {
                     double2* other = (cur == smem) ? smem + nbuf : smem;
                     dit_generic<false>(cur, other, N, L, R, kt, lay, tw2, st);
@@ -615,16 +715,21 @@ __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int
                                            d.tw + rp.hf_off, ldc, nost);
     }
 
-    // FFT mapping: m -> bin on the frequency circle (stored at position perm[bin]), phase, fold
+    // FFT mapping: m -> bin on the frequency circle (stored at position perm[bin]), phase, fold.
+    // A thread keeps its map (nt is a multiple of kt) and walks m with a fixed stride: m mod N, m mod 2N and the
+    // workspace address advance incrementally (no division, no 64-bit multiply in the loop).
     const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
-    const int total = rp.mlim << ktsh;
-    double2* Fc = reinterpret_cast<double2*>(F);
+    const int kk = tid & (kt - 1), k = kbase + kk;
+    if (k >= kmaps) return;
+    const int dm = nt >> ktsh, dmN = dm % N, dm2N = dm % (2 * N);
+    int m = tid >> ktsh;
+    int b = m % N, m2 = m % (2 * N);
+    const size_t cstride = (size_t)d.ncomp * 2 * KG;                       // double2 per order m
+    double2* Fp = reinterpret_cast<double2*>(F) + f_cell(d, p, k >> 2, 0, comp, 0) + (k & 3) + (size_t)m * cstride;
+    const int mlim = rp.mlim;
 #pragma unroll 2
-    for (int idx = tid; idx < total; idx += nt) {
-        const int kk = idx & (kt - 1), m = idx >> ktsh;
-        const int k = kbase + kk;
-        if (k >= kmaps) continue;
-        const int b = m % N, bc = b == 0 ? 0 : N - b;
+    for (; m < mlim; m += dm) {
+        const int bc = b == 0 ? 0 : N - b;
         double2 A, B;
         if (!blue) {
             A = cur[lay((int)perm[b], kk)]; B = cur[lay((int)perm[bc], kk)];
@@ -637,16 +742,18 @@ __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int
         const double2 gs = make_double2(0.5 * (A.y + B.y), -0.5 * (A.x - B.x));
         double2 ph = make_double2(dsig, 0.0);
         if (rp.shift) {                                   // e^{-i m phi0}, phi0 = pi / N
-            ph = __ldg(tw2 + (m % (2 * N)));
+            ph = __ldg(tw2 + m2);
             ph.x *= dsig; ph.y *= dsig;
         }
         double2 E, O;
         if (equator) { E = cmul(ph, gn); O = make_double2(0.0, 0.0); }
         else { E = cmul(ph, cadd(gn, gs)); O = cmul(ph, csub(gn, gs)); }
         if (comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }      // i U
-        const size_t cell = f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
-        Fc[cell] = E;
-        Fc[cell + KG] = O;
+        Fp[0] = E;
+        Fp[KG] = O;
+        Fp += (size_t)dm * cstride;
+        b += dmN; if (b >= N) b -= N;
+        m2 += dm2N; if (m2 >= 2 * N) m2 -= 2 * N;
     }
 }
 
@@ -675,45 +782,51 @@ __global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const in
 
     // ring spectrum of the packed sequence, Z[b] = Y_north[b] + i Y_south[b]; bins b <= N/2 are assembled
     // from the workspace (each cell read once), bins N - b follow from the Hermitian symmetry of Y_n, Y_s
-    const double2* Fc = reinterpret_cast<const double2*>(F);
-    const int total = (N / 2 + 1) << ktsh;
-    for (int idx = tid; idx < total; idx += nt) {
-        const int kk = idx & (kt - 1), b = idx >> ktsh;
-        const int k = kbase + kk;
-        double2 yn = make_double2(0.0, 0.0), ys = make_double2(0.0, 0.0);
-        if (k < kmaps) {
-            // m = b (mod N): + (w/2) d_m ;  m = -b (mod N): + (w/2) conj(d_m);  d_m = e^{+i m phi0} T_m
-            for (int pass = 0; pass < 2; ++pass) {
-                const int mfirst = pass == 0 ? b : (b == 0 ? 0 : N - b);
-                for (int m = mfirst; m < mlim; m += N) {
-                    const double w = (m == 0) ? 0.5 : 1.0;
-                    double2 ph = make_double2(1.0, 0.0);
-                    if (rp.shift) { ph = __ldg(tw2 + (m % (2 * N))); ph.y = -ph.y; }
-                    const size_t cell = f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
-                    double2 fn = Fc[cell], fs = Fc[cell + KG];
-                    if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }   // U = -i (iU)
-                    double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
-                    if (pass == 1) { dn.y = -dn.y; ds.y = -ds.y; }
-                    yn.x = fma(w, dn.x, yn.x); yn.y = fma(w, dn.y, yn.y);
-                    ys.x = fma(w, ds.x, ys.x); ys.y = fma(w, ds.y, ys.y);
+    // A thread keeps its map and walks the bins with a fixed stride; workspace addresses advance incrementally.
+    {
+        const int kk = tid & (kt - 1), k = kbase + kk;
+        const int db = nt >> ktsh;
+        const size_t cstride = (size_t)d.ncomp * 2 * KG;                   // double2 per order m
+        const double2* Fb = reinterpret_cast<const double2*>(F) + f_cell(d, p, (k < kmaps ? k : kbase) >> 2, 0, comp, 0) + (k & 3);
+        for (int b = tid >> ktsh; b <= N / 2; b += db) {
+            double2 yn = make_double2(0.0, 0.0), ys = make_double2(0.0, 0.0);
+            if (k < kmaps) {
+                // m = b (mod N): + (w/2) d_m ;  m = -b (mod N): + (w/2) conj(d_m);  d_m = e^{+i m phi0} T_m
+#pragma unroll
+                for (int pass = 0; pass < 2; ++pass) {
+                    const int mfirst = pass == 0 ? b : (b == 0 ? 0 : N - b);
+                    int m2 = mfirst;                                       // m mod 2N
+                    const double2* Fp = Fb + (size_t)mfirst * cstride;
+                    for (int m = mfirst; m < mlim; m += N, Fp += (size_t)N * cstride) {
+                        const double w = (m == 0) ? 0.5 : 1.0;
+                        double2 ph = make_double2(1.0, 0.0);
+                        if (rp.shift) { ph = __ldg(tw2 + m2); ph.y = -ph.y; }
+                        double2 fn = Fp[0], fs = Fp[KG];
+                        if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }   // U = -i (iU)
+                        double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
+                        if (pass == 1) { dn.y = -dn.y; ds.y = -ds.y; }
+                        yn.x = fma(w, dn.x, yn.x); yn.y = fma(w, dn.y, yn.y);
+                        ys.x = fma(w, ds.x, ys.x); ys.y = fma(w, ds.y, ys.y);
+                        m2 += N; if (m2 >= 2 * N) m2 -= 2 * N;
+                    }
                 }
             }
-        }
-        if (equator) ys = make_double2(0.0, 0.0);
-        if (b == 0 || 2 * b == N) { yn.y = 0.0; ys.y = 0.0; }
-        const double2 zb = make_double2(yn.x - ys.y, yn.y + ys.x);
-        const double2 zc = make_double2(yn.x + ys.y, ys.x - yn.y);           // Z[N - b]
-        if (!blue) {
-            cur[lay((int)perm[b], kk)] = zb;
-            if (b > 0 && 2 * b < N) cur[lay((int)perm[N - b], kk)] = zc;
-        } else {
-            // x_n = conj(c)_n sum_b (Z_b conj(c)_b) c_{n-b}
-            double2 c = __ldg(tw2 + (b * b) % (2 * N)); c.y = -c.y;
-            cur[lay(b, kk)] = cmul(zb, c);
-            if (b > 0 && 2 * b < N) {
-                const int bb = N - b;
-                double2 c2 = __ldg(tw2 + (bb * bb) % (2 * N)); c2.y = -c2.y;
-                cur[lay(bb, kk)] = cmul(zc, c2);
+            if (equator) ys = make_double2(0.0, 0.0);
+            if (b == 0 || 2 * b == N) { yn.y = 0.0; ys.y = 0.0; }
+            const double2 zb = make_double2(yn.x - ys.y, yn.y + ys.x);
+            const double2 zc = make_double2(yn.x + ys.y, ys.x - yn.y);           // Z[N - b]
+            if (!blue) {
+                cur[lay((int)perm[b], kk)] = zb;
+                if (b > 0 && 2 * b < N) cur[lay((int)perm[N - b], kk)] = zc;
+            } else {
+                // x_n = conj(c)_n sum_b (Z_b conj(c)_b) c_{n-b}
+                double2 c = __ldg(tw2 + (b * b) % (2 * N)); c.y = -c.y;
+                cur[lay(b, kk)] = cmul(zb, c);
+                if (b > 0 && 2 * b < N) {
+                    const int bb = N - b;
+                    double2 c2 = __ldg(tw2 + (bb * bb) % (2 * N)); c2.y = -c2.y;
+                    cur[lay(bb, kk)] = cmul(zc, c2);
+                }
             }
         }
     }
