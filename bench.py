@@ -25,7 +25,7 @@ import numpy as np
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
-from paper_2208_10154_b200 import inputs  # noqa: E402
+from paper_2208_10154_b200 import inputs, shard  # noqa: E402
 
 METRIC = "maps/sec (analysis+synthesis, FP64) at nside=512 lmax=1535"
 FP64_NOMINAL_TFLOPS = 37.2     # 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz
@@ -195,7 +195,7 @@ def main():
     alm = torch.empty((nmaps, ncomp, nalm), dtype=torch.complex128, device=dev)
     blk = 50
     for k0 in range(0, nmaps, blk):
-        ks = np.arange(k0, min(nmaps, k0 + blk)) + rank * nmaps
+        ks = shard.rank_map_indices(rank, world, nmaps)[k0:min(nmaps, k0 + blk)]
         alm[k0:k0 + len(ks)] = torch.from_numpy(inputs.gaussian_alm(lmax, ks, c["seed"], spin)).to(dev)
     maps = torch.empty((nmaps, ncomp, npix), dtype=torch.float64, device=dev)
     alm_out = torch.empty_like(alm)
@@ -234,10 +234,7 @@ def main():
     launches = plan.kernel_launches() - l0
     stage_ms, stage_n = plan.sht_plan_stage_ms()
     plan.sht_plan_set_timing(False)
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = shard.max_over_ranks(ms_total, dev)
     ms_step = ms_total / args.steps
     value = world * nmaps / (ms_step * 1e-3)
 
@@ -292,10 +289,7 @@ def main():
                 plan.sht_analysis_host(h_maps, h_alm_out)
             torch.cuda.synchronize()
             dt = (time.perf_counter() - t0) / nrep
-            if world > 1:
-                t = torch.tensor([dt], dtype=torch.float64, device=dev)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                dt = float(t.item())
+            dt = shard.max_over_ranks(dt, dev)
             bytes_alm = h_alm.numel() * 16
             bytes_maps = h_maps.numel() * 8
             e2e = {"value": world * nmaps / dt, "unit": "maps/s", "h2d_bytes_per_step": bytes_alm + bytes_maps,
