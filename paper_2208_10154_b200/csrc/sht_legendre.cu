@@ -178,7 +178,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                 const int rs = ls - l0;                             // first row of the tile with a started recurrence
                 mbar_wait(empty + stage, phase ^ 1);
                 double* Ls = reinterpret_cast<double*>(stage_base + (size_t)stage * A_STAGE_BYTES + A_XBYTES) + lane * A_SL;
-#pragma unroll 8
+#pragma unroll 32
                 for (int r = 0; r < A_ML; ++r) {
                     const double2 ab = cft[r];
                     const double t = fma(ab.x * z, x1, -(ab.y * x2));
@@ -338,7 +338,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
             const int rs = ls - lc;
             mbar_wait(empty + stage, phase ^ 1);
             double* Ls = reinterpret_cast<double*>(stage_base + (size_t)stage * S_STAGE_BYTES + S_ABYTES) + rl;
-#pragma unroll 8
+#pragma unroll
             for (int r = 0; r < S_LC; ++r) {
                 const double2 ab = cfw[buf * S_LC + r];
                 const double t = fma(ab.x * z, x1, -(ab.y * x2));

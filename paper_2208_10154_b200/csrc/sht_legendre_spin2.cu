@@ -211,7 +211,7 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                 }
                 double* Ls = reinterpret_cast<double*>(Xs + A2_XBYTES) + (sg * 2 * A2_PC + rr) * A2_SL;
                 const double2* tu = ctu + sg * A2_ML;
-#pragma unroll 4
+#pragma unroll 16
                 for (int r = 0; r < A2_ML; ++r) {
                     const double2 ab = cft[r];
                     const double2 uv = tu[r];
@@ -398,7 +398,7 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
                     tma_load_3d(As + q * (S2_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0, 0);
             }
             double* Ls = reinterpret_cast<double*>(As + S2_ABYTES) + sg * S2_LC * S2_SL + rl;
-#pragma unroll 4
+#pragma unroll
             for (int r = 0; r < S2_LC; ++r) {
                 const double2 ab = cb[r];
                 const double2 uv = cb[S2_LC + r];
