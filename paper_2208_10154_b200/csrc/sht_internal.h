@@ -13,6 +13,7 @@ constexpr int KG = 4;                        // maps per workspace group (one 12
 constexpr int KTILE_MAPS = 64;               // maps per Legendre k-tile (spin 0); spin 2: 32 (Q,U) pairs
 constexpr int NK = 2 * KTILE_MAPS;           // real columns per k-tile (re,im interleaved)
 constexpr int LEG_A_ML = 128;                // l rows per tile of the Legendre analysis kernel
+constexpr int LEG_CS = 16;                   // l granularity of the plan's recurrence-state table
 constexpr int MAX_RADIX_LIST = 16;           // factors of one ring length
 constexpr int RING_THREADS = 256;            // threads per CTA of the ring kernels (two CTAs per SM)
 constexpr int RING_EMAX = 8192;              // most complex elements (ring length x maps) one ring CTA holds in smem
@@ -59,6 +60,11 @@ struct DevicePlan {
     const double2* coef;            // [nalm] (alpha_lm, beta_lm), m-major like alm
     const int* lstart;              // [lmax+1][nh] l_safe(m, p)
     const double2* seed;            // [lmax+1][nh] (lambda_{ls-1}, lambda_{ls-2})
+    // recurrence state (lambda_{b-1}, lambda_{b-2}) at every LEG_CS-th l of every order, b = m + LEG_CS c, exactly as the
+    // running recurrence from l_safe would hold it (the start seed while b <= l_safe): lets several generator warps
+    // work on different l ranges of one ring at the same time.  Index (csoff[m] + c) * nh + p.
+    const double2* cseed;
+    const long long* csoff;         // [lmax+2] chunks before order m
     const double2* spin2c;          // [lmax+1] per-l constants for spin 2 (unused for spin 0)
     const int* mlim;                // [nh] copy of RingPair::mlim (monotone non-decreasing in p)
     const int* pst;                 // [lmax+1][ntile_max] first ring pair that takes part in l tile t of order m
@@ -126,5 +132,6 @@ cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d,
                                             cudaStream_t st);
 // plan-time seed table (sht_plan.cu)
 cudaError_t launch_seed_table(const DevicePlan& d, const double* cm, int* lstart, double2* seed, cudaStream_t st);
+cudaError_t launch_chunk_seeds(const DevicePlan& d, double2* cseed, cudaStream_t st);
 
 }  // namespace sht

@@ -45,15 +45,11 @@ static_assert(2 * S_PB * S_SC * 8 <= S_STAGES * S_STAGE_BYTES, "epilogue staging
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
-                    int nkt, int accumulate, double2* __restrict__ gstate)
+                    int nkt, int accumulate)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
-    // (lambda_{l-1}, lambda_{l-2}) per ring, carried from one l tile to the next: in shared memory, or (when 2 nside
-    // ring pairs x 16 B do not fit beside the stages, nside >= 1024) in a per-CTA global scratch row
-    double2* smem_state = reinterpret_cast<double2*>(smem_raw + A_STAGES * A_STAGE_BYTES);
-    double2* state = gstate ? gstate + (size_t)blockIdx.x * d.nh : smem_state;
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_state + (gstate ? 0 : d.nh));
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + A_STAGES * A_STAGE_BYTES);
     uint64_t* empty = full + A_STAGES;
     double2* cft = reinterpret_cast<double2*>(empty + A_STAGES);                           // (alpha, beta) of the current l tile
     int* pst = reinterpret_cast<int*>(cft + A_ML);                                         // first ring of every l tile
@@ -64,10 +60,9 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     const int comp = 0;
     const int ntile = (lmax - m) / A_ML + 1;
 
-    for (int p = tid; p < nh; p += LEG_THREADS) state[p] = d.seed[(size_t)m * nh + p];
     for (int t = tid; t < ntile; t += LEG_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
     if (tid == 0) {
-        for (int s = 0; s < A_STAGES; ++s) { mbar_init(full + s, 1 + 32); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
+        for (int s = 0; s < A_STAGES; ++s) { mbar_init(full + s, 1 + 64); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
         fence_barrier_init();
         tma_prefetch_desc(&tmF);
     }
@@ -127,67 +122,62 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                 }
             }
         }
-    } else if (warp == LEG_CONSUMER_WARPS) {
-        // ===== TMA producer: the E/O rows of 32 rings x 64 maps per stage =====
-        if (lane == 0) {
-            int stage = 0; uint32_t phase = 0;
-            for (int tile = 0; tile < ntile; ++tile) {
-                for (int pc = pst[tile]; pc < nh; pc += A_PC) {
-                    mbar_wait(empty + stage, phase ^ 1);
-                    unsigned char* Xs = stage_base + (size_t)stage * A_STAGE_BYTES;
-                    mbar_arrive_expect_tx(full + stage, A_XBYTES);
-                    tma_load_4d(Xs, &tmF, full + stage, 0, pc, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
-                    tma_load_4d(Xs + A_XBYTES / 2, &tmF, full + stage, 0, pc + 16, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
-                    if (++stage == A_STAGES) { stage = 0; phase ^= 1; }
-                }
-            }
-        }
-    } else if (warp <= LEG_CONSUMER_WARPS + 2) {
-        // ===== lambda generators: warp w fills the chunks with index = w (mod 2); lane = ring inside the chunk =====
-        const int gw = warp - LEG_CONSUMER_WARPS - 1;
-        const int gl = gw * 32 + lane;                          // 0 .. 63
+    } else {
+        // ===== lambda generators (warps 8..11): warp = (stage it owns) + 2 (half of the tile's 128 l rows); lane = ring of
+        // the chunk.  The recurrence restarts from the plan's state table at l0 and l0 + 64, so the two halves of a
+        // stage are generated at the same time.  Lane 0 of the first-half warp also issues the stage's TMA loads.
+        const int gw = warp - LEG_CONSUMER_WARPS;
+        const int gs = gw & 1, gh = gw >> 1;
+        const int gl = gw * 32 + lane;                          // 0 .. 127 = one l of the tile per thread
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+        const double2* csm = d.cseed + (size_t)d.csoff[m] * nh;
         // (alpha, beta) of an l tile are staged in shared memory once per tile (a dependent global load per
         // recurrence step would cost an L2 round trip per l); rows past lmax get (0, 0)
-        auto load_cf = [&](int l0, int j) -> double2 {
-            const int l = l0 + gl + 64 * j;
+        auto load_cf = [&](int l0) -> double2 {
+            const int l = l0 + gl;
             return l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
         };
-        double2 cf0 = load_cf(m, 0), cf1 = load_cf(m, 1);
+        double2 cf0 = load_cf(m);
         int chunk = 0;
         for (int tile = 0; tile < ntile; ++tile) {
             const int l0 = m + tile * A_ML;
-            // both generator warps are done with the previous tile (its coefficients, and a ring's state written
-            // in the previous l tile may come from the other generator warp)
-            named_bar_sync(1, 64);
-            cft[gl] = cf0; cft[gl + 64] = cf1;
-            named_bar_sync(1, 64);
-            if (tile + 1 < ntile) { cf0 = load_cf(l0 + A_ML, 0); cf1 = load_cf(l0 + A_ML, 1); }
+            named_bar_sync(1, 128);                             // every generator is done with the previous tile
+            cft[gl] = cf0;
+            named_bar_sync(1, 128);
+            if (tile + 1 < ntile) cf0 = load_cf(l0 + A_ML);
+            const int lh = l0 + (A_ML / 2) * gh;                // first l of this warp's half
+            const double2* cst = csm + (size_t)((lh - m) / LEG_CS) * nh;
             for (int pc = pst[tile]; pc < nh; pc += A_PC, ++chunk) {
-                if ((chunk & 1) != gw) continue;
-                const int stage = chunk % A_STAGES;
-                const uint32_t phase = (chunk / A_STAGES) & 1;
+                if ((chunk & 1) != gs) continue;
+                const int stage = gs;
+                const uint32_t phase = (chunk >> 1) & 1;
                 const int p = pc + lane;
                 double x1 = 0.0, x2 = 0.0, z = 0.0;
                 int ls = lmax + 1;
-                if (p < nh) {
-                    const double2 sd = state[p];
+                if (p < nh && lh <= lmax) {
+                    const double2 sd = __ldg(cst + p);
                     x1 = sd.x; x2 = sd.y; z = d.z[p];
                     ls = d.lstart[(size_t)m * nh + p];
                 }
-                const int rs = ls - l0;                             // first row of the tile with a started recurrence
+                const int rs = ls - lh;                             // first row of the half with a started recurrence
                 mbar_wait(empty + stage, phase ^ 1);
-                double* Ls = reinterpret_cast<double*>(stage_base + (size_t)stage * A_STAGE_BYTES + A_XBYTES) + lane * A_SL;
-#pragma unroll 32
-                for (int r = 0; r < A_ML; ++r) {
-                    const double2 ab = cft[r];
+                unsigned char* Xs = stage_base + (size_t)stage * A_STAGE_BYTES;
+                if (gh == 0 && lane == 0) {
+                    mbar_arrive_expect_tx(full + stage, A_XBYTES);
+                    tma_load_4d(Xs, &tmF, full + stage, 0, pc, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
+                    tma_load_4d(Xs + A_XBYTES / 2, &tmF, full + stage, 0, pc + 16, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
+                }
+                double* Ls = reinterpret_cast<double*>(Xs + A_XBYTES) + lane * A_SL + (A_ML / 4) * gh;
+                const double2* cfh = cft + (A_ML / 2) * gh;
+#pragma unroll 16
+                for (int r = 0; r < A_ML / 2; ++r) {
+                    const double2 ab = cfh[r];
                     const double t = fma(ab.x * z, x1, -(ab.y * x2));
                     const bool on = r >= rs;
                     const double v = on ? t : 0.0;
                     x2 = on ? x1 : x2; x1 = on ? t : x1;
                     Ls[(r & 1) * (A_PC * A_SL) + (r >> 1)] = v;
                 }
-                if (p < nh) state[p] = make_double2(x1, x2);
                 mbar_arrive(full + stage);
             }
         }
@@ -206,7 +196,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
     unsigned char* stage_base = smem_raw;
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S_STAGES * S_STAGE_BYTES);
     uint64_t* empty = full + S_STAGES;
-    double2* cfs = reinterpret_cast<double2*>(empty + S_STAGES);      // 2 generator warps x 2 buffers x S_LC (alpha, beta)
+    double2* cfs = reinterpret_cast<double2*>(empty + S_STAGES);      // 4 generator warps x 2 buffers x S_LC/2 (alpha, beta)
     int* lmin_s = reinterpret_cast<int*>(cfs + 4 * S_LC);
 
     // block order: m slowest (long m first), then ring block, k-tile fastest
@@ -221,7 +211,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
     if (m >= d.mlim[plast]) return;                    // no ring of this block takes part in order m (never read)
 
     if (tid == 0) {
-        for (int s = 0; s < S_STAGES; ++s) { mbar_init(full + s, 1 + 64); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
+        for (int s = 0; s < S_STAGES; ++s) { mbar_init(full + s, 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
         fence_barrier_init();
         tma_prefetch_desc(&tmA);
         *lmin_s = lmax + 1;
@@ -294,53 +284,52 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
             dst[0] = make_double2(ee.x + oo.x, ee.y + oo.y);
             dst[KG] = make_double2(ee.x - oo.x, ee.y - oo.y);
         }
-    } else if (warp == LEG_CONSUMER_WARPS) {
-        // ===== TMA producer: a_lm of 32 l x 64 maps per stage, straight from the m-major ABI layout =====
-        if (lane == 0) {
-            int stage = 0; uint32_t phase = 0;
-            const int row0 = (k0 + kt * KTILE_MAPS) * d.ncomp + comp;
-            for (int lc = cfirst; lc <= lmax; lc += S_LC) {
-                mbar_wait(empty + stage, phase ^ 1);
-                unsigned char* As = stage_base + (size_t)stage * S_STAGE_BYTES;
+    } else {
+        // ===== lambda generators (warps 8..11): warp = (half of the block's 64 rings) + 2 (half of the stage's 32 l);
+        // the recurrence restarts from the plan's state table every 16 l, so the two l halves of a stage are generated
+        // at the same time.  Lane 0 of generator 0 also issues the stage's TMA loads (a_lm, straight from the m-major
+        // ABI layout).
+        const int gw = warp - LEG_CONSUMER_WARPS;
+        const int gh = gw >> 1;
+        const int rl = (gw & 1) * 32 + lane;
+        const int p = pb + rl;
+        double z = 0.0;
+        int ls = lmax + 1;
+        if (p < nh) { ls = d.lstart[(size_t)m * nh + p]; z = d.z[p]; }
+        const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+        const double2* csm = d.cseed + (size_t)d.csoff[m] * nh + (p < nh ? p : 0);
+        constexpr int HL = S_LC / 2;                            // l per warp and stage
+        // (alpha, beta) and the start state of the next stage are fetched while the current one is computed
+        double2* cfw = cfs + gw * (2 * HL);
+        auto load_cf = [&](int lb) -> double2 {
+            const int l = lb + (lane & (HL - 1));
+            return l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+        };
+        auto load_state = [&](int lb) -> double2 {
+            return (p < nh && lb <= lmax) ? __ldg(csm + (size_t)((lb - m) / LEG_CS) * nh) : make_double2(0.0, 0.0);
+        };
+        double2 cf = load_cf(cfirst + HL * gh), sd = load_state(cfirst + HL * gh);
+        int stage = 0, buf = 0; uint32_t phase = 0;
+        const int row0 = (k0 + kt * KTILE_MAPS) * d.ncomp + comp;
+        for (int lc = cfirst; lc <= lmax; lc += S_LC) {
+            const int lb = lc + HL * gh;
+            if (lane < HL) cfw[buf * HL + lane] = cf;
+            __syncwarp();
+            double x1 = sd.x, x2 = sd.y;
+            cf = load_cf(lb + S_LC); sd = load_state(lb + S_LC);
+            const int rs = ls - lb;
+            mbar_wait(empty + stage, phase ^ 1);
+            unsigned char* As = stage_base + (size_t)stage * S_STAGE_BYTES;
+            if (gw == 0 && lane == 0) {
                 mbar_arrive_expect_tx(full + stage, S_ABYTES);
 #pragma unroll
                 for (int q = 0; q < 4; ++q)
                     tma_load_2d(As + q * (S_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0);
-                if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
             }
-        }
-    } else if (warp <= LEG_CONSUMER_WARPS + 2) {
-        // ===== lambda generators: 64 lanes = the 64 rings of the block, recurrence state in registers =====
-        const int gw = warp - LEG_CONSUMER_WARPS - 1;
-        const int rl = gw * 32 + lane;
-        const int p = pb + rl;
-        double x1 = 0.0, x2 = 0.0, z = 0.0;
-        int ls = lmax + 1;
-        if (p < nh) {
-            const double2 sd = d.seed[(size_t)m * nh + p];
-            x1 = sd.x; x2 = sd.y; ls = d.lstart[(size_t)m * nh + p]; z = d.z[p];
-        }
-        const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
-        // (alpha, beta) of the next l chunk are fetched by the 32 lanes in one coalesced load while the current chunk
-        // is computed, and handed round through a per-warp shared buffer (a dependent global load per recurrence
-        // step would cost an L2 round trip per l)
-        double2* cfw = cfs + gw * (2 * S_LC);
-        auto load_cf = [&](int lc) -> double2 {
-            const int l = lc + lane;
-            return l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
-        };
-        double2 cf = load_cf(cfirst);
-        int stage = 0, buf = 0; uint32_t phase = 0;
-        for (int lc = cfirst; lc <= lmax; lc += S_LC) {
-            cfw[buf * S_LC + lane] = cf;
-            __syncwarp();
-            cf = load_cf(lc + S_LC);
-            const int rs = ls - lc;
-            mbar_wait(empty + stage, phase ^ 1);
-            double* Ls = reinterpret_cast<double*>(stage_base + (size_t)stage * S_STAGE_BYTES + S_ABYTES) + rl;
+            double* Ls = reinterpret_cast<double*>(As + S_ABYTES) + (HL * gh) * S_SL + rl;
 #pragma unroll
-            for (int r = 0; r < S_LC; ++r) {
-                const double2 ab = cfw[buf * S_LC + r];
+            for (int r = 0; r < HL; ++r) {
+                const double2 ab = cfw[buf * HL + r];
                 const double t = fma(ab.x * z, x1, -(ab.y * x2));
                 const bool on = r >= rs;
                 const double v = on ? t : 0.0;
@@ -364,16 +353,17 @@ static cudaError_t make_tmap_alm(const DevicePlan& d, const double* alm, long lo
     return make_tmap_f64(tm, alm, 2, dims, strides, box);
 }
 
-static size_t analysis_smem(int nh, int ntile, bool state_in_smem = true)
+static size_t analysis_smem(int ntile)
 {
-    return (size_t)A_STAGES * A_STAGE_BYTES + (state_in_smem ? (size_t)nh * sizeof(double2) : 0) + 2 * A_STAGES * sizeof(uint64_t) +
-           (size_t)A_ML * sizeof(double2) + (size_t)ntile * sizeof(int);
+    return (size_t)A_STAGES * A_STAGE_BYTES + 2 * A_STAGES * sizeof(uint64_t) + (size_t)A_ML * sizeof(double2) +
+           (size_t)ntile * sizeof(int);
 }
 static size_t synthesis_smem() { return (size_t)S_STAGES * S_STAGE_BYTES + 2 * S_STAGES * sizeof(uint64_t) + 4 * S_LC * sizeof(double2) + 16; }
 
 size_t legendre_smem_bytes(int nh, int ntile_max)
 {
-    const size_t a = analysis_smem(nh, ntile_max), s = synthesis_smem();
+    const size_t a = analysis_smem(ntile_max), s = synthesis_smem();
+    (void)nh;
     return a > s ? a : s;
 }
 
@@ -383,23 +373,14 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
     if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const unsigned grid = (unsigned)((d.lmax + 1) * nkt);
-    size_t sm = analysis_smem(d.nh, d.ntile_max);
-    double2* gstate = nullptr;
-    cudaError_t e;
-    if (sm > (size_t)227 * 1024) {
-        sm = analysis_smem(d.nh, d.ntile_max, false);
-        if ((e = cudaMallocAsync((void**)&gstate, (size_t)grid * d.nh * sizeof(double2), st)) != cudaSuccess) return e;
-    }
-    e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    const size_t sm = analysis_smem(d.ntile_max);
+    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
     CUtensorMap tmF;
-    if (e == cudaSuccess) e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, &tmF);
-    if (e == cudaSuccess) {
-        k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, gstate);
-        pl->launches++;
-        e = cudaGetLastError();
-    }
-    if (gstate) cudaFreeAsync(gstate, st);
-    return e;
+    if ((e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, &tmF)) != cudaSuccess) return e;
+    k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
+    pl->launches++;
+    return cudaGetLastError();
 }
 
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st)

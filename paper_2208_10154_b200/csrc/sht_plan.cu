@@ -69,6 +69,39 @@ __global__ void k_seed_table(DevicePlan d, const double* __restrict__ cm, int* _
     seed[gid] = make_double2(x1, x2);
 }
 
+// Recurrence state at every LEG_CS-th l (DevicePlan::cseed): the same arithmetic, in the same order, as the
+// generator warps of the Legendre kernels, so a chain restarted from a table entry reproduces the sequential chain
+// bit for bit.
+__global__ void k_chunk_seeds(DevicePlan d, double2* __restrict__ cseed)
+{
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)(d.lmax + 1) * d.nh;
+    if (gid >= total) return;
+    const int m = (int)(gid / d.nh), p = (int)(gid % d.nh);
+    const double z = d.z[p];
+    const double2 sd = d.seed[gid];
+    double x1 = sd.x, x2 = sd.y;
+    const int ls = d.lstart[gid];
+    const double2* cf = d.coef + ((long long)m * (2 * d.lmax + 1 - m) / 2);
+    double2* out = cseed + (size_t)d.csoff[m] * d.nh + p;
+    for (int l = m; l <= d.lmax; ++l) {
+        if (((l - m) & (LEG_CS - 1)) == 0) { *out = make_double2(x1, x2); out += d.nh; }
+        if (l >= ls) {
+            const double2 ab = cf[l];
+            const double t = fma(ab.x * z, x1, -(ab.y * x2));
+            x2 = x1; x1 = t;
+        }
+    }
+}
+
+cudaError_t launch_chunk_seeds(const DevicePlan& d, double2* cseed, cudaStream_t st)
+{
+    const long long total = (long long)(d.lmax + 1) * d.nh;
+    const int bs = 128;
+    k_chunk_seeds<<<(unsigned)((total + bs - 1) / bs), bs, 0, st>>>(d, cseed);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_seed_table(const DevicePlan& d, const double* cm, int* lstart, double2* seed, cudaStream_t st)
 {
     const long long total = (long long)(d.lmax + 1) * d.nh;
@@ -391,6 +424,22 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
         ce = launch_seed_table(d, d_cm, ls, sd, 0);
         if (ce == cudaSuccess) ce = cudaDeviceSynchronize();
         if (ce != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
+
+        // recurrence state every LEG_CS-th l
+        {
+            std::vector<long long> csoff(lmax + 2, 0);
+            for (int m = 0; m <= lmax; ++m) csoff[m + 1] = csoff[m] + (lmax - m) / LEG_CS + 1;
+            if (upload(pl, csoff, &d.csoff) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+            const size_t bytes = (size_t)csoff[lmax + 1] * d.nh * sizeof(double2);
+            double2* cs = nullptr;
+            if (cudaMalloc(&cs, bytes) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+            pl->dev_allocs[pl->n_allocs++] = cs;
+            pl->table_bytes += bytes;
+            d.cseed = cs;
+            ce = launch_chunk_seeds(d, cs, 0);
+            if (ce == cudaSuccess) ce = cudaDeviceSynchronize();
+            if (ce != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
+        }
 
         // ring optimisation (item 10): ring p takes part in order m only if lambda_lm(theta_p) reaches
         // the threshold for some l <= lmax, i.e. l_safe(m, p) <= lmax.  mlim[p] = 1 + the largest such m, made
