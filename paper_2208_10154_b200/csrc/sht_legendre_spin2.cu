@@ -59,12 +59,12 @@ __device__ __forceinline__ void spin2_consts(const DevicePlan& d, int l, int m, 
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
-                          int nkt, int accumulate, int nst)
+                          int nkt, int accumulate)
 {
+    constexpr int nst = 3;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
-    double2* state = reinterpret_cast<double2*>(smem_raw + (size_t)nst * A2_STAGE_BYTES);   // (lambda_{l-1}, lambda_{l-2}) per ring
-    uint64_t* full = reinterpret_cast<uint64_t*>(state + d.nh);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)nst * A2_STAGE_BYTES);
     uint64_t* empty = full + 4;
     double2* cft = reinterpret_cast<double2*>(empty + 4);        // (alpha, beta) of the current l tile
     double2* ctu = cft + A2_ML;                                  // [sign][l]: (t1, t2) / (t4, 0)
@@ -76,10 +76,9 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
     const int lmax = d.lmax, nh = d.nh;
     const int ntile = (lmax - m) / A2_ML + 1;
 
-    for (int p = tid; p < nh; p += LEG2_THREADS) state[p] = d.seed[(size_t)m * nh + p];
     for (int t = tid; t < ntile; t += LEG2_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
     if (tid == 0) {
-        for (int s = 0; s < nst; ++s) { mbar_init(full + s, 1 + 32); mbar_init(empty + s, LEG_CONSUMER_WARPS_S2); }
+        for (int s = 0; s < nst; ++s) { mbar_init(full + s, 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS_S2); }
         fence_barrier_init();
         tma_prefetch_desc(&tmF);
     }
@@ -155,67 +154,59 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
             }
         }
     } else {
-        // ===== generators (warps 8 .. 8+nst-1): generator g owns stage g, i.e. the chunks c = g (mod nst) -- a warp that
-        // ran further ahead than the number of stages would defeat the parity waits; lane = (ring 0..15) + 16 (sign of F).
-        // Lane 0 also issues the TMA load of the chunk's Q / iU lines as soon as the stage is free.
+        // ===== generators (warps 8..11): every warp works on every chunk, warp g on the l rows [32 g, 32 g + 32) of the
+        // tile (the recurrence restarts from the plan's state table every 16 l); lane = (ring 0..15) + 16 (sign of F).
+        // Lane 0 of generator 0 also issues the TMA load of the chunk's Q / iU lines as soon as the stage is free.
         const int gw = warp - 8;
-        if (gw >= nst) return;
-        const int ngen = nst * 32;
         const int rr = lane & 15, sg = lane >> 4;
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
-        // per-l constants of the next tile: generators 0 and 1 fetch 64 l each while the current tile is computed
-        const int gl = gw * 64 + lane;
-        auto load_consts = [&](int l0, int j, double2& ab, double2& tp, double2& tm, double& t3) {
-            const int l = l0 + gl + 32 * j;
-            ab = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
-            spin2_consts(d, l, m, tp, tm, t3);
+        const double2* csm = d.cseed + (size_t)d.csoff[m] * nh;
+        constexpr int QL = A2_ML / 4;                           // l rows per generator warp
+        // per-l constants of the next tile: one l per generator thread, fetched while the current tile is computed
+        const int gl = gw * 32 + lane;
+        double2 nab, ntp, ntm; double nt3;
+        auto load_consts = [&](int l0) {
+            const int l = l0 + gl;
+            nab = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+            spin2_consts(d, l, m, ntp, ntm, nt3);
         };
-        double2 nab[2], ntp[2], ntm[2]; double nt3[2];
-        if (gw < 2) { load_consts(m, 0, nab[0], ntp[0], ntm[0], nt3[0]); load_consts(m, 1, nab[1], ntp[1], ntm[1], nt3[1]); }
-        int chunk = 0;
+        load_consts(m);
+        int stage = 0; uint32_t phase = 0;
         for (int tile = 0; tile < ntile; ++tile) {
             const int l0 = m + tile * A2_ML;
-            named_bar_sync(1, ngen);                            // every generator is done with the previous tile
-            if (gw < 2) {
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const int i = gl + 32 * j;
-                    cft[i] = nab[j]; ctu[i] = ntp[j]; ctu[A2_ML + i] = ntm[j]; ct3[i] = nt3[j];
-                }
-            }
-            named_bar_sync(1, ngen);
-            if (gw < 2 && tile + 1 < ntile) {
-                load_consts(l0 + A2_ML, 0, nab[0], ntp[0], ntm[0], nt3[0]);
-                load_consts(l0 + A2_ML, 1, nab[1], ntp[1], ntm[1], nt3[1]);
-            }
-            for (int pc = pst[tile]; pc < nh; pc += A2_PC, ++chunk) {
-                const int stage = chunk % nst;
-                if (stage != gw) continue;
-                const uint32_t phase = (chunk / nst) & 1;
+            named_bar_sync(1, 128);                             // every generator is done with the previous tile
+            cft[gl] = nab; ctu[gl] = ntp; ctu[A2_ML + gl] = ntm; ct3[gl] = nt3;
+            named_bar_sync(1, 128);
+            if (tile + 1 < ntile) load_consts(l0 + A2_ML);
+            const int lq = l0 + QL * gw;                        // first l of this warp's quarter
+            const double2* cst = csm + (size_t)((lq - m) / LEG_CS) * nh;
+            for (int pc = pst[tile]; pc < nh; pc += A2_PC) {
                 const int p = pc + rr;
                 double x1 = 0.0, x2 = 0.0, z = 0.0, is2 = 0.0;
                 int ls = lmax + 1;
-                if (p < nh) {
-                    const double2 sd = state[p];
+                if (p < nh && lq <= lmax) {
+                    const double2 sd = __ldg(cst + p);
                     x1 = sd.x; x2 = sd.y; z = d.z[p]; is2 = 1.0 / d.sin2[p];
                     ls = d.lstart[(size_t)m * nh + p];
                 }
                 const double ra = sg ? (double)m * z * is2 : is2;       // multiplies t1 (F+) / t4 (F-)
                 const double rc = sg ? (double)m * is2 : z * is2;       // multiplies t3
-                const int rs = ls - l0;
+                const int rs = ls - lq;
                 mbar_wait(empty + stage, phase ^ 1);
                 unsigned char* Xs = stage_base + (size_t)stage * A2_STAGE_BYTES;
-                if (lane == 0) {
+                if (gw == 0 && lane == 0) {
                     mbar_arrive_expect_tx(full + stage, A2_XBYTES);
                     tma_load_4d(Xs, &tmF, full + stage, 0, pc, kt * P_KG, m * 2);
                 }
-                double* Ls = reinterpret_cast<double*>(Xs + A2_XBYTES) + (sg * 2 * A2_PC + rr) * A2_SL;
-                const double2* tu = ctu + sg * A2_ML;
-#pragma unroll 16
-                for (int r = 0; r < A2_ML; ++r) {
-                    const double2 ab = cft[r];
+                double* Ls = reinterpret_cast<double*>(Xs + A2_XBYTES) + (sg * 2 * A2_PC + rr) * A2_SL + (QL / 2) * gw;
+                const double2* cfq = cft + QL * gw;
+                const double2* tu = ctu + sg * A2_ML + QL * gw;
+                const double* t3q = ct3 + QL * gw;
+#pragma unroll 8
+                for (int r = 0; r < QL; ++r) {
+                    const double2 ab = cfq[r];
                     const double2 uv = tu[r];
-                    const double t3 = ct3[r];
+                    const double t3 = t3q[r];
                     const double lam = fma(ab.x * z, x1, -(ab.y * x2));
                     const double U = fma(uv.x, ra, uv.y), W = t3 * rc;
                     const double f = fma(lam, U, -(x1 * W));             // x1 = lambda_{l-1}
@@ -223,8 +214,8 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                     x2 = on ? x1 : x2; x1 = on ? lam : x1;
                     Ls[(r & 1) * (A2_PC * A2_SL) + (r >> 1)] = on ? f : 0.0;
                 }
-                if (sg == 0 && p < nh) state[p] = make_double2(x1, x2);
                 mbar_arrive(full + stage);
+                if (++stage == nst) { stage = 0; phase ^= 1; }
             }
         }
     }
@@ -356,39 +347,44 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
             dst[KG] = make_double2(ev.x - od.x, ev.y - od.y);
         }
     } else {
-        // ===== generators (warps 8..11): warp = (sign of F) x (half of the 64 rings), recurrence state in registers;
-        // lane 0 of generator 0 issues the TMA loads of a_E / a_B for the stage
+        // ===== generators (warps 8..11): warp = (half of the 64 rings) + 2 (half of the stage's 32 l); a lane forms F+
+        // and F- of its ring; the recurrence restarts from the plan's state table every 16 l.  Lane 0 of generator 0
+        // issues the TMA loads of a_E / a_B for the stage.
         const int gw = warp - 8;
-        const int sg = gw >> 1;
+        const int gh = gw >> 1;
         const int rl = (gw & 1) * 32 + lane;
         const int p = pb + rl;
-        double x1 = 0.0, x2 = 0.0, z = 0.0, is2 = 0.0;
+        double z = 0.0, is2 = 0.0;
         int ls = lmax + 1;
-        if (p < nh) {
-            const double2 sd = d.seed[(size_t)m * nh + p];
-            x1 = sd.x; x2 = sd.y; ls = d.lstart[(size_t)m * nh + p]; z = d.z[p]; is2 = 1.0 / d.sin2[p];
-        }
-        const double ra = sg ? (double)m * z * is2 : is2;
-        const double rc = sg ? (double)m * is2 : z * is2;
+        if (p < nh) { ls = d.lstart[(size_t)m * nh + p]; z = d.z[p]; is2 = 1.0 / d.sin2[p]; }
+        const double rap = is2, rcp = z * is2;                               // F+: multiply t1, t3
+        const double ram = (double)m * z * is2, rcm = (double)m * is2;       // F-: multiply t4, t3
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
-        double2* cfw = cfs + gw * (2 * S2_LC * 3);
-        double2 nab, nuv; double nt3;
-        auto load_consts = [&](int lc) {
-            const int l = lc + lane;
+        const double2* csm = d.cseed + (size_t)d.csoff[m] * nh + (p < nh ? p : 0);
+        constexpr int HL = S2_LC / 2;                           // l per warp and stage
+        double2* cfw = cfs + gw * (2 * HL * 3);
+        double2 nab, ntp, ntm; double nt3;
+        auto load_consts = [&](int lb) {
+            const int l = lb + (lane & (HL - 1));
             nab = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
-            double2 tp, tm;
-            spin2_consts(d, l, m, tp, tm, nt3);
-            nuv = sg ? tm : tp;
+            spin2_consts(d, l, m, ntp, ntm, nt3);
         };
-        load_consts(cfirst);
+        auto load_state = [&](int lb) -> double2 {
+            return (p < nh && lb <= lmax) ? __ldg(csm + (size_t)((lb - m) / LEG_CS) * nh) : make_double2(0.0, 0.0);
+        };
+        load_consts(cfirst + HL * gh);
+        double2 sd = load_state(cfirst + HL * gh);
         int stage = 0, buf = 0; uint32_t phase = 0;
         const int row0 = k0 + kt * P_KT;
         for (int lc = cfirst; lc <= lmax; lc += S2_LC) {
-            double2* cb = cfw + buf * (S2_LC * 3);
-            cb[lane] = nab; cb[S2_LC + lane] = nuv; cb[2 * S2_LC + lane] = make_double2(nt3, 0.0);
+            const int lb = lc + HL * gh;
+            double2* cb = cfw + buf * (HL * 3);
+            if (lane < HL) { cb[lane] = nab; cb[HL + lane] = make_double2(ntp.x, ntp.y); cb[2 * HL + lane] = make_double2(ntm.x, nt3); }
             __syncwarp();
-            load_consts(lc + S2_LC);
-            const int rs = ls - lc;
+            double x1 = sd.x, x2 = sd.y;
+            load_consts(lb + S2_LC);
+            sd = load_state(lb + S2_LC);
+            const int rs = ls - lb;
             mbar_wait(empty + stage, phase ^ 1);
             unsigned char* As = stage_base + (size_t)stage * S2_STAGE_BYTES;
             if (gw == 0 && lane == 0) {
@@ -397,18 +393,20 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
                 for (int q = 0; q < 4; ++q)
                     tma_load_3d(As + q * (S2_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0, 0);
             }
-            double* Ls = reinterpret_cast<double*>(As + S2_ABYTES) + sg * S2_LC * S2_SL + rl;
+            double* Lp = reinterpret_cast<double*>(As + S2_ABYTES) + (HL * gh) * S2_SL + rl;
+            double* Lm = Lp + S2_LC * S2_SL;
 #pragma unroll
-            for (int r = 0; r < S2_LC; ++r) {
+            for (int r = 0; r < HL; ++r) {
                 const double2 ab = cb[r];
-                const double2 uv = cb[S2_LC + r];
-                const double t3 = cb[2 * S2_LC + r].x;
+                const double2 tp = cb[HL + r];                  // (t1, t2)
+                const double2 tm = cb[2 * HL + r];              // (t4, t3)
                 const double lam = fma(ab.x * z, x1, -(ab.y * x2));
-                const double U = fma(uv.x, ra, uv.y), W = t3 * rc;
-                const double f = fma(lam, U, -(x1 * W));
+                const double fp = fma(lam, fma(tp.x, rap, tp.y), -(x1 * (tm.y * rcp)));      // x1 = lambda_{l-1}
+                const double fm = fma(lam, tm.x * ram, -(x1 * (tm.y * rcm)));
                 const bool on = r >= rs;
                 x2 = on ? x1 : x2; x1 = on ? lam : x1;
-                Ls[r * S2_SL] = on ? f : 0.0;
+                Lp[r * S2_SL] = on ? fp : 0.0;
+                Lm[r * S2_SL] = on ? fm : 0.0;
             }
             mbar_arrive(full + stage);
             buf ^= 1;
@@ -428,10 +426,10 @@ static cudaError_t make_tmap_alm_spin2(const DevicePlan& d, const double* alm, l
     return make_tmap_f64(tm, alm, 3, dims, strides, box);
 }
 
-static size_t analysis2_smem(int nh, int ntile, int nst)
+static size_t analysis2_smem(int ntile)
 {
-    return (size_t)nst * A2_STAGE_BYTES + (size_t)nh * sizeof(double2) + 8 * sizeof(uint64_t) +
-           (size_t)A2_ML * (3 * sizeof(double2) + sizeof(double)) + (size_t)ntile * sizeof(int);
+    return (size_t)3 * A2_STAGE_BYTES + 8 * sizeof(uint64_t) + (size_t)A2_ML * (3 * sizeof(double2) + sizeof(double)) +
+           (size_t)ntile * sizeof(int);
 }
 static size_t synthesis2_smem()
 {
@@ -441,16 +439,13 @@ static size_t synthesis2_smem()
 cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                            bool accumulate, cudaStream_t st)
 {
-    int nst = 3;
-    if (analysis2_smem(d.nh, d.ntile_max, nst) > (size_t)227 * 1024) nst = 2;
-    const size_t sm = analysis2_smem(d.nh, d.ntile_max, nst);
-    if (sm > (size_t)227 * 1024) return cudaErrorInvalidConfiguration;
+    const size_t sm = analysis2_smem(d.ntile_max);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis_spin2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tmF;
     if ((e = make_tmap_F(d, F, P_KG, 2, &tmF)) != cudaSuccess) return e;
     const int nkt = (kmaps + P_KT - 1) / P_KT;
-    k_legendre_analysis_spin2<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, nst);
+    k_legendre_analysis_spin2<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
 }
