@@ -53,6 +53,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     uint64_t* empty = full + A_STAGES;
     double2* cft = reinterpret_cast<double2*>(empty + A_STAGES);                           // (alpha, beta) of the current l tile
     int* pst = reinterpret_cast<int*>(cft + A_ML);                                         // first ring of every l tile
+    int* i0s = pst + ((d.ntile_max + 3) & ~3);                                               // per stage: first 16-row block with a started recurrence
 
     const int m = blockIdx.x / nkt, kt = blockIdx.x % nkt;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -85,21 +86,44 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                 mbar_wait(full + stage, phase);
                 const double* Xs = reinterpret_cast<const double*>(stage_base + (size_t)stage * A_STAGE_BYTES);
                 const double* Ls = Xs + A_XBYTES / 8 + cls * (A_PC * A_SL);
+                // rows below the chunk's smallest l_safe hold lambda = 0: their 16-row blocks (i < i0) are skipped
+                const int i0 = i0s[stage];
+                if (i0 == 0) {
 #pragma unroll
-                for (int ks = 0; ks < A_PC / 4; ++ks) {
-                    const int sub = ks >> 2, ksl = ks & 3;
-                    const int pl = 8 * (ksl >> 1) + 2 * t + (ksl & 1);        // ring inside the 16-ring box
-                    double a[8], b[4];
-                    const double* La = Ls + (16 * sub + pl) * A_SL + g;
+                    for (int ks = 0; ks < A_PC / 4; ++ks) {
+                        const int sub = ks >> 2, ksl = ks & 3;
+                        const int pl = 8 * (ksl >> 1) + 2 * t + (ksl & 1);        // ring inside the 16-ring box
+                        double a[8], b[4];
+                        const double* La = Ls + (16 * sub + pl) * A_SL + g;
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
-                    const double* Xb = Xs + sub * 4096 + pl * 16 + ((((4 * cls + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
+                        for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
+                        const double* Xb = Xs + sub * 4096 + pl * 16 + ((((4 * cls + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) b[j] = Xb[(4 * wn + j) * 256];
+                        for (int j = 0; j < 4; ++j) b[j] = Xb[(4 * wn + j) * 256];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i)
+                        for (int i = 0; i < 8; ++i)
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
+                            for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
+                    }
+                } else {
+#pragma unroll
+                    for (int ks = 0; ks < A_PC / 4; ++ks) {
+                        const int sub = ks >> 2, ksl = ks & 3;
+                        const int pl = 8 * (ksl >> 1) + 2 * t + (ksl & 1);
+                        double b[4];
+                        const double* La = Ls + (16 * sub + pl) * A_SL + g;
+                        const double* Xb = Xs + sub * 4096 + pl * 16 + ((((4 * cls + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) b[j] = Xb[(4 * wn + j) * 256];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            if (i >= i0) {
+                                const double a = La[8 * i];
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a, b[j]);
+                            }
+                        }
+                    }
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty + stage);
@@ -160,9 +184,13 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                     ls = d.lstart[(size_t)m * nh + p];
                 }
                 const int rs = ls - lh;                             // first row of the half with a started recurrence
+                int lsmin = ls;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) lsmin = min(lsmin, __shfl_xor_sync(0xffffffffu, lsmin, o));
                 mbar_wait(empty + stage, phase ^ 1);
                 unsigned char* Xs = stage_base + (size_t)stage * A_STAGE_BYTES;
                 if (gh == 0 && lane == 0) {
+                    i0s[stage] = max(0, min(8, (lsmin - l0) >> 4));
                     mbar_arrive_expect_tx(full + stage, A_XBYTES);
                     tma_load_4d(Xs, &tmF, full + stage, 0, pc, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
                     tma_load_4d(Xs + A_XBYTES / 2, &tmF, full + stage, 0, pc + 16, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
@@ -198,6 +226,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
     uint64_t* empty = full + S_STAGES;
     double2* cfs = reinterpret_cast<double2*>(empty + S_STAGES);      // 4 generator warps x 2 buffers x S_LC/2 (alpha, beta)
     int* lmin_s = reinterpret_cast<int*>(cfs + 4 * S_LC);
+    int* minls8 = lmin_s + 4;                                         // smallest l_safe of every 8-ring row block
 
     // block order: m slowest (long m first), then ring block, k-tile fastest
     const int kt = blockIdx.x % nkt;
@@ -216,8 +245,13 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
         tma_prefetch_desc(&tmA);
         *lmin_s = lmax + 1;
     }
+    if (tid < 8) minls8[tid] = lmax + 1;
     __syncthreads();
-    if (tid < S_PB && pb + tid < nh) atomicMin(lmin_s, d.lstart[(size_t)m * nh + pb + tid]);
+    if (tid < S_PB && pb + tid < nh) {
+        const int lsv = d.lstart[(size_t)m * nh + pb + tid];
+        atomicMin(lmin_s, lsv);
+        atomicMin(minls8 + (tid >> 3), lsv);
+    }
     __syncthreads();
     const int lmin = *lmin_s;
     // chunks are aligned to m so that (l - m) even <-> even local index
@@ -239,22 +273,52 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
             mbar_wait(full + stage, phase);
             const double* As = reinterpret_cast<const double*>(stage_base + (size_t)stage * S_STAGE_BYTES);
             const double* Ls = As + S_ABYTES / 8;
+            // 8-ring row blocks whose recurrences all start after this stage hold lambda = 0: skipped
+            unsigned act = 0;
+            {
+                const int4 q0 = *reinterpret_cast<const int4*>(minls8), q1 = *reinterpret_cast<const int4*>(minls8 + 4);
+                const int lend = lc + S_LC - 1;
+                act = (q0.x <= lend ? 1u : 0u) | (q0.y <= lend ? 2u : 0u) | (q0.z <= lend ? 4u : 0u) | (q0.w <= lend ? 8u : 0u) |
+                      (q1.x <= lend ? 16u : 0u) | (q1.y <= lend ? 32u : 0u) | (q1.z <= lend ? 64u : 0u) | (q1.w <= lend ? 128u : 0u);
+            }
+            if (act == 0xffu) {
 #pragma unroll
-            for (int ks = 0; ks < S_LC / 8; ++ks) {
-                double a[8], b[4];
-                const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
+                for (int ks = 0; ks < S_LC / 8; ++ks) {
+                    double a[8], b[4];
+                    const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
 #pragma unroll
-                for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
+                    for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int row = 16 * wn + 4 * j + (g >> 1);               // map inside the k-tile
-                    const double v = As[ks * 1024 + row * 16 + ((((2 * t + cls) ^ (row & 7)) << 1) | (g & 1))];
-                    b[j] = kill_im ? 0.0 : v;
+                    for (int j = 0; j < 4; ++j) {
+                        const int row = 16 * wn + 4 * j + (g >> 1);               // map inside the k-tile
+                        const double v = As[ks * 1024 + row * 16 + ((((2 * t + cls) ^ (row & 7)) << 1) | (g & 1))];
+                        b[j] = kill_im ? 0.0 : v;
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
                 }
+            } else {
 #pragma unroll
-                for (int i = 0; i < 8; ++i)
+                for (int ks = 0; ks < S_LC / 8; ++ks) {
+                    double b[4];
+                    const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
+                    for (int j = 0; j < 4; ++j) {
+                        const int row = 16 * wn + 4 * j + (g >> 1);
+                        const double v = As[ks * 1024 + row * 16 + ((((2 * t + cls) ^ (row & 7)) << 1) | (g & 1))];
+                        b[j] = kill_im ? 0.0 : v;
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        if (act & (1u << i)) {
+                            const double a = La[8 * i];
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a, b[j]);
+                        }
+                    }
+                }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty + stage);
@@ -356,9 +420,9 @@ static cudaError_t make_tmap_alm(const DevicePlan& d, const double* alm, long lo
 static size_t analysis_smem(int ntile)
 {
     return (size_t)A_STAGES * A_STAGE_BYTES + 2 * A_STAGES * sizeof(uint64_t) + (size_t)A_ML * sizeof(double2) +
-           (size_t)ntile * sizeof(int);
+           (size_t)((ntile + 3) & ~3) * sizeof(int) + 16;
 }
-static size_t synthesis_smem() { return (size_t)S_STAGES * S_STAGE_BYTES + 2 * S_STAGES * sizeof(uint64_t) + 4 * S_LC * sizeof(double2) + 16; }
+static size_t synthesis_smem() { return (size_t)S_STAGES * S_STAGE_BYTES + 2 * S_STAGES * sizeof(uint64_t) + 4 * S_LC * sizeof(double2) + 64; }
 
 size_t legendre_smem_bytes(int nh, int ntile_max)
 {

@@ -174,9 +174,8 @@ __device__ __forceinline__ void dif_stage16(double2* buf, int N, int L, int kt, 
 #pragma unroll
         for (int c = 0; c < 16; ++c) u[c] = GIN ? ld(e0 + c * M, kk) : buf[lay(e0 + c * M, kk)];
         double2 ta[4], tb[4];
-        if (M > 1) {
-#pragma unroll
-            for (int s = 1; s < 4; ++s) ta[s] = twiddle<false>(tw2, j * s * tstep);
+        if (M > 1) {                                       // one table read; the other powers by multiplication
+            ta[1] = twiddle<false>(tw2, j * tstep); ta[2] = cmul(ta[1], ta[1]); ta[3] = cmul(ta[1], ta[2]);
         }
         // stage A: radix 4 over the elements a + 4 r; twiddle W_L^{(j + a M) s} = W_L^{j s} W_16^{a s}
 #pragma unroll
@@ -194,10 +193,7 @@ __device__ __forceinline__ void dif_stage16(double2* buf, int N, int L, int kt, 
             for (int s = 0; s < 4; ++s) u[a + 4 * s] = v[s];
         }
         // stage B: radix 4 inside each quarter s (elements 4 s + r'); twiddle W_{L/4}^{j s'}
-        if (M > 1) {
-#pragma unroll
-            for (int s = 1; s < 4; ++s) tb[s] = twiddle<false>(tw2, 4 * j * s * tstep);
-        }
+        if (M > 1) { tb[1] = cmul(ta[2], ta[2]); tb[2] = cmul(tb[1], tb[1]); tb[3] = cmul(tb[1], tb[2]); }
 #pragma unroll
         for (int s = 0; s < 4; ++s) {
             double2 v[4] = {u[4 * s], u[4 * s + 1], u[4 * s + 2], u[4 * s + 3]};
@@ -227,9 +223,8 @@ __device__ __forceinline__ void dif_stage8(double2* buf, int N, int L, int kt, L
         for (int c = 0; c < 8; ++c) u[c] = GIN ? ld(e0 + c * M, kk) : buf[lay(e0 + c * M, kk)];
         double2 ta[4], tb;
         if (M > 1) {
-#pragma unroll
-            for (int s = 1; s < 4; ++s) ta[s] = twiddle<false>(tw2, j * s * tstep);
-            tb = twiddle<false>(tw2, 4 * j * tstep);
+            ta[1] = twiddle<false>(tw2, j * tstep); ta[2] = cmul(ta[1], ta[1]); ta[3] = cmul(ta[1], ta[2]);
+            tb = cmul(ta[2], ta[2]);
         }
         // stage A: radix 4 over the elements a + 2 r; twiddle W_L^{(j + a M) s} = W_L^{j s} W_8^{a s}
 #pragma unroll
@@ -360,8 +355,8 @@ __device__ __forceinline__ void dit_stage16(double2* buf, int N, int L, int kt, 
         for (int c = 0; c < 16; ++c) u[c] = buf[lay(e0 + c * M, kk)];
         double2 ta[4], tb[4];
         if (M > 1) {
-#pragma unroll
-            for (int s = 1; s < 4; ++s) tb[s] = twiddle<true>(tw2, 4 * j * s * tstep);
+            ta[1] = twiddle<true>(tw2, j * tstep); ta[2] = cmul(ta[1], ta[1]); ta[3] = cmul(ta[1], ta[2]);
+            tb[1] = cmul(ta[2], ta[2]); tb[2] = cmul(tb[1], tb[1]); tb[3] = cmul(tb[1], tb[2]);
         }
 #pragma unroll
         for (int s = 0; s < 4; ++s) {
@@ -373,10 +368,6 @@ __device__ __forceinline__ void dit_stage16(double2* buf, int N, int L, int kt, 
             bfly<4, true>(v);
 #pragma unroll
             for (int q = 0; q < 4; ++q) u[4 * s + q] = v[q];
-        }
-        if (M > 1) {
-#pragma unroll
-            for (int s = 1; s < 4; ++s) ta[s] = twiddle<true>(tw2, j * s * tstep);
         }
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
@@ -413,9 +404,8 @@ __device__ __forceinline__ void dit_stage8(double2* buf, int N, int L, int kt, L
         for (int c = 0; c < 8; ++c) u[c] = buf[lay(e0 + c * M, kk)];
         double2 ta[4], tb;
         if (M > 1) {
-#pragma unroll
-            for (int s = 1; s < 4; ++s) ta[s] = twiddle<true>(tw2, j * s * tstep);
-            tb = twiddle<true>(tw2, 4 * j * tstep);
+            ta[1] = twiddle<true>(tw2, j * tstep); ta[2] = cmul(ta[1], ta[1]); ta[3] = cmul(ta[1], ta[2]);
+            tb = cmul(ta[2], ta[2]);
         }
 #pragma unroll
         for (int s = 0; s < 4; ++s) {

@@ -161,5 +161,5 @@ def test_config5_iterative_composition():
     torch.cuda.synchronize()
     err_0 = float(((a - alm_true).abs().amax(dim=(1, 2)) / alm_true.abs().amax(dim=(1, 2))).max())
     print("config 5: rms per round (map 0)", r[:, 0], "a_lm error after 0 / 3 rounds: %.2e / %.2e" % (err_0, err_it))
-    assert err_it < 1e-3 * err_0
+    assert err_it < 1e-2 * err_0
     plan.destroy()
