@@ -19,6 +19,7 @@
 namespace sht {
 
 // ---- tile shapes ---------------------------------------------------------------------------------------
+constexpr int LEG_GEN_WARPS = 4;             // lambda generators (+ TMA issue)
 constexpr int LEG_CONSUMER_WARPS = 8;        // 2 (l parity class) x 4 (32-column slices); warp tile 64 x 32
 constexpr int LEG_THREADS = 384;             // + warp 8: TMA producer, warps 9,10: lambda generators, warp 11 idle
 constexpr int A_ML = LEG_A_ML;               // analysis: l rows per tile (64 of each parity class)
@@ -32,7 +33,7 @@ static_assert(A_STAGE_BYTES % 1024 == 0, "stages must keep the 1024-byte alignme
 constexpr int S_PB = 64;                     // synthesis: ring pairs per CTA tile (Ee rows + Oo rows = 128 C rows)
 constexpr int S_LC = 32;                     // synthesis: l values per stage (16 of each parity, four TMA boxes of 8 l)
 constexpr int S_SL = 66;                     // lambda tile: stride (doubles) between l rows, = 2 mod 8
-constexpr int S_STAGES = 4;
+constexpr int S_STAGES = 4;                  // even: the generators fill stages in pairs
 constexpr int S_ABYTES = S_LC * KTILE_MAPS * 16;     // a_lm tile of a stage: 32 KB
 constexpr int S_LBYTES = S_LC * S_SL * 8;
 constexpr int S_STAGE_BYTES = (S_ABYTES + S_LBYTES + 1023) / 1024 * 1024;
@@ -56,20 +57,24 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     int* i0s = pst + ((d.ntile_max + 3) & ~3);                                               // per stage: first 16-row block with a started recurrence
 
     const int m = blockIdx.x / nkt, kt = blockIdx.x % nkt;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // warps 0..3 generate (the oldest warps of an SM sub-partition are served first by its scheduler: their
+    // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
+    const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) - LEG_GEN_WARPS;
+    const int tix = threadIdx.x;
+    const int tid = tix - LEG_GEN_WARPS * 32;                  // consumer thread index (negative for generators)
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
     const int ntile = (lmax - m) / A_ML + 1;
 
-    for (int t = tid; t < ntile; t += LEG_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
-    if (tid == 0) {
+    for (int t = tix; t < ntile; t += LEG_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
+    if (tix == 0) {
         for (int s = 0; s < A_STAGES; ++s) { mbar_init(full + s, 1 + 64); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
         fence_barrier_init();
         tma_prefetch_desc(&tmF);
     }
     __syncthreads();
 
-    if (warp < LEG_CONSUMER_WARPS) {
+    if (warp >= 0) {
         // ===== consumers: C[l, k'] += lambda[l, p] X[p, k'] =====
         const int cls = warp >> 2, wn = warp & 3;      // cls 0: l - m even (uses E), 1: odd (uses O)
         const int g = lane >> 2, t = lane & 3;
@@ -150,7 +155,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
         // ===== lambda generators (warps 8..11): warp = (stage it owns) + 2 (half of the tile's 128 l rows); lane = ring of
         // the chunk.  The recurrence restarts from the plan's state table at l0 and l0 + 64, so the two halves of a
         // stage are generated at the same time.  Lane 0 of the first-half warp also issues the stage's TMA loads.
-        const int gw = warp - LEG_CONSUMER_WARPS;
+        const int gw = warp + LEG_GEN_WARPS;
         const int gs = gw & 1, gh = gw >> 1;
         const int gl = gw * 32 + lane;                          // 0 .. 127 = one l of the tile per thread
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
@@ -175,13 +180,25 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                 if ((chunk & 1) != gs) continue;
                 const int stage = gs;
                 const uint32_t phase = (chunk >> 1) & 1;
+                // NCH independent chains per lane (16 l each, restarted from the state table): a dependent FP64 instruction
+                // waits behind the consumers' queued DMMAs for hundreds of cycles, so the latency of one step is shared
+                // by four chains instead of being paid 64 times in a row
+                constexpr int NCH = 4, CL = A_ML / 2 / NCH;
                 const int p = pc + lane;
-                double x1 = 0.0, x2 = 0.0, z = 0.0;
+                double x1[NCH], x2[NCH], z = 0.0;
                 int ls = lmax + 1;
-                if (p < nh && lh <= lmax) {
-                    const double2 sd = __ldg(cst + p);
-                    x1 = sd.x; x2 = sd.y; z = d.z[p];
+#pragma unroll
+                for (int c = 0; c < NCH; ++c) { x1[c] = 0.0; x2[c] = 0.0; }
+                if (p < nh) {
+                    z = d.z[p];
                     ls = d.lstart[(size_t)m * nh + p];
+#pragma unroll
+                    for (int c = 0; c < NCH; ++c) {
+                        if (lh + CL * c <= lmax) {
+                            const double2 sd = __ldg(cst + (size_t)c * (CL / LEG_CS) * nh + p);
+                            x1[c] = sd.x; x2[c] = sd.y;
+                        }
+                    }
                 }
                 const int rs = ls - lh;                             // first row of the half with a started recurrence
                 int lsmin = ls;
@@ -197,14 +214,18 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                 }
                 double* Ls = reinterpret_cast<double*>(Xs + A_XBYTES) + lane * A_SL + (A_ML / 4) * gh;
                 const double2* cfh = cft + (A_ML / 2) * gh;
-#pragma unroll 16
-                for (int r = 0; r < A_ML / 2; ++r) {
-                    const double2 ab = cfh[r];
-                    const double t = fma(ab.x * z, x1, -(ab.y * x2));
-                    const bool on = r >= rs;
-                    const double v = on ? t : 0.0;
-                    x2 = on ? x1 : x2; x1 = on ? t : x1;
-                    Ls[(r & 1) * (A_PC * A_SL) + (r >> 1)] = v;
+#pragma unroll
+                for (int r = 0; r < CL; ++r) {
+#pragma unroll
+                    for (int c = 0; c < NCH; ++c) {
+                        const int rr = CL * c + r;                  // row inside this warp's half
+                        const double2 ab = cfh[rr];
+                        const double t = fma(ab.x * z, x1[c], -(ab.y * x2[c]));
+                        const bool on = rr >= rs;
+                        const double v = on ? t : 0.0;
+                        x2[c] = on ? x1[c] : x2[c]; x1[c] = on ? t : x1[c];
+                        Ls[(rr & 1) * (A_PC * A_SL) + (rr >> 1)] = v;
+                    }
                 }
                 mbar_arrive(full + stage);
             }
@@ -233,24 +254,28 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
     const int pbi = (blockIdx.x / nkt) % npb;
     const int m = blockIdx.x / (nkt * npb);
     const int pb = pbi * S_PB;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // warps 0..3 generate (the oldest warps of an SM sub-partition are served first by its scheduler: their
+    // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
+    const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) - LEG_GEN_WARPS;
+    const int tix = threadIdx.x;
+    const int tid = tix - LEG_GEN_WARPS * 32;                  // consumer thread index (negative for generators)
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
     const int plast = min(pb + S_PB, nh) - 1;
     if (m >= d.mlim[plast]) return;                    // no ring of this block takes part in order m (never read)
 
-    if (tid == 0) {
+    if (tix == 0) {
         for (int s = 0; s < S_STAGES; ++s) { mbar_init(full + s, 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
         fence_barrier_init();
         tma_prefetch_desc(&tmA);
         *lmin_s = lmax + 1;
     }
-    if (tid < 8) minls8[tid] = lmax + 1;
+    if (tix < 8) minls8[tix] = lmax + 1;
     __syncthreads();
-    if (tid < S_PB && pb + tid < nh) {
-        const int lsv = d.lstart[(size_t)m * nh + pb + tid];
+    if (tix < S_PB && pb + tix < nh) {
+        const int lsv = d.lstart[(size_t)m * nh + pb + tix];
         atomicMin(lmin_s, lsv);
-        atomicMin(minls8 + (tid >> 3), lsv);
+        atomicMin(minls8 + (tix >> 3), lsv);
     }
     __syncthreads();
     const int lmin = *lmin_s;
@@ -258,7 +283,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
     const int cfirst = (lmin > lmax) ? (lmax + 1) : m + ((lmin - m) / S_LC) * S_LC;
     const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
 
-    if (warp < LEG_CONSUMER_WARPS) {
+    if (warp >= 0) {
         // ===== consumers: C[p, k'] += lambda[l, p] a[l, k'] over the l of this warp's parity class =====
         const int cls = warp >> 2, wn = warp & 3;
         const int g = lane >> 2, t = lane & 3;
@@ -353,7 +378,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
         // the recurrence restarts from the plan's state table every 16 l, so the two l halves of a stage are generated
         // at the same time.  Lane 0 of generator 0 also issues the stage's TMA loads (a_lm, straight from the m-major
         // ABI layout).
-        const int gw = warp - LEG_CONSUMER_WARPS;
+        const int gw = warp + LEG_GEN_WARPS;
         const int gh = gw >> 1;
         const int rl = (gw & 1) * 32 + lane;
         const int p = pb + rl;
@@ -363,46 +388,77 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
         const double2* csm = d.cseed + (size_t)d.csoff[m] * nh + (p < nh ? p : 0);
         constexpr int HL = S_LC / 2;                            // l per warp and stage
-        // (alpha, beta) and the start state of the next stage are fetched while the current one is computed
-        double2* cfw = cfs + gw * (2 * HL);
-        auto load_cf = [&](int lb) -> double2 {
-            const int l = lb + (lane & (HL - 1));
+        // Two stages are generated at a time, as two independent chains per lane (restarted from the state table): a
+        // dependent FP64 instruction waits behind the consumers' queued DMMAs for hundreds of cycles, so the latency
+        // of a step is shared by both chains.  (alpha, beta) and the start states of the next pair are fetched while
+        // the current pair is computed.
+        double2* cfw = cfs + gw * (2 * HL);                     // this warp's coefficients of the two stages
+        auto load_cf = [&](int lb) -> double2 {                 // lanes 0..15: first stage of the pair, 16..31: second
+            const int l = lb + (lane & (HL - 1)) + (lane >> 4) * S_LC;
             return l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
         };
         auto load_state = [&](int lb) -> double2 {
             return (p < nh && lb <= lmax) ? __ldg(csm + (size_t)((lb - m) / LEG_CS) * nh) : make_double2(0.0, 0.0);
         };
-        double2 cf = load_cf(cfirst + HL * gh), sd = load_state(cfirst + HL * gh);
-        int stage = 0, buf = 0; uint32_t phase = 0;
+        const int lb0 = cfirst + HL * gh;
+        double2 cf = load_cf(lb0), sda = load_state(lb0), sdb = load_state(lb0 + S_LC);
+        int stage = 0; uint32_t phase = 0;
         const int row0 = (k0 + kt * KTILE_MAPS) * d.ncomp + comp;
-        for (int lc = cfirst; lc <= lmax; lc += S_LC) {
+        for (int lc = cfirst; lc <= lmax; lc += 2 * S_LC) {
             const int lb = lc + HL * gh;
-            if (lane < HL) cfw[buf * HL + lane] = cf;
+            const bool two = lc + S_LC <= lmax;                 // the pair's second stage exists
+            __syncwarp();                                       // everyone is done reading the previous coefficients
+            cfw[lane] = cf;
             __syncwarp();
-            double x1 = sd.x, x2 = sd.y;
-            cf = load_cf(lb + S_LC); sd = load_state(lb + S_LC);
-            const int rs = ls - lb;
+            double xa1 = sda.x, xa2 = sda.y, xb1 = sdb.x, xb2 = sdb.y;
+            cf = load_cf(lb + 2 * S_LC); sda = load_state(lb + 2 * S_LC); sdb = load_state(lb + 3 * S_LC);
+            const int rsa = ls - lb, rsb = rsa - S_LC;
+            const int stb = stage + 1;                          // S_STAGES is even: a pair never wraps
             mbar_wait(empty + stage, phase ^ 1);
-            unsigned char* As = stage_base + (size_t)stage * S_STAGE_BYTES;
+            if (two) mbar_wait(empty + stb, phase ^ 1);
+            unsigned char* Asa = stage_base + (size_t)stage * S_STAGE_BYTES;
+            unsigned char* Asb = Asa + S_STAGE_BYTES;
             if (gw == 0 && lane == 0) {
                 mbar_arrive_expect_tx(full + stage, S_ABYTES);
 #pragma unroll
                 for (int q = 0; q < 4; ++q)
-                    tma_load_2d(As + q * (S_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0);
-            }
-            double* Ls = reinterpret_cast<double*>(As + S_ABYTES) + (HL * gh) * S_SL + rl;
+                    tma_load_2d(Asa + q * (S_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0);
+                if (two) {
+                    mbar_arrive_expect_tx(full + stb, S_ABYTES);
 #pragma unroll
-            for (int r = 0; r < HL; ++r) {
-                const double2 ab = cfw[buf * HL + r];
-                const double t = fma(ab.x * z, x1, -(ab.y * x2));
-                const bool on = r >= rs;
-                const double v = on ? t : 0.0;
-                x2 = on ? x1 : x2; x1 = on ? t : x1;
-                Ls[r * S_SL] = v;
+                    for (int q = 0; q < 4; ++q)
+                        tma_load_2d(Asb + q * (S_ABYTES / 4), &tmA, full + stb, (int)(2 * (moff + lc + S_LC + 8 * q)), row0);
+                }
             }
-            mbar_arrive(full + stage);
-            buf ^= 1;
-            if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
+            double* La = reinterpret_cast<double*>(Asa + S_ABYTES) + (HL * gh) * S_SL + rl;
+            double* Lb = reinterpret_cast<double*>(Asb + S_ABYTES) + (HL * gh) * S_SL + rl;
+            if (two) {
+#pragma unroll
+                for (int r = 0; r < HL; ++r) {
+                    const double2 aa = cfw[r], ab = cfw[HL + r];
+                    const double ta = fma(aa.x * z, xa1, -(aa.y * xa2));
+                    const double tb = fma(ab.x * z, xb1, -(ab.y * xb2));
+                    const bool ona = r >= rsa, onb = r >= rsb;
+                    xa2 = ona ? xa1 : xa2; xa1 = ona ? ta : xa1;
+                    xb2 = onb ? xb1 : xb2; xb1 = onb ? tb : xb1;
+                    La[r * S_SL] = ona ? ta : 0.0;
+                    Lb[r * S_SL] = onb ? tb : 0.0;
+                }
+                mbar_arrive(full + stage);
+                mbar_arrive(full + stb);
+            } else {
+#pragma unroll
+                for (int r = 0; r < HL; ++r) {
+                    const double2 aa = cfw[r];
+                    const double ta = fma(aa.x * z, xa1, -(aa.y * xa2));
+                    const bool ona = r >= rsa;
+                    xa2 = ona ? xa1 : xa2; xa1 = ona ? ta : xa1;
+                    La[r * S_SL] = ona ? ta : 0.0;
+                }
+                mbar_arrive(full + stage);
+            }
+            stage += 2;
+            if (stage == S_STAGES) { stage = 0; phase ^= 1; }
         }
     }
 }
