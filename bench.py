@@ -29,6 +29,11 @@ from paper_2208_10154_b200 import inputs, shard  # noqa: E402
 
 METRIC = "maps/sec (analysis+synthesis, FP64) at nside=512 lmax=1535"
 FP64_NOMINAL_TFLOPS = 37.2     # 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz
+# DRAM bytes per launch from the committed ncu capture (profiles/r1_v2_summary.md), keyed by (config, nmaps, kernel)
+NCU_TRAFFIC_BYTES = {
+    (3, 1000, "k_legendre_analysis"): 251379450880 + 19061606400,
+    (3, 1000, "k_legendre_synthesis"): 20458497000 + 37875944000,
+}
 
 
 def read_measured_peaks():
@@ -238,28 +243,34 @@ def main():
     ms_step = ms_total / args.steps
     value = world * nmaps / (ms_step * 1e-3)
 
-    # ---- roofline of the dominant kernel (Legendre contraction, both directions) -----------------------
+    # ---- roofline of the dominant kernel: k_legendre_analysis (the slower of the two Legendre launches; the synthesis
+    # kernel, same design, is reported beside it in "stages") ---------------------------------------------------------
     peaks, peak_src = read_measured_peaks()
     fl_dir = legendre_flops_per_direction(c)
-    leg_ms = stage_ms[1] + stage_ms[2]
-    leg_n = max(1, stage_n[1] + stage_n[2])
-    leg_launch_ms = leg_ms / leg_n
-    flops_per_launch = fl_dir * 2 * args.steps / leg_n
-    achieved = flops_per_launch / (leg_launch_ms * 1e-3) * 1e-12
     mma_peak = sht_measure_fp64_mma_peak(300.0)
-    roofline = {"bound": "tensor", "kernel": "k_legendre_analysis + k_legendre_synthesis (DMMA.8x8x4, FP64)",
-                "achieved": achieved, "peak": mma_peak, "unit": "TFLOP/s", "frac": achieved / mma_peak,
-                "traffic": None,
-                "peak_source": "FP64 DMMA.8x8x4 register-resident loop measured live in this run "
-                               "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = %.1f; "
-                               "rule-derived bf16 %s x 45/2250 = %.1f)"
-                               % (FP64_NOMINAL_TFLOPS, peak_src, peaks.get("bf16_tflops", 0) * 45.0 / 2250.0),
-                "algorithmic_flops_per_launch": flops_per_launch, "launch_ms": leg_launch_ms,
-                "share_of_step": leg_ms / ms_total}
+    peak_note = ("FP64 DMMA.8x8x4 register-resident loop measured live in this run "
+                 "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = %.1f; "
+                 "rule-derived bf16 %s x 45/2250 = %.1f)"
+                 % (FP64_NOMINAL_TFLOPS, peak_src, peaks.get("bf16_tflops", 0) * 45.0 / 2250.0))
+
+    def leg_roofline(stage, kernel):
+        n = max(1, stage_n[stage])
+        launch_ms = stage_ms[stage] / n
+        flops_per_launch = fl_dir * args.steps / n          # algorithmic (folded, unpruned) flops of one launch
+        ach = flops_per_launch / (launch_ms * 1e-3) * 1e-12
+        return {"bound": "tensor", "kernel": kernel, "achieved": ach, "peak": mma_peak, "unit": "TFLOP/s",
+                "frac": ach / mma_peak, "traffic": NCU_TRAFFIC_BYTES.get((args.config, nmaps, kernel)),
+                "algorithmic_flops_per_launch": flops_per_launch, "launch_ms": launch_ms,
+                "share_of_step": stage_ms[stage] / ms_total}
+
+    roofline = leg_roofline(1, "k_legendre_analysis")
+    roofline["peak_source"] = peak_note
+    roofline["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_v2_summary.md"
+    roofline_syn = leg_roofline(2, "k_legendre_synthesis")
     ring_ms = stage_ms[0] + stage_ms[3]
     ring_bytes = 2 * args.steps * (8 * npix * nmaps * ncomp + 16 * (lmax + 1) * 2 * nside * 2 * nmaps * ncomp)
     ring_gbs = ring_bytes / (ring_ms * 1e-3) * 1e-9 if ring_ms > 0 else None
-    stages = {"ring_fft_analysis_ms": stage_ms[0] / args.steps, "legendre_analysis_ms": stage_ms[1] / args.steps,
+    stages = {"legendre_synthesis_roofline": roofline_syn, "ring_fft_analysis_ms": stage_ms[0] / args.steps, "legendre_analysis_ms": stage_ms[1] / args.steps,
               "legendre_synthesis_ms": stage_ms[2] / args.steps, "ring_fft_synthesis_ms": stage_ms[3] / args.steps,
               "ring_fft_hbm": {"bound": "hbm", "achieved": ring_gbs, "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
                                "frac": (ring_gbs / peaks["hbm_gbs"]) if ring_gbs else None,

@@ -44,6 +44,10 @@ struct RingPair {
     int hf_off;            // offset (double2) of FFT_lc(conj chirp) / lc in forward-output position order
     int psh;               // shared-memory padding: one element every 2^psh (power-of-two transforms), 31 = none
     int nbuf;              // elements per map of one transform buffer, padding included
+    // power-of-two rings: the digit reversal is a bit permutation, computed instead of read from the table:
+    // r = brev(k) >> (32 - pbits); pos = ((r & pm_hi) >> 1) | ((r & pm_lo) << 1) | (r & pm_keep);  pbits = 0: use the table
+    int pbits;
+    unsigned pm_hi, pm_lo, pm_keep;
 };
 
 struct DevicePlan {

@@ -368,6 +368,20 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
             r.nbuf = r.n + (r.n >> r.psh);
         }
         r.kt = ring_kt((size_t)r.nbuf * sizeof(double2) * (r.oop ? 2 : 1));
+        r.pbits = 0; r.pm_hi = r.pm_lo = r.pm_keep = 0;
+        if (!r.lc && (r.n & (r.n - 1)) == 0) {
+            int a = 0;
+            while ((1 << a) < r.n) ++a;
+            // plain factor list of a power of two: 4s, then at most one 2; digit of width w at bits [lo, lo + w) of the bin
+            int lo = 0;
+            for (int rem = r.n; rem > 1;) {
+                const int w = (rem % 4 == 0) ? 2 : 1;
+                if (w == 2) { r.pm_hi |= 1u << (a - 1 - lo); r.pm_lo |= 1u << (a - 2 - lo); }
+                else r.pm_keep |= 1u << (a - 1 - lo);
+                lo += w; rem >>= w;
+            }
+            r.pbits = a;
+        }
         r.mlim = lmax + 1;                               // tightened below from the l_safe table
         zs[p] = (double)absz; sin2s[p] = (double)s2;
     }

@@ -35,6 +35,21 @@ struct Lay {
     __device__ __forceinline__ int operator()(int e, int kk) const { return ((e + (e >> psh)) << ktsh) + kk; }
 };
 
+// position of bin k in the forward-transformed buffer: computed for power-of-two rings, tabulated otherwise
+struct BinPos {
+    const unsigned short* perm;
+    int pbits;
+    unsigned hi, lo, keep;
+    __device__ __forceinline__ int operator()(int k) const
+    {
+        if (pbits) {
+            const unsigned r = __brev((unsigned)k) >> (32 - pbits);
+            return (int)(((r & hi) >> 1) | ((r & lo) << 1) | (r & keep));
+        }
+        return (int)__ldg(perm + k);
+    }
+};
+
 // exp(-2 pi i k / 16)
 __host__ __device__ constexpr double w16_cos(int k)
 {
@@ -677,7 +692,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int
     if (kbase >= kmaps) return;
     const int tid = threadIdx.x, nt = blockDim.x;
     const double2* tw2 = d.tw + rp.tw_off;
-    const unsigned short* perm = d.perm + rp.perm_off;
+    const BinPos perm{d.perm + rp.perm_off, rp.pbits, rp.pm_hi, rp.pm_lo, rp.pm_keep};
     const bool equator = rp.start_s < 0;
     const bool blue = rp.lc > 0;
 
@@ -717,12 +732,12 @@ __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int
     const size_t cstride = (size_t)d.ncomp * 2 * KG;                       // double2 per order m
     double2* Fp = reinterpret_cast<double2*>(F) + f_cell(d, p, k >> 2, 0, comp, 0) + (k & 3) + (size_t)m * cstride;
     const int mlim = rp.mlim;
-#pragma unroll 2
+#pragma unroll 4
     for (; m < mlim; m += dm) {
         const int bc = b == 0 ? 0 : N - b;
         double2 A, B;
         if (!blue) {
-            A = cur[lay((int)perm[b], kk)]; B = cur[lay((int)perm[bc], kk)];
+            A = cur[lay(perm(b), kk)]; B = cur[lay(perm(bc), kk)];
         } else {
             A = cmul(cur[lay(b, kk)], __ldg(tw2 + (b * b) % (2 * N)));
             B = cmul(cur[lay(bc, kk)], __ldg(tw2 + (bc * bc) % (2 * N)));
@@ -764,7 +779,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const in
     if (kbase >= kmaps) return;
     const int tid = threadIdx.x, nt = blockDim.x;
     const double2* tw2 = d.tw + rp.tw_off;
-    const unsigned short* perm = d.perm + rp.perm_off;
+    const BinPos perm{d.perm + rp.perm_off, rp.pbits, rp.pm_hi, rp.pm_lo, rp.pm_keep};
     const bool equator = rp.start_s < 0;
     const bool blue = rp.lc > 0;
     const int mlim = rp.mlim;
@@ -806,8 +821,8 @@ __global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const in
             const double2 zb = make_double2(yn.x - ys.y, yn.y + ys.x);
             const double2 zc = make_double2(yn.x + ys.y, ys.x - yn.y);           // Z[N - b]
             if (!blue) {
-                cur[lay((int)perm[b], kk)] = zb;
-                if (b > 0 && 2 * b < N) cur[lay((int)perm[N - b], kk)] = zc;
+                cur[lay(perm(b), kk)] = zb;
+                if (b > 0 && 2 * b < N) cur[lay(perm(N - b), kk)] = zc;
             } else {
                 // x_n = conj(c)_n sum_b (Z_b conj(c)_b) c_{n-b}
                 double2 c = __ldg(tw2 + (b * b) % (2 * N)); c.y = -c.y;
