@@ -18,16 +18,23 @@ if not os.path.exists(LIB_PATH):
 _lib = ctypes.CDLL(LIB_PATH)
 
 SHT_OK = 0
+SHT_POL_E, SHT_POL_B = 1, 2
 _vp, _i, _ll, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_double
 
 _lib.sht_plan_create.argtypes = [ctypes.POINTER(_vp), _i, _i, _i, _i]
 _lib.sht_plan_create.restype = _i
+_lib.sht_plan_create_ex.argtypes = [ctypes.POINTER(_vp), _i, _i, _i, _i, ctypes.c_size_t]
+_lib.sht_plan_create_ex.restype = _i
 _lib.sht_plan_destroy.argtypes = [_vp]
 _lib.sht_plan_destroy.restype = _i
 _lib.sht_analysis.argtypes = [_vp, _vp, _vp, _vp]
 _lib.sht_analysis.restype = _i
 _lib.sht_synthesis.argtypes = [_vp, _vp, _vp, _vp]
 _lib.sht_synthesis.restype = _i
+_lib.sht_analysis_pol.argtypes = [_vp, _vp, _vp, _i, _vp]
+_lib.sht_analysis_pol.restype = _i
+_lib.sht_synthesis_pol.argtypes = [_vp, _vp, _vp, _i, _vp]
+_lib.sht_synthesis_pol.restype = _i
 _lib.sht_analysis_iter.argtypes = [_vp, _vp, _vp, _i, _vp, _vp]
 _lib.sht_analysis_iter.restype = _i
 _lib.sht_analysis_host.argtypes = [_vp, _vp, _vp]
@@ -58,7 +65,7 @@ _lib.sht_measure_fp64_mma_peak.argtypes = [_d]
 _lib.sht_measure_fp64_mma_peak.restype = _d
 
 EXPORTED = [
-    "sht_plan_create", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter",
+    "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol",
     "sht_analysis_host", "sht_synthesis_host", "sht_npix", "sht_nalm", "sht_alm_index",
     "sht_plan_workspace_bytes", "sht_plan_chunk_maps", "sht_plan_kernel_launches", "sht_status_string",
     "sht_last_error", "sht_measure_fp64_mma_peak", "sht_plan_set_timing", "sht_plan_stage_ms",
@@ -111,9 +118,9 @@ def _stream(stream):
 class Plan:
     """sht_plan_create / sht_plan_destroy with the transform entries as methods (same names as the ABI)."""
 
-    def __init__(self, nside, lmax, nmaps, spin=0):
+    def __init__(self, nside, lmax, nmaps, spin=0, workspace_limit=0):
         self._h = ctypes.c_void_p()
-        st = _lib.sht_plan_create(ctypes.byref(self._h), nside, lmax, nmaps, spin)
+        st = _lib.sht_plan_create_ex(ctypes.byref(self._h), nside, lmax, nmaps, spin, workspace_limit)
         if st != SHT_OK:
             self._h = None
             raise ShtError("sht_plan_create(%d,%d,%d,%d): %s" % (nside, lmax, nmaps, spin, sht_status_string(st)))
@@ -134,6 +141,12 @@ class Plan:
     def sht_analysis_iter(self, maps, alm, niter, resid_rms=None, stream=None):
         self._check(_lib.sht_analysis_iter(self._h, _ptr(maps), _ptr(alm), niter, _ptr(resid_rms), _stream(stream)),
                     "sht_analysis_iter")
+
+    def sht_analysis_pol(self, maps, alm, which, stream=None):
+        self._check(_lib.sht_analysis_pol(self._h, _ptr(maps), _ptr(alm), which, _stream(stream)), "sht_analysis_pol")
+
+    def sht_synthesis_pol(self, alm, maps, which, stream=None):
+        self._check(_lib.sht_synthesis_pol(self._h, _ptr(alm), _ptr(maps), which, _stream(stream)), "sht_synthesis_pol")
 
     def sht_analysis_host(self, maps_host, alm_host):
         self._check(_lib.sht_analysis_host(self._h, _ptr(maps_host), _ptr(alm_host)), "sht_analysis_host")

@@ -156,6 +156,38 @@ extern "C" sht_status_t sht_synthesis(sht_plan_t pl, const double* alm, double* 
     return SHT_OK;
 }
 
+// E-only / B-only polarisation transforms (item 9)
+static sht_status_t pol_run(sht_plan_t pl, const double* maps, const double* alm_in, double* maps_out, double* alm_out, int which,
+                            void* stream)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if ((!maps && !maps_out) || (!alm_in && !alm_out)) { snprintf(pl->err, sizeof(pl->err), "null data pointer"); return SHT_ERR_NULL; }
+    if (pl->d.spin != 2 || (which != SHT_POL_E && which != SHT_POL_B)) {
+        snprintf(pl->err, sizeof(pl->err), "E-only / B-only transforms need a spin-2 plan and which = SHT_POL_E or SHT_POL_B");
+        return SHT_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    pl->pol = which;
+    sht_status_t s = SHT_OK;
+    for (int k0 = 0; k0 < pl->nmaps && s == SHT_OK; k0 += pl->chunk) {
+        const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
+        s = alm_out ? analysis_chunk(pl, pl->d, maps, k0, alm_out, k0, pl->F, kmaps, false, st)
+                    : synthesis_chunk(pl, pl->d, alm_in, k0, maps_out, k0, pl->F, kmaps, nullptr, 0, st);
+    }
+    pl->pol = 0;
+    return s;
+}
+
+extern "C" sht_status_t sht_analysis_pol(sht_plan_t pl, const double* maps, double* alm, int which, void* stream)
+{
+    return pol_run(pl, maps, nullptr, nullptr, alm, which, stream);
+}
+
+extern "C" sht_status_t sht_synthesis_pol(sht_plan_t pl, const double* alm, double* maps, int which, void* stream)
+{
+    return pol_run(pl, nullptr, alm, maps, nullptr, which, stream);
+}
+
 extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, double* alm, int niter,
                                           double* resid_rms, void* stream)
 {

@@ -102,6 +102,7 @@ struct sht_plan_s {
     size_t class_smem[sht::RING_NCLASS];
     int sm_count;
     long long launches;
+    int pol;                        // spin 2: 0 = E and B, 1 = E only, 2 = B only (set by the *_pol entries around a call)
     char err[512];
     // host-entry staging (allocated on first use)
     double* stage_maps[2];

@@ -57,6 +57,9 @@ __device__ __forceinline__ void spin2_consts(const DevicePlan& d, int l, int m, 
 // analysis, spin 2: one CTA per (m, k-tile of 32 pairs); l tiles outer, ring chunks of 16 inner.
 // Stage: [X: comp(Q,iU) x 8 kg x 16 p x 128 B, 128B-swizzled] [F: sign(+,-) x class x 16 p x A2_SL]
 // ------------------------------------------------------------------------------------------------
+// WHICH = 0: both a_E and a_B; 1: only a_E; 2: only a_B (item 9: half of the block products, output
+// alm[map][nalm] of that component alone)
+template <int WHICH>
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
                           int nkt, int accumulate)
@@ -122,8 +125,8 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                         for (int i = 0; i < 8; ++i)
 #pragma unroll
                             for (int j = 0; j < 2; ++j) {
-                                dmma884(cE[i][j][0], cE[i][j][1], a[i], sg ? bu[j] : bq[j]);
-                                dmma884(cB[i][j][0], cB[i][j][1], a[i], sg ? bq[j] : bu[j]);
+                                if (WHICH != 2) dmma884(cE[i][j][0], cE[i][j][1], a[i], sg ? bu[j] : bq[j]);
+                                if (WHICH != 1) dmma884(cB[i][j][0], cB[i][j][1], a[i], sg ? bq[j] : bu[j]);
                             }
                     }
                 }
@@ -139,15 +142,22 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                 for (int j = 0; j < 2; ++j) {
                     const int kk = kt * P_KT + (2 * wn + j) * KG + t;
                     if (l <= lmax && kk < kmaps) {
-                        double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * 2) * d.nalm + moff + l;
                         double2 ve = make_double2(cE[i][j][0], m == 0 ? 0.0 : cE[i][j][1]);
                         double2 vb = make_double2(cB[i][j][1], m == 0 ? 0.0 : -cB[i][j][0]);
-                        if (accumulate) {
-                            const double2 oe = dst[0], ob = dst[d.nalm];
-                            ve.x += oe.x; ve.y += oe.y; vb.x += ob.x; vb.y += ob.y;
+                        if (WHICH == 0) {
+                            double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * 2) * d.nalm + moff + l;
+                            if (accumulate) {
+                                const double2 oe = dst[0], ob = dst[d.nalm];
+                                ve.x += oe.x; ve.y += oe.y; vb.x += ob.x; vb.y += ob.y;
+                            }
+                            dst[0] = ve;
+                            dst[d.nalm] = vb;
+                        } else {
+                            double2* dst = reinterpret_cast<double2*>(alm) + (size_t)(k0 + kk) * d.nalm + moff + l;
+                            double2 v = WHICH == 1 ? ve : vb;
+                            if (accumulate) { const double2 o = *dst; v.x += o.x; v.y += o.y; }
+                            *dst = v;
                         }
-                        dst[0] = ve;
-                        dst[d.nalm] = vb;
                     }
                     cE[i][j][0] = cE[i][j][1] = 0.0; cB[i][j][0] = cB[i][j][1] = 0.0;
                 }
@@ -227,6 +237,8 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
 // With Qe = sum_{l-m even} F+ A^E + sum_{l-m odd} F- iA^B (even under the fold) and Qo the complementary sums,
 // Q(north) = Qe + Qo, Q(south) = Qe - Qo; iU likewise with A^E and iA^B exchanged.
 // ------------------------------------------------------------------------------------------------
+// WHICH = 0: alm holds (a_E, a_B) per pair; 1 / 2: alm[map][nalm] holds only a_E / only a_B, the other one is zero
+template <int WHICH>
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
                            int nkt, int npb)
@@ -305,7 +317,7 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
                 for (int j = 0; j < 2; ++j) {
                     const double* Ab = As + q * 1024 + (sg ? ab1[j] : ab0[j]);
                     const double e = Ab[im];                    // A^E: (re, im) of a_E
-                    const double b = Ab[P_KT * 16 + (im ^ 1)];  // iA^B = (-Im a_B, Re a_B)
+                    const double b = Ab[(WHICH == 2 ? 0 : P_KT * 16) + (im ^ 1)];  // iA^B = (-Im a_B, Re a_B)
                     be[j] = (dead || zero_e) ? 0.0 : e;
                     bb[j] = (dead || zero_b) ? 0.0 : (im ? b : -b);
                 }
@@ -313,8 +325,16 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
                 for (int i = 0; i < 8; ++i)
 #pragma unroll
                     for (int j = 0; j < 2; ++j) {
-                        dmma884(cQ[i][j][0], cQ[i][j][1], a[i], sg ? bb[j] : be[j]);
-                        dmma884(cU[i][j][0], cU[i][j][1], a[i], sg ? be[j] : bb[j]);
+                        if (WHICH == 0) {
+                            dmma884(cQ[i][j][0], cQ[i][j][1], a[i], sg ? bb[j] : be[j]);
+                            dmma884(cU[i][j][0], cU[i][j][1], a[i], sg ? be[j] : bb[j]);
+                        } else if (WHICH == 1) {                // a_B = 0: Q takes F+ A^E, iU takes F- A^E
+                            if (sg) dmma884(cU[i][j][0], cU[i][j][1], a[i], be[j]);
+                            else dmma884(cQ[i][j][0], cQ[i][j][1], a[i], be[j]);
+                        } else {                                // a_E = 0: Q takes F- iA^B, iU takes F+ iA^B
+                            if (sg) dmma884(cQ[i][j][0], cQ[i][j][1], a[i], bb[j]);
+                            else dmma884(cU[i][j][0], cU[i][j][1], a[i], bb[j]);
+                        }
                     }
             }
             __syncwarp();
@@ -418,10 +438,12 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
 // ---- host side -------------------------------------------------------------------------------------------
 // alm[pair][comp][nalm*2 doubles] as a 3-D tensor (innermost first: doubles of one (pair, comp) row, pair, comp);
 // box = 8 l (128 bytes) x 32 pairs x (E, B): lands in shared memory as [comp][pair][128 B]
-static cudaError_t make_tmap_alm_spin2(const DevicePlan& d, const double* alm, long long pairs, CUtensorMap* tm)
+static cudaError_t make_tmap_alm_spin2(const DevicePlan& d, const double* alm, long long pairs, int ncomp_mem, CUtensorMap* tm)
 {
-    const cuuint64_t dims[3] = {(cuuint64_t)d.nalm * 2, (cuuint64_t)pairs, 2};
-    const cuuint64_t strides[2] = {(cuuint64_t)d.nalm * 32, (cuuint64_t)d.nalm * 16};
+    // ncomp_mem = 1: single-component a_lm (E-only / B-only transforms): the box's second component is out of bounds
+    // and arrives as zeros
+    const cuuint64_t dims[3] = {(cuuint64_t)d.nalm * 2, (cuuint64_t)pairs, (cuuint64_t)ncomp_mem};
+    const cuuint64_t strides[2] = {(cuuint64_t)d.nalm * 16 * ncomp_mem, (cuuint64_t)d.nalm * 16};
     const cuuint32_t box[3] = {16, P_KT, 2};
     return make_tmap_f64(tm, alm, 3, dims, strides, box);
 }
@@ -440,12 +462,13 @@ cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, 
                                            bool accumulate, cudaStream_t st)
 {
     const size_t sm = analysis2_smem(d.ntile_max);
-    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis_spin2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    auto kern = pl->pol == 1 ? k_legendre_analysis_spin2<1> : pl->pol == 2 ? k_legendre_analysis_spin2<2> : k_legendre_analysis_spin2<0>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tmF;
     if ((e = make_tmap_F(d, F, P_KG, 2, &tmF)) != cudaSuccess) return e;
     const int nkt = (kmaps + P_KT - 1) / P_KT;
-    k_legendre_analysis_spin2<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
+    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -454,13 +477,14 @@ cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d,
                                             cudaStream_t st)
 {
     const size_t sm = synthesis2_smem();
-    cudaError_t e = cudaFuncSetAttribute(k_legendre_synthesis_spin2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    auto kern = pl->pol == 1 ? k_legendre_synthesis_spin2<1> : pl->pol == 2 ? k_legendre_synthesis_spin2<2> : k_legendre_synthesis_spin2<0>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tmA;
-    if ((e = make_tmap_alm_spin2(d, alm, (long long)(k0 + kmaps), &tmA)) != cudaSuccess) return e;
+    if ((e = make_tmap_alm_spin2(d, alm, (long long)(k0 + kmaps), pl->pol ? 1 : 2, &tmA)) != cudaSuccess) return e;
     const int nkt = (kmaps + P_KT - 1) / P_KT;
     const int npb = (d.nh + S2_PB - 1) / S2_PB;
-    k_legendre_synthesis_spin2<<<(d.lmax + 1) * nkt * npb, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb);
+    kern<<<(d.lmax + 1) * nkt * npb, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb);
     pl->launches++;
     return cudaGetLastError();
 }

@@ -224,6 +224,11 @@ static int ring_kt(size_t bytes_per_map)
 
 extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, int nmaps, int spin)
 {
+    return sht_plan_create_ex(out, nside, lmax, nmaps, spin, 0);
+}
+
+extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax, int nmaps, int spin, size_t workspace_limit)
+{
     if (!out) return SHT_ERR_NULL;
     *out = nullptr;
     if (nside < 1 || nside > 2048 || lmax < 0 || nmaps < 1 || (spin != 0 && spin != 2)) return SHT_ERR_INVALID_ARG;
@@ -524,6 +529,7 @@ extern "C" sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, in
         size_t budget = (size_t)(0.6 * (double)freeb);
         const size_t cap = (size_t)64 << 30;
         if (budget > cap) budget = cap;
+        if (workspace_limit && budget > workspace_limit) budget = workspace_limit;
         long long fit = (long long)(budget / per_map) / KTILE_MAPS * KTILE_MAPS;
         if (fit < KTILE_MAPS) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
         long long need = ((long long)nmaps + KTILE_MAPS - 1) / KTILE_MAPS * KTILE_MAPS;

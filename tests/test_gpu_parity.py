@@ -99,6 +99,38 @@ def test_spin2_ignores_low_l_and_im_m0_on_input():
     plan.destroy()
 
 
+@pytest.mark.parametrize("nside,lmax,nmaps", [(4, 11, 3), (16, 47, 40), (32, 95, 33), (48, 143, 2)])
+@pytest.mark.parametrize("which", [1, 2])
+def test_spin2_e_only_b_only(nside, lmax, nmaps, which):
+    """item 9: transforms of a^E or a^B alone against the oracle (synthesis with the other component
+    zero; the chosen component of the full analysis)"""
+    import torch
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan
+    c = which - 1
+    alm = inputs.gaussian_alm(lmax, np.arange(nmaps), seed=300 + nside, spin=2)
+    one = np.ascontiguousarray(alm[:, c, :])
+    zeroed = np.zeros_like(alm)
+    zeroed[:, c, :] = one
+    ref_maps = O.synthesis(nside, lmax, zeroed, spin=2)
+    plan = Plan(nside, lmax, nmaps, 2)
+    dev = _dev()
+    maps = torch.full((nmaps, 2, plan.npix), float("nan"), dtype=torch.float64, device=dev)
+    plan.sht_synthesis_pol(torch.from_numpy(one).to(dev), maps, which)
+    torch.cuda.synchronize()
+    assert inputs.rel_err(maps.cpu().numpy(), ref_maps) <= TOL
+    # analysis: a general (Q,U) input with both E and B power
+    qu = O.synthesis(nside, lmax, alm, spin=2) + inputs.white_noise(nside, np.arange(nmaps), 5, 1e-3, spin=2)
+    ref_alm = O.analysis(nside, lmax, qu, spin=2)[:, c, :]
+    got = torch.full((nmaps, plan.nalm), float("nan"), dtype=torch.complex128, device=dev)
+    plan.sht_analysis_pol(torch.from_numpy(qu).to(dev), got, which)
+    torch.cuda.synchronize()
+    assert inputs.rel_err(got.cpu().numpy(), ref_alm) <= TOL
+    # the full transform is untouched by the single-component calls
+    assert inputs.rel_err(_gpu_synthesis(plan, alm), O.synthesis(nside, lmax, alm, spin=2)) <= TOL
+    plan.destroy()
+
+
 def test_config1():
     """BASELINE.json configs[0]: nside 16, lmax 47, 8 maps: synthesise, analyse back, compare both."""
     from oracle import oracle as O
@@ -132,6 +164,36 @@ def test_config2_sampled_maps():
     ref_alm = O.analysis(nside, lmax, maps_in[ks])
     assert inputs.rel_err(got_alm[ks], ref_alm) <= TOL
     plan.destroy()
+
+
+@pytest.mark.parametrize("spin", [0, 2])
+def test_internal_map_chunks_match_single_chunk(spin):
+    """a workspace limit forces internal chunks of 64 maps (ragged last chunk); results must be bit-identical"""
+    import torch
+    from paper_2208_10154_b200.binding import Plan
+    nside, lmax, nmaps, niter = 16, 47, 150, 2
+    ncomp = 2 if spin == 2 else 1
+    alm = inputs.gaussian_alm(lmax, np.arange(nmaps), 11, spin)
+    full = Plan(nside, lmax, nmaps, spin)
+    per_map = 2 * nside * (lmax + 1) * ncomp * 2 * 16
+    small = Plan(nside, lmax, nmaps, spin, workspace_limit=70 * per_map)
+    assert full.chunk_maps() == nmaps and small.chunk_maps() == 64
+    m_full, m_small = _gpu_synthesis(full, alm), _gpu_synthesis(small, alm)
+    assert np.array_equal(m_full, m_small)
+    assert np.array_equal(_gpu_analysis(full, m_full), _gpu_analysis(small, m_full))
+    mp = torch.from_numpy(m_full).to(_dev())
+    outs = []
+    for plan in (full, small):
+        a = torch.zeros((nmaps, ncomp, plan.nalm), dtype=torch.complex128, device=_dev())
+        rms = torch.zeros((niter, nmaps * ncomp), dtype=torch.float64, device=_dev())
+        plan.sht_analysis_iter(mp, a, niter, rms)
+        torch.cuda.synchronize()
+        outs.append((a.cpu().numpy(), rms.cpu().numpy()))
+    assert np.array_equal(outs[0][0], outs[1][0])
+    # the per-map sum of squares is reduced with atomics: equal up to the summation order
+    assert np.allclose(outs[0][1], outs[1][1], rtol=1e-12, atol=0.0)
+    full.destroy()
+    small.destroy()
 
 
 def test_host_entries_match_device_entries():
