@@ -169,6 +169,8 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--nmaps", type=int, default=0, help="override the workload's map count (debug only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--pol", default="", choices=["", "E", "B"],
+                    help="spin-2 workloads: time the E-only / B-only transforms (PAPER.md:228) instead of the full ones")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
@@ -211,9 +213,21 @@ def main():
     plan_s = time.time() - t0
     stream = torch.cuda.current_stream()
 
-    def step():
-        plan.sht_synthesis(alm, maps, stream)
-        plan.sht_analysis(maps, alm_out, stream)
+    if args.pol:
+        assert spin == 2, "--pol needs a spin-2 workload (--config 4)"
+        which = 1 if args.pol == "E" else 2
+        c["name"] += "_%s_only" % args.pol
+        alm = alm[:, which - 1, :].contiguous()
+        alm_out = torch.empty_like(alm)
+        args.no_e2e = True
+
+        def step():
+            plan.sht_synthesis_pol(alm, maps, which, stream)
+            plan.sht_analysis_pol(maps, alm_out, which, stream)
+    else:
+        def step():
+            plan.sht_synthesis(alm, maps, stream)
+            plan.sht_analysis(maps, alm_out, stream)
 
     for _ in range(args.warmup):
         step()
@@ -246,7 +260,7 @@ def main():
     # ---- roofline of the dominant kernel: k_legendre_analysis (the slower of the two Legendre launches; the synthesis
     # kernel, same design, is reported beside it in "stages") ---------------------------------------------------------
     peaks, peak_src = read_measured_peaks()
-    fl_dir = legendre_flops_per_direction(c)
+    fl_dir = legendre_flops_per_direction(c) / (2 if args.pol else 1)   # half of the block products
     mma_peak = sht_measure_fp64_mma_peak(300.0)
     peak_note = ("FP64 DMMA.8x8x4 register-resident loop measured live in this run "
                  "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = %.1f; "
