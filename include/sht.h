@@ -85,6 +85,13 @@ sht_status_t sht_synthesis_pol(sht_plan_t plan, const double* alm, double* maps,
 sht_status_t sht_analysis_host(sht_plan_t plan, const double* maps_host, double* alm_host);
 sht_status_t sht_synthesis_host(sht_plan_t plan, const double* alm_host, double* maps_host);
 
+/* The paper's packed storage (eq. A7): all a_lm of one map in a real (lmax+1) x (lmax+1) matrix,
+ * row-major, Re a_lm at (row l, column m), Im a_lm (m >= 1) at (row l - m, column lmax - m + 1); Im a_l0 is not stored
+ * and reads back as 0 (0-based indices, reading G20).  Converters between it and the m-major `alm` layout:
+ * `rows` = nmaps * ncomp matrices, DEVICE pointers, asynchronous on `stream`; no plan needed. */
+sht_status_t sht_alm_pack_a7(int lmax, long long rows, const double* alm, double* packed, void* stream);
+sht_status_t sht_alm_unpack_a7(int lmax, long long rows, const double* packed, double* alm, void* stream);
+
 /* Introspection (host, pure). */
 long long sht_npix(int nside);                       /* 12 nside^2                                  */
 long long sht_nalm(int lmax);                        /* (lmax+1)(lmax+2)/2                          */

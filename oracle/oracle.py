@@ -146,3 +146,28 @@ def analysis_iter(nside, lmax, maps, niter, spin=0):
     rms = np.zeros((max(niter, 1), nm * nc))
     lib().oracle_analysis_iter(nside, lmax, nm, spin, _dp(maps), _dp(alm.view(np.float64)), niter, _dp(rms))
     return alm, rms[:niter]
+
+
+def pack_a7(lmax, alm):
+    """eq. A7, written out entry by entry: alm complex128 [rows][nalm] (m-major) ->
+    real squares [rows][lmax+1][lmax+1] with Re a_lm at (l, m) and Im a_lm (m >= 1) at (l - m, lmax - m + 1)."""
+    alm = np.asarray(alm, dtype=np.complex128).reshape(-1, nalm(lmax))
+    sq = np.zeros((alm.shape[0], lmax + 1, lmax + 1))
+    for m in range(lmax + 1):
+        for l in range(m, lmax + 1):
+            i = m * (2 * lmax + 1 - m) // 2 + l
+            sq[:, l, m] = alm[:, i].real
+            if m >= 1:
+                sq[:, l - m, lmax - m + 1] = alm[:, i].imag
+    return sq
+
+
+def unpack_a7(lmax, sq):
+    """inverse of pack_a7; Im a_l0 is not stored and comes back as 0"""
+    sq = np.asarray(sq, dtype=np.float64).reshape(-1, lmax + 1, lmax + 1)
+    alm = np.zeros((sq.shape[0], nalm(lmax)), dtype=np.complex128)
+    for m in range(lmax + 1):
+        for l in range(m, lmax + 1):
+            i = m * (2 * lmax + 1 - m) // 2 + l
+            alm[:, i] = sq[:, l, m] + (1j * sq[:, l - m, lmax - m + 1] if m >= 1 else 0.0)
+    return alm

@@ -35,6 +35,10 @@ _lib.sht_analysis_pol.argtypes = [_vp, _vp, _vp, _i, _vp]
 _lib.sht_analysis_pol.restype = _i
 _lib.sht_synthesis_pol.argtypes = [_vp, _vp, _vp, _i, _vp]
 _lib.sht_synthesis_pol.restype = _i
+_lib.sht_alm_pack_a7.argtypes = [_i, _ll, _vp, _vp, _vp]
+_lib.sht_alm_pack_a7.restype = _i
+_lib.sht_alm_unpack_a7.argtypes = [_i, _ll, _vp, _vp, _vp]
+_lib.sht_alm_unpack_a7.restype = _i
 _lib.sht_analysis_iter.argtypes = [_vp, _vp, _vp, _i, _vp, _vp]
 _lib.sht_analysis_iter.restype = _i
 _lib.sht_analysis_host.argtypes = [_vp, _vp, _vp]
@@ -65,7 +69,7 @@ _lib.sht_measure_fp64_mma_peak.argtypes = [_d]
 _lib.sht_measure_fp64_mma_peak.restype = _d
 
 EXPORTED = [
-    "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol",
+    "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol", "sht_alm_pack_a7", "sht_alm_unpack_a7",
     "sht_analysis_host", "sht_synthesis_host", "sht_npix", "sht_nalm", "sht_alm_index",
     "sht_plan_workspace_bytes", "sht_plan_chunk_maps", "sht_plan_kernel_launches", "sht_status_string",
     "sht_last_error", "sht_measure_fp64_mma_peak", "sht_plan_set_timing", "sht_plan_stage_ms",
@@ -94,6 +98,18 @@ def sht_status_string(status):
 
 def sht_measure_fp64_mma_peak(ms=200.0):
     return float(_lib.sht_measure_fp64_mma_peak(ms))
+
+
+def sht_alm_pack_a7(lmax, rows, alm, packed, stream=None):
+    st = _lib.sht_alm_pack_a7(lmax, rows, _ptr(alm), _ptr(packed), _stream(stream))
+    if st != SHT_OK:
+        raise ShtError("sht_alm_pack_a7: %s" % sht_status_string(st))
+
+
+def sht_alm_unpack_a7(lmax, rows, packed, alm, stream=None):
+    st = _lib.sht_alm_unpack_a7(lmax, rows, _ptr(packed), _ptr(alm), _stream(stream))
+    if st != SHT_OK:
+        raise ShtError("sht_alm_unpack_a7: %s" % sht_status_string(st))
 
 
 def _ptr(t):

@@ -33,6 +33,35 @@ __global__ void k_rms_finish(const double* __restrict__ acc, int n, double inv_n
     if (i < n) out[i] = sqrt(acc[i] * inv_npix);
 }
 
+// eq. A7: all a_lm of one map in a real (lmax+1) x (lmax+1) square,
+//   Re a_lm -> (l, m),   Im a_lm (m >= 1) -> (l - m, lmax - m + 1);   Im a_l0 is not stored (it is zero).
+// One thread per a_lm slot of the m-major ABI layout.
+template <bool PACK>
+__global__ void k_a7(int lmax, long long nalm, long long rows, double* __restrict__ alm, double* __restrict__ sq)
+{
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= rows * nalm) return;
+    const long long row = gid / nalm;
+    const long long idx = gid - row * nalm;
+    // m from idx = m (2 lmax + 1 - m)/2 + l: largest m with offset(m) + m <= idx
+    int m = (int)(((2.0 * lmax + 3.0) - sqrt((2.0 * lmax + 3.0) * (2.0 * lmax + 3.0) - 8.0 * (double)idx)) * 0.5);
+    if (m < 0) m = 0;
+    if (m > lmax) m = lmax;
+    while (m > 0 && (long long)m * (2 * lmax + 1 - m) / 2 + m > idx) --m;
+    while (m < lmax && (long long)(m + 1) * (2 * lmax - m) / 2 + (m + 1) <= idx) ++m;
+    const int l = (int)(idx - (long long)m * (2 * lmax + 1 - m) / 2);
+    const long long n1 = lmax + 1;
+    double* s = sq + row * n1 * n1;
+    double2* a = reinterpret_cast<double2*>(alm) + gid;
+    if (PACK) {
+        const double2 v = *a;
+        s[(long long)l * n1 + m] = v.x;
+        if (m >= 1) s[(long long)(l - m) * n1 + (lmax - m + 1)] = v.y;
+    } else {
+        *a = make_double2(s[(long long)l * n1 + m], m >= 1 ? s[(long long)(l - m) * n1 + (lmax - m + 1)] : 0.0);
+    }
+}
+
 // register-resident DMMA loop for the roofline denominator
 __global__ void k_mma_peak(double* out, int iters)
 {
@@ -301,6 +330,29 @@ extern "C" sht_status_t sht_analysis_host(sht_plan_t pl, const double* maps_host
 extern "C" sht_status_t sht_synthesis_host(sht_plan_t pl, const double* alm_host, double* maps_host)
 {
     return host_run(pl, alm_host, maps_host, false);
+}
+
+// ---- eq. A7 packed real-square a_lm format -----------------------------------------------------------------
+static sht_status_t a7_run(int lmax, long long rows, double* alm, double* sq, bool pack, void* stream)
+{
+    if (!alm || !sq) return SHT_ERR_NULL;
+    if (lmax < 0 || lmax > 16383 || rows < 0) return SHT_ERR_INVALID_ARG;
+    if (rows == 0) return SHT_OK;
+    const long long nalm = (long long)(lmax + 1) * (lmax + 2) / 2, total = rows * nalm;
+    const unsigned grid = (unsigned)((total + 255) / 256);
+    if (pack) k_a7<true><<<grid, 256, 0, (cudaStream_t)stream>>>(lmax, nalm, rows, alm, sq);
+    else k_a7<false><<<grid, 256, 0, (cudaStream_t)stream>>>(lmax, nalm, rows, alm, sq);
+    return cudaGetLastError() == cudaSuccess ? SHT_OK : SHT_ERR_CUDA;
+}
+
+extern "C" sht_status_t sht_alm_pack_a7(int lmax, long long rows, const double* alm, double* packed, void* stream)
+{
+    return a7_run(lmax, rows, const_cast<double*>(alm), packed, true, stream);
+}
+
+extern "C" sht_status_t sht_alm_unpack_a7(int lmax, long long rows, const double* packed, double* alm, void* stream)
+{
+    return a7_run(lmax, rows, alm, const_cast<double*>(packed), false, stream);
 }
 
 // ---- introspection -----------------------------------------------------------------------------------
