@@ -60,6 +60,17 @@ sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, int nmaps, in
 sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax, int nmaps, int spin, size_t workspace_limit);
 sht_status_t sht_plan_destroy(sht_plan_t plan);   /* NULL is a no-op returning SHT_OK */
 
+/* Where the P_lm (lambda) tiles of the Legendre stage are produced (spin-0 plans; both run the same recurrence from
+ * the same seeds and give bit-identical tiles, regenerated on every transform as in the paper):
+ *   SHT_LAMBDA_FUSED  : inside the DMMA contraction kernel, by its generator warps, tiles never leave shared memory;
+ *   SHT_LAMBDA_STAGED : by a separate kernel into an HBM scratch owned by the plan, streamed into the contraction
+ *                       kernel with one bulk copy per stage (a scalar FP64 instruction next to DMMA costs the FP64 pipe
+ *                       ~25 cycles on B200; this mode is the default when the scratch fits).
+ * sht_plan_set_lambda_mode returns SHT_ERR_UNSUPPORTED if the plan cannot run the requested mode. */
+enum { SHT_LAMBDA_FUSED = 0, SHT_LAMBDA_STAGED = 1 };
+sht_status_t sht_plan_set_lambda_mode(sht_plan_t plan, int mode);
+int sht_plan_lambda_mode(sht_plan_t plan);
+
 /* Alg. 1: maps (device, in) -> alm (device, out). */
 sht_status_t sht_analysis(sht_plan_t plan, const double* maps, double* alm, void* stream);
 /* eq. 4-5: alm (device, in) -> maps (device, out). */

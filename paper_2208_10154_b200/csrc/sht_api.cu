@@ -355,6 +355,19 @@ extern "C" sht_status_t sht_alm_unpack_a7(int lmax, long long rows, const double
     return a7_run(lmax, rows, alm, const_cast<double*>(packed), false, stream);
 }
 
+extern "C" sht_status_t sht_plan_set_lambda_mode(sht_plan_t pl, int mode)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (mode != SHT_LAMBDA_FUSED && mode != SHT_LAMBDA_STAGED) return SHT_ERR_INVALID_ARG;
+    if (mode == SHT_LAMBDA_STAGED && !pl->lam) {
+        snprintf(pl->err, sizeof(pl->err), "staged lambda mode needs a spin-0 plan whose scratch fits");
+        return SHT_ERR_UNSUPPORTED;
+    }
+    pl->lam_mode = mode;
+    return SHT_OK;
+}
+extern "C" int sht_plan_lambda_mode(sht_plan_t pl) { return pl ? pl->lam_mode : -1; }
+
 // ---- introspection -----------------------------------------------------------------------------------
 extern "C" long long sht_npix(int nside) { return 12LL * nside * nside; }
 extern "C" long long sht_nalm(int lmax) { return (long long)(lmax + 1) * (lmax + 2) / 2; }
@@ -363,7 +376,7 @@ extern "C" long long sht_alm_index(int lmax, int l, int m)
     if (lmax < 0 || m < 0 || l < m || l > lmax) return -1;
     return (long long)m * (2 * lmax + 1 - m) / 2 + l;
 }
-extern "C" size_t sht_plan_workspace_bytes(sht_plan_t pl) { return pl ? pl->F_bytes + pl->table_bytes : 0; }
+extern "C" size_t sht_plan_workspace_bytes(sht_plan_t pl) { return pl ? pl->F_bytes + pl->table_bytes + pl->lam_bytes : 0; }
 extern "C" int sht_plan_chunk_maps(sht_plan_t pl) { return pl ? pl->chunk : 0; }
 extern "C" long long sht_plan_kernel_launches(sht_plan_t pl) { return pl ? pl->launches : 0; }
 extern "C" const char* sht_status_string(sht_status_t s)

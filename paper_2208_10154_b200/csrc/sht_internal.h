@@ -73,6 +73,13 @@ struct DevicePlan {
     const int* mlim;                // [nh] copy of RingPair::mlim (monotone non-decreasing in p)
     const int* pst;                 // [lmax+1][ntile_max] first ring pair that takes part in l tile t of order m
     int ntile_max;                  // l tiles of order 0
+    // staged-lambda mode (spin 0): lambda tiles are written by a generator kernel to a scratch in HBM, block by block in
+    // the order the contraction kernels consume them, and fetched with one bulk copy per stage
+    const int* ablk_off;            // [lmax+1][ntile_max] first analysis block (32 rings x 128 l) of (m, l tile)
+    const int* sblk_off;            // [lmax+1][npb] first synthesis block (32 l x 64 rings) of (m, ring block)
+    const int* scfirst;             // [lmax+1][npb] first l of the first synthesis block (lmax + 1: none)
+    int npb;                        // ring blocks of 64
+    int nck_max, nst_max;           // most analysis chunks per (m, tile), most synthesis stages per (m, ring block)
 };
 
 // Workspace F (both directions): T_m^k(theta) of PAPER.md:52 for one chunk of maps,
@@ -102,6 +109,11 @@ struct sht_plan_s {
     size_t class_smem[sht::RING_NCLASS];
     int sm_count;
     long long launches;
+    double* lam;                    // staged-lambda scratch (nullptr: fused generation inside the contraction kernels)
+    size_t lam_bytes;
+    int* lam_i0;                    // [analysis blocks] first 16-row block with a started recurrence
+    int lam_mode;                   // SHT_LAMBDA_FUSED / SHT_LAMBDA_STAGED
+    long long n_ablk, n_sblk;
     int pol;                        // spin 2: 0 = E and B, 1 = E only, 2 = B only (set by the *_pol entries around a call)
     char err[512];
     // host-entry staging (allocated on first use)
@@ -130,6 +142,8 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
                                      bool accumulate, cudaStream_t st);
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
 size_t legendre_smem_bytes(int nh, int ntile_max);
+constexpr size_t LAM_ABLK_BYTES = 2 * 32 * 66 * 8;      // one analysis lambda block: [class][32 rings][66] doubles
+constexpr size_t LAM_SBLK_BYTES = 32 * 66 * 8;          // one synthesis lambda block: [32 l][66] doubles
 // spin 2 (sht_legendre_spin2.cu); the spin-0 launchers dispatch to these
 cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                            bool accumulate, cudaStream_t st);

@@ -41,12 +41,101 @@ constexpr int S_SC = NK + 8;                 // epilogue staging row stride (dou
 static_assert(2 * S_PB * S_SC * 8 <= S_STAGES * S_STAGE_BYTES, "epilogue staging reuses the stage memory");
 
 // ------------------------------------------------------------------------------------------------
+// Staged-lambda mode: the lambda tiles of one transform, written block by block to an HBM scratch in exactly the
+// layout and order the contraction kernels consume them (same recurrence, same seeds, same arithmetic as the fused
+// generators: bit-identical tiles).  Here the scalar FP64 work runs at the full DFMA rate, away from the DMMA pipe.
+// ------------------------------------------------------------------------------------------------
+static_assert(LAM_ABLK_BYTES == (size_t)A_LBYTES && LAM_SBLK_BYTES == (size_t)S_LBYTES, "block sizes");
+
+// analysis block (m, l tile, chunk of 32 rings): [class][ring][A_SL]; 128 threads: warp = 32 l rows, lane = ring
+__global__ void __launch_bounds__(128) k_lambda_blocks_analysis(DevicePlan d, double* __restrict__ lam, int* __restrict__ i0tab)
+{
+    __shared__ __align__(16) double tile[2 * A_PC * A_SL];
+    const int m = blockIdx.y, lmax = d.lmax, nh = d.nh;
+    const int t = blockIdx.x / d.nck_max, ck = blockIdx.x % d.nck_max;
+    if (t > (lmax - m) / A_ML) return;
+    const int pc = d.pst[(size_t)m * d.ntile_max + t] + A_PC * ck;
+    if (pc >= nh) return;
+    const size_t blk = (size_t)d.ablk_off[(size_t)m * d.ntile_max + t] + ck;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int l0 = m + t * A_ML, lw = l0 + 32 * w;
+    const int p = pc + lane;
+    for (int i = threadIdx.x; i < 2 * A_PC * A_SL; i += 128) tile[i] = 0.0;      // padding columns included
+    __syncthreads();
+    double x1 = 0.0, x2 = 0.0, z = 0.0;
+    int ls = lmax + 1;
+    if (p < nh) {
+        z = d.z[p];
+        ls = d.lstart[(size_t)m * nh + p];
+        if (lw <= lmax) {
+            const double2 sd = d.cseed[((size_t)d.csoff[m] + (lw - m) / LEG_CS) * nh + p];
+            x1 = sd.x; x2 = sd.y;
+        }
+    }
+    const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+    const int rs = ls - lw;
+#pragma unroll 4
+    for (int r = 0; r < 32; ++r) {
+        const int l = lw + r;
+        const double2 ab = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+        const double tv = fma(ab.x * z, x1, -(ab.y * x2));
+        const bool on = r >= rs;
+        x2 = on ? x1 : x2; x1 = on ? tv : x1;
+        const int rr = 32 * w + r;
+        tile[(rr & 1) * (A_PC * A_SL) + lane * A_SL + (rr >> 1)] = on ? tv : 0.0;
+    }
+    if (w == 0) {                                           // first 16-row block with a started recurrence
+        int lsmin = ls;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) lsmin = min(lsmin, __shfl_xor_sync(0xffffffffu, lsmin, o));
+        if (lane == 0) i0tab[blk] = max(0, min(8, (lsmin - l0) >> 4));
+    }
+    __syncthreads();
+    double2* dst = reinterpret_cast<double2*>(lam + blk * (size_t)(A_LBYTES / 8));
+    const double2* src = reinterpret_cast<const double2*>(tile);
+    for (int i = threadIdx.x; i < A_LBYTES / 16; i += 128) dst[i] = src[i];
+}
+
+// synthesis block (m, block of 64 rings, stage of 32 l): [l][S_SL]; 64 threads = rings (stores are coalesced over rings)
+__global__ void __launch_bounds__(64) k_lambda_blocks_synthesis(DevicePlan d, double* __restrict__ lam)
+{
+    const int m = blockIdx.z, pbi = blockIdx.y, n = blockIdx.x, lmax = d.lmax, nh = d.nh;
+    const int cfirst = d.scfirst[(size_t)m * d.npb + pbi];
+    const int lc = cfirst + S_LC * n;
+    if (cfirst > lmax || lc > lmax) return;
+    const size_t blk = (size_t)d.sblk_off[(size_t)m * d.npb + pbi] + n;
+    const int p = pbi * S_PB + threadIdx.x;
+    double x1 = 0.0, x2 = 0.0, z = 0.0;
+    int ls = lmax + 1;
+    if (p < nh) {
+        z = d.z[p];
+        ls = d.lstart[(size_t)m * nh + p];
+        const double2 sd = d.cseed[((size_t)d.csoff[m] + (lc - m) / LEG_CS) * nh + p];
+        x1 = sd.x; x2 = sd.y;
+    }
+    const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+    double* dst = lam + blk * (size_t)(S_LBYTES / 8) + threadIdx.x;
+    const int rs = ls - lc;
+#pragma unroll 4
+    for (int r = 0; r < S_LC; ++r) {
+        const int l = lc + r;
+        const double2 ab = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+        const double tv = fma(ab.x * z, x1, -(ab.y * x2));
+        const bool on = r >= rs;
+        x2 = on ? x1 : x2; x1 = on ? tv : x1;
+        dst[r * S_SL] = on ? tv : 0.0;
+    }
+    if (threadIdx.x < S_SL - S_PB)                          // padding columns
+        for (int r = 0; r < S_LC; ++r) dst[r * S_SL + S_PB] = 0.0;
+}
+
+// ------------------------------------------------------------------------------------------------
 // analysis kernel: one CTA per (m, k-tile); l tiles outer, ring chunks inner.
 // Stage layout: [X: 2 boxes x (16 kg x 16 p x 128 B, 128B-swizzled)] [lambda: 2 classes x 32 p x A_SL]
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
-                    int nkt, int accumulate)
+                    int nkt, int accumulate, const double* __restrict__ lam, const int* __restrict__ i0tab)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
@@ -68,7 +157,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
 
     for (int t = tix; t < ntile; t += LEG_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
     if (tix == 0) {
-        for (int s = 0; s < A_STAGES; ++s) { mbar_init(full + s, 1 + 64); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
+        for (int s = 0; s < A_STAGES; ++s) { mbar_init(full + s, lam ? 1 : 1 + 64); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
         fence_barrier_init();
         tma_prefetch_desc(&tmF);
     }
@@ -156,6 +245,29 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
         // the chunk.  The recurrence restarts from the plan's state table at l0 and l0 + 64, so the two halves of a
         // stage are generated at the same time.  Lane 0 of the first-half warp also issues the stage's TMA loads.
         const int gw = warp + LEG_GEN_WARPS;
+        if (lam) {
+            // ===== staged mode: one thread streams, per stage, the chunk's operand lines (TMA) and its lambda block (bulk
+            // copy from the scratch the generator kernel filled), and hands the consumers the block's first active row
+            if (gw != 0 || lane != 0) return;
+            int chunk = 0;
+            for (int tile = 0; tile < ntile; ++tile) {
+                const size_t blk0 = (size_t)d.ablk_off[(size_t)m * d.ntile_max + tile];
+                int ck = 0;
+                for (int pc = pst[tile]; pc < nh; pc += A_PC, ++chunk, ++ck) {
+                    const int stage = chunk & 1;
+                    const uint32_t phase = (chunk >> 1) & 1;
+                    const int i0v = __ldg(i0tab + blk0 + ck);
+                    mbar_wait(empty + stage, phase ^ 1);
+                    unsigned char* Xs = stage_base + (size_t)stage * A_STAGE_BYTES;
+                    i0s[stage] = i0v;
+                    mbar_arrive_expect_tx(full + stage, A_XBYTES + A_LBYTES);
+                    tma_load_4d(Xs, &tmF, full + stage, 0, pc, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
+                    tma_load_4d(Xs + A_XBYTES / 2, &tmF, full + stage, 0, pc + 16, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
+                    bulk_load(Xs + A_XBYTES, lam + (blk0 + ck) * (size_t)(A_LBYTES / 8), A_LBYTES, full + stage);
+                }
+            }
+            return;
+        }
         const int gs = gw & 1, gh = gw >> 1;
         const int gl = gw * 32 + lane;                          // 0 .. 127 = one l of the tile per thread
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
@@ -239,7 +351,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
-                     int nkt, int npb)
+                     int nkt, int npb, const double* __restrict__ lam)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
@@ -265,7 +377,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
     if (m >= d.mlim[plast]) return;                    // no ring of this block takes part in order m (never read)
 
     if (tix == 0) {
-        for (int s = 0; s < S_STAGES; ++s) { mbar_init(full + s, 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
+        for (int s = 0; s < S_STAGES; ++s) { mbar_init(full + s, lam ? 1 : 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
         fence_barrier_init();
         tma_prefetch_desc(&tmA);
         *lmin_s = lmax + 1;
@@ -379,6 +491,24 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
         // at the same time.  Lane 0 of generator 0 also issues the stage's TMA loads (a_lm, straight from the m-major
         // ABI layout).
         const int gw = warp + LEG_GEN_WARPS;
+        if (lam) {
+            // ===== staged mode: one thread streams, per stage, the a_lm boxes (TMA) and the lambda block (bulk copy)
+            if (gw != 0 || lane != 0) return;
+            const size_t blk0 = (size_t)d.sblk_off[(size_t)m * d.npb + pbi];
+            const int row0s = (k0 + kt * KTILE_MAPS) * d.ncomp + comp;
+            int stage = 0, n = 0; uint32_t phase = 0;
+            for (int lc = cfirst; lc <= lmax; lc += S_LC, ++n) {
+                mbar_wait(empty + stage, phase ^ 1);
+                unsigned char* As = stage_base + (size_t)stage * S_STAGE_BYTES;
+                mbar_arrive_expect_tx(full + stage, S_ABYTES + S_LBYTES);
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    tma_load_2d(As + q * (S_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0s);
+                bulk_load(As + S_ABYTES, lam + (blk0 + n) * (size_t)(S_LBYTES / 8), S_LBYTES, full + stage);
+                if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
+            }
+            return;
+        }
         const int gh = gw >> 1;
         const int rl = (gw & 1) * 32 + lane;
         const int p = pb + rl;
@@ -498,7 +628,13 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
     if (e != cudaSuccess) return e;
     CUtensorMap tmF;
     if ((e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, &tmF)) != cudaSuccess) return e;
-    k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
+    const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
+    if (staged) {
+        k_lambda_blocks_analysis<<<dim3((unsigned)(d.ntile_max * d.nck_max), (unsigned)(d.lmax + 1)), 128, 0, st>>>(d, pl->lam, pl->lam_i0);
+        pl->launches++;
+    }
+    k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0,
+                                                       staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -513,7 +649,12 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
     if ((e = make_tmap_alm(d, alm, (long long)(k0 + kmaps) * d.ncomp, &tmA)) != cudaSuccess) return e;
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
-    k_legendre_synthesis<<<(d.lmax + 1) * nkt * npb, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb);
+    const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
+    if (staged && d.nst_max > 0) {
+        k_lambda_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
+        pl->launches++;
+    }
+    k_legendre_synthesis<<<(d.lmax + 1) * nkt * npb, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr);
     pl->launches++;
     return cudaGetLastError();
 }

@@ -493,6 +493,41 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             for (int t = 1; t < nt; ++t) if (row[t - 1] < row[t]) row[t] = row[t - 1];
         }
         if ((ce = upload(pl, pst, &d.pst)) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+        // block tables of the staged-lambda mode (the same loops as the contraction kernels)
+        {
+            d.npb = (d.nh + 63) / 64;
+            std::vector<int> aoff((size_t)(lmax + 1) * d.ntile_max, 0), soff((size_t)(lmax + 1) * d.npb, 0),
+                scf((size_t)(lmax + 1) * d.npb, lmax + 1);
+            long long na = 0, nsb = 0;
+            d.nck_max = 0; d.nst_max = 0;
+            for (int m = 0; m <= lmax; ++m) {
+                const int nt = (lmax - m) / LEG_A_ML + 1;
+                for (int t = 0; t < nt; ++t) {
+                    aoff[(size_t)m * d.ntile_max + t] = (int)na;
+                    const int p0 = pst[(size_t)m * d.ntile_max + t];
+                    const int nck = p0 < d.nh ? (d.nh - p0 + 31) / 32 : 0;
+                    na += nck;
+                    if (nck > d.nck_max) d.nck_max = nck;
+                }
+                for (int b = 0; b < d.npb; ++b) {
+                    soff[(size_t)m * d.npb + b] = (int)nsb;
+                    const int plast = (b * 64 + 64 < d.nh ? b * 64 + 64 : d.nh) - 1;
+                    if (m >= mlim[plast]) continue;
+                    int lmin = lmax + 1;
+                    for (int p = b * 64; p <= plast; ++p) lmin = hls[(size_t)m * d.nh + p] < lmin ? hls[(size_t)m * d.nh + p] : lmin;
+                    if (lmin > lmax) continue;
+                    const int cf = m + ((lmin - m) / 32) * 32;
+                    scf[(size_t)m * d.npb + b] = cf;
+                    const int nst = (lmax - cf) / 32 + 1;
+                    nsb += nst;
+                    if (nst > d.nst_max) d.nst_max = nst;
+                }
+            }
+            pl->n_ablk = na; pl->n_sblk = nsb;
+            if (na > 0x7fffffffLL || nsb > 0x7fffffffLL) { sht_plan_destroy(pl); return SHT_ERR_UNSUPPORTED; }
+            if (upload(pl, aoff, &d.ablk_off) != cudaSuccess || upload(pl, soff, &d.sblk_off) != cudaSuccess ||
+                upload(pl, scf, &d.scfirst) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+        }
         if ((ce = upload(pl, rings, &d.rings)) != cudaSuccess || (ce = upload(pl, mlim, &d.mlim)) != cudaSuccess) {
             sht_plan_destroy(pl);
             return SHT_ERR_ALLOC;
@@ -541,6 +576,23 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
         // padded map columns are never written by the ring kernels: keep them finite (zero) forever
         if (cudaMemset(pl->F, 0, pl->F_bytes) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
     }
+    // ---- staged-lambda scratch (spin 0): default mode when it fits beside the workspace ------------------------
+    pl->lam = nullptr; pl->lam_i0 = nullptr; pl->lam_mode = SHT_LAMBDA_FUSED; pl->lam_bytes = 0;
+    if (spin == 0) {
+        size_t freeb = 0, totalb = 0;
+        cudaMemGetInfo(&freeb, &totalb);
+        const size_t a = (size_t)pl->n_ablk * LAM_ABLK_BYTES, sb = (size_t)pl->n_sblk * LAM_SBLK_BYTES;
+        const size_t need = (a > sb ? a : sb) + 1024;
+        if (need <= ((size_t)40 << 30) && need <= freeb / 4) {
+            if (cudaMalloc(&pl->lam, need) == cudaSuccess && cudaMalloc(&pl->lam_i0, ((size_t)pl->n_ablk + 1) * sizeof(int)) == cudaSuccess) {
+                pl->lam_bytes = need;
+                pl->lam_mode = SHT_LAMBDA_STAGED;
+            } else {
+                cudaGetLastError();
+                if (pl->lam) { cudaFree(pl->lam); pl->lam = nullptr; }
+            }
+        }
+    }
     if (cudaDeviceSynchronize() != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
     pl->err[0] = 0;
     (void)fail;
@@ -554,6 +606,8 @@ extern "C" sht_status_t sht_plan_destroy(sht_plan_t pl)
     cudaDeviceSynchronize();
     for (int i = 0; i < pl->n_allocs; ++i) cudaFree(pl->dev_allocs[i]);
     if (pl->F) cudaFree(pl->F);
+    if (pl->lam) cudaFree(pl->lam);
+    if (pl->lam_i0) cudaFree(pl->lam_i0);
     for (int i = 0; i < 256; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
         if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
