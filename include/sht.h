@@ -60,7 +60,7 @@ sht_status_t sht_plan_create(sht_plan_t* out, int nside, int lmax, int nmaps, in
 sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax, int nmaps, int spin, size_t workspace_limit);
 sht_status_t sht_plan_destroy(sht_plan_t plan);   /* NULL is a no-op returning SHT_OK */
 
-/* Where the P_lm (lambda) tiles of the Legendre stage are produced (spin-0 plans; both run the same recurrence from
+/* Where the P_lm (lambda; spin 2: F+/F-) tiles of the Legendre stage are produced (both run the same recurrence from
  * the same seeds and give bit-identical tiles, regenerated on every transform as in the paper):
  *   SHT_LAMBDA_FUSED  : inside the DMMA contraction kernel, by its generator warps, tiles never leave shared memory;
  *   SHT_LAMBDA_STAGED : by a separate kernel into an HBM scratch owned by the plan, streamed into the contraction

@@ -360,7 +360,7 @@ extern "C" sht_status_t sht_plan_set_lambda_mode(sht_plan_t pl, int mode)
     if (!pl) return SHT_ERR_NULL;
     if (mode != SHT_LAMBDA_FUSED && mode != SHT_LAMBDA_STAGED) return SHT_ERR_INVALID_ARG;
     if (mode == SHT_LAMBDA_STAGED && !pl->lam) {
-        snprintf(pl->err, sizeof(pl->err), "staged lambda mode needs a spin-0 plan whose scratch fits");
+        snprintf(pl->err, sizeof(pl->err), "staged lambda mode needs a plan whose scratch fits");
         return SHT_ERR_UNSUPPORTED;
     }
     pl->lam_mode = mode;

@@ -150,7 +150,6 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
     const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) - LEG_GEN_WARPS;
     const int tix = threadIdx.x;
-    const int tid = tix - LEG_GEN_WARPS * 32;                  // consumer thread index (negative for generators)
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
     const int ntile = (lmax - m) / A_ML + 1;

@@ -54,6 +54,119 @@ __device__ __forceinline__ void spin2_consts(const DevicePlan& d, int l, int m, 
 }
 
 // ------------------------------------------------------------------------------------------------
+// Staged-lambda mode (see sht_legendre.cu): F+/F- tiles written block by block to the plan's scratch, in the layout
+// and order the contraction kernels consume them; same arithmetic as the fused generators (bit-identical tiles).
+// ------------------------------------------------------------------------------------------------
+static_assert(LAM_ABLK_BYTES == (size_t)A2_LBYTES && 2 * LAM_SBLK_BYTES == (size_t)S2_LBYTES, "block sizes");
+
+// analysis block (m, l tile, chunk of 16 rings): [sign][class][ring][A2_SL]; warp = 32 l rows, lane = ring + 16 sign
+__global__ void __launch_bounds__(128) k_fpm_blocks_analysis(DevicePlan d, double* __restrict__ lam)
+{
+    __shared__ __align__(16) double tile[A2_LBYTES / 8];
+    __shared__ double2 cft[A2_ML], ctu[2 * A2_ML];
+    __shared__ double ct3[A2_ML];
+    const int m = blockIdx.y, lmax = d.lmax, nh = d.nh;
+    const int t = blockIdx.x / d.nck_max, ck = blockIdx.x % d.nck_max;
+    if (t > (lmax - m) / A2_ML) return;
+    const int pc = d.pst[(size_t)m * d.ntile_max + t] + A2_PC * ck;
+    if (pc >= nh) return;
+    const size_t blk = (size_t)d.ablk_off[(size_t)m * d.ntile_max + t] + ck;
+    const int lane = threadIdx.x & 31, gw = threadIdx.x >> 5;
+    const int rr = lane & 15, sg = lane >> 4;
+    const int l0 = m + t * A2_ML;
+    const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+    {
+        const int l = l0 + threadIdx.x;
+        double2 tp, tm; double t3;
+        spin2_consts(d, l, m, tp, tm, t3);
+        cft[threadIdx.x] = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+        ctu[threadIdx.x] = tp; ctu[A2_ML + threadIdx.x] = tm; ct3[threadIdx.x] = t3;
+    }
+    for (int i = threadIdx.x; i < A2_LBYTES / 8; i += 128) tile[i] = 0.0;
+    __syncthreads();
+    constexpr int QL = A2_ML / 4;
+    const int lq = l0 + QL * gw;
+    const int p = pc + rr;
+    double x1 = 0.0, x2 = 0.0, z = 0.0, is2 = 0.0;
+    int ls = lmax + 1;
+    if (p < nh && lq <= lmax) {
+        const double2 sd = d.cseed[((size_t)d.csoff[m] + (lq - m) / LEG_CS) * nh + p];
+        x1 = sd.x; x2 = sd.y; z = d.z[p]; is2 = 1.0 / d.sin2[p];
+        ls = d.lstart[(size_t)m * nh + p];
+    }
+    const double ra = sg ? (double)m * z * is2 : is2;
+    const double rc = sg ? (double)m * is2 : z * is2;
+    const int rs = ls - lq;
+    double* Ls = tile + (sg * 2 * A2_PC + rr) * A2_SL + (QL / 2) * gw;
+    const double2* cfq = cft + QL * gw;
+    const double2* tu = ctu + sg * A2_ML + QL * gw;
+    const double* t3q = ct3 + QL * gw;
+#pragma unroll 4
+    for (int r = 0; r < QL; ++r) {
+        const double2 ab = cfq[r];
+        const double2 uv = tu[r];
+        const double t3 = t3q[r];
+        const double lamv = fma(ab.x * z, x1, -(ab.y * x2));
+        const double U = fma(uv.x, ra, uv.y), W = t3 * rc;
+        const double f = fma(lamv, U, -(x1 * W));
+        const bool on = r >= rs;
+        x2 = on ? x1 : x2; x1 = on ? lamv : x1;
+        Ls[(r & 1) * (A2_PC * A2_SL) + (r >> 1)] = on ? f : 0.0;
+    }
+    __syncthreads();
+    double2* dst = reinterpret_cast<double2*>(lam + blk * (size_t)(A2_LBYTES / 8));
+    const double2* src = reinterpret_cast<const double2*>(tile);
+    for (int i = threadIdx.x; i < A2_LBYTES / 16; i += 128) dst[i] = src[i];
+}
+
+// synthesis block (m, block of 64 rings, stage of 32 l): [sign][l][S2_SL]; 64 threads = rings, a thread forms F+ and F-
+__global__ void __launch_bounds__(64) k_fpm_blocks_synthesis(DevicePlan d, double* __restrict__ lam)
+{
+    __shared__ double2 cab[S2_LC], ctp[S2_LC], ctm[S2_LC];
+    const int m = blockIdx.z, pbi = blockIdx.y, n = blockIdx.x, lmax = d.lmax, nh = d.nh;
+    const int cfirst = d.scfirst[(size_t)m * d.npb + pbi];
+    const int lc = cfirst + S2_LC * n;
+    if (cfirst > lmax || lc > lmax) return;
+    const size_t blk = (size_t)d.sblk_off[(size_t)m * d.npb + pbi] + n;
+    const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
+    if (threadIdx.x < S2_LC) {
+        const int l = lc + threadIdx.x;
+        double2 tp, tm; double t3;
+        spin2_consts(d, l, m, tp, tm, t3);
+        cab[threadIdx.x] = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
+        ctp[threadIdx.x] = tp; ctm[threadIdx.x] = make_double2(tm.x, t3);
+    }
+    __syncthreads();
+    const int p = pbi * S2_PB + threadIdx.x;
+    double x1 = 0.0, x2 = 0.0, z = 0.0, is2 = 0.0;
+    int ls = lmax + 1;
+    if (p < nh) {
+        z = d.z[p]; is2 = 1.0 / d.sin2[p];
+        ls = d.lstart[(size_t)m * nh + p];
+        const double2 sd = d.cseed[((size_t)d.csoff[m] + (lc - m) / LEG_CS) * nh + p];
+        x1 = sd.x; x2 = sd.y;
+    }
+    const double rap = is2, rcp = z * is2;
+    const double ram = (double)m * z * is2, rcm = (double)m * is2;
+    double* Lp = lam + blk * (size_t)(S2_LBYTES / 8) + threadIdx.x;
+    double* Lm = Lp + S2_LC * S2_SL;
+    const int rs = ls - lc;
+#pragma unroll 4
+    for (int r = 0; r < S2_LC; ++r) {
+        const double2 ab = cab[r], tp = ctp[r], tm = ctm[r];
+        const double lamv = fma(ab.x * z, x1, -(ab.y * x2));
+        const double fp = fma(lamv, fma(tp.x, rap, tp.y), -(x1 * (tm.y * rcp)));
+        const double fm = fma(lamv, tm.x * ram, -(x1 * (tm.y * rcm)));
+        const bool on = r >= rs;
+        x2 = on ? x1 : x2; x1 = on ? lamv : x1;
+        Lp[r * S2_SL] = on ? fp : 0.0;
+        Lm[r * S2_SL] = on ? fm : 0.0;
+    }
+    if (threadIdx.x < S2_SL - S2_PB)
+        for (int r = 0; r < S2_LC; ++r) { Lp[r * S2_SL + S2_PB] = 0.0; Lm[r * S2_SL + S2_PB] = 0.0; }
+}
+
+// ------------------------------------------------------------------------------------------------
 // analysis, spin 2: one CTA per (m, k-tile of 32 pairs); l tiles outer, ring chunks of 16 inner.
 // Stage: [X: comp(Q,iU) x 8 kg x 16 p x 128 B, 128B-swizzled] [F: sign(+,-) x class x 16 p x A2_SL]
 // ------------------------------------------------------------------------------------------------
@@ -62,7 +175,7 @@ __device__ __forceinline__ void spin2_consts(const DevicePlan& d, int l, int m, 
 template <int WHICH>
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
-                          int nkt, int accumulate)
+                          int nkt, int accumulate, const double* __restrict__ lam)
 {
     constexpr int nst = 3;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -81,7 +194,7 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
 
     for (int t = tid; t < ntile; t += LEG2_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
     if (tid == 0) {
-        for (int s = 0; s < nst; ++s) { mbar_init(full + s, 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS_S2); }
+        for (int s = 0; s < nst; ++s) { mbar_init(full + s, lam ? 1 : 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS_S2); }
         fence_barrier_init();
         tma_prefetch_desc(&tmF);
     }
@@ -168,6 +281,24 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
         // tile (the recurrence restarts from the plan's state table every 16 l); lane = (ring 0..15) + 16 (sign of F).
         // Lane 0 of generator 0 also issues the TMA load of the chunk's Q / iU lines as soon as the stage is free.
         const int gw = warp - 8;
+        if (lam) {
+            // ===== staged mode: one thread streams, per stage, the chunk's Q / iU lines (TMA) and its F+/F- block (bulk copy)
+            if (gw != 0 || lane != 0) return;
+            int stage = 0; uint32_t phase = 0;
+            for (int tile = 0; tile < ntile; ++tile) {
+                const size_t blk0 = (size_t)d.ablk_off[(size_t)m * d.ntile_max + tile];
+                int ck = 0;
+                for (int pc = pst[tile]; pc < nh; pc += A2_PC, ++ck) {
+                    mbar_wait(empty + stage, phase ^ 1);
+                    unsigned char* Xs = stage_base + (size_t)stage * A2_STAGE_BYTES;
+                    mbar_arrive_expect_tx(full + stage, A2_XBYTES + A2_LBYTES);
+                    tma_load_4d(Xs, &tmF, full + stage, 0, pc, kt * P_KG, m * 2);
+                    bulk_load(Xs + A2_XBYTES, lam + (blk0 + ck) * (size_t)(A2_LBYTES / 8), A2_LBYTES, full + stage);
+                    if (++stage == nst) { stage = 0; phase ^= 1; }
+                }
+            }
+            return;
+        }
         const int rr = lane & 15, sg = lane >> 4;
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
         const double2* csm = d.cseed + (size_t)d.csoff[m] * nh;
@@ -241,7 +372,7 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
 template <int WHICH>
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
-                           int nkt, int npb)
+                           int nkt, int npb, const double* __restrict__ lam)
 {
     constexpr int NST = 3;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -261,7 +392,7 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
     if (m >= d.mlim[plast]) return;                    // no ring of this block takes part in order m (never read)
 
     if (tid == 0) {
-        for (int s = 0; s < NST; ++s) { mbar_init(full + s, 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS_S2); }
+        for (int s = 0; s < NST; ++s) { mbar_init(full + s, lam ? 1 : 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS_S2); }
         fence_barrier_init();
         tma_prefetch_desc(&tmA);
         *lmin_s = lmax + 1;
@@ -371,6 +502,23 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
         // and F- of its ring; the recurrence restarts from the plan's state table every 16 l.  Lane 0 of generator 0
         // issues the TMA loads of a_E / a_B for the stage.
         const int gw = warp - 8;
+        if (lam) {
+            // ===== staged mode: one thread streams, per stage, the a_E / a_B boxes (TMA) and the F+/F- block (bulk copy)
+            if (gw != 0 || lane != 0) return;
+            const size_t blk0 = (size_t)d.sblk_off[(size_t)m * d.npb + pbi];
+            int stage = 0, n = 0; uint32_t phase = 0;
+            for (int lc = cfirst; lc <= lmax; lc += S2_LC, ++n) {
+                mbar_wait(empty + stage, phase ^ 1);
+                unsigned char* As = stage_base + (size_t)stage * S2_STAGE_BYTES;
+                mbar_arrive_expect_tx(full + stage, S2_ABYTES + S2_LBYTES);
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    tma_load_3d(As + q * (S2_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), k0 + kt * P_KT, 0);
+                bulk_load(As + S2_ABYTES, lam + (blk0 + n) * (size_t)(S2_LBYTES / 8), S2_LBYTES, full + stage);
+                if (++stage == NST) { stage = 0; phase ^= 1; }
+            }
+            return;
+        }
         const int gh = gw >> 1;
         const int rl = (gw & 1) * 32 + lane;
         const int p = pb + rl;
@@ -468,7 +616,12 @@ cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, 
     CUtensorMap tmF;
     if ((e = make_tmap_F(d, F, P_KG, 2, &tmF)) != cudaSuccess) return e;
     const int nkt = (kmaps + P_KT - 1) / P_KT;
-    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0);
+    const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
+    if (staged) {
+        k_fpm_blocks_analysis<<<dim3((unsigned)(d.ntile_max * d.nck_max), (unsigned)(d.lmax + 1)), 128, 0, st>>>(d, pl->lam);
+        pl->launches++;
+    }
+    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, staged ? pl->lam : nullptr);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -484,7 +637,12 @@ cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d,
     if ((e = make_tmap_alm_spin2(d, alm, (long long)(k0 + kmaps), pl->pol ? 1 : 2, &tmA)) != cudaSuccess) return e;
     const int nkt = (kmaps + P_KT - 1) / P_KT;
     const int npb = (d.nh + S2_PB - 1) / S2_PB;
-    kern<<<(d.lmax + 1) * nkt * npb, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb);
+    const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
+    if (staged && d.nst_max > 0) {
+        k_fpm_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
+        pl->launches++;
+    }
+    kern<<<(d.lmax + 1) * nkt * npb, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr);
     pl->launches++;
     return cudaGetLastError();
 }

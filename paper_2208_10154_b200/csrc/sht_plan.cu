@@ -505,7 +505,8 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
                 for (int t = 0; t < nt; ++t) {
                     aoff[(size_t)m * d.ntile_max + t] = (int)na;
                     const int p0 = pst[(size_t)m * d.ntile_max + t];
-                    const int nck = p0 < d.nh ? (d.nh - p0 + 31) / 32 : 0;
+                    const int apc = spin == 2 ? 16 : 32;               // rings per analysis stage
+                    const int nck = p0 < d.nh ? (d.nh - p0 + apc - 1) / apc : 0;
                     na += nck;
                     if (nck > d.nck_max) d.nck_max = nck;
                 }
@@ -576,12 +577,12 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
         // padded map columns are never written by the ring kernels: keep them finite (zero) forever
         if (cudaMemset(pl->F, 0, pl->F_bytes) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
     }
-    // ---- staged-lambda scratch (spin 0): default mode when it fits beside the workspace ------------------------
+    // ---- staged-lambda scratch: default mode when it fits beside the workspace ------------------------
     pl->lam = nullptr; pl->lam_i0 = nullptr; pl->lam_mode = SHT_LAMBDA_FUSED; pl->lam_bytes = 0;
-    if (spin == 0) {
+    {
         size_t freeb = 0, totalb = 0;
         cudaMemGetInfo(&freeb, &totalb);
-        const size_t a = (size_t)pl->n_ablk * LAM_ABLK_BYTES, sb = (size_t)pl->n_sblk * LAM_SBLK_BYTES;
+        const size_t a = (size_t)pl->n_ablk * LAM_ABLK_BYTES, sb = (size_t)pl->n_sblk * LAM_SBLK_BYTES * (spin == 2 ? 2 : 1);
         const size_t need = (a > sb ? a : sb) + 1024;
         if (need <= ((size_t)40 << 30) && need <= freeb / 4) {
             if (cudaMalloc(&pl->lam, need) == cudaSuccess && cudaMalloc(&pl->lam_i0, ((size_t)pl->n_ablk + 1) * sizeof(int)) == cudaSuccess) {
