@@ -171,6 +171,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--pol", default="", choices=["", "E", "B"],
                     help="spin-2 workloads: time the E-only / B-only transforms (PAPER.md:228) instead of the full ones")
+    ap.add_argument("--lambda-mode", default="", choices=["", "fused", "staged"],
+                    help="where the P_lm tiles are generated (include/sht.h); default: the plan's own choice")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
@@ -211,6 +213,9 @@ def main():
     plan = Plan(nside, lmax, nmaps, spin)
     torch.cuda.synchronize()
     plan_s = time.time() - t0
+    if args.lambda_mode:
+        plan.sht_plan_set_lambda_mode(1 if args.lambda_mode == "staged" else 0)
+    lambda_mode = "staged" if plan.sht_plan_lambda_mode() == 1 else "fused"
     stream = torch.cuda.current_stream()
 
     if args.pol:
@@ -268,7 +273,7 @@ def main():
                  % (FP64_NOMINAL_TFLOPS, peak_src, peaks.get("bf16_tflops", 0) * 45.0 / 2250.0))
 
     def leg_roofline(stage, kernel):
-        n = max(1, stage_n[stage])
+        n = max(1, stage_n[stage])                          # timed brackets = calls of the stage (generator + contraction)
         launch_ms = stage_ms[stage] / n
         flops_per_launch = fl_dir * args.steps / n          # algorithmic (folded, unpruned) flops of one launch
         ach = flops_per_launch / (launch_ms * 1e-3) * 1e-12
@@ -277,6 +282,7 @@ def main():
                 "algorithmic_flops_per_launch": flops_per_launch, "launch_ms": launch_ms,
                 "share_of_step": stage_ms[stage] / ms_total}
 
+    # staged mode: a Legendre "launch" is the lambda-block generator kernel plus the contraction kernel (both timed)
     roofline = leg_roofline(1, "k_legendre_analysis")
     roofline["peak_source"] = peak_note
     roofline["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_v2_summary.md"
@@ -335,7 +341,7 @@ def main():
                 "config": {"workload": c["name"], "nside": nside, "lmax": lmax, "nmaps_per_gpu": nmaps, "spin": spin,
                            "l2": "inputs (%.1f GB maps, %.1f GB a_lm per GPU) are far larger than the 126 MB L2"
                                  % (8e-9 * npix * nmaps * ncomp, 16e-9 * nalm * nmaps * ncomp),
-                           "plan_create_s": plan_s, "chunk_maps": plan.chunk_maps(),
+                           "plan_create_s": plan_s, "chunk_maps": plan.chunk_maps(), "lambda_mode": lambda_mode,
                            "workspace_GB": plan.workspace_bytes() * 1e-9},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "stages": stages, "cpu_baseline": cpu}
