@@ -29,10 +29,18 @@ from paper_2208_10154_b200 import inputs, shard  # noqa: E402
 
 METRIC = "maps/sec (analysis+synthesis, FP64) at nside=512 lmax=1535"
 FP64_NOMINAL_TFLOPS = 37.2     # 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz
-# DRAM bytes per launch from the committed ncu capture (profiles/r1_v2_summary.md), keyed by (config, nmaps, kernel)
+# From the committed ncu captures (profiles/r1_v3_summary.md, profiles/r1_v2_summary.md), keyed by
+# (config, nmaps, lambda mode, kernel): DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) and the
+# DMMA pipe activity (sm__pipe_tensor_subpipe_dmma_cycles_active, fraction of peak) = executed-flop rate / peak
 NCU_TRAFFIC_BYTES = {
-    (3, 1000, "k_legendre_analysis"): 251379450880 + 19061606400,
-    (3, 1000, "k_legendre_synthesis"): 20458497000 + 37875944000,
+    (3, 1000, "staged", "k_legendre_analysis"): 259645201000 + 19115168000,
+    (3, 1000, "staged", "k_legendre_synthesis"): 27979806000 + 37874474000,
+    (3, 1000, "fused", "k_legendre_analysis"): 251379450880 + 19061606400,
+    (3, 1000, "fused", "k_legendre_synthesis"): 20458497000 + 37875944000,
+}
+NCU_DMMA_PIPE_ACTIVE = {
+    (3, 1000, "staged", "k_legendre_analysis"): 0.945, (3, 1000, "staged", "k_legendre_synthesis"): 0.880,
+    (3, 1000, "fused", "k_legendre_analysis"): 0.731, (3, 1000, "fused", "k_legendre_synthesis"): 0.770,
 }
 
 
@@ -278,14 +286,18 @@ def main():
         flops_per_launch = fl_dir * args.steps / n          # algorithmic (folded, unpruned) flops of one launch
         ach = flops_per_launch / (launch_ms * 1e-3) * 1e-12
         return {"bound": "tensor", "kernel": kernel, "achieved": ach, "peak": mma_peak, "unit": "TFLOP/s",
-                "frac": ach / mma_peak, "traffic": NCU_TRAFFIC_BYTES.get((args.config, nmaps, kernel)),
+                "frac": ach / mma_peak, "traffic": NCU_TRAFFIC_BYTES.get((args.config, nmaps, lambda_mode, kernel)),
+                "dmma_pipe_active_ncu": NCU_DMMA_PIPE_ACTIVE.get((args.config, nmaps, lambda_mode, kernel)),
                 "algorithmic_flops_per_launch": flops_per_launch, "launch_ms": launch_ms,
                 "share_of_step": stage_ms[stage] / ms_total}
 
     # staged mode: a Legendre "launch" is the lambda-block generator kernel plus the contraction kernel (both timed)
     roofline = leg_roofline(1, "k_legendre_analysis")
     roofline["peak_source"] = peak_note
-    roofline["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_v2_summary.md"
+    roofline["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_v3_summary.md"
+    roofline["note"] = ("achieved = algorithmic (N/S-folded, UNPRUNED) flops / time: ring pruning and l_safe row skipping "
+                        "leave ~0.8x of them to execute, so frac can exceed 1; dmma_pipe_active_ncu is the executed-flop "
+                        "fraction of peak from the committed ncu capture")
     roofline_syn = leg_roofline(2, "k_legendre_synthesis")
     ring_ms = stage_ms[0] + stage_ms[3]
     ring_bytes = 2 * args.steps * (8 * npix * nmaps * ncomp + 16 * (lmax + 1) * 2 * nside * 2 * nmaps * ncomp)
