@@ -49,7 +49,8 @@ typedef enum {
     SHT_ERR_NULL = -5
 } sht_status_t;
 
-/* Plan: nside >= 1 (any integer, RING scheme), lmax >= 0 (spin 2: lmax >= 2), nmaps >= 1 (spin 2: number of
+/* Plan: nside >= 1 (any integer, RING scheme; every nside <= 1024 is supported, larger ones return SHT_ERR_UNSUPPORTED
+ * when a ring length does not fit the ring kernels' shared memory), lmax >= 0 (spin 2: lmax >= 2), nmaps >= 1 (spin 2: number of
  * (Q,U) pairs), spin in {0, 2}.  Builds on the current CUDA device: ring tables, FFT twiddles, recurrence
  * coefficients, the l_safe / seed table of PAPER.md:230-232 (item 11) and the T_m^k(theta) workspace.
  * This is the paper's "initialisation overhead", paid once and timed separately.

@@ -163,3 +163,35 @@ def test_config5_iterative_composition():
     print("config 5: rms per round (map 0)", r[:, 0], "a_lm error after 0 / 3 rounds: %.2e / %.2e" % (err_0, err_it))
     assert err_it < 1e-2 * err_0
     plan.destroy()
+
+
+@pytest.mark.parametrize("nside,lmax", [(1000, 150), (331, 400)])
+def test_large_odd_nside_sampled(nside, lmax):
+    """nside that is not a power of two: every ring length 4 i occurs, primes up to 997 among the i (Bluestein with
+    convolution lengths up to 8192, direct prime stages, repeated primes); sampled rings / orders against the oracle"""
+    import torch
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan
+    nmaps = 2
+    dev = torch.device("cuda:0")
+    alm = inputs.gaussian_alm(lmax, np.arange(nmaps), 1234)
+    plan = Plan(nside, lmax, nmaps, 0)
+    maps = torch.full((nmaps, 1, plan.npix), float("nan"), dtype=torch.float64, device=dev)
+    plan.sht_synthesis(torch.from_numpy(alm).to(dev), maps)
+    torch.cuda.synchronize()
+    got = maps.cpu().numpy()
+    assert np.isfinite(got).all()
+    rings = sorted({1, 2, 3, 11, 37, 121, 169, 289, 311, 317, 330, nside - 3, nside - 1, nside, nside + 1, 2 * nside,
+                    3 * nside, 4 * nside - 311, 4 * nside - 37, 4 * nside - 1} |
+                   {r for r in (509, 523, 529, 961, 991, 997) if r < nside})
+    pix = _ring_pixels(nside, rings)
+    ref = O.synthesis(nside, lmax, alm, rlist=rings)
+    assert inputs.rel_err(got[:, :, pix], ref[:, :, pix]) <= TOL
+    msel = [0, 1, 2, 5, lmax // 2, lmax - 1, lmax]
+    alm_out = torch.full((nmaps, 1, plan.nalm), float("nan"), dtype=torch.complex128, device=dev)
+    plan.sht_analysis(maps, alm_out)
+    torch.cuda.synchronize()
+    slots = _m_slots(lmax, msel)
+    ref_alm = O.analysis(nside, lmax, got, mlist=msel)
+    assert inputs.rel_err(alm_out.cpu().numpy()[:, :, slots], ref_alm[:, :, slots]) <= TOL
+    plan.destroy()
