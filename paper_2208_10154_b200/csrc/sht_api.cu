@@ -257,27 +257,33 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
     return s;
 }
 
-// ---- host-buffer entries: chunked H2D -> transform -> D2H on two streams ---------------------------
+// ---- host-buffer entries: chunked H2D -> transform -> D2H, up to four chunks in flight -----------------
+// Each chunk has its own stream, staging buffers and slice of the workspace, so the upload of chunk i+2 does not
+// wait for the download of chunk i (PCIe is full duplex; with two slots the uploads queued behind the downloads).
 static sht_status_t host_setup(sht_plan_t pl)
 {
     if (pl->host_ready) return SHT_OK;
     const DevicePlan& d = pl->d;
-    // chunk of the host path: two chunks are in flight and share the plan's workspace, each with
-    // host_kpad <= kpad/2 columns per row (a multiple of the k-tile); a single chunk if the plan is that small
+    // chunk size: about an eighth of the maps, a multiple of the k-tile, and small enough for host_nb workspace slices
+    int nb = d.kpad / KTILE_MAPS;
+    if (nb > 4) nb = 4;
+    if (nb < 1) nb = 1;
     int hc;
-    if (d.kpad >= 2 * KTILE_MAPS) {
+    if (nb > 1) {
         hc = ((pl->nmaps / 8 + KTILE_MAPS - 1) / KTILE_MAPS) * KTILE_MAPS;
         if (hc < KTILE_MAPS) hc = KTILE_MAPS;
-        if (hc > d.kpad / 2 / KTILE_MAPS * KTILE_MAPS) hc = d.kpad / 2 / KTILE_MAPS * KTILE_MAPS;
+        const int cap = d.kpad / nb / KTILE_MAPS * KTILE_MAPS;
+        if (hc > cap) hc = cap;
         pl->host_kpad = hc;
     } else {
         hc = pl->chunk;
         pl->host_kpad = d.kpad;
     }
     pl->host_chunk = hc;
+    pl->host_nb = nb;
     const size_t mbytes = (size_t)hc * d.ncomp * d.npix * sizeof(double);
     const size_t abytes = (size_t)hc * d.ncomp * d.nalm * 2 * sizeof(double);
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < nb; ++i) {
         SHT_TRY(cudaMalloc((void**)&pl->stage_maps[i], mbytes), "host-path map staging");
         SHT_TRY(cudaMalloc((void**)&pl->stage_alm[i], abytes), "host-path alm staging");
         SHT_TRY(cudaStreamCreateWithFlags(&pl->hstream[i], cudaStreamNonBlocking), "host-path stream");
@@ -298,16 +304,15 @@ static sht_status_t host_run(sht_plan_t pl, const double* in_host, double* out_h
     DevicePlan dh = d;
     dh.kpad = pl->host_kpad;
     dh.nkg = dh.kpad / KG;
-    const bool two = (2 * (size_t)pl->host_kpad <= (size_t)d.kpad);
-    const size_t f_half = (size_t)d.nh * (d.lmax + 1) * d.ncomp * 2 * pl->host_kpad * 2;   // doubles per chunk workspace
+    const size_t f_slice = (size_t)d.nh * (d.lmax + 1) * d.ncomp * 2 * pl->host_kpad * 2;   // doubles per chunk workspace
     int idx = 0;
     for (int k0 = 0; k0 < pl->nmaps; k0 += pl->host_chunk, ++idx) {
-        const int b = two ? (idx & 1) : 0;
+        const int b = idx % pl->host_nb;
         const int kmaps = pl->nmaps - k0 < pl->host_chunk ? pl->nmaps - k0 : pl->host_chunk;
         cudaStream_t st = pl->hstream[b];
         double* dmaps = pl->stage_maps[b]; double* dalm = pl->stage_alm[b];
         double* din = analysis ? dmaps : dalm; double* dout = analysis ? dalm : dmaps;
-        double* F = pl->F + (size_t)b * f_half;
+        double* F = pl->F + (size_t)b * f_slice;
         SHT_TRY(cudaMemcpyAsync(din, in_host + (size_t)k0 * in_elems, (size_t)kmaps * in_elems * sizeof(double),
                                 cudaMemcpyHostToDevice, st), "H2D");
         // staging buffers are indexed from the chunk start: pass k0 = 0
@@ -317,8 +322,7 @@ static sht_status_t host_run(sht_plan_t pl, const double* in_host, double* out_h
         SHT_TRY(cudaMemcpyAsync(out_host + (size_t)k0 * out_elems, dout, (size_t)kmaps * out_elems * sizeof(double),
                                 cudaMemcpyDeviceToHost, st), "D2H");
     }
-    SHT_TRY(cudaStreamSynchronize(pl->hstream[0]), "host-path sync");
-    SHT_TRY(cudaStreamSynchronize(pl->hstream[1]), "host-path sync");
+    for (int i = 0; i < pl->host_nb; ++i) SHT_TRY(cudaStreamSynchronize(pl->hstream[i]), "host-path sync");
     return SHT_OK;
 }
 

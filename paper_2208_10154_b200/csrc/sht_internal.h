@@ -117,11 +117,12 @@ struct sht_plan_s {
     int pol;                        // spin 2: 0 = E and B, 1 = E only, 2 = B only (set by the *_pol entries around a call)
     char err[512];
     // host-entry staging (allocated on first use)
-    double* stage_maps[2];
-    double* stage_alm[2];
-    int host_kpad;                  // workspace columns per row in the host path (two chunks share F)
+    double* stage_maps[4];
+    double* stage_alm[4];
+    int host_kpad;                  // workspace columns per row in the host path (host_nb chunks share F)
+    int host_nb;                    // chunks in flight in the host path (streams, staging buffers, workspace slices)
     int host_chunk;
-    cudaStream_t hstream[2];
+    cudaStream_t hstream[4];
     bool host_ready;
     // optional per-stage timing (sht_plan_set_timing)
     bool timing;

@@ -613,7 +613,7 @@ extern "C" sht_status_t sht_plan_destroy(sht_plan_t pl)
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
         if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
     }
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < 4; ++i) {
         if (pl->stage_maps[i]) cudaFree(pl->stage_maps[i]);
         if (pl->stage_alm[i]) cudaFree(pl->stage_alm[i]);
         if (pl->hstream[i]) cudaStreamDestroy(pl->hstream[i]);
