@@ -37,7 +37,7 @@ struct RingPair {
     int mlim;              // only m < mlim are needed from / for this ring (ring optimisation)
     int perm_off;          // offset of this ring length's table perm[bin] = position after the forward transform
     // Bluestein (chirp-z) rings: ring lengths with a prime factor > BLUESTEIN_MIN_PRIME are transformed as a
-    // circular convolution of power-of-two length lc >= 2 n - 1 (lc = 0: plain mixed radix)
+    // circular convolution of length lc >= 2 n - 1, lc = 2^a, 3 2^a or 5 2^a (lc = 0: plain mixed radix)
     int lc;
     int b_tw_off;          // offset (double2) of W_{2 lc}[j] = exp(-i pi j / lc)
     int b_fac_off, b_nfac; // radix list of the length-lc transform (4s and a 2)

@@ -160,29 +160,53 @@ static sht_status_t fail(sht_plan_s* pl, sht_status_t s, const char* what, cudaE
     return s;
 }
 
-// plan-time power-of-two FFT in long double (iterative radix 2), for the Bluestein filter spectra
-static void host_fft_pow2(std::vector<long double>& re, std::vector<long double>& im)
+// plan-time FFT in long double (recursive decimation in time over the prime factors 2, 3, 5 of the length), for the
+// Bluestein filter spectra; wr/wi = exp(-2 pi i e / N) of the top-level length N, this level has length N / stride
+static void host_fft_rec(std::vector<long double>& re, std::vector<long double>& im, const std::vector<long double>& wr,
+                         const std::vector<long double>& wi, size_t stride)
 {
     const size_t n = re.size();
-    for (size_t i = 1, j = 0; i < n; ++i) {
-        size_t bit = n >> 1;
-        for (; j & bit; bit >>= 1) j ^= bit;
-        j ^= bit;
-        if (i < j) { std::swap(re[i], re[j]); std::swap(im[i], im[j]); }
-    }
-    for (size_t len = 2; len <= n; len <<= 1) {
-        const size_t half = len >> 1;
-        for (size_t k = 0; k < half; ++k) {
-            const long double ang = -2.0L * PI_LD * (long double)k / (long double)len;
-            const long double wr = cosl(ang), wi = sinl(ang);
-            for (size_t i = k; i < n; i += len) {
-                const size_t j = i + half;
-                const long double tr = re[j] * wr - im[j] * wi, ti = re[j] * wi + im[j] * wr;
-                re[j] = re[i] - tr; im[j] = im[i] - ti;
-                re[i] += tr; im[i] += ti;
-            }
+    if (n <= 1) return;
+    size_t r = n;                                            // prime length: direct sum
+    for (size_t f : {2, 3, 5, 7}) if (n % f == 0) { r = f; break; }
+    const size_t mlen = n / r;
+    std::vector<std::vector<long double>> sre(r, std::vector<long double>(mlen)), sim(r, std::vector<long double>(mlen));
+    for (size_t q = 0; q < r; ++q)
+        for (size_t j = 0; j < mlen; ++j) { sre[q][j] = re[j * r + q]; sim[q][j] = im[j * r + q]; }
+    for (size_t q = 0; q < r; ++q) host_fft_rec(sre[q], sim[q], wr, wi, stride * r);
+    for (size_t k = 0; k < n; ++k) {
+        long double ar = 0.0L, ai = 0.0L;
+        for (size_t q = 0; q < r; ++q) {
+            const size_t e = ((q * k) % n) * stride;
+            const long double xr = sre[q][k % mlen], xi = sim[q][k % mlen];
+            ar += xr * wr[e] - xi * wi[e]; ai += xr * wi[e] + xi * wr[e];
         }
+        re[k] = ar; im[k] = ai;
     }
+}
+
+static void host_fft(std::vector<long double>& re, std::vector<long double>& im)
+{
+    const size_t n = re.size();
+    std::vector<long double> wr(n), wi(n);
+    for (size_t e = 0; e < n; ++e) {
+        const long double ang = -2.0L * PI_LD * (long double)e / (long double)n;
+        wr[e] = cosl(ang); wi[e] = sinl(ang);
+    }
+    host_fft_rec(re, im, wr, wi, 1);
+}
+
+// convolution length of a Bluestein ring: the smallest of 2^a, 3 2^a, 5 2^a (a >= 2) that is >= minlen -- one odd
+// pass at most, so the register-fused power-of-two passes keep doing the bulk of the work
+static int bluestein_len(int minlen)
+{
+    int best = 0;
+    for (int odd : {1, 3, 5}) {
+        int v = 4 * odd;
+        while (v < minlen) v *= 2;
+        if (best == 0 || v < best) best = v;
+    }
+    return best;
 }
 
 // Kernel-side radix list: the power-of-two run of `f` (4s and at most one 2) is regrouped into register-fused
@@ -286,8 +310,7 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
         for (int v : f) maxp = v > maxp ? v : maxp;
         int lc = 0;
         if (maxp >= BLUESTEIN_MIN_PRIME) {
-            lc = 4;
-            while (lc < 2 * n - 1) lc *= 2;
+            lc = bluestein_len(2 * n - 1);
             if (lc > RING_EMAX) lc = 0;                  // does not fit one CTA: stay with the direct stage
         }
         lc_of_q[q] = lc;
@@ -299,14 +322,12 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
                     tw.push_back(make_double2((double)cosl(ang), (double)-sinl(ang)));
                 }
                 std::vector<int> pf, pg;
-                int r = lc;
-                while (r % 4 == 0) { pf.push_back(4); r /= 4; }
-                if (r == 2) pf.push_back(2);
+                factorize_ring(lc, pf);                  // 4s, a 2, then at most one 3 or 5
                 group_radices(pf, pg);
                 pow2_fac_off[lc] = (int)radix.size();
                 for (int v : pg) radix.push_back(v);
                 pow2_nfac[lc] = (int)pg.size();
-                pow2_psh[lc] = pad_shift(pg, true);
+                pow2_psh[lc] = pad_shift(pg, (lc & (lc - 1)) == 0);
             }
             // filter h_j = conj(c_j) = exp(+i pi j^2 / n) at j = -(n-1) .. n-1 (mod lc); Hf = FFT_lc(h) / lc
             std::vector<long double> hr(lc, 0.0L), hi(lc, 0.0L);
@@ -316,10 +337,10 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
                 hr[j] = cosl(ang); hi[j] = sinl(ang);
                 if (j > 0) { hr[lc - j] = hr[j]; hi[lc - j] = hi[j]; }
             }
-            host_fft_pow2(hr, hi);
+            host_fft(hr, hi);
             hf_off_of_q[q] = (int)tw.size();
             std::vector<int> lf;
-            for (int r = lc; r > 1;) { const int v = (r % 4 == 0) ? 4 : 2; lf.push_back(v); r /= v; }
+            factorize_ring(lc, lf);
             std::vector<double2> hf(lc);
             for (int k = 0; k < lc; ++k) {
                 int kk = k, pos = 0, M = lc;

@@ -624,7 +624,7 @@ __device__ __forceinline__ void fft_backward(double2* smem, double2* cur, int N,
     }
 }
 
-// Bluestein (chirp-z) circular convolution of power-of-two length Lc, in place in `buf`:
+// Bluestein (chirp-z) circular convolution of length Lc = 2^a, 3 2^a or 5 2^a, in place in `buf`:
 //   buf <- IFFT_Lc( FFT_Lc(x) . Hf ),  x delivered by `ld` (first forward stage), result handed to `st` by the
 // last backward stage when GOUT, else left in buf in natural order.  Hf is stored in forward-output position order.
 template <bool GIN, bool GOUT, bool CONJ, class LD, class ST>
@@ -643,6 +643,8 @@ __device__ __forceinline__ void bluestein_conv(double2* buf, int Lc, const int* 
             if (R == 16) dif_stage16<false>(buf, Lc, L, kt, lay, btw, ld);
             else if (R == 8) dif_stage8<false>(buf, Lc, L, kt, lay, btw, ld);
             else if (R == 4) dif_stage<4, false>(buf, Lc, L, kt, lay, btw, ld);
+            else if (R == 3) dif_stage<3, false>(buf, Lc, L, kt, lay, btw, ld);
+            else if (R == 5) dif_stage<5, false>(buf, Lc, L, kt, lay, btw, ld);
             else dif_stage<2, false>(buf, Lc, L, kt, lay, btw, ld);
         }
         L /= R;
@@ -669,6 +671,8 @@ __device__ __forceinline__ void bluestein_conv(double2* buf, int Lc, const int* 
             if (R == 16) dit_stage16<false>(buf, Lc, L, kt, lay, btw, st);
             else if (R == 8) dit_stage8<false>(buf, Lc, L, kt, lay, btw, st);
             else if (R == 4) dit_stage<4, false>(buf, Lc, L, kt, lay, btw, st);
+            else if (R == 3) dit_stage<3, false>(buf, Lc, L, kt, lay, btw, st);
+            else if (R == 5) dit_stage<5, false>(buf, Lc, L, kt, lay, btw, st);
             else dit_stage<2, false>(buf, Lc, L, kt, lay, btw, st);
         }
     }
