@@ -17,8 +17,6 @@ constexpr int LEG_CS = 16;                   // l granularity of the plan's recu
 constexpr int MAX_RADIX_LIST = 16;           // factors of one ring length
 constexpr int RING_THREADS = 256;            // threads per CTA of the ring kernels (two CTAs per SM)
 constexpr int RING_EMAX = 8192;              // most complex elements (ring length x maps) one ring CTA holds in smem
-constexpr int RING_ETARGET = 4096;           // preferred element count: 64 KB + padding, two or three CTAs per SM
-constexpr int RING_EMAX_OOP = 6400;          // same for rings that need an out-of-place pass (two buffers)
 constexpr int BLUESTEIN_MIN_PRIME = 37;      // smallest prime factor of a ring length that switches to Bluestein
 constexpr int RING_NCLASS = 4;               // launch classes of the ring kernels (by dynamic smem size)
 
@@ -142,7 +140,6 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st);
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
-size_t legendre_smem_bytes(int nh, int ntile_max);
 constexpr size_t LAM_ABLK_BYTES = 2 * 32 * 66 * 8;      // one analysis lambda block: [class][32 rings][66] doubles
 constexpr size_t LAM_SBLK_BYTES = 32 * 66 * 8;          // one synthesis lambda block: [32 l][66] doubles
 // spin 2 (sht_legendre_spin2.cu); the spin-0 launchers dispatch to these

@@ -609,13 +609,6 @@ static size_t analysis_smem(int ntile)
 }
 static size_t synthesis_smem() { return (size_t)S_STAGES * S_STAGE_BYTES + 2 * S_STAGES * sizeof(uint64_t) + 4 * S_LC * sizeof(double2) + 64; }
 
-size_t legendre_smem_bytes(int nh, int ntile_max)
-{
-    const size_t a = analysis_smem(ntile_max), s = synthesis_smem();
-    (void)nh;
-    return a > s ? a : s;
-}
-
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st)
 {

@@ -154,12 +154,6 @@ static cudaError_t upload(sht_plan_s* pl, const std::vector<T>& h, const T** dpt
     return e;
 }
 
-static sht_status_t fail(sht_plan_s* pl, sht_status_t s, const char* what, cudaError_t e)
-{
-    snprintf(pl->err, sizeof(pl->err), "%s: %s", what, e == cudaSuccess ? "" : cudaGetErrorString(e));
-    return s;
-}
-
 // plan-time FFT in long double (recursive decimation in time over the prime factors 2, 3, 5 of the length), for the
 // Bluestein filter spectra; wr/wi = exp(-2 pi i e / N) of the top-level length N, this level has length N / stride
 static void host_fft_rec(std::vector<long double>& re, std::vector<long double>& im, const std::vector<long double>& wr,
@@ -617,7 +611,6 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
     }
     if (cudaDeviceSynchronize() != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_CUDA; }
     pl->err[0] = 0;
-    (void)fail;
     *out = pl;
     return SHT_OK;
 }
