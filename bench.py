@@ -179,6 +179,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--pol", default="", choices=["", "E", "B"],
                     help="spin-2 workloads: time the E-only / B-only transforms (PAPER.md:228) instead of the full ones")
+    ap.add_argument("--iter", type=int, default=-1,
+                    help="time sht_analysis_iter with this many Jacobi rounds (Alg. 2; BASELINE.json configs[4] uses 3) "
+                         "instead of the synthesis + analysis step")
     ap.add_argument("--lambda-mode", default="", choices=["", "fused", "staged"],
                     help="where the P_lm tiles are generated (include/sht.h); default: the plan's own choice")
     ap.add_argument("--no-e2e", action="store_true")
@@ -237,6 +240,15 @@ def main():
         def step():
             plan.sht_synthesis_pol(alm, maps, which, stream)
             plan.sht_analysis_pol(maps, alm_out, which, stream)
+    elif args.iter >= 0:
+        # Alg. 2 on maps synthesised once outside the timed region: 2 niter + 1 transforms per step (eq. B8)
+        c["name"] += "_iter%d" % args.iter
+        args.no_e2e = True
+        plan.sht_synthesis(alm, maps, stream)
+        rms = torch.empty((max(args.iter, 1), nmaps * ncomp), dtype=torch.float64, device=dev)
+
+        def step():
+            plan.sht_analysis_iter(maps, alm_out, args.iter, rms, stream)
     else:
         def step():
             plan.sht_synthesis(alm, maps, stream)
@@ -274,6 +286,8 @@ def main():
     # kernel, same design, is reported beside it in "stages") ---------------------------------------------------------
     peaks, peak_src = read_measured_peaks()
     fl_dir = legendre_flops_per_direction(c) / (2 if args.pol else 1)   # half of the block products
+    if args.iter >= 0:
+        fl_dir *= (args.iter + 1)                           # analysis launches per step (the synthesis ones: niter)
     mma_peak = sht_measure_fp64_mma_peak(300.0)
     peak_note = ("FP64 DMMA.8x8x4 register-resident loop measured live in this run "
                  "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = %.1f; "
