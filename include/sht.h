@@ -82,6 +82,13 @@ sht_status_t sht_synthesis(sht_plan_t plan, const double* alm, double* maps, voi
 sht_status_t sht_analysis_iter(sht_plan_t plan, const double* maps, double* alm, int niter,
                                double* resid_rms, void* stream);
 
+/* How sht_analysis_iter forms the residual of a round (same result up to rounding):
+ *   SHT_ITER_TM    : on the ring spectra T_m(theta), the maps are read once (item 8; default; allocates a
+ *                    second workspace on the first call and falls back to SHT_ITER_PIXEL if that does not fit);
+ *   SHT_ITER_PIXEL : as residual maps (one backward and one forward ring FFT more per round). */
+enum { SHT_ITER_TM = 0, SHT_ITER_PIXEL = 1 };
+sht_status_t sht_plan_set_iter_mode(sht_plan_t plan, int mode);
+
 /* Spin-2 plans: transforms of a_lm^E or a_lm^B alone (item 9: "forward and backward transforms of a^E
  * and a^B separately ... the speed of SHTs can be increased by 100% for free"): half of the block products of eq. 14 /
  * eq. 15 are skipped.  `alm` holds ONE component: [nmaps][nalm][2] doubles, m-major.

@@ -20,6 +20,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 SHT_OK = 0
 SHT_POL_E, SHT_POL_B = 1, 2
 SHT_LAMBDA_FUSED, SHT_LAMBDA_STAGED = 0, 1
+SHT_ITER_TM, SHT_ITER_PIXEL = 0, 1
 _vp, _i, _ll, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_double
 
 _lib.sht_plan_create.argtypes = [ctypes.POINTER(_vp), _i, _i, _i, _i]
@@ -40,6 +41,8 @@ _lib.sht_alm_pack_a7.argtypes = [_i, _ll, _vp, _vp, _vp]
 _lib.sht_alm_pack_a7.restype = _i
 _lib.sht_alm_unpack_a7.argtypes = [_i, _ll, _vp, _vp, _vp]
 _lib.sht_alm_unpack_a7.restype = _i
+_lib.sht_plan_set_iter_mode.argtypes = [_vp, _i]
+_lib.sht_plan_set_iter_mode.restype = _i
 _lib.sht_plan_set_lambda_mode.argtypes = [_vp, _i]
 _lib.sht_plan_set_lambda_mode.restype = _i
 _lib.sht_plan_lambda_mode.argtypes = [_vp]
@@ -74,7 +77,7 @@ _lib.sht_measure_fp64_mma_peak.argtypes = [_d]
 _lib.sht_measure_fp64_mma_peak.restype = _d
 
 EXPORTED = [
-    "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol", "sht_alm_pack_a7", "sht_alm_unpack_a7", "sht_plan_set_lambda_mode", "sht_plan_lambda_mode",
+    "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol", "sht_alm_pack_a7", "sht_alm_unpack_a7", "sht_plan_set_lambda_mode", "sht_plan_lambda_mode", "sht_plan_set_iter_mode",
     "sht_analysis_host", "sht_synthesis_host", "sht_npix", "sht_nalm", "sht_alm_index",
     "sht_plan_workspace_bytes", "sht_plan_chunk_maps", "sht_plan_kernel_launches", "sht_status_string",
     "sht_last_error", "sht_measure_fp64_mma_peak", "sht_plan_set_timing", "sht_plan_stage_ms",
@@ -168,6 +171,9 @@ class Plan:
 
     def sht_synthesis_pol(self, alm, maps, which, stream=None):
         self._check(_lib.sht_synthesis_pol(self._h, _ptr(alm), _ptr(maps), which, _stream(stream)), "sht_synthesis_pol")
+
+    def sht_plan_set_iter_mode(self, mode):
+        self._check(_lib.sht_plan_set_iter_mode(self._h, mode), "sht_plan_set_iter_mode")
 
     def sht_plan_set_lambda_mode(self, mode):
         self._check(_lib.sht_plan_set_lambda_mode(self._h, mode), "sht_plan_set_lambda_mode")

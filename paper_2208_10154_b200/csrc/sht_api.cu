@@ -217,6 +217,49 @@ extern "C" sht_status_t sht_synthesis_pol(sht_plan_t pl, const double* alm, doub
     return pol_run(pl, nullptr, alm, maps, nullptr, which, stream);
 }
 
+// Alg. 2 kept between T_m and a_lm (item 8): one ring-FFT pass over the maps, then per round a Legendre
+// synthesis, the residual on the ring spectra (k_ring_residual) and a Legendre analysis with accumulation.  Needs a
+// second workspace (the folded T_m of the maps); if that does not fit, falls back to forming the residual maps.
+static sht_status_t iter_tm_space(sht_plan_t pl, const double* maps, double* alm, int niter, double* resid_rms, cudaStream_t st)
+{
+    const DevicePlan& d = pl->d;
+    double* acc = nullptr;
+    SHT_TRY(cudaMallocAsync((void**)&acc, (size_t)pl->chunk * d.ncomp * sizeof(double), st), "rms scratch");
+    const size_t ubytes = (size_t)d.nh * d.ncomp * d.kpad * sizeof(double);
+    sht_status_t s = SHT_OK;
+    for (int k0 = 0; k0 < pl->nmaps && s == SHT_OK; k0 += pl->chunk) {
+        const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
+        const int nrow = kmaps * d.ncomp;
+        SHT_TRY(cudaMemsetAsync(pl->upow, 0, ubytes, st), "uncovered-power memset");
+        int t = timing_begin(pl, 0, st);
+        SHT_TRY(launch_ring_analysis(pl, d, maps, pl->Fmap, k0, kmaps, st, pl->upow), "ring analysis");
+        timing_end(pl, t, st);
+        t = timing_begin(pl, 1, st);
+        SHT_TRY(launch_legendre_analysis(pl, d, pl->Fmap, alm, k0, kmaps, false, st), "legendre analysis");
+        timing_end(pl, t, st);
+        for (int it = 0; it < niter && s == SHT_OK; ++it) {
+            t = timing_begin(pl, 2, st);
+            SHT_TRY(launch_legendre_synthesis(pl, d, alm, pl->F, k0, kmaps, st), "legendre synthesis");
+            timing_end(pl, t, st);
+            SHT_TRY(cudaMemsetAsync(acc, 0, (size_t)nrow * sizeof(double), st), "rms memset");
+            t = timing_begin(pl, 3, st);
+            SHT_TRY(launch_ring_residual(pl, d, pl->F, pl->Fmap, pl->upow, acc, kmaps, st), "ring residual");
+            timing_end(pl, t, st);
+            if (resid_rms) {
+                k_rms_finish<<<(nrow + 127) / 128, 128, 0, st>>>(acc, nrow, 1.0 / (double)d.npix,
+                                                                 resid_rms + (size_t)it * pl->nmaps * d.ncomp + (size_t)k0 * d.ncomp);
+                pl->launches++;
+                SHT_TRY(cudaGetLastError(), "rms kernel");
+            }
+            t = timing_begin(pl, 1, st);
+            SHT_TRY(launch_legendre_analysis(pl, d, pl->F, alm, k0, kmaps, true, st), "legendre analysis");
+            timing_end(pl, t, st);
+        }
+    }
+    cudaFreeAsync(acc, st);
+    return s;
+}
+
 extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, double* alm, int niter,
                                           double* resid_rms, void* stream)
 {
@@ -225,6 +268,18 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
     if (niter < 0) { snprintf(pl->err, sizeof(pl->err), "niter < 0"); return SHT_ERR_INVALID_ARG; }
     cudaStream_t st = (cudaStream_t)stream;
     const DevicePlan& d = pl->d;
+    if (niter > 0 && pl->iter_mode != SHT_ITER_PIXEL) {
+        if (!pl->Fmap) {                                 // first iterative call: second workspace + uncovered-power table
+            const size_t ubytes = (size_t)d.nh * d.ncomp * d.kpad * sizeof(double);
+            if (cudaMalloc((void**)&pl->Fmap, pl->F_bytes) != cudaSuccess || cudaMalloc((void**)&pl->upow, ubytes) != cudaSuccess) {
+                cudaGetLastError();
+                if (pl->Fmap) { cudaFree(pl->Fmap); pl->Fmap = nullptr; }
+            } else if (cudaMemset(pl->Fmap, 0, pl->F_bytes) != cudaSuccess) {
+                return cuda_fail(pl, "workspace memset", cudaGetLastError());
+            }
+        }
+        if (pl->Fmap) return iter_tm_space(pl, maps, alm, niter, resid_rms, st);
+    }
     // residual maps of one chunk + sum-of-squares accumulators (stream-ordered scratch)
     double* res = nullptr; double* acc = nullptr;
     if (niter > 0) {
@@ -255,6 +310,14 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
     if (res) cudaFreeAsync(res, st);
     if (acc) cudaFreeAsync(acc, st);
     return s;
+}
+
+extern "C" sht_status_t sht_plan_set_iter_mode(sht_plan_t pl, int mode)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (mode != SHT_ITER_TM && mode != SHT_ITER_PIXEL) return SHT_ERR_INVALID_ARG;
+    pl->iter_mode = mode;
+    return SHT_OK;
 }
 
 // ---- host-buffer entries: chunked H2D -> transform -> D2H, up to four chunks in flight -----------------

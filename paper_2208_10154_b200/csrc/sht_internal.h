@@ -107,6 +107,9 @@ struct sht_plan_s {
     size_t class_smem[sht::RING_NCLASS];
     int sm_count;
     long long launches;
+    double* Fmap;                   // Alg. 2: folded T_m of the input maps (allocated on the first iterative call)
+    double* upow;                   // Alg. 2: [nh][ncomp][kpad] uncovered ring power
+    int iter_mode;                  // SHT_ITER_TM (default) / SHT_ITER_PIXEL
     double* lam;                    // staged-lambda scratch (nullptr: fused generation inside the contraction kernels)
     size_t lam_bytes;
     int* lam_i0;                    // [analysis blocks] first 16-row block with a started recurrence
@@ -132,7 +135,11 @@ struct sht_plan_s {
 namespace sht {
 
 // ring FFT stage (sht_ring_fft.cu)
-cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st);
+// upow (may be null): [nh][ncomp][kpad], += power of each ring pair in the bins no stored order reaches (Alg. 2 rms)
+cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st,
+                                 double* upow = nullptr);
+cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F, const double* Fmap, const double* upow, double* acc,
+                                 int kmaps, cudaStream_t st);
 // maps of the chunk are maps[k0 .. k0+kmaps); if sub_from != nullptr the output is sub_from[ksub0 + k] - synthesis
 cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps,
                                   const double* sub_from, int ksub0, cudaStream_t st);

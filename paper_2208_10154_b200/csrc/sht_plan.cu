@@ -621,6 +621,8 @@ extern "C" sht_status_t sht_plan_destroy(sht_plan_t pl)
     cudaDeviceSynchronize();
     for (int i = 0; i < pl->n_allocs; ++i) cudaFree(pl->dev_allocs[i]);
     if (pl->F) cudaFree(pl->F);
+    if (pl->Fmap) cudaFree(pl->Fmap);
+    if (pl->upow) cudaFree(pl->upow);
     if (pl->lam) cudaFree(pl->lam);
     if (pl->lam_i0) cudaFree(pl->lam_i0);
     for (int i = 0; i < 256; ++i) {

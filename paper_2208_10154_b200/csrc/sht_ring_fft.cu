@@ -684,7 +684,7 @@ __device__ __forceinline__ void bluestein_conv(double2* buf, int Lc, const int* 
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int* __restrict__ ring_list,
                                                      const double* __restrict__ maps, double* __restrict__ F,
-                                                     int k0, int kmaps)
+                                                     int k0, int kmaps, double* __restrict__ upow)
 {
     extern __shared__ double2 smem[];
     const int p = ring_list[blockIdx.y], comp = blockIdx.z;
@@ -736,6 +736,26 @@ __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int
     const size_t cstride = (size_t)d.ncomp * 2 * KG;                       // double2 per order m
     double2* Fp = reinterpret_cast<double2*>(F) + f_cell(d, p, k >> 2, 0, comp, 0) + (k & 3) + (size_t)m * cstride;
     const int mlim = rp.mlim;
+    if (upow && mlim <= N / 2) {
+        // Alg. 2 in T_m-space: power of the ring pair in the bins no stored order m < mlim reaches (b = mlim .. N/2); the
+        // residual of those bins never changes, its power enters the per-round rms through this table [p][comp][map]
+        double acc = 0.0;
+        for (int bb = mlim + (tid >> ktsh); bb <= N / 2; bb += dm) {
+            const int bc2 = N - bb;
+            double2 A, B;
+            if (!blue) {
+                A = cur[lay(perm(bb), kk)]; B = cur[lay(perm(bc2), kk)];
+            } else {
+                A = cmul(cur[lay(bb, kk)], __ldg(tw2 + (bb * bb) % (2 * N)));
+                B = cmul(cur[lay(bc2, kk)], __ldg(tw2 + (bc2 * bc2) % (2 * N)));
+            }
+            const double2 gn = make_double2(0.5 * (A.x + B.x), 0.5 * (A.y - B.y));
+            const double2 gs = make_double2(0.5 * (A.y + B.y), -0.5 * (A.x - B.x));
+            const double w = (2 * bb == N) ? 1.0 : 2.0;
+            acc += w * (gn.x * gn.x + gn.y * gn.y + (equator ? 0.0 : gs.x * gs.x + gs.y * gs.y));
+        }
+        if (acc != 0.0) atomicAdd(upow + ((size_t)p * d.ncomp + comp) * d.kpad + k, acc);
+    }
 #pragma unroll 4
     for (; m < mlim; m += dm) {
         const int bc = b == 0 ? 0 : N - b;
@@ -876,6 +896,104 @@ __global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const in
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Alg. 2 kept between T_m and a_lm (item 8): the ring FFTs are lossless, so the
+// residual map - synthesis(a) is formed on the ring spectra.  F holds the synthesised T_m (north / south) of one round,
+// Fmap the folded T_m of the input maps.  Per ring pair: the synthesised ring spectrum Y[b] is assembled exactly as in
+// k_ring_synthesis, re-expanded to every m < mlim on the frequency circle (FFT(ring)[b] = N Y[b]; the phases and d sigma
+// of the analysis side) and subtracted; F is overwritten with the folded residual.  By Parseval the sum of squares of the
+// residual pixels of the pair is (1/N) sum_b |R[b]|^2: bins b < mlim from the residual itself, the others from `upow`.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(NT, 1) k_ring_residual(DevicePlan d, const int* __restrict__ ring_list,
+                                                     double* __restrict__ F, const double* __restrict__ Fmap,
+                                                     const double* __restrict__ upow, double* __restrict__ acc_out,
+                                                     int kmaps)
+{
+    extern __shared__ double2 smem[];
+    const int p = ring_list[blockIdx.y], comp = blockIdx.z;
+    const RingPair rp = d.rings[p];
+    const int N = rp.n, kt = rp.kt, ktsh = __ffs(kt) - 1;
+    const int kbase = blockIdx.x * kt;
+    if (kbase >= kmaps) return;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const double2* tw2 = d.tw + rp.tw_off;
+    const bool equator = rp.start_s < 0;
+    const int mlim = rp.mlim, nb = N / 2 + 1;
+    double2* Yn = smem;                                   // [b][kk]
+    double2* Ys = smem + ((size_t)nb << ktsh);
+    const int kk = tid & (kt - 1), k = kbase + kk;
+    const int db = nt >> ktsh;
+    const size_t cstride = (size_t)d.ncomp * 2 * KG;
+    const size_t cell0 = f_cell(d, p, (k < kmaps ? k : kbase) >> 2, 0, comp, 0) + (k & 3);
+    const double2* Fs = reinterpret_cast<const double2*>(F) + cell0;
+    // ---- ring spectrum of the synthesised pair (same arithmetic as k_ring_synthesis)
+    for (int b = tid >> ktsh; b < nb; b += db) {
+        double2 yn = make_double2(0.0, 0.0), ys = make_double2(0.0, 0.0);
+        if (k < kmaps) {
+#pragma unroll
+            for (int pass = 0; pass < 2; ++pass) {
+                const int mfirst = pass == 0 ? b : (b == 0 ? 0 : N - b);
+                int m2 = mfirst;
+                const double2* Fp = Fs + (size_t)mfirst * cstride;
+                for (int m = mfirst; m < mlim; m += N, Fp += (size_t)N * cstride) {
+                    const double w = (m == 0) ? 0.5 : 1.0;
+                    double2 ph = make_double2(1.0, 0.0);
+                    if (rp.shift) { ph = __ldg(tw2 + m2); ph.y = -ph.y; }
+                    double2 fn = Fp[0], fs = Fp[KG];
+                    if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }
+                    double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
+                    if (pass == 1) { dn.y = -dn.y; ds.y = -ds.y; }
+                    yn.x = fma(w, dn.x, yn.x); yn.y = fma(w, dn.y, yn.y);
+                    ys.x = fma(w, ds.x, ys.x); ys.y = fma(w, ds.y, ys.y);
+                    m2 += N; if (m2 >= 2 * N) m2 -= 2 * N;
+                }
+            }
+        }
+        if (equator) ys = make_double2(0.0, 0.0);
+        if (b == 0 || 2 * b == N) { yn.y = 0.0; ys.y = 0.0; }
+        Yn[(b << ktsh) + kk] = yn;
+        Ys[(b << ktsh) + kk] = ys;
+    }
+    __syncthreads();
+    if (k >= kmaps) return;
+    // ---- residual of every order m < mlim, folded; sum of squares of the covered bins
+    const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
+    const double scale = dsig * (double)N;                // FFT(ring)[b] = N Y[b], times d sigma of the analysis side
+    const double2* Fm = reinterpret_cast<const double2*>(Fmap) + cell0;
+    double2* Fo = reinterpret_cast<double2*>(F) + cell0;
+    const int dmN = db % N, dm2N = db % (2 * N);
+    int m = tid >> ktsh;
+    int b = m % N, m2 = m % (2 * N);
+    double ssq = 0.0;
+    for (; m < mlim; m += db) {
+        const bool cj = 2 * b > N;
+        const int bb = cj ? N - b : b;
+        double2 tn = Yn[(bb << ktsh) + kk], ts = Ys[(bb << ktsh) + kk];
+        if (cj) { tn.y = -tn.y; ts.y = -ts.y; }
+        double2 ph = make_double2(scale, 0.0);
+        if (rp.shift) { ph = __ldg(tw2 + m2); ph.x *= scale; ph.y *= scale; }
+        double2 se, so;
+        if (equator) { se = cmul(ph, tn); so = make_double2(0.0, 0.0); }
+        else { se = cmul(ph, cadd(tn, ts)); so = cmul(ph, csub(tn, ts)); }
+        if (comp == 1) { se = make_double2(-se.y, se.x); so = make_double2(-so.y, so.x); }
+        const size_t off = (size_t)m * cstride;
+        const double2 E = csub(Fm[off], se), O = csub(Fm[off + KG], so);
+        Fo[off] = E;
+        Fo[off + KG] = O;
+        if (2 * m <= N) {                                 // m is its own bin: |R_north|^2 + |R_south|^2 (times d sigma^2)
+            const double w = (m == 0 || 2 * m == N) ? 1.0 : 2.0;
+            const double q = equator ? (E.x * E.x + E.y * E.y)
+                                     : 0.5 * (E.x * E.x + E.y * E.y + O.x * O.x + O.y * O.y);
+            ssq = fma(w, q, ssq);
+        }
+        b += dmN; if (b >= N) b -= N;
+        m2 += dm2N; if (m2 >= 2 * N) m2 -= 2 * N;
+    }
+    double tot = ssq / (dsig * dsig);
+    if ((tid >> ktsh) == 0) tot += upow[((size_t)p * d.ncomp + comp) * d.kpad + k];
+    if (tot != 0.0) atomicAdd(acc_out + (size_t)k * d.ncomp + comp, tot / (double)N);
+}
+
 // CTAs that share an SM with another one run RING_THREADS threads; a CTA that owns the SM runs twice as many
 static int ring_threads(size_t smem) { return smem <= (size_t)113 * 1024 ? RING_THREADS : 2 * RING_THREADS; }
 
@@ -890,7 +1008,8 @@ static cudaError_t ring_attr(sht_plan_s* pl)
     return e;
 }
 
-cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
+cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st,
+                                 double* upow)
 {
     cudaError_t e = ring_attr(pl);
     if (e != cudaSuccess) return e;
@@ -898,7 +1017,7 @@ cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const doub
     for (int c = RING_NCLASS - 1; c >= 0; --c) {
         if (pl->class_count[c] == 0) continue;
         dim3 grid((kmaps + pl->class_ktmin[c] - 1) / pl->class_ktmin[c], pl->class_count[c], d.ncomp);
-        k_ring_analysis<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c], st>>>(d, pl->class_rings[c], maps, F, k0, kmaps);
+        k_ring_analysis<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c], st>>>(d, pl->class_rings[c], maps, F, k0, kmaps, upow);
         pl->launches++;
     }
     return cudaGetLastError();
@@ -913,6 +1032,26 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
         if (pl->class_count[c] == 0) continue;
         dim3 grid((kmaps + pl->class_ktmin[c] - 1) / pl->class_ktmin[c], pl->class_count[c], d.ncomp);
         k_ring_synthesis<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c], st>>>(d, pl->class_rings[c], F, maps, k0, kmaps, sub_from, ksub0);
+        pl->launches++;
+    }
+    return cudaGetLastError();
+}
+
+// residual of one Jacobi round in T_m-space: F (synthesised, north / south) <- Fmap - alias(F), folded; acc[k][comp] +=
+// sum of squares of the residual pixels
+cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F, const double* Fmap, const double* upow, double* acc,
+                                 int kmaps, cudaStream_t st)
+{
+    cudaError_t e = ring_attr(pl);
+    if (e == cudaSuccess) {
+        static bool set = false;
+        if (!set) { e = cudaFuncSetAttribute(k_ring_residual, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024); set = e == cudaSuccess; }
+    }
+    if (e != cudaSuccess) return e;
+    for (int c = RING_NCLASS - 1; c >= 0; --c) {
+        if (pl->class_count[c] == 0) continue;
+        dim3 grid((kmaps + pl->class_ktmin[c] - 1) / pl->class_ktmin[c], pl->class_count[c], d.ncomp);
+        k_ring_residual<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c] + 512, st>>>(d, pl->class_rings[c], F, Fmap, upow, acc, kmaps);
         pl->launches++;
     }
     return cudaGetLastError();

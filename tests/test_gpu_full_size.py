@@ -152,7 +152,8 @@ def test_config5_iterative_composition():
     rms_ref = torch.stack(rms_ref)
     scale = a.abs().amax(dim=(1, 2), keepdim=True)
     assert float(((alm_it - a).abs() / scale).max()) <= 1e-13
-    assert float(((rms - rms_ref).abs() / rms_ref).max()) <= 1e-10
+    # the entry forms the residual on the ring spectra and gets the rms by Parseval; the composition squares pixels
+    assert float(((rms - rms_ref).abs() / rms_ref).max()) <= 1e-8
     r = rms.cpu().numpy()
     assert np.all(r[1:] < 0.25 * r[:-1]), r[:, :3]
     # converges to the input a_lm (fixed point, paper: errors "negligible" when lmax <= 2 nside)
