@@ -267,36 +267,47 @@ __device__ __forceinline__ void dif_stage8(double2* buf, int N, int L, int kt, L
     __syncthreads();
 }
 
-// Direct stage for a prime 11 <= R <= 31: one thread owns a whole butterfly, its R inputs live in registers, every
-// output is a dot product with a row of W_R (read through the W_N table, the same address for the whole warp);
-// in place.  R^2 complex multiply-adds per butterfly, but one pass and no second buffer.
+// Direct stage for a prime 11 <= R <= 31: one thread owns a whole butterfly and keeps it in registers as the sums
+// a_j = x_j + x_{R-j} and differences b_j = x_j - x_{R-j} (j = 1 .. H = (R-1)/2); the outputs s and R - s are then
+// x_0 + sum_j cos(2 pi j s / R) a_j -+ i sum_j sin(2 pi j s / R) b_j: R^2 / 2 real multiply-adds per output pair, the
+// cosines / sines read through the W_N table (the same address for the whole warp).  In place, no second buffer.
 template <int R, bool GIN, class LD>
 __device__ __forceinline__ void dif_prime(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, LD ld)
 {
+    constexpr int H = (R - 1) / 2;
     const int M = L / R, nw = (N / R) << lay.ktsh, tstep = N / L, rstep = 2 * (N / R);
     for (int w = threadIdx.x; w < nw; w += blockDim.x) {
         const int kk = w & (kt - 1), bf = w >> lay.ktsh;
         const int blk = bf / M, j = bf - blk * M;
         const int e0 = blk * L + j;
-        double2 x[R];
+        double2 a[H], b[H];
+        const double2 x0 = GIN ? ld(e0, kk) : buf[lay(e0, kk)];
+        double2 sum = x0;
 #pragma unroll
-        for (int r = 0; r < R; ++r) x[r] = GIN ? ld(e0 + r * M, kk) : buf[lay(e0 + r * M, kk)];
-        double2 sum = x[0];
-#pragma unroll
-        for (int r = 1; r < R; ++r) sum = cadd(sum, x[r]);
+        for (int q = 1; q <= H; ++q) {
+            const double2 xa = GIN ? ld(e0 + q * M, kk) : buf[lay(e0 + q * M, kk)];
+            const double2 xb = GIN ? ld(e0 + (R - q) * M, kk) : buf[lay(e0 + (R - q) * M, kk)];
+            a[q - 1] = cadd(xa, xb); b[q - 1] = csub(xa, xb);
+            sum = cadd(sum, a[q - 1]);
+        }
         buf[lay(e0, kk)] = sum;
-        for (int sx = 1; sx < R; ++sx) {
-            double2 acc = x[0];
+        for (int sx = 1; sx <= H; ++sx) {
+            double2 re = x0, im = make_double2(0.0, 0.0);
             int idx = 0;
 #pragma unroll
-            for (int r = 1; r < R; ++r) {
+            for (int q = 0; q < H; ++q) {
                 idx += sx; if (idx >= R) idx -= R;
-                const double2 wv = __ldg(tw2 + idx * rstep);             // W_R^{r s}
-                acc.x = fma(x[r].x, wv.x, fma(-x[r].y, wv.y, acc.x));
-                acc.y = fma(x[r].x, wv.y, fma(x[r].y, wv.x, acc.y));
+                const double2 wv = __ldg(tw2 + idx * rstep);             // (cos, -sin) of 2 pi (q+1) s / R
+                re.x = fma(wv.x, a[q].x, re.x); re.y = fma(wv.x, a[q].y, re.y);
+                im.x = fma(-wv.y, b[q].x, im.x); im.y = fma(-wv.y, b[q].y, im.y);
             }
-            if (M > 1) acc = cmul(acc, twiddle<false>(tw2, j * sx * tstep));
-            buf[lay(e0 + sx * M, kk)] = acc;
+            double2 lo = make_double2(re.x + im.y, re.y - im.x), hi = make_double2(re.x - im.y, re.y + im.x);
+            if (M > 1) {
+                lo = cmul(lo, twiddle<false>(tw2, j * sx * tstep));
+                hi = cmul(hi, twiddle<false>(tw2, j * (R - sx) * tstep));
+            }
+            buf[lay(e0 + sx * M, kk)] = lo;
+            buf[lay(e0 + (R - sx) * M, kk)] = hi;
         }
     }
     __syncthreads();
@@ -448,7 +459,8 @@ __device__ __forceinline__ void dit_stage8(double2* buf, int N, int L, int kt, L
     if (!GOUT) __syncthreads();
 }
 
-// adjoint of dif_prime
+// adjoint of dif_prime (plain form: all R inputs in registers, every output a dot product with a row of conj W_R; the
+// sum / difference form costs more registers here because the inputs carry their twiddles)
 template <int R, bool GOUT, class ST>
 __device__ __forceinline__ void dit_prime(double2* buf, int N, int L, int kt, Lay lay, const double2* __restrict__ tw2, ST st)
 {
