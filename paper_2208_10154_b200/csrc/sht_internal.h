@@ -39,7 +39,8 @@ struct RingPair {
     int lc;
     int b_tw_off;          // offset (double2) of W_{2 lc}[j] = exp(-i pi j / lc)
     int b_fac_off, b_nfac; // radix list of the length-lc transform (4s and a 2)
-    int hf_off;            // offset (double2) of FFT_lc(conj chirp) / lc in forward-output position order
+    int hf_off;            // offset (double2) of FFT_lc(conj chirp) / lc in forward-output position order; the chirp
+                           // c_j, j < n, follows at hf_off + lc
     int psh;               // shared-memory padding: one element every 2^psh (power-of-two transforms), 31 = none
     int nbuf;              // elements per map of one transform buffer, padding included
     // power-of-two rings: the digit reversal is a bit permutation, computed instead of read from the table:

@@ -342,6 +342,11 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
                 hf[pos] = make_double2((double)(hr[k] / lc), (double)(hi[k] / lc));
             }
             tw.insert(tw.end(), hf.begin(), hf.end());
+            // chirp c_j = W_{2n}^{j^2 mod 2n}, j < n, right behind Hf (the kernels index it by j: no modulo per element)
+            for (int j = 0; j < n; ++j) {
+                const double2 cj = tw[tw_off_of_q[q] + (int)(((long long)j * j) % (2LL * n))];
+                tw.push_back(cj);
+            }
         }
         // forward (decimation in frequency) output order: bin k = s_1 + R_1 (s_2 + R_2 (...)) sits at
         // position s_1 n/R_1 + s_2 n/(R_1 R_2) + ...

@@ -711,6 +711,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int
     const BinPos perm{d.perm + rp.perm_off, rp.pbits, rp.pm_hi, rp.pm_lo, rp.pm_keep};
     const bool equator = rp.start_s < 0;
     const bool blue = rp.lc > 0;
+    const double2* chirp = d.tw + rp.hf_off + rp.lc;      // c_j = exp(-i pi j^2 / N), j < N (Bluestein rings)
 
     // z[n] = T_north[n] + i T_south[n] of map kbase + kk
     const size_t map_stride = (size_t)d.ncomp * d.npix;
@@ -729,7 +730,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int
         // X_b = c_b sum_n (x_n c_n) conj(c)_{b-n},  c_n = exp(-i pi n^2 / N) = W_{2N}^{n^2 mod 2N}
         auto ldc = [&](int e, int kk) -> double2 {
             if (e >= N) return make_double2(0.0, 0.0);
-            return cmul(ld(e, kk), __ldg(tw2 + (e * e) % (2 * N)));
+            return cmul(ld(e, kk), __ldg(chirp + e));
         };
         auto nost = [](int, int, double2) {};
         bluestein_conv<true, false, false>(smem, rp.lc, d.radix + rp.b_fac_off, rp.b_nfac, kt, lay, d.tw + rp.b_tw_off,
@@ -758,8 +759,8 @@ __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int
             if (!blue) {
                 A = cur[lay(perm(bb), kk)]; B = cur[lay(perm(bc2), kk)];
             } else {
-                A = cmul(cur[lay(bb, kk)], __ldg(tw2 + (bb * bb) % (2 * N)));
-                B = cmul(cur[lay(bc2, kk)], __ldg(tw2 + (bc2 * bc2) % (2 * N)));
+                A = cmul(cur[lay(bb, kk)], __ldg(chirp + bb));
+                B = cmul(cur[lay(bc2, kk)], __ldg(chirp + bc2));
             }
             const double2 gn = make_double2(0.5 * (A.x + B.x), 0.5 * (A.y - B.y));
             const double2 gs = make_double2(0.5 * (A.y + B.y), -0.5 * (A.x - B.x));
@@ -775,8 +776,8 @@ __global__ void __launch_bounds__(NT, 1) k_ring_analysis(DevicePlan d, const int
         if (!blue) {
             A = cur[lay(perm(b), kk)]; B = cur[lay(perm(bc), kk)];
         } else {
-            A = cmul(cur[lay(b, kk)], __ldg(tw2 + (b * b) % (2 * N)));
-            B = cmul(cur[lay(bc, kk)], __ldg(tw2 + (bc * bc) % (2 * N)));
+            A = cmul(cur[lay(b, kk)], __ldg(chirp + b));
+            B = cmul(cur[lay(bc, kk)], __ldg(chirp + bc));
         }
         // G_north = (A + conj B)/2, G_south = (A - conj B)/(2i)
         const double2 gn = make_double2(0.5 * (A.x + B.x), 0.5 * (A.y - B.y));
@@ -818,6 +819,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const in
     const BinPos perm{d.perm + rp.perm_off, rp.pbits, rp.pm_hi, rp.pm_lo, rp.pm_keep};
     const bool equator = rp.start_s < 0;
     const bool blue = rp.lc > 0;
+    const double2* chirp = d.tw + rp.hf_off + rp.lc;      // c_j = exp(-i pi j^2 / N), j < N (Bluestein rings)
     const int mlim = rp.mlim;
     double2* cur = smem;
 
@@ -861,11 +863,11 @@ __global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const in
                 if (b > 0 && 2 * b < N) cur[lay(perm(N - b), kk)] = zc;
             } else {
                 // x_n = conj(c)_n sum_b (Z_b conj(c)_b) c_{n-b}
-                double2 c = __ldg(tw2 + (b * b) % (2 * N)); c.y = -c.y;
+                double2 c = __ldg(chirp + b); c.y = -c.y;
                 cur[lay(b, kk)] = cmul(zb, c);
                 if (b > 0 && 2 * b < N) {
                     const int bb = N - b;
-                    double2 c2 = __ldg(tw2 + (bb * bb) % (2 * N)); c2.y = -c2.y;
+                    double2 c2 = __ldg(chirp + bb); c2.y = -c2.y;
                     cur[lay(bb, kk)] = cmul(zc, c2);
                 }
             }
@@ -899,7 +901,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const in
     } else {
         auto stc = [&](int e, int kk, double2 v) {
             if (e >= N) return;
-            double2 c = __ldg(tw2 + (e * e) % (2 * N)); c.y = -c.y;
+            double2 c = __ldg(chirp + e); c.y = -c.y;
             st(e, kk, cmul(v, c));
         };
         auto nold = [](int, int) -> double2 { return make_double2(0.0, 0.0); };
