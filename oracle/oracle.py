@@ -2,7 +2,10 @@
 
 TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and the cpu_baseline /
 ``--impl reference`` legs of bench.py.  Nothing here imports, links or reads the CUDA library.
-Argument marshalling only -- all arithmetic is in the C file, which cites PAPER.md passage by passage.
+Argument marshalling only -- all arithmetic is in the C file, which cites PAPER.md passage by passage -- with two
+exceptions written here in numpy on top of the C transforms: the eq. A7 packed format (pack_a7 / unpack_a7, pinned by
+tests/test_oracle_a7.py) and Alg. 3's sweep over the orders m (analysis_iter_immediate, pinned by
+tests/test_oracle_immediate.py against a dense block-triangular solve).
 """
 import ctypes
 import os
@@ -146,6 +149,31 @@ def analysis_iter(nside, lmax, maps, niter, spin=0):
     rms = np.zeros((max(niter, 1), nm * nc))
     lib().oracle_analysis_iter(nside, lmax, nm, spin, _dp(maps), _dp(alm.view(np.float64)), niter, _dp(rms))
     return alm, rms[:niter]
+
+
+def analysis_iter_immediate(nside, lmax, maps, niter, spin=0):
+    """Alg. 3, the "immediate" iteration, in the reading DESIGN.md lists as G21: a Gauss-Seidel
+    sweep over the orders m.  a^0 = analysis(map) and r = map - synthesis(a^0); then, niter times, for m = 0 .. lmax in
+    this order: delta a_m = the order-m part of analysis(r) (line 13, P . T remapped from the *current* F), a_m += delta
+    a_m, and r -= synthesis(delta a_m) at once (lines 8-9, "update F from delta T_m"), so that the orders that follow
+    see, through the ring aliasing, the corrections already made.  Written out on the pixels with the single-order
+    analysis and the plain synthesis of this oracle; no ring-spectrum shortcuts.
+    Returns (alm, resid_rms[niter][nmaps*ncomp]): the rms of r at the start of each sweep."""
+    nc = _ncomp(spin)
+    maps = np.ascontiguousarray(maps, dtype=np.float64).reshape(-1, nc, npix(nside))
+    nm = maps.shape[0]
+    alm = analysis(nside, lmax, maps, spin)
+    rms = np.zeros((niter, nm * nc))
+    if niter == 0:
+        return alm, rms
+    res = maps - synthesis(nside, lmax, alm, spin)
+    for it in range(niter):
+        rms[it] = np.sqrt(np.mean(res * res, axis=2)).reshape(-1)
+        for m in range(lmax + 1):
+            da = analysis(nside, lmax, res, spin, mlist=[m])
+            alm += da
+            res -= synthesis(nside, lmax, da, spin)
+    return alm, rms
 
 
 def pack_a7(lmax, alm):
