@@ -82,11 +82,20 @@ sht_status_t sht_synthesis(sht_plan_t plan, const double* alm, double* maps, voi
 sht_status_t sht_analysis_iter(sht_plan_t plan, const double* maps, double* alm, int niter,
                                double* resid_rms, void* stream);
 
-/* How sht_analysis_iter forms the residual of a round (same result up to rounding):
- *   SHT_ITER_TM    : on the ring spectra T_m(theta), the maps are read once (item 8; default; allocates a
- *                    second workspace on the first call and falls back to SHT_ITER_PIXEL if that does not fit);
- *   SHT_ITER_PIXEL : as residual maps (one backward and one forward ring FFT more per round). */
-enum { SHT_ITER_TM = 0, SHT_ITER_PIXEL = 1 };
+/* Which iteration sht_analysis_iter runs and how it forms the residual.
+ * Alg. 2, the "traditional" scheme, a_lm updated outside the m-loop -- two forms, same result up to
+ * rounding:
+ *   SHT_ITER_TM    : residual on the ring spectra T_m(theta), the maps are read once (item 8; default;
+ *                    allocates a second workspace on the first call and falls back to SHT_ITER_PIXEL if that does not fit);
+ *   SHT_ITER_PIXEL : as residual maps (one backward and one forward ring FFT more per round).
+ * Alg. 3, the "immediate" scheme, a_lm updated inside the m-loop:
+ *   SHT_ITER_IMMEDIATE : a(0) = analysis(map), r = map - synthesis(a(0)); then niter sweeps over m = 0 .. lmax in this
+ *                    order: delta a_m = order m of analysis(r), a_m += delta a_m, r -= synthesis(delta a_m) at once, so the
+ *                    orders after m see it through the ring aliasing (a Gauss-Seidel sweep; a different result from Alg. 2,
+ *                    more accurate for lmax < 3 nside).  r is kept as ring spectra T_m(theta).  resid_rms
+ *                    entry n = rms of r at the start of sweep n.  Spin-0 plans only (SHT_ERR_UNSUPPORTED otherwise); needs
+ *                    the second workspace (SHT_ERR_CUDA if it does not fit).  Sequential in m: 3 launches per order. */
+enum { SHT_ITER_TM = 0, SHT_ITER_PIXEL = 1, SHT_ITER_IMMEDIATE = 2 };
 sht_status_t sht_plan_set_iter_mode(sht_plan_t plan, int mode);
 
 /* Spin-2 plans: transforms of a_lm^E or a_lm^B alone (item 9: "forward and backward transforms of a^E

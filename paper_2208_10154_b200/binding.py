@@ -20,7 +20,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 SHT_OK = 0
 SHT_POL_E, SHT_POL_B = 1, 2
 SHT_LAMBDA_FUSED, SHT_LAMBDA_STAGED = 0, 1
-SHT_ITER_TM, SHT_ITER_PIXEL = 0, 1
+SHT_ITER_TM, SHT_ITER_PIXEL, SHT_ITER_IMMEDIATE = 0, 1, 2
 _vp, _i, _ll, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_double
 
 _lib.sht_plan_create.argtypes = [ctypes.POINTER(_vp), _i, _i, _i, _i]

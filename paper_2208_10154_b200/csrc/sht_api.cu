@@ -260,6 +260,64 @@ static sht_status_t iter_tm_space(sht_plan_t pl, const double* maps, double* alm
     return s;
 }
 
+// Alg. 3, the "immediate" iteration (reading G21 in DESIGN.md): a^0 by the plain analysis, the
+// residual R = T_m(map) - alias(T_m(synthesis a^0)) for all orders, then niter sweeps over m = 0 .. lmax in this order:
+// delta a_m = Legendre analysis of R at order m, a_m += delta a_m, Legendre synthesis of delta a_m at order m, and R
+// corrected at every order that shares a ring bin with m -- so the orders that follow see the correction (Gauss-Seidel).
+// Inherently sequential in m: 3 launches per order and sweep.  Spin 0.
+static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* alm, int niter, double* resid_rms, cudaStream_t st)
+{
+    const DevicePlan& d = pl->d;
+    double* acc = nullptr; double* da = nullptr;
+    SHT_TRY(cudaMallocAsync((void**)&acc, (size_t)pl->chunk * d.ncomp * sizeof(double), st), "rms scratch");
+    SHT_TRY(cudaMallocAsync((void**)&da, (size_t)pl->chunk * d.ncomp * d.nalm * 2 * sizeof(double), st), "increment scratch");
+    const size_t ubytes = (size_t)d.nh * d.ncomp * d.kpad * sizeof(double);
+    double* R = pl->F;              // residual, folded (even / odd), all orders
+    double* S = pl->Fmap;           // T_m(map) first, then the synthesised increment of one order at a time
+    for (int k0 = 0; k0 < pl->nmaps; k0 += pl->chunk) {
+        const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
+        const int nrow = kmaps * d.ncomp;
+        SHT_TRY(cudaMemsetAsync(pl->upow, 0, ubytes, st), "uncovered-power memset");
+        int t = timing_begin(pl, 0, st);
+        SHT_TRY(launch_ring_analysis(pl, d, maps, S, k0, kmaps, st, pl->upow), "ring analysis");
+        timing_end(pl, t, st);
+        t = timing_begin(pl, 1, st);
+        SHT_TRY(launch_legendre_analysis(pl, d, S, alm, k0, kmaps, false, st), "legendre analysis");
+        timing_end(pl, t, st);
+        t = timing_begin(pl, 2, st);
+        SHT_TRY(launch_legendre_synthesis(pl, d, alm, R, k0, kmaps, st), "legendre synthesis");
+        timing_end(pl, t, st);
+        SHT_TRY(cudaMemsetAsync(acc, 0, (size_t)nrow * sizeof(double), st), "rms memset");
+        t = timing_begin(pl, 3, st);
+        SHT_TRY(launch_ring_residual(pl, d, R, S, pl->upow, acc, kmaps, st), "ring residual");
+        timing_end(pl, t, st);
+        CUtensorMap tmF, tmA;
+        SHT_TRY(legendre_order_maps(d, R, da, kmaps, &tmF, &tmA), "tensor maps");
+        for (int it = 0; it < niter; ++it) {
+            if (it > 0 && resid_rms) {
+                SHT_TRY(cudaMemsetAsync(acc, 0, (size_t)nrow * sizeof(double), st), "rms memset");
+                SHT_TRY(launch_ring_power(pl, d, R, pl->upow, acc, kmaps, st), "ring power");
+            }
+            if (resid_rms) {
+                k_rms_finish<<<(nrow + 127) / 128, 128, 0, st>>>(acc, nrow, 1.0 / (double)d.npix,
+                                                                 resid_rms + (size_t)it * pl->nmaps * d.ncomp + (size_t)k0 * d.ncomp);
+                pl->launches++;
+                SHT_TRY(cudaGetLastError(), "rms kernel");
+            }
+            t = timing_begin(pl, 1, st);
+            for (int m = 0; m <= d.lmax; ++m) {
+                SHT_TRY(launch_legendre_analysis_order(pl, d, tmF, alm, da, k0, kmaps, m, st), "legendre analysis (one order)");
+                SHT_TRY(launch_legendre_synthesis_order(pl, d, tmA, S, kmaps, m, st), "legendre synthesis (one order)");
+                SHT_TRY(launch_gs_update(pl, d, S, R, m, kmaps, st), "residual update");
+            }
+            timing_end(pl, t, st);
+        }
+    }
+    cudaFreeAsync(da, st);
+    cudaFreeAsync(acc, st);
+    return SHT_OK;
+}
+
 extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, double* alm, int niter,
                                           double* resid_rms, void* stream)
 {
@@ -277,6 +335,10 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
             } else if (cudaMemset(pl->Fmap, 0, pl->F_bytes) != cudaSuccess) {
                 return cuda_fail(pl, "workspace memset", cudaGetLastError());
             }
+        }
+        if (pl->iter_mode == SHT_ITER_IMMEDIATE) {
+            if (!pl->Fmap) { snprintf(pl->err, sizeof(pl->err), "immediate iteration: no memory for the second workspace"); return SHT_ERR_CUDA; }
+            return iter_immediate(pl, maps, alm, niter, resid_rms, st);
         }
         if (pl->Fmap) return iter_tm_space(pl, maps, alm, niter, resid_rms, st);
     }
@@ -315,7 +377,11 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
 extern "C" sht_status_t sht_plan_set_iter_mode(sht_plan_t pl, int mode)
 {
     if (!pl) return SHT_ERR_NULL;
-    if (mode != SHT_ITER_TM && mode != SHT_ITER_PIXEL) return SHT_ERR_INVALID_ARG;
+    if (mode != SHT_ITER_TM && mode != SHT_ITER_PIXEL && mode != SHT_ITER_IMMEDIATE) return SHT_ERR_INVALID_ARG;
+    if (mode == SHT_ITER_IMMEDIATE && pl->d.spin != 0) {
+        snprintf(pl->err, sizeof(pl->err), "immediate iteration (Alg. 3) is built for spin 0 only");
+        return SHT_ERR_UNSUPPORTED;
+    }
     pl->iter_mode = mode;
     return SHT_OK;
 }

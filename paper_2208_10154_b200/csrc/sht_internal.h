@@ -110,7 +110,7 @@ struct sht_plan_s {
     long long launches;
     double* Fmap;                   // Alg. 2: folded T_m of the input maps (allocated on the first iterative call)
     double* upow;                   // Alg. 2: [nh][ncomp][kpad] uncovered ring power
-    int iter_mode;                  // SHT_ITER_TM (default) / SHT_ITER_PIXEL
+    int iter_mode;                  // SHT_ITER_TM (default) / SHT_ITER_PIXEL / SHT_ITER_IMMEDIATE
     double* lam;                    // staged-lambda scratch (nullptr: fused generation inside the contraction kernels)
     size_t lam_bytes;
     int* lam_i0;                    // [analysis blocks] first 16-row block with a started recurrence
@@ -148,6 +148,15 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st);
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
+// Alg. 3, one order m at a time (spin 0): tensor maps once per chunk, then per order analysis (alm += , da = increment),
+// synthesis of the increment into the cells of order m of S, and the update of the residual workspace R
+cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA);
+cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
+                                           int k0, int kmaps, int m, cudaStream_t st);
+cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
+                                            cudaStream_t st);
+cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int kmaps, cudaStream_t st);
+cudaError_t launch_ring_power(sht_plan_s* pl, const DevicePlan& d, const double* R, const double* upow, double* acc, int kmaps, cudaStream_t st);
 constexpr size_t LAM_ABLK_BYTES = 2 * 32 * 66 * 8;      // one analysis lambda block: [class][32 rings][66] doubles
 constexpr size_t LAM_SBLK_BYTES = 32 * 66 * 8;          // one synthesis lambda block: [32 l][66] doubles
 // spin 2 (sht_legendre_spin2.cu); the spin-0 launchers dispatch to these

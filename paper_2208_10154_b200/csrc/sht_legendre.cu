@@ -135,7 +135,8 @@ __global__ void __launch_bounds__(64) k_lambda_blocks_synthesis(DevicePlan d, do
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
-                    int nkt, int accumulate, const double* __restrict__ lam, const int* __restrict__ i0tab)
+                    int nkt, int accumulate, const double* __restrict__ lam, const int* __restrict__ i0tab,
+                    int m0, int tsplit, double* __restrict__ dout)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
@@ -145,7 +146,9 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     int* pst = reinterpret_cast<int*>(cft + A_ML);                                         // first ring of every l tile
     int* i0s = pst + ((d.ntile_max + 3) & ~3);                                               // per stage: first 16-row block with a started recurrence
 
-    const int m = blockIdx.x / nkt, kt = blockIdx.x % nkt;
+    // whole transform: one CTA per (m, k-tile), all l tiles.  One order at a time (Alg. 3, tsplit = 1, m = m0): one CTA
+    // per (l tile, k-tile) -- the tiles restart from the state table, so they are independent
+    const int m = tsplit ? m0 : m0 + blockIdx.x / nkt, kt = blockIdx.x % nkt;
     // warps 0..3 generate (the oldest warps of an SM sub-partition are served first by its scheduler: their
     // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
     const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) - LEG_GEN_WARPS;
@@ -153,6 +156,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
     const int ntile = (lmax - m) / A_ML + 1;
+    const int tb = tsplit ? (int)(blockIdx.x / nkt) : 0, te = tsplit ? tb + 1 : ntile;
 
     for (int t = tix; t < ntile; t += LEG_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
     if (tix == 0) {
@@ -173,7 +177,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
             for (int j = 0; j < 4; ++j) { c[i][j][0] = 0.0; c[i][j][1] = 0.0; }
         int stage = 0; uint32_t phase = 0;
         const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
-        for (int tile = 0; tile < ntile; ++tile) {
+        for (int tile = tb; tile < te; ++tile) {
             const int l0 = m + tile * A_ML;
             for (int pc = pst[tile]; pc < nh; pc += A_PC) {
                 mbar_wait(full + stage, phase);
@@ -232,6 +236,8 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                     if (l <= lmax && kk < kmaps) {
                         double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + l;
                         double2 v = make_double2(c[i][j][0], m == 0 ? 0.0 : c[i][j][1]);
+                        if (dout)                            // the increment itself, rows indexed from the chunk start
+                            reinterpret_cast<double2*>(dout)[((size_t)kk * d.ncomp + comp) * d.nalm + moff + l] = v;
                         if (accumulate) { const double2 o = *dst; v.x += o.x; v.y += o.y; }
                         *dst = v;
                     }
@@ -249,7 +255,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
             // copy from the scratch the generator kernel filled), and hands the consumers the block's first active row
             if (gw != 0 || lane != 0) return;
             int chunk = 0;
-            for (int tile = 0; tile < ntile; ++tile) {
+            for (int tile = tb; tile < te; ++tile) {
                 const size_t blk0 = (size_t)d.ablk_off[(size_t)m * d.ntile_max + tile];
                 int ck = 0;
                 for (int pc = pst[tile]; pc < nh; pc += A_PC, ++chunk, ++ck) {
@@ -277,14 +283,14 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
             const int l = l0 + gl;
             return l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
         };
-        double2 cf0 = load_cf(m);
+        double2 cf0 = load_cf(m + tb * A_ML);
         int chunk = 0;
-        for (int tile = 0; tile < ntile; ++tile) {
+        for (int tile = tb; tile < te; ++tile) {
             const int l0 = m + tile * A_ML;
             named_bar_sync(1, 128);                             // every generator is done with the previous tile
             cft[gl] = cf0;
             named_bar_sync(1, 128);
-            if (tile + 1 < ntile) cf0 = load_cf(l0 + A_ML);
+            if (tile + 1 < te) cf0 = load_cf(l0 + A_ML);
             const int lh = l0 + (A_ML / 2) * gh;                // first l of this warp's half
             const double2* cst = csm + (size_t)((lh - m) / LEG_CS) * nh;
             for (int pc = pst[tile]; pc < nh; pc += A_PC, ++chunk) {
@@ -350,7 +356,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
-                     int nkt, int npb, const double* __restrict__ lam)
+                     int nkt, int npb, const double* __restrict__ lam, int m0)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
@@ -363,7 +369,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
     // block order: m slowest (long m first), then ring block, k-tile fastest
     const int kt = blockIdx.x % nkt;
     const int pbi = (blockIdx.x / nkt) % npb;
-    const int m = blockIdx.x / (nkt * npb);
+    const int m = m0 + blockIdx.x / (nkt * npb);       // m0 > 0: one order at a time (Alg. 3)
     const int pb = pbi * S_PB;
     // warps 0..3 generate (the oldest warps of an SM sub-partition are served first by its scheduler: their
     // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
@@ -626,7 +632,41 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
         pl->launches++;
     }
     k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0,
-                                                       staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr);
+                                                       staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr, 0, 0, nullptr);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+// ---- one order m at a time (Alg. 3): the same kernels on the cells of order m only, lambda generated
+// in the kernel (fused mode).  The tensor maps are built once per sweep by the caller.
+cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)analysis_smem(d.ntile_max));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synthesis_smem());
+    if (e == cudaSuccess) e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, tmF);
+    if (e == cudaSuccess) e = make_tmap_alm(d, da, (long long)kmaps * d.ncomp, tmA);
+    return e;
+}
+
+// alm (rows from k0) += analysis of order m of F; da (rows from 0) = that increment
+cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
+                                           int k0, int kmaps, int m, cudaStream_t st)
+{
+    const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
+    const int ntile = (d.lmax - m) / A_ML + 1;
+    k_legendre_analysis<<<(unsigned)(ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
+                                                                                                 nullptr, m, 1, da);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+// F (north / south) at order m = synthesis of order m of da (rows from 0)
+cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
+                                            cudaStream_t st)
+{
+    const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
+    const int npb = (d.nh + S_PB - 1) / S_PB;
+    k_legendre_synthesis<<<(unsigned)(nkt * npb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -646,7 +686,7 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
         k_lambda_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
         pl->launches++;
     }
-    k_legendre_synthesis<<<(d.lmax + 1) * nkt * npb, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr);
+    k_legendre_synthesis<<<(d.lmax + 1) * nkt * npb, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0);
     pl->launches++;
     return cudaGetLastError();
 }

@@ -1008,6 +1008,85 @@ __global__ void __launch_bounds__(NT, 1) k_ring_residual(DevicePlan d, const int
     if (tot != 0.0) atomicAdd(acc_out + (size_t)k * d.ncomp + comp, tot / (double)N);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Alg. 3 ("update F from delta T_m"; reading G21): the residual R (folded T_m of map - synthesis(a),
+// all orders) is kept up to date order by order.  S holds, at order m only, the synthesised T_m (north / south) of the
+// increment delta a_m; its ring spectrum has one bin, bb = the bin m falls on, and every order m'' < mlim of the ring
+// pair that falls on the same bin (directly or as the conjugate) is corrected -- the arithmetic of k_ring_residual
+// restricted to one source order.  One thread per (ring pair, map).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* __restrict__ S, double* __restrict__ R, int m, int kmaps)
+{
+    const int p = blockIdx.y, comp = blockIdx.z;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const RingPair& rp = d.rings[p];
+    const int N = rp.n, mlim = rp.mlim;
+    if (k >= kmaps || m >= mlim) return;
+    const double2* tw2 = d.tw + rp.tw_off;
+    const bool equator = rp.start_s < 0, shift = rp.shift != 0;
+    const size_t cstride = (size_t)d.ncomp * 2 * KG;
+    const size_t cell0 = f_cell(d, p, k >> 2, 0, comp, 0) + (k & 3);
+    const double2* Sp = reinterpret_cast<const double2*>(S) + cell0 + (size_t)m * cstride;
+    double2 fn = Sp[0], fs = Sp[KG];
+    if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }
+    double2 ph = make_double2(1.0, 0.0);
+    if (shift) { ph = __ldg(tw2 + m % (2 * N)); ph.y = -ph.y; }
+    const double w = (m == 0) ? 0.5 : 1.0;
+    double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
+    dn.x *= w; dn.y *= w; ds.x *= w; ds.y *= w;
+    const int b = m % N;
+    const bool selfc = b == 0 || 2 * b == N;              // the bin is its own conjugate: both passes of the assembly hit it
+    const int bb = 2 * b > N ? N - b : b;
+    double2 yn, ys;
+    if (selfc) { yn = make_double2(2.0 * dn.x, 0.0); ys = make_double2(2.0 * ds.x, 0.0); }
+    else if (2 * b < N) { yn = dn; ys = ds; }
+    else { yn = make_double2(dn.x, -dn.y); ys = make_double2(ds.x, -ds.y); }
+    if (equator) ys = make_double2(0.0, 0.0);
+    const double scale = 4.0 * 3.14159265358979323846 / (double)d.npix * (double)N;
+    double2* Rp = reinterpret_cast<double2*>(R) + cell0;
+    for (int pass = 0; pass < (selfc ? 1 : 2); ++pass) {
+        double2 tn = yn, ts = ys;
+        if (pass == 1) { tn.y = -tn.y; ts.y = -ts.y; }
+        for (int mm = pass == 0 ? bb : N - bb; mm < mlim; mm += N) {
+            double2 p2 = make_double2(scale, 0.0);
+            if (shift) { p2 = __ldg(tw2 + mm % (2 * N)); p2.x *= scale; p2.y *= scale; }
+            double2 se, so;
+            if (equator) { se = cmul(p2, tn); so = make_double2(0.0, 0.0); }
+            else { se = cmul(p2, cadd(tn, ts)); so = cmul(p2, csub(tn, ts)); }
+            if (comp == 1) { se = make_double2(-se.y, se.x); so = make_double2(-so.y, so.x); }
+            double2* c = Rp + (size_t)mm * cstride;
+            c[0] = csub(c[0], se);
+            c[KG] = csub(c[KG], so);
+        }
+    }
+}
+
+// sum of squares of the residual pixels from R by Parseval (the accumulation of k_ring_residual on its own):
+// acc[k][comp] += (1/N) (sum over the orders m <= N/2, m < mlim of w |R_m|^2 / d sigma^2 + upow)
+__global__ void __launch_bounds__(128) k_ring_power(DevicePlan d, const double* __restrict__ R, const double* __restrict__ upow,
+                                                    double* __restrict__ acc_out, int kmaps)
+{
+    const int p = blockIdx.y, comp = blockIdx.z;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= kmaps) return;
+    const RingPair& rp = d.rings[p];
+    const int N = rp.n;
+    const bool equator = rp.start_s < 0;
+    const int mend = min(rp.mlim, N / 2 + 1);
+    const size_t cstride = (size_t)d.ncomp * 2 * KG;
+    const double2* Rp = reinterpret_cast<const double2*>(R) + f_cell(d, p, k >> 2, 0, comp, 0) + (k & 3);
+    double ssq = 0.0;
+    for (int m = 0; m < mend; ++m, Rp += cstride) {
+        const double2 E = Rp[0], O = Rp[KG];
+        const double w = (m == 0 || 2 * m == N) ? 1.0 : 2.0;
+        const double q = equator ? (E.x * E.x + E.y * E.y) : 0.5 * (E.x * E.x + E.y * E.y + O.x * O.x + O.y * O.y);
+        ssq = fma(w, q, ssq);
+    }
+    const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
+    const double tot = ssq / (dsig * dsig) + upow[((size_t)p * d.ncomp + comp) * d.kpad + k];
+    if (tot != 0.0) atomicAdd(acc_out + (size_t)k * d.ncomp + comp, tot / (double)N);
+}
+
 // CTAs that share an SM with another one run RING_THREADS threads; a CTA that owns the SM runs twice as many
 static int ring_threads(size_t smem) { return smem <= (size_t)113 * 1024 ? RING_THREADS : 2 * RING_THREADS; }
 
@@ -1068,6 +1147,20 @@ cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F,
         k_ring_residual<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c] + 512, st>>>(d, pl->class_rings[c], F, Fmap, upow, acc, kmaps);
         pl->launches++;
     }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int kmaps, cudaStream_t st)
+{
+    k_gs_update<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)d.nh, (unsigned)d.ncomp), 128, 0, st>>>(d, S, R, m, kmaps);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ring_power(sht_plan_s* pl, const DevicePlan& d, const double* R, const double* upow, double* acc, int kmaps, cudaStream_t st)
+{
+    k_ring_power<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)d.nh, (unsigned)d.ncomp), 128, 0, st>>>(d, R, upow, acc, kmaps);
+    pl->launches++;
     return cudaGetLastError();
 }
 
