@@ -182,6 +182,9 @@ def main():
     ap.add_argument("--iter", type=int, default=-1,
                     help="time sht_analysis_iter with this many Jacobi rounds (Alg. 2; BASELINE.json configs[4] uses 3) "
                          "instead of the synthesis + analysis step")
+    ap.add_argument("--iter-mode", default="tm", choices=["tm", "pixel", "immediate"],
+                    help="with --iter: Alg. 2 with the residual on the ring spectra (tm, default) or as maps (pixel), or "
+                         "Alg. 3, the immediate iteration (one order m at a time, spin 0)")
     ap.add_argument("--lambda-mode", default="", choices=["", "fused", "staged"],
                     help="where the P_lm tiles are generated (include/sht.h); default: the plan's own choice")
     ap.add_argument("--no-e2e", action="store_true")
@@ -242,8 +245,9 @@ def main():
             plan.sht_analysis_pol(maps, alm_out, which, stream)
     elif args.iter >= 0:
         # Alg. 2 on maps synthesised once outside the timed region: 2 niter + 1 transforms per step (eq. B8)
-        c["name"] += "_iter%d" % args.iter
+        c["name"] += "_iter%d" % args.iter + ("" if args.iter_mode == "tm" else "_" + args.iter_mode)
         args.no_e2e = True
+        plan.sht_plan_set_iter_mode({"tm": 0, "pixel": 1, "immediate": 2}[args.iter_mode])
         plan.sht_synthesis(alm, maps, stream)
         rms = torch.empty((max(args.iter, 1), nmaps * ncomp), dtype=torch.float64, device=dev)
 
@@ -286,8 +290,12 @@ def main():
     # kernel, same design, is reported beside it in "stages") ---------------------------------------------------------
     peaks, peak_src = read_measured_peaks()
     fl_dir = legendre_flops_per_direction(c) / (2 if args.pol else 1)   # half of the block products
+    # transforms per step inside the timed brackets of the Legendre stages (1 = analysis, 2 = synthesis).  Alg. 2: niter + 1
+    # analyses, niter syntheses.  Alg. 3: the "analysis" brackets hold the initial analysis and the sweeps, and a sweep does
+    # the analysis and the synthesis of every order (2 transforms); the one full synthesis is the initial residual
+    dirs = {1: 1, 2: 1}
     if args.iter >= 0:
-        fl_dir *= (args.iter + 1)                           # analysis launches per step (the synthesis ones: niter)
+        dirs = {1: 2 * args.iter + 1, 2: 1} if args.iter_mode == "immediate" else {1: args.iter + 1, 2: max(args.iter, 1)}
     mma_peak = sht_measure_fp64_mma_peak(300.0)
     peak_note = ("FP64 DMMA.8x8x4 register-resident loop measured live in this run "
                  "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = %.1f; "
@@ -297,7 +305,7 @@ def main():
     def leg_roofline(stage, kernel):
         n = max(1, stage_n[stage])                          # timed brackets = calls of the stage (generator + contraction)
         launch_ms = stage_ms[stage] / n
-        flops_per_launch = fl_dir * args.steps / n          # algorithmic (folded, unpruned) flops of one launch
+        flops_per_launch = fl_dir * dirs[stage] * args.steps / n          # algorithmic (folded, unpruned) flops of one launch
         ach = flops_per_launch / (launch_ms * 1e-3) * 1e-12
         return {"bound": "tensor", "kernel": kernel, "achieved": ach, "peak": mma_peak, "unit": "TFLOP/s",
                 "frac": ach / mma_peak, "traffic": NCU_TRAFFIC_BYTES.get((args.config, nmaps, lambda_mode, kernel)),
