@@ -94,7 +94,8 @@ sht_status_t sht_analysis_iter(sht_plan_t plan, const double* maps, double* alm,
  *                    orders after m see it through the ring aliasing (a Gauss-Seidel sweep; a different result from Alg. 2,
  *                    more accurate for lmax < 3 nside).  r is kept as ring spectra T_m(theta).  resid_rms
  *                    entry n = rms of r at the start of sweep n.  Spin-0 plans only (SHT_ERR_UNSUPPORTED otherwise); needs
- *                    the second workspace (SHT_ERR_CUDA if it does not fit).  Sequential in m: 3 launches per order. */
+ *                    the second workspace (SHT_ERR_CUDA if it does not fit).  Sequential in m within each parity class of m:
+ *                    3 launches per pair of orders (m even, m + 1). */
 enum { SHT_ITER_TM = 0, SHT_ITER_PIXEL = 1, SHT_ITER_IMMEDIATE = 2 };
 sht_status_t sht_plan_set_iter_mode(sht_plan_t plan, int mode);
 

@@ -264,7 +264,7 @@ static sht_status_t iter_tm_space(sht_plan_t pl, const double* maps, double* alm
 // residual R = T_m(map) - alias(T_m(synthesis a^0)) for all orders, then niter sweeps over m = 0 .. lmax in this order:
 // delta a_m = Legendre analysis of R at order m, a_m += delta a_m, Legendre synthesis of delta a_m at order m, and R
 // corrected at every order that shares a ring bin with m -- so the orders that follow see the correction (Gauss-Seidel).
-// Inherently sequential in m: 3 launches per order and sweep.  Spin 0.
+// Sequential in m within each parity class: 3 launches per pair of orders (m even, m + 1) and sweep.  Spin 0.
 static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* alm, int niter, double* resid_rms, cudaStream_t st)
 {
     const DevicePlan& d = pl->d;
@@ -305,10 +305,13 @@ static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* al
                 SHT_TRY(cudaGetLastError(), "rms kernel");
             }
             t = timing_begin(pl, 1, st);
-            for (int m = 0; m <= d.lmax; ++m) {
-                SHT_TRY(launch_legendre_analysis_order(pl, d, tmF, alm, da, k0, kmaps, m, st), "legendre analysis (one order)");
-                SHT_TRY(launch_legendre_synthesis_order(pl, d, tmA, S, kmaps, m, st), "legendre synthesis (one order)");
-                SHT_TRY(launch_gs_update(pl, d, S, R, m, kmaps, st), "residual update");
+            // an even and an odd order never fall on the same bin of a ring of 4q pixels (m' = +-m mod 4q keeps the parity):
+            // the orders m, m + 1 of a step are independent, and the sweep equals the one-by-one sweep bit for bit
+            for (int m = 0; m <= d.lmax; m += 2) {
+                const int nm = m < d.lmax ? 2 : 1;
+                SHT_TRY(launch_legendre_analysis_order(pl, d, tmF, alm, da, k0, kmaps, m, nm, st), "legendre analysis (orders m, m+1)");
+                SHT_TRY(launch_legendre_synthesis_order(pl, d, tmA, S, kmaps, m, nm, st), "legendre synthesis (orders m, m+1)");
+                SHT_TRY(launch_gs_update(pl, d, S, R, m, nm, kmaps, st), "residual update");
             }
             timing_end(pl, t, st);
         }

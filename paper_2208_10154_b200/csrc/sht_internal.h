@@ -148,14 +148,14 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st);
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
-// Alg. 3, one order m at a time (spin 0): tensor maps once per chunk, then per order analysis (alm += , da = increment),
-// synthesis of the increment into the cells of order m of S, and the update of the residual workspace R
+// Alg. 3, the orders m .. m + nm - 1 at a time (spin 0): tensor maps once per chunk, then per step analysis (alm += , da =
+// increment), synthesis of the increment into the cells of these orders of S, and the update of the residual workspace R
 cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA);
 cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
-                                           int k0, int kmaps, int m, cudaStream_t st);
+                                           int k0, int kmaps, int m, int nm, cudaStream_t st);
 cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
-                                            cudaStream_t st);
-cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int kmaps, cudaStream_t st);
+                                            int nm, cudaStream_t st);
+cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st);
 cudaError_t launch_ring_power(sht_plan_s* pl, const DevicePlan& d, const double* R, const double* upow, double* acc, int kmaps, cudaStream_t st);
 constexpr size_t LAM_ABLK_BYTES = 2 * 32 * 66 * 8;      // one analysis lambda block: [class][32 rings][66] doubles
 constexpr size_t LAM_SBLK_BYTES = 32 * 66 * 8;          // one synthesis lambda block: [32 l][66] doubles

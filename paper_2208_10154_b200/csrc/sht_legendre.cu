@@ -146,9 +146,11 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     int* pst = reinterpret_cast<int*>(cft + A_ML);                                         // first ring of every l tile
     int* i0s = pst + ((d.ntile_max + 3) & ~3);                                               // per stage: first 16-row block with a started recurrence
 
-    // whole transform: one CTA per (m, k-tile), all l tiles.  One order at a time (Alg. 3, tsplit = 1, m = m0): one CTA
-    // per (l tile, k-tile) -- the tiles restart from the state table, so they are independent
-    const int m = tsplit ? m0 : m0 + blockIdx.x / nkt, kt = blockIdx.x % nkt;
+    // whole transform: one CTA per (m, k-tile), all l tiles.  A few orders at a time (Alg. 3, tsplit = number of orders
+    // m0, m0 + 1, ..): one CTA per (order, l tile, k-tile) -- the tiles restart from the state table, so they are
+    // independent; the grid is sized for the tiles of m0, the CTAs past the last tile of their order leave
+    const int nt0 = (d.lmax - m0) / A_ML + 1;
+    const int m = tsplit ? m0 + blockIdx.x / (nkt * nt0) : m0 + blockIdx.x / nkt, kt = blockIdx.x % nkt;
     // warps 0..3 generate (the oldest warps of an SM sub-partition are served first by its scheduler: their
     // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
     const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) - LEG_GEN_WARPS;
@@ -156,7 +158,8 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
     const int ntile = (lmax - m) / A_ML + 1;
-    const int tb = tsplit ? (int)(blockIdx.x / nkt) : 0, te = tsplit ? tb + 1 : ntile;
+    const int tb = tsplit ? (int)(blockIdx.x / nkt) % nt0 : 0, te = tsplit ? tb + 1 : ntile;
+    if (tb >= ntile) return;
 
     for (int t = tix; t < ntile; t += LEG_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
     if (tix == 0) {
@@ -648,25 +651,25 @@ cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const doub
     return e;
 }
 
-// alm (rows from k0) += analysis of order m of F; da (rows from 0) = that increment
+// alm (rows from k0) += analysis of the orders m .. m + nm - 1 of F; da (rows from 0) = that increment
 cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
-                                           int k0, int kmaps, int m, cudaStream_t st)
+                                           int k0, int kmaps, int m, int nm, cudaStream_t st)
 {
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int ntile = (d.lmax - m) / A_ML + 1;
-    k_legendre_analysis<<<(unsigned)(ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
-                                                                                                 nullptr, m, 1, da);
+    k_legendre_analysis<<<(unsigned)(nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
+                                                                                                      nullptr, m, nm, da);
     pl->launches++;
     return cudaGetLastError();
 }
 
-// F (north / south) at order m = synthesis of order m of da (rows from 0)
+// F (north / south) at the orders m .. m + nm - 1 = synthesis of those orders of da (rows from 0)
 cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
-                                            cudaStream_t st)
+                                            int nm, cudaStream_t st)
 {
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
-    k_legendre_synthesis<<<(unsigned)(nkt * npb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m);
+    k_legendre_synthesis<<<(unsigned)(nm * nkt * npb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m);
     pl->launches++;
     return cudaGetLastError();
 }

@@ -1015,9 +1015,9 @@ __global__ void __launch_bounds__(NT, 1) k_ring_residual(DevicePlan d, const int
 // pair that falls on the same bin (directly or as the conjugate) is corrected -- the arithmetic of k_ring_residual
 // restricted to one source order.  One thread per (ring pair, map).
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* __restrict__ S, double* __restrict__ R, int m, int kmaps)
+__global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* __restrict__ S, double* __restrict__ R, int m0, int kmaps)
 {
-    const int p = blockIdx.y, comp = blockIdx.z;
+    const int p = blockIdx.y, comp = 0, m = m0 + blockIdx.z;      // spin 0; the orders of one launch never share a bin
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const RingPair& rp = d.rings[p];
     const int N = rp.n, mlim = rp.mlim;
@@ -1150,9 +1150,9 @@ cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F,
     return cudaGetLastError();
 }
 
-cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int kmaps, cudaStream_t st)
+cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st)
 {
-    k_gs_update<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)d.nh, (unsigned)d.ncomp), 128, 0, st>>>(d, S, R, m, kmaps);
+    k_gs_update<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)d.nh, (unsigned)nm), 128, 0, st>>>(d, S, R, m, kmaps);
     pl->launches++;
     return cudaGetLastError();
 }
