@@ -93,7 +93,7 @@ sht_status_t sht_analysis_iter(sht_plan_t plan, const double* maps, double* alm,
  *                    order: delta a_m = order m of analysis(r), a_m += delta a_m, r -= synthesis(delta a_m) at once, so the
  *                    orders after m see it through the ring aliasing (a Gauss-Seidel sweep; a different result from Alg. 2,
  *                    more accurate for lmax < 3 nside).  r is kept as ring spectra T_m(theta).  resid_rms
- *                    entry n = rms of r at the start of sweep n.  Spin-0 plans only (SHT_ERR_UNSUPPORTED otherwise); needs
+ *                    entry n = rms of r at the start of sweep n.  Spin 0 and spin 2 (E and B of an order together); needs
  *                    the second workspace (SHT_ERR_CUDA if it does not fit).  Sequential in m within each parity class of m:
  *                    3 launches per pair of orders (m even, m + 1). */
 enum { SHT_ITER_TM = 0, SHT_ITER_PIXEL = 1, SHT_ITER_IMMEDIATE = 2 };

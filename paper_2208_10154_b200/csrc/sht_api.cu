@@ -264,7 +264,8 @@ static sht_status_t iter_tm_space(sht_plan_t pl, const double* maps, double* alm
 // residual R = T_m(map) - alias(T_m(synthesis a^0)) for all orders, then niter sweeps over m = 0 .. lmax in this order:
 // delta a_m = Legendre analysis of R at order m, a_m += delta a_m, Legendre synthesis of delta a_m at order m, and R
 // corrected at every order that shares a ring bin with m -- so the orders that follow see the correction (Gauss-Seidel).
-// Sequential in m within each parity class: 3 launches per pair of orders (m even, m + 1) and sweep.  Spin 0.
+// Sequential in m within each parity class: 3 launches per pair of orders (m even, m + 1) and sweep.  Spin 0 and spin 2
+// (E and B of an order are corrected together).
 static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* alm, int niter, double* resid_rms, cudaStream_t st)
 {
     const DevicePlan& d = pl->d;
@@ -381,10 +382,6 @@ extern "C" sht_status_t sht_plan_set_iter_mode(sht_plan_t pl, int mode)
 {
     if (!pl) return SHT_ERR_NULL;
     if (mode != SHT_ITER_TM && mode != SHT_ITER_PIXEL && mode != SHT_ITER_IMMEDIATE) return SHT_ERR_INVALID_ARG;
-    if (mode == SHT_ITER_IMMEDIATE && pl->d.spin != 0) {
-        snprintf(pl->err, sizeof(pl->err), "immediate iteration (Alg. 3) is built for spin 0 only");
-        return SHT_ERR_UNSUPPORTED;
-    }
     pl->iter_mode = mode;
     return SHT_OK;
 }

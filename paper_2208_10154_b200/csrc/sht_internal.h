@@ -148,7 +148,7 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st);
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
-// Alg. 3, the orders m .. m + nm - 1 at a time (spin 0): tensor maps once per chunk, then per step analysis (alm += , da =
+// Alg. 3, the orders m .. m + nm - 1 at a time: tensor maps once per chunk, then per step analysis (alm += , da =
 // increment), synthesis of the increment into the cells of these orders of S, and the update of the residual workspace R
 cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA);
 cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
@@ -164,6 +164,11 @@ cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, 
                                            bool accumulate, cudaStream_t st);
 cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps,
                                             cudaStream_t st);
+cudaError_t legendre_order_maps_spin2(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA);
+cudaError_t launch_legendre_analysis_order_spin2(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
+                                                 int k0, int kmaps, int m, int nm, cudaStream_t st);
+cudaError_t launch_legendre_synthesis_order_spin2(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
+                                                  int nm, cudaStream_t st);
 // plan-time seed table (sht_plan.cu)
 cudaError_t launch_seed_table(const DevicePlan& d, const double* cm, int* lstart, double2* seed, cudaStream_t st);
 cudaError_t launch_chunk_seeds(const DevicePlan& d, double2* cseed, cudaStream_t st);

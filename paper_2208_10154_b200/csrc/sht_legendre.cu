@@ -644,6 +644,7 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
 // in the kernel (fused mode).  The tensor maps are built once per sweep by the caller.
 cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA)
 {
+    if (d.spin == 2) return legendre_order_maps_spin2(d, F, da, kmaps, tmF, tmA);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)analysis_smem(d.ntile_max));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synthesis_smem());
     if (e == cudaSuccess) e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, tmF);
@@ -655,6 +656,7 @@ cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const doub
 cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
                                            int k0, int kmaps, int m, int nm, cudaStream_t st)
 {
+    if (d.spin == 2) return launch_legendre_analysis_order_spin2(pl, d, tmF, alm, da, k0, kmaps, m, nm, st);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int ntile = (d.lmax - m) / A_ML + 1;
     k_legendre_analysis<<<(unsigned)(nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
@@ -667,6 +669,7 @@ cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, 
 cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
                                             int nm, cudaStream_t st)
 {
+    if (d.spin == 2) return launch_legendre_synthesis_order_spin2(pl, d, tmA, F, kmaps, m, nm, st);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
     k_legendre_synthesis<<<(unsigned)(nm * nkt * npb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m);

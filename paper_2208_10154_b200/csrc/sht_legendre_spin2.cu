@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(64) k_fpm_blocks_synthesis(DevicePlan d, doubl
 template <int WHICH>
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
-                          int nkt, int accumulate, const double* __restrict__ lam)
+                          int nkt, int accumulate, const double* __restrict__ lam, int m0, int tsplit, double* __restrict__ dout)
 {
     constexpr int nst = 3;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -187,10 +187,15 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
     double* ct3 = reinterpret_cast<double*>(ctu + 2 * A2_ML);
     int* pst = reinterpret_cast<int*>(ct3 + A2_ML);
 
-    const int m = blockIdx.x / nkt, kt = blockIdx.x % nkt;
+    // whole transform: one CTA per (m, k-tile), all l tiles.  Alg. 3 (tsplit = number of orders m0, m0 + 1, ..): one CTA
+    // per (order, l tile, k-tile), as in the spin-0 kernel
+    const int nt0 = (d.lmax - m0) / A2_ML + 1;
+    const int m = tsplit ? m0 + blockIdx.x / (nkt * nt0) : m0 + blockIdx.x / nkt, kt = blockIdx.x % nkt;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lmax = d.lmax, nh = d.nh;
     const int ntile = (lmax - m) / A2_ML + 1;
+    const int tb = tsplit ? (int)(blockIdx.x / nkt) % nt0 : 0, te = tsplit ? tb + 1 : ntile;
+    if (tb >= ntile) return;
 
     for (int t = tid; t < ntile; t += LEG2_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
     if (tid == 0) {
@@ -211,7 +216,7 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
             for (int j = 0; j < 2; ++j) { cE[i][j][0] = cE[i][j][1] = 0.0; cB[i][j][0] = cB[i][j][1] = 0.0; }
         int stage = 0; uint32_t phase = 0;
         const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
-        for (int tile = 0; tile < ntile; ++tile) {
+        for (int tile = tb; tile < te; ++tile) {
             const int l0 = m + tile * A2_ML;
             for (int pc = pst[tile]; pc < nh; pc += A2_PC) {
                 mbar_wait(full + stage, phase);
@@ -259,6 +264,11 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                         double2 vb = make_double2(cB[i][j][1], m == 0 ? 0.0 : -cB[i][j][0]);
                         if (WHICH == 0) {
                             double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * 2) * d.nalm + moff + l;
+                            if (dout) {                          // the increment itself, pairs indexed from the chunk start
+                                double2* dd = reinterpret_cast<double2*>(dout) + ((size_t)kk * 2) * d.nalm + moff + l;
+                                dd[0] = ve;
+                                dd[d.nalm] = vb;
+                            }
                             if (accumulate) {
                                 const double2 oe = dst[0], ob = dst[d.nalm];
                                 ve.x += oe.x; ve.y += oe.y; vb.x += ob.x; vb.y += ob.y;
@@ -285,7 +295,7 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
             // ===== staged mode: one thread streams, per stage, the chunk's Q / iU lines (TMA) and its F+/F- block (bulk copy)
             if (gw != 0 || lane != 0) return;
             int stage = 0; uint32_t phase = 0;
-            for (int tile = 0; tile < ntile; ++tile) {
+            for (int tile = tb; tile < te; ++tile) {
                 const size_t blk0 = (size_t)d.ablk_off[(size_t)m * d.ntile_max + tile];
                 int ck = 0;
                 for (int pc = pst[tile]; pc < nh; pc += A2_PC, ++ck) {
@@ -311,14 +321,14 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
             nab = l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
             spin2_consts(d, l, m, ntp, ntm, nt3);
         };
-        load_consts(m);
+        load_consts(m + tb * A2_ML);
         int stage = 0; uint32_t phase = 0;
-        for (int tile = 0; tile < ntile; ++tile) {
+        for (int tile = tb; tile < te; ++tile) {
             const int l0 = m + tile * A2_ML;
             named_bar_sync(1, 128);                             // every generator is done with the previous tile
             cft[gl] = nab; ctu[gl] = ntp; ctu[A2_ML + gl] = ntm; ct3[gl] = nt3;
             named_bar_sync(1, 128);
-            if (tile + 1 < ntile) load_consts(l0 + A2_ML);
+            if (tile + 1 < te) load_consts(l0 + A2_ML);
             const int lq = l0 + QL * gw;                        // first l of this warp's quarter
             const double2* cst = csm + (size_t)((lq - m) / LEG_CS) * nh;
             for (int pc = pst[tile]; pc < nh; pc += A2_PC) {
@@ -369,10 +379,10 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
 // Q(north) = Qe + Qo, Q(south) = Qe - Qo; iU likewise with A^E and iA^B exchanged.
 // ------------------------------------------------------------------------------------------------
 // WHICH = 0: alm holds (a_E, a_B) per pair; 1 / 2: alm[map][nalm] holds only a_E / only a_B, the other one is zero
-template <int WHICH>
+template <int WHICH, bool ORD = false>
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
-                           int nkt, int npb, const double* __restrict__ lam)
+                           int nkt, int npb, const double* __restrict__ lam, int m0)
 {
     constexpr int NST = 3;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -384,7 +394,8 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
 
     const int kt = blockIdx.x % nkt;
     const int pbi = (blockIdx.x / nkt) % npb;
-    const int m = blockIdx.x / (nkt * npb);
+    // ORD: a few orders at a time from m0 (Alg. 3); a separate instantiation keeps the whole-transform kernel's registers
+    const int m = (ORD ? m0 : 0) + blockIdx.x / (nkt * npb);
     const int pb = pbi * S2_PB;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lmax = d.lmax, nh = d.nh;
@@ -621,7 +632,7 @@ cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, 
         k_fpm_blocks_analysis<<<dim3((unsigned)(d.ntile_max * d.nck_max), (unsigned)(d.lmax + 1)), 128, 0, st>>>(d, pl->lam);
         pl->launches++;
     }
-    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, staged ? pl->lam : nullptr);
+    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, staged ? pl->lam : nullptr, 0, 0, nullptr);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -642,7 +653,38 @@ cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d,
         k_fpm_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
         pl->launches++;
     }
-    kern<<<(d.lmax + 1) * nkt * npb, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr);
+    kern<<<(d.lmax + 1) * nkt * npb, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+// ---- a few orders at a time (Alg. 3): the spin-2 side of the per-order launchers of sht_legendre.cu
+cudaError_t legendre_order_maps_spin2(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis_spin2<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)analysis2_smem(d.ntile_max));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_legendre_synthesis_spin2<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synthesis2_smem());
+    if (e == cudaSuccess) e = make_tmap_F(d, F, P_KG, 2, tmF);
+    if (e == cudaSuccess) e = make_tmap_alm_spin2(d, da, (long long)kmaps, 2, tmA);
+    return e;
+}
+
+cudaError_t launch_legendre_analysis_order_spin2(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
+                                                 int k0, int kmaps, int m, int nm, cudaStream_t st)
+{
+    const int nkt = (kmaps + P_KT - 1) / P_KT;
+    const int ntile = (d.lmax - m) / A2_ML + 1;
+    k_legendre_analysis_spin2<0><<<(unsigned)(nm * ntile * nkt), LEG2_THREADS, analysis2_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1,
+                                                                                                                 nullptr, m, nm, da);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_legendre_synthesis_order_spin2(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
+                                                  int nm, cudaStream_t st)
+{
+    const int nkt = (kmaps + P_KT - 1) / P_KT;
+    const int npb = (d.nh + S2_PB - 1) / S2_PB;
+    k_legendre_synthesis_spin2<0, true><<<(unsigned)(nm * nkt * npb), LEG2_THREADS, synthesis2_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m);
     pl->launches++;
     return cudaGetLastError();
 }

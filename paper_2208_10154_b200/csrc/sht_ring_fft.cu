@@ -1017,7 +1017,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_residual(DevicePlan d, const int
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* __restrict__ S, double* __restrict__ R, int m0, int kmaps)
 {
-    const int p = blockIdx.y, comp = 0, m = m0 + blockIdx.z;      // spin 0; the orders of one launch never share a bin
+    const int p = blockIdx.y, comp = blockIdx.z % d.ncomp, m = m0 + blockIdx.z / d.ncomp;   // the orders of one launch never share a bin
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const RingPair& rp = d.rings[p];
     const int N = rp.n, mlim = rp.mlim;
@@ -1152,7 +1152,7 @@ cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F,
 
 cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st)
 {
-    k_gs_update<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)d.nh, (unsigned)nm), 128, 0, st>>>(d, S, R, m, kmaps);
+    k_gs_update<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)d.nh, (unsigned)(nm * d.ncomp)), 128, 0, st>>>(d, S, R, m, kmaps);
     pl->launches++;
     return cudaGetLastError();
 }

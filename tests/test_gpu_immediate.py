@@ -94,9 +94,25 @@ def test_immediate_chunked_workspace_and_repeat():
     assert np.allclose(r_full, r_small, rtol=1e-12, atol=0.0)
 
 
-def test_immediate_is_refused_for_spin2_plans():
+@pytest.mark.parametrize("nside,lmax,nmaps,niter,noise", [
+    (16, 31, 3, 3, 0.0),
+    (16, 47, 2, 2, 0.2),       # lmax = 3 nside - 1, not band-limited
+    (32, 95, 40, 2, 0.0),      # two k-tiles of 32 pairs
+    (64, 150, 2, 1, 0.0),      # two l tiles per order
+    (5, 14, 2, 3, 0.1),
+])
+def test_immediate_iteration_spin2_against_oracle(nside, lmax, nmaps, niter, noise):
+    """spin 2: E and B of an order are corrected together; (Q, U) residual kept as ring spectra of Q and iU"""
+    from oracle import oracle as O
     from paper_2208_10154_b200.binding import Plan, SHT_ITER_IMMEDIATE
-    plan = Plan(8, 15, 2, 2)
-    with pytest.raises(Exception, match="spin 0"):
-        plan.sht_plan_set_iter_mode(SHT_ITER_IMMEDIATE)
+    alm_true = inputs.gaussian_alm(lmax, np.arange(nmaps), 95, 2)
+    maps = O.synthesis(nside, lmax, alm_true, spin=2)
+    if noise > 0.0:
+        maps = maps + inputs.white_noise(nside, np.arange(nmaps), 96, noise, spin=2)
+    ref_alm, ref_rms = O.analysis_iter_immediate(nside, lmax, maps, niter, spin=2)
+    plan = Plan(nside, lmax, nmaps, 2)
+    got_alm, got_rms = _run(plan, maps, niter, SHT_ITER_IMMEDIATE)
     plan.destroy()
+    assert np.isfinite(got_alm).all()
+    assert inputs.rel_err(got_alm, ref_alm) <= TOL
+    assert np.abs(got_rms - ref_rms).max() <= 1e-9 * ref_rms[0].max()
