@@ -166,6 +166,50 @@ def test_config5_iterative_composition():
     plan.destroy()
 
 
+def test_config5_immediate_iteration_properties():
+    """Alg. 3 (SHT_ITER_IMMEDIATE) at BASELINE.json configs[4] shapes (nside 1024, lmax 2047; 64 maps = one k-tile, 3
+    sweeps).  The oracle's sweep needs ~6000 single-order transforms here, so at full size the entry is checked through
+    properties that hold at any size: the first rms entry is the residual of the plain analysis, i.e. equal to Alg. 2's
+    first entry; a band-limited input is a fixed point the sweeps converge to (PAPER.md:382); the rms falls every sweep;
+    a second call repeats the first bit for bit.  Element-by-element parity with the oracle: tests/test_gpu_immediate.py."""
+    import torch
+    from paper_2208_10154_b200.binding import Plan, SHT_ITER_IMMEDIATE, SHT_ITER_TM
+    c = inputs.CONFIGS[5]
+    nside, lmax, niter, nmaps = c["nside"], c["lmax"], c["niter"], 64
+    dev = torch.device("cuda:0")
+    plan = Plan(nside, lmax, nmaps, 0)
+    alm_true = torch.empty((nmaps, 1, plan.nalm), dtype=torch.complex128, device=dev)
+    for k0 in range(0, nmaps, 16):
+        kk = np.arange(k0, min(nmaps, k0 + 16))
+        alm_true[k0:k0 + len(kk)] = torch.from_numpy(inputs.gaussian_alm(lmax, kk, c["seed"])).to(dev)
+    maps = torch.empty((nmaps, 1, plan.npix), dtype=torch.float64, device=dev)
+    plan.sht_synthesis(alm_true, maps)
+    out = {}
+    for name, mode in (("imm", SHT_ITER_IMMEDIATE), ("imm2", SHT_ITER_IMMEDIATE), ("trad", SHT_ITER_TM)):
+        plan.sht_plan_set_iter_mode(mode)
+        a = torch.full_like(alm_true, float("nan"))
+        rms = torch.full((niter, nmaps), float("nan"), dtype=torch.float64, device=dev)
+        plan.sht_analysis_iter(maps, a, niter, rms)
+        torch.cuda.synchronize()
+        out[name] = (a, rms.cpu().numpy())
+    a_imm, r_imm = out["imm"]
+    assert torch.isfinite(a_imm.real).all() and torch.isfinite(a_imm.imag).all()
+    assert torch.equal(a_imm, out["imm2"][0])
+    assert np.allclose(r_imm[0], out["trad"][1][0], rtol=1e-9, atol=0.0)
+    assert np.all(r_imm[1:] < 0.25 * r_imm[:-1]), r_imm[:, :3]
+    amax = alm_true.abs().amax(dim=(1, 2))
+    err_imm = float(((a_imm - alm_true).abs().amax(dim=(1, 2)) / amax).max())
+    a0 = torch.empty_like(alm_true)
+    plan.sht_analysis(maps, a0)
+    torch.cuda.synchronize()
+    err_0 = float(((a0 - alm_true).abs().amax(dim=(1, 2)) / amax).max())
+    err_trad = float(((out["trad"][0] - alm_true).abs().amax(dim=(1, 2)) / amax).max())
+    print("config 5 shapes, 64 maps: a_lm error after 0 rounds %.2e, 3 immediate sweeps %.2e, 3 traditional rounds %.2e"
+          % (err_0, err_imm, err_trad))
+    assert err_imm < 1e-2 * err_0
+    plan.destroy()
+
+
 @pytest.mark.parametrize("nside,lmax", [(1000, 150), (331, 400)])
 def test_large_odd_nside_sampled(nside, lmax):
     """nside that is not a power of two: every ring length 4 i occurs, primes up to 997 among the i (Bluestein with
