@@ -77,6 +77,7 @@ struct DevicePlan {
     const int* ablk_off;            // [lmax+1][ntile_max] first analysis block (32 rings x 128 l) of (m, l tile)
     const int* sblk_off;            // [lmax+1][npb] first synthesis block (32 l x 64 rings) of (m, ring block)
     const int* scfirst;             // [lmax+1][npb] first l of the first synthesis block (lmax + 1: none)
+    const int* sminls8;             // [lmax+1][npb][8] smallest l_safe of every 8 ring pairs of a synthesis ring block
     int npb;                        // ring blocks of 64
     int nck_max, nst_max;           // most analysis chunks per (m, tile), most synthesis stages per (m, ring block)
 };

@@ -37,8 +37,6 @@ constexpr int S_STAGES = 4;                  // even: the generators fill stages
 constexpr int S_ABYTES = S_LC * KTILE_MAPS * 16;     // a_lm tile of a stage: 32 KB
 constexpr int S_LBYTES = S_LC * S_SL * 8;
 constexpr int S_STAGE_BYTES = (S_ABYTES + S_LBYTES + 1023) / 1024 * 1024;
-constexpr int S_SC = NK + 8;                 // epilogue staging row stride (doubles)
-static_assert(2 * S_PB * S_SC * 8 <= S_STAGES * S_STAGE_BYTES, "epilogue staging reuses the stage memory");
 
 // ------------------------------------------------------------------------------------------------
 // Staged-lambda mode: the lambda tiles of one transform, written block by block to an HBM scratch in exactly the
@@ -354,54 +352,44 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
 }
 
 // ------------------------------------------------------------------------------------------------
-// synthesis kernel: one CTA per (m, block of 64 ring pairs, k-tile); loops over l chunks of 32.
+// synthesis kernel: one CTA per (m, k-tile, share of the blocks of 64 ring pairs); per block it loops over l chunks of
+// 32.  The CTA walks its ring blocks back to back: the mbarrier pipeline keeps running across them (the generators
+// fill the stages of the next block while the consumers finish and store the current one), so its fill and drain are
+// paid once per CTA instead of once per block.  Whole transforms give a CTA all blocks of (m, k-tile) (nsplit = 1);
+// the one-order launches of Alg. 3 spread the blocks over nsplit CTAs.
+// The even sum Ee (l - m even) and the odd sum Oo of a ring pair are stored as they leave the accumulators, in the two
+// halves of the pair's workspace line; north = Ee + Oo and south = Ee - Oo are formed by the ring kernels on load.
 // Stage layout: [a_lm: 4 boxes x (64 maps x 8 l x 16 B, 128B-swizzled)] [lambda: 32 l x S_SL]
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
-                     int nkt, int npb, const double* __restrict__ lam, int m0)
+                     int nkt, int npb, const double* __restrict__ lam, int m0, int nsplit)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S_STAGES * S_STAGE_BYTES);
     uint64_t* empty = full + S_STAGES;
     double2* cfs = reinterpret_cast<double2*>(empty + S_STAGES);      // 4 generator warps x 2 buffers x S_LC/2 (alpha, beta)
-    int* lmin_s = reinterpret_cast<int*>(cfs + 4 * S_LC);
-    int* minls8 = lmin_s + 4;                                         // smallest l_safe of every 8-ring row block
 
-    // block order: m slowest (long m first), then ring block, k-tile fastest
+    // block order: m slowest (long m first), then the share of ring blocks, k-tile fastest
     const int kt = blockIdx.x % nkt;
-    const int pbi = (blockIdx.x / nkt) % npb;
-    const int m = m0 + blockIdx.x / (nkt * npb);       // m0 > 0: one order at a time (Alg. 3)
-    const int pb = pbi * S_PB;
+    const int sp = (blockIdx.x / nkt) % nsplit;
+    const int m = m0 + blockIdx.x / (nkt * nsplit);
     // warps 0..3 generate (the oldest warps of an SM sub-partition are served first by its scheduler: their
     // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
     const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) - LEG_GEN_WARPS;
     const int tix = threadIdx.x;
-    const int tid = tix - LEG_GEN_WARPS * 32;                  // consumer thread index (negative for generators)
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
-    const int plast = min(pb + S_PB, nh) - 1;
-    if (m >= d.mlim[plast]) return;                    // no ring of this block takes part in order m (never read)
 
     if (tix == 0) {
         for (int s = 0; s < S_STAGES; ++s) { mbar_init(full + s, lam ? 1 : 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS); }
         fence_barrier_init();
         tma_prefetch_desc(&tmA);
-        *lmin_s = lmax + 1;
-    }
-    if (tix < 8) minls8[tix] = lmax + 1;
-    __syncthreads();
-    if (tix < S_PB && pb + tix < nh) {
-        const int lsv = d.lstart[(size_t)m * nh + pb + tix];
-        atomicMin(lmin_s, lsv);
-        atomicMin(minls8 + (tix >> 3), lsv);
     }
     __syncthreads();
-    const int lmin = *lmin_s;
-    // chunks are aligned to m so that (l - m) even <-> even local index
-    const int cfirst = (lmin > lmax) ? (lmax + 1) : m + ((lmin - m) / S_LC) * S_LC;
     const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
+    const int* scf = d.scfirst + (size_t)m * npb;
 
     if (warp >= 0) {
         // ===== consumers: C[p, k'] += lambda[l, p] a[l, k'] over the l of this warp's parity class =====
@@ -414,87 +402,81 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
             for (int j = 0; j < 4; ++j) { c[i][j][0] = 0.0; c[i][j][1] = 0.0; }
         int stage = 0; uint32_t phase = 0;
         const bool kill_im = (m == 0) && (g & 1);      // Im(a_l0) is ignored
-        for (int lc = cfirst; lc <= lmax; lc += S_LC) {
-            mbar_wait(full + stage, phase);
-            const double* As = reinterpret_cast<const double*>(stage_base + (size_t)stage * S_STAGE_BYTES);
-            const double* Ls = As + S_ABYTES / 8;
-            // 8-ring row blocks whose recurrences all start after this stage hold lambda = 0: skipped
-            unsigned act = 0;
-            {
-                const int4 q0 = *reinterpret_cast<const int4*>(minls8), q1 = *reinterpret_cast<const int4*>(minls8 + 4);
+        // this lane's workspace cell of (ring pb + g, maps 4 (16 kt + 4 wn) + t .., half cls); + i: 8 rings, + j: 4 maps
+        const size_t kgs = (size_t)(lmax + 1) * d.ncomp * 2 * KG, ps = (size_t)d.nkg * kgs;
+        double2* Fl = reinterpret_cast<double2*>(F) + f_cell(d, g, kt * (KTILE_MAPS / KG) + wn * 4, m, comp, cls) + t;
+        for (int pbi = sp; pbi < npb; pbi += nsplit) {
+            const int pb = pbi * S_PB;
+            if (m >= d.mlim[min(pb + S_PB, nh) - 1]) continue;        // no ring of this block takes part in order m (never read)
+            const int cfirst = scf[pbi];
+            // smallest l_safe of every 8-ring row block
+            const int4 q0 = __ldg(reinterpret_cast<const int4*>(d.sminls8 + ((size_t)m * npb + pbi) * 8));
+            const int4 q1 = __ldg(reinterpret_cast<const int4*>(d.sminls8 + ((size_t)m * npb + pbi) * 8 + 4));
+            for (int lc = cfirst; lc <= lmax; lc += S_LC) {
+                mbar_wait(full + stage, phase);
+                const double* As = reinterpret_cast<const double*>(stage_base + (size_t)stage * S_STAGE_BYTES);
+                const double* Ls = As + S_ABYTES / 8;
+                // 8-ring row blocks whose recurrences all start after this stage hold lambda = 0: skipped
                 const int lend = lc + S_LC - 1;
-                act = (q0.x <= lend ? 1u : 0u) | (q0.y <= lend ? 2u : 0u) | (q0.z <= lend ? 4u : 0u) | (q0.w <= lend ? 8u : 0u) |
-                      (q1.x <= lend ? 16u : 0u) | (q1.y <= lend ? 32u : 0u) | (q1.z <= lend ? 64u : 0u) | (q1.w <= lend ? 128u : 0u);
-            }
-            if (act == 0xffu) {
+                const unsigned act = (q0.x <= lend ? 1u : 0u) | (q0.y <= lend ? 2u : 0u) | (q0.z <= lend ? 4u : 0u) | (q0.w <= lend ? 8u : 0u) |
+                                     (q1.x <= lend ? 16u : 0u) | (q1.y <= lend ? 32u : 0u) | (q1.z <= lend ? 64u : 0u) | (q1.w <= lend ? 128u : 0u);
+                if (act == 0xffu) {
 #pragma unroll
-                for (int ks = 0; ks < S_LC / 8; ++ks) {
-                    double a[8], b[4];
-                    const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
+                    for (int ks = 0; ks < S_LC / 8; ++ks) {
+                        double a[8], b[4];
+                        const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
+                        for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const int row = 16 * wn + 4 * j + (g >> 1);               // map inside the k-tile
-                        const double v = As[ks * 1024 + row * 16 + ((((2 * t + cls) ^ (row & 7)) << 1) | (g & 1))];
-                        b[j] = kill_im ? 0.0 : v;
+                        for (int j = 0; j < 4; ++j) {
+                            const int row = 16 * wn + 4 * j + (g >> 1);               // map inside the k-tile
+                            const double v = As[ks * 1024 + row * 16 + ((((2 * t + cls) ^ (row & 7)) << 1) | (g & 1))];
+                            b[j] = kill_im ? 0.0 : v;
+                        }
+#pragma unroll
+                        for (int i = 0; i < 8; ++i)
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
                     }
+                } else {
 #pragma unroll
-                    for (int i = 0; i < 8; ++i)
+                    for (int ks = 0; ks < S_LC / 8; ++ks) {
+                        double b[4];
+                        const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
-                }
-            } else {
+                        for (int j = 0; j < 4; ++j) {
+                            const int row = 16 * wn + 4 * j + (g >> 1);
+                            const double v = As[ks * 1024 + row * 16 + ((((2 * t + cls) ^ (row & 7)) << 1) | (g & 1))];
+                            b[j] = kill_im ? 0.0 : v;
+                        }
 #pragma unroll
-                for (int ks = 0; ks < S_LC / 8; ++ks) {
-                    double b[4];
-                    const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
+                        for (int i = 0; i < 8; ++i) {
+                            if (act & (1u << i)) {
+                                const double a = La[8 * i];
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        const int row = 16 * wn + 4 * j + (g >> 1);
-                        const double v = As[ks * 1024 + row * 16 + ((((2 * t + cls) ^ (row & 7)) << 1) | (g & 1))];
-                        b[j] = kill_im ? 0.0 : v;
-                    }
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        if (act & (1u << i)) {
-                            const double a = La[8 * i];
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a, b[j]);
+                                for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a, b[j]);
+                            }
                         }
                     }
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty + stage);
+                if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty + stage);
-            if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
-        }
-        // ---- epilogue: exchange Ee / Oo through smem, write north = Ee + Oo, south = Ee - Oo lines
-        named_bar_sync(2, LEG_CONSUMER_WARPS * 32);   // every consumer is done with the stage memory
-        double* Cs = reinterpret_cast<double*>(smem_raw);
+            // ---- epilogue: a lane holds (re, im) of (ring pb + 8 i + g, map 16 wn + 4 j + t): 64-byte runs per ring
+            double2* Fb = Fl + (size_t)pb * ps;
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+            for (int i = 0; i < 8; ++i) {
+                const bool inr = pb + 8 * i + g < nh;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int row = cls * S_PB + 8 * i + g;
-                const int col = wn * 32 + 8 * j + 2 * t;
-                *reinterpret_cast<double2*>(&Cs[row * S_SC + col]) = make_double2(c[i][j][0], c[i][j][1]);
+                for (int j = 0; j < 4; ++j) {
+                    if (inr) Fb[(size_t)(8 * i) * ps + (size_t)j * kgs] = make_double2(c[i][j][0], c[i][j][1]);
+                    c[i][j][0] = 0.0; c[i][j][1] = 0.0;
+                }
             }
-        named_bar_sync(2, LEG_CONSUMER_WARPS * 32);
-        double2* Fc = reinterpret_cast<double2*>(F);
-        for (int e = tid; e < S_PB * (NK / 2); e += LEG_CONSUMER_WARPS * 32) {
-            const int col2 = e % (NK / 2), r = e / (NK / 2);
-            const int p = pb + r;
-            if (p >= nh) continue;
-            const double2 ee = *reinterpret_cast<const double2*>(&Cs[r * S_SC + 2 * col2]);
-            const double2 oo = *reinterpret_cast<const double2*>(&Cs[(S_PB + r) * S_SC + 2 * col2]);
-            const int k = kt * KTILE_MAPS + col2;
-            double2* dst = Fc + f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
-            dst[0] = make_double2(ee.x + oo.x, ee.y + oo.y);
-            dst[KG] = make_double2(ee.x - oo.x, ee.y - oo.y);
         }
     } else {
-        // ===== lambda generators (warps 8..11): warp = (half of the block's 64 rings) + 2 (half of the stage's 32 l);
+        // ===== lambda generators (warps 0..3): warp = (half of the block's 64 rings) + 2 (half of the stage's 32 l);
         // the recurrence restarts from the plan's state table every 16 l, so the two l halves of a stage are generated
         // at the same time.  Lane 0 of generator 0 also issues the stage's TMA loads (a_lm, straight from the m-major
         // ABI layout).
@@ -502,101 +484,113 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
         if (lam) {
             // ===== staged mode: one thread streams, per stage, the a_lm boxes (TMA) and the lambda block (bulk copy)
             if (gw != 0 || lane != 0) return;
-            const size_t blk0 = (size_t)d.sblk_off[(size_t)m * d.npb + pbi];
             const int row0s = (k0 + kt * KTILE_MAPS) * d.ncomp + comp;
-            int stage = 0, n = 0; uint32_t phase = 0;
-            for (int lc = cfirst; lc <= lmax; lc += S_LC, ++n) {
-                mbar_wait(empty + stage, phase ^ 1);
-                unsigned char* As = stage_base + (size_t)stage * S_STAGE_BYTES;
-                mbar_arrive_expect_tx(full + stage, S_ABYTES + S_LBYTES);
+            int stage = 0; uint32_t phase = 0;
+            for (int pbi = sp; pbi < npb; pbi += nsplit) {
+                if (m >= d.mlim[min(pbi * S_PB + S_PB, nh) - 1]) continue;
+                const size_t blk0 = (size_t)d.sblk_off[(size_t)m * d.npb + pbi];
+                int n = 0;
+                for (int lc = scf[pbi]; lc <= lmax; lc += S_LC, ++n) {
+                    mbar_wait(empty + stage, phase ^ 1);
+                    unsigned char* As = stage_base + (size_t)stage * S_STAGE_BYTES;
+                    mbar_arrive_expect_tx(full + stage, S_ABYTES + S_LBYTES);
 #pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    tma_load_2d(As + q * (S_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0s);
-                bulk_load(As + S_ABYTES, lam + (blk0 + n) * (size_t)(S_LBYTES / 8), S_LBYTES, full + stage);
-                if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
+                    for (int q = 0; q < 4; ++q)
+                        tma_load_2d(As + q * (S_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0s);
+                    bulk_load(As + S_ABYTES, lam + (blk0 + n) * (size_t)(S_LBYTES / 8), S_LBYTES, full + stage);
+                    if (++stage == S_STAGES) { stage = 0; phase ^= 1; }
+                }
             }
             return;
         }
         const int gh = gw >> 1;
         const int rl = (gw & 1) * 32 + lane;
-        const int p = pb + rl;
-        double z = 0.0;
-        int ls = lmax + 1;
-        if (p < nh) { ls = d.lstart[(size_t)m * nh + p]; z = d.z[p]; }
         const double2* coefm = d.coef + ((long long)m * (2 * lmax + 1 - m) / 2);
-        const double2* csm = d.cseed + (size_t)d.csoff[m] * nh + (p < nh ? p : 0);
         constexpr int HL = S_LC / 2;                            // l per warp and stage
-        // Two stages are generated at a time, as two independent chains per lane (restarted from the state table): a
-        // dependent FP64 instruction waits behind the consumers' queued DMMAs for hundreds of cycles, so the latency
-        // of a step is shared by both chains.  (alpha, beta) and the start states of the next pair are fetched while
-        // the current pair is computed.
         double2* cfw = cfs + gw * (2 * HL);                     // this warp's coefficients of the two stages
         auto load_cf = [&](int lb) -> double2 {                 // lanes 0..15: first stage of the pair, 16..31: second
             const int l = lb + (lane & (HL - 1)) + (lane >> 4) * S_LC;
             return l <= lmax ? __ldg(coefm + l) : make_double2(0.0, 0.0);
         };
-        auto load_state = [&](int lb) -> double2 {
-            return (p < nh && lb <= lmax) ? __ldg(csm + (size_t)((lb - m) / LEG_CS) * nh) : make_double2(0.0, 0.0);
-        };
-        const int lb0 = cfirst + HL * gh;
-        double2 cf = load_cf(lb0), sda = load_state(lb0), sdb = load_state(lb0 + S_LC);
         int stage = 0; uint32_t phase = 0;
         const int row0 = (k0 + kt * KTILE_MAPS) * d.ncomp + comp;
-        for (int lc = cfirst; lc <= lmax; lc += 2 * S_LC) {
-            const int lb = lc + HL * gh;
-            const bool two = lc + S_LC <= lmax;                 // the pair's second stage exists
-            __syncwarp();                                       // everyone is done reading the previous coefficients
-            cfw[lane] = cf;
-            __syncwarp();
-            double xa1 = sda.x, xa2 = sda.y, xb1 = sdb.x, xb2 = sdb.y;
-            cf = load_cf(lb + 2 * S_LC); sda = load_state(lb + 2 * S_LC); sdb = load_state(lb + 3 * S_LC);
-            const int rsa = ls - lb, rsb = rsa - S_LC;
-            const int stb = stage + 1;                          // S_STAGES is even: a pair never wraps
-            mbar_wait(empty + stage, phase ^ 1);
-            if (two) mbar_wait(empty + stb, phase ^ 1);
-            unsigned char* Asa = stage_base + (size_t)stage * S_STAGE_BYTES;
-            unsigned char* Asb = Asa + S_STAGE_BYTES;
-            if (gw == 0 && lane == 0) {
-                mbar_arrive_expect_tx(full + stage, S_ABYTES);
-#pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    tma_load_2d(Asa + q * (S_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0);
-                if (two) {
-                    mbar_arrive_expect_tx(full + stb, S_ABYTES);
+        for (int pbi = sp; pbi < npb; pbi += nsplit) {
+            const int pb = pbi * S_PB;
+            if (m >= d.mlim[min(pb + S_PB, nh) - 1]) continue;
+            const int cfirst = scf[pbi];
+            const int p = pb + rl;
+            double z = 0.0;
+            int ls = lmax + 1;
+            if (p < nh) { ls = d.lstart[(size_t)m * nh + p]; z = d.z[p]; }
+            const double2* csm = d.cseed + (size_t)d.csoff[m] * nh + (p < nh ? p : 0);
+            auto load_state = [&](int lb) -> double2 {
+                return (p < nh && lb <= lmax) ? __ldg(csm + (size_t)((lb - m) / LEG_CS) * nh) : make_double2(0.0, 0.0);
+            };
+            // Two stages are generated at a time, as two independent chains per lane (restarted from the state table): a
+            // dependent FP64 instruction waits behind the consumers' queued DMMAs for hundreds of cycles, so the latency
+            // of a step is shared by both chains.  (alpha, beta) and the start states of the next pair are fetched while
+            // the current pair is computed.
+            const int lb0 = cfirst + HL * gh;
+            double2 cf = load_cf(lb0), sda = load_state(lb0), sdb = load_state(lb0 + S_LC);
+            for (int lc = cfirst; lc <= lmax; lc += 2 * S_LC) {
+                const int lb = lc + HL * gh;
+                const bool two = lc + S_LC <= lmax;             // the pair's second stage exists
+                __syncwarp();                                   // everyone is done reading the previous coefficients
+                cfw[lane] = cf;
+                __syncwarp();
+                double xa1 = sda.x, xa2 = sda.y, xb1 = sdb.x, xb2 = sdb.y;
+                cf = load_cf(lb + 2 * S_LC); sda = load_state(lb + 2 * S_LC); sdb = load_state(lb + 3 * S_LC);
+                const int rsa = ls - lb, rsb = rsa - S_LC;
+                // a block with an odd number of stages leaves the pairs of the next block on an odd stage: the second
+                // stage of a pair may be the wrapped one
+                const int stb = stage + 1 == S_STAGES ? 0 : stage + 1;
+                const uint32_t phb = stb == 0 ? phase ^ 1 : phase;
+                mbar_wait(empty + stage, phase ^ 1);
+                if (two) mbar_wait(empty + stb, phb ^ 1);
+                unsigned char* Asa = stage_base + (size_t)stage * S_STAGE_BYTES;
+                unsigned char* Asb = stage_base + (size_t)stb * S_STAGE_BYTES;
+                if (gw == 0 && lane == 0) {
+                    mbar_arrive_expect_tx(full + stage, S_ABYTES);
 #pragma unroll
                     for (int q = 0; q < 4; ++q)
-                        tma_load_2d(Asb + q * (S_ABYTES / 4), &tmA, full + stb, (int)(2 * (moff + lc + S_LC + 8 * q)), row0);
-                }
-            }
-            double* La = reinterpret_cast<double*>(Asa + S_ABYTES) + (HL * gh) * S_SL + rl;
-            double* Lb = reinterpret_cast<double*>(Asb + S_ABYTES) + (HL * gh) * S_SL + rl;
-            if (two) {
+                        tma_load_2d(Asa + q * (S_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), row0);
+                    if (two) {
+                        mbar_arrive_expect_tx(full + stb, S_ABYTES);
 #pragma unroll
-                for (int r = 0; r < HL; ++r) {
-                    const double2 aa = cfw[r], ab = cfw[HL + r];
-                    const double ta = fma(aa.x * z, xa1, -(aa.y * xa2));
-                    const double tb = fma(ab.x * z, xb1, -(ab.y * xb2));
-                    const bool ona = r >= rsa, onb = r >= rsb;
-                    xa2 = ona ? xa1 : xa2; xa1 = ona ? ta : xa1;
-                    xb2 = onb ? xb1 : xb2; xb1 = onb ? tb : xb1;
-                    La[r * S_SL] = ona ? ta : 0.0;
-                    Lb[r * S_SL] = onb ? tb : 0.0;
+                        for (int q = 0; q < 4; ++q)
+                            tma_load_2d(Asb + q * (S_ABYTES / 4), &tmA, full + stb, (int)(2 * (moff + lc + S_LC + 8 * q)), row0);
+                    }
                 }
-                mbar_arrive(full + stage);
-                mbar_arrive(full + stb);
-            } else {
+                double* La = reinterpret_cast<double*>(Asa + S_ABYTES) + (HL * gh) * S_SL + rl;
+                double* Lb = reinterpret_cast<double*>(Asb + S_ABYTES) + (HL * gh) * S_SL + rl;
+                if (two) {
 #pragma unroll
-                for (int r = 0; r < HL; ++r) {
-                    const double2 aa = cfw[r];
-                    const double ta = fma(aa.x * z, xa1, -(aa.y * xa2));
-                    const bool ona = r >= rsa;
-                    xa2 = ona ? xa1 : xa2; xa1 = ona ? ta : xa1;
-                    La[r * S_SL] = ona ? ta : 0.0;
+                    for (int r = 0; r < HL; ++r) {
+                        const double2 aa = cfw[r], ab = cfw[HL + r];
+                        const double ta = fma(aa.x * z, xa1, -(aa.y * xa2));
+                        const double tb = fma(ab.x * z, xb1, -(ab.y * xb2));
+                        const bool ona = r >= rsa, onb = r >= rsb;
+                        xa2 = ona ? xa1 : xa2; xa1 = ona ? ta : xa1;
+                        xb2 = onb ? xb1 : xb2; xb1 = onb ? tb : xb1;
+                        La[r * S_SL] = ona ? ta : 0.0;
+                        Lb[r * S_SL] = onb ? tb : 0.0;
+                    }
+                    mbar_arrive(full + stage);
+                    mbar_arrive(full + stb);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < HL; ++r) {
+                        const double2 aa = cfw[r];
+                        const double ta = fma(aa.x * z, xa1, -(aa.y * xa2));
+                        const bool ona = r >= rsa;
+                        xa2 = ona ? xa1 : xa2; xa1 = ona ? ta : xa1;
+                        La[r * S_SL] = ona ? ta : 0.0;
+                    }
+                    mbar_arrive(full + stage);
                 }
-                mbar_arrive(full + stage);
+                stage += two ? 2 : 1;
+                if (stage >= S_STAGES) { stage -= S_STAGES; phase ^= 1; }
             }
-            stage += 2;
-            if (stage == S_STAGES) { stage = 0; phase ^= 1; }
         }
     }
 }
@@ -672,7 +666,7 @@ cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d,
     if (d.spin == 2) return launch_legendre_synthesis_order_spin2(pl, d, tmA, F, kmaps, m, nm, st);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
-    k_legendre_synthesis<<<(unsigned)(nm * nkt * npb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m);
+    k_legendre_synthesis<<<(unsigned)(nm * nkt * npb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, npb);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -692,7 +686,7 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
         k_lambda_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
         pl->launches++;
     }
-    k_legendre_synthesis<<<(d.lmax + 1) * nkt * npb, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0);
+    k_legendre_synthesis<<<(d.lmax + 1) * nkt, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, 1);
     pl->launches++;
     return cudaGetLastError();
 }

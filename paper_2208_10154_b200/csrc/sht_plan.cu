@@ -517,7 +517,7 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
         {
             d.npb = (d.nh + 63) / 64;
             std::vector<int> aoff((size_t)(lmax + 1) * d.ntile_max, 0), soff((size_t)(lmax + 1) * d.npb, 0),
-                scf((size_t)(lmax + 1) * d.npb, lmax + 1);
+                scf((size_t)(lmax + 1) * d.npb, lmax + 1), sm8((size_t)(lmax + 1) * d.npb * 8, lmax + 1);
             long long na = 0, nsb = 0;
             d.nck_max = 0; d.nst_max = 0;
             for (int m = 0; m <= lmax; ++m) {
@@ -535,7 +535,12 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
                     const int plast = (b * 64 + 64 < d.nh ? b * 64 + 64 : d.nh) - 1;
                     if (m >= mlim[plast]) continue;
                     int lmin = lmax + 1;
-                    for (int p = b * 64; p <= plast; ++p) lmin = hls[(size_t)m * d.nh + p] < lmin ? hls[(size_t)m * d.nh + p] : lmin;
+                    for (int p = b * 64; p <= plast; ++p) {
+                        const int lsv = hls[(size_t)m * d.nh + p];
+                        lmin = lsv < lmin ? lsv : lmin;
+                        int& q = sm8[((size_t)m * d.npb + b) * 8 + (p - b * 64) / 8];
+                        q = lsv < q ? lsv : q;
+                    }
                     if (lmin > lmax) continue;
                     const int cf = m + ((lmin - m) / 32) * 32;
                     scf[(size_t)m * d.npb + b] = cf;
@@ -547,7 +552,10 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             pl->n_ablk = na; pl->n_sblk = nsb;
             if (na > 0x7fffffffLL || nsb > 0x7fffffffLL) { sht_plan_destroy(pl); return SHT_ERR_UNSUPPORTED; }
             if (upload(pl, aoff, &d.ablk_off) != cudaSuccess || upload(pl, soff, &d.sblk_off) != cudaSuccess ||
-                upload(pl, scf, &d.scfirst) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+                upload(pl, scf, &d.scfirst) != cudaSuccess || upload(pl, sm8, &d.sminls8) != cudaSuccess) {
+                sht_plan_destroy(pl);
+                return SHT_ERR_ALLOC;
+            }
         }
         if ((ce = upload(pl, rings, &d.rings)) != cudaSuccess || (ce = upload(pl, mlim, &d.mlim)) != cudaSuccess) {
             sht_plan_destroy(pl);
