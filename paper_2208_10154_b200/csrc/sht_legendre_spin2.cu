@@ -37,7 +37,6 @@ constexpr int S2_ABYTES = S2_LC * 2 * P_KT * 16;            // a_E, a_B of a sta
 constexpr int S2_LBYTES = 2 * S2_LC * S2_SL * 8;            // [sign][l][ring]
 constexpr int S2_STAGE_BYTES = S2_ABYTES + S2_LBYTES;
 static_assert(S2_STAGE_BYTES % 1024 == 0, "stages must keep the 1024-byte alignment of the swizzled TMA boxes");
-constexpr int S2_SC = 128 + 8;                  // epilogue staging row stride (doubles)
 
 // per-l constants of F+/F- for order m: tp = (t1, t2) = N_l (l - m^2, l(l-1)/2), tm = (t4, 0) = N_l (l-1, 0),
 // t3 = N_l c_lm; all zero for l < 2 (reading G13) and beyond lmax
@@ -382,7 +381,7 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
 template <int WHICH, bool ORD = false>
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
-                           int nkt, int npb, const double* __restrict__ lam, int m0)
+                           int nkt, int npb, const double* __restrict__ lam, int m0, int nsplit)
 {
     constexpr int NST = 3;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -390,30 +389,24 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + NST * S2_STAGE_BYTES);
     uint64_t* empty = full + 4;
     double2* cfs = reinterpret_cast<double2*>(empty + 4);       // 4 generator warps x 2 buffers x S2_LC x (ab, uv, t3)
-    int* lmin_s = reinterpret_cast<int*>(cfs + 4 * 2 * S2_LC * 3);
 
+    // the CTA walks its share of the ring blocks of (m, k-tile) back to back, the pipeline running across them (see the
+    // spin-0 kernel): whole transforms nsplit = 1, the one-order launches of Alg. 3 one block per CTA
     const int kt = blockIdx.x % nkt;
-    const int pbi = (blockIdx.x / nkt) % npb;
+    const int sp = (blockIdx.x / nkt) % nsplit;
     // ORD: a few orders at a time from m0 (Alg. 3); a separate instantiation keeps the whole-transform kernel's registers
-    const int m = (ORD ? m0 : 0) + blockIdx.x / (nkt * npb);
-    const int pb = pbi * S2_PB;
+    const int m = (ORD ? m0 : 0) + blockIdx.x / (nkt * nsplit);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lmax = d.lmax, nh = d.nh;
-    const int plast = min(pb + S2_PB, nh) - 1;
-    if (m >= d.mlim[plast]) return;                    // no ring of this block takes part in order m (never read)
 
     if (tid == 0) {
         for (int s = 0; s < NST; ++s) { mbar_init(full + s, lam ? 1 : 1 + 128); mbar_init(empty + s, LEG_CONSUMER_WARPS_S2); }
         fence_barrier_init();
         tma_prefetch_desc(&tmA);
-        *lmin_s = lmax + 1;
     }
     __syncthreads();
-    if (tid < S2_PB && pb + tid < nh) atomicMin(lmin_s, d.lstart[(size_t)m * nh + pb + tid]);
-    __syncthreads();
-    const int lmin = *lmin_s;
-    const int cfirst = (lmin > lmax) ? (lmax + 1) : m + ((lmin - m) / S2_LC) * S2_LC;
     const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
+    const int* scf = d.scfirst + (size_t)m * npb;
 
     if (warp < 8) {
         // ===== consumers: warp (par, wn): rows = 64 rings of the even (par 0) / odd (par 1) fold part, 8 pairs =====
@@ -439,7 +432,13 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
             ab0[j] = pr * 16 + (((2 * t + par) ^ (pr & 7)) << 1);
             ab1[j] = pr * 16 + (((2 * t + (par ^ 1)) ^ (pr & 7)) << 1);
         }
-        for (int lc = cfirst; lc <= lmax; lc += S2_LC) {
+        // this lane's workspace cell of (ring g, pairs 4 (8 kt + 2 wn) + t .., Q, fold part par); + i: 8 rings, + j: 4 pairs
+        const size_t kgs = (size_t)(lmax + 1) * 2 * 2 * KG, ps = (size_t)d.nkg * kgs;
+        double2* Fl = reinterpret_cast<double2*>(F) + f_cell(d, g, kt * P_KG + wn * 2, m, 0, par) + t;
+        for (int pbi = sp; pbi < npb; pbi += nsplit) {
+        const int pb = pbi * S2_PB;
+        if (m >= d.mlim[min(pb + S2_PB, nh) - 1]) continue;       // no ring of this block takes part in order m (never read)
+        for (int lc = scf[pbi]; lc <= lmax; lc += S2_LC) {
             mbar_wait(full + stage, phase);
             const double* As = reinterpret_cast<const double*>(stage_base + (size_t)stage * S2_STAGE_BYTES);
             const double* Ls = As + S2_ABYTES / 8;
@@ -483,30 +482,22 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
             if (lane == 0) mbar_arrive(empty + stage);
             if (++stage == NST) { stage = 0; phase ^= 1; }
         }
-        // ---- epilogue: exchange the even / odd fold parts through smem, write north = e + o, south = e - o lines
-        named_bar_sync(2, 256);                           // every consumer is done with the stage memory
-        double* Cs = reinterpret_cast<double*>(smem_raw);
+        // ---- epilogue: the even (par 0) / odd (par 1) fold parts go straight from the accumulators into the two halves of
+        // the workspace lines of Q and iU; north = e + o, south = e - o are formed by the ring kernels on load
+        double2* Fb = Fl + (size_t)pb * ps;
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+        for (int i = 0; i < 8; ++i) {
+            const bool inr = pb + 8 * i + g < nh;
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
-                const int row = par * S2_PB + 8 * i + g;
-                const int col = 2 * (8 * wn + 4 * j + t);                       // (pair, re/im) of component Q
-                *reinterpret_cast<double2*>(&Cs[row * S2_SC + col]) = make_double2(cQ[i][j][0], cQ[i][j][1]);
-                *reinterpret_cast<double2*>(&Cs[row * S2_SC + 2 * P_KT + col]) = make_double2(cU[i][j][0], cU[i][j][1]);
+                if (inr) {
+                    double2* dst = Fb + (size_t)(8 * i) * ps + (size_t)j * kgs;
+                    dst[0] = make_double2(cQ[i][j][0], cQ[i][j][1]);
+                    dst[2 * KG] = make_double2(cU[i][j][0], cU[i][j][1]);
+                }
+                cQ[i][j][0] = cQ[i][j][1] = 0.0; cU[i][j][0] = cU[i][j][1] = 0.0;
             }
-        named_bar_sync(2, 256);
-        double2* Fc = reinterpret_cast<double2*>(F);
-        for (int e = tid; e < S2_PB * 2 * P_KT; e += 256) {
-            const int pr = e % P_KT, comp = (e / P_KT) & 1, r = e / (2 * P_KT);
-            const int p = pb + r;
-            if (p >= nh) continue;
-            const double2 ev = *reinterpret_cast<const double2*>(&Cs[r * S2_SC + comp * 2 * P_KT + 2 * pr]);
-            const double2 od = *reinterpret_cast<const double2*>(&Cs[(S2_PB + r) * S2_SC + comp * 2 * P_KT + 2 * pr]);
-            const int k = kt * P_KT + pr;
-            double2* dst = Fc + f_cell(d, p, k >> 2, m, comp, 0) + (k & 3);
-            dst[0] = make_double2(ev.x + od.x, ev.y + od.y);
-            dst[KG] = make_double2(ev.x - od.x, ev.y - od.y);
+        }
         }
     } else {
         // ===== generators (warps 8..11): warp = (half of the 64 rings) + 2 (half of the stage's 32 l); a lane forms F+
@@ -516,22 +507,32 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
         if (lam) {
             // ===== staged mode: one thread streams, per stage, the a_E / a_B boxes (TMA) and the F+/F- block (bulk copy)
             if (gw != 0 || lane != 0) return;
-            const size_t blk0 = (size_t)d.sblk_off[(size_t)m * d.npb + pbi];
-            int stage = 0, n = 0; uint32_t phase = 0;
-            for (int lc = cfirst; lc <= lmax; lc += S2_LC, ++n) {
-                mbar_wait(empty + stage, phase ^ 1);
-                unsigned char* As = stage_base + (size_t)stage * S2_STAGE_BYTES;
-                mbar_arrive_expect_tx(full + stage, S2_ABYTES + S2_LBYTES);
+            int stage = 0; uint32_t phase = 0;
+            for (int pbi = sp; pbi < npb; pbi += nsplit) {
+                if (m >= d.mlim[min(pbi * S2_PB + S2_PB, nh) - 1]) continue;
+                const size_t blk0 = (size_t)d.sblk_off[(size_t)m * d.npb + pbi];
+                int n = 0;
+                for (int lc = scf[pbi]; lc <= lmax; lc += S2_LC, ++n) {
+                    mbar_wait(empty + stage, phase ^ 1);
+                    unsigned char* As = stage_base + (size_t)stage * S2_STAGE_BYTES;
+                    mbar_arrive_expect_tx(full + stage, S2_ABYTES + S2_LBYTES);
 #pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    tma_load_3d(As + q * (S2_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), k0 + kt * P_KT, 0);
-                bulk_load(As + S2_ABYTES, lam + (blk0 + n) * (size_t)(S2_LBYTES / 8), S2_LBYTES, full + stage);
-                if (++stage == NST) { stage = 0; phase ^= 1; }
+                    for (int q = 0; q < 4; ++q)
+                        tma_load_3d(As + q * (S2_ABYTES / 4), &tmA, full + stage, (int)(2 * (moff + lc + 8 * q)), k0 + kt * P_KT, 0);
+                    bulk_load(As + S2_ABYTES, lam + (blk0 + n) * (size_t)(S2_LBYTES / 8), S2_LBYTES, full + stage);
+                    if (++stage == NST) { stage = 0; phase ^= 1; }
+                }
             }
             return;
         }
         const int gh = gw >> 1;
         const int rl = (gw & 1) * 32 + lane;
+        int stage = 0, buf = 0; uint32_t phase = 0;
+        const int row0 = k0 + kt * P_KT;
+        for (int pbi = sp; pbi < npb; pbi += nsplit) {
+        const int pb = pbi * S2_PB;
+        if (m >= d.mlim[min(pb + S2_PB, nh) - 1]) continue;
+        const int cfirst = scf[pbi];
         const int p = pb + rl;
         double z = 0.0, is2 = 0.0;
         int ls = lmax + 1;
@@ -553,8 +554,6 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
         };
         load_consts(cfirst + HL * gh);
         double2 sd = load_state(cfirst + HL * gh);
-        int stage = 0, buf = 0; uint32_t phase = 0;
-        const int row0 = k0 + kt * P_KT;
         for (int lc = cfirst; lc <= lmax; lc += S2_LC) {
             const int lb = lc + HL * gh;
             double2* cb = cfw + buf * (HL * 3);
@@ -590,6 +589,7 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
             mbar_arrive(full + stage);
             buf ^= 1;
             if (++stage == NST) { stage = 0; phase ^= 1; }
+        }
         }
     }
 }
@@ -653,7 +653,7 @@ cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d,
         k_fpm_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
         pl->launches++;
     }
-    kern<<<(d.lmax + 1) * nkt * npb, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0);
+    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, 1);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -684,7 +684,7 @@ cudaError_t launch_legendre_synthesis_order_spin2(sht_plan_s* pl, const DevicePl
 {
     const int nkt = (kmaps + P_KT - 1) / P_KT;
     const int npb = (d.nh + S2_PB - 1) / S2_PB;
-    k_legendre_synthesis_spin2<0, true><<<(unsigned)(nm * nkt * npb), LEG2_THREADS, synthesis2_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m);
+    k_legendre_synthesis_spin2<0, true><<<(unsigned)(nm * nkt * npb), LEG2_THREADS, synthesis2_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, npb);
     pl->launches++;
     return cudaGetLastError();
 }

@@ -821,8 +821,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const in
     const bool blue = rp.lc > 0;
     const double2* chirp = d.tw + rp.hf_off + rp.lc;      // c_j = exp(-i pi j^2 / N), j < N (Bluestein rings)
     const int mlim = rp.mlim;
-    // the spin-0 Legendre synthesis stores the even and the odd sum of a ring pair: north = even + odd, south = even - odd
-    const bool eo = d.spin == 0;
+    // the Legendre synthesis stores the even and the odd sum of a ring pair: north = even + odd, south = even - odd
     double2* cur = smem;
 
     // ring spectrum of the packed sequence, Z[b] = Y_north[b] + i Y_south[b]; bins b <= N/2 are assembled
@@ -847,7 +846,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_synthesis(DevicePlan d, const in
                         double2 ph = make_double2(1.0, 0.0);
                         if (rp.shift) { ph = __ldg(tw2 + m2); ph.y = -ph.y; }
                         double2 fn = Fp[0], fs = Fp[KG];
-                        if (eo) { const double2 e = fn, o = fs; fn = cadd(e, o); fs = csub(e, o); }
+                        { const double2 e = fn, o = fs; fn = cadd(e, o); fs = csub(e, o); }       // stored as (even, odd) sums
                         if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }   // U = -i (iU)
                         double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
                         if (pass == 1) { dn.y = -dn.y; ds.y = -ds.y; }
@@ -936,7 +935,6 @@ __global__ void __launch_bounds__(NT, 1) k_ring_residual(DevicePlan d, const int
     const double2* tw2 = d.tw + rp.tw_off;
     const bool equator = rp.start_s < 0;
     const int mlim = rp.mlim, nb = N / 2 + 1;
-    const bool eo = d.spin == 0;                          // synthesised T_m stored as (even, odd) sums (spin 0) or (north, south)
     double2* Yn = smem;                                   // [b][kk]
     double2* Ys = smem + ((size_t)nb << ktsh);
     const int kk = tid & (kt - 1), k = kbase + kk;
@@ -958,7 +956,7 @@ __global__ void __launch_bounds__(NT, 1) k_ring_residual(DevicePlan d, const int
                     double2 ph = make_double2(1.0, 0.0);
                     if (rp.shift) { ph = __ldg(tw2 + m2); ph.y = -ph.y; }
                     double2 fn = Fp[0], fs = Fp[KG];
-                    if (eo) { const double2 e = fn, o = fs; fn = cadd(e, o); fs = csub(e, o); }
+                    { const double2 e = fn, o = fs; fn = cadd(e, o); fs = csub(e, o); }       // stored as (even, odd) sums
                     if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }
                     double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
                     if (pass == 1) { dn.y = -dn.y; ds.y = -ds.y; }
@@ -1033,7 +1031,7 @@ __global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* _
     const size_t cell0 = f_cell(d, p, k >> 2, 0, comp, 0) + (k & 3);
     const double2* Sp = reinterpret_cast<const double2*>(S) + cell0 + (size_t)m * cstride;
     double2 fn = Sp[0], fs = Sp[KG];
-    if (d.spin == 0) { const double2 e = fn, o = fs; fn = cadd(e, o); fs = csub(e, o); }      // stored as (even, odd) sums
+    { const double2 e = fn, o = fs; fn = cadd(e, o); fs = csub(e, o); }       // stored as (even, odd) sums
     if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }
     double2 ph = make_double2(1.0, 0.0);
     if (shift) { ph = __ldg(tw2 + m % (2 * N)); ph.y = -ph.y; }
