@@ -45,6 +45,19 @@ constexpr int S_STAGE_BYTES = (S_ABYTES + S_LBYTES + 1023) / 1024 * 1024;
 // ------------------------------------------------------------------------------------------------
 static_assert(LAM_ABLK_BYTES == (size_t)A_LBYTES && LAM_SBLK_BYTES == (size_t)S_LBYTES, "block sizes");
 
+// Rows of a lambda tile below the smallest l_safe of a group of 8 rings hold zeros for those rings: the consumers skip their
+// 16-row blocks.  One nibble per group of 8 lanes (= rings of the chunk): the first 16-row block (0..8) with a started
+// recurrence; called by a full warp with its lanes' l_safe.
+__device__ __forceinline__ int pack_i0(int ls, int l0)
+{
+    int lsmin = ls;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) lsmin = min(lsmin, __shfl_xor_sync(0xffffffffu, lsmin, o));
+    const int v = max(0, min(8, (lsmin - l0) >> 4));
+    return __shfl_sync(0xffffffffu, v, 0) | (__shfl_sync(0xffffffffu, v, 8) << 4) | (__shfl_sync(0xffffffffu, v, 16) << 8) |
+           (__shfl_sync(0xffffffffu, v, 24) << 12);
+}
+
 // analysis block (m, l tile, chunk of 32 rings): [class][ring][A_SL]; 128 threads: warp = 32 l rows, lane = ring
 __global__ void __launch_bounds__(128) k_lambda_blocks_analysis(DevicePlan d, double* __restrict__ lam, int* __restrict__ i0tab)
 {
@@ -82,11 +95,9 @@ __global__ void __launch_bounds__(128) k_lambda_blocks_analysis(DevicePlan d, do
         const int rr = 32 * w + r;
         tile[(rr & 1) * (A_PC * A_SL) + lane * A_SL + (rr >> 1)] = on ? tv : 0.0;
     }
-    if (w == 0) {                                           // first 16-row block with a started recurrence
-        int lsmin = ls;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) lsmin = min(lsmin, __shfl_xor_sync(0xffffffffu, lsmin, o));
-        if (lane == 0) i0tab[blk] = max(0, min(8, (lsmin - l0) >> 4));
+    if (w == 0) {                                           // per 8 rings: first 16-row block with a started recurrence
+        const int pk = pack_i0(ls, l0);
+        if (lane == 0) i0tab[blk] = pk;
     }
     __syncthreads();
     double2* dst = reinterpret_cast<double2*>(lam + blk * (size_t)(A_LBYTES / 8));
@@ -180,13 +191,14 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
         const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
         for (int tile = tb; tile < te; ++tile) {
             const int l0 = m + tile * A_ML;
+            const int i1 = min(8, (lmax - l0) / 16 + 1);        // 16-row blocks of the tile that reach down to l <= lmax
             for (int pc = pst[tile]; pc < nh; pc += A_PC) {
                 mbar_wait(full + stage, phase);
                 const double* Xs = reinterpret_cast<const double*>(stage_base + (size_t)stage * A_STAGE_BYTES);
                 const double* Ls = Xs + A_XBYTES / 8 + cls * (A_PC * A_SL);
-                // rows below the chunk's smallest l_safe hold lambda = 0: their 16-row blocks (i < i0) are skipped
-                const int i0 = i0s[stage];
-                if (i0 == 0) {
+                // rows below the smallest l_safe of 8 rings hold lambda = 0 for them: their 16-row blocks (i < i0) are skipped
+                const int i0p = i0s[stage];
+                if (i0p == 0 && i1 == 8) {
 #pragma unroll
                     for (int ks = 0; ks < A_PC / 4; ++ks) {
                         const int sub = ks >> 2, ksl = ks & 3;
@@ -208,6 +220,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                     for (int ks = 0; ks < A_PC / 4; ++ks) {
                         const int sub = ks >> 2, ksl = ks & 3;
                         const int pl = 8 * (ksl >> 1) + 2 * t + (ksl & 1);
+                        const int i0 = (i0p >> (4 * (2 * sub + (ksl >> 1)))) & 15;       // the 8 rings this step draws from
                         double b[4];
                         const double* La = Ls + (16 * sub + pl) * A_SL + g;
                         const double* Xb = Xs + sub * 4096 + pl * 16 + ((((4 * cls + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
@@ -215,7 +228,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                         for (int j = 0; j < 4; ++j) b[j] = Xb[(4 * wn + j) * 256];
 #pragma unroll
                         for (int i = 0; i < 8; ++i) {
-                            if (i >= i0) {
+                            if (i >= i0 && i < i1) {
                                 const double a = La[8 * i];
 #pragma unroll
                                 for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a, b[j]);
@@ -319,13 +332,11 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                     }
                 }
                 const int rs = ls - lh;                             // first row of the half with a started recurrence
-                int lsmin = ls;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) lsmin = min(lsmin, __shfl_xor_sync(0xffffffffu, lsmin, o));
+                const int i0pk = pack_i0(ls, l0);
                 mbar_wait(empty + stage, phase ^ 1);
                 unsigned char* Xs = stage_base + (size_t)stage * A_STAGE_BYTES;
                 if (gh == 0 && lane == 0) {
-                    i0s[stage] = max(0, min(8, (lsmin - l0) >> 4));
+                    i0s[stage] = i0pk;
                     mbar_arrive_expect_tx(full + stage, A_XBYTES);
                     tma_load_4d(Xs, &tmF, full + stage, 0, pc, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
                     tma_load_4d(Xs + A_XBYTES / 2, &tmF, full + stage, 0, pc + 16, kt * (KTILE_MAPS / KG), m * d.ncomp + comp);
@@ -417,10 +428,12 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
                 const double* As = reinterpret_cast<const double*>(stage_base + (size_t)stage * S_STAGE_BYTES);
                 const double* Ls = As + S_ABYTES / 8;
                 // 8-ring row blocks whose recurrences all start after this stage hold lambda = 0: skipped
-                const int lend = lc + S_LC - 1;
-                const unsigned act = (q0.x <= lend ? 1u : 0u) | (q0.y <= lend ? 2u : 0u) | (q0.z <= lend ? 4u : 0u) | (q0.w <= lend ? 8u : 0u) |
-                                     (q1.x <= lend ? 16u : 0u) | (q1.y <= lend ? 32u : 0u) | (q1.z <= lend ? 64u : 0u) | (q1.w <= lend ? 128u : 0u);
-                if (act == 0xffu) {
+                auto active = [&](int lend) -> unsigned {
+                    return (q0.x <= lend ? 1u : 0u) | (q0.y <= lend ? 2u : 0u) | (q0.z <= lend ? 4u : 0u) | (q0.w <= lend ? 8u : 0u) |
+                           (q1.x <= lend ? 16u : 0u) | (q1.y <= lend ? 32u : 0u) | (q1.z <= lend ? 64u : 0u) | (q1.w <= lend ? 128u : 0u);
+                };
+                const int ks1 = min(S_LC / 8, (lmax - lc) / 8 + 1);          // steps of 8 l that reach down to l <= lmax
+                if (active(lc + 7) == 0xffu && ks1 == S_LC / 8) {  // every recurrence has started by the first 8 l of the stage
 #pragma unroll
                     for (int ks = 0; ks < S_LC / 8; ++ks) {
                         double a[8], b[4];
@@ -441,6 +454,8 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
                 } else {
 #pragma unroll
                     for (int ks = 0; ks < S_LC / 8; ++ks) {
+                        if (ks >= ks1) break;
+                        const unsigned act = active(lc + 8 * ks + 7);               // the step's 8 l: lc + 8 ks ..
                         double b[4];
                         const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
 #pragma unroll
