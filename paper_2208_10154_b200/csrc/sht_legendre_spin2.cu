@@ -15,6 +15,7 @@
 // Same warp-specialised structure as the spin-0 kernels: 8 DMMA consumer warps (CTA tile 128 x 128 real outputs), but
 // the four remaining warps all generate (lane = ring x sign of F), and lane 0 of the generator that owns a stage
 // also issues its TMA loads.
+#include <type_traits>
 #include "sht_legendre_common.cuh"
 
 namespace sht {
@@ -217,10 +218,14 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
         const size_t moff = (size_t)((long long)m * (2 * lmax + 1 - m) / 2);
         for (int tile = tb; tile < te; ++tile) {
             const int l0 = m + tile * A2_ML;
+            const int i1 = min(8, (lmax - l0) / 16 + 1);        // 16-row blocks of the tile that reach down to l <= lmax
             for (int pc = pst[tile]; pc < nh; pc += A2_PC) {
                 mbar_wait(full + stage, phase);
                 const double* Xs = reinterpret_cast<const double*>(stage_base + (size_t)stage * A2_STAGE_BYTES);
                 const double* Ls = Xs + A2_XBYTES / 8;
+                // 16-row blocks of the last tile past lmax are skipped (TAIL); the other tiles run the plain loop
+                auto contract = [&](auto tail_tag) {
+                constexpr bool TAIL = decltype(tail_tag)::value;
 #pragma unroll
                 for (int ks = 0; ks < A2_PC / 4; ++ks) {
                     const int pl = 8 * (ks >> 1) + 2 * t + (ks & 1);          // ring inside the 16-ring box
@@ -239,14 +244,19 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                             bu[j] = Xb[(P_KG + 2 * wn + j) * 256];
                         }
 #pragma unroll
-                        for (int i = 0; i < 8; ++i)
+                        for (int i = 0; i < 8; ++i) {
+                            if (!TAIL || i < i1) {
 #pragma unroll
-                            for (int j = 0; j < 2; ++j) {
-                                if (WHICH != 2) dmma884(cE[i][j][0], cE[i][j][1], a[i], sg ? bu[j] : bq[j]);
-                                if (WHICH != 1) dmma884(cB[i][j][0], cB[i][j][1], a[i], sg ? bq[j] : bu[j]);
+                                for (int j = 0; j < 2; ++j) {
+                                    if (WHICH != 2) dmma884(cE[i][j][0], cE[i][j][1], a[i], sg ? bu[j] : bq[j]);
+                                    if (WHICH != 1) dmma884(cB[i][j][0], cB[i][j][1], a[i], sg ? bq[j] : bu[j]);
+                                }
                             }
+                        }
                     }
                 }
+                };
+                if (i1 == 8) contract(std::false_type{}); else contract(std::true_type{});
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty + stage);
                 if (++stage == nst) { stage = 0; phase ^= 1; }
@@ -443,8 +453,10 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
             const double* As = reinterpret_cast<const double*>(stage_base + (size_t)stage * S2_STAGE_BYTES);
             const double* Ls = As + S2_ABYTES / 8;
             const int lrow = lc + 2 * t - 2;                // (l - 2) of this lane's first row of box 0, without the class bit
+            const int ks1 = min(S2_LC / 4, 2 * ((lmax - lc) / 8 + 1));          // boxes of 8 l that reach down to l <= lmax
 #pragma unroll
             for (int ks = 0; ks < S2_LC / 4; ++ks) {
+                if (ks >= ks1) break;
                 // box q of 8 l; sg = 0: the 4 l whose class matches this warp's fold part (F+), sg = 1: the others (F-)
                 const int q = ks >> 1, sg = ks & 1;
                 double a[8], be[2], bb[2];
