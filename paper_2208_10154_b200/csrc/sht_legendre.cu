@@ -13,6 +13,7 @@
 // warps run the three-term recurrence from the plan's l_safe(m,p) (item 11)
 // into the same stages.  The lambda tile and the operand tile of a stage are released together by the consumers.
 // Rings whose lambda is below threshold for a whole tile are skipped (ring optimisation, item 10, :229).
+#include <type_traits>
 #include <cstdio>
 #include "sht_legendre_common.cuh"
 
@@ -198,23 +199,32 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                 const double* Ls = Xs + A_XBYTES / 8 + cls * (A_PC * A_SL);
                 // rows below the smallest l_safe of 8 rings hold lambda = 0 for them: their 16-row blocks (i < i0) are skipped
                 const int i0p = i0s[stage];
-                if (i0p == 0 && i1 == 8) {
+                if (i0p == 0) {
+                    // plain loop over the first NI 16-row blocks (NI = 8 except in the last tile, whose blocks past lmax
+                    // are left out in steps of two: a block-by-block test costs more than the blocks it saves)
+                    auto contract = [&](auto ni_tag) {
+                        constexpr int NI = decltype(ni_tag)::value;
 #pragma unroll
-                    for (int ks = 0; ks < A_PC / 4; ++ks) {
-                        const int sub = ks >> 2, ksl = ks & 3;
-                        const int pl = 8 * (ksl >> 1) + 2 * t + (ksl & 1);        // ring inside the 16-ring box
-                        double a[8], b[4];
-                        const double* La = Ls + (16 * sub + pl) * A_SL + g;
+                        for (int ks = 0; ks < A_PC / 4; ++ks) {
+                            const int sub = ks >> 2, ksl = ks & 3;
+                            const int pl = 8 * (ksl >> 1) + 2 * t + (ksl & 1);        // ring inside the 16-ring box
+                            double a[NI], b[4];
+                            const double* La = Ls + (16 * sub + pl) * A_SL + g;
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
-                        const double* Xb = Xs + sub * 4096 + pl * 16 + ((((4 * cls + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
+                            for (int i = 0; i < NI; ++i) a[i] = La[8 * i];
+                            const double* Xb = Xs + sub * 4096 + pl * 16 + ((((4 * cls + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) b[j] = Xb[(4 * wn + j) * 256];
+                            for (int j = 0; j < 4; ++j) b[j] = Xb[(4 * wn + j) * 256];
 #pragma unroll
-                        for (int i = 0; i < 8; ++i)
+                            for (int i = 0; i < NI; ++i)
 #pragma unroll
-                            for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
-                    }
+                                for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
+                        }
+                    };
+                    if (i1 > 6) contract(std::integral_constant<int, 8>{});
+                    else if (i1 > 4) contract(std::integral_constant<int, 6>{});
+                    else if (i1 > 2) contract(std::integral_constant<int, 4>{});
+                    else contract(std::integral_constant<int, 2>{});
                 } else {
 #pragma unroll
                     for (int ks = 0; ks < A_PC / 4; ++ks) {

@@ -223,9 +223,9 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                 mbar_wait(full + stage, phase);
                 const double* Xs = reinterpret_cast<const double*>(stage_base + (size_t)stage * A2_STAGE_BYTES);
                 const double* Ls = Xs + A2_XBYTES / 8;
-                // 16-row blocks of the last tile past lmax are skipped (TAIL); the other tiles run the plain loop
-                auto contract = [&](auto tail_tag) {
-                constexpr bool TAIL = decltype(tail_tag)::value;
+                // the first NI 16-row blocks: 8 except in the last tile, whose blocks past lmax are left out in steps of two
+                auto contract = [&](auto ni_tag) {
+                constexpr int NI = decltype(ni_tag)::value;
 #pragma unroll
                 for (int ks = 0; ks < A2_PC / 4; ++ks) {
                     const int pl = 8 * (ks >> 1) + 2 * t + (ks & 1);          // ring inside the 16-ring box
@@ -233,10 +233,10 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                     for (int sg = 0; sg < 2; ++sg) {
                         // sg = 0: F+ with the fold of this class; sg = 1: F- with the other fold and swapped components
                         const int h = cls ^ sg;
-                        double a[8], bq[2], bu[2];
+                        double a[NI], bq[2], bu[2];
                         const double* La = Ls + ((sg * 2 + cls) * A2_PC + pl) * A2_SL + g;
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) a[i] = La[8 * i];
+                        for (int i = 0; i < NI; ++i) a[i] = La[8 * i];
                         const double* Xb = Xs + pl * 16 + ((((4 * h + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
 #pragma unroll
                         for (int j = 0; j < 2; ++j) {
@@ -244,19 +244,19 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                             bu[j] = Xb[(P_KG + 2 * wn + j) * 256];
                         }
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            if (!TAIL || i < i1) {
+                        for (int i = 0; i < NI; ++i)
 #pragma unroll
-                                for (int j = 0; j < 2; ++j) {
-                                    if (WHICH != 2) dmma884(cE[i][j][0], cE[i][j][1], a[i], sg ? bu[j] : bq[j]);
-                                    if (WHICH != 1) dmma884(cB[i][j][0], cB[i][j][1], a[i], sg ? bq[j] : bu[j]);
-                                }
+                            for (int j = 0; j < 2; ++j) {
+                                if (WHICH != 2) dmma884(cE[i][j][0], cE[i][j][1], a[i], sg ? bu[j] : bq[j]);
+                                if (WHICH != 1) dmma884(cB[i][j][0], cB[i][j][1], a[i], sg ? bq[j] : bu[j]);
                             }
-                        }
                     }
                 }
                 };
-                if (i1 == 8) contract(std::false_type{}); else contract(std::true_type{});
+                if (i1 > 6) contract(std::integral_constant<int, 8>{});
+                else if (i1 > 4) contract(std::integral_constant<int, 6>{});
+                else if (i1 > 2) contract(std::integral_constant<int, 4>{});
+                else contract(std::integral_constant<int, 2>{});
                 __syncwarp();
                 if (lane == 0) mbar_arrive(empty + stage);
                 if (++stage == nst) { stage = 0; phase ^= 1; }
