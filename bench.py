@@ -29,17 +29,17 @@ from paper_2208_10154_b200 import inputs, shard  # noqa: E402
 
 METRIC = "maps/sec (analysis+synthesis, FP64) at nside=512 lmax=1535"
 FP64_NOMINAL_TFLOPS = 37.2     # 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz
-# From the committed ncu captures (profiles/r1_v3_summary.md, profiles/r1_v2_summary.md), keyed by
+# From the committed ncu captures (profiles/r1_v4_summary.md staged, profiles/r1_v2_summary.md fused), keyed by
 # (config, nmaps, lambda mode, kernel): DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) and the
 # DMMA pipe activity (sm__pipe_tensor_subpipe_dmma_cycles_active, fraction of peak) = executed-flop rate / peak
 NCU_TRAFFIC_BYTES = {
-    (3, 1000, "staged", "k_legendre_analysis"): 259645201000 + 19115168000,
-    (3, 1000, "staged", "k_legendre_synthesis"): 27979806000 + 37874474000,
+    (3, 1000, "staged", "k_legendre_analysis"): 259432695040 + 19052913408,
+    (3, 1000, "staged", "k_legendre_synthesis"): 222430966528 + 37874563584,
     (3, 1000, "fused", "k_legendre_analysis"): 251379450880 + 19061606400,
     (3, 1000, "fused", "k_legendre_synthesis"): 20458497000 + 37875944000,
 }
 NCU_DMMA_PIPE_ACTIVE = {
-    (3, 1000, "staged", "k_legendre_analysis"): 0.945, (3, 1000, "staged", "k_legendre_synthesis"): 0.880,
+    (3, 1000, "staged", "k_legendre_analysis"): 0.907, (3, 1000, "staged", "k_legendre_synthesis"): 0.912,
     (3, 1000, "fused", "k_legendre_analysis"): 0.731, (3, 1000, "fused", "k_legendre_synthesis"): 0.770,
 }
 
@@ -316,7 +316,7 @@ def main():
     # staged mode: a Legendre "launch" is the lambda-block generator kernel plus the contraction kernel (both timed)
     roofline = leg_roofline(1, "k_legendre_analysis")
     roofline["peak_source"] = peak_note
-    roofline["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_v3_summary.md"
+    roofline["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_v4_summary.md (staged) / r1_v2_summary.md (fused)"
     roofline["note"] = ("achieved = algorithmic (N/S-folded, UNPRUNED) flops / time: ring pruning and l_safe row skipping "
                         "leave ~0.8x of them to execute, so frac can exceed 1; dmma_pipe_active_ncu is the executed-flop "
                         "fraction of peak from the committed ncu capture")
