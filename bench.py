@@ -35,11 +35,14 @@ FP64_NOMINAL_TFLOPS = 37.2     # 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz (DESI
 NCU_TRAFFIC_BYTES = {
     (3, 1000, "staged", "k_legendre_analysis"): 259432695040 + 19052913408,
     (3, 1000, "staged", "k_legendre_synthesis"): 222430966528 + 37874563584,
+    (4, 1000, "staged", "k_legendre_analysis"): 71304026880 + 9527154944,       # k_legendre_analysis_spin2
+    (4, 1000, "staged", "k_legendre_synthesis"): 45836310272 + 20283129600,     # k_legendre_synthesis_spin2
     (3, 1000, "fused", "k_legendre_analysis"): 251379450880 + 19061606400,
     (3, 1000, "fused", "k_legendre_synthesis"): 20458497000 + 37875944000,
 }
 NCU_DMMA_PIPE_ACTIVE = {
     (3, 1000, "staged", "k_legendre_analysis"): 0.907, (3, 1000, "staged", "k_legendre_synthesis"): 0.912,
+    (4, 1000, "staged", "k_legendre_analysis"): 0.945, (4, 1000, "staged", "k_legendre_synthesis"): 0.888,
     (3, 1000, "fused", "k_legendre_analysis"): 0.731, (3, 1000, "fused", "k_legendre_synthesis"): 0.770,
 }
 
