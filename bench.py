@@ -305,14 +305,17 @@ def main():
                  "rule-derived bf16 %s x 45/2250 = %.1f)"
                  % (FP64_NOMINAL_TFLOPS, peak_src, peaks.get("bf16_tflops", 0) * 45.0 / 2250.0))
 
+    # the committed captures describe the plain analysis + synthesis step only (no --pol, no --iter)
+    plain_key = None if (args.pol or args.iter >= 0) else (args.config, nmaps, lambda_mode)
+
     def leg_roofline(stage, kernel):
         n = max(1, stage_n[stage])                          # timed brackets = calls of the stage (generator + contraction)
         launch_ms = stage_ms[stage] / n
         flops_per_launch = fl_dir * dirs[stage] * args.steps / n          # algorithmic (folded, unpruned) flops of one launch
         ach = flops_per_launch / (launch_ms * 1e-3) * 1e-12
         return {"bound": "tensor", "kernel": kernel, "achieved": ach, "peak": mma_peak, "unit": "TFLOP/s",
-                "frac": ach / mma_peak, "traffic": NCU_TRAFFIC_BYTES.get((args.config, nmaps, lambda_mode, kernel)),
-                "dmma_pipe_active_ncu": NCU_DMMA_PIPE_ACTIVE.get((args.config, nmaps, lambda_mode, kernel)),
+                "frac": ach / mma_peak, "traffic": None if plain_key is None else NCU_TRAFFIC_BYTES.get(plain_key + (kernel,)),
+                "dmma_pipe_active_ncu": None if plain_key is None else NCU_DMMA_PIPE_ACTIVE.get(plain_key + (kernel,)),
                 "algorithmic_flops_per_launch": flops_per_launch, "launch_ms": launch_ms,
                 "share_of_step": stage_ms[stage] / ms_total}
 
