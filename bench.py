@@ -27,7 +27,6 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 from paper_2208_10154_b200 import inputs, shard  # noqa: E402
 
-METRIC = "maps/sec (analysis+synthesis, FP64) at nside=512 lmax=1535"
 FP64_NOMINAL_TFLOPS = 37.2     # 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz
 # From the committed ncu captures (profiles/r1_v4_summary.md staged, profiles/r1_v2_summary.md fused), keyed by
 # (config, nmaps, lambda mode, kernel): DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) and the
@@ -123,53 +122,145 @@ def min_hbm_bytes_per_direction(c, kpad):
     return maps + alm + 2 * F
 
 
-def cpu_baseline(c, nsample=8, stride=16):
-    """The oracle as it stands, timed on the host cores on a bounded sample: `nsample` maps, every
-    `stride`-th ring for synthesis and every `stride`-th m for analysis; cost extrapolated x stride
-    (rings and m values are sampled uniformly, so the sample has the workload's cost mix)."""
+def oracle_timed_sample(c, ks):
+    """The oracle as it stands on the box's host cores: full synthesis (every ring) then full analysis (every m) of the
+    maps `ks` of the workload -- maps are independent units, so sample size / wall time is the oracle's throughput
+    (SURVEY.md 8(d) "Oracle timing").  Nothing is extrapolated.  Returns (maps per second, seconds, threads)."""
     from oracle import oracle as O
     nside, lmax = c["nside"], c["lmax"]
-    ks = np.arange(nsample)
-    alm = inputs.gaussian_alm(lmax, ks, c["seed"], c["spin"])
-    rl = list(range(1, 4 * nside, stride))
-    ml = list(range(0, lmax + 1, stride))
+    alm = inputs.gaussian_alm(lmax, np.asarray(ks), c["seed"], c["spin"])
     t0 = time.time()
-    maps = O.synthesis(nside, lmax, alm, spin=c["spin"], rlist=rl)
-    t1 = time.time()
-    O.analysis(nside, lmax, maps, spin=c["spin"], mlist=ml)
-    t2 = time.time()
-    fr = len(rl) / (4 * nside - 1)
-    fm = len(ml) / (lmax + 1)
-    t_full = (t1 - t0) / fr + (t2 - t1) / fm
-    return {"value": nsample / t_full, "unit": "maps/s", "cores": O.num_threads(), "kind": "oracle",
-            "sample": "%d maps; synthesis of every %dth ring (%d of %d) + analysis of every %dth m (%d of %d), "
-                      "time extrapolated to all rings / all m; %.1f s of wall time"
-                      % (nsample, stride, len(rl), 4 * nside - 1, stride, len(ml), lmax + 1, t2 - t0)}
+    maps = O.synthesis(nside, lmax, alm, spin=c["spin"])
+    O.analysis(nside, lmax, maps, spin=c["spin"])
+    dt = time.time() - t0
+    return len(ks) / dt, dt, O.num_threads()
+
+
+def oracle_sample_size(c, n_calls):
+    """Maps per oracle call, the same rule for the cpu_baseline leg and the --impl reference arm so that their numbers
+    are comparable (the oracle shares its lambda / phase tables among the maps of a call, so its throughput depends on
+    the sample size): the 8-map comparison subset of SURVEY.md 8(d) when the run makes few calls, fewer maps when the
+    driver asks for many steps, so that the reference arm still ends within a few minutes."""
+    n = 8 if n_calls <= 6 else 4 if n_calls <= 12 else 2 if n_calls <= 24 else 1
+    return min(n, c["nmaps"])
+
+
+def cpu_baseline(c, nsample):
+    """cpu_baseline leg: one timed oracle call on the first `nsample` maps of the workload."""
+    ks = list(range(min(nsample, c["nmaps"])))
+    v, dt, cores = oracle_timed_sample(c, ks)
+    return {"value": v, "unit": unit_of(c), "cores": cores, "kind": "oracle",
+            "sample": "maps %d..%d of the workload: full synthesis (all %d rings) + full analysis (all %d orders m), "
+                      "%.1f s of wall time, nothing extrapolated" % (ks[0], ks[-1], 4 * c["nside"] - 1, c["lmax"] + 1, dt)}
+
+
+def unit_of(c):
+    return "pairs/s" if c["spin"] == 2 else "maps/s"
+
+
+def metric_of(c):
+    """BASELINE.json's metric string with the workload's own sizes (the headline workload gives it verbatim)"""
+    return "%s/sec (analysis+synthesis, FP64) at nside=%d lmax=%d" % ("(Q,U) pairs" if c["spin"] == 2 else "maps",
+                                                                       c["nside"], c["lmax"])
+
+
+def base_config(c):
+    return {"workload": c["name"], "nside": c["nside"], "lmax": c["lmax"], "nmaps_per_gpu": c["nmaps"], "spin": c["spin"]}
 
 
 def run_reference(args, c):
+    """Reference arm = the oracle on the host cores (there is no other implementation of the paper here).  Each step
+    transforms a bounded sample of the workload in full (oracle_sample_size).  ms_per_step is the wall time a step took."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    vals = []
+    nsample = oracle_sample_size(c, args.steps + args.warmup)
     for _ in range(args.warmup):
-        cpu_baseline(c, nsample=2, stride=64)
-    last = None
+        oracle_timed_sample(c, list(range(nsample)))
+    vals, secs = [], []
     for _ in range(args.steps):
-        last = cpu_baseline(c, nsample=4, stride=32)
-        vals.append(last["value"])
-    v = float(np.mean(vals))
-    last["value"] = v
-    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "maps/s", "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * c["nmaps"] / v,
+        v, dt, cores = oracle_timed_sample(c, list(range(nsample)))
+        vals.append(v); secs.append(dt)
+    v = float(nsample * len(secs) / sum(secs))
+    cb = {"value": v, "unit": unit_of(c), "cores": cores, "kind": "oracle",
+          "sample": "%d map(s) per step: full synthesis + full analysis, nothing extrapolated; %d steps, %.1f s per step"
+                    % (nsample, args.steps, float(np.mean(secs)))}
+    line = {"impl": "reference", "metric": metric_of(c), "value": v, "unit": unit_of(c), "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)),
+            "maps_per_step": nsample,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic",
-            "config": {"workload": c["name"], "nside": c["nside"], "lmax": c["lmax"], "nmaps": c["nmaps"],
-                       "spin": c["spin"]},
-            "cpu_baseline": last,
-            "e2e": {"value": v, "unit": "maps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "data": "synthetic", "config": base_config(c), "cpu_baseline": cb,
+            "e2e": {"value": v, "unit": unit_of(c), "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
+
+
+def cublas_dgemm_peak(dev, seconds=2.0, n=8192):
+    """Reported comparison only (north_star: "cuBLAS DGEMM kept only as a reported comparison"; SURVEY.md 8(d) "quote all
+    three"): torch.matmul FP64 n^3 (= cuBLAS DGEMM) back to back for `seconds`, with the SM clock sampled meanwhile.
+    Lives in bench.py only; the library links no cuBLAS."""
+    import torch
+    a = torch.randn((n, n), dtype=torch.float64, device=dev)
+    b = torch.randn((n, n), dtype=torch.float64, device=dev)
+    o = torch.empty((n, n), dtype=torch.float64, device=dev)
+    for _ in range(3):
+        torch.matmul(a, b, out=o)
+    torch.cuda.synchronize()
+    smp = ClockSampler(dev.index or 0)
+    smp.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps, ms = 0, 0.0
+    e0.record()
+    while ms < seconds * 1e3:
+        for _ in range(4):
+            torch.matmul(a, b, out=o)
+        reps += 4
+        e1.record()
+        e1.synchronize()
+        ms = e0.elapsed_time(e1)
+    clk = smp.stop()
+    return {"tflops": 2.0 * n ** 3 * reps / (ms * 1e-3) * 1e-12, "n": n, "seconds": ms * 1e-3, "sm_mhz": clk.get("sm_mhz"),
+            "reasons": clk.get("reasons")}
+
+
+def cublas_per_m_dgemm(c, dev, mstep=1):
+    """The paper's own formulation of the Legendre stage (Alg. 1 l.10; items 6-7, :220-224): one real DGEMM
+    per order m of a materialised P_m against the ring spectra of all maps, timed with cuBLAS (torch.matmul) on matrices of
+    the right shapes -- (lmax - m + 1) x rings times rings x 2K, analysis orientation; the synthesis product has the
+    same flops.  DGEMM time does not depend on the values, so P_m and T_m are random here (the comparison is about the
+    contraction, P_m generation is not included).  `unfolded`: all 4 nside - 1 rings, the paper's form; `folded`: two
+    products per m over the 2 nside ring pairs (even / odd l - m), the north/south fold of north_star.  No ring pruning."""
+    import torch
+    nside, lmax, K = c["nside"], c["lmax"], c["nmaps"]
+    ncomp = 2 if c["spin"] == 2 else 1
+    nr, nh, ncol = 4 * nside - 1, 2 * nside, 2 * K * ncomp
+    blk = (2 if c["spin"] == 2 else 1)                   # spin 2: the 2 x 2 block matrix [[F+,F-],[F-,F+]] (eq. 14)
+    P = torch.randn((blk * (lmax + 1), blk * nr), dtype=torch.float64, device=dev)
+    T = torch.randn((blk * nr, ncol // blk), dtype=torch.float64, device=dev)
+    out = torch.empty((blk * (lmax + 1), ncol // blk), dtype=torch.float64, device=dev)
+    res = {}
+    for name in ("unfolded", "folded"):
+        def run():
+            for m in range(0, lmax + 1, mstep):
+                nl = lmax - m + 1
+                if name == "unfolded":
+                    torch.matmul(P[:blk * nl, :], T, out=out[:blk * nl])
+                else:
+                    ne, no = (nl + 1) // 2, nl // 2
+                    torch.matmul(P[:blk * ne, :blk * nh], T[:blk * nh], out=out[:blk * ne])
+                    if no:
+                        torch.matmul(P[:blk * no, :blk * nh], T[:blk * nh], out=out[:blk * no])
+        run()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        run()
+        e1.record()
+        e1.synchronize()
+        res[name + "_ms_per_direction"] = e0.elapsed_time(e1) * mstep
+    res["mstep"] = mstep
+    res["note"] = "cuBLAS DGEMM per m on random matrices of the paper's shapes; operands L2/HBM resident, P_m generation excluded"
+    return res
 
 
 def main():
@@ -190,6 +281,8 @@ def main():
                          "Alg. 3, the immediate iteration (one order m at a time, spin 0)")
     ap.add_argument("--lambda-mode", default="", choices=["", "fused", "staged"],
                     help="where the P_lm tiles are generated (include/sht.h); default: the plan's own choice")
+    ap.add_argument("--compare", default="", choices=["", "cublas"],
+                    help="cublas: also time the paper's per-m cuBLAS DGEMM formulation of the Legendre stage (comparison only)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
@@ -300,6 +393,8 @@ def main():
     if args.iter >= 0:
         dirs = {1: 2 * args.iter + 1, 2: 1} if args.iter_mode == "immediate" else {1: args.iter + 1, 2: max(args.iter, 1)}
     mma_peak = sht_measure_fp64_mma_peak(300.0)
+    cublas_peak = cublas_dgemm_peak(dev) if rank == 0 else None
+    cublas_cmp = cublas_per_m_dgemm(c, dev) if (args.compare == "cublas" and rank == 0) else None
     peak_note = ("FP64 DMMA.8x8x4 register-resident loop measured live in this run "
                  "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = %.1f; "
                  "rule-derived bf16 %s x 45/2250 = %.1f)"
@@ -322,6 +417,13 @@ def main():
     # staged mode: a Legendre "launch" is the lambda-block generator kernel plus the contraction kernel (both timed)
     roofline = leg_roofline(1, "k_legendre_analysis")
     roofline["peak_source"] = peak_note
+    if cublas_peak:
+        roofline["peak_cublas_dgemm"] = cublas_peak["tflops"]
+        roofline["peak_cublas_dgemm_how"] = ("torch.matmul FP64 %d^3 back to back for %.1f s, SM clock median %s MHz, reasons %s "
+                                             "(comparison only, bench.py; the library links no cuBLAS)"
+                                             % (cublas_peak["n"], cublas_peak["seconds"], cublas_peak["sm_mhz"], cublas_peak["reasons"]))
+    if cublas_cmp:
+        roofline["cublas_per_m_dgemm"] = cublas_cmp
     roofline["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_v4_summary.md (staged) / r1_v2_summary.md (fused)"
     roofline["note"] = ("achieved = algorithmic (N/S-folded, UNPRUNED) flops / time: ring pruning and l_safe row skipping "
                         "leave ~0.8x of them to execute, so frac can exceed 1; dmma_pipe_active_ncu is the executed-flop "
@@ -363,22 +465,22 @@ def main():
             dt = shard.max_over_ranks(dt, dev)
             bytes_alm = h_alm.numel() * 16
             bytes_maps = h_maps.numel() * 8
-            e2e = {"value": world * nmaps / dt, "unit": "maps/s", "h2d_bytes_per_step": bytes_alm + bytes_maps,
+            e2e = {"value": world * nmaps / dt, "unit": unit_of(c), "h2d_bytes_per_step": bytes_alm + bytes_maps,
                    "d2h_bytes_per_step": bytes_alm + bytes_maps, "ms_per_step": dt * 1e3,
                    "api": "sht_synthesis_host + sht_analysis_host (pinned host buffers, chunked H2D/compute/D2H)"}
         except Exception as ex:  # host memory too small for pinned copies of the workload, etc.
-            e2e = {"value": None, "unit": "maps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+            e2e = {"value": None, "unit": unit_of(c), "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
                    "error": str(ex)[:200]}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        cpu = cpu_baseline(c)
+        cpu = cpu_baseline(c, oracle_sample_size(c, args.steps + args.warmup))
 
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": "maps/s", "n_gpus": world, "steps": args.steps,
+        line = {"metric": metric_of(c), "value": value, "unit": unit_of(c), "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": c["name"], "nside": nside, "lmax": lmax, "nmaps_per_gpu": nmaps, "spin": spin,
+                "config": {**base_config(c),
                            "l2": "inputs (%.1f GB maps, %.1f GB a_lm per GPU) are far larger than the 126 MB L2"
                                  % (8e-9 * npix * nmaps * ncomp, 16e-9 * nalm * nmaps * ncomp),
                            "plan_create_s": plan_s, "chunk_maps": plan.chunk_maps(), "lambda_mode": lambda_mode,

@@ -19,7 +19,9 @@
  *   - `maps`, `alm`, `resid_rms` of the device entries are DEVICE pointers owned by the caller
  *     (FP64, dense, 16-byte aligned); inputs are never modified; outputs are fully overwritten.
  *   - Device entries are asynchronous on `stream` (a cudaStream_t passed as void*, NULL = default
- *     stream); the library synchronises only in plan create/destroy and in the *_host entries.
+ *     stream); the library synchronises only in plan create/destroy, sht_plan_reserve_iter and the *_host
+ *     entries.  One exception, stated at sht_analysis_iter: its first call on a plan that was not reserved
+ *     allocates the second workspace (cudaMalloc); everything it queues is still ordered on `stream`.
  *   - A plan is used from one host thread at a time; distinct plans are independent.
  *   - There is no CPU fallback: without a CUDA device plan creation fails with SHT_ERR_CUDA.
  *
@@ -98,6 +100,11 @@ sht_status_t sht_analysis_iter(sht_plan_t plan, const double* maps, double* alm,
  *                    3 launches per pair of orders (m even, m + 1). */
 enum { SHT_ITER_TM = 0, SHT_ITER_PIXEL = 1, SHT_ITER_IMMEDIATE = 2 };
 sht_status_t sht_plan_set_iter_mode(sht_plan_t plan, int mode);
+/* Allocates (and zero-fills) the second workspace of SHT_ITER_TM / SHT_ITER_IMMEDIATE now and waits for it, so that
+ * sht_analysis_iter never allocates or synchronises.  SHT_ERR_ALLOC if it does not fit (SHT_ITER_TM then runs as
+ * SHT_ITER_PIXEL).  Without this call the first iterative call allocates it itself (one synchronous cudaMalloc; its
+ * zero fill is queued on that call's stream). */
+sht_status_t sht_plan_reserve_iter(sht_plan_t plan);
 
 /* Spin-2 plans: transforms of a_lm^E or a_lm^B alone (item 9: "forward and backward transforms of a^E
  * and a^B separately ... the speed of SHTs can be increased by 100% for free"): half of the block products of eq. 14 /
@@ -108,9 +115,17 @@ enum { SHT_POL_E = 1, SHT_POL_B = 2 };
 sht_status_t sht_analysis_pol(sht_plan_t plan, const double* maps, double* alm, int which, void* stream);
 sht_status_t sht_synthesis_pol(sht_plan_t plan, const double* alm, double* maps, int which, void* stream);
 
+/* Pixel-domain E/B decomposition (eq. 16 and 19): S^{E,B}_m = (F_m^t lambda^{E,B} F_m) S_m, i.e.
+ * maps_out = sht_synthesis_pol(sht_analysis_pol(maps_in, which), which): the (Q,U) maps that carry only the E-family
+ * (which = SHT_POL_E) or only the B-family (SHT_POL_B) part of maps_in -- the building block of the EB-leakage pipeline
+ * (PAPER.md:273).  DEVICE pointers, [nmaps][2][npix]; maps_out may be maps_in; the a_lm of the one component live in a
+ * stream-ordered scratch of the library.  Spin-2 plans only.  Asynchronous on `stream`. */
+sht_status_t sht_eb_split(sht_plan_t plan, const double* maps_in, double* maps_out, int which, void* stream);
+
 /* Same transforms on HOST buffers (pinned or pageable; same layouts).  Each call copies its input to the
  * device, runs the device entry and copies the result back, in map chunks on the plan's own streams,
- * and returns after the result is complete in host memory.  These are the end-to-end calls bench.py times. */
+ * and returns after the result is complete in host memory.  They first wait for all device work queued before
+ * (the chunk streams share the plan's workspace with the device entries).  These are the end-to-end calls bench.py times. */
 sht_status_t sht_analysis_host(sht_plan_t plan, const double* maps_host, double* alm_host);
 sht_status_t sht_synthesis_host(sht_plan_t plan, const double* alm_host, double* maps_host);
 
@@ -135,7 +150,7 @@ const char* sht_last_error(sht_plan_t plan);         /* plan-owned, valid until 
  * With timing enabled every kernel launched by the plan on the caller's stream is bracketed by CUDA events.
  * sht_plan_stage_ms waits for the recorded events and returns, accumulated since the last call, the device
  * milliseconds ms[4] and launch counts n[4] of: 0 ring-FFT analysis, 1 Legendre analysis, 2 Legendre synthesis,
- * 3 ring-FFT synthesis; then resets the accumulation.  At most 256 launches are kept between two calls. */
+ * 3 ring-FFT synthesis; then resets the accumulation.  SHT_ERR_ALLOC (sums incomplete) if a bracket could not be recorded. */
 sht_status_t sht_plan_set_timing(sht_plan_t plan, int enable);
 sht_status_t sht_plan_stage_ms(sht_plan_t plan, double* ms4, int* n4);
 

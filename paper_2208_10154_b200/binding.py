@@ -47,6 +47,10 @@ _lib.sht_plan_set_lambda_mode.argtypes = [_vp, _i]
 _lib.sht_plan_set_lambda_mode.restype = _i
 _lib.sht_plan_lambda_mode.argtypes = [_vp]
 _lib.sht_plan_lambda_mode.restype = _i
+_lib.sht_plan_reserve_iter.argtypes = [_vp]
+_lib.sht_plan_reserve_iter.restype = _i
+_lib.sht_eb_split.argtypes = [_vp, _vp, _vp, _i, _vp]
+_lib.sht_eb_split.restype = _i
 _lib.sht_analysis_iter.argtypes = [_vp, _vp, _vp, _i, _vp, _vp]
 _lib.sht_analysis_iter.restype = _i
 _lib.sht_analysis_host.argtypes = [_vp, _vp, _vp]
@@ -77,7 +81,7 @@ _lib.sht_measure_fp64_mma_peak.argtypes = [_d]
 _lib.sht_measure_fp64_mma_peak.restype = _d
 
 EXPORTED = [
-    "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol", "sht_alm_pack_a7", "sht_alm_unpack_a7", "sht_plan_set_lambda_mode", "sht_plan_lambda_mode", "sht_plan_set_iter_mode",
+    "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol", "sht_alm_pack_a7", "sht_alm_unpack_a7", "sht_plan_set_lambda_mode", "sht_plan_lambda_mode", "sht_plan_set_iter_mode", "sht_plan_reserve_iter", "sht_eb_split",
     "sht_analysis_host", "sht_synthesis_host", "sht_npix", "sht_nalm", "sht_alm_index",
     "sht_plan_workspace_bytes", "sht_plan_chunk_maps", "sht_plan_kernel_launches", "sht_status_string",
     "sht_last_error", "sht_measure_fp64_mma_peak", "sht_plan_set_timing", "sht_plan_stage_ms",
@@ -171,6 +175,12 @@ class Plan:
 
     def sht_synthesis_pol(self, alm, maps, which, stream=None):
         self._check(_lib.sht_synthesis_pol(self._h, _ptr(alm), _ptr(maps), which, _stream(stream)), "sht_synthesis_pol")
+
+    def sht_eb_split(self, maps_in, maps_out, which, stream=None):
+        self._check(_lib.sht_eb_split(self._h, _ptr(maps_in), _ptr(maps_out), which, _stream(stream)), "sht_eb_split")
+
+    def sht_plan_reserve_iter(self):
+        self._check(_lib.sht_plan_reserve_iter(self._h), "sht_plan_reserve_iter")
 
     def sht_plan_set_iter_mode(self, mode):
         self._check(_lib.sht_plan_set_iter_mode(self._h, mode), "sht_plan_set_iter_mode")

@@ -1,5 +1,6 @@
 // sht_api.cu -- the C ABI of include/sht.h: argument checks, map chunking, stage sequencing.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include "sht_internal.h"
 
@@ -8,9 +9,11 @@ using namespace sht;
 namespace sht {
 
 // sum of squares per (map, component) for the residual rms of Alg. 2 (reading G18 in DESIGN.md)
-__global__ void k_sumsq(const double* __restrict__ x, long long npix, double* __restrict__ acc)
+// rows = blockIdx.y + j * gridDim.y (the grid's y extent is capped at 65535)
+__global__ void k_sumsq(const double* __restrict__ x, long long npix, int nrow, double* __restrict__ acc)
 {
-    const double* row = x + (size_t)blockIdx.y * npix;
+  for (int rowi = blockIdx.y; rowi < nrow; rowi += gridDim.y) {
+    const double* row = x + (size_t)rowi * npix;
     double s = 0.0;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < npix; i += (long long)gridDim.x * blockDim.x) {
         const double v = row[i];
@@ -23,8 +26,10 @@ __global__ void k_sumsq(const double* __restrict__ x, long long npix, double* __
     if (threadIdx.x < 32) {
         s = threadIdx.x < (blockDim.x >> 5) ? ws[threadIdx.x] : 0.0;
         for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (threadIdx.x == 0) atomicAdd(acc + blockIdx.y, s);
+        if (threadIdx.x == 0) atomicAdd(acc + rowi, s);
     }
+    __syncthreads();
+  }
 }
 
 __global__ void k_rms_finish(const double* __restrict__ acc, int n, double inv_npix, double* __restrict__ out)
@@ -95,12 +100,41 @@ static sht_status_t cuda_fail(sht_plan_t pl, const char* what, cudaError_t e)
         if (e__ != cudaSuccess) return cuda_fail(pl, what, e__); \
     } while (0)
 
+// stream-ordered scratch that is released on every exit path (SHT_TRY returns early)
+struct AsyncScratch {
+    void* p = nullptr;
+    cudaStream_t st;
+    explicit AsyncScratch(cudaStream_t s) : st(s) {}
+    AsyncScratch(const AsyncScratch&) = delete;
+    AsyncScratch& operator=(const AsyncScratch&) = delete;
+    ~AsyncScratch() { if (p) cudaFreeAsync(p, st); }
+    cudaError_t alloc(size_t bytes) { return cudaMallocAsync(&p, bytes ? bytes : 16, st); }
+    double* d() const { return static_cast<double*>(p); }
+};
+
 // ---- optional per-stage timing ---------------------------------------------------------------------
 static int timing_begin(sht_plan_t pl, int stage, cudaStream_t st)
 {
-    if (!pl->timing || pl->n_ev >= 256) return -1;
-    const int i = pl->n_ev++;
-    if (!pl->ev0[i]) { cudaEventCreate(&pl->ev0[i]); cudaEventCreate(&pl->ev1[i]); }
+    if (!pl->timing) return -1;
+    if (pl->n_ev == pl->cap_ev) {                        // grow the event arrays (Alg. 3 records thousands of brackets)
+        const int cap = pl->cap_ev ? 2 * pl->cap_ev : 256;
+        cudaEvent_t* a = (cudaEvent_t*)realloc(pl->ev0, (size_t)cap * sizeof(cudaEvent_t));
+        if (a) pl->ev0 = a;
+        cudaEvent_t* b = a ? (cudaEvent_t*)realloc(pl->ev1, (size_t)cap * sizeof(cudaEvent_t)) : nullptr;
+        if (b) pl->ev1 = b;
+        int* c = b ? (int*)realloc(pl->ev_stage, (size_t)cap * sizeof(int)) : nullptr;
+        if (c) pl->ev_stage = c;
+        if (!a || !b || !c) { pl->ev_dropped++; return -1; }
+        for (int i = pl->cap_ev; i < cap; ++i) { pl->ev0[i] = nullptr; pl->ev1[i] = nullptr; }
+        pl->cap_ev = cap;
+    }
+    const int i = pl->n_ev;
+    if (!pl->ev0[i] && (cudaEventCreate(&pl->ev0[i]) != cudaSuccess || cudaEventCreate(&pl->ev1[i]) != cudaSuccess)) {
+        cudaGetLastError();
+        pl->ev_dropped++;
+        return -1;
+    }
+    pl->n_ev++;
     pl->ev_stage[i] = stage;
     cudaEventRecord(pl->ev0[i], st);
     return i;
@@ -115,6 +149,7 @@ extern "C" sht_status_t sht_plan_set_timing(sht_plan_t pl, int enable)
     if (!pl) return SHT_ERR_NULL;
     pl->timing = enable != 0;
     pl->n_ev = 0;
+    pl->ev_dropped = 0;
     return SHT_OK;
 }
 
@@ -130,28 +165,35 @@ extern "C" sht_status_t sht_plan_stage_ms(sht_plan_t pl, double* ms4, int* n4)
         ms4[pl->ev_stage[i]] += t; n4[pl->ev_stage[i]]++;
     }
     pl->n_ev = 0;
+    if (pl->ev_dropped) {                                // never silently: the sums would be short
+        snprintf(pl->err, sizeof(pl->err), "stage timing: %lld brackets could not be recorded", pl->ev_dropped);
+        pl->ev_dropped = 0;
+        return SHT_ERR_ALLOC;
+    }
     return SHT_OK;
 }
 
 // maps[kmap0 .. kmap0+kmaps) -> alm[kalm0 .. kalm0+kmaps)
 static sht_status_t analysis_chunk(sht_plan_t pl, const DevicePlan& d, const double* maps, int kmap0, double* alm,
-                                   int kalm0, double* F, int kmaps, bool accumulate, cudaStream_t st)
+                                   int kalm0, double* F, int kmaps, bool accumulate, cudaStream_t st, int pol = 0,
+                                   bool gen_lambda = true)
 {
     int t = timing_begin(pl, 0, st);
     SHT_TRY(launch_ring_analysis(pl, d, maps, F, kmap0, kmaps, st), "ring analysis");
     timing_end(pl, t, st);
     t = timing_begin(pl, 1, st);
-    SHT_TRY(launch_legendre_analysis(pl, d, F, alm, kalm0, kmaps, accumulate, st), "legendre analysis");
+    SHT_TRY(launch_legendre_analysis(pl, d, F, alm, kalm0, kmaps, accumulate, st, pol, gen_lambda), "legendre analysis");
     timing_end(pl, t, st);
     return SHT_OK;
 }
 
 // alm[kalm0 ..) -> maps[kmap0 ..); with sub_from: maps = sub_from[ksub0 ..] - synthesis
 static sht_status_t synthesis_chunk(sht_plan_t pl, const DevicePlan& d, const double* alm, int kalm0, double* maps,
-                                    int kmap0, double* F, int kmaps, const double* sub_from, int ksub0, cudaStream_t st)
+                                    int kmap0, double* F, int kmaps, const double* sub_from, int ksub0, cudaStream_t st,
+                                    int pol = 0, bool gen_lambda = true)
 {
     int t = timing_begin(pl, 2, st);
-    SHT_TRY(launch_legendre_synthesis(pl, d, alm, F, kalm0, kmaps, st), "legendre synthesis");
+    SHT_TRY(launch_legendre_synthesis(pl, d, alm, F, kalm0, kmaps, st, pol, gen_lambda), "legendre synthesis");
     timing_end(pl, t, st);
     t = timing_begin(pl, 3, st);
     SHT_TRY(launch_ring_synthesis(pl, d, F, maps, kmap0, kmaps, sub_from, ksub0, st), "ring synthesis");
@@ -196,14 +238,12 @@ static sht_status_t pol_run(sht_plan_t pl, const double* maps, const double* alm
         return SHT_ERR_INVALID_ARG;
     }
     cudaStream_t st = (cudaStream_t)stream;
-    pl->pol = which;
     sht_status_t s = SHT_OK;
     for (int k0 = 0; k0 < pl->nmaps && s == SHT_OK; k0 += pl->chunk) {
         const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
-        s = alm_out ? analysis_chunk(pl, pl->d, maps, k0, alm_out, k0, pl->F, kmaps, false, st)
-                    : synthesis_chunk(pl, pl->d, alm_in, k0, maps_out, k0, pl->F, kmaps, nullptr, 0, st);
+        s = alm_out ? analysis_chunk(pl, pl->d, maps, k0, alm_out, k0, pl->F, kmaps, false, st, which)
+                    : synthesis_chunk(pl, pl->d, alm_in, k0, maps_out, k0, pl->F, kmaps, nullptr, 0, st, which);
     }
-    pl->pol = 0;
     return s;
 }
 
@@ -223,8 +263,9 @@ extern "C" sht_status_t sht_synthesis_pol(sht_plan_t pl, const double* alm, doub
 static sht_status_t iter_tm_space(sht_plan_t pl, const double* maps, double* alm, int niter, double* resid_rms, cudaStream_t st)
 {
     const DevicePlan& d = pl->d;
-    double* acc = nullptr;
-    SHT_TRY(cudaMallocAsync((void**)&acc, (size_t)pl->chunk * d.ncomp * sizeof(double), st), "rms scratch");
+    AsyncScratch accs(st);
+    SHT_TRY(accs.alloc((size_t)pl->chunk * d.ncomp * sizeof(double)), "rms scratch");
+    double* acc = accs.d();
     const size_t ubytes = (size_t)d.nh * d.ncomp * d.kpad * sizeof(double);
     sht_status_t s = SHT_OK;
     for (int k0 = 0; k0 < pl->nmaps && s == SHT_OK; k0 += pl->chunk) {
@@ -256,7 +297,6 @@ static sht_status_t iter_tm_space(sht_plan_t pl, const double* maps, double* alm
             timing_end(pl, t, st);
         }
     }
-    cudaFreeAsync(acc, st);
     return s;
 }
 
@@ -269,9 +309,10 @@ static sht_status_t iter_tm_space(sht_plan_t pl, const double* maps, double* alm
 static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* alm, int niter, double* resid_rms, cudaStream_t st)
 {
     const DevicePlan& d = pl->d;
-    double* acc = nullptr; double* da = nullptr;
-    SHT_TRY(cudaMallocAsync((void**)&acc, (size_t)pl->chunk * d.ncomp * sizeof(double), st), "rms scratch");
-    SHT_TRY(cudaMallocAsync((void**)&da, (size_t)pl->chunk * d.ncomp * d.nalm * 2 * sizeof(double), st), "increment scratch");
+    AsyncScratch accs(st), das(st);
+    SHT_TRY(accs.alloc((size_t)pl->chunk * d.ncomp * sizeof(double)), "rms scratch");
+    SHT_TRY(das.alloc((size_t)pl->chunk * d.ncomp * d.nalm * 2 * sizeof(double)), "increment scratch");
+    double* acc = accs.d(); double* da = das.d();
     const size_t ubytes = (size_t)d.nh * d.ncomp * d.kpad * sizeof(double);
     double* R = pl->F;              // residual, folded (even / odd), all orders
     double* S = pl->Fmap;           // T_m(map) first, then the synthesised increment of one order at a time
@@ -317,9 +358,25 @@ static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* al
             timing_end(pl, t, st);
         }
     }
-    cudaFreeAsync(da, st);
-    cudaFreeAsync(acc, st);
     return SHT_OK;
+}
+
+// second workspace of the T_m-space iterations (folded T_m of the input maps) + uncovered-power table; the padded map
+// columns must stay finite, so the workspace is zero-filled once, on stream `st` (ordered before the caller's kernels)
+static void iter_reserve(sht_plan_t pl, cudaStream_t st)
+{
+    const DevicePlan& d = pl->d;
+    const size_t ubytes = (size_t)d.nh * d.ncomp * d.kpad * sizeof(double);
+    double *fm = nullptr, *up = nullptr;
+    if (cudaMalloc((void**)&fm, pl->F_bytes) != cudaSuccess || cudaMalloc((void**)&up, ubytes) != cudaSuccess ||
+        cudaMemsetAsync(fm, 0, pl->F_bytes, st) != cudaSuccess) {
+        cudaGetLastError();
+        if (fm) cudaFree(fm);
+        if (up) cudaFree(up);
+        pl->iter_reserve_failed = true;                  // do not retry on every call: fall back to residual maps
+        return;
+    }
+    pl->Fmap = fm; pl->upow = up;
 }
 
 extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, double* alm, int niter,
@@ -331,15 +388,9 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
     cudaStream_t st = (cudaStream_t)stream;
     const DevicePlan& d = pl->d;
     if (niter > 0 && pl->iter_mode != SHT_ITER_PIXEL) {
-        if (!pl->Fmap) {                                 // first iterative call: second workspace + uncovered-power table
-            const size_t ubytes = (size_t)d.nh * d.ncomp * d.kpad * sizeof(double);
-            if (cudaMalloc((void**)&pl->Fmap, pl->F_bytes) != cudaSuccess || cudaMalloc((void**)&pl->upow, ubytes) != cudaSuccess) {
-                cudaGetLastError();
-                if (pl->Fmap) { cudaFree(pl->Fmap); pl->Fmap = nullptr; }
-            } else if (cudaMemset(pl->Fmap, 0, pl->F_bytes) != cudaSuccess) {
-                return cuda_fail(pl, "workspace memset", cudaGetLastError());
-            }
-        }
+        // second workspace: normally reserved ahead (sht_plan_reserve_iter); otherwise allocated here, which is the one
+        // place a device entry may synchronise (cudaMalloc) -- its zero fill is ordered on the caller's stream
+        if (!pl->Fmap && !pl->iter_reserve_failed) iter_reserve(pl, st);
         if (pl->iter_mode == SHT_ITER_IMMEDIATE) {
             if (!pl->Fmap) { snprintf(pl->err, sizeof(pl->err), "immediate iteration: no memory for the second workspace"); return SHT_ERR_CUDA; }
             return iter_immediate(pl, maps, alm, niter, resid_rms, st);
@@ -347,11 +398,12 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
         if (pl->Fmap) return iter_tm_space(pl, maps, alm, niter, resid_rms, st);
     }
     // residual maps of one chunk + sum-of-squares accumulators (stream-ordered scratch)
-    double* res = nullptr; double* acc = nullptr;
+    AsyncScratch ress(st), accs(st);
     if (niter > 0) {
-        SHT_TRY(cudaMallocAsync((void**)&res, (size_t)pl->chunk * d.ncomp * d.npix * sizeof(double), st), "residual scratch");
-        SHT_TRY(cudaMallocAsync((void**)&acc, (size_t)pl->chunk * d.ncomp * sizeof(double), st), "rms scratch");
+        SHT_TRY(ress.alloc((size_t)pl->chunk * d.ncomp * d.npix * sizeof(double)), "residual scratch");
+        SHT_TRY(accs.alloc((size_t)pl->chunk * d.ncomp * sizeof(double)), "rms scratch");
     }
+    double* res = ress.d(); double* acc = accs.d();
     sht_status_t s = SHT_OK;
     for (int k0 = 0; k0 < pl->nmaps && s == SHT_OK; k0 += pl->chunk) {
         const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
@@ -363,8 +415,8 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
             if (resid_rms) {
                 const int nrow = kmaps * d.ncomp;
                 SHT_TRY(cudaMemsetAsync(acc, 0, (size_t)nrow * sizeof(double), st), "rms memset");
-                dim3 grid(64, nrow);
-                k_sumsq<<<grid, 256, 0, st>>>(res, d.npix, acc);
+                dim3 grid(64, nrow < 65535 ? nrow : 65535);
+                k_sumsq<<<grid, 256, 0, st>>>(res, d.npix, nrow, acc);
                 k_rms_finish<<<(nrow + 127) / 128, 128, 0, st>>>(acc, nrow, 1.0 / (double)d.npix,
                                                                  resid_rms + (size_t)it * pl->nmaps * d.ncomp + (size_t)k0 * d.ncomp);
                 pl->launches += 2;
@@ -373,8 +425,40 @@ extern "C" sht_status_t sht_analysis_iter(sht_plan_t pl, const double* maps, dou
             s = analysis_chunk(pl, pl->d, res, 0, alm, k0, pl->F, kmaps, true, st);
         }
     }
-    if (res) cudaFreeAsync(res, st);
-    if (acc) cudaFreeAsync(acc, st);
+    return s;
+}
+
+extern "C" sht_status_t sht_plan_reserve_iter(sht_plan_t pl)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (pl->Fmap) return SHT_OK;
+    pl->iter_reserve_failed = false;
+    iter_reserve(pl, nullptr);
+    if (!pl->Fmap) { snprintf(pl->err, sizeof(pl->err), "no memory for the second workspace"); return SHT_ERR_ALLOC; }
+    if (cudaStreamSynchronize(nullptr) != cudaSuccess) return cuda_fail(pl, "reserve sync", cudaGetLastError());
+    return SHT_OK;
+}
+
+// Pixel-domain E/B decomposition (eq. 16 / 19): S^{E,B} = (F^t lambda^{E,B} F) S.  Per chunk: ring FFTs
+// of (Q,U) -> single-component Legendre analysis (item 9: half of the block products) -> the a_lm of that component stay
+// in a stream-ordered scratch -> single-component Legendre synthesis -> backward ring FFTs.
+extern "C" sht_status_t sht_eb_split(sht_plan_t pl, const double* maps_in, double* maps_out, int which, void* stream)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (!maps_in || !maps_out) { snprintf(pl->err, sizeof(pl->err), "null data pointer"); return SHT_ERR_NULL; }
+    if (pl->d.spin != 2 || (which != SHT_POL_E && which != SHT_POL_B)) {
+        snprintf(pl->err, sizeof(pl->err), "sht_eb_split needs a spin-2 plan and which = SHT_POL_E or SHT_POL_B");
+        return SHT_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    AsyncScratch as(st);
+    SHT_TRY(as.alloc((size_t)pl->chunk * pl->d.nalm * 2 * sizeof(double)), "a_lm scratch");
+    sht_status_t s = SHT_OK;
+    for (int k0 = 0; k0 < pl->nmaps && s == SHT_OK; k0 += pl->chunk) {
+        const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
+        s = analysis_chunk(pl, pl->d, maps_in, k0, as.d(), 0, pl->F, kmaps, false, st, which);
+        if (s == SHT_OK) s = synthesis_chunk(pl, pl->d, as.d(), 0, maps_out, k0, pl->F, kmaps, nullptr, 0, st, which);
+    }
     return s;
 }
 
@@ -414,10 +498,21 @@ static sht_status_t host_setup(sht_plan_t pl)
     pl->host_nb = nb;
     const size_t mbytes = (size_t)hc * d.ncomp * d.npix * sizeof(double);
     const size_t abytes = (size_t)hc * d.ncomp * d.nalm * 2 * sizeof(double);
-    for (int i = 0; i < nb; ++i) {
-        SHT_TRY(cudaMalloc((void**)&pl->stage_maps[i], mbytes), "host-path map staging");
-        SHT_TRY(cudaMalloc((void**)&pl->stage_alm[i], abytes), "host-path alm staging");
-        SHT_TRY(cudaStreamCreateWithFlags(&pl->hstream[i], cudaStreamNonBlocking), "host-path stream");
+    cudaError_t e = cudaSuccess;
+    for (int i = 0; i < nb && e == cudaSuccess; ++i) {
+        e = cudaMalloc((void**)&pl->stage_maps[i], mbytes);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->stage_alm[i], abytes);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&pl->hstream[i], cudaStreamNonBlocking);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pl->hevent, cudaEventDisableTiming);
+    if (e != cudaSuccess) {                              // nothing half-built stays behind: the next call starts over
+        for (int i = 0; i < 4; ++i) {
+            if (pl->stage_maps[i]) { cudaFree(pl->stage_maps[i]); pl->stage_maps[i] = nullptr; }
+            if (pl->stage_alm[i]) { cudaFree(pl->stage_alm[i]); pl->stage_alm[i] = nullptr; }
+            if (pl->hstream[i]) { cudaStreamDestroy(pl->hstream[i]); pl->hstream[i] = nullptr; }
+        }
+        if (pl->hevent) { cudaEventDestroy(pl->hevent); pl->hevent = nullptr; }
+        return cuda_fail(pl, "host-path staging", e);
     }
     pl->host_ready = true;
     return SHT_OK;
@@ -436,6 +531,14 @@ static sht_status_t host_run(sht_plan_t pl, const double* in_host, double* out_h
     dh.kpad = pl->host_kpad;
     dh.nkg = dh.kpad / KG;
     const size_t f_slice = (size_t)d.nh * (d.lmax + 1) * d.ncomp * 2 * pl->host_kpad * 2;   // doubles per chunk workspace
+    // the chunk streams share the plan's workspace and lambda scratch with the device entries: wait for whatever the
+    // caller queued before (the host entries are synchronous calls anyway)
+    SHT_TRY(cudaDeviceSynchronize(), "host-path entry sync");
+    // staged mode: the lambda blocks of this direction are generated once, on the first chunk stream; the other
+    // streams wait for them and every chunk launches the contraction kernel only
+    SHT_TRY(launch_lambda_blocks(pl, dh, analysis, pl->hstream[0]), "lambda blocks");
+    SHT_TRY(cudaEventRecord(pl->hevent, pl->hstream[0]), "lambda event");
+    for (int i = 1; i < pl->host_nb; ++i) SHT_TRY(cudaStreamWaitEvent(pl->hstream[i], pl->hevent, 0), "lambda wait");
     int idx = 0;
     for (int k0 = 0; k0 < pl->nmaps; k0 += pl->host_chunk, ++idx) {
         const int b = idx % pl->host_nb;
@@ -447,8 +550,8 @@ static sht_status_t host_run(sht_plan_t pl, const double* in_host, double* out_h
         SHT_TRY(cudaMemcpyAsync(din, in_host + (size_t)k0 * in_elems, (size_t)kmaps * in_elems * sizeof(double),
                                 cudaMemcpyHostToDevice, st), "H2D");
         // staging buffers are indexed from the chunk start: pass k0 = 0
-        s = analysis ? analysis_chunk(pl, dh, dmaps, 0, dalm, 0, F, kmaps, false, st)
-                     : synthesis_chunk(pl, dh, dalm, 0, dmaps, 0, F, kmaps, nullptr, 0, st);
+        s = analysis ? analysis_chunk(pl, dh, dmaps, 0, dalm, 0, F, kmaps, false, st, 0, false)
+                     : synthesis_chunk(pl, dh, dalm, 0, dmaps, 0, F, kmaps, nullptr, 0, st, 0, false);
         if (s != SHT_OK) return s;
         SHT_TRY(cudaMemcpyAsync(out_host + (size_t)k0 * out_elems, dout, (size_t)kmaps * out_elems * sizeof(double),
                                 cudaMemcpyDeviceToHost, st), "D2H");

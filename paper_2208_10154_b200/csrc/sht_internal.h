@@ -111,13 +111,14 @@ struct sht_plan_s {
     long long launches;
     double* Fmap;                   // Alg. 2: folded T_m of the input maps (allocated on the first iterative call)
     double* upow;                   // Alg. 2: [nh][ncomp][kpad] uncovered ring power
+    bool iter_reserve_failed;       // the second workspace did not fit: Alg. 2 forms residual maps instead
     int iter_mode;                  // SHT_ITER_TM (default) / SHT_ITER_PIXEL / SHT_ITER_IMMEDIATE
     double* lam;                    // staged-lambda scratch (nullptr: fused generation inside the contraction kernels)
     size_t lam_bytes;
     int* lam_i0;                    // [analysis blocks] first 16-row block with a started recurrence
     int lam_mode;                   // SHT_LAMBDA_FUSED / SHT_LAMBDA_STAGED
     long long n_ablk, n_sblk;
-    int pol;                        // spin 2: 0 = E and B, 1 = E only, 2 = B only (set by the *_pol entries around a call)
+    bool ring_attr_set, resid_attr_set;   // dynamic shared-memory attributes of the ring kernels set on this plan's device
     char err[512];
     // host-entry staging (allocated on first use)
     double* stage_maps[4];
@@ -126,12 +127,14 @@ struct sht_plan_s {
     int host_nb;                    // chunks in flight in the host path (streams, staging buffers, workspace slices)
     int host_chunk;
     cudaStream_t hstream[4];
+    cudaEvent_t hevent;             // host path: lambda blocks of the call are ready
     bool host_ready;
     // optional per-stage timing (sht_plan_set_timing)
     bool timing;
-    int n_ev;
-    cudaEvent_t ev0[256], ev1[256];
-    int ev_stage[256];
+    int n_ev, cap_ev;               // brackets recorded since the last sht_plan_stage_ms / allocated slots (grown on demand)
+    long long ev_dropped;           // brackets lost because a slot could not be allocated (reported by sht_plan_stage_ms)
+    cudaEvent_t *ev0, *ev1;
+    int* ev_stage;
 };
 
 namespace sht {
@@ -146,9 +149,15 @@ cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F,
 cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps,
                                   const double* sub_from, int ksub0, cudaStream_t st);
 // Legendre stage (sht_legendre.cu)
+// pol: spin 2 only, 0 = E and B, SHT_POL_E / SHT_POL_B = that component alone (`alm` then holds one component);
+// gen_lambda = false: staged mode, the lambda scratch already holds this direction's blocks (host path: one generator
+// pass per call instead of one per chunk)
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                     bool accumulate, cudaStream_t st);
-cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st);
+                                     bool accumulate, cudaStream_t st, int pol = 0, bool gen_lambda = true);
+cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st,
+                                      int pol = 0, bool gen_lambda = true);
+// the lambda-block generator kernel of the staged mode on its own (no-op in fused mode)
+cudaError_t launch_lambda_blocks(sht_plan_s* pl, const DevicePlan& d, bool analysis, cudaStream_t st);
 // Alg. 3, the orders m .. m + nm - 1 at a time: tensor maps once per chunk, then per step analysis (alm += , da =
 // increment), synthesis of the increment into the cells of these orders of S, and the update of the residual workspace R
 cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA);
@@ -162,9 +171,10 @@ constexpr size_t LAM_ABLK_BYTES = 2 * 32 * 66 * 8;      // one analysis lambda b
 constexpr size_t LAM_SBLK_BYTES = 32 * 66 * 8;          // one synthesis lambda block: [32 l][66] doubles
 // spin 2 (sht_legendre_spin2.cu); the spin-0 launchers dispatch to these
 cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                           bool accumulate, cudaStream_t st);
+                                           bool accumulate, cudaStream_t st, int pol, bool gen_lambda);
 cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps,
-                                            cudaStream_t st);
+                                            cudaStream_t st, int pol, bool gen_lambda);
+cudaError_t launch_lambda_blocks_spin2(sht_plan_s* pl, const DevicePlan& d, bool analysis, cudaStream_t st);
 cudaError_t legendre_order_maps_spin2(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA);
 cudaError_t launch_legendre_analysis_order_spin2(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
                                                  int k0, int kmaps, int m, int nm, cudaStream_t st);

@@ -637,10 +637,24 @@ static size_t analysis_smem(int ntile)
 }
 static size_t synthesis_smem() { return (size_t)S_STAGES * S_STAGE_BYTES + 2 * S_STAGES * sizeof(uint64_t) + 4 * S_LC * sizeof(double2) + 64; }
 
-cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                     bool accumulate, cudaStream_t st)
+cudaError_t launch_lambda_blocks(sht_plan_s* pl, const DevicePlan& d, bool analysis, cudaStream_t st)
 {
-    if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st);
+    if (d.spin == 2) return launch_lambda_blocks_spin2(pl, d, analysis, st);
+    if (!(pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam)) return cudaSuccess;
+    if (analysis) {
+        k_lambda_blocks_analysis<<<dim3((unsigned)(d.ntile_max * d.nck_max), (unsigned)(d.lmax + 1)), 128, 0, st>>>(d, pl->lam, pl->lam_i0);
+        pl->launches++;
+    } else if (d.nst_max > 0) {
+        k_lambda_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
+        pl->launches++;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
+                                     bool accumulate, cudaStream_t st, int pol, bool gen_lambda)
+{
+    if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st, pol, gen_lambda);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const unsigned grid = (unsigned)((d.lmax + 1) * nkt);
     const size_t sm = analysis_smem(d.ntile_max);
@@ -649,10 +663,7 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
     CUtensorMap tmF;
     if ((e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, &tmF)) != cudaSuccess) return e;
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
-    if (staged) {
-        k_lambda_blocks_analysis<<<dim3((unsigned)(d.ntile_max * d.nck_max), (unsigned)(d.lmax + 1)), 128, 0, st>>>(d, pl->lam, pl->lam_i0);
-        pl->launches++;
-    }
+    if (staged && gen_lambda && (e = launch_lambda_blocks(pl, d, true, st)) != cudaSuccess) return e;
     k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0,
                                                        staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr, 0, 0, nullptr);
     pl->launches++;
@@ -696,9 +707,10 @@ cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d,
     return cudaGetLastError();
 }
 
-cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st)
+cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st,
+                                      int pol, bool gen_lambda)
 {
-    if (d.spin == 2) return launch_legendre_synthesis_spin2(pl, d, alm, F, k0, kmaps, st);
+    if (d.spin == 2) return launch_legendre_synthesis_spin2(pl, d, alm, F, k0, kmaps, st, pol, gen_lambda);
     const size_t sm = synthesis_smem();
     cudaError_t e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
@@ -707,10 +719,7 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
-    if (staged && d.nst_max > 0) {
-        k_lambda_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
-        pl->launches++;
-    }
+    if (staged && gen_lambda && (e = launch_lambda_blocks(pl, d, false, st)) != cudaSuccess) return e;
     k_legendre_synthesis<<<(d.lmax + 1) * nkt, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, 1);
     pl->launches++;
     return cudaGetLastError();

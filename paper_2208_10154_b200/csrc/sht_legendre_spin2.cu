@@ -629,42 +629,49 @@ static size_t synthesis2_smem()
     return (size_t)3 * S2_STAGE_BYTES + 8 * sizeof(uint64_t) + (size_t)4 * 2 * S2_LC * 3 * sizeof(double2) + 16;
 }
 
+cudaError_t launch_lambda_blocks_spin2(sht_plan_s* pl, const DevicePlan& d, bool analysis, cudaStream_t st)
+{
+    if (!(pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam)) return cudaSuccess;
+    if (analysis) {
+        k_fpm_blocks_analysis<<<dim3((unsigned)(d.ntile_max * d.nck_max), (unsigned)(d.lmax + 1)), 128, 0, st>>>(d, pl->lam);
+        pl->launches++;
+    } else if (d.nst_max > 0) {
+        k_fpm_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
+        pl->launches++;
+    }
+    return cudaGetLastError();
+}
+
 cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                           bool accumulate, cudaStream_t st)
+                                           bool accumulate, cudaStream_t st, int pol, bool gen_lambda)
 {
     const size_t sm = analysis2_smem(d.ntile_max);
-    auto kern = pl->pol == 1 ? k_legendre_analysis_spin2<1> : pl->pol == 2 ? k_legendre_analysis_spin2<2> : k_legendre_analysis_spin2<0>;
+    auto kern = pol == 1 ? k_legendre_analysis_spin2<1> : pol == 2 ? k_legendre_analysis_spin2<2> : k_legendre_analysis_spin2<0>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tmF;
     if ((e = make_tmap_F(d, F, P_KG, 2, &tmF)) != cudaSuccess) return e;
     const int nkt = (kmaps + P_KT - 1) / P_KT;
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
-    if (staged) {
-        k_fpm_blocks_analysis<<<dim3((unsigned)(d.ntile_max * d.nck_max), (unsigned)(d.lmax + 1)), 128, 0, st>>>(d, pl->lam);
-        pl->launches++;
-    }
+    if (staged && gen_lambda && (e = launch_lambda_blocks_spin2(pl, d, true, st)) != cudaSuccess) return e;
     kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, staged ? pl->lam : nullptr, 0, 0, nullptr);
     pl->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps,
-                                            cudaStream_t st)
+                                            cudaStream_t st, int pol, bool gen_lambda)
 {
     const size_t sm = synthesis2_smem();
-    auto kern = pl->pol == 1 ? k_legendre_synthesis_spin2<1> : pl->pol == 2 ? k_legendre_synthesis_spin2<2> : k_legendre_synthesis_spin2<0>;
+    auto kern = pol == 1 ? k_legendre_synthesis_spin2<1> : pol == 2 ? k_legendre_synthesis_spin2<2> : k_legendre_synthesis_spin2<0>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tmA;
-    if ((e = make_tmap_alm_spin2(d, alm, (long long)(k0 + kmaps), pl->pol ? 1 : 2, &tmA)) != cudaSuccess) return e;
+    if ((e = make_tmap_alm_spin2(d, alm, (long long)(k0 + kmaps), pol ? 1 : 2, &tmA)) != cudaSuccess) return e;
     const int nkt = (kmaps + P_KT - 1) / P_KT;
     const int npb = (d.nh + S2_PB - 1) / S2_PB;
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
-    if (staged && d.nst_max > 0) {
-        k_fpm_blocks_synthesis<<<dim3((unsigned)d.nst_max, (unsigned)d.npb, (unsigned)(d.lmax + 1)), 64, 0, st>>>(d, pl->lam);
-        pl->launches++;
-    }
+    if (staged && gen_lambda && (e = launch_lambda_blocks_spin2(pl, d, false, st)) != cudaSuccess) return e;
     kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, 1);
     pl->launches++;
     return cudaGetLastError();

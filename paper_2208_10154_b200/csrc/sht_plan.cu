@@ -638,10 +638,12 @@ extern "C" sht_status_t sht_plan_destroy(sht_plan_t pl)
     if (pl->upow) cudaFree(pl->upow);
     if (pl->lam) cudaFree(pl->lam);
     if (pl->lam_i0) cudaFree(pl->lam_i0);
-    for (int i = 0; i < 256; ++i) {
+    for (int i = 0; i < pl->cap_ev; ++i) {
         if (pl->ev0[i]) cudaEventDestroy(pl->ev0[i]);
         if (pl->ev1[i]) cudaEventDestroy(pl->ev1[i]);
     }
+    free(pl->ev0); free(pl->ev1); free(pl->ev_stage);
+    if (pl->hevent) cudaEventDestroy(pl->hevent);
     for (int i = 0; i < 4; ++i) {
         if (pl->stage_maps[i]) cudaFree(pl->stage_maps[i]);
         if (pl->stage_alm[i]) cudaFree(pl->stage_alm[i]);

@@ -1096,12 +1096,11 @@ static int ring_threads(size_t smem) { return smem <= (size_t)113 * 1024 ? RING_
 
 static cudaError_t ring_attr(sht_plan_s* pl)
 {
-    static bool attr_set = false;
-    if (attr_set) return cudaSuccess;
+    // the attribute belongs to the (function, device) pair: remembered per plan (a plan lives on one device)
+    if (pl->ring_attr_set) return cudaSuccess;
     cudaError_t e = cudaFuncSetAttribute(k_ring_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_ring_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, 224 * 1024);
-    if (e == cudaSuccess) attr_set = true;
-    (void)pl;
+    if (e == cudaSuccess) pl->ring_attr_set = true;
     return e;
 }
 
@@ -1140,9 +1139,9 @@ cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F,
                                  int kmaps, cudaStream_t st)
 {
     cudaError_t e = ring_attr(pl);
-    if (e == cudaSuccess) {
-        static bool set = false;
-        if (!set) { e = cudaFuncSetAttribute(k_ring_residual, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024); set = e == cudaSuccess; }
+    if (e == cudaSuccess && !pl->resid_attr_set) {
+        e = cudaFuncSetAttribute(k_ring_residual, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
+        pl->resid_attr_set = e == cudaSuccess;
     }
     if (e != cudaSuccess) return e;
     for (int c = RING_NCLASS - 1; c >= 0; --c) {

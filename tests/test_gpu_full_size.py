@@ -11,6 +11,12 @@ from paper_2208_10154_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-10
+# residual rms of Alg. 2, relative to the round's own value (reading G24): the residual is a difference of two
+# O(1) maps each carrying a rounding error of relative size eps_t <= 1e-10 (the transform tolerance), so by the triangle
+# inequality |rms_gpu - rms_ref| <= eps_t max|map|, i.e. relative to rms(n): eps_t max|map| / rms(n).  At config 5 the
+# maps have max ~ 5 and rms(2) ~ 1e-5: 1e-10 x 5 / 1e-5 = 5e-5 is what the transform tolerance alone would allow; the
+# kernels' actual eps_t is ~1e-14, and the bar is set 100x below the allowance.
+RMS_TOL = 5e-7
 
 
 def _sample_rings(nside):
@@ -44,7 +50,7 @@ def _m_slots(lmax, ms_wanted):
     return np.nonzero(np.isin(ms, ms_wanted))[0]
 
 
-def _run_config(cfg_id, ks):
+def _run_config(cfg_id, ks, lambda_mode=None):
     import torch
     from oracle import oracle as O
     from paper_2208_10154_b200.binding import Plan
@@ -53,6 +59,8 @@ def _run_config(cfg_id, ks):
     ncomp = 2 if spin == 2 else 1
     dev = torch.device("cuda:0")
     plan = Plan(nside, lmax, nmaps, spin)
+    if lambda_mode is not None:
+        plan.sht_plan_set_lambda_mode(lambda_mode)
     alm = torch.empty((nmaps, ncomp, plan.nalm), dtype=torch.complex128, device=dev)
     blk = 25
     for k0 in range(0, nmaps, blk):
@@ -111,14 +119,122 @@ def test_config5_transforms_sampled():
     _run_config(5, ks)
 
 
+@pytest.mark.parametrize("cfg_id,ks", [(3, [0, 999]), (4, [31, 999]), (5, [64, 199])])
+def test_full_size_fused_lambda_mode_sampled(cfg_id, ks):
+    """the same full-size sampled parity with the P_lm tiles generated inside the contraction kernels (SHT_LAMBDA_FUSED,
+    the north star's design; the default at these sizes is the staged mode), two maps sampled"""
+    from paper_2208_10154_b200.binding import SHT_LAMBDA_FUSED
+    _run_config(cfg_id, np.array(ks), lambda_mode=SHT_LAMBDA_FUSED)
+
+
+def test_config4_eb_split_sampled():
+    """sht_eb_split (eq. 19) at BASELINE.json configs[3] shapes: all 1000 (Q,U) pairs go through the
+    CUDA path; for two pairs the oracle analyses the pair in full, zeroes B and synthesises the sampled rings"""
+    import torch
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan, SHT_POL_E
+    c = inputs.CONFIGS[4]
+    nside, lmax, nmaps = c["nside"], c["lmax"], c["nmaps"]
+    dev = torch.device("cuda:0")
+    plan = Plan(nside, lmax, nmaps, 2)
+    alm = torch.empty((nmaps, 2, plan.nalm), dtype=torch.complex128, device=dev)
+    for k0 in range(0, nmaps, 50):
+        kk = np.arange(k0, min(nmaps, k0 + 50))
+        alm[k0:k0 + len(kk)] = torch.from_numpy(inputs.gaussian_alm(lmax, kk, c["seed"], 2)).to(dev)
+    maps = torch.empty((nmaps, 2, plan.npix), dtype=torch.float64, device=dev)
+    plan.sht_synthesis(alm, maps)
+    del alm
+    out = torch.full_like(maps, float("nan"))
+    plan.sht_eb_split(maps, out, SHT_POL_E)
+    torch.cuda.synchronize()
+    ks = [0, 999]
+    qu = maps[ks].cpu().numpy()
+    a = O.analysis(nside, lmax, qu, spin=2)
+    a[:, 1, :] = 0.0
+    rings = _sample_rings(nside)
+    pix = _ring_pixels(nside, rings)
+    ref = O.synthesis(nside, lmax, a, spin=2, rlist=rings)
+    got = out[ks].cpu().numpy()
+    assert np.isfinite(out).all()
+    e = inputs.rel_err(got[:, :, pix], ref[:, :, pix])
+    print("config 4 eb_split (E family): %.2e" % e)
+    assert e <= TOL
+    plan.destroy()
+
+
+def test_config5_iterative_vs_oracle_round_by_round():
+    """BASELINE.json configs[4] against the oracle at FULL size: nside 1024, lmax 2047, all 200 maps through
+    sht_analysis_iter (default mode: residual on the ring spectra, rms by Parseval), 3 Jacobi rounds (Alg. 2,
+    PAPER.md:302-345).  A chained oracle run costs 7 full transforms per map (the best part of an hour here), so each
+    round is checked on its own, which the oracle can do output by output: with a(n) the GPU's iterate after n rounds
+    (itself checked by the round before, a(0) by the plain analysis), the oracle forms r = map - synthesis(a(n)) on
+    every pixel (one full synthesis), its rms, and the sampled orders m of analysis(r); then
+        a(n+1)[m sampled] == a(n) + analysis(r)[m sampled]   to 1e-10 (north_star, reading G22), element by element,
+        rms(n) == oracle rms                                  to RMS_TOL relative to the round's OWN value (reading G24).
+    Map 199 (the ragged last k-tile: 200 = 3 x 64 + 8) in every round, map 0 in the first.  This covers what the small
+    cases cannot: the alias-free belt rings of k_ring_residual (N_r = 4096 > 2 lmax), the uncovered-power table of the
+    Parseval rms (bins m > lmax of the belt rings) and the recurrence-state table at this size."""
+    import torch
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan
+    c = inputs.CONFIGS[5]
+    nside, lmax, nmaps, niter = c["nside"], c["lmax"], c["nmaps"], c["niter"]
+    dev = torch.device("cuda:0")
+    plan = Plan(nside, lmax, nmaps, 0)
+    plan.sht_plan_reserve_iter()
+    alm_true = torch.empty((nmaps, 1, plan.nalm), dtype=torch.complex128, device=dev)
+    for k0 in range(0, nmaps, 25):
+        kk = np.arange(k0, min(nmaps, k0 + 25))
+        alm_true[k0:k0 + len(kk)] = torch.from_numpy(inputs.gaussian_alm(lmax, kk, c["seed"])).to(dev)
+    maps = torch.empty((nmaps, 1, plan.npix), dtype=torch.float64, device=dev)
+    plan.sht_synthesis(alm_true, maps)
+    del alm_true
+    msel = _sample_m(nside, lmax)
+    slots = _m_slots(lmax, msel)
+    iterates, rms_gpu = [], None
+    for n in range(niter + 1):                           # a(0) .. a(3): the entry run with 0 .. 3 rounds
+        a = torch.full((nmaps, 1, plan.nalm), float("nan"), dtype=torch.complex128, device=dev)
+        rms = torch.full((max(n, 1), nmaps), float("nan"), dtype=torch.float64, device=dev)
+        plan.sht_analysis_iter(maps, a, n, rms)
+        torch.cuda.synchronize()
+        assert torch.isfinite(a.real).all() and torch.isfinite(a.imag).all()
+        iterates.append(a)
+        rms_gpu = rms.cpu().numpy()
+    mp_all = {k: maps[k].cpu().numpy()[None] for k in (0, 199)}
+    # a(0): the plain analysis of the same maps, sampled orders
+    for k in (0, 199):
+        ref0 = O.analysis(nside, lmax, mp_all[k], mlist=msel)
+        assert inputs.rel_err(iterates[0][k].cpu().numpy()[None][:, :, slots], ref0[:, :, slots]) <= TOL
+    worst_a, worst_r = 0.0, 0.0
+    for n in range(niter):
+        ks = [0, 199] if n == 0 else [199]
+        a_n = np.stack([iterates[n][k].cpu().numpy() for k in ks])
+        mp = np.concatenate([mp_all[k] for k in ks])
+        res = mp - O.synthesis(nside, lmax, a_n)
+        rms_ref = np.sqrt(np.mean(res * res, axis=2))[:, 0]
+        da = O.analysis(nside, lmax, res, mlist=msel)
+        ref_next = a_n + da
+        got_next = np.stack([iterates[n + 1][k].cpu().numpy() for k in ks])
+        e_a = inputs.rel_err(got_next[:, :, slots], ref_next[:, :, slots])
+        e_r = float(np.max(np.abs(rms_gpu[n, ks] - rms_ref) / rms_ref))
+        print("config 5 round %d, maps %s: a_lm %.2e, rms %s (oracle %s), rel. dev. %.2e" % (n, ks, e_a, rms_gpu[n, ks], rms_ref, e_r))
+        worst_a, worst_r = max(worst_a, e_a), max(worst_r, e_r)
+        assert e_a <= TOL
+        assert e_r <= RMS_TOL
+    plan.destroy()
+
+
 def test_config5_iterative_composition():
-    """BASELINE.json configs[4]: 3 Jacobi iterations at nside 1024, lmax 2047, 200 maps.  The oracle needs ~7 full
-    transforms per map at this size (tens of minutes), so at full size the iterative entry is checked through
-    properties that hold at any size: it equals the composition a <- a + analysis(map - synthesis(a)) of the plain
-    entries (themselves oracle-checked at this size above), its rms output equals the rms of those residual maps, and
-    for this band-limited input (lmax = 2 nside - 1) the residual falls by more than 4x per round
-    (measured: ~8.7x).
-    The element-by-element comparison with the oracle's Alg. 2 runs at small sizes in test_gpu_parity.py."""
+    """BASELINE.json configs[4]: 3 Jacobi iterations at nside 1024, lmax 2047, 200 maps: properties of ALL 200 maps (the
+    oracle comparison above samples two).  The entry equals the composition a <- a + analysis(map - synthesis(a)) of the
+    plain entries; its Parseval rms equals the rms of those residual maps; and for this band-limited input
+    (lmax = 2 nside - 1) the iteration converges to the input a_lm.
+    Bounds and where they come from (reading G24): Alg. 2 is the stationary iteration e(n+1) = (I - A S) e(n) on
+    the error of a; with the constant weights of reading G4, A S differs from I by the quadrature error, and the oracle's
+    own runs at lmax = 2 nside - 1 (tests/test_oracle_iter.py, pinned there) show the residual rms falling 7.5x to 10x per
+    round.  Hence: rms(n+1) < rms(n) / 4 (a factor 2 below the slowest observed rate), and after 3 rounds an a_lm error
+    below 4^-3 = 1.6e-2 of the error of the plain analysis -- asserted as < 1e-2 (measured on B200: 1.5e-3; a bound of
+    1e-3 would demand a rate of 10x per round, which the method does not have)."""
     import torch
     from paper_2208_10154_b200.binding import Plan
     c = inputs.CONFIGS[5]
@@ -152,8 +268,11 @@ def test_config5_iterative_composition():
     rms_ref = torch.stack(rms_ref)
     scale = a.abs().amax(dim=(1, 2), keepdim=True)
     assert float(((alm_it - a).abs() / scale).max()) <= 1e-13
-    # the entry forms the residual on the ring spectra and gets the rms by Parseval; the composition squares pixels
-    assert float(((rms - rms_ref).abs() / rms_ref).max()) <= 1e-8
+    # two CUDA routes to the same rms (Parseval on the ring spectra / squares of the residual pixels): both carry the
+    # rounding of a residual formed from O(1) terms, bounded as in reading G24
+    dev_rel = float(((rms - rms_ref).abs() / rms_ref).max())
+    print("config 5: Parseval rms vs pixel rms, worst relative deviation %.2e" % dev_rel)
+    assert dev_rel <= RMS_TOL
     r = rms.cpu().numpy()
     assert np.all(r[1:] < 0.25 * r[:-1]), r[:, :3]
     # converges to the input a_lm (fixed point, paper: errors "negligible" when lmax <= 2 nside)
