@@ -100,13 +100,19 @@ struct sht_plan_s {
     double* F;                      // workspace, layout above
     size_t F_bytes;
     size_t table_bytes;
-    void* dev_allocs[32];
+    void* dev_allocs[48];
     int n_allocs;
     // ring-kernel launch classes: rings grouped by the dynamic shared memory their CTA needs
     int* class_rings[sht::RING_NCLASS];     // device lists of ring-pair indices
     int class_count[sht::RING_NCLASS];
     int class_ktmin[sht::RING_NCLASS];      // smallest kt in the class (decides grid.x)
     size_t class_smem[sht::RING_NCLASS];
+    // belt fast path (sht_ring_pow2.cu): ring pairs belt_first .. belt_first + belt_count - 1 have length 2^belt_logn
+    // (belt_logn = 0: none); class_*_nb are the launch classes of the general kernels without those pairs
+    int belt_logn, belt_first, belt_count, p2_syn_occ;
+    int* class_rings_nb[sht::RING_NCLASS];
+    int class_count_nb[sht::RING_NCLASS];
+    int class_ktmin_nb[sht::RING_NCLASS];
     int sm_count;
     long long launches;
     double* Fmap;                   // Alg. 2: folded T_m of the input maps (allocated on the first iterative call)
@@ -148,6 +154,9 @@ cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F,
 // maps of the chunk are maps[k0 .. k0+kmaps); if sub_from != nullptr the output is sub_from[ksub0 + k] - synthesis
 cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps,
                                   const double* sub_from, int ksub0, cudaStream_t st);
+// belt fast path (sht_ring_pow2.cu)
+cudaError_t launch_ring_analysis_belt(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st);
+cudaError_t launch_ring_synthesis_belt(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps, cudaStream_t st);
 // Legendre stage (sht_legendre.cu)
 // pol: spin 2 only, 0 = E and B, SHT_POL_E / SHT_POL_B = that component alone (`alm` then holds one component);
 // gen_lambda = false: staged mode, the lambda scratch already holds this direction's blocks (host path: one generator

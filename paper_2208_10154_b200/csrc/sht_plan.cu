@@ -583,6 +583,26 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             if (upload(pl, lists[c], &dp) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
             pl->class_rings[c] = const_cast<int*>(dp);
         }
+        // belt fast path: nside a power of two with a ring length the compiled transforms cover
+        pl->belt_logn = 0; pl->belt_first = nside - 1; pl->belt_count = nside + 1; pl->p2_syn_occ = 2;
+        if ((nside & (nside - 1)) == 0 && 4 * nside >= 512 && 4 * nside <= 2048) {
+            int a = 0;
+            while ((1 << a) < 4 * nside) ++a;
+            pl->belt_logn = a;
+        }
+        for (int c = 0; c < RING_NCLASS; ++c) {
+            std::vector<int> nb;
+            pl->class_ktmin_nb[c] = 16;
+            for (int p : lists[c]) {
+                if (pl->belt_logn && p >= pl->belt_first) continue;
+                nb.push_back(p);
+                if (rings[p].kt < pl->class_ktmin_nb[c]) pl->class_ktmin_nb[c] = rings[p].kt;
+            }
+            pl->class_count_nb[c] = (int)nb.size();
+            const int* dp = nullptr;
+            if (upload(pl, nb, &dp) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+            pl->class_rings_nb[c] = const_cast<int*>(dp);
+        }
     }
 
     // ---- workspace: T_m^k(theta) for one chunk of maps ----------------------------------------

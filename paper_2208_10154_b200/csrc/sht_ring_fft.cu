@@ -1109,11 +1109,17 @@ cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const doub
 {
     cudaError_t e = ring_attr(pl);
     if (e != cudaSuccess) return e;
+    // the belt (two thirds of the pixels) goes through the fast path, except when the uncovered power is wanted
+    const bool belt = pl->belt_logn != 0 && upow == nullptr;
+    if (belt && (e = launch_ring_analysis_belt(pl, d, maps, F, k0, kmaps, st)) != cudaSuccess) return e;
+    int* const* lists = belt ? pl->class_rings_nb : pl->class_rings;
+    const int* count = belt ? pl->class_count_nb : pl->class_count;
+    const int* ktmin = belt ? pl->class_ktmin_nb : pl->class_ktmin;
     // longest rings first: their CTAs are the slowest
     for (int c = RING_NCLASS - 1; c >= 0; --c) {
-        if (pl->class_count[c] == 0) continue;
-        dim3 grid((kmaps + pl->class_ktmin[c] - 1) / pl->class_ktmin[c], pl->class_count[c], d.ncomp);
-        k_ring_analysis<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c], st>>>(d, pl->class_rings[c], maps, F, k0, kmaps, upow);
+        if (count[c] == 0) continue;
+        dim3 grid((kmaps + ktmin[c] - 1) / ktmin[c], count[c], d.ncomp);
+        k_ring_analysis<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c], st>>>(d, lists[c], maps, F, k0, kmaps, upow);
         pl->launches++;
     }
     return cudaGetLastError();
@@ -1124,10 +1130,15 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
 {
     cudaError_t e = ring_attr(pl);
     if (e != cudaSuccess) return e;
+    const bool belt = pl->belt_logn != 0 && sub_from == nullptr;
+    if (belt && (e = launch_ring_synthesis_belt(pl, d, F, maps, k0, kmaps, st)) != cudaSuccess) return e;
+    int* const* lists = belt ? pl->class_rings_nb : pl->class_rings;
+    const int* count = belt ? pl->class_count_nb : pl->class_count;
+    const int* ktmin = belt ? pl->class_ktmin_nb : pl->class_ktmin;
     for (int c = RING_NCLASS - 1; c >= 0; --c) {
-        if (pl->class_count[c] == 0) continue;
-        dim3 grid((kmaps + pl->class_ktmin[c] - 1) / pl->class_ktmin[c], pl->class_count[c], d.ncomp);
-        k_ring_synthesis<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c], st>>>(d, pl->class_rings[c], F, maps, k0, kmaps, sub_from, ksub0);
+        if (count[c] == 0) continue;
+        dim3 grid((kmaps + ktmin[c] - 1) / ktmin[c], count[c], d.ncomp);
+        k_ring_synthesis<<<grid, ring_threads(pl->class_smem[c]), pl->class_smem[c], st>>>(d, lists[c], F, maps, k0, kmaps, sub_from, ksub0);
         pl->launches++;
     }
     return cudaGetLastError();

@@ -1,0 +1,583 @@
+// sht_ring_pow2.cu -- subsystem (1), fast path for the equatorial belt: the 2 nside + 1 rings of 4 nside pixels hold two
+// thirds of all pixels, and for nside a power of two their length N = 4 nside is a power of two.
+//
+// Same mathematics as sht_ring_fft.cu (eq. 2 row 3 and App. A.1 :412-416 for the analysis side,
+// :66-70 eq. 4 and :78 for the synthesis side); what differs is how the bytes move and how the transform is laid out:
+//   * persistent CTAs (one per SM) loop over work items (ring pair, component, KT maps);
+//   * analysis input: the map rows of the next items are fetched by 1-D bulk copies (cp.async.bulk, mbarrier
+//     complete_tx) into a double-buffered staging area while the current item is transformed; analysis output: the
+//     folded T_m lines are staged in shared memory and written by tiled TMA stores (cp.async.bulk.tensor) -- no thread
+//     ever waits on a global load or issues a global store;
+//   * synthesis input: the T_m lines arrive by tiled TMA loads through a ring of shared-memory slots;
+//   * the length-N transform is compiled for its length (N = R1 R2 R3, radices 16 / 8, three passes in registers, no
+//     divisions, no runtime radix list) as decimation in time on the analysis side -- first pass straight from the
+//     staged rows, bins come out in NATURAL order, so the FFT mapping reads shared memory contiguously -- and as the
+//     exact adjoint network (decimation in frequency) on the synthesis side: bins go in in natural order, the last pass
+//     writes the pixels of the two rings coalesced.
+// The north and the south ring of a pair are the real and the imaginary part of one complex sequence, as in the
+// general kernels.  Twiddles: one table value per butterfly, the other powers by multiplication.
+#include "sht_legendre_common.cuh"
+
+namespace sht {
+
+namespace p2 {
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b)
+{
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+
+// multiply by exp(-+ 2 pi i k / 16), k compile-time (- forward, + if INV)
+template <int K, bool INV>
+__device__ __forceinline__ double2 mul_w16(double2 a)
+{
+    constexpr int k = K & 15;
+    constexpr double C1 = 0.92387953251128675613, S1 = 0.38268343236508977173, H = 0.70710678118654752440;
+    if constexpr (k == 0) return a;
+    else if constexpr (k == 4) return INV ? make_double2(-a.y, a.x) : make_double2(a.y, -a.x);
+    else if constexpr (k == 8) return make_double2(-a.x, -a.y);
+    else if constexpr (k == 12) return INV ? make_double2(a.y, -a.x) : make_double2(-a.y, a.x);
+    else {
+        // w = c - i s (forward), c + i s (inverse), angle 2 pi k / 16
+        constexpr double c = (k == 1 || k == 15) ? C1 : (k == 2 || k == 14) ? H : (k == 3 || k == 13) ? S1
+                           : (k == 5 || k == 11) ? -S1 : (k == 6 || k == 10) ? -H : -C1;
+        constexpr double s0 = (k == 1 || k == 7) ? S1 : (k == 2 || k == 6) ? H : (k == 3 || k == 5) ? C1
+                            : (k == 9 || k == 15) ? -S1 : (k == 10 || k == 14) ? -H : -C1;       // sin(2 pi k / 16)
+        constexpr double sn = INV ? s0 : -s0;                                                 // imaginary part of w
+        return make_double2(fma(a.x, c, -(a.y * sn)), fma(a.x, sn, a.y * c));
+    }
+}
+
+template <bool INV>
+__device__ __forceinline__ void bfly4(double2& x0, double2& x1, double2& x2, double2& x3)
+{
+    const double2 v0 = cadd(x0, x2), v1 = csub(x0, x2), v2 = cadd(x1, x3), dd = csub(x1, x3);
+    const double2 v3 = INV ? make_double2(-dd.y, dd.x) : make_double2(dd.y, -dd.x);      // (-+ i)(x1 - x3)
+    x0 = cadd(v0, v2); x1 = cadd(v1, v3); x2 = csub(v0, v2); x3 = csub(v1, v3);
+}
+
+// R-point DFT in registers, natural order in and out: u[k] <- sum_n u[n] exp(-+ 2 pi i n k / R)
+template <int R, bool INV>
+__device__ __forceinline__ void dft(double2 (&u)[R])
+{
+    static_assert(R == 8 || R == 16, "radix");
+    if constexpr (R == 16) {
+        // n = a + 4 r, k = s + 4 q:  X[s + 4 q] = sum_a w4^{a q} { w16^{a s} sum_r x[a + 4 r] w4^{r s} }
+        double2 t[4][4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            double2 v0 = u[a], v1 = u[a + 4], v2 = u[a + 8], v3 = u[a + 12];
+            bfly4<INV>(v0, v1, v2, v3);
+            t[a][0] = v0;
+            t[a][1] = a == 0 ? v1 : a == 1 ? mul_w16<1, INV>(v1) : a == 2 ? mul_w16<2, INV>(v1) : mul_w16<3, INV>(v1);
+            t[a][2] = a == 0 ? v2 : a == 1 ? mul_w16<2, INV>(v2) : a == 2 ? mul_w16<4, INV>(v2) : mul_w16<6, INV>(v2);
+            t[a][3] = a == 0 ? v3 : a == 1 ? mul_w16<3, INV>(v3) : a == 2 ? mul_w16<6, INV>(v3) : mul_w16<9, INV>(v3);
+        }
+#pragma unroll
+        for (int s = 0; s < 4; ++s) {
+            double2 w0 = t[0][s], w1 = t[1][s], w2 = t[2][s], w3 = t[3][s];
+            bfly4<INV>(w0, w1, w2, w3);
+            u[s] = w0; u[s + 4] = w1; u[s + 8] = w2; u[s + 12] = w3;
+        }
+    } else {
+        // n = a + 2 r, k = s + 4 q:  X[s + 4 q] = sum_a (-1)^{a q} { w8^{a s} sum_r x[a + 2 r] w4^{r s} }
+        double2 e0 = u[0], e1 = u[2], e2 = u[4], e3 = u[6];
+        double2 o0 = u[1], o1 = u[3], o2 = u[5], o3 = u[7];
+        bfly4<INV>(e0, e1, e2, e3);
+        bfly4<INV>(o0, o1, o2, o3);
+        o1 = mul_w16<2, INV>(o1); o2 = mul_w16<4, INV>(o2); o3 = mul_w16<6, INV>(o3);
+        u[0] = cadd(e0, o0); u[4] = csub(e0, o0);
+        u[1] = cadd(e1, o1); u[5] = csub(e1, o1);
+        u[2] = cadd(e2, o2); u[6] = csub(e2, o2);
+        u[3] = cadd(e3, o3); u[7] = csub(e3, o3);
+    }
+}
+
+// u[k] *= w^k, k = 1 .. R-1: the powers by multiplication, w^k = w^{hb(k)} w^{k - hb(k)}, hb = highest bit (depth <= 4)
+template <int R>
+__device__ __forceinline__ void mul_powers(double2 (&u)[R], double2 w)
+{
+    double2 pw[R];
+    pw[1] = w;
+#pragma unroll
+    for (int k = 2; k < R; ++k) {
+        const int hb = k >= 8 ? 8 : k >= 4 ? 4 : 2;
+        pw[k] = (k == hb) ? cmul(pw[k / 2], pw[k / 2]) : cmul(pw[hb], pw[k - hb]);
+    }
+#pragma unroll
+    for (int k = 1; k < R; ++k) u[k] = cmul(u[k], pw[k]);
+}
+
+// transform geometry of a ring length N = 2^LOGN = R1 R2 R3
+template <int LOGN>
+struct Geo {
+    static constexpr int N = 1 << LOGN;
+    static constexpr int R1 = LOGN >= 10 ? 16 : 8;       // 512 = 8.8.8, 1024 = 16.8.8, 2048 = 16.16.8, 4096 = 16.16.16
+    static constexpr int R2 = LOGN >= 11 ? 16 : 8;
+    static constexpr int R3 = LOGN >= 12 ? 16 : 8;
+    static constexpr int LR1 = R1 == 16 ? 4 : 3, LR2 = R2 == 16 ? 4 : 3, LR3 = R3 == 16 ? 4 : 3;
+    static_assert(R1 * R2 * R3 == N, "radix split");
+    // shared-memory position of element p: one element of padding per R1 and one more per R1 R2 elements makes all
+    // three passes free of bank conflicts (16-byte elements, quarter-warp phases)
+    static constexpr int NPAD = N + N / R1 + N / (R1 * R2);
+    __device__ static __forceinline__ int phys(int p) { return p + (p >> LR1) + (p >> (LR1 + LR2)); }
+};
+
+// per-map buffer stride (elements): = 8 / KT mod 8, so that the KT maps a quarter-warp touches in the FFT mapping fall
+// into different bank groups
+template <int LOGN, int KT>
+__host__ __device__ constexpr int buf_stride()
+{
+    constexpr int np = Geo<LOGN>::NPAD, want = (8 / KT) & 7;
+    return np + ((want - (np & 7)) & 7);
+}
+
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int NKEEP>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(NKEEP) : "memory"); }
+template <int NKEEP>
+__device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(NKEEP) : "memory"); }
+__device__ __forceinline__ void tma_store_5d(const CUtensorMap* map, const void* src, int c0, int c1, int c2, int c3, int c4)
+{
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];"
+                 ::"l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2, int c3, int c4)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+        : "memory");
+}
+
+constexpr int NT = 256;                                  // threads per CTA (one CTA per SM)
+
+// work item -> (ring pair, component, first map of the KT maps)
+struct Item {
+    int p, comp, kfirst;
+};
+__device__ __forceinline__ Item decode_item(long long it, int nkp, int ncomp, int p_first, int kt)
+{
+    const int kp = (int)(it % nkp);
+    const long long r = it / nkp;
+    Item o;
+    o.comp = (int)(r % ncomp);
+    o.p = p_first + (int)(r / ncomp);
+    o.kfirst = kp * kt;
+    return o;
+}
+
+}  // namespace p2
+
+// ------------------------------------------------------------------------------------------------
+// analysis: maps -> F for the belt ring pairs p_first .. p_first + npairs - 1 (all of length N = 2^LOGN)
+// shared memory: [2 input buffers: KT maps x (north row, south row) of N doubles][KT transform buffers][2 output slots]
+// ------------------------------------------------------------------------------------------------
+template <int LOGN, int KT>
+__global__ void __launch_bounds__(p2::NT, 1)
+k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const double* __restrict__ maps, int k0, int kmaps,
+                   int p_first, int npairs, int planes)
+{
+    using namespace p2;
+    using G = Geo<LOGN>;
+    constexpr int N = G::N, R1 = G::R1, R2 = G::R2, R3 = G::R3;
+    constexpr int TPM = NT / KT;                          // threads per map in the passes
+    constexpr int MB = NT / KT;                           // orders m per mapping sweep (one TMA store box)
+    constexpr int BS = buf_stride<LOGN, KT>();
+    constexpr int IN_DOUBLES = KT * 2 * N;                // one input buffer
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double* in_buf = reinterpret_cast<double*>(smem_raw);
+    double2* tr = reinterpret_cast<double2*>(smem_raw + (size_t)2 * IN_DOUBLES * 8);
+    double2* out = tr + KT * BS;                          // 2 slots of MB * 2 * KT elements
+    uint64_t* full = reinterpret_cast<uint64_t*>(out + 2 * MB * 2 * KT);
+
+    const int tid = threadIdx.x;
+    const int nkp = (kmaps + KT - 1) / KT;
+    const long long nitems = (long long)npairs * d.ncomp * nkp;
+    // layout of an output slot = layout of the TMA box: [h][m][map] (planes) or [m][h][map]
+    const int out_hs = planes ? MB : 1, out_ms = planes ? 1 : 2;
+    const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
+
+    if (tid == 0) {
+        mbar_init(full + 0, 1); mbar_init(full + 1, 1);
+        fence_barrier_init();
+        tma_prefetch_desc(&tmF);
+    }
+    __syncthreads();
+
+    // the rows of one item: KT maps x (north, south); a map past kmaps is replaced by the last valid one (its workspace
+    // column is padding: it only has to stay finite)
+    auto issue_loads = [&](long long it, int buf) {
+        const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
+        const RingPair& rp = d.rings[w.p];
+        const bool eq = rp.start_s < 0;
+        mbar_arrive_expect_tx(full + buf, (uint32_t)(KT * (eq ? 1 : 2) * N * 8));
+#pragma unroll
+        for (int kk = 0; kk < KT; ++kk) {
+            const int k = min(w.kfirst + kk, kmaps - 1);
+            const double* mp = maps + ((size_t)(k0 + k) * d.ncomp + w.comp) * d.npix;
+            double* dst = in_buf + (size_t)buf * IN_DOUBLES + kk * 2 * N;
+            bulk_load(dst, mp + rp.start_n, N * 8, full + buf);
+            if (!eq) bulk_load(dst + N, mp + rp.start_s, N * 8, full + buf);
+        }
+    };
+    if (tid == 0) {
+        if ((long long)blockIdx.x < nitems) issue_loads(blockIdx.x, 0);
+        if ((long long)blockIdx.x + gridDim.x < nitems) issue_loads((long long)blockIdx.x + gridDim.x, 1);
+    }
+
+    const int kkp = tid / TPM, tm = tid - kkp * TPM;      // passes: map and thread inside the map
+    const int kkm = tid & (KT - 1), mi = tid / KT;        // mapping: map (fastest) and order inside the sweep
+    int li = 0, nstore = 0;
+    for (long long it = blockIdx.x; it < nitems; it += gridDim.x, ++li) {
+        const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
+        const RingPair rp = d.rings[w.p];
+        const bool equator = rp.start_s < 0;
+        const double2* __restrict__ tw2 = d.tw + rp.tw_off;          // W_{2N}^j; W_N^e = tw2[2 e]
+        const int buf = li & 1;
+        mbar_wait(full + buf, (li >> 1) & 1);
+        const double* rows = in_buf + (size_t)buf * IN_DOUBLES + kkp * 2 * N;
+        double2* trk = tr + kkp * BS;
+
+        // ---- pass A: R1-point transforms over n1 (input stride N / R1), twiddle W_N^{n2 k1}, R1 consecutive positions
+        for (int j = tm; j < N / R1; j += TPM) {
+            double2 u[R1];
+#pragma unroll
+            for (int r = 0; r < R1; ++r) {
+                u[r].x = rows[j + r * (N / R1)];
+                u[r].y = equator ? 0.0 : rows[N + j + r * (N / R1)];
+            }
+            dft<R1, false>(u);
+            mul_powers<R1>(u, __ldg(tw2 + 2 * j));
+            const int B = (j >> G::LR3) + R2 * (j & (R3 - 1));       // n1' + R2 n2'
+            double2* dst = trk + R1 * B + B + (j & (R3 - 1));        // phys(R1 B + k1) = R1 B + k1 + B + n2'
+#pragma unroll
+            for (int k = 0; k < R1; ++k) dst[k] = u[k];
+        }
+        __syncthreads();
+        // the input buffer is free: fetch the rows of the item after the next one
+        if (tid == 0 && it + 2LL * gridDim.x < nitems) issue_loads(it + 2LL * gridDim.x, buf);
+
+        // ---- pass B: R2-point transforms over n1' at positions k1 + R1 t + R1 R2 n2', twiddle W_{R2 R3}^{n2' k1'}
+        for (int wq = tm; wq < N / R2; wq += TPM) {
+            const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
+            double2* base = trk + k1 + (R1 * R2 + R2 + 1) * n2p;
+            double2 u[R2];
+#pragma unroll
+            for (int t = 0; t < R2; ++t) u[t] = base[(R1 + 1) * t];
+            dft<R2, false>(u);
+            mul_powers<R2>(u, __ldg(tw2 + 2 * R1 * n2p));
+#pragma unroll
+            for (int t = 0; t < R2; ++t) base[(R1 + 1) * t] = u[t];
+        }
+        __syncthreads();
+        // ---- pass C: R3-point transforms over n2' at positions k1 + R1 k1' + R1 R2 t; bin k1 + R1 k1' + R1 R2 k2' in place
+        for (int wq = tm; wq < N / R3; wq += TPM) {
+            const int k1 = wq & (R1 - 1), k1p = wq >> G::LR1;
+            double2* base = trk + k1 + (R1 + 1) * k1p;
+            double2 u[R3];
+#pragma unroll
+            for (int t = 0; t < R3; ++t) u[t] = base[(R1 * R2 + R2 + 1) * t];
+            dft<R3, false>(u);
+#pragma unroll
+            for (int t = 0; t < R3; ++t) base[(R1 * R2 + R2 + 1) * t] = u[t];
+        }
+        __syncthreads();
+
+        // ---- FFT mapping: order m -> bin m mod N, phase, fold; lines leave by TMA store
+        const int mlim = rp.mlim;
+        const double2* trm = tr + kkm * BS;
+        const int kg = w.kfirst / KG, csel = (w.kfirst % KG) / KT;
+        for (int m0 = 0; m0 < mlim; m0 += MB, ++nstore) {
+            const int m = m0 + mi;
+            const int b = m & (N - 1), bc = (N - b) & (N - 1);
+            const double2 A = trm[G::phys(b)], Bv = trm[G::phys(bc)];
+            // G_north = (A + conj B) / 2, G_south = (A - conj B) / (2 i)
+            const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
+            const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
+            double2 ph = make_double2(dsig, 0.0);
+            if (rp.shift) {                               // e^{-i m phi0}, phi0 = pi / N
+                ph = __ldg(tw2 + (m & (2 * N - 1)));
+                ph.x *= dsig; ph.y *= dsig;
+            }
+            double2 E, O;
+            if (equator) { E = cmul(ph, gn); O = make_double2(0.0, 0.0); }
+            else { E = cmul(ph, cadd(gn, gs)); O = cmul(ph, csub(gn, gs)); }
+            if (w.comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }      // i U
+            double2* slot = out + (nstore & 1) * (MB * 2 * KT);
+            slot[(mi * out_ms) * KT + kkm] = E;
+            slot[(out_hs + mi * out_ms) * KT + kkm] = O;
+            fence_async_smem();
+            if (tid == 0) bulk_wait_read<0>();            // the store that used the other slot has read it
+            __syncthreads();
+            if (tid == 0) {
+                if (planes) tma_store_5d(&tmF, slot, 0, m0, 2 * w.comp, csel, w.p * d.nkg + kg);
+                else tma_store_5d(&tmF, slot, 0, csel, 2 * w.comp, m0, w.p * d.nkg + kg);
+                bulk_commit();
+            }
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
+// ------------------------------------------------------------------------------------------------
+// synthesis: F (even / odd sums of the Legendre synthesis) -> maps for the belt ring pairs.
+// shared memory: [KT transform buffers][NSL input slots of MB orders][mbarriers]
+// The ring spectrum of the packed sequence z = north + i south is accumulated cell by cell: order m adds
+// (w_m / 2)(d_n + i d_s) to bin m mod N and (w_m / 2)(conj d_n + i conj d_s) to bin -m mod N, d = e^{+i m phi0} T_m
+// (eq. 4; at the self-conjugate bins 0 and N/2 the two add up to the real parts, reading G8).
+// ------------------------------------------------------------------------------------------------
+template <int LOGN, int KT, int NSL>
+__global__ void __launch_bounds__(p2::NT, 1)
+k_ring_synthesis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ maps, int k0, int kmaps,
+                    int p_first, int npairs, int planes)
+{
+    using namespace p2;
+    using G = Geo<LOGN>;
+    constexpr int N = G::N, R1 = G::R1, R2 = G::R2, R3 = G::R3;
+    constexpr int TPM = NT / KT, MB = NT / KT;
+    constexpr int BS = buf_stride<LOGN, KT>();
+    constexpr int SLOT = MB * 2 * KT;                     // double2 per input slot
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* in_slots = reinterpret_cast<double2*>(smem_raw);
+    double2* tr = in_slots + NSL * SLOT;
+    uint64_t* full = reinterpret_cast<uint64_t*>(tr + KT * BS);
+
+    const int tid = threadIdx.x;
+    const int nkp = (kmaps + KT - 1) / KT;
+    const long long nitems = (long long)npairs * d.ncomp * nkp;
+    const int in_hs = planes ? MB : 1, in_ms = planes ? 1 : 2;
+    if (tid == 0) {
+        for (int s = 0; s < NSL; ++s) mbar_init(full + s, 1);
+        fence_barrier_init();
+        tma_prefetch_desc(&tmF);
+    }
+    __syncthreads();
+
+    // producer state (thread 0): the flattened sequence of (item, chunk) this CTA consumes, NSL chunks ahead
+    long long pit = blockIdx.x;
+    int pm0 = 0, pmlim = 0, pslot = 0;
+    Item pw{0, 0, 0};
+    auto producer_begin_item = [&]() {
+        if (pit < nitems) { pw = decode_item(pit, nkp, d.ncomp, p_first, KT); pmlim = d.rings[pw.p].mlim; pm0 = 0; }
+    };
+    auto produce_one = [&]() {                            // issue the next chunk if there is one
+        if (pit >= nitems) return;
+        mbar_arrive_expect_tx(full + pslot, SLOT * 16);
+        const int kg = pw.kfirst / KG, csel = (pw.kfirst % KG) / KT;
+        if (planes) tma_load_5d(in_slots + pslot * SLOT, &tmF, full + pslot, 0, pm0, 2 * pw.comp, csel, pw.p * d.nkg + kg);
+        else tma_load_5d(in_slots + pslot * SLOT, &tmF, full + pslot, 0, csel, 2 * pw.comp, pm0, pw.p * d.nkg + kg);
+        pslot = pslot + 1 == NSL ? 0 : pslot + 1;
+        pm0 += MB;
+        if (pm0 >= pmlim) { pit += gridDim.x; producer_begin_item(); }
+    };
+    if (tid == 0) {
+        producer_begin_item();
+        for (int s = 0; s < NSL; ++s) produce_one();
+    }
+
+    const int kkp = tid / TPM, tm = tid - kkp * TPM;
+    const int kkm = tid & (KT - 1), mi = tid / KT;
+    int cslot = 0; uint32_t cphase = 0;
+    for (long long it = blockIdx.x; it < nitems; it += gridDim.x) {
+        const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
+        const RingPair rp = d.rings[w.p];
+        const bool equator = rp.start_s < 0;
+        const double2* __restrict__ tw2 = d.tw + rp.tw_off;
+        for (int i = tid; i < KT * BS; i += NT) tr[i] = make_double2(0.0, 0.0);
+        __syncthreads();
+        // ---- inverse FFT mapping: accumulate the ring spectrum
+        const int mlim = rp.mlim;
+        double2* trm = tr + kkm * BS;
+        for (int m0 = 0; m0 < mlim; m0 += MB) {
+            mbar_wait(full + cslot, cphase);
+            const double2* slot = in_slots + cslot * SLOT;
+            const int m = m0 + mi;
+            const bool live = m < mlim;
+            double2 zd = make_double2(0.0, 0.0), zc = zd;
+            if (live) {
+                const double2 e = slot[(mi * in_ms) * KT + kkm], o = slot[(in_hs + mi * in_ms) * KT + kkm];
+                double2 fn = cadd(e, o), fs = csub(e, o);                        // stored as (even, odd) sums
+                if (w.comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }   // U = -i (iU)
+                if (equator) fs = make_double2(0.0, 0.0);
+                double2 ph = make_double2(1.0, 0.0);
+                if (rp.shift) { ph = __ldg(tw2 + (m & (2 * N - 1))); ph.y = -ph.y; }
+                const double wgt = (m == 0) ? 0.5 : 1.0;
+                ph.x *= wgt; ph.y *= wgt;
+                const double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
+                zd = make_double2(dn.x - ds.y, dn.y + ds.x);                     // d_n + i d_s
+                zc = make_double2(dn.x + ds.y, ds.x - dn.y);                     // conj d_n + i conj d_s
+            }
+            const int b1 = m & (N - 1), b2 = (N - b1) & (N - 1);
+            // two orders of one chunk meet in a bin only if m + m' = 0 mod N for some pair of the chunk
+            const bool clash = ((2 * m0 + N - 1) / N) * N <= 2 * m0 + 2 * MB - 2;
+            if (live) { double2* c1 = trm + G::phys(b1); *c1 = cadd(*c1, zd); }
+            if (clash) __syncthreads();
+            if (live) { double2* c2 = trm + G::phys(b2); *c2 = cadd(*c2, zc); }
+            __syncthreads();                              // slot consumed (and bins of this chunk settled)
+            if (tid == 0) produce_one();
+            if (++cslot == NSL) { cslot = 0; cphase ^= 1; }
+        }
+        double2* trk = tr + kkp * BS;
+        // ---- pass C^-1: inverse R3-point transforms over k2', then the conjugate twiddle W_{R2 R3}^{-n2' k1'}
+        for (int wq = tm; wq < N / R3; wq += TPM) {
+            const int k1 = wq & (R1 - 1), k1p = wq >> G::LR1;
+            double2* base = trk + k1 + (R1 + 1) * k1p;
+            double2 u[R3];
+#pragma unroll
+            for (int t = 0; t < R3; ++t) u[t] = base[(R1 * R2 + R2 + 1) * t];
+            dft<R3, true>(u);
+            double2 wv = __ldg(tw2 + 2 * R1 * k1p);       // W_N^{R1 k1'}: (W^{k1'})^{n2'}, n2' = t
+            wv.y = -wv.y;
+            mul_powers<R3>(u, wv);
+#pragma unroll
+            for (int t = 0; t < R3; ++t) base[(R1 * R2 + R2 + 1) * t] = u[t];
+        }
+        __syncthreads();
+        // ---- pass B^-1: inverse R2-point transforms over k1' at positions k1 + R1 t + R1 R2 n2'
+        for (int wq = tm; wq < N / R2; wq += TPM) {
+            const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
+            double2* base = trk + k1 + (R1 * R2 + R2 + 1) * n2p;
+            double2 u[R2];
+#pragma unroll
+            for (int t = 0; t < R2; ++t) u[t] = base[(R1 + 1) * t];
+            dft<R2, true>(u);
+#pragma unroll
+            for (int t = 0; t < R2; ++t) base[(R1 + 1) * t] = u[t];
+        }
+        __syncthreads();
+        // ---- pass A^-1: conjugate twiddle W_N^{-n2 k1}, inverse R1-point transforms over k1 -> pixels n1 N / R1 + n2
+        const int k = w.kfirst + kkp;
+        double* mp = maps + ((size_t)(k0 + (k < kmaps ? k : 0)) * d.ncomp + w.comp) * d.npix;
+        for (int j = tm; j < N / R1; j += TPM) {
+            const int B = (j >> G::LR3) + R2 * (j & (R3 - 1));
+            const double2* src = trk + R1 * B + B + (j & (R3 - 1));
+            double2 u[R1];
+#pragma unroll
+            for (int q = 0; q < R1; ++q) u[q] = src[q];
+            double2 wv = __ldg(tw2 + 2 * j);
+            wv.y = -wv.y;
+            mul_powers<R1>(u, wv);
+            dft<R1, true>(u);
+            if (k < kmaps) {
+#pragma unroll
+                for (int r = 0; r < R1; ++r) {
+                    mp[rp.start_n + j + r * (N / R1)] = u[r].x;
+                    if (!equator) mp[rp.start_s + j + r * (N / R1)] = u[r].y;
+                }
+            }
+        }
+        __syncthreads();                                  // the transform buffers are rewritten by the next item
+    }
+}
+
+// ---- host side -------------------------------------------------------------------------------------------
+// Workspace F as a 5-D tensor for the ring kernels' boxes of [MB orders] x [E, O] x [KT maps]: innermost the 2 KT
+// doubles of KT maps (re, im); c = which KT-map part of the 4-map line; ch = 2 comp + h; m; (p, kg).
+// planes: dimension order (doubles, m, ch, c, pkg) -> box lands as [h][m][map] (conflict-free staging); otherwise
+// ascending strides (doubles, c, ch, m, pkg) -> [m][h][map].
+static cudaError_t make_tmap_ring(const DevicePlan& d, const double* F, int kt, int mb, bool planes, CUtensorMap* tm)
+{
+    PFN_tmapEncodeTiled enc = tmap_encoder();
+    if (!enc) return cudaErrorNotSupported;
+    const cuuint64_t line = 128, mstr = (cuuint64_t)d.ncomp * line, pstr = (cuuint64_t)(d.lmax + 1) * mstr;
+    const cuuint64_t n_m = (cuuint64_t)d.lmax + 1, n_ch = 2 * (cuuint64_t)d.ncomp, n_c = (cuuint64_t)(KG / kt),
+                     n_pkg = (cuuint64_t)d.nh * d.nkg;
+    cuuint64_t dims[5], strides[4];
+    cuuint32_t box[5];
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    dims[0] = 2 * (cuuint64_t)kt; box[0] = 2 * (cuuint32_t)kt;
+    if (planes) {
+        dims[1] = n_m; strides[0] = mstr; box[1] = (cuuint32_t)mb;
+        dims[2] = n_ch; strides[1] = 64; box[2] = 2;
+        dims[3] = n_c; strides[2] = (cuuint64_t)kt * 16; box[3] = 1;
+    } else {
+        dims[1] = n_c; strides[0] = (cuuint64_t)kt * 16; box[1] = 1;
+        dims[2] = n_ch; strides[1] = 64; box[2] = 2;
+        dims[3] = n_m; strides[2] = mstr; box[3] = (cuuint32_t)mb;
+    }
+    dims[4] = n_pkg; strides[3] = pstr; box[4] = 1;
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<double*>(F), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+template <int LOGN, int KT>
+static size_t analysis_p2_smem()
+{
+    return (size_t)2 * KT * 2 * (1 << LOGN) * 8 + (size_t)KT * p2::buf_stride<LOGN, KT>() * 16 +
+           (size_t)2 * (p2::NT / KT) * 2 * KT * 16 + 64;
+}
+template <int LOGN, int KT, int NSL>
+static size_t synthesis_p2_smem()
+{
+    return (size_t)NSL * (p2::NT / KT) * 2 * KT * 16 + (size_t)KT * p2::buf_stride<LOGN, KT>() * 16 + 8 * NSL + 64;
+}
+
+template <int LOGN, int KT>
+static cudaError_t run_analysis_p2(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
+{
+    const size_t sm = analysis_p2_smem<LOGN, KT>();
+    cudaError_t e = cudaFuncSetAttribute(k_ring_analysis_p2<LOGN, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    CUtensorMap tm;
+    bool planes = true;
+    if (make_tmap_ring(d, F, KT, p2::NT / KT, true, &tm) != cudaSuccess) {
+        planes = false;
+        if ((e = make_tmap_ring(d, F, KT, p2::NT / KT, false, &tm)) != cudaSuccess) return e;
+    }
+    const long long nitems = (long long)pl->belt_count * d.ncomp * ((kmaps + KT - 1) / KT);
+    const unsigned grid = (unsigned)(nitems < pl->sm_count ? nitems : pl->sm_count);
+    k_ring_analysis_p2<LOGN, KT><<<grid, p2::NT, sm, st>>>(tm, d, maps, k0, kmaps, pl->belt_first, pl->belt_count, planes ? 1 : 0);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+template <int LOGN, int KT, int NSL>
+static cudaError_t run_synthesis_p2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps, cudaStream_t st)
+{
+    const size_t sm = synthesis_p2_smem<LOGN, KT, NSL>();
+    cudaError_t e = cudaFuncSetAttribute(k_ring_synthesis_p2<LOGN, KT, NSL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    CUtensorMap tm;
+    bool planes = true;
+    if (make_tmap_ring(d, F, KT, p2::NT / KT, true, &tm) != cudaSuccess) {
+        planes = false;
+        if ((e = make_tmap_ring(d, F, KT, p2::NT / KT, false, &tm)) != cudaSuccess) return e;
+    }
+    const long long nitems = (long long)pl->belt_count * d.ncomp * ((kmaps + KT - 1) / KT);
+    const int occ = pl->p2_syn_occ > 0 ? pl->p2_syn_occ : 1;
+    long long want = (long long)pl->sm_count * occ;
+    const unsigned grid = (unsigned)(nitems < want ? nitems : want);
+    k_ring_synthesis_p2<LOGN, KT, NSL><<<grid, p2::NT, sm, st>>>(tm, d, maps, k0, kmaps, pl->belt_first, pl->belt_count, planes ? 1 : 0);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+// belt ring pairs of a power-of-two nside through the fast path; returns cudaErrorNotSupported if this plan has none
+cudaError_t launch_ring_analysis_belt(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
+{
+    switch (pl->belt_logn) {
+        case 9: return run_analysis_p2<9, 4>(pl, d, maps, F, k0, kmaps, st);
+        case 10: return run_analysis_p2<10, 4>(pl, d, maps, F, k0, kmaps, st);
+        case 11: return run_analysis_p2<11, 2>(pl, d, maps, F, k0, kmaps, st);
+        default: return cudaErrorNotSupported;
+    }
+}
+
+cudaError_t launch_ring_synthesis_belt(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps, cudaStream_t st)
+{
+    switch (pl->belt_logn) {
+        case 9: return run_synthesis_p2<9, 4, 4>(pl, d, F, maps, k0, kmaps, st);
+        case 10: return run_synthesis_p2<10, 4, 4>(pl, d, F, maps, k0, kmaps, st);
+        case 11: return run_synthesis_p2<11, 2, 4>(pl, d, F, maps, k0, kmaps, st);
+        default: return cudaErrorNotSupported;
+    }
+}
+
+}  // namespace sht
