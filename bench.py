@@ -28,22 +28,18 @@ sys.path.insert(0, ROOT)
 from paper_2208_10154_b200 import inputs, shard  # noqa: E402
 
 FP64_NOMINAL_TFLOPS = 37.2     # 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz
-# From the committed ncu captures (profiles/r1_v4_summary.md staged, profiles/r1_v2_summary.md fused), keyed by
-# (config, nmaps, lambda mode, kernel): DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) and the
-# DMMA pipe activity (sm__pipe_tensor_subpipe_dmma_cycles_active, fraction of peak) = executed-flop rate / peak
-NCU_TRAFFIC_BYTES = {
-    (3, 1000, "staged", "k_legendre_analysis"): 259432695040 + 19052913408,
-    (3, 1000, "staged", "k_legendre_synthesis"): 222430966528 + 37874563584,
-    (4, 1000, "staged", "k_legendre_analysis"): 71304026880 + 9527154944,       # k_legendre_analysis_spin2
-    (4, 1000, "staged", "k_legendre_synthesis"): 45836310272 + 20283129600,     # k_legendre_synthesis_spin2
-    (3, 1000, "fused", "k_legendre_analysis"): 251379450880 + 19061606400,
-    (3, 1000, "fused", "k_legendre_synthesis"): 20458497000 + 37875944000,
-}
-NCU_DMMA_PIPE_ACTIVE = {
-    (3, 1000, "staged", "k_legendre_analysis"): 0.907, (3, 1000, "staged", "k_legendre_synthesis"): 0.912,
-    (4, 1000, "staged", "k_legendre_analysis"): 0.945, (4, 1000, "staged", "k_legendre_synthesis"): 0.888,
-    (3, 1000, "fused", "k_legendre_analysis"): 0.731, (3, 1000, "fused", "k_legendre_synthesis"): 0.770,
-}
+def ncu_capture_row(config, nmaps, lambda_mode, kernel):
+    """dram bytes per launch / DMMA pipe activity of `kernel` from the newest committed ncu capture of exactly this
+    workload (profiles/ncu_latest.csv: config,nmaps,lambda_mode,kernel,dram_bytes,dmma_pipe_active,capture,commit), or
+    None.  The values describe the commit named there; the line says so."""
+    path = os.path.join(ROOT, "profiles", "ncu_latest.csv")
+    if not os.path.exists(path):
+        return None
+    for ln in open(path):
+        f = [x.strip() for x in ln.split(",")]
+        if len(f) >= 8 and f[0] == str(config) and f[1] == str(nmaps) and f[2] == lambda_mode and f[3] == kernel:
+            return {"traffic": int(float(f[4])), "dmma_pipe_active": float(f[5]), "capture": f[6], "commit": f[7]}
+    return None
 
 
 def read_measured_peaks():
@@ -408,9 +404,15 @@ def main():
         launch_ms = stage_ms[stage] / n
         flops_per_launch = fl_dir * dirs[stage] * args.steps / n          # algorithmic (folded, unpruned) flops of one launch
         ach = flops_per_launch / (launch_ms * 1e-3) * 1e-12
+        cap = None if plain_key is None else ncu_capture_row(*plain_key, kernel)
+        # flops the contraction kernel really executes (pruning, l_safe skipping, tile padding), counted by the plan
+        ex = plan.executed_flops(stage - 1) if not args.pol else -1.0
+        ex_rate = ex * dirs[stage] * args.steps / n / (launch_ms * 1e-3) * 1e-12 if ex > 0 else None
         return {"bound": "tensor", "kernel": kernel, "achieved": ach, "peak": mma_peak, "unit": "TFLOP/s",
-                "frac": ach / mma_peak, "traffic": None if plain_key is None else NCU_TRAFFIC_BYTES.get(plain_key + (kernel,)),
-                "dmma_pipe_active_ncu": None if plain_key is None else NCU_DMMA_PIPE_ACTIVE.get(plain_key + (kernel,)),
+                "frac": ach / mma_peak, "traffic": cap["traffic"] if cap else None,
+                "executed_flops_per_launch": ex * dirs[stage] * args.steps / n if ex > 0 else None,
+                "achieved_executed": ex_rate, "frac_executed": ex_rate / mma_peak if ex_rate else None,
+                "ncu_capture": cap,
                 "algorithmic_flops_per_launch": flops_per_launch, "launch_ms": launch_ms,
                 "share_of_step": stage_ms[stage] / ms_total}
 
@@ -424,10 +426,12 @@ def main():
                                              % (cublas_peak["n"], cublas_peak["seconds"], cublas_peak["sm_mhz"], cublas_peak["reasons"]))
     if cublas_cmp:
         roofline["cublas_per_m_dgemm"] = cublas_cmp
-    roofline["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r1_v4_summary.md (staged) / r1_v2_summary.md (fused)"
-    roofline["note"] = ("achieved = algorithmic (N/S-folded, UNPRUNED) flops / time: ring pruning and l_safe row skipping "
-                        "leave ~0.8x of them to execute, so frac can exceed 1; dmma_pipe_active_ncu is the executed-flop "
-                        "fraction of peak from the committed ncu capture")
+    roofline["traffic_source"] = ("dram__bytes_read.sum + dram__bytes_write.sum per launch from the capture named in ncu_capture "
+                                  "(profiles/ncu_latest.csv); null if no capture of this exact workload is committed")
+    roofline["note"] = ("achieved / frac = algorithmic (N/S-folded, UNPRUNED) flops / time, as SURVEY.md 8(d) defines the unit "
+                        "(can exceed 1: ring pruning and l_safe skipping are the method's own saving); achieved_executed / "
+                        "frac_executed = the DMMA flops the kernel really executes (sht_plan_executed_flops) / the same time = "
+                        "the hardware rate against the same live peak")
     roofline_syn = leg_roofline(2, "k_legendre_synthesis")
     ring_ms = stage_ms[0] + stage_ms[3]
     ring_bytes = 2 * args.steps * (8 * npix * nmaps * ncomp + 16 * (lmax + 1) * 2 * nside * 2 * nmaps * ncomp)

@@ -142,6 +142,11 @@ long long sht_nalm(int lmax);                        /* (lmax+1)(lmax+2)/2      
 long long sht_alm_index(int lmax, int l, int m);     /* m(2 lmax+1-m)/2 + l; -1 if out of range     */
 size_t sht_plan_workspace_bytes(sht_plan_t plan);    /* device bytes held by the plan               */
 int sht_plan_chunk_maps(sht_plan_t plan);            /* maps processed per internal chunk           */
+/* FP64 tensor-core flops ONE call of sht_analysis (direction 0) / sht_synthesis (1) executes in its contraction kernel
+ * after ring pruning (item 10), l_safe row skipping (item 11, :230-232) and tile padding -- the kernels' skip
+ * logic replayed on the plan's tables (measurement only: bench.py's hardware-rate roofline fraction).  -1: not counted
+ * (spin-2 plans). */
+double sht_plan_executed_flops(sht_plan_t plan, int direction);
 long long sht_plan_kernel_launches(sht_plan_t plan); /* kernels launched by this plan so far        */
 const char* sht_status_string(sht_status_t s);       /* static storage                              */
 const char* sht_last_error(sht_plan_t plan);         /* plan-owned, valid until the next call       */

@@ -65,6 +65,8 @@ _lib.sht_alm_index.argtypes = [_i, _i, _i]
 _lib.sht_alm_index.restype = _ll
 _lib.sht_plan_workspace_bytes.argtypes = [_vp]
 _lib.sht_plan_workspace_bytes.restype = ctypes.c_size_t
+_lib.sht_plan_executed_flops.argtypes = [_vp, _i]
+_lib.sht_plan_executed_flops.restype = _d
 _lib.sht_plan_chunk_maps.argtypes = [_vp]
 _lib.sht_plan_chunk_maps.restype = _i
 _lib.sht_plan_kernel_launches.argtypes = [_vp]
@@ -83,7 +85,7 @@ _lib.sht_measure_fp64_mma_peak.restype = _d
 EXPORTED = [
     "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol", "sht_alm_pack_a7", "sht_alm_unpack_a7", "sht_plan_set_lambda_mode", "sht_plan_lambda_mode", "sht_plan_set_iter_mode", "sht_plan_reserve_iter", "sht_eb_split",
     "sht_analysis_host", "sht_synthesis_host", "sht_npix", "sht_nalm", "sht_alm_index",
-    "sht_plan_workspace_bytes", "sht_plan_chunk_maps", "sht_plan_kernel_launches", "sht_status_string",
+    "sht_plan_workspace_bytes", "sht_plan_chunk_maps", "sht_plan_executed_flops", "sht_plan_kernel_launches", "sht_status_string",
     "sht_last_error", "sht_measure_fp64_mma_peak", "sht_plan_set_timing", "sht_plan_stage_ms",
 ]
 
@@ -209,6 +211,9 @@ class Plan:
 
     def workspace_bytes(self):
         return int(_lib.sht_plan_workspace_bytes(self._h))
+
+    def executed_flops(self, direction):
+        return float(_lib.sht_plan_executed_flops(self._h, direction))
 
     def chunk_maps(self):
         return int(_lib.sht_plan_chunk_maps(self._h))

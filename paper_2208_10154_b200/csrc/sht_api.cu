@@ -615,6 +615,16 @@ extern "C" long long sht_alm_index(int lmax, int l, int m)
     return (long long)m * (2 * lmax + 1 - m) / 2 + l;
 }
 extern "C" size_t sht_plan_workspace_bytes(sht_plan_t pl) { return pl ? pl->F_bytes + pl->table_bytes + pl->lam_bytes : 0; }
+extern "C" double sht_plan_executed_flops(sht_plan_t pl, int direction)
+{
+    if (!pl || direction < 0 || direction > 1 || pl->exec_flops_tile[direction] < 0.0) return -1.0;
+    double tiles = 0.0;                                  // k-tiles of one call over all internal chunks
+    for (int k0 = 0; k0 < pl->nmaps; k0 += pl->chunk) {
+        const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
+        tiles += (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
+    }
+    return tiles * pl->exec_flops_tile[direction];
+}
 extern "C" int sht_plan_chunk_maps(sht_plan_t pl) { return pl ? pl->chunk : 0; }
 extern "C" long long sht_plan_kernel_launches(sht_plan_t pl) { return pl ? pl->launches : 0; }
 extern "C" const char* sht_status_string(sht_status_t s)

@@ -47,6 +47,9 @@ struct RingPair {
     // r = brev(k) >> (32 - pbits); pos = ((r & pm_hi) >> 1) | ((r & pm_lo) << 1) | (r & pm_keep);  pbits = 0: use the table
     int pbits;
     unsigned pm_hi, pm_lo, pm_keep;
+    // chirp-z fast path of the cap rings (sht_ring_pow2.cu): convolution length (0: not on that path) and the offset
+    // (double2) of [filter spectrum FFT_L(conj chirp) / L in natural order: cz_len][chirp c_j: n]
+    int cz_len, cz_off;
 };
 
 struct DevicePlan {
@@ -109,10 +112,15 @@ struct sht_plan_s {
     size_t class_smem[sht::RING_NCLASS];
     // belt fast path (sht_ring_pow2.cu): ring pairs belt_first .. belt_first + belt_count - 1 have length 2^belt_logn
     // (belt_logn = 0: none); class_*_nb are the launch classes of the general kernels without those pairs
-    int belt_logn, belt_first, belt_count, p2_syn_occ;
+    int belt_logn, belt_first, belt_count, p2_syn_occ, p2_variant;
+    int leg_tsplit, leg_nsplit;     // grid shapes of the spin-0 Legendre kernels (sht_legendre.cu launchers)
+    bool fast_ring;                 // the kernels of sht_ring_pow2.cu are in use (experiment switch; default on)
     int* class_rings_nb[sht::RING_NCLASS];
     int class_count_nb[sht::RING_NCLASS];
     int class_ktmin_nb[sht::RING_NCLASS];
+    // chirp-z fast path: ring pairs by convolution length (CZ_NCLASS compiled lengths), their W_L tables
+    int* cz_rings[8];
+    int cz_count[8], cz_tw_off[8];
     int sm_count;
     long long launches;
     double* Fmap;                   // Alg. 2: folded T_m of the input maps (allocated on the first iterative call)
@@ -124,6 +132,7 @@ struct sht_plan_s {
     int* lam_i0;                    // [analysis blocks] first 16-row block with a started recurrence
     int lam_mode;                   // SHT_LAMBDA_FUSED / SHT_LAMBDA_STAGED
     long long n_ablk, n_sblk;
+    double exec_flops_tile[2];      // DMMA flops one k-tile executes (0 analysis, 1 synthesis; spin 0; -1 = not counted)
     bool ring_attr_set, resid_attr_set;   // dynamic shared-memory attributes of the ring kernels set on this plan's device
     char err[512];
     // host-entry staging (allocated on first use)
@@ -157,6 +166,12 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
 // belt fast path (sht_ring_pow2.cu)
 cudaError_t launch_ring_analysis_belt(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st);
 cudaError_t launch_ring_synthesis_belt(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps, cudaStream_t st);
+// chirp-z fast path of the cap rings: the compiled convolution lengths
+constexpr int CZ_NCLASS = 7;
+constexpr int CZ_LEN[CZ_NCLASS] = {512, 768, 1024, 1536, 2048, 3072, 4096};
+constexpr int CZ_MIN_N = 132;                // shorter rings stay with the general kernels
+cudaError_t launch_ring_analysis_cz(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st);
+cudaError_t launch_ring_synthesis_cz(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps, cudaStream_t st);
 // Legendre stage (sht_legendre.cu)
 // pol: spin 2 only, 0 = E and B, SHT_POL_E / SHT_POL_B = that component alone (`alm` then holds one component);
 // gen_lambda = false: staged mode, the lambda scratch already holds this direction's blocks (host path: one generator

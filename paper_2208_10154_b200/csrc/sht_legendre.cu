@@ -656,7 +656,10 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
 {
     if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st, pol, gen_lambda);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
-    const unsigned grid = (unsigned)((d.lmax + 1) * nkt);
+    // leg_tsplit: one CTA per (m, l tile, k-tile) instead of per (m, k-tile): the l tiles of an (m, k-tile) then read the
+    // same T_m boxes at about the same time from different SMs, and L2 serves the re-reads
+    const int tsplit = pl->leg_tsplit;
+    const unsigned grid = (unsigned)((d.lmax + 1) * nkt * (tsplit ? d.ntile_max : 1));
     const size_t sm = analysis_smem(d.ntile_max);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
@@ -665,7 +668,7 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
     if (staged && gen_lambda && (e = launch_lambda_blocks(pl, d, true, st)) != cudaSuccess) return e;
     k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0,
-                                                       staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr, 0, 0, nullptr);
+                                                       staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr, 0, tsplit, nullptr);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -720,7 +723,10 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
     const int npb = (d.nh + S_PB - 1) / S_PB;
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
     if (staged && gen_lambda && (e = launch_lambda_blocks(pl, d, false, st)) != cudaSuccess) return e;
-    k_legendre_synthesis<<<(d.lmax + 1) * nkt, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, 1);
+    // leg_nsplit CTAs share the ring blocks of an (m, k-tile) (block b goes to CTA b mod nsplit): they re-read the same
+    // a_lm tile at about the same time, and the set in flight (148 / nsplit tiles of up to 1.5 MB) fits L2
+    const int nsplit = pl->leg_nsplit < 1 ? 1 : (pl->leg_nsplit > npb ? npb : pl->leg_nsplit);
+    k_legendre_synthesis<<<(d.lmax + 1) * nkt * nsplit, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, nsplit);
     pl->launches++;
     return cudaGetLastError();
 }

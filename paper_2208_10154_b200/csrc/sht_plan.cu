@@ -1,11 +1,13 @@
 // sht_plan.cu -- plan creation: ring tables, FFT twiddles / radix lists, recurrence coefficients and the
 // l_safe / seed table of PAPER.md:230-232 (item 11: "the recursion starts from safe positions ... computed
 // once and saved as an input table l_safe(m, theta)").
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <thread>
 #include <utility>
 #include <vector>
 #include "sht_internal.h"
@@ -357,6 +359,55 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             perm.push_back((unsigned short)pos);
         }
     }
+    // ---- chirp-z fast path of the cap rings: per ring length N = 4 q >= CZ_MIN_N with 2 N - 1 <= 4096 the filter spectrum
+    // FFT_L(h) / L (h_j = exp(+i pi j^2 / N) at j = -(N-1) .. N-1 mod L; long double, natural order) and the chirp
+    std::vector<int> cz_len_of_q(nside + 1, 0), cz_off_of_q(nside + 1, 0);
+    int cz_tw_off[CZ_NCLASS];
+    {
+        std::vector<int> todo;
+        for (int q = 1; q < nside; ++q) {
+            const int n = 4 * q;
+            if (n < CZ_MIN_N) continue;
+            for (int c = 0; c < CZ_NCLASS; ++c)
+                if (CZ_LEN[c] >= 2 * n - 1) { cz_len_of_q[q] = CZ_LEN[c]; break; }
+            if (cz_len_of_q[q]) {
+                cz_off_of_q[q] = (int)tw.size();
+                tw.resize(tw.size() + (size_t)cz_len_of_q[q] + n);
+                todo.push_back(q);
+            }
+        }
+        auto work = [&](size_t first, size_t step) {
+            for (size_t t = first; t < todo.size(); t += step) {
+                const int q = todo[t], n = 4 * q, L = cz_len_of_q[q];
+                std::vector<long double> hr(L, 0.0L), hi(L, 0.0L);
+                for (int j = 0; j < n; ++j) {
+                    const long long e = ((long long)j * j) % (2LL * n);
+                    const long double ang = PI_LD * (long double)e / (long double)n;
+                    hr[j] = cosl(ang); hi[j] = sinl(ang);
+                    if (j > 0) { hr[L - j] = hr[j]; hi[L - j] = hi[j]; }
+                }
+                host_fft(hr, hi);
+                double2* dst = tw.data() + cz_off_of_q[q];
+                for (int k = 0; k < L; ++k) dst[k] = make_double2((double)(hr[k] / L), (double)(hi[k] / L));
+                for (int j = 0; j < n; ++j) dst[L + j] = tw[tw_off_of_q[q] + (int)(((long long)j * j) % (2LL * n))];
+            }
+        };
+        unsigned nthr = std::thread::hardware_concurrency();
+        if (nthr < 1) nthr = 1;
+        if (nthr > 16) nthr = 16;
+        std::vector<std::thread> pool;
+        for (unsigned t = 1; t < nthr; ++t) pool.emplace_back(work, (size_t)t, (size_t)nthr);
+        work(0, nthr);
+        for (auto& th : pool) th.join();
+        for (int c = 0; c < CZ_NCLASS; ++c) {                // W_L^e, e < L
+            cz_tw_off[c] = (int)tw.size();
+            const int L = CZ_LEN[c];
+            for (int e = 0; e < L; ++e) {
+                const long double ang = 2.0L * PI_LD * (long double)e / (long double)L;
+                tw.push_back(make_double2((double)cosl(ang), (double)-sinl(ang)));
+            }
+        }
+    }
     const long long ns = nside;
     for (int p = 0; p < d.nh; ++p) {
         const long long i = p + 1;                       // north ring index, 1 .. 2 nside
@@ -407,6 +458,8 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             }
             r.pbits = a;
         }
+        r.cz_len = (i < ns) ? cz_len_of_q[q] : 0;
+        r.cz_off = cz_off_of_q[q];
         r.mlim = lmax + 1;                               // tightened below from the l_safe table
         zs[p] = (double)absz; sin2s[p] = (double)s2;
     }
@@ -549,6 +602,50 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
                     if (nst > d.nst_max) d.nst_max = nst;
                 }
             }
+            // DMMA flops one k-tile (64 maps = 128 real columns) EXECUTES per direction (spin 0): the contraction
+            // kernels' own skip logic (ring pruning per l tile, l_safe row blocks, blocks past lmax) replayed on the host
+            // tables -- what bench.py divides by the time for the hardware-rate roofline fraction
+            pl->exec_flops_tile[0] = pl->exec_flops_tile[1] = spin == 2 ? -1.0 : 0.0;
+            if (spin == 0) {
+                double fa = 0.0, fs = 0.0;
+                for (int m = 0; m <= lmax; ++m) {
+                    const int nt = (lmax - m) / LEG_A_ML + 1;
+                    for (int t = 0; t < nt; ++t) {
+                        const int l0 = m + t * LEG_A_ML;
+                        const int i1 = std::min(8, (lmax - l0) / 16 + 1);
+                        for (int pc = pst[(size_t)m * d.ntile_max + t]; pc < d.nh; pc += 32) {
+                            int v[4]; bool plain = true;
+                            for (int g = 0; g < 4; ++g) {
+                                int lsmin = lmax + 1;
+                                for (int p = pc + 8 * g; p < pc + 8 * g + 8 && p < d.nh; ++p) lsmin = std::min(lsmin, hls[(size_t)m * d.nh + p]);
+                                v[g] = std::max(0, std::min(8, (lsmin - l0) >> 4));
+                                plain = plain && v[g] == 0;
+                            }
+                            long long units = 0;
+                            if (plain) units = 4LL * (i1 > 6 ? 8 : i1 > 4 ? 6 : i1 > 2 ? 4 : 2);
+                            else for (int g = 0; g < 4; ++g) units += std::max(0, i1 - v[g]);
+                            fa += (double)units * (2.0 * 16 * 8 * 128);
+                        }
+                    }
+                    for (int b = 0; b < d.npb; ++b) {
+                        const int cf = scf[(size_t)m * d.npb + b];
+                        const int plast = (b * 64 + 64 < d.nh ? b * 64 + 64 : d.nh) - 1;
+                        if (m >= mlim[plast] || cf > lmax) continue;
+                        const int* q = &sm8[((size_t)m * d.npb + b) * 8];
+                        for (int lc = cf; lc <= lmax; lc += 32) {
+                            const int ks1 = std::min(4, (lmax - lc) / 8 + 1);
+                            long long units = 0;
+                            for (int ks = 0; ks < ks1; ++ks)
+                                for (int i = 0; i < 8; ++i) units += q[i] <= lc + 8 * ks + 7 ? 1 : 0;
+                            bool all0 = true;
+                            for (int i = 0; i < 8; ++i) all0 = all0 && q[i] <= lc + 7;
+                            if (all0 && ks1 == 4) units = 32;
+                            fs += (double)units * (2.0 * 8 * 8 * 128);
+                        }
+                    }
+                }
+                pl->exec_flops_tile[0] = fa; pl->exec_flops_tile[1] = fs;
+            }
             pl->n_ablk = na; pl->n_sblk = nsb;
             if (na > 0x7fffffffLL || nsb > 0x7fffffffLL) { sht_plan_destroy(pl); return SHT_ERR_UNSUPPORTED; }
             if (upload(pl, aoff, &d.ablk_off) != cudaSuccess || upload(pl, soff, &d.sblk_off) != cudaSuccess ||
@@ -584,7 +681,13 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             pl->class_rings[c] = const_cast<int*>(dp);
         }
         // belt fast path: nside a power of two with a ring length the compiled transforms cover
-        pl->belt_logn = 0; pl->belt_first = nside - 1; pl->belt_count = nside + 1; pl->p2_syn_occ = 2;
+        pl->belt_logn = 0; pl->belt_first = nside - 1; pl->belt_count = nside + 1; pl->p2_syn_occ = 2; pl->p2_variant = 1; pl->fast_ring = true;
+        if (const char* ev = getenv("SHT_FAST_RING")) pl->fast_ring = atoi(ev) != 0;
+        pl->leg_tsplit = 0; pl->leg_nsplit = 1;
+        if (const char* ev = getenv("SHT_LEG_TSPLIT")) pl->leg_tsplit = atoi(ev);
+        if (const char* ev = getenv("SHT_LEG_NSPLIT")) pl->leg_nsplit = atoi(ev);
+        if (const char* ev = getenv("SHT_P2_VARIANT")) pl->p2_variant = atoi(ev);      // experiment switch
+        if (const char* ev = getenv("SHT_P2_SYN_OCC")) pl->p2_syn_occ = atoi(ev);
         if ((nside & (nside - 1)) == 0 && 4 * nside >= 512 && 4 * nside <= 2048) {
             int a = 0;
             while ((1 << a) < 4 * nside) ++a;
@@ -595,6 +698,7 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             pl->class_ktmin_nb[c] = 16;
             for (int p : lists[c]) {
                 if (pl->belt_logn && p >= pl->belt_first) continue;
+                if (rings[p].cz_len) continue;
                 nb.push_back(p);
                 if (rings[p].kt < pl->class_ktmin_nb[c]) pl->class_ktmin_nb[c] = rings[p].kt;
             }
@@ -602,6 +706,16 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             const int* dp = nullptr;
             if (upload(pl, nb, &dp) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
             pl->class_rings_nb[c] = const_cast<int*>(dp);
+        }
+        for (int c = 0; c < CZ_NCLASS; ++c) {                // longest rings first
+            std::vector<int> lst;
+            for (int p = d.nh - 1; p >= 0; --p)
+                if (rings[p].cz_len == CZ_LEN[c]) lst.push_back(p);
+            pl->cz_count[c] = (int)lst.size();
+            pl->cz_tw_off[c] = cz_tw_off[c];
+            const int* dp = nullptr;
+            if (upload(pl, lst, &dp) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+            pl->cz_rings[c] = const_cast<int*>(dp);
         }
     }
 

@@ -1109,12 +1109,14 @@ cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const doub
 {
     cudaError_t e = ring_attr(pl);
     if (e != cudaSuccess) return e;
-    // the belt (two thirds of the pixels) goes through the fast path, except when the uncovered power is wanted
-    const bool belt = pl->belt_logn != 0 && upow == nullptr;
-    if (belt && (e = launch_ring_analysis_belt(pl, d, maps, F, k0, kmaps, st)) != cudaSuccess) return e;
-    int* const* lists = belt ? pl->class_rings_nb : pl->class_rings;
-    const int* count = belt ? pl->class_count_nb : pl->class_count;
-    const int* ktmin = belt ? pl->class_ktmin_nb : pl->class_ktmin;
+    // the belt (two thirds of the pixels) and the cap rings on the chirp-z path go through the kernels of
+    // sht_ring_pow2.cu, except when the uncovered power is wanted
+    const bool fast = upow == nullptr && pl->fast_ring;
+    if (fast && pl->belt_logn && (e = launch_ring_analysis_belt(pl, d, maps, F, k0, kmaps, st)) != cudaSuccess) return e;
+    if (fast && (e = launch_ring_analysis_cz(pl, d, maps, F, k0, kmaps, st)) != cudaSuccess) return e;
+    int* const* lists = fast ? pl->class_rings_nb : pl->class_rings;
+    const int* count = fast ? pl->class_count_nb : pl->class_count;
+    const int* ktmin = fast ? pl->class_ktmin_nb : pl->class_ktmin;
     // longest rings first: their CTAs are the slowest
     for (int c = RING_NCLASS - 1; c >= 0; --c) {
         if (count[c] == 0) continue;
@@ -1130,11 +1132,12 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
 {
     cudaError_t e = ring_attr(pl);
     if (e != cudaSuccess) return e;
-    const bool belt = pl->belt_logn != 0 && sub_from == nullptr;
-    if (belt && (e = launch_ring_synthesis_belt(pl, d, F, maps, k0, kmaps, st)) != cudaSuccess) return e;
-    int* const* lists = belt ? pl->class_rings_nb : pl->class_rings;
-    const int* count = belt ? pl->class_count_nb : pl->class_count;
-    const int* ktmin = belt ? pl->class_ktmin_nb : pl->class_ktmin;
+    const bool fast = sub_from == nullptr && pl->fast_ring;
+    if (fast && pl->belt_logn && (e = launch_ring_synthesis_belt(pl, d, F, maps, k0, kmaps, st)) != cudaSuccess) return e;
+    if (fast && (e = launch_ring_synthesis_cz(pl, d, F, maps, k0, kmaps, st)) != cudaSuccess) return e;
+    int* const* lists = fast ? pl->class_rings_nb : pl->class_rings;
+    const int* count = fast ? pl->class_count_nb : pl->class_count;
+    const int* ktmin = fast ? pl->class_ktmin_nb : pl->class_ktmin;
     for (int c = RING_NCLASS - 1; c >= 0; --c) {
         if (count[c] == 0) continue;
         dim3 grid((kmaps + ktmin[c] - 1) / ktmin[c], count[c], d.ncomp);

@@ -50,6 +50,21 @@ __device__ __forceinline__ double2 mul_w16(double2 a)
     }
 }
 
+// multiply by exp(-+ 2 pi i k / 12), k in {1, 2, 3, 4, 6}
+template <int K, bool INV>
+__device__ __forceinline__ double2 mul_w12(double2 a)
+{
+    constexpr double C30 = 0.86602540378443864676;       // cos(pi / 6)
+    if constexpr (K == 3) return INV ? make_double2(-a.y, a.x) : make_double2(a.y, -a.x);
+    else if constexpr (K == 6) return make_double2(-a.x, -a.y);
+    else {
+        constexpr double c = K == 1 ? C30 : K == 2 ? 0.5 : -0.5;                  // cos(2 pi K / 12)
+        constexpr double s0 = K == 1 ? 0.5 : C30;                                // sin(2 pi K / 12), K = 1, 2, 4
+        constexpr double sn = INV ? s0 : -s0;
+        return make_double2(fma(a.x, c, -(a.y * sn)), fma(a.x, sn, a.y * c));
+    }
+}
+
 template <bool INV>
 __device__ __forceinline__ void bfly4(double2& x0, double2& x1, double2& x2, double2& x3)
 {
@@ -62,8 +77,32 @@ __device__ __forceinline__ void bfly4(double2& x0, double2& x1, double2& x2, dou
 template <int R, bool INV>
 __device__ __forceinline__ void dft(double2 (&u)[R])
 {
-    static_assert(R == 8 || R == 16, "radix");
-    if constexpr (R == 16) {
+    static_assert(R == 8 || R == 12 || R == 16, "radix");
+    if constexpr (R == 12) {
+        // n = 4 n1 + n2, k = k1 + 3 k2:  X[k1 + 3 k2] = sum_n2 w4^{n2 k2} { w12^{n2 k1} sum_n1 x[4 n1 + n2] w3^{n1 k1} }
+        constexpr double S3 = 0.86602540378443864676;    // sin(2 pi / 6)
+        double2 t[4][3];
+#pragma unroll
+        for (int n2 = 0; n2 < 4; ++n2) {
+            const double2 x0 = u[n2], x1 = u[n2 + 4], x2 = u[n2 + 8];
+            const double2 sm = cadd(x1, x2), df = csub(x1, x2);
+            const double2 re = make_double2(fma(-0.5, sm.x, x0.x), fma(-0.5, sm.y, x0.y));
+            // forward: X1 = re - i S3 df, X2 = re + i S3 df; inverse: the other way round
+            const double2 im = make_double2(S3 * df.y, -S3 * df.x);              // -i S3 df
+            double2 y1 = INV ? csub(re, im) : cadd(re, im), y2 = INV ? cadd(re, im) : csub(re, im);
+            // twiddle w12^{n2 k1}: exponents n2 (k1 = 1), 2 n2 (k1 = 2)
+            if (n2 == 1) { y1 = mul_w12<1, INV>(y1); y2 = mul_w12<2, INV>(y2); }
+            if (n2 == 2) { y1 = mul_w12<2, INV>(y1); y2 = mul_w12<4, INV>(y2); }
+            if (n2 == 3) { y1 = mul_w12<3, INV>(y1); y2 = mul_w12<6, INV>(y2); }
+            t[n2][0] = cadd(x0, sm); t[n2][1] = y1; t[n2][2] = y2;
+        }
+#pragma unroll
+        for (int k1 = 0; k1 < 3; ++k1) {
+            double2 w0 = t[0][k1], w1 = t[1][k1], w2 = t[2][k1], w3 = t[3][k1];
+            bfly4<INV>(w0, w1, w2, w3);
+            u[k1] = w0; u[k1 + 3] = w1; u[k1 + 6] = w2; u[k1 + 9] = w3;
+        }
+    } else if constexpr (R == 16) {
         // n = a + 4 r, k = s + 4 q:  X[s + 4 q] = sum_a w4^{a q} { w16^{a s} sum_r x[a + 4 r] w4^{r s} }
         double2 t[4][4];
 #pragma unroll
@@ -189,11 +228,14 @@ k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
     constexpr int MB = NT / KT;                           // orders m per mapping sweep (one TMA store box)
     constexpr int BS = buf_stride<LOGN, KT>();
     constexpr int IN_DOUBLES = KT * 2 * N;                // one input buffer
+    constexpr int SLOT = MB * 2 * KT;                     // double2 per TMA box
+    constexpr int NSLOTS = (KT * N) / SLOT;               // boxes an input buffer holds when it serves as output staging
+    constexpr int U = NSLOTS >= 6 ? 3 : NSLOTS / 2;       // boxes per round (two rounds never share a slot)
+    static_assert(U >= 1 && 2 * U <= NSLOTS, "output staging");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* in_buf = reinterpret_cast<double*>(smem_raw);
     double2* tr = reinterpret_cast<double2*>(smem_raw + (size_t)2 * IN_DOUBLES * 8);
-    double2* out = tr + KT * BS;                          // 2 slots of MB * 2 * KT elements
-    uint64_t* full = reinterpret_cast<uint64_t*>(out + 2 * MB * 2 * KT);
+    uint64_t* full = reinterpret_cast<uint64_t*>(tr + KT * BS);
 
     const int tid = threadIdx.x;
     const int nkp = (kmaps + KT - 1) / KT;
@@ -259,8 +301,6 @@ k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
             for (int k = 0; k < R1; ++k) dst[k] = u[k];
         }
         __syncthreads();
-        // the input buffer is free: fetch the rows of the item after the next one
-        if (tid == 0 && it + 2LL * gridDim.x < nitems) issue_loads(it + 2LL * gridDim.x, buf);
 
         // ---- pass B: R2-point transforms over n1' at positions k1 + R1 t + R1 R2 n2', twiddle W_{R2 R3}^{n2' k1'}
         for (int wq = tm; wq < N / R2; wq += TPM) {
@@ -288,38 +328,211 @@ k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
         }
         __syncthreads();
 
-        // ---- FFT mapping: order m -> bin m mod N, phase, fold; lines leave by TMA store
+        // ---- FFT mapping: order m -> bin m mod N, phase, fold.  The lines are staged in the
+        // input buffer this item has just consumed (NSLOTS boxes of MB orders) and leave by TMA stores, U boxes per round;
+        // a round's slots are rewritten two rounds later, after thread 0 has seen its stores read them.
         const int mlim = rp.mlim;
         const double2* trm = tr + kkm * BS;
         const int kg = w.kfirst / KG, csel = (w.kfirst % KG) / KT;
-        for (int m0 = 0; m0 < mlim; m0 += MB, ++nstore) {
-            const int m = m0 + mi;
-            const int b = m & (N - 1), bc = (N - b) & (N - 1);
-            const double2 A = trm[G::phys(b)], Bv = trm[G::phys(bc)];
-            // G_north = (A + conj B) / 2, G_south = (A - conj B) / (2 i)
-            const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
-            const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
-            double2 ph = make_double2(dsig, 0.0);
-            if (rp.shift) {                               // e^{-i m phi0}, phi0 = pi / N
-                ph = __ldg(tw2 + (m & (2 * N - 1)));
-                ph.x *= dsig; ph.y *= dsig;
+        double2* const ostage = reinterpret_cast<double2*>(in_buf + (size_t)buf * IN_DOUBLES);
+        for (int m0 = 0; m0 < mlim; m0 += U * MB) {
+#pragma unroll
+            for (int q = 0; q < U; ++q) {
+                const int m = m0 + q * MB + mi;
+                const int b = m & (N - 1), bc = (N - b) & (N - 1);
+                const double2 A = trm[G::phys(b)], Bv = trm[G::phys(bc)];
+                // G_north = (A + conj B) / 2, G_south = (A - conj B) / (2 i)
+                const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
+                const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
+                double2 ph = make_double2(dsig, 0.0);
+                if (rp.shift) {                           // e^{-i m phi0}, phi0 = pi / N
+                    ph = __ldg(tw2 + (m & (2 * N - 1)));
+                    ph.x *= dsig; ph.y *= dsig;
+                }
+                double2 E, O;
+                if (equator) { E = cmul(ph, gn); O = make_double2(0.0, 0.0); }
+                else { E = cmul(ph, cadd(gn, gs)); O = cmul(ph, csub(gn, gs)); }
+                if (w.comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }      // i U
+                double2* slot = ostage + ((nstore + q) % NSLOTS) * SLOT;
+                slot[(mi * out_ms) * KT + kkm] = E;
+                slot[(out_hs + mi * out_ms) * KT + kkm] = O;
             }
-            double2 E, O;
-            if (equator) { E = cmul(ph, gn); O = make_double2(0.0, 0.0); }
-            else { E = cmul(ph, cadd(gn, gs)); O = cmul(ph, csub(gn, gs)); }
-            if (w.comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }      // i U
-            double2* slot = out + (nstore & 1) * (MB * 2 * KT);
-            slot[(mi * out_ms) * KT + kkm] = E;
-            slot[(out_hs + mi * out_ms) * KT + kkm] = O;
             fence_async_smem();
-            if (tid == 0) bulk_wait_read<0>();            // the store that used the other slot has read it
+            if (tid == 0) bulk_wait_read<0>();            // the previous round's stores have read their slots
             __syncthreads();
             if (tid == 0) {
-                if (planes) tma_store_5d(&tmF, slot, 0, m0, 2 * w.comp, csel, w.p * d.nkg + kg);
-                else tma_store_5d(&tmF, slot, 0, csel, 2 * w.comp, m0, w.p * d.nkg + kg);
+#pragma unroll
+                for (int q = 0; q < U; ++q) {
+                    const int mq = m0 + q * MB;
+                    if (mq >= mlim) break;
+                    const double2* slot = ostage + ((nstore + q) % NSLOTS) * SLOT;
+                    if (planes) tma_store_5d(&tmF, slot, 0, mq, 2 * w.comp, csel, w.p * d.nkg + kg);
+                    else tma_store_5d(&tmF, slot, 0, csel, 2 * w.comp, mq, w.p * d.nkg + kg);
+                }
                 bulk_commit();
             }
+            nstore += U;
         }
+        // the buffer is free once this item's stores have read it: fetch the rows of the item after the next one
+        if (tid == 0 && it + 2LL * gridDim.x < nitems) {
+            bulk_wait_read<0>();
+            issue_loads(it + 2LL * gridDim.x, buf);
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
+// ------------------------------------------------------------------------------------------------
+// analysis, variant with in-place staging (two CTAs per SM): the rows of an item are bulk-copied straight into the
+// transform buffers; every thread owns exactly one pass-A butterfly, reads its inputs into registers, and the pass
+// writes the buffers in place after a barrier.  No prefetch inside a CTA -- the copy of the next item is in flight while
+// the OTHER CTA of the SM computes -- but twice as many warps per SM as the prefetching variant above.
+// shared memory: [KT transform buffers][4 output slots][mbarrier]
+// ------------------------------------------------------------------------------------------------
+template <int LOGN, int KT>
+__global__ void __launch_bounds__(p2::NT, 2)
+k_ring_analysis_p2i(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const double* __restrict__ maps, int k0, int kmaps,
+                    int p_first, int npairs, int planes)
+{
+    using namespace p2;
+    using G = Geo<LOGN>;
+    constexpr int N = G::N, R1 = G::R1, R2 = G::R2, R3 = G::R3;
+    constexpr int TPM = NT / KT, MB = NT / KT;
+    constexpr int BS = buf_stride<LOGN, KT>();
+    constexpr int SLOT = MB * 2 * KT, NSLOTS = 4, U = 2;
+    static_assert(N / R1 <= TPM, "one pass-A butterfly per thread");
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* tr = reinterpret_cast<double2*>(smem_raw);
+    double2* ostage = tr + KT * BS;
+    uint64_t* full = reinterpret_cast<uint64_t*>(ostage + NSLOTS * SLOT);
+
+    const int tid = threadIdx.x;
+    const int nkp = (kmaps + KT - 1) / KT;
+    const long long nitems = (long long)npairs * d.ncomp * nkp;
+    const int out_hs = planes ? MB : 1, out_ms = planes ? 1 : 2;
+    const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
+    if (tid == 0) {
+        mbar_init(full, 1);
+        fence_barrier_init();
+        tma_prefetch_desc(&tmF);
+    }
+    __syncthreads();
+    auto issue_loads = [&](long long it) {
+        const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
+        const RingPair& rp = d.rings[w.p];
+        const bool eq = rp.start_s < 0;
+        mbar_arrive_expect_tx(full, (uint32_t)(KT * (eq ? 1 : 2) * N * 8));
+#pragma unroll
+        for (int kk = 0; kk < KT; ++kk) {
+            const int k = min(w.kfirst + kk, kmaps - 1);
+            const double* mp = maps + ((size_t)(k0 + k) * d.ncomp + w.comp) * d.npix;
+            double* dst = reinterpret_cast<double*>(tr + kk * BS);
+            bulk_load(dst, mp + rp.start_n, N * 8, full);
+            if (!eq) bulk_load(dst + N, mp + rp.start_s, N * 8, full);
+        }
+    };
+    if (tid == 0 && (long long)blockIdx.x < nitems) issue_loads(blockIdx.x);
+
+    const int kkp = tid / TPM, tm = tid - kkp * TPM;
+    const int kkm = tid & (KT - 1), mi = tid / KT;
+    int li = 0, nstore = 0;
+    for (long long it = blockIdx.x; it < nitems; it += gridDim.x, ++li) {
+        const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
+        const RingPair rp = d.rings[w.p];
+        const bool equator = rp.start_s < 0;
+        const double2* __restrict__ tw2 = d.tw + rp.tw_off;
+        mbar_wait(full, li & 1);
+        double2* trk = tr + kkp * BS;
+        // ---- pass A in place: inputs to registers, barrier, transform, write
+        {
+            const int j = tm;
+            const bool act = j < N / R1;
+            double2 u[R1];
+            if (act) {
+                const double* rows = reinterpret_cast<const double*>(trk);
+#pragma unroll
+                for (int r = 0; r < R1; ++r) {
+                    u[r].x = rows[j + r * (N / R1)];
+                    u[r].y = equator ? 0.0 : rows[N + j + r * (N / R1)];
+                }
+            }
+            __syncthreads();
+            if (act) {
+                dft<R1, false>(u);
+                mul_powers<R1>(u, __ldg(tw2 + 2 * j));
+                const int B = (j >> G::LR3) + R2 * (j & (R3 - 1));
+                double2* dst = trk + R1 * B + B + (j & (R3 - 1));
+#pragma unroll
+                for (int k = 0; k < R1; ++k) dst[k] = u[k];
+            }
+        }
+        __syncthreads();
+        for (int wq = tm; wq < N / R2; wq += TPM) {
+            const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
+            double2* base = trk + k1 + (R1 * R2 + R2 + 1) * n2p;
+            double2 u[R2];
+#pragma unroll
+            for (int t = 0; t < R2; ++t) u[t] = base[(R1 + 1) * t];
+            dft<R2, false>(u);
+            mul_powers<R2>(u, __ldg(tw2 + 2 * R1 * n2p));
+#pragma unroll
+            for (int t = 0; t < R2; ++t) base[(R1 + 1) * t] = u[t];
+        }
+        __syncthreads();
+        for (int wq = tm; wq < N / R3; wq += TPM) {
+            const int k1 = wq & (R1 - 1), k1p = wq >> G::LR1;
+            double2* base = trk + k1 + (R1 + 1) * k1p;
+            double2 u[R3];
+#pragma unroll
+            for (int t = 0; t < R3; ++t) u[t] = base[(R1 * R2 + R2 + 1) * t];
+            dft<R3, false>(u);
+#pragma unroll
+            for (int t = 0; t < R3; ++t) base[(R1 * R2 + R2 + 1) * t] = u[t];
+        }
+        __syncthreads();
+        // ---- FFT mapping, U boxes per round through a ring of NSLOTS output slots
+        const int mlim = rp.mlim;
+        const double2* trm = tr + kkm * BS;
+        const int kg = w.kfirst / KG, csel = (w.kfirst % KG) / KT;
+        for (int m0 = 0; m0 < mlim; m0 += U * MB) {
+#pragma unroll
+            for (int q = 0; q < U; ++q) {
+                const int m = m0 + q * MB + mi;
+                const int b = m & (N - 1), bc = (N - b) & (N - 1);
+                const double2 A = trm[G::phys(b)], Bv = trm[G::phys(bc)];
+                const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
+                const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
+                double2 ph = make_double2(dsig, 0.0);
+                if (rp.shift) {
+                    ph = __ldg(tw2 + (m & (2 * N - 1)));
+                    ph.x *= dsig; ph.y *= dsig;
+                }
+                double2 E, O;
+                if (equator) { E = cmul(ph, gn); O = make_double2(0.0, 0.0); }
+                else { E = cmul(ph, cadd(gn, gs)); O = cmul(ph, csub(gn, gs)); }
+                if (w.comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }
+                double2* slot = ostage + ((nstore + q) % NSLOTS) * SLOT;
+                slot[(mi * out_ms) * KT + kkm] = E;
+                slot[(out_hs + mi * out_ms) * KT + kkm] = O;
+            }
+            fence_async_smem();
+            if (tid == 0) bulk_wait_read<0>();
+            __syncthreads();
+            if (tid == 0) {
+#pragma unroll
+                for (int q = 0; q < U; ++q) {
+                    const int mq = m0 + q * MB;
+                    if (mq >= mlim) break;
+                    const double2* slot = ostage + ((nstore + q) % NSLOTS) * SLOT;
+                    if (planes) tma_store_5d(&tmF, slot, 0, mq, 2 * w.comp, csel, w.p * d.nkg + kg);
+                    else tma_store_5d(&tmF, slot, 0, csel, 2 * w.comp, mq, w.p * d.nkg + kg);
+                }
+                bulk_commit();
+            }
+            nstore += U;
+        }
+        // every thread has passed the last round's barrier, i.e. finished reading the transform buffers
+        if (tid == 0 && it + gridDim.x < nitems) issue_loads(it + gridDim.x);
     }
     if (tid == 0) bulk_wait<0>();
 }
@@ -475,6 +688,384 @@ k_ring_synthesis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     }
 }
 
+// ================================================================================================
+// Cap rings (length N = 4 i, any i) by the chirp-z transform (Bluestein) on top of the compiled transforms:
+//   X_b = c_b sum_n (x_n c_n) h_{b-n},   c_j = exp(-i pi j^2 / N),  h = conj c,
+// a circular convolution of a compiled length L >= 2 N - 1 (L = 2^a or 3 2^a): forward transform (decimation in time,
+// natural-order spectrum), product with the plan's filter spectrum FFT_L(h) / L, inverse transform (the adjoint
+// network), chirp.  The last forward pass, the filter product and the first inverse pass work on the same elements
+// and are one pass in registers.  Data movement as for the belt: bulk copies in, TMA stores out, persistent CTAs.
+// Per ring pair the plan holds [filter spectrum, natural order: L][chirp c_j: N] (cz table).
+// ================================================================================================
+namespace p2 {
+
+template <int R1_, int R2_, int R3_>
+struct GeoT {
+    static constexpr int R1 = R1_, R2 = R2_, R3 = R3_, L = R1_ * R2_ * R3_;
+    static constexpr int LR1 = R1 == 16 ? 4 : 3, LR2 = R2 == 16 ? 4 : 3;
+    static_assert((R1 == 8 || R1 == 16) && (R2 == 8 || R2 == 16), "the first two radices are powers of two");
+    static constexpr int S2 = R1 + 1, S3 = R1 * R2 + R2 + 1;          // physical strides of the second / third digit
+    static constexpr int LPAD = L + L / R1 + L / (R1 * R2);
+    __device__ static __forceinline__ int phys(int p) { return p + (p >> LR1) + (p >> (LR1 + LR2)); }
+};
+
+// forward passes B and the fused [C, filter, C^-1] pass, inverse pass B^-1 of one map's buffer; `tm`, `TPM`: thread
+// inside the map / threads per map; twL[e] = W_L^e; hf: filter spectrum in natural order (CONJ: conjugated)
+template <class G, int TPM, bool CONJ>
+__device__ __forceinline__ void cz_middle(double2* trk, int tm, const double2* __restrict__ twL, const double2* __restrict__ hf)
+{
+    constexpr int R1 = G::R1, R2 = G::R2, R3 = G::R3, L = G::L;
+    for (int wq = tm; wq < L / R2; wq += TPM) {
+        const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
+        double2* base = trk + k1 + G::S3 * n2p;
+        double2 u[R2];
+#pragma unroll
+        for (int t = 0; t < R2; ++t) u[t] = base[G::S2 * t];
+        dft<R2, false>(u);
+        mul_powers<R2>(u, __ldg(twL + R1 * n2p));
+#pragma unroll
+        for (int t = 0; t < R2; ++t) base[G::S2 * t] = u[t];
+    }
+    __syncthreads();
+    for (int wq = tm; wq < L / R3; wq += TPM) {
+        const int k1 = wq & (R1 - 1), k1p = wq >> G::LR1;
+        double2* base = trk + k1 + G::S2 * k1p;
+        double2 u[R3];
+#pragma unroll
+        for (int t = 0; t < R3; ++t) u[t] = base[G::S3 * t];
+        dft<R3, false>(u);
+#pragma unroll
+        for (int t = 0; t < R3; ++t) {                    // spectrum bin k1 + R1 k1' + R1 R2 t
+            double2 h = __ldg(hf + k1 + R1 * k1p + R1 * R2 * t);
+            if (CONJ) h.y = -h.y;
+            u[t] = cmul(u[t], h);
+        }
+        dft<R3, true>(u);
+        double2 wv = __ldg(twL + R1 * k1p);
+        wv.y = -wv.y;
+        mul_powers<R3>(u, wv);
+#pragma unroll
+        for (int t = 0; t < R3; ++t) base[G::S3 * t] = u[t];
+    }
+    __syncthreads();
+    for (int wq = tm; wq < L / R2; wq += TPM) {
+        const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
+        double2* base = trk + k1 + G::S3 * n2p;
+        double2 u[R2];
+#pragma unroll
+        for (int t = 0; t < R2; ++t) u[t] = base[G::S2 * t];
+        dft<R2, true>(u);
+#pragma unroll
+        for (int t = 0; t < R2; ++t) base[G::S2 * t] = u[t];
+    }
+    __syncthreads();
+}
+
+}  // namespace p2
+
+// analysis of the cap ring pairs listed in `ring_list` (all with chirp-z length G::L)
+// shared memory: [KT transform buffers of LPAD][KT row / bin buffers of NB][2 output slots][mbarrier]
+template <class G, int KT>
+__global__ void __launch_bounds__(p2::NT, 1)
+k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const int* __restrict__ ring_list, int nrings,
+                   const double* __restrict__ maps, int k0, int kmaps, const double2* __restrict__ twL, int planes)
+{
+    using namespace p2;
+    constexpr int R1 = G::R1, R2 = G::R2, R3 = G::R3, L = G::L;
+    constexpr int TPM = NT / KT, MB = NT / KT;
+    constexpr int NB = L / 2 + 8;                         // double2 per map of the row / bin buffer (N <= L / 2 + 1)
+    constexpr int SLOT = MB * 2 * KT;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* tr = reinterpret_cast<double2*>(smem_raw);
+    double2* rb = tr + KT * G::LPAD;
+    double2* ostage = rb + KT * NB;
+    uint64_t* full = reinterpret_cast<uint64_t*>(ostage + 2 * SLOT);
+
+    const int tid = threadIdx.x;
+    const int nkp = (kmaps + KT - 1) / KT;
+    const long long nitems = (long long)nrings * d.ncomp * nkp;
+    const int out_hs = planes ? MB : 1, out_ms = planes ? 1 : 2;
+    const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
+    if (tid == 0) {
+        mbar_init(full, 1);
+        fence_barrier_init();
+        tma_prefetch_desc(&tmF);
+    }
+    __syncthreads();
+    auto item_of = [&](long long it, int& p, int& comp, int& kfirst) {
+        const int kp = (int)(it % nkp);
+        const long long r = it / nkp;
+        comp = (int)(r % d.ncomp);
+        p = ring_list[(int)(r / d.ncomp)];
+        kfirst = kp * KT;
+    };
+    auto issue_loads = [&](long long it) {
+        int p, comp, kfirst;
+        item_of(it, p, comp, kfirst);
+        const RingPair& rp = d.rings[p];
+        const int N = rp.n;
+        mbar_arrive_expect_tx(full, (uint32_t)(KT * 2 * N * 8));
+#pragma unroll
+        for (int kk = 0; kk < KT; ++kk) {
+            const int k = min(kfirst + kk, kmaps - 1);
+            const double* mp = maps + ((size_t)(k0 + k) * d.ncomp + comp) * d.npix;
+            double* dst = reinterpret_cast<double*>(rb + kk * NB);
+            bulk_load(dst, mp + rp.start_n, N * 8, full);
+            bulk_load(dst + N, mp + rp.start_s, N * 8, full);
+        }
+    };
+    if (tid == 0 && (long long)blockIdx.x < nitems) issue_loads(blockIdx.x);
+
+    const int kkp = tid / TPM, tm = tid - kkp * TPM;
+    const int kkm = tid & (KT - 1), mi = tid / KT;
+    int li = 0, nstore = 0;
+    for (long long it = blockIdx.x; it < nitems; it += gridDim.x, ++li) {
+        int p, comp, kfirst;
+        item_of(it, p, comp, kfirst);
+        const RingPair rp = d.rings[p];
+        const int N = rp.n;
+        const double2* __restrict__ hf = d.tw + rp.cz_off;          // [L] filter spectrum, then [N] chirp
+        const double2* __restrict__ chirp = hf + L;
+        const double2* __restrict__ tw2 = d.tw + rp.tw_off;          // W_{2N}^j (phase of the FFT mapping)
+        mbar_wait(full, li & 1);
+        double2* trk = tr + kkp * G::LPAD;
+        // ---- pass A: a_n = x_n c_n (zero past N), R1-point transforms over n1 (stride L / R1), twiddle W_L^{n2 k1}
+        {
+            const double* rows = reinterpret_cast<const double*>(rb + kkp * NB);
+            for (int j = tm; j < L / R1; j += TPM) {
+                double2 u[R1];
+#pragma unroll
+                for (int r = 0; r < R1; ++r) {
+                    const int n = j + r * (L / R1);
+                    u[r] = make_double2(0.0, 0.0);
+                    if (n < N) u[r] = cmul(make_double2(rows[n], rows[N + n]), __ldg(chirp + n));
+                }
+                dft<R1, false>(u);
+                mul_powers<R1>(u, __ldg(twL + j));
+                const int n1p = j / R3, n2p = j - n1p * R3;
+                const int B = n1p + R2 * n2p;
+                double2* dst = trk + R1 * B + B + n2p;
+#pragma unroll
+                for (int k = 0; k < R1; ++k) dst[k] = u[k];
+            }
+        }
+        __syncthreads();
+        cz_middle<G, TPM, false>(trk, tm, twL, hf);
+        // ---- pass A^-1: y_n, n = n1 L / R1 + n2; bins X_n = y_n c_n for n < N go to the row buffer (the rows are consumed)
+        {
+            double2* bins = rb + kkp * NB;
+            for (int j = tm; j < L / R1; j += TPM) {
+                const int n1p = j / R3, n2p = j - n1p * R3;
+                const int B = n1p + R2 * n2p;
+                const double2* src = trk + R1 * B + B + n2p;
+                double2 u[R1];
+#pragma unroll
+                for (int q = 0; q < R1; ++q) u[q] = src[q];
+                double2 wv = __ldg(twL + j);
+                wv.y = -wv.y;
+                mul_powers<R1>(u, wv);
+                dft<R1, true>(u);
+#pragma unroll
+                for (int r = 0; r < R1; ++r) {
+                    const int n = j + r * (L / R1);
+                    if (n < N) bins[n] = cmul(u[r], __ldg(chirp + n));
+                }
+            }
+        }
+        __syncthreads();
+        // ---- FFT mapping from the natural-order bins
+        const int mlim = rp.mlim;
+        const double2* bm = rb + kkm * NB;
+        const int kg = kfirst / KG, csel = (kfirst % KG) / KT;
+        for (int m0 = 0; m0 < mlim; m0 += MB, ++nstore) {
+            const int m = m0 + mi;
+            int b = m < N ? m : m % N;
+            const int bc = b == 0 ? 0 : N - b;
+            const double2 A = bm[b], Bv = bm[bc];
+            const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
+            const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
+            double2 ph = make_double2(dsig, 0.0);
+            if (rp.shift) {
+                const int m2 = m < 2 * N ? m : m % (2 * N);
+                ph = __ldg(tw2 + m2);
+                ph.x *= dsig; ph.y *= dsig;
+            }
+            double2 E = cmul(ph, cadd(gn, gs)), O = cmul(ph, csub(gn, gs));
+            if (comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }
+            double2* slot = ostage + (nstore & 1) * SLOT;
+            slot[(mi * out_ms) * KT + kkm] = E;
+            slot[(out_hs + mi * out_ms) * KT + kkm] = O;
+            fence_async_smem();
+            if (tid == 0) bulk_wait_read<0>();
+            __syncthreads();
+            if (tid == 0) {
+                if (planes) tma_store_5d(&tmF, slot, 0, m0, 2 * comp, csel, p * d.nkg + kg);
+                else tma_store_5d(&tmF, slot, 0, csel, 2 * comp, m0, p * d.nkg + kg);
+                bulk_commit();
+            }
+        }
+        if (tid == 0 && it + gridDim.x < nitems) issue_loads(it + gridDim.x);
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
+// synthesis of the cap ring pairs listed in `ring_list` by the chirp-z transform:
+//   x_n = conj(c_n) sum_b (Z_b conj(c_b)) c_{n-b}: the same convolution with the conjugated chirp and filter spectrum.
+// shared memory: [KT transform buffers of LPAD][KT bin buffers of NB][NSL input slots][mbarriers]
+template <class G, int KT, int NSL>
+__global__ void __launch_bounds__(p2::NT, 1)
+k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const int* __restrict__ ring_list, int nrings,
+                    double* __restrict__ maps, int k0, int kmaps, const double2* __restrict__ twL, int planes)
+{
+    using namespace p2;
+    constexpr int R1 = G::R1, R2 = G::R2, R3 = G::R3, L = G::L;
+    constexpr int TPM = NT / KT, MB = NT / KT;
+    constexpr int NB = L / 2 + 8;
+    constexpr int SLOT = MB * 2 * KT;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* in_slots = reinterpret_cast<double2*>(smem_raw);
+    double2* tr = in_slots + NSL * SLOT;
+    double2* zb = tr + KT * G::LPAD;
+    uint64_t* full = reinterpret_cast<uint64_t*>(zb + KT * NB);
+
+    const int tid = threadIdx.x;
+    const int nkp = (kmaps + KT - 1) / KT;
+    const long long nitems = (long long)nrings * d.ncomp * nkp;
+    const int in_hs = planes ? MB : 1, in_ms = planes ? 1 : 2;
+    if (tid == 0) {
+        for (int s = 0; s < NSL; ++s) mbar_init(full + s, 1);
+        fence_barrier_init();
+        tma_prefetch_desc(&tmF);
+    }
+    __syncthreads();
+    auto item_of = [&](long long it, int& p, int& comp, int& kfirst) {
+        const int kp = (int)(it % nkp);
+        const long long r = it / nkp;
+        comp = (int)(r % d.ncomp);
+        p = ring_list[(int)(r / d.ncomp)];
+        kfirst = kp * KT;
+    };
+    // producer (thread 0): the flattened (item, chunk) sequence, NSL chunks ahead
+    long long pit = blockIdx.x;
+    int pm0 = 0, pmlim = 0, pslot = 0, pp = 0, pcomp = 0, pkf = 0;
+    auto producer_begin_item = [&]() {
+        if (pit < nitems) { item_of(pit, pp, pcomp, pkf); pmlim = d.rings[pp].mlim; pm0 = 0; }
+    };
+    auto produce_one = [&]() {
+        if (pit >= nitems) return;
+        mbar_arrive_expect_tx(full + pslot, SLOT * 16);
+        const int kg = pkf / KG, csel = (pkf % KG) / KT;
+        if (planes) tma_load_5d(in_slots + pslot * SLOT, &tmF, full + pslot, 0, pm0, 2 * pcomp, csel, pp * d.nkg + kg);
+        else tma_load_5d(in_slots + pslot * SLOT, &tmF, full + pslot, 0, csel, 2 * pcomp, pm0, pp * d.nkg + kg);
+        pslot = pslot + 1 == NSL ? 0 : pslot + 1;
+        pm0 += MB;
+        if (pm0 >= pmlim) { pit += gridDim.x; producer_begin_item(); }
+    };
+    if (tid == 0) {
+        producer_begin_item();
+        for (int s = 0; s < NSL; ++s) produce_one();
+    }
+
+    const int kkp = tid / TPM, tm = tid - kkp * TPM;
+    const int kkm = tid & (KT - 1), mi = tid / KT;
+    int cslot = 0; uint32_t cphase = 0;
+    for (long long it = blockIdx.x; it < nitems; it += gridDim.x) {
+        int p, comp, kfirst;
+        item_of(it, p, comp, kfirst);
+        const RingPair rp = d.rings[p];
+        const int N = rp.n;
+        const double2* __restrict__ hf = d.tw + rp.cz_off;
+        const double2* __restrict__ chirp = hf + L;
+        const double2* __restrict__ tw2 = d.tw + rp.tw_off;
+        for (int i = tid; i < KT * NB; i += NT) zb[i] = make_double2(0.0, 0.0);
+        __syncthreads();
+        // ---- inverse FFT mapping: accumulate the ring spectrum Z_b, b < N (as in the belt kernel)
+        const int mlim = rp.mlim;
+        double2* zm = zb + kkm * NB;
+        for (int m0 = 0; m0 < mlim; m0 += MB) {
+            mbar_wait(full + cslot, cphase);
+            const double2* slot = in_slots + cslot * SLOT;
+            const int m = m0 + mi;
+            const bool live = m < mlim;
+            double2 zd = make_double2(0.0, 0.0), zc = zd;
+            if (live) {
+                const double2 e = slot[(mi * in_ms) * KT + kkm], o = slot[(in_hs + mi * in_ms) * KT + kkm];
+                double2 fn = cadd(e, o), fs = csub(e, o);
+                if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }
+                double2 ph = make_double2(1.0, 0.0);
+                if (rp.shift) { ph = __ldg(tw2 + (m < 2 * N ? m : m % (2 * N))); ph.y = -ph.y; }
+                const double wgt = (m == 0) ? 0.5 : 1.0;
+                ph.x *= wgt; ph.y *= wgt;
+                const double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
+                zd = make_double2(dn.x - ds.y, dn.y + ds.x);
+                zc = make_double2(dn.x + ds.y, ds.x - dn.y);
+            }
+            const int b1 = m < N ? m : m % N, b2 = b1 == 0 ? 0 : N - b1;
+            // two orders of one chunk meet in a bin only if m + m' = 0 mod N for some pair of the chunk
+            const bool clash = ((2 * m0 + N - 1) / N) * N <= 2 * m0 + 2 * MB - 2;
+            if (live) { double2* c1 = zm + b1; *c1 = cadd(*c1, zd); }
+            if (clash) __syncthreads();
+            if (live) { double2* c2 = zm + b2; *c2 = cadd(*c2, zc); }
+            __syncthreads();
+            if (tid == 0) produce_one();
+            if (++cslot == NSL) { cslot = 0; cphase ^= 1; }
+        }
+        double2* trk = tr + kkp * G::LPAD;
+        // ---- pass A: a_b = Z_b conj(c_b) (zero past N)
+        {
+            const double2* zk = zb + kkp * NB;
+            for (int j = tm; j < L / R1; j += TPM) {
+                double2 u[R1];
+#pragma unroll
+                for (int r = 0; r < R1; ++r) {
+                    const int n = j + r * (L / R1);
+                    u[r] = make_double2(0.0, 0.0);
+                    if (n < N) { double2 c = __ldg(chirp + n); c.y = -c.y; u[r] = cmul(zk[n], c); }
+                }
+                dft<R1, false>(u);
+                mul_powers<R1>(u, __ldg(twL + j));
+                const int n1p = j / R3, n2p = j - n1p * R3;
+                const int B = n1p + R2 * n2p;
+                double2* dst = trk + R1 * B + B + n2p;
+#pragma unroll
+                for (int k = 0; k < R1; ++k) dst[k] = u[k];
+            }
+        }
+        __syncthreads();
+        cz_middle<G, TPM, true>(trk, tm, twL, hf);
+        // ---- pass A^-1: pixels x_n = y_n conj(c_n), north = real part, south = imaginary part
+        {
+            const int k = kfirst + kkp;
+            double* mp = maps + ((size_t)(k0 + (k < kmaps ? k : 0)) * d.ncomp + comp) * d.npix;
+            for (int j = tm; j < L / R1; j += TPM) {
+                const int n1p = j / R3, n2p = j - n1p * R3;
+                const int B = n1p + R2 * n2p;
+                const double2* src = trk + R1 * B + B + n2p;
+                double2 u[R1];
+#pragma unroll
+                for (int q = 0; q < R1; ++q) u[q] = src[q];
+                double2 wv = __ldg(twL + j);
+                wv.y = -wv.y;
+                mul_powers<R1>(u, wv);
+                dft<R1, true>(u);
+                if (k < kmaps) {
+#pragma unroll
+                    for (int r = 0; r < R1; ++r) {
+                        const int n = j + r * (L / R1);
+                        if (n < N) {
+                            double2 c = __ldg(chirp + n); c.y = -c.y;
+                            const double2 x = cmul(u[r], c);
+                            mp[rp.start_n + n] = x.x;
+                            mp[rp.start_s + n] = x.y;
+                        }
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
 // ---- host side -------------------------------------------------------------------------------------------
 // Workspace F as a 5-D tensor for the ring kernels' boxes of [MB orders] x [E, O] x [KT maps]: innermost the 2 KT
 // doubles of KT maps (re, im); c = which KT-map part of the 4-map line; ch = 2 comp + h; m; (p, kg).
@@ -510,13 +1101,32 @@ static cudaError_t make_tmap_ring(const DevicePlan& d, const double* F, int kt, 
 template <int LOGN, int KT>
 static size_t analysis_p2_smem()
 {
-    return (size_t)2 * KT * 2 * (1 << LOGN) * 8 + (size_t)KT * p2::buf_stride<LOGN, KT>() * 16 +
-           (size_t)2 * (p2::NT / KT) * 2 * KT * 16 + 64;
+    return (size_t)2 * KT * 2 * (1 << LOGN) * 8 + (size_t)KT * p2::buf_stride<LOGN, KT>() * 16 + 64;
 }
 template <int LOGN, int KT, int NSL>
 static size_t synthesis_p2_smem()
 {
     return (size_t)NSL * (p2::NT / KT) * 2 * KT * 16 + (size_t)KT * p2::buf_stride<LOGN, KT>() * 16 + 8 * NSL + 64;
+}
+
+template <int LOGN, int KT>
+static cudaError_t run_analysis_p2i(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
+{
+    const size_t sm = (size_t)KT * p2::buf_stride<LOGN, KT>() * 16 + (size_t)4 * (p2::NT / KT) * 2 * KT * 16 + 64;
+    cudaError_t e = cudaFuncSetAttribute(k_ring_analysis_p2i<LOGN, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    CUtensorMap tm;
+    bool planes = true;
+    if (make_tmap_ring(d, F, KT, p2::NT / KT, true, &tm) != cudaSuccess) {
+        planes = false;
+        if ((e = make_tmap_ring(d, F, KT, p2::NT / KT, false, &tm)) != cudaSuccess) return e;
+    }
+    const long long nitems = (long long)pl->belt_count * d.ncomp * ((kmaps + KT - 1) / KT);
+    const long long want = 2LL * pl->sm_count;
+    const unsigned grid = (unsigned)(nitems < want ? nitems : want);
+    k_ring_analysis_p2i<LOGN, KT><<<grid, p2::NT, sm, st>>>(tm, d, maps, k0, kmaps, pl->belt_first, pl->belt_count, planes ? 1 : 0);
+    pl->launches++;
+    return cudaGetLastError();
 }
 
 template <int LOGN, int KT>
@@ -559,9 +1169,106 @@ static cudaError_t run_synthesis_p2(sht_plan_s* pl, const DevicePlan& d, const d
     return cudaGetLastError();
 }
 
+template <class G, int KT>
+static cudaError_t run_analysis_cz(sht_plan_s* pl, const DevicePlan& d, int cls, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
+{
+    constexpr int MB = p2::NT / KT;
+    const size_t sm = (size_t)KT * G::LPAD * 16 + (size_t)KT * (G::L / 2 + 8) * 16 + (size_t)2 * MB * 2 * KT * 16 + 64;
+    auto kern = k_ring_analysis_cz<G, KT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    CUtensorMap tm;
+    bool planes = true;
+    if (make_tmap_ring(d, F, KT, MB, true, &tm) != cudaSuccess) {
+        planes = false;
+        if ((e = make_tmap_ring(d, F, KT, MB, false, &tm)) != cudaSuccess) return e;
+    }
+    int occ = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, p2::NT, sm) != cudaSuccess || occ < 1) { cudaGetLastError(); occ = 1; }
+    const long long nitems = (long long)pl->cz_count[cls] * d.ncomp * ((kmaps + KT - 1) / KT);
+    const long long want = (long long)pl->sm_count * occ;
+    const unsigned grid = (unsigned)(nitems < want ? nitems : want);
+    kern<<<grid, p2::NT, sm, st>>>(tm, d, pl->cz_rings[cls], pl->cz_count[cls], maps, k0, kmaps, d.tw + pl->cz_tw_off[cls], planes ? 1 : 0);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+template <class G, int KT>
+static cudaError_t run_synthesis_cz(sht_plan_s* pl, const DevicePlan& d, int cls, const double* F, double* maps, int k0, int kmaps, cudaStream_t st)
+{
+    constexpr int MB = p2::NT / KT, NSL = 2;
+    const size_t sm = (size_t)KT * G::LPAD * 16 + (size_t)KT * (G::L / 2 + 8) * 16 + (size_t)NSL * MB * 2 * KT * 16 + 64;
+    auto kern = k_ring_synthesis_cz<G, KT, NSL>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) return e;
+    CUtensorMap tm;
+    bool planes = true;
+    if (make_tmap_ring(d, F, KT, MB, true, &tm) != cudaSuccess) {
+        planes = false;
+        if ((e = make_tmap_ring(d, F, KT, MB, false, &tm)) != cudaSuccess) return e;
+    }
+    int occ = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, p2::NT, sm) != cudaSuccess || occ < 1) { cudaGetLastError(); occ = 1; }
+    const long long nitems = (long long)pl->cz_count[cls] * d.ncomp * ((kmaps + KT - 1) / KT);
+    const long long want = (long long)pl->sm_count * occ;
+    const unsigned grid = (unsigned)(nitems < want ? nitems : want);
+    kern<<<grid, p2::NT, sm, st>>>(tm, d, pl->cz_rings[cls], pl->cz_count[cls], maps, k0, kmaps, d.tw + pl->cz_tw_off[cls], planes ? 1 : 0);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+// cap rings on the chirp-z path: one persistent launch per compiled convolution length, longest first
+cudaError_t launch_ring_analysis_cz(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
+{
+    using namespace p2;
+    cudaError_t e = cudaSuccess;
+    for (int c = CZ_NCLASS - 1; c >= 0 && e == cudaSuccess; --c) {
+        if (pl->cz_count[c] == 0) continue;
+        switch (CZ_LEN[c]) {
+            case 512: e = run_analysis_cz<GeoT<8, 8, 8>, 4>(pl, d, c, maps, F, k0, kmaps, st); break;
+            case 768: e = run_analysis_cz<GeoT<8, 8, 12>, 4>(pl, d, c, maps, F, k0, kmaps, st); break;
+            case 1024: e = run_analysis_cz<GeoT<16, 8, 8>, 4>(pl, d, c, maps, F, k0, kmaps, st); break;
+            case 1536: e = run_analysis_cz<GeoT<16, 8, 12>, 2>(pl, d, c, maps, F, k0, kmaps, st); break;
+            case 2048: e = run_analysis_cz<GeoT<16, 16, 8>, 2>(pl, d, c, maps, F, k0, kmaps, st); break;
+            case 3072: e = run_analysis_cz<GeoT<16, 16, 12>, 2>(pl, d, c, maps, F, k0, kmaps, st); break;
+            case 4096: e = run_analysis_cz<GeoT<16, 16, 16>, 2>(pl, d, c, maps, F, k0, kmaps, st); break;
+            default: e = cudaErrorNotSupported;
+        }
+    }
+    return e;
+}
+
+cudaError_t launch_ring_synthesis_cz(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps, cudaStream_t st)
+{
+    using namespace p2;
+    cudaError_t e = cudaSuccess;
+    for (int c = CZ_NCLASS - 1; c >= 0 && e == cudaSuccess; --c) {
+        if (pl->cz_count[c] == 0) continue;
+        switch (CZ_LEN[c]) {
+            case 512: e = run_synthesis_cz<GeoT<8, 8, 8>, 4>(pl, d, c, F, maps, k0, kmaps, st); break;
+            case 768: e = run_synthesis_cz<GeoT<8, 8, 12>, 4>(pl, d, c, F, maps, k0, kmaps, st); break;
+            case 1024: e = run_synthesis_cz<GeoT<16, 8, 8>, 4>(pl, d, c, F, maps, k0, kmaps, st); break;
+            case 1536: e = run_synthesis_cz<GeoT<16, 8, 12>, 2>(pl, d, c, F, maps, k0, kmaps, st); break;
+            case 2048: e = run_synthesis_cz<GeoT<16, 16, 8>, 2>(pl, d, c, F, maps, k0, kmaps, st); break;
+            case 3072: e = run_synthesis_cz<GeoT<16, 16, 12>, 2>(pl, d, c, F, maps, k0, kmaps, st); break;
+            case 4096: e = run_synthesis_cz<GeoT<16, 16, 16>, 2>(pl, d, c, F, maps, k0, kmaps, st); break;
+            default: e = cudaErrorNotSupported;
+        }
+    }
+    return e;
+}
+
 // belt ring pairs of a power-of-two nside through the fast path; returns cudaErrorNotSupported if this plan has none
 cudaError_t launch_ring_analysis_belt(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
 {
+    if (pl->p2_variant == 1) {
+        switch (pl->belt_logn) {
+            case 9: return run_analysis_p2i<9, 4>(pl, d, maps, F, k0, kmaps, st);
+            case 10: return run_analysis_p2i<10, 4>(pl, d, maps, F, k0, kmaps, st);
+            case 11: return run_analysis_p2i<11, 2>(pl, d, maps, F, k0, kmaps, st);
+            default: return cudaErrorNotSupported;
+        }
+    }
     switch (pl->belt_logn) {
         case 9: return run_analysis_p2<9, 4>(pl, d, maps, F, k0, kmaps, st);
         case 10: return run_analysis_p2<10, 4>(pl, d, maps, F, k0, kmaps, st);
