@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsht_b200.so")
-SOURCES = ["sht_plan.cu", "sht_ring_fft.cu", "sht_ring_pow2.cu", "sht_legendre.cu", "sht_legendre_spin2.cu", "sht_api.cu"]
+SOURCES = ["sht_plan.cu", "sht_ring_fft.cu", "sht_ring_pow2.cu", "sht_ring_mixed.cu", "sht_legendre.cu", "sht_legendre_spin2.cu", "sht_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

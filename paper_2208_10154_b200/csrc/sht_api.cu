@@ -335,6 +335,39 @@ static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* al
         timing_end(pl, t, st);
         CUtensorMap tmF, tmA;
         SHT_TRY(legendre_order_maps(d, R, da, kmaps, &tmF, &tmA), "tensor maps");
+        // One sweep is the same sequence of (lmax + 1) / 2 x 3 dependent launches for every iteration of the chunk: it is
+        // captured once into a CUDA graph and replayed (launch overhead of ~9 k launches per sweep at config 5).  If the
+        // caller's stream cannot be captured (it is itself under capture), the launches are issued directly.
+        // an even and an odd order never fall on the same bin of a ring of 4q pixels (m' = +-m mod 4q keeps the parity):
+        // the orders m, m + 1 of a step are independent, and the sweep equals the one-by-one sweep bit for bit
+        auto sweep = [&](cudaStream_t ss) -> sht_status_t {
+            for (int m = 0; m <= d.lmax; m += 2) {
+                const int nm = m < d.lmax ? 2 : 1;
+                SHT_TRY(launch_legendre_analysis_order(pl, d, tmF, alm, da, k0, kmaps, m, nm, ss), "legendre analysis (orders m, m+1)");
+                SHT_TRY(launch_legendre_synthesis_order(pl, d, tmA, S, kmaps, m, nm, ss), "legendre synthesis (orders m, m+1)");
+                SHT_TRY(launch_gs_update(pl, d, S, R, m, nm, kmaps, ss), "residual update");
+            }
+            return SHT_OK;
+        };
+        // captured on a stream of the plan's own (the legacy default stream cannot be captured), replayed on the caller's
+        cudaGraphExec_t gexec = nullptr;
+        long long sweep_launches = 0;
+        if (niter > 0 && !pl->cap_stream && cudaStreamCreateWithFlags(&pl->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+            pl->cap_stream = nullptr;
+            cudaGetLastError();
+        }
+        if (niter > 0 && pl->cap_stream && cudaStreamBeginCapture(pl->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            const long long l0 = pl->launches;
+            const sht_status_t cs = sweep(pl->cap_stream);
+            sweep_launches = pl->launches - l0;
+            pl->launches = l0;
+            cudaGraph_t graph = nullptr;
+            const cudaError_t ce = cudaStreamEndCapture(pl->cap_stream, &graph);
+            if (cs != SHT_OK || ce != cudaSuccess || !graph || cudaGraphInstantiate(&gexec, graph, 0) != cudaSuccess) gexec = nullptr;
+            if (graph) cudaGraphDestroy(graph);
+            if (cs != SHT_OK) return cs;
+        }
+        cudaGetLastError();
         for (int it = 0; it < niter; ++it) {
             if (it > 0 && resid_rms) {
                 SHT_TRY(cudaMemsetAsync(acc, 0, (size_t)nrow * sizeof(double), st), "rms memset");
@@ -347,16 +380,17 @@ static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* al
                 SHT_TRY(cudaGetLastError(), "rms kernel");
             }
             t = timing_begin(pl, 1, st);
-            // an even and an odd order never fall on the same bin of a ring of 4q pixels (m' = +-m mod 4q keeps the parity):
-            // the orders m, m + 1 of a step are independent, and the sweep equals the one-by-one sweep bit for bit
-            for (int m = 0; m <= d.lmax; m += 2) {
-                const int nm = m < d.lmax ? 2 : 1;
-                SHT_TRY(launch_legendre_analysis_order(pl, d, tmF, alm, da, k0, kmaps, m, nm, st), "legendre analysis (orders m, m+1)");
-                SHT_TRY(launch_legendre_synthesis_order(pl, d, tmA, S, kmaps, m, nm, st), "legendre synthesis (orders m, m+1)");
-                SHT_TRY(launch_gs_update(pl, d, S, R, m, nm, kmaps, st), "residual update");
+            if (gexec) {
+                const cudaError_t ge = cudaGraphLaunch(gexec, st);
+                if (ge != cudaSuccess) { cudaGraphExecDestroy(gexec); return cuda_fail(pl, "sweep graph launch", ge); }
+                pl->launches += sweep_launches;
+            } else {
+                const sht_status_t ss = sweep(st);
+                if (ss != SHT_OK) return ss;
             }
             timing_end(pl, t, st);
         }
+        if (gexec) cudaGraphExecDestroy(gexec);          // released once its queued launches have run
     }
     return SHT_OK;
 }

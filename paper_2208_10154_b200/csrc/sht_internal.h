@@ -50,6 +50,8 @@ struct RingPair {
     // chirp-z fast path of the cap rings (sht_ring_pow2.cu): convolution length (0: not on that path) and the offset
     // (double2) of [filter spectrum FFT_L(conj chirp) / L in natural order: cz_len][chirp c_j: n]
     int cz_len, cz_off;
+    // mixed-radix fast path (sht_ring_mixed.cu): n = mr_r1 mr_r2 mr_r3, all >= 2 (mr_r1 = 0: not on that path)
+    int mr_r1, mr_r2, mr_r3;
 };
 
 struct DevicePlan {
@@ -103,7 +105,7 @@ struct sht_plan_s {
     double* F;                      // workspace, layout above
     size_t F_bytes;
     size_t table_bytes;
-    void* dev_allocs[48];
+    void* dev_allocs[64];
     int n_allocs;
     // ring-kernel launch classes: rings grouped by the dynamic shared memory their CTA needs
     int* class_rings[sht::RING_NCLASS];     // device lists of ring-pair indices
@@ -118,6 +120,9 @@ struct sht_plan_s {
     int* class_rings_nb[sht::RING_NCLASS];
     int class_count_nb[sht::RING_NCLASS];
     int class_ktmin_nb[sht::RING_NCLASS];
+    // mixed-radix fast path: ring pairs by length class (MR_NCLASS), the longest ring of each class
+    int* mr_rings[6];
+    int mr_count[6], mr_nmax[6];
     // chirp-z fast path: ring pairs by convolution length (CZ_NCLASS compiled lengths), their W_L tables
     int* cz_rings[8];
     int cz_count[8], cz_tw_off[8];
@@ -142,6 +147,7 @@ struct sht_plan_s {
     int host_nb;                    // chunks in flight in the host path (streams, staging buffers, workspace slices)
     int host_chunk;
     cudaStream_t hstream[4];
+    cudaStream_t cap_stream;        // Alg. 3: the sweep is captured on this stream (created on first use)
     cudaEvent_t hevent;             // host path: lambda blocks of the call are ready
     bool host_ready;
     // optional per-stage timing (sht_plan_set_timing)
@@ -166,6 +172,11 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
 // belt fast path (sht_ring_pow2.cu)
 cudaError_t launch_ring_analysis_belt(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st);
 cudaError_t launch_ring_synthesis_belt(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps, cudaStream_t st);
+// mixed-radix fast path of the cap rings (sht_ring_mixed.cu): length classes N <= 512, <= 1024, <= 2048
+constexpr int MR_NCLASS = 3;
+constexpr int MR_MIN_N = 256, MR_MAX_N = 2048;
+cudaError_t launch_ring_analysis_mr(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st);
+cudaError_t launch_ring_synthesis_mr(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps, cudaStream_t st);
 // chirp-z fast path of the cap rings: the compiled convolution lengths
 constexpr int CZ_NCLASS = 7;
 constexpr int CZ_LEN[CZ_NCLASS] = {512, 768, 1024, 1536, 2048, 3072, 4096};

@@ -159,7 +159,8 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     // whole transform: one CTA per (m, k-tile), all l tiles.  A few orders at a time (Alg. 3, tsplit = number of orders
     // m0, m0 + 1, ..): one CTA per (order, l tile, k-tile) -- the tiles restart from the state table, so they are
     // independent; the grid is sized for the tiles of m0, the CTAs past the last tile of their order leave
-    const int nt0 = (d.lmax - m0) / A_ML + 1;
+    // tsplit > 0: tile-split mode, tsplit = l tiles per CTA (the grid is sized for the tile groups of order m0)
+    const int nt0 = ((d.lmax - m0) / A_ML + tsplit) / (tsplit > 0 ? tsplit : 1);
     const int m = tsplit ? m0 + blockIdx.x / (nkt * nt0) : m0 + blockIdx.x / nkt, kt = blockIdx.x % nkt;
     // warps 0..3 generate (the oldest warps of an SM sub-partition are served first by its scheduler: their
     // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
@@ -168,7 +169,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
     const int ntile = (lmax - m) / A_ML + 1;
-    const int tb = tsplit ? (int)(blockIdx.x / nkt) % nt0 : 0, te = tsplit ? tb + 1 : ntile;
+    const int tb = tsplit ? ((int)(blockIdx.x / nkt) % nt0) * tsplit : 0, te = tsplit ? min(tb + tsplit, ntile) : ntile;
     if (tb >= ntile) return;
 
     for (int t = tix; t < ntile; t += LEG_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
@@ -659,7 +660,7 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
     // leg_tsplit: one CTA per (m, l tile, k-tile) instead of per (m, k-tile): the l tiles of an (m, k-tile) then read the
     // same T_m boxes at about the same time from different SMs, and L2 serves the re-reads
     const int tsplit = pl->leg_tsplit;
-    const unsigned grid = (unsigned)((d.lmax + 1) * nkt * (tsplit ? d.ntile_max : 1));
+    const unsigned grid = (unsigned)((d.lmax + 1) * nkt * (tsplit ? (d.ntile_max + tsplit - 1) / tsplit : 1));
     const size_t sm = analysis_smem(d.ntile_max);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
@@ -693,7 +694,7 @@ cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, 
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int ntile = (d.lmax - m) / A_ML + 1;
     k_legendre_analysis<<<(unsigned)(nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
-                                                                                                      nullptr, m, nm, da);
+                                                                                                      nullptr, m, 1, da);
     pl->launches++;
     return cudaGetLastError();
 }

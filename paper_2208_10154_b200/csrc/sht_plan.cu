@@ -359,6 +359,38 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             perm.push_back((unsigned short)pos);
         }
     }
+    // ---- mixed-radix fast path of the cap rings: N = 4 q = r1 r2 r3 with r1 >= r2 >= r3 >= 2 from the codelet set of
+    // sht_ring_mixed.cu -- radices up to 16 if such a split exists (two CTAs per SM), else also 17, 19, 20, 23, 29, 31;
+    // among the splits the one with the smallest largest radix (registers), then the largest smallest radix
+    std::vector<int> mr1_of_q(nside + 1, 0), mr2_of_q(nside + 1, 0), mr3_of_q(nside + 1, 0);
+    {
+        const int small_set[] = {2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16};
+        const int big_set[] = {2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17, 19, 20, 23, 29, 31};
+        for (int q = 1; q < nside; ++q) {
+            const int n = 4 * q;
+            if (n < MR_MIN_N || n > MR_MAX_N) continue;
+            for (int pass = 0; pass < 2 && !mr1_of_q[q]; ++pass) {
+                const int* set = pass == 0 ? small_set : big_set;
+                const int ns_ = pass == 0 ? 15 : 21;
+                int best[3] = {0, 0, 0};
+                for (int ia = 0; ia < ns_; ++ia) {
+                    const int a = set[ia];
+                    if (n % a) continue;
+                    for (int ib = 0; ib <= ia; ++ib) {
+                        const int b = set[ib];
+                        if ((n / a) % b) continue;
+                        const int c = n / a / b;
+                        if (c < 2 || c > b) continue;
+                        bool ok = false;
+                        for (int ic = 0; ic < ns_; ++ic) ok = ok || set[ic] == c;
+                        if (!ok) continue;
+                        if (!best[0] || a < best[0] || (a == best[0] && c > best[2])) { best[0] = a; best[1] = b; best[2] = c; }
+                    }
+                }
+                if (best[0]) { mr1_of_q[q] = best[0]; mr2_of_q[q] = best[1]; mr3_of_q[q] = best[2]; }
+            }
+        }
+    }
     // ---- chirp-z fast path of the cap rings: per ring length N = 4 q >= CZ_MIN_N with 2 N - 1 <= 4096 the filter spectrum
     // FFT_L(h) / L (h_j = exp(+i pi j^2 / N) at j = -(N-1) .. N-1 mod L; long double, natural order) and the chirp
     std::vector<int> cz_len_of_q(nside + 1, 0), cz_off_of_q(nside + 1, 0);
@@ -367,7 +399,7 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
         std::vector<int> todo;
         for (int q = 1; q < nside; ++q) {
             const int n = 4 * q;
-            if (n < CZ_MIN_N) continue;
+            if (n < CZ_MIN_N || mr1_of_q[q]) continue;       // the mixed-radix path comes first
             for (int c = 0; c < CZ_NCLASS; ++c)
                 if (CZ_LEN[c] >= 2 * n - 1) { cz_len_of_q[q] = CZ_LEN[c]; break; }
             if (cz_len_of_q[q]) {
@@ -458,6 +490,7 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             }
             r.pbits = a;
         }
+        r.mr_r1 = (i < ns) ? mr1_of_q[q] : 0; r.mr_r2 = mr2_of_q[q]; r.mr_r3 = mr3_of_q[q];
         r.cz_len = (i < ns) ? cz_len_of_q[q] : 0;
         r.cz_off = cz_off_of_q[q];
         r.mlim = lmax + 1;                               // tightened below from the l_safe table
@@ -698,7 +731,7 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             pl->class_ktmin_nb[c] = 16;
             for (int p : lists[c]) {
                 if (pl->belt_logn && p >= pl->belt_first) continue;
-                if (rings[p].cz_len) continue;
+                if (rings[p].cz_len || rings[p].mr_r1) continue;
                 nb.push_back(p);
                 if (rings[p].kt < pl->class_ktmin_nb[c]) pl->class_ktmin_nb[c] = rings[p].kt;
             }
@@ -706,6 +739,24 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             const int* dp = nullptr;
             if (upload(pl, nb, &dp) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
             pl->class_rings_nb[c] = const_cast<int*>(dp);
+        }
+        for (int c = 0; c < 2 * MR_NCLASS; ++c) {            // mixed-radix classes: length class + 3 (radix above 16)
+            std::vector<int> lst;
+            int nmax = 0;
+            for (int p = d.nh - 1; p >= 0; --p) {
+                const RingPair& r = rings[p];
+                if (!r.mr_r1) continue;
+                const int lc = r.n <= 512 ? 0 : r.n <= 1024 ? 1 : 2;
+                const int big = (r.mr_r1 > 16) ? 1 : 0;
+                if (lc + MR_NCLASS * big != c) continue;
+                lst.push_back(p);
+                if (r.n > nmax) nmax = r.n;
+            }
+            pl->mr_count[c] = (int)lst.size();
+            pl->mr_nmax[c] = nmax;
+            const int* dp = nullptr;
+            if (upload(pl, lst, &dp) != cudaSuccess) { sht_plan_destroy(pl); return SHT_ERR_ALLOC; }
+            pl->mr_rings[c] = const_cast<int*>(dp);
         }
         for (int c = 0; c < CZ_NCLASS; ++c) {                // longest rings first
             std::vector<int> lst;
@@ -778,6 +829,7 @@ extern "C" sht_status_t sht_plan_destroy(sht_plan_t pl)
     }
     free(pl->ev0); free(pl->ev1); free(pl->ev_stage);
     if (pl->hevent) cudaEventDestroy(pl->hevent);
+    if (pl->cap_stream) cudaStreamDestroy(pl->cap_stream);
     for (int i = 0; i < 4; ++i) {
         if (pl->stage_maps[i]) cudaFree(pl->stage_maps[i]);
         if (pl->stage_alm[i]) cudaFree(pl->stage_alm[i]);

@@ -1114,6 +1114,7 @@ cudaError_t launch_ring_analysis(sht_plan_s* pl, const DevicePlan& d, const doub
     const bool fast = upow == nullptr && pl->fast_ring;
     if (fast && pl->belt_logn && (e = launch_ring_analysis_belt(pl, d, maps, F, k0, kmaps, st)) != cudaSuccess) return e;
     if (fast && (e = launch_ring_analysis_cz(pl, d, maps, F, k0, kmaps, st)) != cudaSuccess) return e;
+    if (fast && (e = launch_ring_analysis_mr(pl, d, maps, F, k0, kmaps, st)) != cudaSuccess) return e;
     int* const* lists = fast ? pl->class_rings_nb : pl->class_rings;
     const int* count = fast ? pl->class_count_nb : pl->class_count;
     const int* ktmin = fast ? pl->class_ktmin_nb : pl->class_ktmin;
@@ -1135,6 +1136,7 @@ cudaError_t launch_ring_synthesis(sht_plan_s* pl, const DevicePlan& d, const dou
     const bool fast = sub_from == nullptr && pl->fast_ring;
     if (fast && pl->belt_logn && (e = launch_ring_synthesis_belt(pl, d, F, maps, k0, kmaps, st)) != cudaSuccess) return e;
     if (fast && (e = launch_ring_synthesis_cz(pl, d, F, maps, k0, kmaps, st)) != cudaSuccess) return e;
+    if (fast && (e = launch_ring_synthesis_mr(pl, d, F, maps, k0, kmaps, st)) != cudaSuccess) return e;
     int* const* lists = fast ? pl->class_rings_nb : pl->class_rings;
     const int* count = fast ? pl->class_count_nb : pl->class_count;
     const int* ktmin = fast ? pl->class_ktmin_nb : pl->class_ktmin;

@@ -16,18 +16,12 @@
 //     writes the pixels of the two rings coalesced.
 // The north and the south ring of a pair are the real and the imaginary part of one complex sequence, as in the
 // general kernels.  Twiddles: one table value per butterfly, the other powers by multiplication.
-#include "sht_legendre_common.cuh"
+#include "sht_ring_common.cuh"
 
 namespace sht {
 
 namespace p2 {
 
-__device__ __forceinline__ double2 cmul(double2 a, double2 b)
-{
-    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
-}
-__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
 
 // multiply by exp(-+ 2 pi i k / 16), k compile-time (- forward, + if INV)
 template <int K, bool INV>
@@ -134,19 +128,23 @@ __device__ __forceinline__ void dft(double2 (&u)[R])
     }
 }
 
-// u[k] *= w^k, k = 1 .. R-1: the powers by multiplication, w^k = w^{hb(k)} w^{k - hb(k)}, hb = highest bit (depth <= 4)
+// u[k] *= w^k, k = 1 .. R-1: the powers by multiplication, w^{4 i + r} = (w^4)^i w^r with w, w^2, w^3 and the running
+// (w^4)^i kept (few live registers; dependency depth <= 5 complex products)
 template <int R>
 __device__ __forceinline__ void mul_powers(double2 (&u)[R], double2 w)
 {
-    double2 pw[R];
-    pw[1] = w;
+    static_assert(R % 4 == 0, "radix");
+    const double2 w2 = cmul(w, w), w3 = cmul(w2, w);
+    u[1] = cmul(u[1], w); u[2] = cmul(u[2], w2); u[3] = cmul(u[3], w3);
+    double2 b = cmul(w2, w2);                             // w^4
 #pragma unroll
-    for (int k = 2; k < R; ++k) {
-        const int hb = k >= 8 ? 8 : k >= 4 ? 4 : 2;
-        pw[k] = (k == hb) ? cmul(pw[k / 2], pw[k / 2]) : cmul(pw[hb], pw[k - hb]);
+    for (int i = 1; i < R / 4; ++i) {
+        u[4 * i] = cmul(u[4 * i], b);
+        u[4 * i + 1] = cmul(u[4 * i + 1], cmul(b, w));
+        u[4 * i + 2] = cmul(u[4 * i + 2], cmul(b, w2));
+        u[4 * i + 3] = cmul(u[4 * i + 3], cmul(b, w3));
+        if (i + 1 < R / 4) b = (i == 1) ? cmul(b, b) : cmul(b, cmul(w2, w2));     // w^8 = (w^4)^2, w^12 = w^8 w^4
     }
-#pragma unroll
-    for (int k = 1; k < R; ++k) u[k] = cmul(u[k], pw[k]);
 }
 
 // transform geometry of a ring length N = 2^LOGN = R1 R2 R3
@@ -171,26 +169,6 @@ __host__ __device__ constexpr int buf_stride()
 {
     constexpr int np = Geo<LOGN>::NPAD, want = (8 / KT) & 7;
     return np + ((want - (np & 7)) & 7);
-}
-
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-template <int NKEEP>
-__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(NKEEP) : "memory"); }
-template <int NKEEP>
-__device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(NKEEP) : "memory"); }
-__device__ __forceinline__ void tma_store_5d(const CUtensorMap* map, const void* src, int c0, int c1, int c2, int c3, int c4)
-{
-    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];"
-                 ::"l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
-                 : "memory");
-}
-__device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2, int c3, int c4)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
-        : "memory");
 }
 
 constexpr int NT = 256;                                  // threads per CTA (one CTA per SM)
@@ -274,19 +252,33 @@ k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
 
     const int kkp = tid / TPM, tm = tid - kkp * TPM;      // passes: map and thread inside the map
     const int kkm = tid & (KT - 1), mi = tid / KT;        // mapping: map (fastest) and order inside the sweep
+    // per-thread constants of the whole launch (every belt ring has the same length): pass twiddles W_N^j, W_N^{R1 n2'},
+    // and the phase recurrence of the FFT mapping, W_{2N}^{mi} d sigma and W_{2N}^{MB}
+    constexpr int NIA = (N / R1 + TPM - 1) / TPM, NIB = (N / R2 + TPM - 1) / TPM;
+    const double2* __restrict__ twc = d.tw + d.rings[p_first].tw_off;
+    double2 twA[NIA], twB[NIB];
+#pragma unroll
+    for (int i = 0; i < NIA; ++i) twA[i] = __ldg(twc + 2 * ((tm + i * TPM) & (N / R1 - 1)));
+#pragma unroll
+    for (int i = 0; i < NIB; ++i) twB[i] = __ldg(twc + 2 * R1 * (((tm + i * TPM) & (N / R2 - 1)) >> G::LR1));
+    double2 ph0 = __ldg(twc + (mi & (2 * N - 1)));
+    ph0.x *= dsig; ph0.y *= dsig;
+    const double2 phs = __ldg(twc + (MB & (2 * N - 1)));
     int li = 0, nstore = 0;
     for (long long it = blockIdx.x; it < nitems; it += gridDim.x, ++li) {
         const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
         const RingPair rp = d.rings[w.p];
         const bool equator = rp.start_s < 0;
-        const double2* __restrict__ tw2 = d.tw + rp.tw_off;          // W_{2N}^j; W_N^e = tw2[2 e]
         const int buf = li & 1;
         mbar_wait(full + buf, (li >> 1) & 1);
         const double* rows = in_buf + (size_t)buf * IN_DOUBLES + kkp * 2 * N;
         double2* trk = tr + kkp * BS;
 
         // ---- pass A: R1-point transforms over n1 (input stride N / R1), twiddle W_N^{n2 k1}, R1 consecutive positions
-        for (int j = tm; j < N / R1; j += TPM) {
+#pragma unroll
+        for (int i = 0; i < NIA; ++i) {
+            const int j = tm + i * TPM;
+            if (j >= N / R1) break;
             double2 u[R1];
 #pragma unroll
             for (int r = 0; r < R1; ++r) {
@@ -294,7 +286,7 @@ k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
                 u[r].y = equator ? 0.0 : rows[N + j + r * (N / R1)];
             }
             dft<R1, false>(u);
-            mul_powers<R1>(u, __ldg(tw2 + 2 * j));
+            mul_powers<R1>(u, twA[i]);
             const int B = (j >> G::LR3) + R2 * (j & (R3 - 1));       // n1' + R2 n2'
             double2* dst = trk + R1 * B + B + (j & (R3 - 1));        // phys(R1 B + k1) = R1 B + k1 + B + n2'
 #pragma unroll
@@ -303,14 +295,17 @@ k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
         __syncthreads();
 
         // ---- pass B: R2-point transforms over n1' at positions k1 + R1 t + R1 R2 n2', twiddle W_{R2 R3}^{n2' k1'}
-        for (int wq = tm; wq < N / R2; wq += TPM) {
+#pragma unroll
+        for (int i = 0; i < NIB; ++i) {
+            const int wq = tm + i * TPM;
+            if (wq >= N / R2) break;
             const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
             double2* base = trk + k1 + (R1 * R2 + R2 + 1) * n2p;
             double2 u[R2];
 #pragma unroll
             for (int t = 0; t < R2; ++t) u[t] = base[(R1 + 1) * t];
             dft<R2, false>(u);
-            mul_powers<R2>(u, __ldg(tw2 + 2 * R1 * n2p));
+            mul_powers<R2>(u, twB[i]);
 #pragma unroll
             for (int t = 0; t < R2; ++t) base[(R1 + 1) * t] = u[t];
         }
@@ -335,6 +330,9 @@ k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
         const double2* trm = tr + kkm * BS;
         const int kg = w.kfirst / KG, csel = (w.kfirst % KG) / KT;
         double2* const ostage = reinterpret_cast<double2*>(in_buf + (size_t)buf * IN_DOUBLES);
+        // phase of order m = m0 + q MB + mi by recurrence from the thread's own W_{2N}^{mi} (no table read per order)
+        double2 phc = rp.shift ? ph0 : make_double2(dsig, 0.0);
+        const double2 pstep = rp.shift ? phs : make_double2(1.0, 0.0);
         for (int m0 = 0; m0 < mlim; m0 += U * MB) {
 #pragma unroll
             for (int q = 0; q < U; ++q) {
@@ -344,11 +342,8 @@ k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
                 // G_north = (A + conj B) / 2, G_south = (A - conj B) / (2 i)
                 const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
                 const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
-                double2 ph = make_double2(dsig, 0.0);
-                if (rp.shift) {                           // e^{-i m phi0}, phi0 = pi / N
-                    ph = __ldg(tw2 + (m & (2 * N - 1)));
-                    ph.x *= dsig; ph.y *= dsig;
-                }
+                const double2 ph = phc;                   // d sigma e^{-i m phi0}, phi0 = pi / N on the shifted rings
+                phc = cmul(phc, pstep);
                 double2 E, O;
                 if (equator) { E = cmul(ph, gn); O = make_double2(0.0, 0.0); }
                 else { E = cmul(ph, cadd(gn, gs)); O = cmul(ph, csub(gn, gs)); }
@@ -435,12 +430,23 @@ k_ring_analysis_p2i(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
 
     const int kkp = tid / TPM, tm = tid - kkp * TPM;
     const int kkm = tid & (KT - 1), mi = tid / KT;
+    // per-thread constants of the whole launch (every belt ring has the same length): pass twiddles W_N^j, W_N^{R1 n2'},
+    // and the phase recurrence of the FFT mapping, W_{2N}^{mi} d sigma and W_{2N}^{MB}
+    constexpr int NIA = (N / R1 + TPM - 1) / TPM, NIB = (N / R2 + TPM - 1) / TPM;
+    const double2* __restrict__ twc = d.tw + d.rings[p_first].tw_off;
+    double2 twA[NIA], twB[NIB];
+#pragma unroll
+    for (int i = 0; i < NIA; ++i) twA[i] = __ldg(twc + 2 * ((tm + i * TPM) & (N / R1 - 1)));
+#pragma unroll
+    for (int i = 0; i < NIB; ++i) twB[i] = __ldg(twc + 2 * R1 * (((tm + i * TPM) & (N / R2 - 1)) >> G::LR1));
+    double2 ph0 = __ldg(twc + (mi & (2 * N - 1)));
+    ph0.x *= dsig; ph0.y *= dsig;
+    const double2 phs = __ldg(twc + (MB & (2 * N - 1)));
     int li = 0, nstore = 0;
     for (long long it = blockIdx.x; it < nitems; it += gridDim.x, ++li) {
         const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
         const RingPair rp = d.rings[w.p];
         const bool equator = rp.start_s < 0;
-        const double2* __restrict__ tw2 = d.tw + rp.tw_off;
         mbar_wait(full, li & 1);
         double2* trk = tr + kkp * BS;
         // ---- pass A in place: inputs to registers, barrier, transform, write
@@ -459,7 +465,7 @@ k_ring_analysis_p2i(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
             __syncthreads();
             if (act) {
                 dft<R1, false>(u);
-                mul_powers<R1>(u, __ldg(tw2 + 2 * j));
+                mul_powers<R1>(u, twA[0]);
                 const int B = (j >> G::LR3) + R2 * (j & (R3 - 1));
                 double2* dst = trk + R1 * B + B + (j & (R3 - 1));
 #pragma unroll
@@ -467,14 +473,17 @@ k_ring_analysis_p2i(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
             }
         }
         __syncthreads();
-        for (int wq = tm; wq < N / R2; wq += TPM) {
+#pragma unroll
+        for (int i = 0; i < NIB; ++i) {
+            const int wq = tm + i * TPM;
+            if (wq >= N / R2) break;
             const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
             double2* base = trk + k1 + (R1 * R2 + R2 + 1) * n2p;
             double2 u[R2];
 #pragma unroll
             for (int t = 0; t < R2; ++t) u[t] = base[(R1 + 1) * t];
             dft<R2, false>(u);
-            mul_powers<R2>(u, __ldg(tw2 + 2 * R1 * n2p));
+            mul_powers<R2>(u, twB[i]);
 #pragma unroll
             for (int t = 0; t < R2; ++t) base[(R1 + 1) * t] = u[t];
         }
@@ -494,6 +503,8 @@ k_ring_analysis_p2i(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
         const int mlim = rp.mlim;
         const double2* trm = tr + kkm * BS;
         const int kg = w.kfirst / KG, csel = (w.kfirst % KG) / KT;
+        double2 phc = rp.shift ? ph0 : make_double2(dsig, 0.0);
+        const double2 pstep = rp.shift ? phs : make_double2(1.0, 0.0);
         for (int m0 = 0; m0 < mlim; m0 += U * MB) {
 #pragma unroll
             for (int q = 0; q < U; ++q) {
@@ -502,11 +513,8 @@ k_ring_analysis_p2i(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
                 const double2 A = trm[G::phys(b)], Bv = trm[G::phys(bc)];
                 const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
                 const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
-                double2 ph = make_double2(dsig, 0.0);
-                if (rp.shift) {
-                    ph = __ldg(tw2 + (m & (2 * N - 1)));
-                    ph.x *= dsig; ph.y *= dsig;
-                }
+                const double2 ph = phc;                   // d sigma e^{-i m phi0}, phi0 = pi / N on the shifted rings
+                phc = cmul(phc, pstep);
                 double2 E, O;
                 if (equator) { E = cmul(ph, gn); O = make_double2(0.0, 0.0); }
                 else { E = cmul(ph, cadd(gn, gs)); O = cmul(ph, csub(gn, gs)); }
@@ -545,7 +553,7 @@ k_ring_analysis_p2i(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
 // (eq. 4; at the self-conjugate bins 0 and N/2 the two add up to the real parts, reading G8).
 // ------------------------------------------------------------------------------------------------
 template <int LOGN, int KT, int NSL>
-__global__ void __launch_bounds__(p2::NT, 1)
+__global__ void __launch_bounds__(p2::NT, 2)
 k_ring_synthesis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ maps, int k0, int kmaps,
                     int p_first, int npairs, int planes)
 {
@@ -595,17 +603,30 @@ k_ring_synthesis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
 
     const int kkp = tid / TPM, tm = tid - kkp * TPM;
     const int kkm = tid & (KT - 1), mi = tid / KT;
+    // per-thread constants of the whole launch: conjugate pass twiddles, and the phase recurrence of the inverse mapping
+    constexpr int NIA = (N / R1 + TPM - 1) / TPM, NIC = (N / R3 + TPM - 1) / TPM;
+    const double2* __restrict__ twc = d.tw + d.rings[p_first].tw_off;
+    double2 twA[NIA], twC[NIC];
+#pragma unroll
+    for (int i = 0; i < NIA; ++i) { twA[i] = __ldg(twc + 2 * ((tm + i * TPM) & (N / R1 - 1))); twA[i].y = -twA[i].y; }
+#pragma unroll
+    for (int i = 0; i < NIC; ++i) { twC[i] = __ldg(twc + 2 * R1 * (((tm + i * TPM) & (N / R3 - 1)) >> G::LR1)); twC[i].y = -twC[i].y; }
+    double2 ph0 = __ldg(twc + (mi & (2 * N - 1)));       // e^{+i mi phi0}
+    ph0.y = -ph0.y;
+    double2 phs = __ldg(twc + (MB & (2 * N - 1)));
+    phs.y = -phs.y;
     int cslot = 0; uint32_t cphase = 0;
     for (long long it = blockIdx.x; it < nitems; it += gridDim.x) {
         const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
         const RingPair rp = d.rings[w.p];
         const bool equator = rp.start_s < 0;
-        const double2* __restrict__ tw2 = d.tw + rp.tw_off;
         for (int i = tid; i < KT * BS; i += NT) tr[i] = make_double2(0.0, 0.0);
         __syncthreads();
         // ---- inverse FFT mapping: accumulate the ring spectrum
         const int mlim = rp.mlim;
         double2* trm = tr + kkm * BS;
+        double2 phc = rp.shift ? ph0 : make_double2(1.0, 0.0);
+        const double2 pstep = rp.shift ? phs : make_double2(1.0, 0.0);
         for (int m0 = 0; m0 < mlim; m0 += MB) {
             mbar_wait(full + cslot, cphase);
             const double2* slot = in_slots + cslot * SLOT;
@@ -617,14 +638,14 @@ k_ring_synthesis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                 double2 fn = cadd(e, o), fs = csub(e, o);                        // stored as (even, odd) sums
                 if (w.comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }   // U = -i (iU)
                 if (equator) fs = make_double2(0.0, 0.0);
-                double2 ph = make_double2(1.0, 0.0);
-                if (rp.shift) { ph = __ldg(tw2 + (m & (2 * N - 1))); ph.y = -ph.y; }
+                double2 ph = phc;
                 const double wgt = (m == 0) ? 0.5 : 1.0;
                 ph.x *= wgt; ph.y *= wgt;
                 const double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
                 zd = make_double2(dn.x - ds.y, dn.y + ds.x);                     // d_n + i d_s
                 zc = make_double2(dn.x + ds.y, ds.x - dn.y);                     // conj d_n + i conj d_s
             }
+            phc = cmul(phc, pstep);
             const int b1 = m & (N - 1), b2 = (N - b1) & (N - 1);
             // two orders of one chunk meet in a bin only if m + m' = 0 mod N for some pair of the chunk
             const bool clash = ((2 * m0 + N - 1) / N) * N <= 2 * m0 + 2 * MB - 2;
@@ -637,16 +658,17 @@ k_ring_synthesis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
         }
         double2* trk = tr + kkp * BS;
         // ---- pass C^-1: inverse R3-point transforms over k2', then the conjugate twiddle W_{R2 R3}^{-n2' k1'}
-        for (int wq = tm; wq < N / R3; wq += TPM) {
+#pragma unroll
+        for (int i = 0; i < NIC; ++i) {
+            const int wq = tm + i * TPM;
+            if (wq >= N / R3) break;
             const int k1 = wq & (R1 - 1), k1p = wq >> G::LR1;
             double2* base = trk + k1 + (R1 + 1) * k1p;
             double2 u[R3];
 #pragma unroll
             for (int t = 0; t < R3; ++t) u[t] = base[(R1 * R2 + R2 + 1) * t];
             dft<R3, true>(u);
-            double2 wv = __ldg(tw2 + 2 * R1 * k1p);       // W_N^{R1 k1'}: (W^{k1'})^{n2'}, n2' = t
-            wv.y = -wv.y;
-            mul_powers<R3>(u, wv);
+            mul_powers<R3>(u, twC[i]);                    // conj W_N^{R1 k1'}: (W^{k1'})^{n2'}, n2' = t
 #pragma unroll
             for (int t = 0; t < R3; ++t) base[(R1 * R2 + R2 + 1) * t] = u[t];
         }
@@ -666,15 +688,16 @@ k_ring_synthesis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
         // ---- pass A^-1: conjugate twiddle W_N^{-n2 k1}, inverse R1-point transforms over k1 -> pixels n1 N / R1 + n2
         const int k = w.kfirst + kkp;
         double* mp = maps + ((size_t)(k0 + (k < kmaps ? k : 0)) * d.ncomp + w.comp) * d.npix;
-        for (int j = tm; j < N / R1; j += TPM) {
+#pragma unroll
+        for (int i = 0; i < NIA; ++i) {
+            const int j = tm + i * TPM;
+            if (j >= N / R1) break;
             const int B = (j >> G::LR3) + R2 * (j & (R3 - 1));
             const double2* src = trk + R1 * B + B + (j & (R3 - 1));
             double2 u[R1];
 #pragma unroll
             for (int q = 0; q < R1; ++q) u[q] = src[q];
-            double2 wv = __ldg(tw2 + 2 * j);
-            wv.y = -wv.y;
-            mul_powers<R1>(u, wv);
+            mul_powers<R1>(u, twA[i]);
             dft<R1, true>(u);
             if (k < kmaps) {
 #pragma unroll
@@ -711,44 +734,73 @@ struct GeoT {
 
 // forward passes B and the fused [C, filter, C^-1] pass, inverse pass B^-1 of one map's buffer; `tm`, `TPM`: thread
 // inside the map / threads per map; twL[e] = W_L^e; hf: filter spectrum in natural order (CONJ: conjugated)
+// per-thread twiddles of a chirp-z launch (the convolution length is the same for every ring of the launch):
+// W_L^j of the butterflies the thread owns in pass A / A^-1, W_L^{R1 n2'} (pass B) and W_L^{R1 k1'} (fused pass)
+template <class G, int TPM>
+struct CzTw {
+    static constexpr int NIA = (G::L / G::R1 + TPM - 1) / TPM, NIB = (G::L / G::R2 + TPM - 1) / TPM,
+                         NIC = (G::L / G::R3 + TPM - 1) / TPM;
+    double2 a[NIA], b[NIB], c[NIC];
+    __device__ __forceinline__ void load(const double2* __restrict__ twL, int tm)
+    {
+#pragma unroll
+        for (int i = 0; i < NIA; ++i) { const int j = tm + i * TPM; a[i] = __ldg(twL + (j < G::L / G::R1 ? j : 0)); }
+#pragma unroll
+        for (int i = 0; i < NIB; ++i) { const int w = tm + i * TPM; b[i] = __ldg(twL + (w < G::L / G::R2 ? G::R1 * (w >> G::LR1) : 0)); }
+#pragma unroll
+        for (int i = 0; i < NIC; ++i) { const int w = tm + i * TPM; c[i] = __ldg(twL + (w < G::L / G::R3 ? G::R1 * (w >> G::LR1) : 0)); }
+    }
+};
+
+// forward pass B, the fused [C, filter, C^-1] pass and the inverse pass B^-1 on one map's buffer; `tm`: thread inside
+// the map; hf: filter spectrum in natural order (CONJ: conjugated)
 template <class G, int TPM, bool CONJ>
-__device__ __forceinline__ void cz_middle(double2* trk, int tm, const double2* __restrict__ twL, const double2* __restrict__ hf)
+__device__ __forceinline__ void cz_middle(double2* trk, int tm, const CzTw<G, TPM>& tw, const double2* __restrict__ hf)
 {
     constexpr int R1 = G::R1, R2 = G::R2, R3 = G::R3, L = G::L;
-    for (int wq = tm; wq < L / R2; wq += TPM) {
+    using T = CzTw<G, TPM>;
+#pragma unroll
+    for (int i = 0; i < T::NIB; ++i) {
+        const int wq = tm + i * TPM;
+        if (wq >= L / R2) break;
         const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
         double2* base = trk + k1 + G::S3 * n2p;
         double2 u[R2];
 #pragma unroll
         for (int t = 0; t < R2; ++t) u[t] = base[G::S2 * t];
         dft<R2, false>(u);
-        mul_powers<R2>(u, __ldg(twL + R1 * n2p));
+        mul_powers<R2>(u, tw.b[i]);
 #pragma unroll
         for (int t = 0; t < R2; ++t) base[G::S2 * t] = u[t];
     }
     __syncthreads();
-    for (int wq = tm; wq < L / R3; wq += TPM) {
+#pragma unroll
+    for (int i = 0; i < T::NIC; ++i) {
+        const int wq = tm + i * TPM;
+        if (wq >= L / R3) break;
         const int k1 = wq & (R1 - 1), k1p = wq >> G::LR1;
         double2* base = trk + k1 + G::S2 * k1p;
         double2 u[R3];
 #pragma unroll
         for (int t = 0; t < R3; ++t) u[t] = base[G::S3 * t];
         dft<R3, false>(u);
+        const double2* __restrict__ hb = hf + k1 + R1 * k1p;             // spectrum bin k1 + R1 k1' + R1 R2 t
 #pragma unroll
-        for (int t = 0; t < R3; ++t) {                    // spectrum bin k1 + R1 k1' + R1 R2 t
-            double2 h = __ldg(hf + k1 + R1 * k1p + R1 * R2 * t);
+        for (int t = 0; t < R3; ++t) {
+            double2 h = __ldg(hb + R1 * R2 * t);
             if (CONJ) h.y = -h.y;
             u[t] = cmul(u[t], h);
         }
         dft<R3, true>(u);
-        double2 wv = __ldg(twL + R1 * k1p);
-        wv.y = -wv.y;
-        mul_powers<R3>(u, wv);
+        mul_powers<R3>(u, make_double2(tw.c[i].x, -tw.c[i].y));
 #pragma unroll
         for (int t = 0; t < R3; ++t) base[G::S3 * t] = u[t];
     }
     __syncthreads();
-    for (int wq = tm; wq < L / R2; wq += TPM) {
+#pragma unroll
+    for (int i = 0; i < T::NIB; ++i) {
+        const int wq = tm + i * TPM;
+        if (wq >= L / R2) break;
         const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
         double2* base = trk + k1 + G::S3 * n2p;
         double2 u[R2];
@@ -764,22 +816,26 @@ __device__ __forceinline__ void cz_middle(double2* trk, int tm, const double2* _
 }  // namespace p2
 
 // analysis of the cap ring pairs listed in `ring_list` (all with chirp-z length G::L)
-// shared memory: [KT transform buffers of LPAD][KT row / bin buffers of NB][2 output slots][mbarrier]
-template <class G, int KT>
-__global__ void __launch_bounds__(p2::NT, 1)
+// shared memory: [KT transform buffers of LPAD][KT row / bin buffers of NB][mbarrier]; the transform buffers are idle
+// during the FFT mapping (the bins sit in the row buffers by then) and serve as the output staging of the TMA stores
+template <class G, int KT, int NTH>
+__global__ void __launch_bounds__(NTH, 1)
 k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const int* __restrict__ ring_list, int nrings,
                    const double* __restrict__ maps, int k0, int kmaps, const double2* __restrict__ twL, int planes)
 {
     using namespace p2;
     constexpr int R1 = G::R1, R2 = G::R2, R3 = G::R3, L = G::L;
-    constexpr int TPM = NT / KT, MB = NT / KT;
+    constexpr int TPM = NTH / KT, MB = NTH / KT;
     constexpr int NB = L / 2 + 8;                         // double2 per map of the row / bin buffer (N <= L / 2 + 1)
     constexpr int SLOT = MB * 2 * KT;
+    constexpr int NSLOTS = (KT * G::LPAD) / SLOT >= 8 ? 8 : (KT * G::LPAD) / SLOT;
+    constexpr int U = NSLOTS >= 6 ? 3 : NSLOTS >= 4 ? 2 : 1;      // boxes per round; two rounds never share a slot
+    static_assert(NSLOTS >= 2 && 2 * U <= NSLOTS && MB <= 256, "output staging");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2* tr = reinterpret_cast<double2*>(smem_raw);
     double2* rb = tr + KT * G::LPAD;
-    double2* ostage = rb + KT * NB;
-    uint64_t* full = reinterpret_cast<uint64_t*>(ostage + 2 * SLOT);
+    double2* const ostage = tr;
+    uint64_t* full = reinterpret_cast<uint64_t*>(rb + KT * NB);
 
     const int tid = threadIdx.x;
     const int nkp = (kmaps + KT - 1) / KT;
@@ -818,6 +874,8 @@ k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
 
     const int kkp = tid / TPM, tm = tid - kkp * TPM;
     const int kkm = tid & (KT - 1), mi = tid / KT;
+    CzTw<G, TPM> tw;
+    tw.load(twL, tm);
     int li = 0, nstore = 0;
     for (long long it = blockIdx.x; it < nitems; it += gridDim.x, ++li) {
         int p, comp, kfirst;
@@ -827,12 +885,21 @@ k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
         const double2* __restrict__ hf = d.tw + rp.cz_off;          // [L] filter spectrum, then [N] chirp
         const double2* __restrict__ chirp = hf + L;
         const double2* __restrict__ tw2 = d.tw + rp.tw_off;          // W_{2N}^j (phase of the FFT mapping)
+        // phase recurrence of the FFT mapping: d sigma W_{2N}^{mi}, step W_{2N}^{MB} (fetched now, used after the passes)
+        double2 phc = __ldg(tw2 + mi % (2 * N));
+        phc.x *= dsig; phc.y *= dsig;
+        const double2 pstep = __ldg(tw2 + MB % (2 * N));
         mbar_wait(full, li & 1);
+        if (tid == 0) bulk_wait_read<0>();                // the stores of the previous item have read the transform buffers
+        __syncthreads();
         double2* trk = tr + kkp * G::LPAD;
         // ---- pass A: a_n = x_n c_n (zero past N), R1-point transforms over n1 (stride L / R1), twiddle W_L^{n2 k1}
         {
             const double* rows = reinterpret_cast<const double*>(rb + kkp * NB);
-            for (int j = tm; j < L / R1; j += TPM) {
+#pragma unroll
+            for (int i = 0; i < CzTw<G, TPM>::NIA; ++i) {
+                const int j = tm + i * TPM;
+                if (j >= L / R1) break;
                 double2 u[R1];
 #pragma unroll
                 for (int r = 0; r < R1; ++r) {
@@ -841,7 +908,7 @@ k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
                     if (n < N) u[r] = cmul(make_double2(rows[n], rows[N + n]), __ldg(chirp + n));
                 }
                 dft<R1, false>(u);
-                mul_powers<R1>(u, __ldg(twL + j));
+                mul_powers<R1>(u, tw.a[i]);
                 const int n1p = j / R3, n2p = j - n1p * R3;
                 const int B = n1p + R2 * n2p;
                 double2* dst = trk + R1 * B + B + n2p;
@@ -850,20 +917,21 @@ k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
             }
         }
         __syncthreads();
-        cz_middle<G, TPM, false>(trk, tm, twL, hf);
+        cz_middle<G, TPM, false>(trk, tm, tw, hf);
         // ---- pass A^-1: y_n, n = n1 L / R1 + n2; bins X_n = y_n c_n for n < N go to the row buffer (the rows are consumed)
         {
             double2* bins = rb + kkp * NB;
-            for (int j = tm; j < L / R1; j += TPM) {
+#pragma unroll
+            for (int i = 0; i < CzTw<G, TPM>::NIA; ++i) {
+                const int j = tm + i * TPM;
+                if (j >= L / R1) break;
                 const int n1p = j / R3, n2p = j - n1p * R3;
                 const int B = n1p + R2 * n2p;
                 const double2* src = trk + R1 * B + B + n2p;
                 double2 u[R1];
 #pragma unroll
                 for (int q = 0; q < R1; ++q) u[q] = src[q];
-                double2 wv = __ldg(twL + j);
-                wv.y = -wv.y;
-                mul_powers<R1>(u, wv);
+                mul_powers<R1>(u, make_double2(tw.a[i].x, -tw.a[i].y));
                 dft<R1, true>(u);
 #pragma unroll
                 for (int r = 0; r < R1; ++r) {
@@ -877,32 +945,38 @@ k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
         const int mlim = rp.mlim;
         const double2* bm = rb + kkm * NB;
         const int kg = kfirst / KG, csel = (kfirst % KG) / KT;
-        for (int m0 = 0; m0 < mlim; m0 += MB, ++nstore) {
-            const int m = m0 + mi;
-            int b = m < N ? m : m % N;
-            const int bc = b == 0 ? 0 : N - b;
-            const double2 A = bm[b], Bv = bm[bc];
-            const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
-            const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
-            double2 ph = make_double2(dsig, 0.0);
-            if (rp.shift) {
-                const int m2 = m < 2 * N ? m : m % (2 * N);
-                ph = __ldg(tw2 + m2);
-                ph.x *= dsig; ph.y *= dsig;
+        for (int m0 = 0; m0 < mlim; m0 += U * MB) {
+#pragma unroll
+            for (int q = 0; q < U; ++q) {
+                const int m = m0 + q * MB + mi;
+                const int b = m < N ? m : m % N;
+                const int bc = b == 0 ? 0 : N - b;
+                const double2 A = bm[b], Bv = bm[bc];
+                const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
+                const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
+                const double2 ph = phc;                   // cap rings are all shifted: phi0 = pi / N
+                phc = cmul(phc, pstep);
+                double2 E = cmul(ph, cadd(gn, gs)), O = cmul(ph, csub(gn, gs));
+                if (comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }
+                double2* slot = ostage + ((nstore + q) % NSLOTS) * SLOT;
+                slot[(mi * out_ms) * KT + kkm] = E;
+                slot[(out_hs + mi * out_ms) * KT + kkm] = O;
             }
-            double2 E = cmul(ph, cadd(gn, gs)), O = cmul(ph, csub(gn, gs));
-            if (comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }
-            double2* slot = ostage + (nstore & 1) * SLOT;
-            slot[(mi * out_ms) * KT + kkm] = E;
-            slot[(out_hs + mi * out_ms) * KT + kkm] = O;
             fence_async_smem();
             if (tid == 0) bulk_wait_read<0>();
             __syncthreads();
             if (tid == 0) {
-                if (planes) tma_store_5d(&tmF, slot, 0, m0, 2 * comp, csel, p * d.nkg + kg);
-                else tma_store_5d(&tmF, slot, 0, csel, 2 * comp, m0, p * d.nkg + kg);
+#pragma unroll
+                for (int q = 0; q < U; ++q) {
+                    const int mq = m0 + q * MB;
+                    if (mq >= mlim) break;
+                    const double2* slot = ostage + ((nstore + q) % NSLOTS) * SLOT;
+                    if (planes) tma_store_5d(&tmF, slot, 0, mq, 2 * comp, csel, p * d.nkg + kg);
+                    else tma_store_5d(&tmF, slot, 0, csel, 2 * comp, mq, p * d.nkg + kg);
+                }
                 bulk_commit();
             }
+            nstore += U;
         }
         if (tid == 0 && it + gridDim.x < nitems) issue_loads(it + gridDim.x);
     }
@@ -911,22 +985,23 @@ k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
 
 // synthesis of the cap ring pairs listed in `ring_list` by the chirp-z transform:
 //   x_n = conj(c_n) sum_b (Z_b conj(c_b)) c_{n-b}: the same convolution with the conjugated chirp and filter spectrum.
-// shared memory: [KT transform buffers of LPAD][KT bin buffers of NB][NSL input slots][mbarriers]
-template <class G, int KT, int NSL>
-__global__ void __launch_bounds__(p2::NT, 1)
+// shared memory: [NSL input slots][KT transform buffers of LPAD][mbarriers].  The ring spectrum is accumulated in the
+// transform buffers themselves (natural order, first N elements); every thread owns at most one pass-A butterfly, reads
+// its inputs into registers, and the pass writes the buffers in place after a barrier.
+template <class G, int KT, int NSL, int NTH>
+__global__ void __launch_bounds__(NTH, 1)
 k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const int* __restrict__ ring_list, int nrings,
                     double* __restrict__ maps, int k0, int kmaps, const double2* __restrict__ twL, int planes)
 {
     using namespace p2;
     constexpr int R1 = G::R1, R2 = G::R2, R3 = G::R3, L = G::L;
-    constexpr int TPM = NT / KT, MB = NT / KT;
-    constexpr int NB = L / 2 + 8;
+    constexpr int TPM = NTH / KT, MB = NTH / KT;
     constexpr int SLOT = MB * 2 * KT;
+    static_assert(L / R1 <= TPM && MB <= 256, "one pass-A butterfly per thread");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2* in_slots = reinterpret_cast<double2*>(smem_raw);
     double2* tr = in_slots + NSL * SLOT;
-    double2* zb = tr + KT * G::LPAD;
-    uint64_t* full = reinterpret_cast<uint64_t*>(zb + KT * NB);
+    uint64_t* full = reinterpret_cast<uint64_t*>(tr + KT * G::LPAD);
 
     const int tid = threadIdx.x;
     const int nkp = (kmaps + KT - 1) / KT;
@@ -968,6 +1043,8 @@ k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
 
     const int kkp = tid / TPM, tm = tid - kkp * TPM;
     const int kkm = tid & (KT - 1), mi = tid / KT;
+    CzTw<G, TPM> tw;
+    tw.load(twL, tm);
     int cslot = 0; uint32_t cphase = 0;
     for (long long it = blockIdx.x; it < nitems; it += gridDim.x) {
         int p, comp, kfirst;
@@ -977,11 +1054,15 @@ k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
         const double2* __restrict__ hf = d.tw + rp.cz_off;
         const double2* __restrict__ chirp = hf + L;
         const double2* __restrict__ tw2 = d.tw + rp.tw_off;
-        for (int i = tid; i < KT * NB; i += NT) zb[i] = make_double2(0.0, 0.0);
+        double2 phc = __ldg(tw2 + mi % (2 * N));          // e^{+i m phi0} by recurrence, step W_{2N}^{-MB}
+        phc.y = -phc.y;
+        double2 pstep = __ldg(tw2 + MB % (2 * N));
+        pstep.y = -pstep.y;
+        for (int i = tid; i < KT * N; i += NTH) { const int kz = i / N; tr[kz * G::LPAD + (i - kz * N)] = make_double2(0.0, 0.0); }
         __syncthreads();
         // ---- inverse FFT mapping: accumulate the ring spectrum Z_b, b < N (as in the belt kernel)
         const int mlim = rp.mlim;
-        double2* zm = zb + kkm * NB;
+        double2* zm = tr + kkm * G::LPAD;
         for (int m0 = 0; m0 < mlim; m0 += MB) {
             mbar_wait(full + cslot, cphase);
             const double2* slot = in_slots + cslot * SLOT;
@@ -992,14 +1073,14 @@ k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
                 const double2 e = slot[(mi * in_ms) * KT + kkm], o = slot[(in_hs + mi * in_ms) * KT + kkm];
                 double2 fn = cadd(e, o), fs = csub(e, o);
                 if (comp == 1) { fn = make_double2(fn.y, -fn.x); fs = make_double2(fs.y, -fs.x); }
-                double2 ph = make_double2(1.0, 0.0);
-                if (rp.shift) { ph = __ldg(tw2 + (m < 2 * N ? m : m % (2 * N))); ph.y = -ph.y; }
+                double2 ph = phc;
                 const double wgt = (m == 0) ? 0.5 : 1.0;
                 ph.x *= wgt; ph.y *= wgt;
                 const double2 dn = cmul(ph, fn), ds = cmul(ph, fs);
                 zd = make_double2(dn.x - ds.y, dn.y + ds.x);
                 zc = make_double2(dn.x + ds.y, ds.x - dn.y);
             }
+            phc = cmul(phc, pstep);
             const int b1 = m < N ? m : m % N, b2 = b1 == 0 ? 0 : N - b1;
             // two orders of one chunk meet in a bin only if m + m' = 0 mod N for some pair of the chunk
             const bool clash = ((2 * m0 + N - 1) / N) * N <= 2 * m0 + 2 * MB - 2;
@@ -1011,19 +1092,23 @@ k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
             if (++cslot == NSL) { cslot = 0; cphase ^= 1; }
         }
         double2* trk = tr + kkp * G::LPAD;
-        // ---- pass A: a_b = Z_b conj(c_b) (zero past N)
+        // ---- pass A in place: a_b = Z_b conj(c_b) (zero past N) to registers, barrier, transform, write
         {
-            const double2* zk = zb + kkp * NB;
-            for (int j = tm; j < L / R1; j += TPM) {
-                double2 u[R1];
+            const int j = tm;
+            const bool act = j < L / R1;
+            double2 u[R1];
+            if (act) {
 #pragma unroll
                 for (int r = 0; r < R1; ++r) {
                     const int n = j + r * (L / R1);
                     u[r] = make_double2(0.0, 0.0);
-                    if (n < N) { double2 c = __ldg(chirp + n); c.y = -c.y; u[r] = cmul(zk[n], c); }
+                    if (n < N) { double2 c = __ldg(chirp + n); c.y = -c.y; u[r] = cmul(trk[n], c); }
                 }
+            }
+            __syncthreads();
+            if (act) {
                 dft<R1, false>(u);
-                mul_powers<R1>(u, __ldg(twL + j));
+                mul_powers<R1>(u, tw.a[0]);
                 const int n1p = j / R3, n2p = j - n1p * R3;
                 const int B = n1p + R2 * n2p;
                 double2* dst = trk + R1 * B + B + n2p;
@@ -1032,21 +1117,22 @@ k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
             }
         }
         __syncthreads();
-        cz_middle<G, TPM, true>(trk, tm, twL, hf);
+        cz_middle<G, TPM, true>(trk, tm, tw, hf);
         // ---- pass A^-1: pixels x_n = y_n conj(c_n), north = real part, south = imaginary part
         {
             const int k = kfirst + kkp;
             double* mp = maps + ((size_t)(k0 + (k < kmaps ? k : 0)) * d.ncomp + comp) * d.npix;
-            for (int j = tm; j < L / R1; j += TPM) {
+#pragma unroll
+            for (int i = 0; i < CzTw<G, TPM>::NIA; ++i) {
+                const int j = tm + i * TPM;
+                if (j >= L / R1) break;
                 const int n1p = j / R3, n2p = j - n1p * R3;
                 const int B = n1p + R2 * n2p;
                 const double2* src = trk + R1 * B + B + n2p;
                 double2 u[R1];
 #pragma unroll
                 for (int q = 0; q < R1; ++q) u[q] = src[q];
-                double2 wv = __ldg(twL + j);
-                wv.y = -wv.y;
-                mul_powers<R1>(u, wv);
+                mul_powers<R1>(u, make_double2(tw.a[i].x, -tw.a[i].y));
                 dft<R1, true>(u);
                 if (k < kmaps) {
 #pragma unroll
@@ -1067,37 +1153,6 @@ k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
 }
 
 // ---- host side -------------------------------------------------------------------------------------------
-// Workspace F as a 5-D tensor for the ring kernels' boxes of [MB orders] x [E, O] x [KT maps]: innermost the 2 KT
-// doubles of KT maps (re, im); c = which KT-map part of the 4-map line; ch = 2 comp + h; m; (p, kg).
-// planes: dimension order (doubles, m, ch, c, pkg) -> box lands as [h][m][map] (conflict-free staging); otherwise
-// ascending strides (doubles, c, ch, m, pkg) -> [m][h][map].
-static cudaError_t make_tmap_ring(const DevicePlan& d, const double* F, int kt, int mb, bool planes, CUtensorMap* tm)
-{
-    PFN_tmapEncodeTiled enc = tmap_encoder();
-    if (!enc) return cudaErrorNotSupported;
-    const cuuint64_t line = 128, mstr = (cuuint64_t)d.ncomp * line, pstr = (cuuint64_t)(d.lmax + 1) * mstr;
-    const cuuint64_t n_m = (cuuint64_t)d.lmax + 1, n_ch = 2 * (cuuint64_t)d.ncomp, n_c = (cuuint64_t)(KG / kt),
-                     n_pkg = (cuuint64_t)d.nh * d.nkg;
-    cuuint64_t dims[5], strides[4];
-    cuuint32_t box[5];
-    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-    dims[0] = 2 * (cuuint64_t)kt; box[0] = 2 * (cuuint32_t)kt;
-    if (planes) {
-        dims[1] = n_m; strides[0] = mstr; box[1] = (cuuint32_t)mb;
-        dims[2] = n_ch; strides[1] = 64; box[2] = 2;
-        dims[3] = n_c; strides[2] = (cuuint64_t)kt * 16; box[3] = 1;
-    } else {
-        dims[1] = n_c; strides[0] = (cuuint64_t)kt * 16; box[1] = 1;
-        dims[2] = n_ch; strides[1] = 64; box[2] = 2;
-        dims[3] = n_m; strides[2] = mstr; box[3] = (cuuint32_t)mb;
-    }
-    dims[4] = n_pkg; strides[3] = pstr; box[4] = 1;
-    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<double*>(F), dims, strides, box, estr,
-                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
-}
-
 template <int LOGN, int KT>
 static size_t analysis_p2_smem()
 {
@@ -1172,9 +1227,9 @@ static cudaError_t run_synthesis_p2(sht_plan_s* pl, const DevicePlan& d, const d
 template <class G, int KT>
 static cudaError_t run_analysis_cz(sht_plan_s* pl, const DevicePlan& d, int cls, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
 {
-    constexpr int MB = p2::NT / KT;
-    const size_t sm = (size_t)KT * G::LPAD * 16 + (size_t)KT * (G::L / 2 + 8) * 16 + (size_t)2 * MB * 2 * KT * 16 + 64;
-    auto kern = k_ring_analysis_cz<G, KT>;
+    constexpr int NTH = 512, MB = NTH / KT;
+    const size_t sm = (size_t)KT * G::LPAD * 16 + (size_t)KT * (G::L / 2 + 8) * 16 + 64;
+    auto kern = k_ring_analysis_cz<G, KT, NTH>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tm;
@@ -1184,11 +1239,11 @@ static cudaError_t run_analysis_cz(sht_plan_s* pl, const DevicePlan& d, int cls,
         if ((e = make_tmap_ring(d, F, KT, MB, false, &tm)) != cudaSuccess) return e;
     }
     int occ = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, p2::NT, sm) != cudaSuccess || occ < 1) { cudaGetLastError(); occ = 1; }
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NTH, sm) != cudaSuccess || occ < 1) { cudaGetLastError(); occ = 1; }
     const long long nitems = (long long)pl->cz_count[cls] * d.ncomp * ((kmaps + KT - 1) / KT);
     const long long want = (long long)pl->sm_count * occ;
     const unsigned grid = (unsigned)(nitems < want ? nitems : want);
-    kern<<<grid, p2::NT, sm, st>>>(tm, d, pl->cz_rings[cls], pl->cz_count[cls], maps, k0, kmaps, d.tw + pl->cz_tw_off[cls], planes ? 1 : 0);
+    kern<<<grid, NTH, sm, st>>>(tm, d, pl->cz_rings[cls], pl->cz_count[cls], maps, k0, kmaps, d.tw + pl->cz_tw_off[cls], planes ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -1196,9 +1251,9 @@ static cudaError_t run_analysis_cz(sht_plan_s* pl, const DevicePlan& d, int cls,
 template <class G, int KT>
 static cudaError_t run_synthesis_cz(sht_plan_s* pl, const DevicePlan& d, int cls, const double* F, double* maps, int k0, int kmaps, cudaStream_t st)
 {
-    constexpr int MB = p2::NT / KT, NSL = 2;
-    const size_t sm = (size_t)KT * G::LPAD * 16 + (size_t)KT * (G::L / 2 + 8) * 16 + (size_t)NSL * MB * 2 * KT * 16 + 64;
-    auto kern = k_ring_synthesis_cz<G, KT, NSL>;
+    constexpr int NTH = 512, MB = NTH / KT, NSL = 2;
+    const size_t sm = (size_t)KT * G::LPAD * 16 + (size_t)NSL * MB * 2 * KT * 16 + 64;
+    auto kern = k_ring_synthesis_cz<G, KT, NSL, NTH>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tm;
@@ -1208,11 +1263,11 @@ static cudaError_t run_synthesis_cz(sht_plan_s* pl, const DevicePlan& d, int cls
         if ((e = make_tmap_ring(d, F, KT, MB, false, &tm)) != cudaSuccess) return e;
     }
     int occ = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, p2::NT, sm) != cudaSuccess || occ < 1) { cudaGetLastError(); occ = 1; }
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NTH, sm) != cudaSuccess || occ < 1) { cudaGetLastError(); occ = 1; }
     const long long nitems = (long long)pl->cz_count[cls] * d.ncomp * ((kmaps + KT - 1) / KT);
     const long long want = (long long)pl->sm_count * occ;
     const unsigned grid = (unsigned)(nitems < want ? nitems : want);
-    kern<<<grid, p2::NT, sm, st>>>(tm, d, pl->cz_rings[cls], pl->cz_count[cls], maps, k0, kmaps, d.tw + pl->cz_tw_off[cls], planes ? 1 : 0);
+    kern<<<grid, NTH, sm, st>>>(tm, d, pl->cz_rings[cls], pl->cz_count[cls], maps, k0, kmaps, d.tw + pl->cz_tw_off[cls], planes ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
 }
