@@ -277,6 +277,10 @@ def main():
                          "Alg. 3, the immediate iteration (one order m at a time, spin 0)")
     ap.add_argument("--lambda-mode", default="", choices=["", "fused", "staged"],
                     help="where the P_lm tiles are generated (include/sht.h); default: the plan's own choice")
+    ap.add_argument("--ring-path", default="", choices=["", "fast", "general"],
+                    help="SHT_OPT_RING_PATH: belt / mixed-radix / chirp-z ring kernels (fast, the default) or the general ones only")
+    ap.add_argument("--leg-tiles", type=int, default=-1, help="SHT_OPT_LEG_TILES_PER_CTA (default: the plan's)")
+    ap.add_argument("--leg-split", type=int, default=-1, help="SHT_OPT_LEG_RING_SPLIT (default: the plan's)")
     ap.add_argument("--compare", default="", choices=["", "cublas"],
                     help="cublas: also time the paper's per-m cuBLAS DGEMM formulation of the Legendre stage (comparison only)")
     ap.add_argument("--no-e2e", action="store_true")
@@ -322,6 +326,14 @@ def main():
     if args.lambda_mode:
         plan.sht_plan_set_lambda_mode(1 if args.lambda_mode == "staged" else 0)
     lambda_mode = "staged" if plan.sht_plan_lambda_mode() == 1 else "fused"
+    if args.ring_path:
+        plan.sht_plan_set_option(0, 1 if args.ring_path == "fast" else 0)
+    if args.leg_tiles >= 0:
+        plan.sht_plan_set_option(1, args.leg_tiles)
+    if args.leg_split >= 0:
+        plan.sht_plan_set_option(2, args.leg_split)
+    options = {"ring_path": "fast" if plan.sht_plan_get_option(0) else "general",
+               "leg_tiles_per_cta": plan.sht_plan_get_option(1), "leg_ring_split": plan.sht_plan_get_option(2)}
     stream = torch.cuda.current_stream()
 
     if args.pol:
@@ -487,7 +499,7 @@ def main():
                 "config": {**base_config(c),
                            "l2": "inputs (%.1f GB maps, %.1f GB a_lm per GPU) are far larger than the 126 MB L2"
                                  % (8e-9 * npix * nmaps * ncomp, 16e-9 * nalm * nmaps * ncomp),
-                           "plan_create_s": plan_s, "chunk_maps": plan.chunk_maps(), "lambda_mode": lambda_mode,
+                           "plan_create_s": plan_s, "chunk_maps": plan.chunk_maps(), "lambda_mode": lambda_mode, "options": options,
                            "workspace_GB": plan.workspace_bytes() * 1e-9},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "stages": stages, "cpu_baseline": cpu}

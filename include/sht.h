@@ -74,6 +74,19 @@ enum { SHT_LAMBDA_FUSED = 0, SHT_LAMBDA_STAGED = 1 };
 sht_status_t sht_plan_set_lambda_mode(sht_plan_t plan, int mode);
 int sht_plan_lambda_mode(sht_plan_t plan);
 
+/* Launch-shape options (measurement and comparison; every setting computes the same transforms, equal up to the order
+ * of floating-point sums):
+ *   SHT_OPT_RING_PATH         1 (default): the belt rings of a power-of-two nside, and the cap rings of 132 .. 2048 pixels,
+ *                             go through the bulk-copy / TMA kernels (compiled power-of-two transforms, three-radix
+ *                             mixed-radix transforms, chirp-z); 0: the general ring kernels do every ring
+ *   SHT_OPT_LEG_TILES_PER_CTA spin-0 Legendre analysis: 0 = one CTA per (m, k-tile) walks all l tiles; n > 0 = one CTA per
+ *                             (m, group of n l tiles, k-tile), so that the tiles of an order share T_m through L2 (default 2)
+ *   SHT_OPT_LEG_RING_SPLIT    spin-0 Legendre synthesis: CTAs that share the ring blocks of an (m, k-tile) (default 3)
+ * SHT_ERR_INVALID_ARG for an unknown option or a negative value. */
+enum { SHT_OPT_RING_PATH = 0, SHT_OPT_LEG_TILES_PER_CTA = 1, SHT_OPT_LEG_RING_SPLIT = 2 };
+sht_status_t sht_plan_set_option(sht_plan_t plan, int option, int value);
+int sht_plan_get_option(sht_plan_t plan, int option);    /* -1: unknown option */
+
 /* Alg. 1: maps (device, in) -> alm (device, out). */
 sht_status_t sht_analysis(sht_plan_t plan, const double* maps, double* alm, void* stream);
 /* eq. 4-5: alm (device, in) -> maps (device, out). */

@@ -640,6 +640,28 @@ extern "C" sht_status_t sht_plan_set_lambda_mode(sht_plan_t pl, int mode)
 }
 extern "C" int sht_plan_lambda_mode(sht_plan_t pl) { return pl ? pl->lam_mode : -1; }
 
+extern "C" sht_status_t sht_plan_set_option(sht_plan_t pl, int option, int value)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (value < 0) return SHT_ERR_INVALID_ARG;
+    switch (option) {
+        case SHT_OPT_RING_PATH: pl->fast_ring = value != 0; return SHT_OK;
+        case SHT_OPT_LEG_TILES_PER_CTA: pl->leg_tsplit = value; return SHT_OK;
+        case SHT_OPT_LEG_RING_SPLIT: pl->leg_nsplit = value < 1 ? 1 : value; return SHT_OK;
+        default: return SHT_ERR_INVALID_ARG;
+    }
+}
+extern "C" int sht_plan_get_option(sht_plan_t pl, int option)
+{
+    if (!pl) return -1;
+    switch (option) {
+        case SHT_OPT_RING_PATH: return pl->fast_ring ? 1 : 0;
+        case SHT_OPT_LEG_TILES_PER_CTA: return pl->leg_tsplit;
+        case SHT_OPT_LEG_RING_SPLIT: return pl->leg_nsplit;
+        default: return -1;
+    }
+}
+
 // ---- introspection -----------------------------------------------------------------------------------
 extern "C" long long sht_npix(int nside) { return 12LL * nside * nside; }
 extern "C" long long sht_nalm(int lmax) { return (long long)(lmax + 1) * (lmax + 2) / 2; }

@@ -19,6 +19,8 @@ constexpr int RING_THREADS = 256;            // threads per CTA of the ring kern
 constexpr int RING_EMAX = 8192;              // most complex elements (ring length x maps) one ring CTA holds in smem
 constexpr int BLUESTEIN_MIN_PRIME = 37;      // smallest prime factor of a ring length that switches to Bluestein
 constexpr int RING_NCLASS = 4;               // launch classes of the ring kernels (by dynamic smem size)
+// default grid shapes of the spin-0 Legendre kernels (SHT_OPT_LEG_TILES_PER_CTA, SHT_OPT_LEG_RING_SPLIT)
+constexpr int LEG_TSPLIT_DEFAULT = 2, LEG_NSPLIT_DEFAULT = 3;
 
 // One folded ring pair p = 0 .. nh-1: north ring i = p+1 and its mirror 4 nside - i (PAPER.md:211 grid;
 // north_star: "ring pairs symmetric about the equator folded").  The equator (p = nh-1) has no partner.
@@ -114,9 +116,9 @@ struct sht_plan_s {
     size_t class_smem[sht::RING_NCLASS];
     // belt fast path (sht_ring_pow2.cu): ring pairs belt_first .. belt_first + belt_count - 1 have length 2^belt_logn
     // (belt_logn = 0: none); class_*_nb are the launch classes of the general kernels without those pairs
-    int belt_logn, belt_first, belt_count, p2_syn_occ, p2_variant;
+    int belt_logn, belt_first, belt_count;
     int leg_tsplit, leg_nsplit;     // grid shapes of the spin-0 Legendre kernels (sht_legendre.cu launchers)
-    bool fast_ring;                 // the kernels of sht_ring_pow2.cu are in use (experiment switch; default on)
+    bool fast_ring;                 // SHT_OPT_RING_PATH: the belt / mixed-radix / chirp-z ring kernels are in use
     int* class_rings_nb[sht::RING_NCLASS];
     int class_count_nb[sht::RING_NCLASS];
     int class_ktmin_nb[sht::RING_NCLASS];

@@ -714,13 +714,8 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             pl->class_rings[c] = const_cast<int*>(dp);
         }
         // belt fast path: nside a power of two with a ring length the compiled transforms cover
-        pl->belt_logn = 0; pl->belt_first = nside - 1; pl->belt_count = nside + 1; pl->p2_syn_occ = 2; pl->p2_variant = 1; pl->fast_ring = true;
-        if (const char* ev = getenv("SHT_FAST_RING")) pl->fast_ring = atoi(ev) != 0;
-        pl->leg_tsplit = 0; pl->leg_nsplit = 1;
-        if (const char* ev = getenv("SHT_LEG_TSPLIT")) pl->leg_tsplit = atoi(ev);
-        if (const char* ev = getenv("SHT_LEG_NSPLIT")) pl->leg_nsplit = atoi(ev);
-        if (const char* ev = getenv("SHT_P2_VARIANT")) pl->p2_variant = atoi(ev);      // experiment switch
-        if (const char* ev = getenv("SHT_P2_SYN_OCC")) pl->p2_syn_occ = atoi(ev);
+        pl->belt_logn = 0; pl->belt_first = nside - 1; pl->belt_count = nside + 1; pl->fast_ring = true;
+        pl->leg_tsplit = LEG_TSPLIT_DEFAULT; pl->leg_nsplit = LEG_NSPLIT_DEFAULT;      // sht_plan_set_option changes them
         if ((nside & (nside - 1)) == 0 && 4 * nside >= 512 && 4 * nside <= 2048) {
             int a = 0;
             while ((1 << a) < 4 * nside) ++a;

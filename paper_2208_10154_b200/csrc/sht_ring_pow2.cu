@@ -191,197 +191,11 @@ __device__ __forceinline__ Item decode_item(long long it, int nkp, int ncomp, in
 }  // namespace p2
 
 // ------------------------------------------------------------------------------------------------
-// analysis: maps -> F for the belt ring pairs p_first .. p_first + npairs - 1 (all of length N = 2^LOGN)
-// shared memory: [2 input buffers: KT maps x (north row, south row) of N doubles][KT transform buffers][2 output slots]
-// ------------------------------------------------------------------------------------------------
-template <int LOGN, int KT>
-__global__ void __launch_bounds__(p2::NT, 1)
-k_ring_analysis_p2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const double* __restrict__ maps, int k0, int kmaps,
-                   int p_first, int npairs, int planes)
-{
-    using namespace p2;
-    using G = Geo<LOGN>;
-    constexpr int N = G::N, R1 = G::R1, R2 = G::R2, R3 = G::R3;
-    constexpr int TPM = NT / KT;                          // threads per map in the passes
-    constexpr int MB = NT / KT;                           // orders m per mapping sweep (one TMA store box)
-    constexpr int BS = buf_stride<LOGN, KT>();
-    constexpr int IN_DOUBLES = KT * 2 * N;                // one input buffer
-    constexpr int SLOT = MB * 2 * KT;                     // double2 per TMA box
-    constexpr int NSLOTS = (KT * N) / SLOT;               // boxes an input buffer holds when it serves as output staging
-    constexpr int U = NSLOTS >= 6 ? 3 : NSLOTS / 2;       // boxes per round (two rounds never share a slot)
-    static_assert(U >= 1 && 2 * U <= NSLOTS, "output staging");
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    double* in_buf = reinterpret_cast<double*>(smem_raw);
-    double2* tr = reinterpret_cast<double2*>(smem_raw + (size_t)2 * IN_DOUBLES * 8);
-    uint64_t* full = reinterpret_cast<uint64_t*>(tr + KT * BS);
-
-    const int tid = threadIdx.x;
-    const int nkp = (kmaps + KT - 1) / KT;
-    const long long nitems = (long long)npairs * d.ncomp * nkp;
-    // layout of an output slot = layout of the TMA box: [h][m][map] (planes) or [m][h][map]
-    const int out_hs = planes ? MB : 1, out_ms = planes ? 1 : 2;
-    const double dsig = 4.0 * 3.14159265358979323846 / (double)d.npix;
-
-    if (tid == 0) {
-        mbar_init(full + 0, 1); mbar_init(full + 1, 1);
-        fence_barrier_init();
-        tma_prefetch_desc(&tmF);
-    }
-    __syncthreads();
-
-    // the rows of one item: KT maps x (north, south); a map past kmaps is replaced by the last valid one (its workspace
-    // column is padding: it only has to stay finite)
-    auto issue_loads = [&](long long it, int buf) {
-        const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
-        const RingPair& rp = d.rings[w.p];
-        const bool eq = rp.start_s < 0;
-        mbar_arrive_expect_tx(full + buf, (uint32_t)(KT * (eq ? 1 : 2) * N * 8));
-#pragma unroll
-        for (int kk = 0; kk < KT; ++kk) {
-            const int k = min(w.kfirst + kk, kmaps - 1);
-            const double* mp = maps + ((size_t)(k0 + k) * d.ncomp + w.comp) * d.npix;
-            double* dst = in_buf + (size_t)buf * IN_DOUBLES + kk * 2 * N;
-            bulk_load(dst, mp + rp.start_n, N * 8, full + buf);
-            if (!eq) bulk_load(dst + N, mp + rp.start_s, N * 8, full + buf);
-        }
-    };
-    if (tid == 0) {
-        if ((long long)blockIdx.x < nitems) issue_loads(blockIdx.x, 0);
-        if ((long long)blockIdx.x + gridDim.x < nitems) issue_loads((long long)blockIdx.x + gridDim.x, 1);
-    }
-
-    const int kkp = tid / TPM, tm = tid - kkp * TPM;      // passes: map and thread inside the map
-    const int kkm = tid & (KT - 1), mi = tid / KT;        // mapping: map (fastest) and order inside the sweep
-    // per-thread constants of the whole launch (every belt ring has the same length): pass twiddles W_N^j, W_N^{R1 n2'},
-    // and the phase recurrence of the FFT mapping, W_{2N}^{mi} d sigma and W_{2N}^{MB}
-    constexpr int NIA = (N / R1 + TPM - 1) / TPM, NIB = (N / R2 + TPM - 1) / TPM;
-    const double2* __restrict__ twc = d.tw + d.rings[p_first].tw_off;
-    double2 twA[NIA], twB[NIB];
-#pragma unroll
-    for (int i = 0; i < NIA; ++i) twA[i] = __ldg(twc + 2 * ((tm + i * TPM) & (N / R1 - 1)));
-#pragma unroll
-    for (int i = 0; i < NIB; ++i) twB[i] = __ldg(twc + 2 * R1 * (((tm + i * TPM) & (N / R2 - 1)) >> G::LR1));
-    double2 ph0 = __ldg(twc + (mi & (2 * N - 1)));
-    ph0.x *= dsig; ph0.y *= dsig;
-    const double2 phs = __ldg(twc + (MB & (2 * N - 1)));
-    int li = 0, nstore = 0;
-    for (long long it = blockIdx.x; it < nitems; it += gridDim.x, ++li) {
-        const Item w = decode_item(it, nkp, d.ncomp, p_first, KT);
-        const RingPair rp = d.rings[w.p];
-        const bool equator = rp.start_s < 0;
-        const int buf = li & 1;
-        mbar_wait(full + buf, (li >> 1) & 1);
-        const double* rows = in_buf + (size_t)buf * IN_DOUBLES + kkp * 2 * N;
-        double2* trk = tr + kkp * BS;
-
-        // ---- pass A: R1-point transforms over n1 (input stride N / R1), twiddle W_N^{n2 k1}, R1 consecutive positions
-#pragma unroll
-        for (int i = 0; i < NIA; ++i) {
-            const int j = tm + i * TPM;
-            if (j >= N / R1) break;
-            double2 u[R1];
-#pragma unroll
-            for (int r = 0; r < R1; ++r) {
-                u[r].x = rows[j + r * (N / R1)];
-                u[r].y = equator ? 0.0 : rows[N + j + r * (N / R1)];
-            }
-            dft<R1, false>(u);
-            mul_powers<R1>(u, twA[i]);
-            const int B = (j >> G::LR3) + R2 * (j & (R3 - 1));       // n1' + R2 n2'
-            double2* dst = trk + R1 * B + B + (j & (R3 - 1));        // phys(R1 B + k1) = R1 B + k1 + B + n2'
-#pragma unroll
-            for (int k = 0; k < R1; ++k) dst[k] = u[k];
-        }
-        __syncthreads();
-
-        // ---- pass B: R2-point transforms over n1' at positions k1 + R1 t + R1 R2 n2', twiddle W_{R2 R3}^{n2' k1'}
-#pragma unroll
-        for (int i = 0; i < NIB; ++i) {
-            const int wq = tm + i * TPM;
-            if (wq >= N / R2) break;
-            const int k1 = wq & (R1 - 1), n2p = wq >> G::LR1;
-            double2* base = trk + k1 + (R1 * R2 + R2 + 1) * n2p;
-            double2 u[R2];
-#pragma unroll
-            for (int t = 0; t < R2; ++t) u[t] = base[(R1 + 1) * t];
-            dft<R2, false>(u);
-            mul_powers<R2>(u, twB[i]);
-#pragma unroll
-            for (int t = 0; t < R2; ++t) base[(R1 + 1) * t] = u[t];
-        }
-        __syncthreads();
-        // ---- pass C: R3-point transforms over n2' at positions k1 + R1 k1' + R1 R2 t; bin k1 + R1 k1' + R1 R2 k2' in place
-        for (int wq = tm; wq < N / R3; wq += TPM) {
-            const int k1 = wq & (R1 - 1), k1p = wq >> G::LR1;
-            double2* base = trk + k1 + (R1 + 1) * k1p;
-            double2 u[R3];
-#pragma unroll
-            for (int t = 0; t < R3; ++t) u[t] = base[(R1 * R2 + R2 + 1) * t];
-            dft<R3, false>(u);
-#pragma unroll
-            for (int t = 0; t < R3; ++t) base[(R1 * R2 + R2 + 1) * t] = u[t];
-        }
-        __syncthreads();
-
-        // ---- FFT mapping: order m -> bin m mod N, phase, fold.  The lines are staged in the
-        // input buffer this item has just consumed (NSLOTS boxes of MB orders) and leave by TMA stores, U boxes per round;
-        // a round's slots are rewritten two rounds later, after thread 0 has seen its stores read them.
-        const int mlim = rp.mlim;
-        const double2* trm = tr + kkm * BS;
-        const int kg = w.kfirst / KG, csel = (w.kfirst % KG) / KT;
-        double2* const ostage = reinterpret_cast<double2*>(in_buf + (size_t)buf * IN_DOUBLES);
-        // phase of order m = m0 + q MB + mi by recurrence from the thread's own W_{2N}^{mi} (no table read per order)
-        double2 phc = rp.shift ? ph0 : make_double2(dsig, 0.0);
-        const double2 pstep = rp.shift ? phs : make_double2(1.0, 0.0);
-        for (int m0 = 0; m0 < mlim; m0 += U * MB) {
-#pragma unroll
-            for (int q = 0; q < U; ++q) {
-                const int m = m0 + q * MB + mi;
-                const int b = m & (N - 1), bc = (N - b) & (N - 1);
-                const double2 A = trm[G::phys(b)], Bv = trm[G::phys(bc)];
-                // G_north = (A + conj B) / 2, G_south = (A - conj B) / (2 i)
-                const double2 gn = make_double2(0.5 * (A.x + Bv.x), 0.5 * (A.y - Bv.y));
-                const double2 gs = make_double2(0.5 * (A.y + Bv.y), -0.5 * (A.x - Bv.x));
-                const double2 ph = phc;                   // d sigma e^{-i m phi0}, phi0 = pi / N on the shifted rings
-                phc = cmul(phc, pstep);
-                double2 E, O;
-                if (equator) { E = cmul(ph, gn); O = make_double2(0.0, 0.0); }
-                else { E = cmul(ph, cadd(gn, gs)); O = cmul(ph, csub(gn, gs)); }
-                if (w.comp == 1) { E = make_double2(-E.y, E.x); O = make_double2(-O.y, O.x); }      // i U
-                double2* slot = ostage + ((nstore + q) % NSLOTS) * SLOT;
-                slot[(mi * out_ms) * KT + kkm] = E;
-                slot[(out_hs + mi * out_ms) * KT + kkm] = O;
-            }
-            fence_async_smem();
-            if (tid == 0) bulk_wait_read<0>();            // the previous round's stores have read their slots
-            __syncthreads();
-            if (tid == 0) {
-#pragma unroll
-                for (int q = 0; q < U; ++q) {
-                    const int mq = m0 + q * MB;
-                    if (mq >= mlim) break;
-                    const double2* slot = ostage + ((nstore + q) % NSLOTS) * SLOT;
-                    if (planes) tma_store_5d(&tmF, slot, 0, mq, 2 * w.comp, csel, w.p * d.nkg + kg);
-                    else tma_store_5d(&tmF, slot, 0, csel, 2 * w.comp, mq, w.p * d.nkg + kg);
-                }
-                bulk_commit();
-            }
-            nstore += U;
-        }
-        // the buffer is free once this item's stores have read it: fetch the rows of the item after the next one
-        if (tid == 0 && it + 2LL * gridDim.x < nitems) {
-            bulk_wait_read<0>();
-            issue_loads(it + 2LL * gridDim.x, buf);
-        }
-    }
-    if (tid == 0) bulk_wait<0>();
-}
-
-// ------------------------------------------------------------------------------------------------
-// analysis, variant with in-place staging (two CTAs per SM): the rows of an item are bulk-copied straight into the
-// transform buffers; every thread owns exactly one pass-A butterfly, reads its inputs into registers, and the pass
-// writes the buffers in place after a barrier.  No prefetch inside a CTA -- the copy of the next item is in flight while
-// the OTHER CTA of the SM computes -- but twice as many warps per SM as the prefetching variant above.
+// analysis: maps -> F for the belt ring pairs p_first .. p_first + npairs - 1 (all of length N = 2^LOGN), two CTAs per
+// SM.  The rows of an item are bulk-copied straight into the transform buffers; every thread owns exactly one pass-A
+// butterfly, reads its inputs into registers, and the pass writes the buffers in place after a barrier.  There is no
+// prefetch inside a CTA: the copy of the next item is in flight while the OTHER CTA of the SM computes (a variant with
+// a double-buffered input staging area and one CTA per SM had half the warps and was 15 % slower).
 // shared memory: [KT transform buffers][4 output slots][mbarrier]
 // ------------------------------------------------------------------------------------------------
 template <int LOGN, int KT>
@@ -1153,11 +967,6 @@ k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
 }
 
 // ---- host side -------------------------------------------------------------------------------------------
-template <int LOGN, int KT>
-static size_t analysis_p2_smem()
-{
-    return (size_t)2 * KT * 2 * (1 << LOGN) * 8 + (size_t)KT * p2::buf_stride<LOGN, KT>() * 16 + 64;
-}
 template <int LOGN, int KT, int NSL>
 static size_t synthesis_p2_smem()
 {
@@ -1184,25 +993,6 @@ static cudaError_t run_analysis_p2i(sht_plan_s* pl, const DevicePlan& d, const d
     return cudaGetLastError();
 }
 
-template <int LOGN, int KT>
-static cudaError_t run_analysis_p2(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
-{
-    const size_t sm = analysis_p2_smem<LOGN, KT>();
-    cudaError_t e = cudaFuncSetAttribute(k_ring_analysis_p2<LOGN, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (e != cudaSuccess) return e;
-    CUtensorMap tm;
-    bool planes = true;
-    if (make_tmap_ring(d, F, KT, p2::NT / KT, true, &tm) != cudaSuccess) {
-        planes = false;
-        if ((e = make_tmap_ring(d, F, KT, p2::NT / KT, false, &tm)) != cudaSuccess) return e;
-    }
-    const long long nitems = (long long)pl->belt_count * d.ncomp * ((kmaps + KT - 1) / KT);
-    const unsigned grid = (unsigned)(nitems < pl->sm_count ? nitems : pl->sm_count);
-    k_ring_analysis_p2<LOGN, KT><<<grid, p2::NT, sm, st>>>(tm, d, maps, k0, kmaps, pl->belt_first, pl->belt_count, planes ? 1 : 0);
-    pl->launches++;
-    return cudaGetLastError();
-}
-
 template <int LOGN, int KT, int NSL>
 static cudaError_t run_synthesis_p2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* maps, int k0, int kmaps, cudaStream_t st)
 {
@@ -1216,8 +1006,7 @@ static cudaError_t run_synthesis_p2(sht_plan_s* pl, const DevicePlan& d, const d
         if ((e = make_tmap_ring(d, F, KT, p2::NT / KT, false, &tm)) != cudaSuccess) return e;
     }
     const long long nitems = (long long)pl->belt_count * d.ncomp * ((kmaps + KT - 1) / KT);
-    const int occ = pl->p2_syn_occ > 0 ? pl->p2_syn_occ : 1;
-    long long want = (long long)pl->sm_count * occ;
+    const long long want = 2LL * pl->sm_count;           // two CTAs per SM
     const unsigned grid = (unsigned)(nitems < want ? nitems : want);
     k_ring_synthesis_p2<LOGN, KT, NSL><<<grid, p2::NT, sm, st>>>(tm, d, maps, k0, kmaps, pl->belt_first, pl->belt_count, planes ? 1 : 0);
     pl->launches++;
@@ -1316,18 +1105,10 @@ cudaError_t launch_ring_synthesis_cz(sht_plan_s* pl, const DevicePlan& d, const 
 // belt ring pairs of a power-of-two nside through the fast path; returns cudaErrorNotSupported if this plan has none
 cudaError_t launch_ring_analysis_belt(sht_plan_s* pl, const DevicePlan& d, const double* maps, double* F, int k0, int kmaps, cudaStream_t st)
 {
-    if (pl->p2_variant == 1) {
-        switch (pl->belt_logn) {
-            case 9: return run_analysis_p2i<9, 4>(pl, d, maps, F, k0, kmaps, st);
-            case 10: return run_analysis_p2i<10, 4>(pl, d, maps, F, k0, kmaps, st);
-            case 11: return run_analysis_p2i<11, 2>(pl, d, maps, F, k0, kmaps, st);
-            default: return cudaErrorNotSupported;
-        }
-    }
     switch (pl->belt_logn) {
-        case 9: return run_analysis_p2<9, 4>(pl, d, maps, F, k0, kmaps, st);
-        case 10: return run_analysis_p2<10, 4>(pl, d, maps, F, k0, kmaps, st);
-        case 11: return run_analysis_p2<11, 2>(pl, d, maps, F, k0, kmaps, st);
+        case 9: return run_analysis_p2i<9, 4>(pl, d, maps, F, k0, kmaps, st);
+        case 10: return run_analysis_p2i<10, 4>(pl, d, maps, F, k0, kmaps, st);
+        case 11: return run_analysis_p2i<11, 2>(pl, d, maps, F, k0, kmaps, st);
         default: return cudaErrorNotSupported;
     }
 }
