@@ -283,6 +283,9 @@ def main():
     ap.add_argument("--leg-split", type=int, default=-1, help="SHT_OPT_LEG_RING_SPLIT (default: the plan's)")
     ap.add_argument("--compare", default="", choices=["", "cublas"],
                     help="cublas: also time the paper's per-m cuBLAS DGEMM formulation of the Legendre stage (comparison only)")
+    ap.add_argument("--no-cublas-peak", action="store_true",
+                    help="skip the 2 s cuBLAS DGEMM peak measurement (comparison leg, after the timed region); used for the "
+                         "ncu launch lists so that they hold the library's own kernels only")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
@@ -401,7 +404,7 @@ def main():
     if args.iter >= 0:
         dirs = {1: 2 * args.iter + 1, 2: 1} if args.iter_mode == "immediate" else {1: args.iter + 1, 2: max(args.iter, 1)}
     mma_peak = sht_measure_fp64_mma_peak(300.0)
-    cublas_peak = cublas_dgemm_peak(dev) if rank == 0 else None
+    cublas_peak = cublas_dgemm_peak(dev) if (rank == 0 and not args.no_cublas_peak) else None
     cublas_cmp = cublas_per_m_dgemm(c, dev) if (args.compare == "cublas" and rank == 0) else None
     peak_note = ("FP64 DMMA.8x8x4 register-resident loop measured live in this run "
                  "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = %.1f; "

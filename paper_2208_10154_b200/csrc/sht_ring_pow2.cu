@@ -718,8 +718,8 @@ k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
 #pragma unroll
                 for (int r = 0; r < R1; ++r) {
                     const int n = j + r * (L / R1);
-                    u[r] = make_double2(0.0, 0.0);
-                    if (n < N) u[r] = cmul(make_double2(rows[n], rows[N + n]), __ldg(chirp + n));
+                    u[r] = make_double2(0.0, 0.0);       // N <= L / 2: the upper half of the inputs is always zero (pruned at compile time)
+                    if (r < R1 / 2 && n < N) u[r] = cmul(make_double2(rows[n], rows[N + n]), __ldg(chirp + n));
                 }
                 dft<R1, false>(u);
                 mul_powers<R1>(u, tw.a[i]);
@@ -748,7 +748,7 @@ k_ring_analysis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const 
                 mul_powers<R1>(u, make_double2(tw.a[i].x, -tw.a[i].y));
                 dft<R1, true>(u);
 #pragma unroll
-                for (int r = 0; r < R1; ++r) {
+                for (int r = 0; r < R1 / 2; ++r) {        // outputs n >= L / 2 >= N are never needed
                     const int n = j + r * (L / R1);
                     if (n < N) bins[n] = cmul(u[r], __ldg(chirp + n));
                 }
@@ -915,8 +915,8 @@ k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
 #pragma unroll
                 for (int r = 0; r < R1; ++r) {
                     const int n = j + r * (L / R1);
-                    u[r] = make_double2(0.0, 0.0);
-                    if (n < N) { double2 c = __ldg(chirp + n); c.y = -c.y; u[r] = cmul(trk[n], c); }
+                    u[r] = make_double2(0.0, 0.0);       // N <= L / 2: the upper half of the inputs is always zero
+                    if (r < R1 / 2 && n < N) { double2 c = __ldg(chirp + n); c.y = -c.y; u[r] = cmul(trk[n], c); }
                 }
             }
             __syncthreads();
@@ -950,7 +950,7 @@ k_ring_synthesis_cz(const __grid_constant__ CUtensorMap tmF, DevicePlan d, const
                 dft<R1, true>(u);
                 if (k < kmaps) {
 #pragma unroll
-                    for (int r = 0; r < R1; ++r) {
+                    for (int r = 0; r < R1 / 2; ++r) {    // pixels n >= L / 2 >= N do not exist
                         const int n = j + r * (L / R1);
                         if (n < N) {
                             double2 c = __ldg(chirp + n); c.y = -c.y;
