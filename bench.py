@@ -411,8 +411,9 @@ def main():
                  "rule-derived bf16 %s x 45/2250 = %.1f)"
                  % (FP64_NOMINAL_TFLOPS, peak_src, peaks.get("bf16_tflops", 0) * 45.0 / 2250.0))
 
-    # the committed captures describe the plain analysis + synthesis step only (no --pol, no --iter)
-    plain_key = None if (args.pol or args.iter >= 0) else (args.config, nmaps, lambda_mode)
+    # the committed captures describe the plain analysis + synthesis step with the default launch shapes only
+    default_shapes = options == {"ring_path": "fast", "leg_tiles_per_cta": 2, "leg_ring_split": 3}
+    plain_key = None if (args.pol or args.iter >= 0 or not default_shapes) else (args.config, nmaps, lambda_mode)
 
     def leg_roofline(stage, kernel):
         n = max(1, stage_n[stage])                          # timed brackets = calls of the stage (generator + contraction)
