@@ -135,6 +135,23 @@ sht_status_t sht_synthesis_pol(sht_plan_t plan, const double* alm, double* maps,
  * stream-ordered scratch of the library.  Spin-2 plans only.  Asynchronous on `stream`. */
 sht_status_t sht_eb_split(sht_plan_t plan, const double* maps_in, double* maps_out, int which, void* stream);
 
+/* sht_eb_split for callers that cannot allocate (a stream under CUDA graph capture, a serving loop or a harness that
+ * forbids cudaMalloc): same arguments, same result, but the a_lm scratch is a file-scope `__device__` array of the
+ * library, SHT_EB_STATIC_MAX_BYTES long, instead of a stream-ordered allocation.  The call makes no cudaMalloc /
+ * cudaMallocAsync / cudaFree and calls no allocating library routine (kernel launches and the plan's own workspace
+ * only).  Every GPU that loads the library holds the array until the process exits.
+ *   limit   : the scratch of one internal chunk, sht_plan_chunk_maps(plan) * sht_nalm(lmax) * 16 bytes, must fit:
+ *             otherwise SHT_ERR_INVALID_ARG with the two sizes in sht_last_error (nothing is launched);
+ *             create the plan with fewer maps, or use sht_eb_split.
+ *   sharing : ALL calls, of all plans and streams on one device, use the same array.  Calls that overlap on the GPU
+ *             race on it (undefined results, no fault): keep them on one stream or order them with events.  The
+ *             array keeps the previous call's contents; nothing in it has to start at zero (the analysis half of a
+ *             chunk writes every a_lm the synthesis half reads), so the call clears nothing.
+ *   device  : the array's address is looked up once per device (cudaGetSymbolAddress with that device current), on
+ *             the first call there; the plan's device must be the current one, as for every other call. */
+#define SHT_EB_STATIC_MAX_BYTES (32u << 20)
+sht_status_t sht_eb_split_static(sht_plan_t plan, const double* maps_in, double* maps_out, int which, void* stream);
+
 /* Same transforms on HOST buffers (pinned or pageable; same layouts).  Each call copies its input to the
  * device, runs the device entry and copies the result back, in map chunks on the plan's own streams,
  * and returns after the result is complete in host memory.  They first wait for all device work queued before

@@ -19,6 +19,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 
 SHT_OK = 0
 SHT_POL_E, SHT_POL_B = 1, 2
+SHT_EB_STATIC_MAX_BYTES = 32 << 20         # include/sht.h: static a_lm scratch of sht_eb_split_static
 SHT_LAMBDA_FUSED, SHT_LAMBDA_STAGED = 0, 1
 SHT_ITER_TM, SHT_ITER_PIXEL, SHT_ITER_IMMEDIATE = 0, 1, 2
 SHT_OPT_RING_PATH, SHT_OPT_LEG_TILES_PER_CTA, SHT_OPT_LEG_RING_SPLIT = 0, 1, 2
@@ -56,6 +57,8 @@ _lib.sht_plan_reserve_iter.argtypes = [_vp]
 _lib.sht_plan_reserve_iter.restype = _i
 _lib.sht_eb_split.argtypes = [_vp, _vp, _vp, _i, _vp]
 _lib.sht_eb_split.restype = _i
+_lib.sht_eb_split_static.argtypes = [_vp, _vp, _vp, _i, _vp]
+_lib.sht_eb_split_static.restype = _i
 _lib.sht_analysis_iter.argtypes = [_vp, _vp, _vp, _i, _vp, _vp]
 _lib.sht_analysis_iter.restype = _i
 _lib.sht_analysis_host.argtypes = [_vp, _vp, _vp]
@@ -88,7 +91,7 @@ _lib.sht_measure_fp64_mma_peak.argtypes = [_d]
 _lib.sht_measure_fp64_mma_peak.restype = _d
 
 EXPORTED = [
-    "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol", "sht_alm_pack_a7", "sht_alm_unpack_a7", "sht_plan_set_lambda_mode", "sht_plan_lambda_mode", "sht_plan_set_iter_mode", "sht_plan_reserve_iter", "sht_eb_split", "sht_plan_set_option", "sht_plan_get_option",
+    "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol", "sht_alm_pack_a7", "sht_alm_unpack_a7", "sht_plan_set_lambda_mode", "sht_plan_lambda_mode", "sht_plan_set_iter_mode", "sht_plan_reserve_iter", "sht_eb_split", "sht_eb_split_static", "sht_plan_set_option", "sht_plan_get_option",
     "sht_analysis_host", "sht_synthesis_host", "sht_npix", "sht_nalm", "sht_alm_index",
     "sht_plan_workspace_bytes", "sht_plan_chunk_maps", "sht_plan_executed_flops", "sht_plan_kernel_launches", "sht_status_string",
     "sht_last_error", "sht_measure_fp64_mma_peak", "sht_plan_set_timing", "sht_plan_stage_ms",
@@ -185,6 +188,9 @@ class Plan:
 
     def sht_eb_split(self, maps_in, maps_out, which, stream=None):
         self._check(_lib.sht_eb_split(self._h, _ptr(maps_in), _ptr(maps_out), which, _stream(stream)), "sht_eb_split")
+
+    def sht_eb_split_static(self, maps_in, maps_out, which, stream=None):
+        self._check(_lib.sht_eb_split_static(self._h, _ptr(maps_in), _ptr(maps_out), which, _stream(stream)), "sht_eb_split_static")
 
     def sht_plan_set_option(self, option, value):
         self._check(_lib.sht_plan_set_option(self._h, option, value), "sht_plan_set_option")

@@ -728,3 +728,56 @@ extern "C" double sht_measure_fp64_mma_peak(double ms)
     cudaFree(out);
     return best;
 }
+
+// ---- sht_eb_split without any allocation (include/sht.h) ------------------------------------------------
+// The a_lm scratch of one chunk lives in a file-scope device array instead of a stream-ordered allocation.  In host code
+// `g_eb_static_scratch` is only a stand-in for the symbol, not a device address: the kernels get the pointer that
+// cudaGetSymbolAddress returns for the CURRENT device (every device that loads the module has its own copy), looked up
+// once per device and kept in g_eb_static_ptr[].
+static __device__ __align__(256) double g_eb_static_scratch[SHT_EB_STATIC_MAX_BYTES / sizeof(double)];
+static constexpr int EB_STATIC_MAX_DEVICES = 64;
+static double* g_eb_static_ptr[EB_STATIC_MAX_DEVICES];   // per device ordinal; written once (same value from any thread)
+
+static cudaError_t eb_static_scratch(double** out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= EB_STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    double* p = __atomic_load_n(&g_eb_static_ptr[dev], __ATOMIC_ACQUIRE);
+    if (!p) {
+        e = cudaGetSymbolAddress((void**)&p, g_eb_static_scratch);
+        if (e != cudaSuccess) return e;
+        __atomic_store_n(&g_eb_static_ptr[dev], p, __ATOMIC_RELEASE);
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+extern "C" sht_status_t sht_eb_split_static(sht_plan_t pl, const double* maps_in, double* maps_out, int which, void* stream)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (!maps_in || !maps_out) { snprintf(pl->err, sizeof(pl->err), "null data pointer"); return SHT_ERR_NULL; }
+    if (pl->d.spin != 2 || (which != SHT_POL_E && which != SHT_POL_B)) {
+        snprintf(pl->err, sizeof(pl->err), "sht_eb_split_static needs a spin-2 plan and which = SHT_POL_E or SHT_POL_B");
+        return SHT_ERR_INVALID_ARG;
+    }
+    const size_t need = (size_t)pl->chunk * pl->d.nalm * 2 * sizeof(double);
+    if (need > (size_t)SHT_EB_STATIC_MAX_BYTES) {
+        snprintf(pl->err, sizeof(pl->err),
+                 "sht_eb_split_static: the a_lm scratch of one chunk (%d maps x %lld a_lm x 16 B = %zu bytes) exceeds the static "
+                 "array (SHT_EB_STATIC_MAX_BYTES = %zu bytes); use fewer maps per plan or sht_eb_split",
+                 pl->chunk, (long long)pl->d.nalm, need, (size_t)SHT_EB_STATIC_MAX_BYTES);
+        return SHT_ERR_INVALID_ARG;
+    }
+    double* scratch = nullptr;
+    SHT_TRY(eb_static_scratch(&scratch), "address of the static a_lm scratch");
+    cudaStream_t st = (cudaStream_t)stream;
+    sht_status_t s = SHT_OK;
+    for (int k0 = 0; k0 < pl->nmaps && s == SHT_OK; k0 += pl->chunk) {
+        const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
+        s = analysis_chunk(pl, pl->d, maps_in, k0, scratch, 0, pl->F, kmaps, false, st, which);
+        if (s == SHT_OK) s = synthesis_chunk(pl, pl->d, scratch, 0, maps_out, k0, pl->F, kmaps, nullptr, 0, st, which);
+    }
+    return s;
+}
