@@ -22,7 +22,7 @@ SHT_POL_E, SHT_POL_B = 1, 2
 SHT_EB_STATIC_MAX_BYTES = 32 << 20         # include/sht.h: static a_lm scratch of sht_eb_split_static
 SHT_LAMBDA_FUSED, SHT_LAMBDA_STAGED = 0, 1
 SHT_ITER_TM, SHT_ITER_PIXEL, SHT_ITER_IMMEDIATE = 0, 1, 2
-SHT_OPT_RING_PATH, SHT_OPT_LEG_TILES_PER_CTA, SHT_OPT_LEG_RING_SPLIT = 0, 1, 2
+SHT_OPT_RING_PATH, SHT_OPT_LEG_TILES_PER_CTA, SHT_OPT_LEG_RING_SPLIT, SHT_OPT_ITER_HYBRID, SHT_OPT_ITER_ALIAS_FREE_FROM = 0, 1, 2, 3, 4
 _vp, _i, _ll, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_double
 
 _lib.sht_plan_create.argtypes = [ctypes.POINTER(_vp), _i, _i, _i, _i]

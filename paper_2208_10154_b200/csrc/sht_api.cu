@@ -340,7 +340,30 @@ static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* al
         // caller's stream cannot be captured (it is itself under capture), the launches are issued directly.
         // an even and an odd order never fall on the same bin of a ring of 4q pixels (m' = +-m mod 4q keeps the parity):
         // the orders m, m + 1 of a step are independent, and the sweep equals the one-by-one sweep bit for bit
+        // Hybrid sweep (spin 0): the ring pairs from gs_pstar on are alias-free (sht_plan.cu), their orders never correct
+        // one another, so what they give to delta a_m does not depend on the sweep's progress and what delta a_m gives
+        // back to them is read by no later order of the sweep.  Their share of the analysis therefore runs first as ONE
+        // whole-transform launch (-> da), the chain of dependent steps covers only the ring pairs below gs_pstar and the
+        // orders below gs_mcut (delta a_m = da_m + their share; a_m += delta a_m; their R corrected at once), and the
+        // alias-free ring pairs get the synthesis of the complete da and their correction as two launches at the end.
+        // Equal to the one-by-one sweep up to the order of the ring sums.  Used when at least half of the ring pairs
+        // are alias-free (lmax <= 2 nside: the paper's case for Alg. 3).
+        const int pstar = pl->gs_pstar, mcut = pl->gs_mcut < d.lmax + 1 ? pl->gs_mcut : d.lmax + 1;
+        const bool hybrid = d.spin == 0 && !pl->gs_plain && pstar <= d.nh / 2;
         auto sweep = [&](cudaStream_t ss) -> sht_status_t {
+            if (hybrid) {
+                SHT_TRY(launch_legendre_analysis(pl, d, R, da, 0, kmaps, false, ss, 0, true, pstar), "legendre analysis (alias-free ring pairs)");
+                for (int m = 0; m < mcut; m += 2) {
+                    const int nm = m < d.lmax ? 2 : 1;
+                    SHT_TRY(launch_legendre_analysis_order(pl, d, tmF, alm, da, k0, kmaps, m, nm, ss, pstar), "legendre analysis (orders m, m+1)");
+                    SHT_TRY(launch_legendre_synthesis_order(pl, d, tmA, S, kmaps, m, nm, ss, pstar / 64), "legendre synthesis (orders m, m+1)");
+                    SHT_TRY(launch_gs_update(pl, d, S, R, m, nm, kmaps, ss, pstar), "residual update");
+                }
+                SHT_TRY(launch_alm_add_from(pl, d, alm, da, k0, kmaps, mcut, ss), "a_lm increment (orders >= gs_mcut)");
+                SHT_TRY(launch_legendre_synthesis(pl, d, da, S, 0, kmaps, ss, 0, true, pstar / 64), "legendre synthesis (alias-free ring pairs)");
+                SHT_TRY(launch_gs_update_free(pl, d, S, R, pstar, kmaps, ss), "residual update (alias-free ring pairs)");
+                return SHT_OK;
+            }
             for (int m = 0; m <= d.lmax; m += 2) {
                 const int nm = m < d.lmax ? 2 : 1;
                 SHT_TRY(launch_legendre_analysis_order(pl, d, tmF, alm, da, k0, kmaps, m, nm, ss), "legendre analysis (orders m, m+1)");
@@ -648,7 +671,8 @@ extern "C" sht_status_t sht_plan_set_option(sht_plan_t pl, int option, int value
         case SHT_OPT_RING_PATH: pl->fast_ring = value != 0; return SHT_OK;
         case SHT_OPT_LEG_TILES_PER_CTA: pl->leg_tsplit = value; return SHT_OK;
         case SHT_OPT_LEG_RING_SPLIT: pl->leg_nsplit = value < 1 ? 1 : value; return SHT_OK;
-        default: return SHT_ERR_INVALID_ARG;
+        case SHT_OPT_ITER_HYBRID: pl->gs_plain = value == 0; return SHT_OK;
+        default: return SHT_ERR_INVALID_ARG;                 // SHT_OPT_ITER_ALIAS_FREE_FROM is read-only
     }
 }
 extern "C" int sht_plan_get_option(sht_plan_t pl, int option)
@@ -658,6 +682,8 @@ extern "C" int sht_plan_get_option(sht_plan_t pl, int option)
         case SHT_OPT_RING_PATH: return pl->fast_ring ? 1 : 0;
         case SHT_OPT_LEG_TILES_PER_CTA: return pl->leg_tsplit;
         case SHT_OPT_LEG_RING_SPLIT: return pl->leg_nsplit;
+        case SHT_OPT_ITER_HYBRID: return pl->gs_plain ? 0 : 1;
+        case SHT_OPT_ITER_ALIAS_FREE_FROM: return pl->gs_pstar;
         default: return -1;
     }
 }

@@ -118,6 +118,9 @@ struct sht_plan_s {
     // (belt_logn = 0: none); class_*_nb are the launch classes of the general kernels without those pairs
     int belt_logn, belt_first, belt_count;
     int leg_tsplit, leg_nsplit;     // grid shapes of the spin-0 Legendre kernels (sht_legendre.cu launchers)
+    bool gs_plain;                        // SHT_OPT_ITER_HYBRID = 0: always the plain sweep
+    int gs_pstar, gs_mcut;                // Alg. 3 hybrid sweep: ring pairs >= gs_pstar (a multiple of 64) are alias-free; orders >= gs_mcut
+                                          // (even) touch no ring pair below gs_pstar.  gs_pstar = nh: no alias-free tail, plain sweep
     bool fast_ring;                 // SHT_OPT_RING_PATH: the belt / mixed-radix / chirp-z ring kernels are in use
     int* class_rings_nb[sht::RING_NCLASS];
     int class_count_nb[sht::RING_NCLASS];
@@ -190,19 +193,25 @@ cudaError_t launch_ring_synthesis_cz(sht_plan_s* pl, const DevicePlan& d, const 
 // gen_lambda = false: staged mode, the lambda scratch already holds this direction's blocks (host path: one generator
 // pass per call instead of one per chunk)
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                     bool accumulate, cudaStream_t st, int pol = 0, bool gen_lambda = true);
+                                     bool accumulate, cudaStream_t st, int pol = 0, bool gen_lambda = true, int pstar = 0);
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st,
-                                      int pol = 0, bool gen_lambda = true);
+                                      int pol = 0, bool gen_lambda = true, int pb0 = 0);
 // the lambda-block generator kernel of the staged mode on its own (no-op in fused mode)
 cudaError_t launch_lambda_blocks(sht_plan_s* pl, const DevicePlan& d, bool analysis, cudaStream_t st);
 // Alg. 3, the orders m .. m + nm - 1 at a time: tensor maps once per chunk, then per step analysis (alm += , da =
 // increment), synthesis of the increment into the cells of these orders of S, and the update of the residual workspace R
 cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA);
 cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
-                                           int k0, int kmaps, int m, int nm, cudaStream_t st);
+                                           int k0, int kmaps, int m, int nm, cudaStream_t st, int pstar = 0);
 cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
-                                            int nm, cudaStream_t st);
-cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st);
+                                            int nm, cudaStream_t st, int pbend = 0);
+// np > 0: only the ring pairs p < np
+cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st, int np = 0);
+// hybrid sweep of Alg. 3 (sht_api.cu): the ring pairs from pstar on are alias-free (no two orders below their mlim share a
+// bin), so all their orders are corrected in one launch: R -= re-expansion of S at every order, ring pairs >= pstar
+cudaError_t launch_gs_update_free(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int pstar, int kmaps, cudaStream_t st);
+// alm (rows from k0) += da (rows from 0) at the orders m >= m0
+cudaError_t launch_alm_add_from(sht_plan_s* pl, const DevicePlan& d, double* alm, const double* da, int k0, int kmaps, int m0, cudaStream_t st);
 cudaError_t launch_ring_power(sht_plan_s* pl, const DevicePlan& d, const double* R, const double* upow, double* acc, int kmaps, cudaStream_t st);
 constexpr size_t LAM_ABLK_BYTES = 2 * 32 * 66 * 8;      // one analysis lambda block: [class][32 rings][66] doubles
 constexpr size_t LAM_SBLK_BYTES = 32 * 66 * 8;          // one synthesis lambda block: [32 l][66] doubles

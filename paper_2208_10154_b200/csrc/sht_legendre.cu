@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(64) k_lambda_blocks_synthesis(DevicePlan d, do
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
                     int nkt, int accumulate, const double* __restrict__ lam, const int* __restrict__ i0tab,
-                    int m0, int tsplit, double* __restrict__ dout)
+                    int m0, int tsplit, double* __restrict__ dout, int pstar, int below)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
@@ -171,6 +171,14 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     const int ntile = (lmax - m) / A_ML + 1;
     const int tb = tsplit ? ((int)(blockIdx.x / nkt) % nt0) * tsplit : 0, te = tsplit ? min(tb + tsplit, ntile) : ntile;
     if (tb >= ntile) return;
+    // ring chunks of an l tile: A_PC ring pairs from the tile's first ring pst on.  Alg. 3 (hybrid sweep) splits them at the
+    // first chunk that starts at or past pstar: `below` = the chunks before it (they hold every ring pair < pstar), else
+    // the chunks from it on (ring pairs >= pstar only).  pstar = 0, below = 0: all chunks.
+    auto chunk_range = [&](int s, int& pb, int& pe) {
+        const int cut = s >= pstar ? s : s + ((pstar - s + A_PC - 1) / A_PC) * A_PC;
+        pb = below ? s : cut;
+        pe = below ? min(cut, nh) : nh;
+    };
 
     for (int t = tix; t < ntile; t += LEG_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
     if (tix == 0) {
@@ -194,7 +202,9 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
         for (int tile = tb; tile < te; ++tile) {
             const int l0 = m + tile * A_ML;
             const int i1 = min(8, (lmax - l0) / 16 + 1);        // 16-row blocks of the tile that reach down to l <= lmax
-            for (int pc = pst[tile]; pc < nh; pc += A_PC) {
+            int pcb, pce;
+            chunk_range(pst[tile], pcb, pce);
+            for (int pc = pcb; pc < pce; pc += A_PC) {
                 mbar_wait(full + stage, phase);
                 const double* Xs = reinterpret_cast<const double*>(stage_base + (size_t)stage * A_STAGE_BYTES);
                 const double* Ls = Xs + A_XBYTES / 8 + cls * (A_PC * A_SL);
@@ -261,8 +271,11 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                     if (l <= lmax && kk < kmaps) {
                         double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + l;
                         double2 v = make_double2(c[i][j][0], m == 0 ? 0.0 : c[i][j][1]);
-                        if (dout)                            // the increment itself, rows indexed from the chunk start
-                            reinterpret_cast<double2*>(dout)[((size_t)kk * d.ncomp + comp) * d.nalm + moff + l] = v;
+                        if (dout) {                          // the increment itself, rows indexed from the chunk start
+                            double2* dd = reinterpret_cast<double2*>(dout) + ((size_t)kk * d.ncomp + comp) * d.nalm + moff + l;
+                            if (below) { const double2 o = *dd; v.x += o.x; v.y += o.y; }    // + the part from the ring pairs >= pstar
+                            *dd = v;
+                        }
                         if (accumulate) { const double2 o = *dst; v.x += o.x; v.y += o.y; }
                         *dst = v;
                     }
@@ -282,8 +295,10 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
             int chunk = 0;
             for (int tile = tb; tile < te; ++tile) {
                 const size_t blk0 = (size_t)d.ablk_off[(size_t)m * d.ntile_max + tile];
-                int ck = 0;
-                for (int pc = pst[tile]; pc < nh; pc += A_PC, ++chunk, ++ck) {
+                int pcb, pce;
+                chunk_range(pst[tile], pcb, pce);
+                int ck = (pcb - pst[tile]) / A_PC;
+                for (int pc = pcb; pc < pce; pc += A_PC, ++chunk, ++ck) {
                     const int stage = chunk & 1;
                     const uint32_t phase = (chunk >> 1) & 1;
                     const int i0v = __ldg(i0tab + blk0 + ck);
@@ -318,7 +333,9 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
             if (tile + 1 < te) cf0 = load_cf(l0 + A_ML);
             const int lh = l0 + (A_ML / 2) * gh;                // first l of this warp's half
             const double2* cst = csm + (size_t)((lh - m) / LEG_CS) * nh;
-            for (int pc = pst[tile]; pc < nh; pc += A_PC, ++chunk) {
+            int pcb, pce;
+            chunk_range(pst[tile], pcb, pce);
+            for (int pc = pcb; pc < pce; pc += A_PC, ++chunk) {
                 if ((chunk & 1) != gs) continue;
                 const int stage = gs;
                 const uint32_t phase = (chunk >> 1) & 1;
@@ -385,7 +402,7 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
-                     int nkt, int npb, const double* __restrict__ lam, int m0, int nsplit)
+                     int nkt, int npb, const double* __restrict__ lam, int m0, int nsplit, int pb0, int pb1)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char* stage_base = smem_raw;
@@ -427,7 +444,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
         // this lane's workspace cell of (ring pb + g, maps 4 (16 kt + 4 wn) + t .., half cls); + i: 8 rings, + j: 4 maps
         const size_t kgs = (size_t)(lmax + 1) * d.ncomp * 2 * KG, ps = (size_t)d.nkg * kgs;
         double2* Fl = reinterpret_cast<double2*>(F) + f_cell(d, g, kt * (KTILE_MAPS / KG) + wn * 4, m, comp, cls) + t;
-        for (int pbi = sp; pbi < npb; pbi += nsplit) {
+        for (int pbi = pb0 + sp; pbi < pb1; pbi += nsplit) {
             const int pb = pbi * S_PB;
             if (m >= d.mlim[min(pb + S_PB, nh) - 1]) continue;        // no ring of this block takes part in order m (never read)
             const int cfirst = scf[pbi];
@@ -512,7 +529,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
             if (gw != 0 || lane != 0) return;
             const int row0s = (k0 + kt * KTILE_MAPS) * d.ncomp + comp;
             int stage = 0; uint32_t phase = 0;
-            for (int pbi = sp; pbi < npb; pbi += nsplit) {
+            for (int pbi = pb0 + sp; pbi < pb1; pbi += nsplit) {
                 if (m >= d.mlim[min(pbi * S_PB + S_PB, nh) - 1]) continue;
                 const size_t blk0 = (size_t)d.sblk_off[(size_t)m * d.npb + pbi];
                 int n = 0;
@@ -540,7 +557,7 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
         };
         int stage = 0; uint32_t phase = 0;
         const int row0 = (k0 + kt * KTILE_MAPS) * d.ncomp + comp;
-        for (int pbi = sp; pbi < npb; pbi += nsplit) {
+        for (int pbi = pb0 + sp; pbi < pb1; pbi += nsplit) {
             const int pb = pbi * S_PB;
             if (m >= d.mlim[min(pb + S_PB, nh) - 1]) continue;
             const int cfirst = scf[pbi];
@@ -652,8 +669,9 @@ cudaError_t launch_lambda_blocks(sht_plan_s* pl, const DevicePlan& d, bool analy
     return cudaGetLastError();
 }
 
+// pstar > 0 (spin 0, hybrid sweep of Alg. 3): only the ring chunks that start at or past ring pair pstar
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                     bool accumulate, cudaStream_t st, int pol, bool gen_lambda)
+                                     bool accumulate, cudaStream_t st, int pol, bool gen_lambda, int pstar)
 {
     if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st, pol, gen_lambda);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
@@ -669,7 +687,8 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
     if (staged && gen_lambda && (e = launch_lambda_blocks(pl, d, true, st)) != cudaSuccess) return e;
     k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0,
-                                                       staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr, 0, tsplit, nullptr);
+                                                       staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr, 0, tsplit, nullptr,
+                                                       pstar, 0);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -687,32 +706,37 @@ cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const doub
 }
 
 // alm (rows from k0) += analysis of the orders m .. m + nm - 1 of F; da (rows from 0) = that increment
+// pstar > 0 (hybrid sweep): only the ring chunks before the first one at or past pstar, and da holds the part of the
+// increment that the later chunks give (launch_legendre_analysis with the same pstar): it is added and da completed
 cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
-                                           int k0, int kmaps, int m, int nm, cudaStream_t st)
+                                           int k0, int kmaps, int m, int nm, cudaStream_t st, int pstar)
 {
     if (d.spin == 2) return launch_legendre_analysis_order_spin2(pl, d, tmF, alm, da, k0, kmaps, m, nm, st);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int ntile = (d.lmax - m) / A_ML + 1;
     k_legendre_analysis<<<(unsigned)(nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
-                                                                                                      nullptr, m, 1, da);
+                                                                                                      nullptr, m, 1, da, pstar, pstar > 0 ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
 }
 
 // F (north / south) at the orders m .. m + nm - 1 = synthesis of those orders of da (rows from 0)
+// pbend > 0 (hybrid sweep): only the first pbend blocks of 64 ring pairs
 cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
-                                            int nm, cudaStream_t st)
+                                            int nm, cudaStream_t st, int pbend)
 {
     if (d.spin == 2) return launch_legendre_synthesis_order_spin2(pl, d, tmA, F, kmaps, m, nm, st);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
-    k_legendre_synthesis<<<(unsigned)(nm * nkt * npb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, npb);
+    const int nb = pbend > 0 && pbend < npb ? pbend : npb;
+    k_legendre_synthesis<<<(unsigned)(nm * nkt * nb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, nb, 0, nb);
     pl->launches++;
     return cudaGetLastError();
 }
 
+// pb0 > 0 (spin 0, hybrid sweep of Alg. 3): only the blocks of 64 ring pairs from block pb0 on
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st,
-                                      int pol, bool gen_lambda)
+                                      int pol, bool gen_lambda, int pb0)
 {
     if (d.spin == 2) return launch_legendre_synthesis_spin2(pl, d, alm, F, k0, kmaps, st, pol, gen_lambda);
     const size_t sm = synthesis_smem();
@@ -726,8 +750,9 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
     if (staged && gen_lambda && (e = launch_lambda_blocks(pl, d, false, st)) != cudaSuccess) return e;
     // leg_nsplit CTAs share the ring blocks of an (m, k-tile) (block b goes to CTA b mod nsplit): they re-read the same
     // a_lm tile at about the same time, and the set in flight (148 / nsplit tiles of up to 1.5 MB) fits L2
-    const int nsplit = pl->leg_nsplit < 1 ? 1 : (pl->leg_nsplit > npb ? npb : pl->leg_nsplit);
-    k_legendre_synthesis<<<(d.lmax + 1) * nkt * nsplit, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, nsplit);
+    const int nsplit = pl->leg_nsplit < 1 ? 1 : (pl->leg_nsplit > npb - pb0 ? npb - pb0 : pl->leg_nsplit);
+    k_legendre_synthesis<<<(d.lmax + 1) * nkt * nsplit, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, nsplit,
+                                                                               pb0, npb);
     pl->launches++;
     return cudaGetLastError();
 }

@@ -582,6 +582,20 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             mlim[p] = run;
             rings[p].mlim = run;
         }
+        // Alg. 3, hybrid sweep (sht_api.cu): a ring pair of N pixels with mlim - 1 <= N / 2 holds no two orders that share a
+        // bin (m'' = +-m mod N needs m + m'' >= N or |m - m''| >= N), so its orders never correct one another.  gs_pstar =
+        // start of the alias-free tail of the ring pairs, rounded up to the synthesis kernel's blocks of 64 ring pairs
+        {
+            int ps = d.nh;
+            for (int p = d.nh - 1; p >= 0; --p) {
+                if (mlim[p] - 1 <= rings[p].n / 2) ps = p; else break;
+            }
+            ps = (ps + 63) / 64 * 64;
+            if (ps > d.nh) ps = d.nh;
+            pl->gs_pstar = ps;
+            int mc = ps > 0 ? mlim[ps - 1] : 0;          // mlim is monotone: no ring pair below ps takes part in an order >= mc
+            pl->gs_mcut = (mc + 1) & ~1;
+        }
         // first ring pair of every (m, l tile) of the Legendre analysis kernel: the smallest p >= the ring-pruning
         // bound whose recurrence has started before the end of the tile (no monotonicity of l_safe assumed)
         d.ntile_max = lmax / LEG_A_ML + 1;

@@ -1018,10 +1018,9 @@ __global__ void __launch_bounds__(NT, 1) k_ring_residual(DevicePlan d, const int
 // pair that falls on the same bin (directly or as the conjugate) is corrected -- the arithmetic of k_ring_residual
 // restricted to one source order.  One thread per (ring pair, map).
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* __restrict__ S, double* __restrict__ R, int m0, int kmaps)
+__device__ __forceinline__ void gs_update_cell(const DevicePlan& d, const double* __restrict__ S, double* __restrict__ R, int p, int comp,
+                                               int m, int k, int kmaps)
 {
-    const int p = blockIdx.y, comp = blockIdx.z % d.ncomp, m = m0 + blockIdx.z / d.ncomp;   // the orders of one launch never share a bin
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const RingPair& rp = d.rings[p];
     const int N = rp.n, mlim = rp.mlim;
     if (k >= kmaps || m >= mlim) return;
@@ -1062,6 +1061,38 @@ __global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* _
             c[0] = csub(c[0], se);
             c[KG] = csub(c[KG], so);
         }
+    }
+}
+
+__global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* __restrict__ S, double* __restrict__ R, int m0, int kmaps)
+{
+    // one thread per (ring pair, map); the orders of one launch never share a bin
+    gs_update_cell(d, S, R, blockIdx.y, blockIdx.z % d.ncomp, m0 + blockIdx.z / d.ncomp, blockIdx.x * blockDim.x + threadIdx.x, kmaps);
+}
+
+// The same correction for ALL orders of the ring pairs p >= pstar in one launch (hybrid sweep of Alg. 3): on a ring pair
+// with mlim - 1 <= N / 2 no two orders share a bin, so the orders are independent there.  One thread per (order, map of
+// the 4-map group): a warp walks 8 consecutive orders of one (ring pair, group), whose cells are consecutive 128-byte lines.
+__global__ void __launch_bounds__(128) k_gs_update_free(DevicePlan d, const double* __restrict__ S, double* __restrict__ R, int pstar, int kmaps)
+{
+    const int p = pstar + blockIdx.y, comp = blockIdx.z % d.ncomp, kg = blockIdx.z / d.ncomp;
+    const int m = blockIdx.x * 32 + (threadIdx.x >> 2), k = kg * KG + (threadIdx.x & 3);
+    if (m > d.lmax) return;
+    gs_update_cell(d, S, R, p, comp, m, k, kmaps);
+}
+
+// alm (rows from k0) += da (rows from 0) at the orders m >= m0: the m-major layout makes them the tail of every row
+__global__ void __launch_bounds__(256) k_alm_add_from(double2* __restrict__ alm, const double2* __restrict__ da, long long nalm, long long off0,
+                                                      int k0, int nrow_per_map)
+{
+    const long long row = blockIdx.y;                          // map * ncomp + comp, from the chunk start
+    double2* a = alm + ((long long)k0 * nrow_per_map + row) * nalm;
+    const double2* b = da + row * nalm;
+    for (long long i = off0 + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nalm; i += (long long)gridDim.x * blockDim.x) {
+        double2 v = a[i];
+        const double2 w = b[i];
+        v.x += w.x; v.y += w.y;
+        a[i] = v;
     }
 }
 
@@ -1169,9 +1200,31 @@ cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F,
     return cudaGetLastError();
 }
 
-cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st)
+cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st, int np)
 {
-    k_gs_update<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)d.nh, (unsigned)(nm * d.ncomp)), 128, 0, st>>>(d, S, R, m, kmaps);
+    const int rings = np > 0 && np < d.nh ? np : d.nh;
+    k_gs_update<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)rings, (unsigned)(nm * d.ncomp)), 128, 0, st>>>(d, S, R, m, kmaps);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gs_update_free(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int pstar, int kmaps, cudaStream_t st)
+{
+    if (pstar >= d.nh) return cudaSuccess;
+    const int nkg = (kmaps + KG - 1) / KG;
+    k_gs_update_free<<<dim3((unsigned)((d.lmax + 32) / 32), (unsigned)(d.nh - pstar), (unsigned)(nkg * d.ncomp)), 128, 0, st>>>(d, S, R, pstar, kmaps);
+    pl->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_alm_add_from(sht_plan_s* pl, const DevicePlan& d, double* alm, const double* da, int k0, int kmaps, int m0, cudaStream_t st)
+{
+    if (m0 > d.lmax) return cudaSuccess;
+    const long long off0 = (long long)m0 * (2 * d.lmax + 1 - m0) / 2 + m0;      // idx(l = m0, m0): first entry of order m0
+    const long long n = d.nalm - off0;
+    const unsigned gx = (unsigned)((n + 255) / 256 < 1024 ? (n + 255) / 256 : 1024);
+    k_alm_add_from<<<dim3(gx, (unsigned)(kmaps * d.ncomp)), 256, 0, st>>>(reinterpret_cast<double2*>(alm), reinterpret_cast<const double2*>(da),
+                                                                        d.nalm, off0, k0, d.ncomp);
     pl->launches++;
     return cudaGetLastError();
 }

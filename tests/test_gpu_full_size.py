@@ -326,6 +326,22 @@ def test_config5_immediate_iteration_properties():
     print("config 5 shapes, 64 maps: a_lm error after 0 rounds %.2e, 3 immediate sweeps %.2e, 3 traditional rounds %.2e"
           % (err_0, err_imm, err_trad))
     assert err_imm < 1e-2 * err_0
+    # at these shapes the call above took the hybrid sweep (the belt and most of the caps are alias-free): the plain sweep,
+    # every ring pair in the chain of dependent steps, gives the same a_lm and rms up to the order of the ring sums
+    from paper_2208_10154_b200.binding import SHT_OPT_ITER_HYBRID, SHT_OPT_ITER_ALIAS_FREE_FROM
+    pstar = plan.sht_plan_get_option(SHT_OPT_ITER_ALIAS_FREE_FROM)
+    assert pstar % 64 == 0 and pstar <= nside and plan.sht_plan_get_option(SHT_OPT_ITER_HYBRID) == 1
+    plan.sht_plan_set_option(SHT_OPT_ITER_HYBRID, 0)
+    plan.sht_plan_set_iter_mode(SHT_ITER_IMMEDIATE)
+    a_pl = torch.full_like(alm_true, float("nan"))
+    rms_pl = torch.full((niter, nmaps), float("nan"), dtype=torch.float64, device=dev)
+    plan.sht_analysis_iter(maps, a_pl, niter, rms_pl)
+    torch.cuda.synchronize()
+    dev_a = float(((a_imm - a_pl).abs().amax(dim=(1, 2)) / amax).max())
+    dev_r = float(np.abs(r_imm / rms_pl.cpu().numpy() - 1.0).max())
+    print("hybrid sweep (alias-free from ring pair %d) against the plain sweep: a_lm %.2e, rms %.2e" % (pstar, dev_a, dev_r))
+    assert dev_a <= 1e-11
+    assert dev_r <= RMS_TOL
     plan.destroy()
 
 

@@ -116,3 +116,42 @@ def test_immediate_iteration_spin2_against_oracle(nside, lmax, nmaps, niter, noi
     assert np.isfinite(got_alm).all()
     assert inputs.rel_err(got_alm, ref_alm) <= TOL
     assert np.abs(got_rms - ref_rms).max() <= 1e-9 * ref_rms[0].max()
+
+
+@pytest.mark.parametrize("nside,lmax,nmaps,niter,noise", [
+    (64, 127, 3, 2, 0.0),      # lmax = 2 nside - 1: the belt is alias-free, the caps are not
+    (64, 127, 70, 2, 0.2),     # two k-tiles, not band-limited
+    (64, 100, 2, 3, 0.1),      # the chain ends well before lmax
+    (128, 255, 2, 2, 0.0),     # two blocks of 64 alias-free ring pairs, two l tiles
+    (128, 150, 3, 1, 0.0),     # the alias-free tail starts inside the caps
+])
+def test_immediate_hybrid_sweep_against_oracle_and_plain_sweep(nside, lmax, nmaps, niter, noise):
+    """the hybrid sweep (include/sht.h, SHT_OPT_ITER_HYBRID: the alias-free ring pairs leave the chain of dependent steps)
+    against the oracle's pixel-space sweep, and against the plain sweep of the same plan (equal up to the order of the
+    ring sums)"""
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan, SHT_ITER_IMMEDIATE, SHT_OPT_ITER_HYBRID, SHT_OPT_ITER_ALIAS_FREE_FROM
+    alm_true = inputs.gaussian_alm(lmax, np.arange(nmaps), 95)
+    maps = O.synthesis(nside, lmax, alm_true)
+    if noise > 0.0:
+        maps = maps + inputs.white_noise(nside, np.arange(nmaps), 96, noise)
+    ref_alm, ref_rms = O.analysis_iter_immediate(nside, lmax, maps, niter)
+    plan = Plan(nside, lmax, nmaps, 0)
+    pstar = plan.sht_plan_get_option(SHT_OPT_ITER_ALIAS_FREE_FROM)
+    assert pstar % 64 == 0 and 0 < pstar <= nside, "this size is meant to take the hybrid sweep (alias-free from %d)" % pstar
+    assert plan.sht_plan_get_option(SHT_OPT_ITER_HYBRID) == 1
+    l0 = plan.kernel_launches()
+    got_alm, got_rms = _run(plan, maps, niter, SHT_ITER_IMMEDIATE)
+    l_hybrid = plan.kernel_launches() - l0
+    plan.sht_plan_set_option(SHT_OPT_ITER_HYBRID, 0)
+    l0 = plan.kernel_launches()
+    plain_alm, plain_rms = _run(plan, maps, niter, SHT_ITER_IMMEDIATE)
+    l_plain = plan.kernel_launches() - l0
+    plan.destroy()
+    assert np.isfinite(got_alm).all()
+    assert inputs.rel_err(got_alm, ref_alm) <= TOL
+    assert inputs.rel_err(plain_alm, ref_alm) <= TOL
+    assert inputs.rel_err(got_alm, plain_alm) <= 1e-12
+    assert np.abs(got_rms - ref_rms).max() <= 1e-9 * ref_rms[0].max()
+    assert np.abs(got_rms - plain_rms).max() <= 1e-11 * ref_rms[0].max()
+    assert l_hybrid != l_plain                                   # the two sweeps really are different launch sequences
