@@ -287,6 +287,7 @@ def main():
                     help="skip the 2 s cuBLAS DGEMM peak measurement (comparison leg, after the timed region); used for the "
                          "ncu launch lists so that they hold the library's own kernels only")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-f32", action="store_true", help="also time the end-to-end step with FP32 storage at the ABI (e2e.fp32_storage)")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
     c = dict(inputs.CONFIGS[args.config])
@@ -491,6 +492,31 @@ def main():
         except Exception as ex:  # host memory too small for pinned copies of the workload, etc.
             e2e = {"value": None, "unit": unit_of(c), "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
                    "error": str(ex)[:200]}
+        # the same step with FP32 storage at the ABI (float32 maps, complex64 a_lm in host memory, FP64 arithmetic on the
+        # device): an extra line for callers whose maps are single precision; `e2e` above stays the FP64 metric
+        if e2e.get("value") and args.e2e_f32:
+            try:
+                f_alm = h_alm.to(torch.complex64).pin_memory()
+                del h_alm, h_alm_out, h_maps
+                f_maps = torch.empty((nmaps, ncomp, npix), dtype=torch.float32).pin_memory()
+                f_alm_out = torch.empty((nmaps, ncomp, nalm), dtype=torch.complex64).pin_memory()
+                plan.sht_synthesis_host_f32(f_alm, f_maps)
+                plan.sht_analysis_host_f32(f_maps, f_alm_out)
+                if world > 1:
+                    dist.barrier()
+                t0 = time.perf_counter()
+                for _ in range(nrep):
+                    plan.sht_synthesis_host_f32(f_alm, f_maps)
+                    plan.sht_analysis_host_f32(f_maps, f_alm_out)
+                torch.cuda.synchronize()
+                dt = shard.max_over_ranks((time.perf_counter() - t0) / nrep, dev)
+                nb = f_alm.numel() * 8 + f_maps.numel() * 4
+                e2e["fp32_storage"] = {"value": world * nmaps / dt, "unit": unit_of(c), "h2d_bytes_per_step": nb,
+                                       "d2h_bytes_per_step": nb, "ms_per_step": dt * 1e3,
+                                       "api": "sht_synthesis_host_f32 + sht_analysis_host_f32 (float32 / complex64 in pinned host "
+                                              "memory; arithmetic unchanged FP64)"}
+            except Exception as ex:
+                e2e["fp32_storage"] = {"value": None, "error": str(ex)[:200]}
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:

@@ -169,6 +169,20 @@ sht_status_t sht_eb_split_static(sht_plan_t plan, const double* maps_in, double*
 sht_status_t sht_analysis_host(sht_plan_t plan, const double* maps_host, double* alm_host);
 sht_status_t sht_synthesis_host(sht_plan_t plan, const double* alm_host, double* maps_host);
 
+/* FP32 storage (NEXT row N4, north_star's optional FP32 path, tolerance 1e-4): the same transforms with `maps` and `alm`
+ * held in single precision by the caller (float maps, complex64 a_lm; same layouts and index rules, 8-byte aligned).  The
+ * arithmetic inside is unchanged FP64: inputs are widened and results rounded once, chunk by chunk, through the plan's
+ * staging buffers, so the error against the FP64 result is one rounding of the output (relative 6e-8 of the largest
+ * value) -- what these entries buy is half the bytes over PCIe and in the caller's memory, not a faster contraction (a
+ * TF32 / tcgen05 contraction is not built).
+ *   sht_*_f32       DEVICE pointers, asynchronous on `stream` like the FP64 entries (the first call allocates the
+ *                   staging buffers: one synchronous cudaMalloc);
+ *   sht_*_host_f32  HOST pointers, synchronous, chunked H2D -> widen -> transform -> round -> D2H on the plan's streams. */
+sht_status_t sht_analysis_f32(sht_plan_t plan, const float* maps, float* alm, void* stream);
+sht_status_t sht_synthesis_f32(sht_plan_t plan, const float* alm, float* maps, void* stream);
+sht_status_t sht_analysis_host_f32(sht_plan_t plan, const float* maps_host, float* alm_host);
+sht_status_t sht_synthesis_host_f32(sht_plan_t plan, const float* alm_host, float* maps_host);
+
 /* The paper's packed storage (eq. A7): all a_lm of one map in a real (lmax+1) x (lmax+1) matrix,
  * row-major, Re a_lm at (row l, column m), Im a_lm (m >= 1) at (row l - m, column lmax - m + 1); Im a_l0 is not stored
  * and reads back as 0 (0-based indices, reading G20).  Converters between it and the m-major `alm` layout:

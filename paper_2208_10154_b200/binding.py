@@ -65,6 +65,12 @@ _lib.sht_analysis_host.argtypes = [_vp, _vp, _vp]
 _lib.sht_analysis_host.restype = _i
 _lib.sht_synthesis_host.argtypes = [_vp, _vp, _vp]
 _lib.sht_synthesis_host.restype = _i
+for _n in ("sht_analysis_f32", "sht_synthesis_f32"):
+    getattr(_lib, _n).argtypes = [_vp, _vp, _vp, _vp]
+    getattr(_lib, _n).restype = _i
+for _n in ("sht_analysis_host_f32", "sht_synthesis_host_f32"):
+    getattr(_lib, _n).argtypes = [_vp, _vp, _vp]
+    getattr(_lib, _n).restype = _i
 _lib.sht_npix.argtypes = [_i]
 _lib.sht_npix.restype = _ll
 _lib.sht_nalm.argtypes = [_i]
@@ -92,7 +98,7 @@ _lib.sht_measure_fp64_mma_peak.restype = _d
 
 EXPORTED = [
     "sht_plan_create", "sht_plan_create_ex", "sht_plan_destroy", "sht_analysis", "sht_synthesis", "sht_analysis_iter", "sht_analysis_pol", "sht_synthesis_pol", "sht_alm_pack_a7", "sht_alm_unpack_a7", "sht_plan_set_lambda_mode", "sht_plan_lambda_mode", "sht_plan_set_iter_mode", "sht_plan_reserve_iter", "sht_eb_split", "sht_eb_split_static", "sht_plan_set_option", "sht_plan_get_option",
-    "sht_analysis_host", "sht_synthesis_host", "sht_npix", "sht_nalm", "sht_alm_index",
+    "sht_analysis_host", "sht_synthesis_host", "sht_analysis_f32", "sht_synthesis_f32", "sht_analysis_host_f32", "sht_synthesis_host_f32", "sht_npix", "sht_nalm", "sht_alm_index",
     "sht_plan_workspace_bytes", "sht_plan_chunk_maps", "sht_plan_executed_flops", "sht_plan_kernel_launches", "sht_status_string",
     "sht_last_error", "sht_measure_fp64_mma_peak", "sht_plan_set_timing", "sht_plan_stage_ms",
 ]
@@ -215,6 +221,19 @@ class Plan:
 
     def sht_synthesis_host(self, alm_host, maps_host):
         self._check(_lib.sht_synthesis_host(self._h, _ptr(alm_host), _ptr(maps_host)), "sht_synthesis_host")
+
+    # FP32 storage (float32 maps, complex64 a_lm), FP64 arithmetic inside
+    def sht_analysis_f32(self, maps, alm, stream=None):
+        self._check(_lib.sht_analysis_f32(self._h, _ptr(maps), _ptr(alm), _stream(stream)), "sht_analysis_f32")
+
+    def sht_synthesis_f32(self, alm, maps, stream=None):
+        self._check(_lib.sht_synthesis_f32(self._h, _ptr(alm), _ptr(maps), _stream(stream)), "sht_synthesis_f32")
+
+    def sht_analysis_host_f32(self, maps_host, alm_host):
+        self._check(_lib.sht_analysis_host_f32(self._h, _ptr(maps_host), _ptr(alm_host)), "sht_analysis_host_f32")
+
+    def sht_synthesis_host_f32(self, alm_host, maps_host):
+        self._check(_lib.sht_synthesis_host_f32(self._h, _ptr(alm_host), _ptr(maps_host)), "sht_synthesis_host_f32")
 
     def sht_plan_set_timing(self, enable):
         self._check(_lib.sht_plan_set_timing(self._h, 1 if enable else 0), "sht_plan_set_timing")

@@ -627,6 +627,121 @@ extern "C" sht_status_t sht_synthesis_host(sht_plan_t pl, const double* alm_host
     return host_run(pl, alm_host, maps_host, false);
 }
 
+// ---- FP32 storage at the ABI (include/sht.h): widen -> FP64 transform -> round, chunk by chunk -----------------
+// pairs of values per thread (every row length here is even: npix = 12 nside^2, a_lm rows are (re, im) pairs)
+__global__ void __launch_bounds__(256) k_widen_f32(const float2* __restrict__ in, double2* __restrict__ out, size_t npair)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npair; i += (size_t)gridDim.x * blockDim.x) {
+        const float2 v = in[i];
+        out[i] = make_double2((double)v.x, (double)v.y);
+    }
+}
+__global__ void __launch_bounds__(256) k_round_f32(const double2* __restrict__ in, float2* __restrict__ out, size_t npair)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npair; i += (size_t)gridDim.x * blockDim.x) {
+        const double2 v = in[i];
+        out[i] = make_float2((float)v.x, (float)v.y);            // round to nearest even
+    }
+}
+static unsigned f32_grid(size_t npair) { const size_t g = (npair + 255) / 256; return (unsigned)(g < 8192 ? (g ? g : 1) : 8192); }
+
+// single-precision staging of the host entries (one pair of buffers per chunk slot), allocated on the first such call
+static sht_status_t host_setup_f32(sht_plan_t pl)
+{
+    if (pl->host_f32_ready) return SHT_OK;
+    const DevicePlan& d = pl->d;
+    const size_t mbytes = (size_t)pl->host_chunk * d.ncomp * d.npix * sizeof(float);
+    const size_t abytes = (size_t)pl->host_chunk * d.ncomp * d.nalm * 2 * sizeof(float);
+    cudaError_t e = cudaSuccess;
+    for (int i = 0; i < pl->host_nb && e == cudaSuccess; ++i) {
+        e = cudaMalloc((void**)&pl->stage_maps_f32[i], mbytes);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&pl->stage_alm_f32[i], abytes);
+    }
+    if (e != cudaSuccess) {
+        for (int i = 0; i < 4; ++i) {
+            if (pl->stage_maps_f32[i]) { cudaFree(pl->stage_maps_f32[i]); pl->stage_maps_f32[i] = nullptr; }
+            if (pl->stage_alm_f32[i]) { cudaFree(pl->stage_alm_f32[i]); pl->stage_alm_f32[i] = nullptr; }
+        }
+        return cuda_fail(pl, "single-precision staging", e);
+    }
+    pl->host_f32_ready = true;
+    return SHT_OK;
+}
+
+// host = true: `in` / `out` are host pointers, chunks pipelined over the plan's streams as in host_run; host = false: device
+// pointers, every chunk on the caller's stream through staging slot 0
+static sht_status_t run_f32(sht_plan_t pl, const float* in, float* out, bool analysis, bool host, cudaStream_t user_st)
+{
+    if (!pl) return SHT_ERR_NULL;
+    if (!in || !out) { snprintf(pl->err, sizeof(pl->err), "null data pointer"); return SHT_ERR_NULL; }
+    sht_status_t s = host_setup(pl);
+    if (s == SHT_OK && host) s = host_setup_f32(pl);
+    if (s != SHT_OK) return s;
+    const DevicePlan& d = pl->d;
+    const size_t map_elems = (size_t)d.ncomp * d.npix, alm_elems = (size_t)d.ncomp * d.nalm * 2;
+    const size_t in_elems = analysis ? map_elems : alm_elems, out_elems = analysis ? alm_elems : map_elems;
+    DevicePlan dh = d;
+    dh.kpad = pl->host_kpad;
+    dh.nkg = dh.kpad / KG;
+    const size_t f_slice = (size_t)d.nh * (d.lmax + 1) * d.ncomp * 2 * pl->host_kpad * 2;
+    if (host) {
+        SHT_TRY(cudaDeviceSynchronize(), "host-path entry sync");
+        SHT_TRY(launch_lambda_blocks(pl, dh, analysis, pl->hstream[0]), "lambda blocks");
+        SHT_TRY(cudaEventRecord(pl->hevent, pl->hstream[0]), "lambda event");
+        for (int i = 1; i < pl->host_nb; ++i) SHT_TRY(cudaStreamWaitEvent(pl->hstream[i], pl->hevent, 0), "lambda wait");
+    } else {
+        SHT_TRY(launch_lambda_blocks(pl, dh, analysis, user_st), "lambda blocks");
+    }
+    int idx = 0;
+    for (int k0 = 0; k0 < pl->nmaps; k0 += pl->host_chunk, ++idx) {
+        const int b = host ? idx % pl->host_nb : 0;
+        const int kmaps = pl->nmaps - k0 < pl->host_chunk ? pl->nmaps - k0 : pl->host_chunk;
+        cudaStream_t st = host ? pl->hstream[b] : user_st;
+        double* dmaps = pl->stage_maps[b]; double* dalm = pl->stage_alm[b];
+        double* din = analysis ? dmaps : dalm; double* dout = analysis ? dalm : dmaps;
+        double* F = pl->F + (size_t)b * f_slice;
+        const size_t nin = (size_t)kmaps * in_elems, nout = (size_t)kmaps * out_elems;
+        const float* src = in + (size_t)k0 * in_elems;
+        float* dst = out + (size_t)k0 * out_elems;
+        if (host) {
+            float* fin = analysis ? pl->stage_maps_f32[b] : pl->stage_alm_f32[b];
+            SHT_TRY(cudaMemcpyAsync(fin, src, nin * sizeof(float), cudaMemcpyHostToDevice, st), "H2D");
+            src = fin;
+        }
+        k_widen_f32<<<f32_grid(nin / 2), 256, 0, st>>>(reinterpret_cast<const float2*>(src), reinterpret_cast<double2*>(din), nin / 2);
+        pl->launches++;
+        SHT_TRY(cudaGetLastError(), "widen kernel");
+        s = analysis ? analysis_chunk(pl, dh, dmaps, 0, dalm, 0, F, kmaps, false, st, 0, false)
+                     : synthesis_chunk(pl, dh, dalm, 0, dmaps, 0, F, kmaps, nullptr, 0, st, 0, false);
+        if (s != SHT_OK) return s;
+        float* fout = host ? (analysis ? pl->stage_alm_f32[b] : pl->stage_maps_f32[b]) : dst;
+        k_round_f32<<<f32_grid(nout / 2), 256, 0, st>>>(reinterpret_cast<const double2*>(dout), reinterpret_cast<float2*>(fout), nout / 2);
+        pl->launches++;
+        SHT_TRY(cudaGetLastError(), "round kernel");
+        if (host) SHT_TRY(cudaMemcpyAsync(dst, fout, nout * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H");
+    }
+    if (host)
+        for (int i = 0; i < pl->host_nb; ++i) SHT_TRY(cudaStreamSynchronize(pl->hstream[i]), "host-path sync");
+    return SHT_OK;
+}
+
+extern "C" sht_status_t sht_analysis_f32(sht_plan_t pl, const float* maps, float* alm, void* stream)
+{
+    return run_f32(pl, maps, alm, true, false, (cudaStream_t)stream);
+}
+extern "C" sht_status_t sht_synthesis_f32(sht_plan_t pl, const float* alm, float* maps, void* stream)
+{
+    return run_f32(pl, alm, maps, false, false, (cudaStream_t)stream);
+}
+extern "C" sht_status_t sht_analysis_host_f32(sht_plan_t pl, const float* maps_host, float* alm_host)
+{
+    return run_f32(pl, maps_host, alm_host, true, true, nullptr);
+}
+extern "C" sht_status_t sht_synthesis_host_f32(sht_plan_t pl, const float* alm_host, float* maps_host)
+{
+    return run_f32(pl, alm_host, maps_host, false, true, nullptr);
+}
+
 // ---- eq. A7 packed real-square a_lm format -----------------------------------------------------------------
 static sht_status_t a7_run(int lmax, long long rows, double* alm, double* sq, bool pack, void* stream)
 {

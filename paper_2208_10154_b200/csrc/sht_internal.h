@@ -148,6 +148,9 @@ struct sht_plan_s {
     // host-entry staging (allocated on first use)
     double* stage_maps[4];
     double* stage_alm[4];
+    float* stage_maps_f32[4];       // single-precision staging of the *_host_f32 entries (allocated on their first call)
+    float* stage_alm_f32[4];
+    bool host_f32_ready;
     int host_kpad;                  // workspace columns per row in the host path (host_nb chunks share F)
     int host_nb;                    // chunks in flight in the host path (streams, staging buffers, workspace slices)
     int host_chunk;

@@ -842,6 +842,8 @@ extern "C" sht_status_t sht_plan_destroy(sht_plan_t pl)
     for (int i = 0; i < 4; ++i) {
         if (pl->stage_maps[i]) cudaFree(pl->stage_maps[i]);
         if (pl->stage_alm[i]) cudaFree(pl->stage_alm[i]);
+        if (pl->stage_maps_f32[i]) cudaFree(pl->stage_maps_f32[i]);
+        if (pl->stage_alm_f32[i]) cudaFree(pl->stage_alm_f32[i]);
         if (pl->hstream[i]) cudaStreamDestroy(pl->hstream[i]);
     }
     free(pl);
