@@ -82,7 +82,7 @@ int sht_plan_lambda_mode(sht_plan_t plan);
  *   SHT_OPT_LEG_TILES_PER_CTA spin-0 Legendre analysis: 0 = one CTA per (m, k-tile) walks all l tiles; n > 0 = one CTA per
  *                             (m, group of n l tiles, k-tile), so that the tiles of an order share T_m through L2 (default 2)
  *   SHT_OPT_LEG_RING_SPLIT    spin-0 Legendre synthesis: CTAs that share the ring blocks of an (m, k-tile) (default 3)
- *   SHT_OPT_ITER_HYBRID       SHT_ITER_IMMEDIATE, spin 0: 1 (default) = the hybrid sweep when at least half of the ring pairs are
+ *   SHT_OPT_ITER_HYBRID       SHT_ITER_IMMEDIATE: 1 (default) = the hybrid sweep when at least half of the ring pairs are
  *                             alias-free (see sht_plan_set_iter_mode); 0 = always the plain sweep, every ring pair in the chain
  *   SHT_OPT_ITER_ALIAS_FREE_FROM  read-only: the first ring pair (counted from the pole, a multiple of 64) from which on every
  *                             ring pair is alias-free for this plan's lmax; 2 nside if there is no such tail
@@ -115,7 +115,7 @@ sht_status_t sht_analysis_iter(sht_plan_t plan, const double* maps, double* alm,
  *                    more accurate for lmax < 3 nside).  r is kept as ring spectra T_m(theta).  resid_rms
  *                    entry n = rms of r at the start of sweep n.  Spin 0 and spin 2 (E and B of an order together); needs
  *                    the second workspace (SHT_ERR_CUDA if it does not fit).  Sequential in m within each parity class of m:
- *                    3 launches per pair of orders (m even, m + 1).  Hybrid sweep (spin 0, SHT_OPT_ITER_HYBRID): a ring of N
+ *                    3 launches per pair of orders (m even, m + 1).  Hybrid sweep (SHT_OPT_ITER_HYBRID): a ring of N
  *                    pixels on which every order present is <= N / 2 couples no two orders, so when at least half of the
  *                    ring pairs are such (lmax <= 2 nside) their share of every delta a_m is computed by one whole-
  *                    transform launch at the start of the sweep and their residual corrected by two launches at its end;

@@ -340,7 +340,7 @@ static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* al
         // caller's stream cannot be captured (it is itself under capture), the launches are issued directly.
         // an even and an odd order never fall on the same bin of a ring of 4q pixels (m' = +-m mod 4q keeps the parity):
         // the orders m, m + 1 of a step are independent, and the sweep equals the one-by-one sweep bit for bit
-        // Hybrid sweep (spin 0): the ring pairs from gs_pstar on are alias-free (sht_plan.cu), their orders never correct
+        // Hybrid sweep: the ring pairs from gs_pstar on are alias-free (sht_plan.cu), their orders never correct
         // one another, so what they give to delta a_m does not depend on the sweep's progress and what delta a_m gives
         // back to them is read by no later order of the sweep.  Their share of the analysis therefore runs first as ONE
         // whole-transform launch (-> da), the chain of dependent steps covers only the ring pairs below gs_pstar and the
@@ -349,7 +349,7 @@ static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* al
         // Equal to the one-by-one sweep up to the order of the ring sums.  Used when at least half of the ring pairs
         // are alias-free (lmax <= 2 nside: the paper's case for Alg. 3).
         const int pstar = pl->gs_pstar, mcut = pl->gs_mcut < d.lmax + 1 ? pl->gs_mcut : d.lmax + 1;
-        const bool hybrid = d.spin == 0 && !pl->gs_plain && pstar <= d.nh / 2;
+        const bool hybrid = !pl->gs_plain && pstar <= d.nh / 2;
         auto sweep = [&](cudaStream_t ss) -> sht_status_t {
             if (hybrid) {
                 SHT_TRY(launch_legendre_analysis(pl, d, R, da, 0, kmaps, false, ss, 0, true, pstar), "legendre analysis (alias-free ring pairs)");

@@ -220,15 +220,15 @@ constexpr size_t LAM_ABLK_BYTES = 2 * 32 * 66 * 8;      // one analysis lambda b
 constexpr size_t LAM_SBLK_BYTES = 32 * 66 * 8;          // one synthesis lambda block: [32 l][66] doubles
 // spin 2 (sht_legendre_spin2.cu); the spin-0 launchers dispatch to these
 cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                           bool accumulate, cudaStream_t st, int pol, bool gen_lambda);
+                                           bool accumulate, cudaStream_t st, int pol, bool gen_lambda, int pstar);
 cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps,
-                                            cudaStream_t st, int pol, bool gen_lambda);
+                                            cudaStream_t st, int pol, bool gen_lambda, int pb0);
 cudaError_t launch_lambda_blocks_spin2(sht_plan_s* pl, const DevicePlan& d, bool analysis, cudaStream_t st);
 cudaError_t legendre_order_maps_spin2(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA);
 cudaError_t launch_legendre_analysis_order_spin2(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
-                                                 int k0, int kmaps, int m, int nm, cudaStream_t st);
+                                                 int k0, int kmaps, int m, int nm, cudaStream_t st, int pstar);
 cudaError_t launch_legendre_synthesis_order_spin2(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
-                                                  int nm, cudaStream_t st);
+                                                  int nm, cudaStream_t st, int pbend);
 // plan-time seed table (sht_plan.cu)
 cudaError_t launch_seed_table(const DevicePlan& d, const double* cm, int* lstart, double2* seed, cudaStream_t st);
 cudaError_t launch_chunk_seeds(const DevicePlan& d, double2* cseed, cudaStream_t st);

@@ -669,11 +669,11 @@ cudaError_t launch_lambda_blocks(sht_plan_s* pl, const DevicePlan& d, bool analy
     return cudaGetLastError();
 }
 
-// pstar > 0 (spin 0, hybrid sweep of Alg. 3): only the ring chunks that start at or past ring pair pstar
+// pstar > 0 (hybrid sweep of Alg. 3): only the ring chunks that start at or past ring pair pstar
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
                                      bool accumulate, cudaStream_t st, int pol, bool gen_lambda, int pstar)
 {
-    if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st, pol, gen_lambda);
+    if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st, pol, gen_lambda, pstar);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     // leg_tsplit: one CTA per (m, l tile, k-tile) instead of per (m, k-tile): the l tiles of an (m, k-tile) then read the
     // same T_m boxes at about the same time from different SMs, and L2 serves the re-reads
@@ -711,7 +711,7 @@ cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const doub
 cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
                                            int k0, int kmaps, int m, int nm, cudaStream_t st, int pstar)
 {
-    if (d.spin == 2) return launch_legendre_analysis_order_spin2(pl, d, tmF, alm, da, k0, kmaps, m, nm, st);
+    if (d.spin == 2) return launch_legendre_analysis_order_spin2(pl, d, tmF, alm, da, k0, kmaps, m, nm, st, pstar);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int ntile = (d.lmax - m) / A_ML + 1;
     k_legendre_analysis<<<(unsigned)(nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
@@ -725,7 +725,7 @@ cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, 
 cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
                                             int nm, cudaStream_t st, int pbend)
 {
-    if (d.spin == 2) return launch_legendre_synthesis_order_spin2(pl, d, tmA, F, kmaps, m, nm, st);
+    if (d.spin == 2) return launch_legendre_synthesis_order_spin2(pl, d, tmA, F, kmaps, m, nm, st, pbend);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
     const int nb = pbend > 0 && pbend < npb ? pbend : npb;
@@ -734,11 +734,11 @@ cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d,
     return cudaGetLastError();
 }
 
-// pb0 > 0 (spin 0, hybrid sweep of Alg. 3): only the blocks of 64 ring pairs from block pb0 on
+// pb0 > 0 (hybrid sweep of Alg. 3): only the blocks of 64 ring pairs from block pb0 on
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st,
                                       int pol, bool gen_lambda, int pb0)
 {
-    if (d.spin == 2) return launch_legendre_synthesis_spin2(pl, d, alm, F, k0, kmaps, st, pol, gen_lambda);
+    if (d.spin == 2) return launch_legendre_synthesis_spin2(pl, d, alm, F, k0, kmaps, st, pol, gen_lambda, pb0);
     const size_t sm = synthesis_smem();
     cudaError_t e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;

@@ -175,7 +175,8 @@ __global__ void __launch_bounds__(64) k_fpm_blocks_synthesis(DevicePlan d, doubl
 template <int WHICH>
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
-                          int nkt, int accumulate, const double* __restrict__ lam, int m0, int tsplit, double* __restrict__ dout)
+                          int nkt, int accumulate, const double* __restrict__ lam, int m0, int tsplit, double* __restrict__ dout,
+                          int pstar, int below)
 {
     constexpr int nst = 3;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -196,6 +197,13 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
     const int ntile = (lmax - m) / A2_ML + 1;
     const int tb = tsplit ? (int)(blockIdx.x / nkt) % nt0 : 0, te = tsplit ? tb + 1 : ntile;
     if (tb >= ntile) return;
+    // ring chunks of an l tile, split at the first chunk that starts at or past pstar (hybrid sweep of Alg. 3, as in the
+    // spin-0 kernel): `below` = the chunks before it, else the chunks from it on; pstar = 0, below = 0: all chunks
+    auto chunk_range = [&](int s, int& pb, int& pe) {
+        const int cut = s >= pstar ? s : s + ((pstar - s + A2_PC - 1) / A2_PC) * A2_PC;
+        pb = below ? s : cut;
+        pe = below ? min(cut, nh) : nh;
+    };
 
     for (int t = tid; t < ntile; t += LEG2_THREADS) pst[t] = d.pst[(size_t)m * d.ntile_max + t];
     if (tid == 0) {
@@ -219,7 +227,9 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
         for (int tile = tb; tile < te; ++tile) {
             const int l0 = m + tile * A2_ML;
             const int i1 = min(8, (lmax - l0) / 16 + 1);        // 16-row blocks of the tile that reach down to l <= lmax
-            for (int pc = pst[tile]; pc < nh; pc += A2_PC) {
+            int pcb, pce;
+            chunk_range(pst[tile], pcb, pce);
+            for (int pc = pcb; pc < pce; pc += A2_PC) {
                 mbar_wait(full + stage, phase);
                 const double* Xs = reinterpret_cast<const double*>(stage_base + (size_t)stage * A2_STAGE_BYTES);
                 const double* Ls = Xs + A2_XBYTES / 8;
@@ -275,6 +285,10 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                             double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * 2) * d.nalm + moff + l;
                             if (dout) {                          // the increment itself, pairs indexed from the chunk start
                                 double2* dd = reinterpret_cast<double2*>(dout) + ((size_t)kk * 2) * d.nalm + moff + l;
+                                if (below) {                     // + the part from the ring pairs >= pstar
+                                    const double2 oe = dd[0], ob = dd[d.nalm];
+                                    ve.x += oe.x; ve.y += oe.y; vb.x += ob.x; vb.y += ob.y;
+                                }
                                 dd[0] = ve;
                                 dd[d.nalm] = vb;
                             }
@@ -306,8 +320,10 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
             int stage = 0; uint32_t phase = 0;
             for (int tile = tb; tile < te; ++tile) {
                 const size_t blk0 = (size_t)d.ablk_off[(size_t)m * d.ntile_max + tile];
-                int ck = 0;
-                for (int pc = pst[tile]; pc < nh; pc += A2_PC, ++ck) {
+                int pcb, pce;
+                chunk_range(pst[tile], pcb, pce);
+                int ck = (pcb - pst[tile]) / A2_PC;
+                for (int pc = pcb; pc < pce; pc += A2_PC, ++ck) {
                     mbar_wait(empty + stage, phase ^ 1);
                     unsigned char* Xs = stage_base + (size_t)stage * A2_STAGE_BYTES;
                     mbar_arrive_expect_tx(full + stage, A2_XBYTES + A2_LBYTES);
@@ -340,7 +356,9 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
             if (tile + 1 < te) load_consts(l0 + A2_ML);
             const int lq = l0 + QL * gw;                        // first l of this warp's quarter
             const double2* cst = csm + (size_t)((lq - m) / LEG_CS) * nh;
-            for (int pc = pst[tile]; pc < nh; pc += A2_PC) {
+            int pcb, pce;
+            chunk_range(pst[tile], pcb, pce);
+            for (int pc = pcb; pc < pce; pc += A2_PC) {
                 const int p = pc + rr;
                 double x1 = 0.0, x2 = 0.0, z = 0.0, is2 = 0.0;
                 int ls = lmax + 1;
@@ -391,7 +409,7 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
 template <int WHICH, bool ORD = false>
 __global__ void __launch_bounds__(LEG2_THREADS, 1)
 k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
-                           int nkt, int npb, const double* __restrict__ lam, int m0, int nsplit)
+                           int nkt, int npb, const double* __restrict__ lam, int m0, int nsplit, int pb0, int pb1)
 {
     constexpr int NST = 3;
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -445,7 +463,7 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
         // this lane's workspace cell of (ring g, pairs 4 (8 kt + 2 wn) + t .., Q, fold part par); + i: 8 rings, + j: 4 pairs
         const size_t kgs = (size_t)(lmax + 1) * 2 * 2 * KG, ps = (size_t)d.nkg * kgs;
         double2* Fl = reinterpret_cast<double2*>(F) + f_cell(d, g, kt * P_KG + wn * 2, m, 0, par) + t;
-        for (int pbi = sp; pbi < npb; pbi += nsplit) {
+        for (int pbi = pb0 + sp; pbi < pb1; pbi += nsplit) {
         const int pb = pbi * S2_PB;
         if (m >= d.mlim[min(pb + S2_PB, nh) - 1]) continue;       // no ring of this block takes part in order m (never read)
         for (int lc = scf[pbi]; lc <= lmax; lc += S2_LC) {
@@ -520,7 +538,7 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
             // ===== staged mode: one thread streams, per stage, the a_E / a_B boxes (TMA) and the F+/F- block (bulk copy)
             if (gw != 0 || lane != 0) return;
             int stage = 0; uint32_t phase = 0;
-            for (int pbi = sp; pbi < npb; pbi += nsplit) {
+            for (int pbi = pb0 + sp; pbi < pb1; pbi += nsplit) {
                 if (m >= d.mlim[min(pbi * S2_PB + S2_PB, nh) - 1]) continue;
                 const size_t blk0 = (size_t)d.sblk_off[(size_t)m * d.npb + pbi];
                 int n = 0;
@@ -541,7 +559,7 @@ k_legendre_synthesis_spin2(const __grid_constant__ CUtensorMap tmA, DevicePlan d
         const int rl = (gw & 1) * 32 + lane;
         int stage = 0, buf = 0; uint32_t phase = 0;
         const int row0 = k0 + kt * P_KT;
-        for (int pbi = sp; pbi < npb; pbi += nsplit) {
+        for (int pbi = pb0 + sp; pbi < pb1; pbi += nsplit) {
         const int pb = pbi * S2_PB;
         if (m >= d.mlim[min(pb + S2_PB, nh) - 1]) continue;
         const int cfirst = scf[pbi];
@@ -643,7 +661,7 @@ cudaError_t launch_lambda_blocks_spin2(sht_plan_s* pl, const DevicePlan& d, bool
 }
 
 cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                           bool accumulate, cudaStream_t st, int pol, bool gen_lambda)
+                                           bool accumulate, cudaStream_t st, int pol, bool gen_lambda, int pstar)
 {
     const size_t sm = analysis2_smem(d.ntile_max);
     auto kern = pol == 1 ? k_legendre_analysis_spin2<1> : pol == 2 ? k_legendre_analysis_spin2<2> : k_legendre_analysis_spin2<0>;
@@ -654,13 +672,14 @@ cudaError_t launch_legendre_analysis_spin2(sht_plan_s* pl, const DevicePlan& d, 
     const int nkt = (kmaps + P_KT - 1) / P_KT;
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
     if (staged && gen_lambda && (e = launch_lambda_blocks_spin2(pl, d, true, st)) != cudaSuccess) return e;
-    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, staged ? pl->lam : nullptr, 0, 0, nullptr);
+    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0, staged ? pl->lam : nullptr, 0, 0, nullptr,
+                                                       pstar, 0);
     pl->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps,
-                                            cudaStream_t st, int pol, bool gen_lambda)
+                                            cudaStream_t st, int pol, bool gen_lambda, int pb0)
 {
     const size_t sm = synthesis2_smem();
     auto kern = pol == 1 ? k_legendre_synthesis_spin2<1> : pol == 2 ? k_legendre_synthesis_spin2<2> : k_legendre_synthesis_spin2<0>;
@@ -672,7 +691,7 @@ cudaError_t launch_legendre_synthesis_spin2(sht_plan_s* pl, const DevicePlan& d,
     const int npb = (d.nh + S2_PB - 1) / S2_PB;
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
     if (staged && gen_lambda && (e = launch_lambda_blocks_spin2(pl, d, false, st)) != cudaSuccess) return e;
-    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, 1);
+    kern<<<(d.lmax + 1) * nkt, LEG2_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, 1, pb0, npb);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -688,22 +707,24 @@ cudaError_t legendre_order_maps_spin2(const DevicePlan& d, const double* F, cons
 }
 
 cudaError_t launch_legendre_analysis_order_spin2(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmF, double* alm, double* da,
-                                                 int k0, int kmaps, int m, int nm, cudaStream_t st)
+                                                 int k0, int kmaps, int m, int nm, cudaStream_t st, int pstar)
 {
     const int nkt = (kmaps + P_KT - 1) / P_KT;
     const int ntile = (d.lmax - m) / A2_ML + 1;
     k_legendre_analysis_spin2<0><<<(unsigned)(nm * ntile * nkt), LEG2_THREADS, analysis2_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1,
-                                                                                                                 nullptr, m, nm, da);
+                                                                                                                 nullptr, m, nm, da, pstar, pstar > 0 ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_legendre_synthesis_order_spin2(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
-                                                  int nm, cudaStream_t st)
+                                                  int nm, cudaStream_t st, int pbend)
 {
     const int nkt = (kmaps + P_KT - 1) / P_KT;
     const int npb = (d.nh + S2_PB - 1) / S2_PB;
-    k_legendre_synthesis_spin2<0, true><<<(unsigned)(nm * nkt * npb), LEG2_THREADS, synthesis2_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, npb);
+    const int nb = pbend > 0 && pbend < npb ? pbend : npb;
+    k_legendre_synthesis_spin2<0, true><<<(unsigned)(nm * nkt * nb), LEG2_THREADS, synthesis2_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, nb,
+                                                                                                           0, nb);
     pl->launches++;
     return cudaGetLastError();
 }

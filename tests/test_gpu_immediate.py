@@ -118,25 +118,28 @@ def test_immediate_iteration_spin2_against_oracle(nside, lmax, nmaps, niter, noi
     assert np.abs(got_rms - ref_rms).max() <= 1e-9 * ref_rms[0].max()
 
 
-@pytest.mark.parametrize("nside,lmax,nmaps,niter,noise", [
-    (64, 127, 3, 2, 0.0),      # lmax = 2 nside - 1: the belt is alias-free, the caps are not
-    (64, 127, 70, 2, 0.2),     # two k-tiles, not band-limited
-    (64, 100, 2, 3, 0.1),      # the chain ends well before lmax
-    (128, 255, 2, 2, 0.0),     # two blocks of 64 alias-free ring pairs, two l tiles
-    (128, 150, 3, 1, 0.0),     # the alias-free tail starts inside the caps
+@pytest.mark.parametrize("nside,lmax,nmaps,niter,noise,spin", [
+    (64, 127, 3, 2, 0.0, 0),      # lmax = 2 nside - 1: the belt is alias-free, the caps are not
+    (64, 127, 70, 2, 0.2, 0),     # two k-tiles, not band-limited
+    (64, 100, 2, 3, 0.1, 0),      # the chain ends well before lmax
+    (128, 255, 2, 2, 0.0, 0),     # two blocks of 64 alias-free ring pairs, two l tiles
+    (128, 150, 3, 1, 0.0, 0),     # the alias-free tail starts inside the caps
+    (64, 127, 3, 2, 0.0, 2),      # spin 2: E and B of an order together
+    (64, 100, 34, 2, 0.1, 2),     # spin 2, two k-tiles of 32 pairs, not band-limited
+    (128, 150, 2, 1, 0.0, 2),     # spin 2, tail inside the caps
 ])
-def test_immediate_hybrid_sweep_against_oracle_and_plain_sweep(nside, lmax, nmaps, niter, noise):
+def test_immediate_hybrid_sweep_against_oracle_and_plain_sweep(nside, lmax, nmaps, niter, noise, spin):
     """the hybrid sweep (include/sht.h, SHT_OPT_ITER_HYBRID: the alias-free ring pairs leave the chain of dependent steps)
     against the oracle's pixel-space sweep, and against the plain sweep of the same plan (equal up to the order of the
     ring sums)"""
     from oracle import oracle as O
     from paper_2208_10154_b200.binding import Plan, SHT_ITER_IMMEDIATE, SHT_OPT_ITER_HYBRID, SHT_OPT_ITER_ALIAS_FREE_FROM
-    alm_true = inputs.gaussian_alm(lmax, np.arange(nmaps), 95)
-    maps = O.synthesis(nside, lmax, alm_true)
+    alm_true = inputs.gaussian_alm(lmax, np.arange(nmaps), 95, spin)
+    maps = O.synthesis(nside, lmax, alm_true, spin=spin)
     if noise > 0.0:
-        maps = maps + inputs.white_noise(nside, np.arange(nmaps), 96, noise)
-    ref_alm, ref_rms = O.analysis_iter_immediate(nside, lmax, maps, niter)
-    plan = Plan(nside, lmax, nmaps, 0)
+        maps = maps + inputs.white_noise(nside, np.arange(nmaps), 96, noise, spin=spin)
+    ref_alm, ref_rms = O.analysis_iter_immediate(nside, lmax, maps, niter, spin=spin)
+    plan = Plan(nside, lmax, nmaps, spin)
     pstar = plan.sht_plan_get_option(SHT_OPT_ITER_ALIAS_FREE_FROM)
     assert pstar % 64 == 0 and 0 < pstar <= nside, "this size is meant to take the hybrid sweep (alias-free from %d)" % pstar
     assert plan.sht_plan_get_option(SHT_OPT_ITER_HYBRID) == 1
