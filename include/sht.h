@@ -198,8 +198,8 @@ size_t sht_plan_workspace_bytes(sht_plan_t plan);    /* device bytes held by the
 int sht_plan_chunk_maps(sht_plan_t plan);            /* maps processed per internal chunk           */
 /* FP64 tensor-core flops ONE call of sht_analysis (direction 0) / sht_synthesis (1) executes in its contraction kernel
  * after ring pruning (item 10), l_safe row skipping (item 11, :230-232) and tile padding -- the kernels' skip
- * logic replayed on the plan's tables (measurement only: bench.py's hardware-rate roofline fraction).  -1: not counted
- * (spin-2 plans). */
+ * logic replayed on the plan's tables (measurement only: bench.py's hardware-rate roofline fraction).  Spin-2 plans: the
+ * count of the E-and-B transforms (the E-only / B-only entries execute half of it).  -1: bad arguments. */
 double sht_plan_executed_flops(sht_plan_t plan, int direction);
 long long sht_plan_kernel_launches(sht_plan_t plan); /* kernels launched by this plan so far        */
 const char* sht_status_string(sht_status_t s);       /* static storage                              */

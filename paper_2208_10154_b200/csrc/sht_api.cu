@@ -818,7 +818,7 @@ extern "C" double sht_plan_executed_flops(sht_plan_t pl, int direction)
     double tiles = 0.0;                                  // k-tiles of one call over all internal chunks
     for (int k0 = 0; k0 < pl->nmaps; k0 += pl->chunk) {
         const int kmaps = pl->nmaps - k0 < pl->chunk ? pl->nmaps - k0 : pl->chunk;
-        tiles += (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
+        tiles += pl->d.spin == 2 ? (kmaps + KTILE_MAPS / 2 - 1) / (KTILE_MAPS / 2) : (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;   // spin 2: 32 pairs per k-tile
     }
     return tiles * pl->exec_flops_tile[direction];
 }

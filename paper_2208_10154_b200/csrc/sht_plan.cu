@@ -652,7 +652,7 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             // DMMA flops one k-tile (64 maps = 128 real columns) EXECUTES per direction (spin 0): the contraction
             // kernels' own skip logic (ring pruning per l tile, l_safe row blocks, blocks past lmax) replayed on the host
             // tables -- what bench.py divides by the time for the hardware-rate roofline fraction
-            pl->exec_flops_tile[0] = pl->exec_flops_tile[1] = spin == 2 ? -1.0 : 0.0;
+            pl->exec_flops_tile[0] = pl->exec_flops_tile[1] = 0.0;
             if (spin == 0) {
                 double fa = 0.0, fs = 0.0;
                 for (int m = 0; m <= lmax; ++m) {
@@ -689,6 +689,29 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
                             if (all0 && ks1 == 4) units = 32;
                             fs += (double)units * (2.0 * 8 * 8 * 128);
                         }
+                    }
+                }
+                pl->exec_flops_tile[0] = fa; pl->exec_flops_tile[1] = fs;
+            } else {
+                // spin 2 (E and B together), per k-tile of 32 pairs = 128 real columns: the analysis kernel runs the first
+                // NI 16-row blocks of every chunk of 16 ring pairs from the tile's first ring on, the synthesis kernel
+                // every step of 4 + 4 l of its stages that reaches down to l <= lmax; both multiply by F+ and by F-
+                double fa = 0.0, fs = 0.0;
+                for (int m = 0; m <= lmax; ++m) {
+                    const int nt = (lmax - m) / LEG_A_ML + 1;
+                    for (int t = 0; t < nt; ++t) {
+                        const int l0 = m + t * LEG_A_ML;
+                        const int i1 = std::min(8, (lmax - l0) / 16 + 1);
+                        const int ni = i1 > 6 ? 8 : i1 > 4 ? 6 : i1 > 2 ? 4 : 2;
+                        const int p0 = pst[(size_t)m * d.ntile_max + t];
+                        if (p0 < d.nh) fa += (double)((d.nh - p0 + 15) / 16) * ni * (2.0 * 16 * 16 * 128 * 2);
+                    }
+                    for (int b = 0; b < d.npb; ++b) {
+                        const int cf = scf[(size_t)m * d.npb + b];
+                        const int plast = (b * 64 + 64 < d.nh ? b * 64 + 64 : d.nh) - 1;
+                        if (m >= mlim[plast] || cf > lmax) continue;
+                        for (int lc = cf; lc <= lmax; lc += 32)
+                            fs += (double)std::min(8, 2 * ((lmax - lc) / 8 + 1)) * (2.0 * 4 * 64 * 128 * 2);
                     }
                 }
                 pl->exec_flops_tile[0] = fa; pl->exec_flops_tile[1] = fs;
