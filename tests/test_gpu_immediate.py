@@ -73,12 +73,13 @@ def test_immediate_differs_from_traditional_and_is_more_accurate():
     assert inputs.rel_err(a_imm, alm_true) < inputs.rel_err(a_trad, alm_true)
 
 
-def test_immediate_chunked_workspace_and_repeat():
+@pytest.mark.parametrize("nside,lmax", [(16, 47), (64, 127)], ids=["plain_sweep", "hybrid_sweep"])
+def test_immediate_chunked_workspace_and_repeat(nside, lmax):
     """a workspace limit that forces 64-map chunks gives the same a_lm as one chunk; a second call on the same plan
     (workspaces reused, their roles swapped inside a call) repeats the first bit for bit"""
     from oracle import oracle as O
     from paper_2208_10154_b200.binding import Plan, SHT_ITER_IMMEDIATE
-    nside, lmax, nmaps, niter = 16, 47, 100, 2
+    nmaps, niter = 100, 2
     alm_true = inputs.gaussian_alm(lmax, np.arange(nmaps), 94)
     maps = O.synthesis(nside, lmax, alm_true)
     full = Plan(nside, lmax, nmaps, 0)
