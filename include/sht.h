@@ -119,8 +119,10 @@ sht_status_t sht_analysis_iter(sht_plan_t plan, const double* maps, double* alm,
  *                    pixels on which every order present is <= N / 2 couples no two orders, so when at least half of the
  *                    ring pairs are such (lmax <= 2 nside) their share of every delta a_m is computed by one whole-
  *                    transform launch at the start of the sweep and their residual corrected by two launches at its end;
- *                    only the polar ring pairs and the low orders stay in the chain.  Same sweep, different order of the
- *                    ring sums (results equal to rounding). */
+ *                    only the polar ring pairs and the low orders stay in the chain.  For 2 nside <= lmax < 4 nside (spin 0)
+ *                    the belt ring pairs leave the chain in two groups of orders (below / from 2 nside: an order meets only
+ *                    its mirror 4 nside - m there).  Same sweep, different order of the ring sums (results equal to
+ *                    rounding). */
 enum { SHT_ITER_TM = 0, SHT_ITER_PIXEL = 1, SHT_ITER_IMMEDIATE = 2 };
 sht_status_t sht_plan_set_iter_mode(sht_plan_t plan, int mode);
 /* Allocates (and zero-fills) the second workspace of SHT_ITER_TM / SHT_ITER_IMMEDIATE now and waits for it, so that

@@ -374,7 +374,30 @@ static sht_status_t iter_immediate(sht_plan_t pl, const double* maps, double* al
         // are alias-free (lmax <= 2 nside: the paper's case for Alg. 3).
         const int pstar = pl->gs_pstar, mcut = pl->gs_mcut < d.lmax + 1 ? pl->gs_mcut : d.lmax + 1;
         const bool hybrid = !pl->gs_plain && pstar <= d.nh / 2;
+        // Two-phase variant (2 nside <= lmax < 4 nside, spin 0): the belt ring pairs (from gs2_pstar on) are not alias-free,
+        // but an order m meets only 4 nside - m there.  The orders below 2 nside never meet one another on the belt, nor do
+        // the orders from 2 nside on: each of the two groups is handled like the alias-free case -- the belt's share of the
+        // group's delta a first (one launch), the chain over the cap ring pairs, then the belt synthesis of the group
+        // and its correction (every target order, also those of the other group) -- and the second group starts from
+        // the belt residual the first one left.
+        const int p2 = pl->gs2_pstar, msplit = pl->gs2_msplit;
+        const bool twophase = !hybrid && !pl->gs_plain && d.spin == 0 && msplit > 0 && msplit <= d.lmax;
         auto sweep = [&](cudaStream_t ss) -> sht_status_t {
+            if (twophase) {
+                for (int ph = 0; ph < 2; ++ph) {
+                    const int ma = ph ? msplit : 0, mb = ph ? d.lmax + 1 : msplit;      // msplit = 2 nside is even: pairs do not straddle
+                    SHT_TRY(launch_legendre_analysis(pl, d, R, da, 0, kmaps, false, ss, 0, true, p2, ma, mb - ma), "legendre analysis (belt)");
+                    for (int m = ma; m < mb; m += 2) {
+                        const int nm = m + 1 < mb ? 2 : 1;
+                        SHT_TRY(launch_legendre_analysis_order(pl, d, tmF, alm, da, k0, kmaps, m, nm, ss, p2), "legendre analysis (orders m, m+1)");
+                        SHT_TRY(launch_legendre_synthesis_order(pl, d, tmA, S, kmaps, m, nm, ss, p2 / 64), "legendre synthesis (orders m, m+1)");
+                        SHT_TRY(launch_gs_update(pl, d, S, R, m, nm, kmaps, ss, p2), "residual update");
+                    }
+                    SHT_TRY(launch_legendre_synthesis(pl, d, da, S, 0, kmaps, ss, 0, true, p2 / 64, ma, mb - ma), "legendre synthesis (belt)");
+                    SHT_TRY(launch_gs_update(pl, d, S, R, ma, mb - ma, kmaps, ss, 0, p2), "residual update (belt)");
+                }
+                return SHT_OK;
+            }
             if (hybrid) {
                 SHT_TRY(launch_legendre_analysis(pl, d, R, da, 0, kmaps, false, ss, 0, true, pstar), "legendre analysis (alias-free ring pairs)");
                 for (int m = 0; m < mcut; m += 2) {

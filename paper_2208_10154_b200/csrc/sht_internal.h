@@ -119,6 +119,8 @@ struct sht_plan_s {
     int belt_logn, belt_first, belt_count;
     int leg_tsplit, leg_nsplit;     // grid shapes of the spin-0 Legendre kernels (sht_legendre.cu launchers)
     bool gs_plain;                        // SHT_OPT_ITER_HYBRID = 0: always the plain sweep
+    int gs2_pstar, gs2_msplit;            // two-phase hybrid sweep (2 nside <= lmax < 4 nside): the belt ring pairs from gs2_pstar on couple an
+                                          // order m only with 4 nside - m, so the orders below / from gs2_msplit = 2 nside are two batches; 0: n/a
     int gs_pstar, gs_mcut;                // Alg. 3 hybrid sweep: ring pairs >= gs_pstar (a multiple of 64) are alias-free; orders >= gs_mcut
                                           // (even) touch no ring pair below gs_pstar.  gs_pstar = nh: no alias-free tail, plain sweep
     bool fast_ring;                 // SHT_OPT_RING_PATH: the belt / mixed-radix / chirp-z ring kernels are in use
@@ -196,9 +198,10 @@ cudaError_t launch_ring_synthesis_cz(sht_plan_s* pl, const DevicePlan& d, const 
 // gen_lambda = false: staged mode, the lambda scratch already holds this direction's blocks (host path: one generator
 // pass per call instead of one per chunk)
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                     bool accumulate, cudaStream_t st, int pol = 0, bool gen_lambda = true, int pstar = 0);
+                                     bool accumulate, cudaStream_t st, int pol = 0, bool gen_lambda = true, int pstar = 0,
+                                     int m_begin = 0, int m_count = -1);      // order range: spin 0 only
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st,
-                                      int pol = 0, bool gen_lambda = true, int pb0 = 0);
+                                      int pol = 0, bool gen_lambda = true, int pb0 = 0, int m_begin = 0, int m_count = -1);
 // the lambda-block generator kernel of the staged mode on its own (no-op in fused mode)
 cudaError_t launch_lambda_blocks(sht_plan_s* pl, const DevicePlan& d, bool analysis, cudaStream_t st);
 // Alg. 3, the orders m .. m + nm - 1 at a time: tensor maps once per chunk, then per step analysis (alm += , da =
@@ -209,7 +212,8 @@ cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, 
 cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d, const CUtensorMap& tmA, double* F, int kmaps, int m,
                                             int nm, cudaStream_t st, int pbend = 0);
 // np > 0: only the ring pairs p < np
-cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st, int np = 0);
+cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st, int np = 0,
+                             int p0 = 0);     // ring pairs p0 <= p < np
 // hybrid sweep of Alg. 3 (sht_api.cu): the ring pairs from pstar on are alias-free (no two orders below their mlim share a
 // bin), so all their orders are corrected in one launch: R -= re-expansion of S at every order, ring pairs >= pstar
 cudaError_t launch_gs_update_free(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int pstar, int kmaps, cudaStream_t st);

@@ -670,15 +670,19 @@ cudaError_t launch_lambda_blocks(sht_plan_s* pl, const DevicePlan& d, bool analy
 }
 
 // pstar > 0 (hybrid sweep of Alg. 3): only the ring chunks that start at or past ring pair pstar
+// m_begin / m_count (spin 0): only the orders m_begin .. m_begin + m_count - 1 (m_count < 0: up to lmax)
 cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const double* F, double* alm, int k0, int kmaps,
-                                     bool accumulate, cudaStream_t st, int pol, bool gen_lambda, int pstar)
+                                     bool accumulate, cudaStream_t st, int pol, bool gen_lambda, int pstar, int m_begin, int m_count)
 {
     if (d.spin == 2) return launch_legendre_analysis_spin2(pl, d, F, alm, k0, kmaps, accumulate, st, pol, gen_lambda, pstar);
+    const int nm = m_count < 0 ? d.lmax + 1 - m_begin : m_count;
+    if (nm <= 0) return cudaSuccess;
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     // leg_tsplit: one CTA per (m, l tile, k-tile) instead of per (m, k-tile): the l tiles of an (m, k-tile) then read the
     // same T_m boxes at about the same time from different SMs, and L2 serves the re-reads
     const int tsplit = pl->leg_tsplit;
-    const unsigned grid = (unsigned)((d.lmax + 1) * nkt * (tsplit ? (d.ntile_max + tsplit - 1) / tsplit : 1));
+    const int ntile0 = (d.lmax - m_begin) / A_ML + 1;      // the grid is sized for the tile groups of the first order
+    const unsigned grid = (unsigned)(nm * nkt * (tsplit ? (ntile0 + tsplit - 1) / tsplit : 1));
     const size_t sm = analysis_smem(d.ntile_max);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
@@ -687,7 +691,7 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
     if (staged && gen_lambda && (e = launch_lambda_blocks(pl, d, true, st)) != cudaSuccess) return e;
     k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0,
-                                                       staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr, 0, tsplit, nullptr,
+                                                       staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr, m_begin, tsplit, nullptr,
                                                        pstar, 0);
     pl->launches++;
     return cudaGetLastError();
@@ -736,7 +740,7 @@ cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d,
 
 // pb0 > 0 (hybrid sweep of Alg. 3): only the blocks of 64 ring pairs from block pb0 on
 cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const double* alm, double* F, int k0, int kmaps, cudaStream_t st,
-                                      int pol, bool gen_lambda, int pb0)
+                                      int pol, bool gen_lambda, int pb0, int m_begin, int m_count)
 {
     if (d.spin == 2) return launch_legendre_synthesis_spin2(pl, d, alm, F, k0, kmaps, st, pol, gen_lambda, pb0);
     const size_t sm = synthesis_smem();
@@ -751,8 +755,10 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
     // leg_nsplit CTAs share the ring blocks of an (m, k-tile) (block b goes to CTA b mod nsplit): they re-read the same
     // a_lm tile at about the same time, and the set in flight (148 / nsplit tiles of up to 1.5 MB) fits L2
     const int nsplit = pl->leg_nsplit < 1 ? 1 : (pl->leg_nsplit > npb - pb0 ? npb - pb0 : pl->leg_nsplit);
-    k_legendre_synthesis<<<(d.lmax + 1) * nkt * nsplit, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, 0, nsplit,
-                                                                               pb0, npb);
+    const int nm = m_count < 0 ? d.lmax + 1 - m_begin : m_count;
+    if (nm <= 0) return cudaSuccess;
+    k_legendre_synthesis<<<nm * nkt * nsplit, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, m_begin, nsplit,
+                                                                     pb0, npb);
     pl->launches++;
     return cudaGetLastError();
 }

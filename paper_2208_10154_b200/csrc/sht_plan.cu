@@ -595,6 +595,12 @@ extern "C" sht_status_t sht_plan_create_ex(sht_plan_t* out, int nside, int lmax,
             pl->gs_pstar = ps;
             int mc = ps > 0 ? mlim[ps - 1] : 0;          // mlim is monotone: no ring pair below ps takes part in an order >= mc
             pl->gs_mcut = (mc + 1) & ~1;
+            // two-phase variant for 2 nside <= lmax < 4 nside: on a belt ring pair (4 nside pixels, every order < 4 nside) an
+            // order m shares its bin only with 4 nside - m, so the orders below 2 nside never meet one another there, nor
+            // do the orders from 2 nside on.  Belt ring pairs from the first block of 64 that lies inside the belt.
+            pl->gs2_pstar = 0; pl->gs2_msplit = 0;
+            const int b0 = ((nside - 1) + 63) / 64 * 64;         // ring pair nside - 1 is the first belt ring
+            if (spin == 0 && lmax >= 2 * nside && lmax < 4 * nside && b0 + 64 <= d.nh) { pl->gs2_pstar = b0; pl->gs2_msplit = 2 * nside; }
         }
         // first ring pair of every (m, l tile) of the Legendre analysis kernel: the smallest p >= the ring-pruning
         // bound whose recurrence has started before the end of the tile (no monotonicity of l_safe assumed)

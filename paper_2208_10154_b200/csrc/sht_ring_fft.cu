@@ -1064,10 +1064,10 @@ __device__ __forceinline__ void gs_update_cell(const DevicePlan& d, const double
     }
 }
 
-__global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* __restrict__ S, double* __restrict__ R, int m0, int kmaps)
+__global__ void __launch_bounds__(128) k_gs_update(DevicePlan d, const double* __restrict__ S, double* __restrict__ R, int m0, int kmaps, int p0)
 {
     // one thread per (ring pair, map); the orders of one launch never share a bin
-    gs_update_cell(d, S, R, blockIdx.y, blockIdx.z % d.ncomp, m0 + blockIdx.z / d.ncomp, blockIdx.x * blockDim.x + threadIdx.x, kmaps);
+    gs_update_cell(d, S, R, p0 + blockIdx.y, blockIdx.z % d.ncomp, m0 + blockIdx.z / d.ncomp, blockIdx.x * blockDim.x + threadIdx.x, kmaps);
 }
 
 // The same correction for ALL orders of the ring pairs p >= pstar in one launch (hybrid sweep of Alg. 3): on a ring pair
@@ -1200,10 +1200,12 @@ cudaError_t launch_ring_residual(sht_plan_s* pl, const DevicePlan& d, double* F,
     return cudaGetLastError();
 }
 
-cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st, int np)
+cudaError_t launch_gs_update(sht_plan_s* pl, const DevicePlan& d, const double* S, double* R, int m, int nm, int kmaps, cudaStream_t st, int np,
+                             int p0)
 {
-    const int rings = np > 0 && np < d.nh ? np : d.nh;
-    k_gs_update<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)rings, (unsigned)(nm * d.ncomp)), 128, 0, st>>>(d, S, R, m, kmaps);
+    const int pend = np > 0 && np < d.nh ? np : d.nh;
+    if (pend <= p0 || nm <= 0) return cudaSuccess;
+    k_gs_update<<<dim3((unsigned)((kmaps + 127) / 128), (unsigned)(pend - p0), (unsigned)(nm * d.ncomp)), 128, 0, st>>>(d, S, R, m, kmaps, p0);
     pl->launches++;
     return cudaGetLastError();
 }

@@ -159,3 +159,38 @@ def test_immediate_hybrid_sweep_against_oracle_and_plain_sweep(nside, lmax, nmap
     assert np.abs(got_rms - ref_rms).max() <= 1e-9 * ref_rms[0].max()
     assert np.abs(got_rms - plain_rms).max() <= 1e-11 * ref_rms[0].max()
     assert l_hybrid != l_plain                                   # the two sweeps really are different launch sequences
+
+
+@pytest.mark.parametrize("nside,lmax,nmaps,niter,noise", [
+    (64, 191, 3, 2, 0.0),      # lmax = 3 nside - 1: every order from nside + 1 on meets its mirror 4 nside - m on the belt
+    (64, 150, 70, 2, 0.2),     # two k-tiles, not band-limited
+    (64, 129, 2, 3, 0.0),      # the second group is the two orders 2 nside, 2 nside + 1
+    (128, 300, 2, 1, 0.0),     # two blocks of belt ring pairs, three l tiles
+])
+def test_immediate_two_phase_sweep_against_oracle_and_plain_sweep(nside, lmax, nmaps, niter, noise):
+    """2 nside <= lmax < 4 nside (spin 0): the belt ring pairs leave the chain of dependent steps in two groups of orders
+    (below / from 2 nside), DESIGN.md section 6.  Against the oracle's pixel-space sweep and the plain sweep of the plan."""
+    from oracle import oracle as O
+    from paper_2208_10154_b200.binding import Plan, SHT_ITER_IMMEDIATE, SHT_OPT_ITER_HYBRID, SHT_OPT_ITER_ALIAS_FREE_FROM
+    alm_true = inputs.gaussian_alm(lmax, np.arange(nmaps), 97)
+    maps = O.synthesis(nside, lmax, alm_true)
+    if noise > 0.0:
+        maps = maps + inputs.white_noise(nside, np.arange(nmaps), 98, noise)
+    ref_alm, ref_rms = O.analysis_iter_immediate(nside, lmax, maps, niter)
+    plan = Plan(nside, lmax, nmaps, 0)
+    assert plan.sht_plan_get_option(SHT_OPT_ITER_ALIAS_FREE_FROM) > nside        # not the one-phase hybrid sweep
+    l0 = plan.kernel_launches()
+    got_alm, got_rms = _run(plan, maps, niter, SHT_ITER_IMMEDIATE)
+    l_two = plan.kernel_launches() - l0
+    plan.sht_plan_set_option(SHT_OPT_ITER_HYBRID, 0)
+    l0 = plan.kernel_launches()
+    plain_alm, plain_rms = _run(plan, maps, niter, SHT_ITER_IMMEDIATE)
+    l_plain = plan.kernel_launches() - l0
+    plan.destroy()
+    assert l_two != l_plain                                       # the two sweeps really are different launch sequences
+    assert np.isfinite(got_alm).all()
+    assert inputs.rel_err(got_alm, ref_alm) <= TOL
+    assert inputs.rel_err(plain_alm, ref_alm) <= TOL
+    assert inputs.rel_err(got_alm, plain_alm) <= 1e-12
+    assert np.abs(got_rms - ref_rms).max() <= 1e-9 * ref_rms[0].max()
+    assert np.abs(got_rms - plain_rms).max() <= 1e-11 * ref_rms[0].max()
