@@ -262,24 +262,40 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                 if (++stage == A_STAGES) { stage = 0; phase ^= 1; }
             }
             // ---- epilogue: scatter to the m-major alm layout; a lane holds (re, im) of one (l, map)
+            // (the old values of two maps of a row are loaded together before anything is stored: a load that follows
+            // a store through the same pointer cannot be moved above it, and 32 dependent round trips to HBM per tile were
+            // a fifth of the accumulating launches of Alg. 2 and most of the per-order launches of Alg. 3)
+            const bool rd_d = dout != nullptr && below, rd_a = accumulate != 0;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
                 const int l = l0 + 2 * (8 * i + g) + cls;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int kk = kt * KTILE_MAPS + wn * 16 + 4 * j + t;
-                    if (l <= lmax && kk < kmaps) {
-                        double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + l;
-                        double2 v = make_double2(c[i][j][0], m == 0 ? 0.0 : c[i][j][1]);
-                        if (dout) {                          // the increment itself, rows indexed from the chunk start
-                            double2* dd = reinterpret_cast<double2*>(dout) + ((size_t)kk * d.ncomp + comp) * d.nalm + moff + l;
-                            if (below) { const double2 o = *dd; v.x += o.x; v.y += o.y; }    // + the part from the ring pairs >= pstar
-                            *dd = v;
+                for (int jh = 0; jh < 4; jh += 2) {               // two maps at a time: the register budget has no room for four
+                    double2 od[2], oa[2];
+#pragma unroll
+                    for (int jj = 0; jj < 2; ++jj) {
+                        const int kk = kt * KTILE_MAPS + wn * 16 + 4 * (jh + jj) + t;
+                        od[jj] = make_double2(0.0, 0.0); oa[jj] = make_double2(0.0, 0.0);
+                        if (l <= lmax && kk < kmaps) {
+                            if (rd_d) od[jj] = reinterpret_cast<const double2*>(dout)[((size_t)kk * d.ncomp + comp) * d.nalm + moff + l];
+                            if (rd_a) oa[jj] = reinterpret_cast<const double2*>(alm)[((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + l];
                         }
-                        if (accumulate) { const double2 o = *dst; v.x += o.x; v.y += o.y; }
-                        *dst = v;
                     }
-                    c[i][j][0] = 0.0; c[i][j][1] = 0.0;
+#pragma unroll
+                    for (int jj = 0; jj < 2; ++jj) {
+                        const int j = jh + jj;
+                        const int kk = kt * KTILE_MAPS + wn * 16 + 4 * j + t;
+                        if (l <= lmax && kk < kmaps) {
+                            double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + l;
+                            // the increment (+ the part from the ring pairs >= pstar, hybrid sweep), then the accumulated a_lm
+                            double2 v = make_double2(c[i][j][0] + od[jj].x, (m == 0 ? 0.0 : c[i][j][1]) + od[jj].y);
+                            if (dout)                            // rows indexed from the chunk start
+                                reinterpret_cast<double2*>(dout)[((size_t)kk * d.ncomp + comp) * d.nalm + moff + l] = v;
+                            v.x += oa[jj].x; v.y += oa[jj].y;
+                            *dst = v;
+                        }
+                        c[i][j][0] = 0.0; c[i][j][1] = 0.0;
+                    }
                 }
             }
         }

@@ -283,19 +283,17 @@ k_legendre_analysis_spin2(const __grid_constant__ CUtensorMap tmF, DevicePlan d,
                         double2 vb = make_double2(cB[i][j][1], m == 0 ? 0.0 : -cB[i][j][0]);
                         if (WHICH == 0) {
                             double2* dst = reinterpret_cast<double2*>(alm) + ((size_t)(k0 + kk) * 2) * d.nalm + moff + l;
-                            if (dout) {                          // the increment itself, pairs indexed from the chunk start
-                                double2* dd = reinterpret_cast<double2*>(dout) + ((size_t)kk * 2) * d.nalm + moff + l;
-                                if (below) {                     // + the part from the ring pairs >= pstar
-                                    const double2 oe = dd[0], ob = dd[d.nalm];
-                                    ve.x += oe.x; ve.y += oe.y; vb.x += ob.x; vb.y += ob.y;
-                                }
+                            double2* dd = dout ? reinterpret_cast<double2*>(dout) + ((size_t)kk * 2) * d.nalm + moff + l : nullptr;
+                            // all old values first: a load that follows a store through the same pointer is not moved above it
+                            double2 de = make_double2(0.0, 0.0), db = de, ae = de, ab = de;
+                            if (dd && below) { de = dd[0]; db = dd[d.nalm]; }     // the part from the ring pairs >= pstar
+                            if (accumulate) { ae = dst[0]; ab = dst[d.nalm]; }
+                            ve.x += de.x; ve.y += de.y; vb.x += db.x; vb.y += db.y;
+                            if (dd) {                            // the increment itself, pairs indexed from the chunk start
                                 dd[0] = ve;
                                 dd[d.nalm] = vb;
                             }
-                            if (accumulate) {
-                                const double2 oe = dst[0], ob = dst[d.nalm];
-                                ve.x += oe.x; ve.y += oe.y; vb.x += ob.x; vb.y += ob.y;
-                            }
+                            ve.x += ae.x; ve.y += ae.y; vb.x += ab.x; vb.y += ab.y;
                             dst[0] = ve;
                             dst[d.nalm] = vb;
                         } else {
