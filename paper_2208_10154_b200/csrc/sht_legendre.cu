@@ -266,6 +266,52 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
             // a store through the same pointer cannot be moved above it, and 32 dependent round trips to HBM per tile were
             // a fifth of the accumulating launches of Alg. 2 and most of the per-order launches of Alg. 3)
             const bool rd_d = dout != nullptr && below, rd_a = accumulate != 0;
+            if ((rd_d || rd_a) && tile == te - 1) {
+                // Last tile of the CTA (the only one of a per-order launch): the pipeline has drained, so the stage buffers
+                // are free.  The tile goes through shared memory ([map][l], rows padded by one element) and the consumer
+                // warps do the read-modify-write together: consecutive threads take consecutive l of one map (coalesced),
+                // and every thread has its eight loads in flight before its first store.
+                double2* T = reinterpret_cast<double2*>(stage_base);
+                constexpr int TROW = A_ML + 1;
+                named_bar_sync(2, LEG_CONSUMER_WARPS * 32);          // every consumer warp is done reading the last stage
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        T[(wn * 16 + 4 * j + t) * TROW + 2 * (8 * i + g) + cls] = make_double2(c[i][j][0], m == 0 ? 0.0 : c[i][j][1]);
+                        c[i][j][0] = 0.0; c[i][j][1] = 0.0;
+                    }
+                named_bar_sync(2, LEG_CONSUMER_WARPS * 32);
+                const int ct = tix - LEG_GEN_WARPS * 32;             // 0 .. 255
+                const int nl = min(A_ML, lmax - l0 + 1), nk = min(KTILE_MAPS, kmaps - kt * KTILE_MAPS);
+                constexpr int EB = 8;                                // elements per thread and batch
+                for (int e0 = ct; e0 < KTILE_MAPS * A_ML; e0 += EB * LEG_CONSUMER_WARPS * 32) {
+                    double2 od[EB], oa[EB];
+#pragma unroll
+                    for (int u = 0; u < EB; ++u) {
+                        const int e = e0 + u * LEG_CONSUMER_WARPS * 32, kl = e / A_ML, ll = e % A_ML;
+                        od[u] = make_double2(0.0, 0.0); oa[u] = make_double2(0.0, 0.0);
+                        if (kl < nk && ll < nl) {
+                            const int kk = kt * KTILE_MAPS + kl;
+                            if (rd_d) od[u] = reinterpret_cast<const double2*>(dout)[((size_t)kk * d.ncomp + comp) * d.nalm + moff + l0 + ll];
+                            if (rd_a) oa[u] = reinterpret_cast<const double2*>(alm)[((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + l0 + ll];
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < EB; ++u) {
+                        const int e = e0 + u * LEG_CONSUMER_WARPS * 32, kl = e / A_ML, ll = e % A_ML;
+                        if (kl < nk && ll < nl) {
+                            const int kk = kt * KTILE_MAPS + kl;
+                            double2 v = T[kl * TROW + ll];
+                            v.x += od[u].x; v.y += od[u].y;
+                            if (dout) reinterpret_cast<double2*>(dout)[((size_t)kk * d.ncomp + comp) * d.nalm + moff + l0 + ll] = v;
+                            v.x += oa[u].x; v.y += oa[u].y;
+                            reinterpret_cast<double2*>(alm)[((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + l0 + ll] = v;
+                        }
+                    }
+                }
+                continue;                                            // (the loop over the tiles ends here)
+            }
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
                 const int l = l0 + 2 * (8 * i + g) + cls;
