@@ -143,6 +143,10 @@ __global__ void __launch_bounds__(64) k_lambda_blocks_synthesis(DevicePlan d, do
 // analysis kernel: one CTA per (m, k-tile); l tiles outer, ring chunks inner.
 // Stage layout: [X: 2 boxes x (16 kg x 16 p x 128 B, 128B-swizzled)] [lambda: 2 classes x 32 p x A_SL]
 // ------------------------------------------------------------------------------------------------
+// WIN = 1 (per-order launches of Alg. 3): four CTAs share an l tile, each owns a window of two 16-row blocks (32 l) -- the
+// launch has a few dozen CTAs for 148 SMs, so the tile is cut up for parallelism; its own instantiation, so that the
+// whole-transform kernel (WIN = 0) keeps its code and register allocation
+template <int WIN>
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, double* __restrict__ alm, int k0, int kmaps,
                     int nkt, int accumulate, const double* __restrict__ lam, const int* __restrict__ i0tab,
@@ -161,7 +165,9 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     // independent; the grid is sized for the tiles of m0, the CTAs past the last tile of their order leave
     // tsplit > 0: tile-split mode, tsplit = l tiles per CTA (the grid is sized for the tile groups of order m0)
     const int nt0 = ((d.lmax - m0) / A_ML + tsplit) / (tsplit > 0 ? tsplit : 1);
-    const int m = tsplit ? m0 + blockIdx.x / (nkt * nt0) : m0 + blockIdx.x / nkt, kt = blockIdx.x % nkt;
+    const int wsel = WIN ? (int)(blockIdx.x & 3) : 0, ib = 2 * wsel;       // WIN: this CTA's window = row blocks ib, ib + 1
+    const unsigned bx = WIN ? blockIdx.x >> 2 : blockIdx.x;
+    const int m = tsplit ? m0 + bx / (nkt * nt0) : m0 + bx / nkt, kt = bx % nkt;
     // warps 0..3 generate (the oldest warps of an SM sub-partition are served first by its scheduler: their
     // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
     const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) - LEG_GEN_WARPS;
@@ -169,8 +175,9 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
     const int lmax = d.lmax, nh = d.nh;
     const int comp = 0;
     const int ntile = (lmax - m) / A_ML + 1;
-    const int tb = tsplit ? ((int)(blockIdx.x / nkt) % nt0) * tsplit : 0, te = tsplit ? min(tb + tsplit, ntile) : ntile;
+    const int tb = tsplit ? ((int)(bx / nkt) % nt0) * tsplit : 0, te = tsplit ? min(tb + tsplit, ntile) : ntile;
     if (tb >= ntile) return;
+    if (WIN && ib >= min(8, (d.lmax - (m + tb * A_ML)) / 16 + 1)) return;      // the window lies past lmax
     // ring chunks of an l tile: A_PC ring pairs from the tile's first ring pst on.  Alg. 3 (hybrid sweep) splits them at the
     // first chunk that starts at or past pstar: `below` = the chunks before it (they hold every ring pair < pstar), else
     // the chunks from it on (ring pairs >= pstar only).  pstar = 0, below = 0: all chunks.
@@ -210,6 +217,28 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
                 const double* Ls = Xs + A_XBYTES / 8 + cls * (A_PC * A_SL);
                 // rows below the smallest l_safe of 8 rings hold lambda = 0 for them: their 16-row blocks (i < i0) are skipped
                 const int i0p = i0s[stage];
+                if constexpr (WIN != 0) {
+#pragma unroll
+                    for (int ks = 0; ks < A_PC / 4; ++ks) {
+                        const int sub = ks >> 2, ksl = ks & 3;
+                        const int pl = 8 * (ksl >> 1) + 2 * t + (ksl & 1);
+                        const int i0 = (i0p >> (4 * (2 * sub + (ksl >> 1)))) & 15;
+                        double a[2], b[4];
+                        const double* La = Ls + (16 * sub + pl) * A_SL + g;
+                        const double* Xb = Xs + sub * 4096 + pl * 16 + ((((4 * cls + (g >> 1)) ^ (pl & 7)) << 1) | (g & 1));
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) a[i] = La[8 * (ib + i)];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) b[j] = Xb[(4 * wn + j) * 256];
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) {
+                            if (ib + i >= i0 && ib + i < i1) {
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
+                            }
+                        }
+                    }
+                } else
                 if (i0p == 0) {
                     // plain loop over the first NI 16-row blocks (NI = 8 except in the last tile, whose blocks past lmax
                     // are left out in steps of two: a block-by-block test costs more than the blocks it saves)
@@ -266,6 +295,47 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
             // a store through the same pointer cannot be moved above it, and 32 dependent round trips to HBM per tile were
             // a fifth of the accumulating launches of Alg. 2 and most of the per-order launches of Alg. 3)
             const bool rd_d = dout != nullptr && below, rd_a = accumulate != 0;
+            if constexpr (WIN != 0) {
+                // the window's 32 l x 64 maps through the (drained) stage buffers, then one cooperative read-modify-write:
+                // eight elements per thread, consecutive threads on consecutive l of one map
+                double2* T = reinterpret_cast<double2*>(stage_base);
+                constexpr int WR = 32, TROW = WR + 1;
+                named_bar_sync(2, LEG_CONSUMER_WARPS * 32);
+#pragma unroll
+                for (int i = 0; i < 2; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        T[(wn * 16 + 4 * j + t) * TROW + 16 * i + 2 * g + cls] = make_double2(c[i][j][0], m == 0 ? 0.0 : c[i][j][1]);
+                named_bar_sync(2, LEG_CONSUMER_WARPS * 32);
+                const int ct = tix - LEG_GEN_WARPS * 32;
+                const int lw = l0 + 16 * ib;                         // first l of the window
+                const int nl = min(WR, lmax - lw + 1), nk = min(KTILE_MAPS, kmaps - kt * KTILE_MAPS);
+                constexpr int EB = KTILE_MAPS * WR / (LEG_CONSUMER_WARPS * 32);      // 8
+                double2 od[EB], oa[EB];
+#pragma unroll
+                for (int u = 0; u < EB; ++u) {
+                    const int e = ct + u * LEG_CONSUMER_WARPS * 32, kl = e / WR, ll = e % WR;
+                    od[u] = make_double2(0.0, 0.0); oa[u] = make_double2(0.0, 0.0);
+                    if (kl < nk && ll < nl) {
+                        const int kk = kt * KTILE_MAPS + kl;
+                        if (rd_d) od[u] = reinterpret_cast<const double2*>(dout)[((size_t)kk * d.ncomp + comp) * d.nalm + moff + lw + ll];
+                        if (rd_a) oa[u] = reinterpret_cast<const double2*>(alm)[((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + lw + ll];
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < EB; ++u) {
+                    const int e = ct + u * LEG_CONSUMER_WARPS * 32, kl = e / WR, ll = e % WR;
+                    if (kl < nk && ll < nl) {
+                        const int kk = kt * KTILE_MAPS + kl;
+                        double2 v = T[kl * TROW + ll];
+                        v.x += od[u].x; v.y += od[u].y;
+                        if (dout) reinterpret_cast<double2*>(dout)[((size_t)kk * d.ncomp + comp) * d.nalm + moff + lw + ll] = v;
+                        v.x += oa[u].x; v.y += oa[u].y;
+                        reinterpret_cast<double2*>(alm)[((size_t)(k0 + kk) * d.ncomp + comp) * d.nalm + moff + lw + ll] = v;
+                    }
+                }
+                continue;                                            // one tile per CTA in this mode
+            }
             if ((rd_d || rd_a) && tile == te - 1) {
                 // Last tile of the CTA (the only one of a per-order launch): the pipeline has drained, so the stage buffers
                 // are free.  The tile goes through shared memory ([map][l], rows padded by one element) and the consumer
@@ -746,13 +816,13 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
     const int ntile0 = (d.lmax - m_begin) / A_ML + 1;      // the grid is sized for the tile groups of the first order
     const unsigned grid = (unsigned)(nm * nkt * (tsplit ? (ntile0 + tsplit - 1) / tsplit : 1));
     const size_t sm = analysis_smem(d.ntile_max);
-    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tmF;
     if ((e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, &tmF)) != cudaSuccess) return e;
     const bool staged = pl->lam_mode == SHT_LAMBDA_STAGED && pl->lam;
     if (staged && gen_lambda && (e = launch_lambda_blocks(pl, d, true, st)) != cudaSuccess) return e;
-    k_legendre_analysis<<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0,
+    k_legendre_analysis<0><<<grid, LEG_THREADS, sm, st>>>(tmF, d, alm, k0, kmaps, nkt, accumulate ? 1 : 0,
                                                        staged ? pl->lam : nullptr, staged ? pl->lam_i0 : nullptr, m_begin, tsplit, nullptr,
                                                        pstar, 0);
     pl->launches++;
@@ -764,7 +834,7 @@ cudaError_t launch_legendre_analysis(sht_plan_s* pl, const DevicePlan& d, const 
 cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const double* da, int kmaps, CUtensorMap* tmF, CUtensorMap* tmA)
 {
     if (d.spin == 2) return legendre_order_maps_spin2(d, F, da, kmaps, tmF, tmA);
-    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)analysis_smem(d.ntile_max));
+    cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)analysis_smem(d.ntile_max));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synthesis_smem());
     if (e == cudaSuccess) e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, tmF);
     if (e == cudaSuccess) e = make_tmap_alm(d, da, (long long)kmaps * d.ncomp, tmA);
@@ -780,7 +850,7 @@ cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, 
     if (d.spin == 2) return launch_legendre_analysis_order_spin2(pl, d, tmF, alm, da, k0, kmaps, m, nm, st, pstar);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int ntile = (d.lmax - m) / A_ML + 1;
-    k_legendre_analysis<<<(unsigned)(nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
+    k_legendre_analysis<1><<<(unsigned)(4 * nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
                                                                                                       nullptr, m, 1, da, pstar, pstar > 0 ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
