@@ -532,6 +532,9 @@ k_legendre_analysis(const __grid_constant__ CUtensorMap tmF, DevicePlan d, doubl
 // halves of the pair's workspace line; north = Ee + Oo and south = Ee - Oo are formed by the ring kernels on load.
 // Stage layout: [a_lm: 4 boxes x (64 maps x 8 l x 16 B, 128B-swizzled)] [lambda: 32 l x S_SL]
 // ------------------------------------------------------------------------------------------------
+// WIN = 1 (per-order launches of Alg. 3): four CTAs share a block of 64 ring pairs, each owns two of its eight 8-ring row
+// blocks, as in k_legendre_analysis<1>
+template <int WIN>
 __global__ void __launch_bounds__(LEG_THREADS, 1)
 k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, double* __restrict__ F, int k0, int kmaps,
                      int nkt, int npb, const double* __restrict__ lam, int m0, int nsplit, int pb0, int pb1)
@@ -543,9 +546,11 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
     double2* cfs = reinterpret_cast<double2*>(empty + S_STAGES);      // 4 generator warps x 2 buffers x S_LC/2 (alpha, beta)
 
     // block order: m slowest (long m first), then the share of ring blocks, k-tile fastest
-    const int kt = blockIdx.x % nkt;
-    const int sp = (blockIdx.x / nkt) % nsplit;
-    const int m = m0 + blockIdx.x / (nkt * nsplit);
+    const int ib = WIN ? 2 * (int)(blockIdx.x & 3) : 0;             // WIN: this CTA's row blocks ib, ib + 1 of every ring block
+    const unsigned bx = WIN ? blockIdx.x >> 2 : blockIdx.x;
+    const int kt = bx % nkt;
+    const int sp = (bx / nkt) % nsplit;
+    const int m = m0 + bx / (nkt * nsplit);
     // warps 0..3 generate (the oldest warps of an SM sub-partition are served first by its scheduler: their
     // FP64 instructions must slip in between the consumers' DMMAs), warps 4..11 consume
     const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) - LEG_GEN_WARPS;
@@ -593,6 +598,30 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
                            (q1.x <= lend ? 16u : 0u) | (q1.y <= lend ? 32u : 0u) | (q1.z <= lend ? 64u : 0u) | (q1.w <= lend ? 128u : 0u);
                 };
                 const int ks1 = min(S_LC / 8, (lmax - lc) / 8 + 1);          // steps of 8 l that reach down to l <= lmax
+                if constexpr (WIN != 0) {
+#pragma unroll
+                    for (int ks = 0; ks < S_LC / 8; ++ks) {
+                        if (ks >= ks1) break;
+                        const unsigned act = active(lc + 8 * ks + 7);
+                        double a[2], b[4];
+                        const double* La = Ls + (8 * ks + 2 * t + cls) * S_SL + g;
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) a[i] = La[8 * (ib + i)];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const int row = 16 * wn + 4 * j + (g >> 1);
+                            const double v = As[ks * 1024 + row * 16 + ((((2 * t + cls) ^ (row & 7)) << 1) | (g & 1))];
+                            b[j] = kill_im ? 0.0 : v;
+                        }
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) {
+                            if (act & (1u << (ib + i))) {
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) dmma884(c[i][j][0], c[i][j][1], a[i], b[j]);
+                            }
+                        }
+                    }
+                } else
                 if (active(lc + 7) == 0xffu && ks1 == S_LC / 8) {  // every recurrence has started by the first 8 l of the stage
 #pragma unroll
                     for (int ks = 0; ks < S_LC / 8; ++ks) {
@@ -641,11 +670,12 @@ k_legendre_synthesis(const __grid_constant__ CUtensorMap tmA, DevicePlan d, doub
             // ---- epilogue: a lane holds (re, im) of (ring pb + 8 i + g, map 16 wn + 4 j + t): 64-byte runs per ring
             double2* Fb = Fl + (size_t)pb * ps;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const bool inr = pb + 8 * i + g < nh;
+            for (int i = 0; i < (WIN ? 2 : 8); ++i) {
+                const int ig = ib + i;                                       // row block inside the ring block
+                const bool inr = pb + 8 * ig + g < nh;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
-                    if (inr) Fb[(size_t)(8 * i) * ps + (size_t)j * kgs] = make_double2(c[i][j][0], c[i][j][1]);
+                    if (inr) Fb[(size_t)(8 * ig) * ps + (size_t)j * kgs] = make_double2(c[i][j][0], c[i][j][1]);
                     c[i][j][0] = 0.0; c[i][j][1] = 0.0;
                 }
             }
@@ -835,7 +865,7 @@ cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const doub
 {
     if (d.spin == 2) return legendre_order_maps_spin2(d, F, da, kmaps, tmF, tmA);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)analysis_smem(d.ntile_max));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synthesis_smem());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_legendre_synthesis<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synthesis_smem());
     if (e == cudaSuccess) e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, tmF);
     if (e == cudaSuccess) e = make_tmap_alm(d, da, (long long)kmaps * d.ncomp, tmA);
     return e;
@@ -865,7 +895,7 @@ cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d,
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
     const int nb = pbend > 0 && pbend < npb ? pbend : npb;
-    k_legendre_synthesis<<<(unsigned)(nm * nkt * nb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, nb, 0, nb);
+    k_legendre_synthesis<1><<<(unsigned)(4 * nm * nkt * nb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, nb, 0, nb);
     pl->launches++;
     return cudaGetLastError();
 }
@@ -876,7 +906,7 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
 {
     if (d.spin == 2) return launch_legendre_synthesis_spin2(pl, d, alm, F, k0, kmaps, st, pol, gen_lambda, pb0);
     const size_t sm = synthesis_smem();
-    cudaError_t e = cudaFuncSetAttribute(k_legendre_synthesis, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    cudaError_t e = cudaFuncSetAttribute(k_legendre_synthesis<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) return e;
     CUtensorMap tmA;
     if ((e = make_tmap_alm(d, alm, (long long)(k0 + kmaps) * d.ncomp, &tmA)) != cudaSuccess) return e;
@@ -889,7 +919,7 @@ cudaError_t launch_legendre_synthesis(sht_plan_s* pl, const DevicePlan& d, const
     const int nsplit = pl->leg_nsplit < 1 ? 1 : (pl->leg_nsplit > npb - pb0 ? npb - pb0 : pl->leg_nsplit);
     const int nm = m_count < 0 ? d.lmax + 1 - m_begin : m_count;
     if (nm <= 0) return cudaSuccess;
-    k_legendre_synthesis<<<nm * nkt * nsplit, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, m_begin, nsplit,
+    k_legendre_synthesis<0><<<nm * nkt * nsplit, LEG_THREADS, sm, st>>>(tmA, d, F, k0, kmaps, nkt, npb, staged ? pl->lam : nullptr, m_begin, nsplit,
                                                                      pb0, npb);
     pl->launches++;
     return cudaGetLastError();
