@@ -123,7 +123,7 @@ def test_immediate_iteration_spin2_against_oracle(nside, lmax, nmaps, niter, noi
     (64, 127, 3, 2, 0.0, 0),      # lmax = 2 nside - 1: the belt is alias-free, the caps are not
     (64, 127, 70, 1, 0.2, 0),     # two k-tiles, not band-limited
     (64, 100, 2, 3, 0.1, 0),      # the chain ends well before lmax
-    (128, 255, 2, 1, 0.0, 0),     # two blocks of 64 alias-free ring pairs, two l tiles
+    (128, 255, 1, 1, 0.0, 0),     # two blocks of 64 alias-free ring pairs, two l tiles
     (128, 150, 3, 1, 0.0, 0),     # the alias-free tail starts inside the caps
     (64, 127, 3, 2, 0.0, 2),      # spin 2: E and B of an order together
     (64, 100, 34, 1, 0.1, 2),     # spin 2, two k-tiles of 32 pairs, not band-limited
@@ -165,7 +165,7 @@ def test_immediate_hybrid_sweep_against_oracle_and_plain_sweep(nside, lmax, nmap
     (64, 191, 3, 2, 0.0),      # lmax = 3 nside - 1: every order from nside + 1 on meets its mirror 4 nside - m on the belt
     (64, 150, 70, 1, 0.2),     # two k-tiles, not band-limited
     (64, 129, 2, 3, 0.0),      # the second group is the two orders 2 nside, 2 nside + 1
-    (128, 300, 2, 1, 0.0),     # two blocks of belt ring pairs, three l tiles
+    (128, 300, 1, 1, 0.0),     # two blocks of belt ring pairs, three l tiles
 ])
 def test_immediate_two_phase_sweep_against_oracle_and_plain_sweep(nside, lmax, nmaps, niter, noise):
     """2 nside <= lmax < 4 nside (spin 0): the belt ring pairs leave the chain of dependent steps in two groups of orders
