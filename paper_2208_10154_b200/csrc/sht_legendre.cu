@@ -865,7 +865,9 @@ cudaError_t legendre_order_maps(const DevicePlan& d, const double* F, const doub
 {
     if (d.spin == 2) return legendre_order_maps_spin2(d, F, da, kmaps, tmF, tmA);
     cudaError_t e = cudaFuncSetAttribute(k_legendre_analysis<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)analysis_smem(d.ntile_max));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_legendre_analysis<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)analysis_smem(d.ntile_max));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_legendre_synthesis<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synthesis_smem());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_legendre_synthesis<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)synthesis_smem());
     if (e == cudaSuccess) e = make_tmap_F(d, F, KTILE_MAPS / KG, 1, tmF);
     if (e == cudaSuccess) e = make_tmap_alm(d, da, (long long)kmaps * d.ncomp, tmA);
     return e;
@@ -880,7 +882,14 @@ cudaError_t launch_legendre_analysis_order(sht_plan_s* pl, const DevicePlan& d, 
     if (d.spin == 2) return launch_legendre_analysis_order_spin2(pl, d, tmF, alm, da, k0, kmaps, m, nm, st, pstar);
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int ntile = (d.lmax - m) / A_ML + 1;
-    k_legendre_analysis<1><<<(unsigned)(4 * nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
+    // windowed (four CTAs per l tile) while the launch would not fill the SMs once: a per-order launch is a link in a chain
+    // of dependent launches, so what counts is the serial work of one CTA (nside 128: 8 - 24 CTAs; 57 -> 24 ms per call);
+    // past one wave the windows only multiply the operand reads (nside 512, 512 maps: 900 ms unwindowed, 979 ms windowed)
+    if (nm * ntile * nkt <= pl->sm_count)
+        k_legendre_analysis<1><<<(unsigned)(4 * nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
+                                                                                                          nullptr, m, 1, da, pstar, pstar > 0 ? 1 : 0);
+    else
+        k_legendre_analysis<0><<<(unsigned)(nm * ntile * nkt), LEG_THREADS, analysis_smem(d.ntile_max), st>>>(tmF, d, alm, k0, kmaps, nkt, 1, nullptr,
                                                                                                       nullptr, m, 1, da, pstar, pstar > 0 ? 1 : 0);
     pl->launches++;
     return cudaGetLastError();
@@ -895,7 +904,10 @@ cudaError_t launch_legendre_synthesis_order(sht_plan_s* pl, const DevicePlan& d,
     const int nkt = (kmaps + KTILE_MAPS - 1) / KTILE_MAPS;
     const int npb = (d.nh + S_PB - 1) / S_PB;
     const int nb = pbend > 0 && pbend < npb ? pbend : npb;
-    k_legendre_synthesis<1><<<(unsigned)(4 * nm * nkt * nb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, nb, 0, nb);
+    if (nm * nkt * nb <= pl->sm_count)       // windowed under the same rule as the per-order analysis launch
+        k_legendre_synthesis<1><<<(unsigned)(4 * nm * nkt * nb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, nb, 0, nb);
+    else
+        k_legendre_synthesis<0><<<(unsigned)(nm * nkt * nb), LEG_THREADS, synthesis_smem(), st>>>(tmA, d, F, 0, kmaps, nkt, npb, nullptr, m, nb, 0, nb);
     pl->launches++;
     return cudaGetLastError();
 }
